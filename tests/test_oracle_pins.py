@@ -1,0 +1,373 @@
+"""Pins P1-P9: the oracle checked against what the paper and the mathematics fix — never
+against itself and never against the CUDA path.  (DESIGN.md "Pins".)"""
+import ctypes
+import math
+import os
+import subprocess
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LEVELS = [0.0, 0.5, 1.0, 1.5, 2.0, 3.0, 4.0, 6.0]          # PAPER.md:124 (also in golden/)
+
+
+def _golden():
+    out = {}
+    with open(os.path.join(HERE, "golden", "paper_constants.txt")) as f:
+        for line in f:
+            line = line.split("#")[0].strip()
+            if "=" in line:
+                k, v = line.split("=")
+                out[k.strip()] = v.strip()
+    return out
+
+
+# ----------------------------------------------------------------------------- P1 Hadamard
+@pytest.mark.parametrize("d", [32, 64, 128, 256])
+def test_p1_hadamard_structure(d):
+    kap = oracle.kappa(d)
+    assert kap == pytest.approx(d ** -0.5, rel=1e-15)
+    # kappa is the CORRECTLY ROUNDED 2^(-log2(d)/2): its square brackets 1/d within 1 ulp
+    assert abs(kap * kap * d - 1.0) < 4e-16
+    H = np.stack([oracle.hadamard(np.eye(d)[j]) for j in range(d)], axis=1) / kap
+    # entries are exactly +-1 with the Sylvester sign pattern (-1)^popcount(i&j)
+    i, j = np.meshgrid(np.arange(d), np.arange(d), indexing="ij")
+    sign = 1 - 2 * (np.vectorize(lambda a: bin(a).count("1"))(i & j) & 1)
+    assert np.array_equal(H, sign.astype(np.float64))
+    # H H^T = d I exactly (integers)
+    assert np.array_equal(H @ H.T, d * np.eye(d))
+    # Kronecker recursion H_{2n} = [[H_n, H_n], [H_n, -H_n]]
+    h = d // 2
+    assert np.array_equal(H[:h, :h], H[:h, h:]) and np.array_equal(H[:h, :h], -H[h:, h:])
+    assert np.array_equal(H[:2, :2], np.array([[1.0, 1.0], [1.0, -1.0]]))
+
+
+def test_p1_rotation_is_orthonormal_involution():
+    rng = np.random.default_rng(0)
+    for d in (64, 128, 256):
+        x = rng.standard_normal(d)
+        y = oracle.hadamard(x)
+        assert np.linalg.norm(y) == pytest.approx(np.linalg.norm(x), rel=1e-14)
+        assert np.allclose(oracle.hadamard(y), x, atol=1e-14)
+        e0 = np.zeros(d)
+        e0[0] = 1.0
+        assert np.array_equal(oracle.hadamard(e0), np.full(d, oracle.kappa(d)))
+        # (Rq).(Rk) = q.k : the identity the decode step relies on
+        q = rng.standard_normal(d)
+        assert np.dot(oracle.hadamard(q), y) == pytest.approx(np.dot(q, x), abs=1e-12)
+
+
+# ----------------------------------------------------------------------------- P2 decode table
+def test_p2_decode_table_matches_eq1():
+    g = _golden()
+    assert [float(v) for v in g["e2m1_levels"].split()] == LEVELS
+    bias = int(g["scale_bias"])
+    for byte in (0, 1, 126, 127, 128, 254):
+        for code in range(16):
+            mag = LEVELS[code & 7]
+            want = (-mag if code & 8 else mag) * 2.0 ** (byte - bias)      # Eq.(1)
+            assert oracle.dequant(code, byte) == want
+    assert oracle.dequant(8, 127) == 0.0                                   # -0 decodes to 0
+    assert oracle.dequant(7, 127) == 6.0 and oracle.dequant(15, 128) == -12.0
+
+
+def test_p2_exact_round_trip_of_representable_values():
+    # a group holding levels of F times 2^k, max level 6: m = 6*2^k, c*m = 0.936*2^k -> E = k
+    rng = np.random.default_rng(1)
+    for k in (-20, -3, 0, 1, 9):
+        idx = rng.integers(0, 8, size=128)
+        idx[::32] = 7                                    # every group contains the level 6
+        sgn = rng.choice([-1.0, 1.0], size=128)
+        y = sgn * np.array(LEVELS)[idx] * 2.0 ** k
+        packed, scales = oracle.quantize_vector(y, 0.156)
+        assert np.all(scales == 127 + k)
+        assert np.array_equal(oracle.dequantize(packed, scales), y)
+        codes = oracle.unpack_codes(packed)
+        assert np.array_equal(codes & 7, idx)
+        assert np.all((codes[idx == 0] & 8) == 0)        # zero never carries a sign (G7)
+
+
+# ----------------------------------------------------------------------------- P3 brute force
+def test_p3_nearest_level_brute_force():
+    """For every r on a grid holding all midpoints, the encoder's code is the argmin of
+    |r - level| over the 8 magnitudes, ties to the even code, clamp above 6."""
+    lev = np.array(LEVELS)
+    for E in (-5, -1, 0, 3):
+        for n in range(0, 10 * 1024 + 1):
+            r = n / 1024.0
+            dist = np.abs(r - lev)
+            best = np.flatnonzero(dist == dist.min())
+            want = int(best[0]) if len(best) == 1 else int([b for b in best if b % 2 == 0][0])
+            y = math.ldexp(r, E)
+            assert oracle.e2m1_encode(y, E) == want, (r, E)
+            got_neg = oracle.e2m1_encode(-y, E)
+            assert got_neg == (want | 8 if want else 0)
+    # all 16 codes x several scales: encode(decode(code)) is the identity (except -0 -> +0)
+    for byte in (100, 127, 140):
+        for code in range(16):
+            v = oracle.dequant(code, byte)
+            assert oracle.e2m1_encode(v, byte - 127) == (0 if code == 8 else code)
+
+
+# ----------------------------------------------------------------------------- P4 thresholds
+def test_p4_scale_thresholds():
+    c = float(np.float32(0.156))                       # the constant reaches the rule as a float
+    assert c == 0.15600000321865082
+    for k in range(-6, 7):
+        thr = 2.0 ** (k - 0.5) / c                     # E switches from k-1 to k here
+        lo, hi = np.nextafter(thr, 0), np.nextafter(thr, np.inf)
+        # thr itself is irrational-adjacent; step a few ulps each side to be independent of
+        # how 2^(k-0.5) rounded
+        for _ in range(4):
+            lo, hi = np.nextafter(lo, 0), np.nextafter(hi, np.inf)
+        assert oracle.scale_exponent(c, lo) == k - 1
+        assert oracle.scale_exponent(c, hi) == k
+        assert oracle.scale_exponent(c, thr * 1.3) == k
+    assert oracle.scale_exponent(c, 0.0) == -127
+    assert oracle.scale_exponent(c, 1e-300) == -127 and oracle.scale_exponent(c, 1e300) == 127
+    # equals round(log2(c*m)) evaluated in extended precision for random m
+    rng = np.random.default_rng(2)
+    for m in np.exp(rng.uniform(-40, 40, 2000)):
+        want = int(np.rint(np.log2(np.longdouble(c) * np.longdouble(m))))
+        assert oracle.scale_exponent(c, m) == want
+    # invariant: the group max lands in [4.5327, 9.0655) grid units (so it encodes to 4 or 6)
+    for m in np.exp(rng.uniform(-10, 10, 500)):
+        E = oracle.scale_exponent(c, m)
+        r = m / 2.0 ** E
+        assert 2.0 ** -0.5 / c * 0.999999 <= r < 2.0 ** 0.5 / c * 1.000001
+        assert oracle.e2m1_encode(m, E) in (6, 7)
+
+
+# ----------------------------------------------------------------------------- P5 fingerprints
+def test_p5_statistical_fingerprints():
+    """i.i.d. N(0,1) groups, c = 0.156 (values from the survey's Monte-Carlo, SURVEY.md §8c P5,
+    an independent numpy prototype): E histogram, clamp rate, code histogram, relative MSE."""
+    rng = np.random.default_rng(3)
+    n = 20000
+    y = rng.standard_normal((n, 128))
+    packs = [oracle.quantize_vector(v, float(np.float32(0.156))) for v in y]
+    packed = np.stack([p[0] for p in packs])
+    scales = np.stack([p[1] for p in packs])
+    frac125 = np.mean(scales == 125)
+    frac126 = np.mean(scales == 126)
+    assert frac125 == pytest.approx(0.468, abs=0.01) and frac126 == pytest.approx(0.532, abs=0.01)
+    assert np.mean((scales < 125) | (scales > 126)) < 2e-3
+    E = np.repeat(scales.astype(np.int64) - 127, 32, axis=1)
+    r = np.abs(y) / 2.0 ** E
+    assert np.mean(r > 6) == pytest.approx(0.0554, abs=0.003)
+    codes = oracle.unpack_codes(packed)
+    hist = np.bincount((codes & 7).ravel(), minlength=8) / codes.size
+    want = [0.0757, 0.1479, 0.1377, 0.1229, 0.1509, 0.1403, 0.1222, 0.1024]
+    assert np.allclose(hist, want, atol=0.004)
+    deq = oracle.dequantize(packed, scales)
+    rel_mse = np.mean((deq - y) ** 2) / np.mean(y ** 2)
+    assert rel_mse == pytest.approx(0.0178, abs=0.001)
+
+
+# ----------------------------------------------------------------------------- P6 sizes
+def test_p6_sizes():
+    g = _golden()
+    packed, scales = oracle.quantize_vector(np.ones(128), 0.156)
+    assert packed.nbytes + scales.nbytes == 68
+    per_group = (packed.nbytes + scales.nbytes) // (128 // int(g["group_size"]))
+    assert per_group == int(g["bytes_per_group"])
+    assert per_group * 8 / int(g["group_size"]) == float(g["bits_per_element"])
+
+
+# ----------------------------------------------------------------------------- P7 the two constants
+def _mse_for_c(y, c, power_of_two):
+    """Eq.(2) objective E[(z - s q(z/s))^2] with s = c*m (continuous) or 2^round(log2(c*m)),
+    evaluated with an INDEPENDENT numpy nearest-level quantiser (argmin over the level set)."""
+    lev = np.array([-6, -4, -3, -2, -1.5, -1, -0.5, 0, 0.5, 1, 1.5, 2, 3, 4, 6], np.float64)
+    m = np.abs(y).max(axis=1, keepdims=True)
+    s = c * m
+    if power_of_two:
+        s = 2.0 ** np.rint(np.log2(s))
+    z = y / s
+    q = lev[np.abs(z[..., None] - lev).argmin(axis=-1)]
+    return np.mean((y - s * q) ** 2)
+
+
+def test_p7_paper_constants_fix_the_reading_of_round():
+    """PAPER.md:128 gives c = 0.156 as the MSE optimum of Eq.(2); PAPER.md:333 calls 0.195 "the
+    power-of-two-optimal value".  With round-to-nearest in E = round(log2(c m)) the power-of-two
+    optimum on Gaussian groups sits at ~0.196 (floor would give ~0.28, ceil ~0.14) and the
+    continuous-scale optimum at ~0.16 — so "round" is round-to-nearest (reading G4)."""
+    g = _golden()
+    rng = np.random.default_rng(4)
+    y = rng.standard_normal((12000, 32))
+    cs = np.arange(0.10, 0.32, 0.004)
+    cont = [_mse_for_c(y, c, False) for c in cs]
+    p2 = [_mse_for_c(y, c, True) for c in cs]
+    c_cont = cs[int(np.argmin(cont))]
+    c_p2 = cs[int(np.argmin(p2))]
+    assert abs(c_cont - float(g["c_default"])) < 0.02
+    assert abs(c_p2 - float(g["c_power_of_two_optimal"])) < 0.02
+    # and the ORACLE's rule reproduces the power-of-two objective at the paper's two constants
+    for c in (0.156, 0.195):
+        deq = np.stack([oracle.dequantize(*oracle.quantize_vector(np.tile(v, 4), c))[:32] for v in y[:3000]])
+        mse_oracle = np.mean((deq - y[:3000]) ** 2)
+        assert mse_oracle == pytest.approx(_mse_for_c(y[:3000], c, True), rel=1e-9)
+
+
+def test_p7_c_equal_one_uses_no_shrinkage():
+    # c = 1.0 is "raw absmax with no shrinkage": the group max maps near 1.0
+    rng = np.random.default_rng(5)
+    y = rng.standard_normal(128)
+    packed, scales = oracle.quantize_vector(y, 1.0)
+    codes = oracle.unpack_codes(packed) & 7
+    assert codes.max() <= 3                              # nothing above 1.5 grid units is used
+
+
+# ----------------------------------------------------------------------------- P8 library casts
+@pytest.fixture(scope="module")
+def libcasts():
+    inc = "/usr/local/cuda/include"
+    if not os.path.exists(os.path.join(inc, "cuda_fp4.h")):
+        pytest.skip("CUDA toolkit headers not present")
+    src = os.path.join(HERE, "helpers", "cuda_host_casts.cpp")
+    so = os.path.join(HERE, "helpers", "cuda_host_casts.so")
+    if not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(src):
+        subprocess.run(["g++", "-O1", "-shared", "-fPIC", f"-I{inc}", "-o", so, src], check=True)
+    lib = ctypes.CDLL(so)
+    for f in (lib.lib_e2m1, lib.lib_e4m3):
+        f.argtypes = [ctypes.c_double]
+        f.restype = ctypes.c_ubyte
+    return lib
+
+
+def test_p8_e2m1_matches_cuda_host_routine(libcasts):
+    rng = np.random.default_rng(6)
+    xs = np.concatenate([np.arange(-8, 8, 1 / 64.0), rng.standard_normal(4000) * 3,
+                         [0.25, 0.75, 1.25, 1.75, 2.5, 3.5, 5.0, 6.0, 1e9, -1e9]])
+    for x in xs:
+        got = oracle.e2m1_encode(float(x), 0)
+        ref = libcasts.lib_e2m1(float(x))
+        if (ref & 7) == 0:
+            ref = 0                                      # G7: we store canonical +0, CUDA keeps the sign
+        assert got == ref, x
+
+
+def test_p8_e4m3_matches_torch_and_cuda_host_routine(libcasts):
+    rng = np.random.default_rng(7)
+    xs = np.concatenate([rng.standard_normal(5000) * 4, rng.standard_normal(2000) * 0.01,
+                         np.arange(0, 2 ** -5, 2 ** -12), [2 ** -10, 1.5 * 2 ** -9, 447.9, 448.0,
+                                                         449.0, 463.9, 1e4, -1e4, 0.0, 2 ** -6]])
+    t = torch.tensor(xs, dtype=torch.float64).to(torch.float8_e4m3fn).view(torch.uint8).numpy()
+    for x, tb in zip(xs, t):
+        got = oracle.e4m3_encode(float(x))
+        ref = libcasts.lib_e4m3(float(x))
+        if (ref & 0x7F) == 0:
+            ref = 0
+        assert got == ref, x
+        if abs(x) < 464 and (tb & 0x7F) != 0:
+            assert got == tb, x                          # torch saturates to NaN beyond 464; we clamp
+    # all 256 bytes decode per the closed form, and encode(decode(b)) == b
+    for b in range(256):
+        if (b & 0x7F) == 0x7F:
+            continue                                     # NaN pattern: never produced
+        v = oracle.e4m3_decode(b)
+        ef, mf = (b >> 3) & 15, b & 7
+        want = (mf / 8.0) * 2.0 ** -6 if ef == 0 else (1 + mf / 8.0) * 2.0 ** (ef - 7)
+        assert abs(v) == want
+        assert oracle.e4m3_encode(v) == (0 if (b & 0x7F) == 0 else b)
+    assert oracle.e4m3_decode(0x7E) == 448.0
+
+
+# ----------------------------------------------------------------------------- P9 attention
+def _random_cache(rng, L, Hkv, d=128):
+    k = rng.standard_normal((L, Hkv, d)).astype(np.float32)
+    v = rng.standard_normal((L, Hkv, d)).astype(np.float32)
+    kb = torch.from_numpy(k).to(torch.bfloat16).view(torch.uint16).numpy()
+    vb = torch.from_numpy(v).to(torch.bfloat16).view(torch.uint16).numpy()
+    return kb, vb
+
+
+def test_p9_attention_closed_forms():
+    rng = np.random.default_rng(8)
+    Hq, Hkv, d = 8, 2, 128
+    kb, vb = _random_cache(rng, 37, Hkv)
+    kc, ks, vc, vs = oracle.encode_kv(kb, vb)
+    qb = torch.from_numpy(rng.standard_normal((Hq, d)).astype(np.float32)).to(torch.bfloat16)
+    q8 = oracle.encode_q(qb.view(torch.uint16).numpy())
+    out, p = oracle.attention(q8, kc, ks, vc, vs, Hq, Hkv, return_probs=True)
+    assert np.allclose(p.sum(axis=1), 1.0, atol=1e-14)               # rows of P sum to 1
+    # L = 1: out = vhat_0
+    out1 = oracle.attention(q8, kc[:1], ks[:1], vc[:1], vs[:1], Hq, Hkv)
+    vhat = oracle.dequantize(vc, vs)
+    for h in range(Hq):
+        assert np.array_equal(out1[h], vhat[0, h // (Hq // Hkv)])
+    # all keys equal: out = mean of vhat
+    kc_eq = np.repeat(kc[:1], 37, axis=0)
+    ks_eq = np.repeat(ks[:1], 37, axis=0)
+    out_eq = oracle.attention(q8, kc_eq, ks_eq, vc, vs, Hq, Hkv)
+    for h in range(Hq):
+        assert np.allclose(out_eq[h], vhat[:, h // (Hq // Hkv)].mean(axis=0), atol=1e-13)
+    # L = 0: zeros
+    assert np.array_equal(oracle.attention(q8, kc[:0], ks[:0], vc[:0], vs[:0], Hq, Hkv), np.zeros((Hq, d)))
+    # equals torch SDPA in float64 on the dequantised tensors (library routine)
+    khat = oracle.dequantize(kc, ks)
+    qd = np.array([[oracle.e4m3_decode(int(b)) for b in row] for row in q8])
+    G = Hq // Hkv
+    tq = torch.from_numpy(qd)[None, :, None, :]
+    tk = torch.from_numpy(khat).permute(1, 0, 2).repeat_interleave(G, dim=0)[None]
+    tv = torch.from_numpy(vhat).permute(1, 0, 2).repeat_interleave(G, dim=0)[None]
+    ref = torch.nn.functional.scaled_dot_product_attention(tq, tk, tv)[0, :, 0].numpy()
+    assert np.allclose(out, ref, atol=1e-12)
+    # the GQA map is contiguous groups: head h <-> kv head h // G (a swapped map would differ)
+    assert not np.allclose(out[0], ref[G], atol=1e-6)
+
+
+def test_p9_split_merge_identity_and_page_permutation():
+    """A split-K evaluation with the merge formula of include/uq.h equals the unsplit oracle."""
+    rng = np.random.default_rng(9)
+    Hq, Hkv, d, L = 4, 1, 128, 203
+    kb, vb = _random_cache(rng, L, Hkv)
+    kc, ks, vc, vs = oracle.encode_kv(kb, vb)
+    q8 = oracle.encode_q(torch.from_numpy(rng.standard_normal((Hq, d)).astype(np.float32))
+                         .to(torch.bfloat16).view(torch.uint16).numpy())
+    full = oracle.attention(q8, kc, ks, vc, vs, Hq, Hkv)
+    khat, vhat = oracle.dequantize(kc, ks)[:, 0], oracle.dequantize(vc, vs)[:, 0]
+    qd = np.array([[oracle.e4m3_decode(int(b)) for b in row] for row in q8])
+    z = (qd @ khat.T) / math.sqrt(d)
+    bounds = [0, 16, 64, 64, 160, L]                    # includes an empty split
+    ms, ls, accs = [], [], []
+    for a, b in zip(bounds[:-1], bounds[1:]):
+        if a == b:
+            ms.append(np.full(Hq, -np.inf)); ls.append(np.zeros(Hq)); accs.append(np.zeros((Hq, d)))
+            continue
+        m = z[:, a:b].max(axis=1)
+        e = np.exp(z[:, a:b] - m[:, None])
+        ms.append(m); ls.append(e.sum(axis=1)); accs.append(e @ vhat[a:b])
+    M = np.max(np.stack(ms), axis=0)
+    w = [np.exp(m - M) for m in ms]
+    num = sum(wi[:, None] * ai for wi, ai in zip(w, accs))
+    den = sum(wi * li for wi, li in zip(w, ls))
+    assert np.allclose(num / den[:, None], full, atol=1e-12)
+    # without quantisation (Rq).(Rk) = q.k: dense attention is rotation invariant
+    qf = rng.standard_normal((Hq, d)); kf = rng.standard_normal((L, 1, d)); vf = rng.standard_normal((L, 1, d))
+    a = oracle.attention_dense(qf, kf, vf)
+    qr = np.stack([oracle.hadamard(x) for x in qf])
+    kr = np.stack([oracle.hadamard(x) for x in kf[:, 0]])[:, None]
+    assert np.allclose(oracle.attention_dense(qr, kr, vf), a, atol=1e-12)
+
+
+def test_k_is_rotated_and_v_is_not():
+    """Alg. 1 l.1: "rotate keys; V unrotated" — V codes equal direct quantisation of V, K codes
+    equal quantisation of R*K, and nothing per-token is stored besides codes + group scales."""
+    rng = np.random.default_rng(10)
+    kb, vb = _random_cache(rng, 5, 2)
+    kc, ks, vc, vs = oracle.encode_kv(kb, vb)
+    for t in range(5):
+        for h in range(2):
+            x = oracle.bf16_to_double(vb[t, h])
+            p, s = oracle.quantize_vector(x, float(np.float32(0.156)))
+            assert np.array_equal(p, vc[t, h]) and np.array_equal(s, vs[t, h])
+            y = oracle.hadamard(oracle.bf16_to_double(kb[t, h]))
+            p, s = oracle.quantize_vector(y, float(np.float32(0.156)))
+            assert np.array_equal(p, kc[t, h]) and np.array_equal(s, ks[t, h])
+    assert kc.shape[-1] + ks.shape[-1] == 68 and vc.shape[-1] + vs.shape[-1] == 68
