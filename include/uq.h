@@ -1,0 +1,156 @@
+/*
+ * uq.h — C ABI of libuq.so: UltraQuant's data-parallel hot path on NVIDIA B200 (sm_100a).
+ *
+ * Implements Algorithm 1 of arxiv/paper_2606_20474 ("UltraQuant: 4-bit KV Caching for
+ * Context-Heavy Agents"), /root/reference/PAPER.md:245-261:
+ *
+ *   Write  (l.1-5): K <- R*K (Walsh-Hadamard over head_dim; V unrotated); 32-channel groups;
+ *                   per group m = max|x|, E = round(log2(c*m)) (UE8M0 exponent, byte = E+127);
+ *                   per coordinate code = nearest level of x/2^E in
+ *                   F = {0,+-.5,+-1,+-1.5,+-2,+-3,+-4,+-6} (E2M1); store 2 codes/byte + 1 scale
+ *                   byte per group (17 B / 32 elements).
+ *   Decode (l.6-8): Q <- cast_fp8_e4m3(R*Q); xhat = code * 2^(byte-127) (Eq.(1));
+ *                   softmax(sm_scale * Q Khat^T) Vhat for every query head of a KV head.
+ *
+ * Paging, block tables, split-K and the merge are not in the paper; they follow
+ * BASELINE.json's north_star.  Readings of everything the paper leaves open: DESIGN.md.
+ *
+ * CONVENTIONS
+ *  - Every pointer is a DEVICE pointer owned by the caller unless it says "host".  The library
+ *    never allocates, frees or keeps device memory, never synchronises the device, and only
+ *    enqueues work on the caller's stream (a cudaStream_t passed as void*; NULL = legacy stream).
+ *  - Every function returns a status code; no C++ exception crosses the boundary.
+ *    uq_last_error_string() (host, thread-local) describes the last failure.
+ *  - Arguments are validated on the host only.  Block-table entries outside [0, num_pages),
+ *    seq_lens beyond max_pages*page_size, NaN/Inf inputs: undefined behaviour.
+ *  - Supported geometry in this version: head_dim = 128, group_size = 32, page_size = 16,
+ *    num_q_heads / num_kv_heads in 1..16 (UQ_ERR_UNSUPPORTED otherwise).
+ *  - GQA map: query head h reads KV head h / (num_q_heads/num_kv_heads).
+ *
+ * PHYSICAL CACHE LAYOUT (uint8).  cache[num_pages][num_kv_heads][UQ_RECORD_BYTES]; the record
+ * of (page p, kv head h) starts at byte (p*num_kv_heads + h)*2176 and holds 16 tokens with
+ * exactly 4.25 bit/element and no padding.  The LOGICAL content (what Alg. 1 defines: packed
+ * codes with element 2j in bits 0-3 and 2j+1 in bits 4-7 of byte j, scale bytes in group
+ * order) is permuted inside a record so that every lane of a warp fetches its tensor-core
+ * fragment with 16-byte loads.  With t = token slot in the page (0..15), d = channel (0..127):
+ *
+ *   [   0,1024)  K codes.  Token t at 64*t.  Logical 32-bit word j (channels 8j..8j+7,
+ *                j = 4*ks + c with ks = group 0..3, c = 0..3) is stored at word 4*c + ks.
+ *   [1024,2048)  V codes, token-pair interleaved.  For mt = d>>4, g = d&7, hi = (d>>3)&1,
+ *                pair p = (t>>3)&1, c = (t&7)>>1:  byte
+ *                   1024 + 512*(mt>>2) + 16*(4*g + c) + 4*(mt&3) + 2*p + hi
+ *                holds the code of token (t & ~1) in bits 0-3 and of token (t | 1) in bits 4-7.
+ *   [2048,2112)  K scale bytes.  Token t's four group bytes (group 0 first) form the 32-bit
+ *                word at index 2*(t&7) + (t>>3).
+ *   [2112,2176)  V scale bytes.  For token t (p, c as above, odd = t&1) and group gr:  byte
+ *                   2112 + 16*c + 4*(2*p + (gr>>1)) + 2*odd + (gr&1).
+ *
+ * tests/uq_layout.py holds an independent unpacker written from this description.
+ */
+#ifndef UQ_H_
+#define UQ_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define UQ_OK 0
+#define UQ_ERR_INVALID_ARG 1  /* null pointer, non-positive size, Hq % Hkv != 0, misaligned pointer */
+#define UQ_ERR_UNSUPPORTED 2  /* geometry outside the supported set above */
+#define UQ_ERR_WORKSPACE 3    /* reserved */
+#define UQ_ERR_CUDA 4         /* launch / driver error */
+
+#define UQ_RECORD_BYTES 2176  /* 16 tokens * (64 + 4 + 64 + 4) bytes */
+
+typedef struct {
+  int32_t num_q_heads;   /* e.g. 64 */
+  int32_t num_kv_heads;  /* e.g. 4  */
+  int32_t head_dim;      /* 128 */
+  int32_t page_size;     /* 16 */
+  int32_t group_size;    /* 32 */
+  float c_k;             /* global constant c for keys   (0.156f); used as (double)c_k */
+  float c_v;             /* global constant c for values (0.156f; same rule, reading G3) */
+  float sm_scale;        /* softmax scale; 0 => 1/sqrt(head_dim) */
+  uint32_t flags;        /* reserved, must be 0 */
+} uq_config;
+
+/* Host.  Static, thread-local description of the last error returned on this thread. */
+const char* uq_last_error_string(void);
+
+/* Host.  Bytes of one (page, kv_head) record: page_size*(d/2 + d/32)*2 = 2176; 0 if unsupported. */
+size_t uq_cache_record_bytes(const uq_config* cfg);
+
+/*
+ * Alg. 1 "Write" l.1-5 and "Decode" l.6: quantize-on-append.
+ *
+ *  k_new, v_new  bf16 [total_new, num_kv_heads, head_dim].  Rows cu_new[b] .. cu_new[b+1]-1 are
+ *                the new tokens of sequence b, written at positions seq_lens[b] + j through
+ *                block_tables[b][pos / page_size], slot pos % page_size.
+ *  cu_new        int32 [batch+1], cu_new[0] = 0.       seq_lens  int32 [batch], lengths BEFORE
+ *                the append (read-only: the caller advances them).
+ *  block_tables  int32 [batch, max_pages].             cache: layout above, num_pages pages.
+ *  total_new     host int: cu_new[batch] (rows in k_new / v_new); may be 0.
+ *  q             bf16 [batch, num_q_heads, head_dim] or NULL.  If given, q_fp8 (uint8, same
+ *                shape) receives cast_fp8_e4m3(R*q): OCP E4M3, round-to-nearest-even,
+ *                saturating at +-448, zero stored as 0x00.
+ *
+ * Every rounding decision (scale exponent, E2M1 code, E4M3 byte) is taken on float64 values of
+ * the exactly-computed rotation (reading G1), so codes, scale bytes and q_fp8 are
+ * bit-identical to the float64 oracle.  Tokens of one sequence that share a V-code byte (slots
+ * 2i, 2i+1) may arrive in one call or in successive calls on the same stream; two concurrent
+ * calls must not append to the same page.  Appending to a page shared by several block tables
+ * is the caller's error.
+ */
+int32_t uq_rotate_quantize_append(const uq_config* cfg, const void* k_new, const void* v_new,
+                                  const int32_t* cu_new, const int32_t* seq_lens,
+                                  const int32_t* block_tables, int32_t max_pages, int32_t batch,
+                                  int32_t total_new, void* cache, int64_t num_pages,
+                                  const void* q, void* q_fp8, void* stream);
+
+/*
+ * Alg. 1 "Decode" l.7-8 for one decode step, split-K over the sequence.
+ *
+ *  q_fp8        uint8 [batch, num_q_heads, head_dim] (E4M3 bytes of the rotated query).
+ *  seq_lens     int32 [batch]: lengths INCLUDING any token appended in this step.
+ *  num_splits   >= 1.  Split s of sequence b covers pages [s*pps, min((s+1)*pps, n_pages_b))
+ *               with n_pages_b = ceil(seq_lens[b]/page_size), pps = ceil(n_pages_b/num_splits);
+ *               a split may be empty.
+ *  partial_acc  float32 [batch, num_q_heads, num_splits, head_dim]
+ *  partial_ml   float32 [batch, num_q_heads, num_splits, 2] = (m_s, l_s)
+ *
+ * Partial format: with z_t = sm_scale * q8 . khat_t (natural-log units),
+ *     m_s   = a reference logit of split s (>= every z_t of the split minus 8*ln2; it need
+ *             not be the exact maximum),  l_s = sum_t exp(z_t - m_s),
+ *     acc_s = sum_t exp(z_t - m_s) * vhat_t   (unnormalised).
+ * An empty split writes m_s = -inf, l_s = 0, acc_s = 0.
+ *
+ * Arithmetic: q8 x code products are exact and accumulate in fp32 on tensor cores; exp in
+ * fp32 (ex2.approx); P and Vhat enter the PV product as fp16 (Vhat relative to a running
+ * reference exponent; values more than 2^23 below the largest V scale seen by a warp flush to
+ * zero); accumulation in fp32.  Error bound vs the float64 oracle: DESIGN.md "Tolerance".
+ */
+int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, const void* cache,
+                            int64_t num_pages, const int32_t* block_tables, int32_t max_pages,
+                            const int32_t* seq_lens, int32_t batch, int32_t num_splits,
+                            float* partial_acc, float* partial_ml, void* stream);
+
+/*
+ * Merge of split partials (exact reassociation of the softmax):
+ *     M = max_s m_s;  out = sum_s e^(m_s-M) acc_s / sum_s e^(m_s-M) l_s,  cast to bf16 (RNE).
+ * Splits with l_s = 0 are ignored; if all are empty (seq_len 0) the output row is zeros.
+ *  out_bf16     bf16 [batch, num_q_heads, head_dim]
+ */
+int32_t uq_merge_splits(const uq_config* cfg, const float* partial_acc, const float* partial_ml,
+                        int32_t batch, int32_t num_splits, void* out_bf16, void* stream);
+
+/* Host.  A num_splits that gives uq_decode_attention about `waves` full waves of CTAs on the
+ * current device for `batch` sequences of about `avg_seq_len` tokens (never below 1). */
+int32_t uq_suggest_num_splits(const uq_config* cfg, int32_t batch, int32_t avg_seq_len);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* UQ_H_ */

@@ -1,0 +1,24 @@
+"""paper_2606_20474_b200 — B200-native UltraQuant KV-cache hot path (arxiv/paper_2606_20474).
+
+Thin Python binding over the C-ABI CUDA library libuq.so (include/uq.h): argument marshalling
+only — every step of the path (rotation, quantiser, paged split-K attention, merge) runs in the
+hand-written sm_100a kernels under csrc/.  PyTorch is used for device memory and streams.
+
+There is NO CPU fallback: if libuq.so is missing or does not load, every entry point raises.
+"""
+from .binding import (  # noqa: F401
+    UQConfig,
+    UQError,
+    RECORD_BYTES,
+    StepBuffers,
+    alloc_cache,
+    cache_record_bytes,
+    decode_attention,
+    decode_step,
+    decode_step_host,
+    last_error,
+    library_path,
+    merge_splits,
+    rotate_quantize_append,
+    suggest_num_splits,
+)

@@ -1,0 +1,204 @@
+"""ctypes binding of libuq.so.  Same names and argument order as include/uq.h; torch tensors
+are passed as raw device pointers, the current torch CUDA stream as the stream argument."""
+from __future__ import annotations
+
+import ctypes
+import dataclasses
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libuq.so")
+_lib = None
+
+RECORD_BYTES = 2176
+
+
+class UQError(RuntimeError):
+    pass
+
+
+class _CConfig(ctypes.Structure):
+    _fields_ = [("num_q_heads", ctypes.c_int32), ("num_kv_heads", ctypes.c_int32),
+                ("head_dim", ctypes.c_int32), ("page_size", ctypes.c_int32),
+                ("group_size", ctypes.c_int32), ("c_k", ctypes.c_float), ("c_v", ctypes.c_float),
+                ("sm_scale", ctypes.c_float), ("flags", ctypes.c_uint32)]
+
+
+@dataclasses.dataclass
+class UQConfig:
+    num_q_heads: int
+    num_kv_heads: int
+    head_dim: int = 128
+    page_size: int = 16
+    group_size: int = 32
+    c_k: float = 0.156
+    c_v: float = 0.156
+    sm_scale: float = 0.0       # 0 => 1/sqrt(head_dim)
+    flags: int = 0
+
+    def c(self) -> _CConfig:
+        return _CConfig(self.num_q_heads, self.num_kv_heads, self.head_dim, self.page_size,
+                        self.group_size, self.c_k, self.c_v, self.sm_scale, self.flags)
+
+
+def library_path() -> str:
+    return _LIB_PATH
+
+
+def _load():
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise UQError(f"{_LIB_PATH} is missing: build it with `python -m paper_2606_20474_b200.build` "
+                      "(there is no CPU fallback)")
+    lib = ctypes.CDLL(_LIB_PATH)
+    vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
+    cfgp = ctypes.POINTER(_CConfig)
+    lib.uq_last_error_string.restype = ctypes.c_char_p
+    lib.uq_last_error_string.argtypes = []
+    lib.uq_cache_record_bytes.restype = ctypes.c_size_t
+    lib.uq_cache_record_bytes.argtypes = [cfgp]
+    lib.uq_rotate_quantize_append.restype = i32
+    lib.uq_rotate_quantize_append.argtypes = [cfgp, vp, vp, vp, vp, vp, i32, i32, i32, vp, i64, vp, vp, vp]
+    lib.uq_decode_attention.restype = i32
+    lib.uq_decode_attention.argtypes = [cfgp, vp, vp, i64, vp, i32, vp, i32, i32, vp, vp, vp]
+    lib.uq_merge_splits.restype = i32
+    lib.uq_merge_splits.argtypes = [cfgp, vp, vp, i32, i32, vp, vp]
+    lib.uq_suggest_num_splits.restype = i32
+    lib.uq_suggest_num_splits.argtypes = [cfgp, i32, i32]
+    _lib = lib
+    return lib
+
+
+def last_error() -> str:
+    return _load().uq_last_error_string().decode()
+
+
+def _check(status: int, what: str) -> None:
+    if status != 0:
+        raise UQError(f"{what} failed with status {status}: {last_error()}")
+
+
+def _p(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def _stream(stream) -> ctypes.c_void_p:
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def _dev(t: torch.Tensor, dtype, name: str) -> torch.Tensor:
+    if not t.is_cuda:
+        raise UQError(f"{name} must be a CUDA tensor (no CPU path exists)")
+    if t.dtype != dtype or not t.is_contiguous():
+        raise UQError(f"{name} must be contiguous {dtype}, got {t.dtype} contiguous={t.is_contiguous()}")
+    return t
+
+
+def cache_record_bytes(cfg: UQConfig) -> int:
+    c = cfg.c()
+    return int(_load().uq_cache_record_bytes(ctypes.byref(c)))
+
+
+def suggest_num_splits(cfg: UQConfig, batch: int, avg_seq_len: int) -> int:
+    c = cfg.c()
+    return int(_load().uq_suggest_num_splits(ctypes.byref(c), int(batch), int(avg_seq_len)))
+
+
+def alloc_cache(cfg: UQConfig, num_pages: int, device="cuda") -> torch.Tensor:
+    """uint8 [num_pages, num_kv_heads, 2176] (layout: include/uq.h)."""
+    return torch.zeros((num_pages, cfg.num_kv_heads, RECORD_BYTES), dtype=torch.uint8, device=device)
+
+
+def rotate_quantize_append(cfg: UQConfig, k_new, v_new, cu_new, seq_lens, block_tables, cache,
+                           q=None, q_fp8=None, stream=None) -> None:
+    """uq_rotate_quantize_append (Alg. 1 l.1-6).  k_new/v_new bf16 [total_new, Hkv, d]."""
+    lib = _load()
+    _dev(k_new, torch.bfloat16, "k_new"); _dev(v_new, torch.bfloat16, "v_new")
+    _dev(cu_new, torch.int32, "cu_new"); _dev(seq_lens, torch.int32, "seq_lens")
+    _dev(block_tables, torch.int32, "block_tables"); _dev(cache, torch.uint8, "cache")
+    if q is not None:
+        _dev(q, torch.bfloat16, "q"); _dev(q_fp8, torch.uint8, "q_fp8")
+    c = cfg.c()
+    batch = seq_lens.shape[0]
+    st = lib.uq_rotate_quantize_append(ctypes.byref(c), _p(k_new), _p(v_new), _p(cu_new), _p(seq_lens),
+                                       _p(block_tables), block_tables.shape[1], batch, k_new.shape[0],
+                                       _p(cache), cache.shape[0], _p(q), _p(q_fp8), _stream(stream))
+    _check(st, "uq_rotate_quantize_append")
+
+
+def decode_attention(cfg: UQConfig, q_fp8, cache, block_tables, seq_lens, num_splits: int,
+                     partial_acc, partial_ml, stream=None) -> None:
+    """uq_decode_attention (Alg. 1 l.7-8, split-K partials)."""
+    lib = _load()
+    _dev(q_fp8, torch.uint8, "q_fp8"); _dev(cache, torch.uint8, "cache")
+    _dev(block_tables, torch.int32, "block_tables"); _dev(seq_lens, torch.int32, "seq_lens")
+    _dev(partial_acc, torch.float32, "partial_acc"); _dev(partial_ml, torch.float32, "partial_ml")
+    c = cfg.c()
+    st = lib.uq_decode_attention(ctypes.byref(c), _p(q_fp8), _p(cache), cache.shape[0], _p(block_tables),
+                                 block_tables.shape[1], _p(seq_lens), seq_lens.shape[0], int(num_splits),
+                                 _p(partial_acc), _p(partial_ml), _stream(stream))
+    _check(st, "uq_decode_attention")
+
+
+def merge_splits(cfg: UQConfig, partial_acc, partial_ml, out, stream=None) -> None:
+    """uq_merge_splits: out bf16 [batch, Hq, d]."""
+    lib = _load()
+    _dev(partial_acc, torch.float32, "partial_acc"); _dev(partial_ml, torch.float32, "partial_ml")
+    _dev(out, torch.bfloat16, "out")
+    c = cfg.c()
+    st = lib.uq_merge_splits(ctypes.byref(c), _p(partial_acc), _p(partial_ml), out.shape[0],
+                             partial_ml.shape[2], _p(out), _stream(stream))
+    _check(st, "uq_merge_splits")
+
+
+class StepBuffers:
+    """Device scratch for one decode step (caller-owned memory, allocated once)."""
+
+    def __init__(self, cfg: UQConfig, batch: int, num_splits: int, device="cuda"):
+        self.num_splits = num_splits
+        self.q_fp8 = torch.empty((batch, cfg.num_q_heads, cfg.head_dim), dtype=torch.uint8, device=device)
+        self.partial_acc = torch.empty((batch, cfg.num_q_heads, num_splits, cfg.head_dim),
+                                       dtype=torch.float32, device=device)
+        self.partial_ml = torch.empty((batch, cfg.num_q_heads, num_splits, 2), dtype=torch.float32, device=device)
+        self.out = torch.empty((batch, cfg.num_q_heads, cfg.head_dim), dtype=torch.bfloat16, device=device)
+        self.seq_lens_after = torch.empty((batch,), dtype=torch.int32, device=device)
+        self.cu_new = torch.empty((batch + 1,), dtype=torch.int32, device=device)
+
+
+def decode_step(cfg: UQConfig, bufs: StepBuffers, q, k_new, v_new, cu_new, seq_lens_before,
+                seq_lens_after, block_tables, cache, stream=None) -> torch.Tensor:
+    """One whole hot-path step on device-resident inputs: quantize-on-append of the step's new
+    tokens (k_new may have 0 rows) with the query rotate+cast, split-K decode, merge."""
+    rotate_quantize_append(cfg, k_new, v_new, cu_new, seq_lens_before, block_tables, cache,
+                           q=q, q_fp8=bufs.q_fp8, stream=stream)
+    decode_attention(cfg, bufs.q_fp8, cache, block_tables, seq_lens_after, bufs.num_splits,
+                     bufs.partial_acc, bufs.partial_ml, stream=stream)
+    merge_splits(cfg, bufs.partial_acc, bufs.partial_ml, bufs.out, stream=stream)
+    return bufs.out
+
+
+def decode_step_host(cfg: UQConfig, bufs: StepBuffers, dev_in: dict, q_host, k_new_host, v_new_host,
+                     cu_new_host, seq_lens_before_host, seq_lens_after_host, block_tables_host,
+                     cache, out_host, stream=None) -> torch.Tensor:
+    """The same step with HOST (pinned) inputs and output: the step's query, new K/V rows,
+    lengths and block tables are copied host->device, the attention output device->host.  The
+    KV cache itself is the resident state and stays in HBM.  dev_in holds preallocated device
+    tensors with keys q, k_new, v_new, cu_new, seq_lens_before, seq_lens_after, block_tables."""
+    dev_in["q"].copy_(q_host, non_blocking=True)
+    if k_new_host.shape[0] > 0:
+        dev_in["k_new"].copy_(k_new_host, non_blocking=True)
+        dev_in["v_new"].copy_(v_new_host, non_blocking=True)
+    dev_in["cu_new"].copy_(cu_new_host, non_blocking=True)
+    dev_in["seq_lens_before"].copy_(seq_lens_before_host, non_blocking=True)
+    dev_in["seq_lens_after"].copy_(seq_lens_after_host, non_blocking=True)
+    dev_in["block_tables"].copy_(block_tables_host, non_blocking=True)
+    out = decode_step(cfg, bufs, dev_in["q"], dev_in["k_new"], dev_in["v_new"], dev_in["cu_new"],
+                      dev_in["seq_lens_before"], dev_in["seq_lens_after"], dev_in["block_tables"],
+                      cache, stream=stream)
+    out_host.copy_(out, non_blocking=True)
+    return out_host

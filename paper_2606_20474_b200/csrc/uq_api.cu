@@ -1,0 +1,84 @@
+// uq_api.cu — host-side plumbing of libuq.so: error string, config validation, small queries.
+#include <stdarg.h>
+
+#include "uq_common.cuh"
+
+namespace uq {
+
+static thread_local char g_err[256] = "no error";
+
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+
+int32_t check_config(const uq_config* cfg) {
+  if (cfg == nullptr) {
+    set_error("uq_config is NULL");
+    return UQ_ERR_INVALID_ARG;
+  }
+  if (cfg->num_q_heads <= 0 || cfg->num_kv_heads <= 0 || cfg->head_dim <= 0 ||
+      cfg->page_size <= 0 || cfg->group_size <= 0) {
+    set_error("uq_config: non-positive dimension");
+    return UQ_ERR_INVALID_ARG;
+  }
+  if (cfg->num_q_heads % cfg->num_kv_heads != 0) {
+    set_error("uq_config: num_q_heads %d not a multiple of num_kv_heads %d", cfg->num_q_heads,
+              cfg->num_kv_heads);
+    return UQ_ERR_INVALID_ARG;
+  }
+  if (!(cfg->c_k > 0.0f) || !(cfg->c_v > 0.0f)) {
+    set_error("uq_config: c_k and c_v must be positive");
+    return UQ_ERR_INVALID_ARG;
+  }
+  if (cfg->flags != 0) {
+    set_error("uq_config: flags must be 0");
+    return UQ_ERR_INVALID_ARG;
+  }
+  if (cfg->head_dim != kHeadDim || cfg->group_size != kGroup || cfg->page_size != kPage) {
+    set_error("unsupported geometry: head_dim %d group %d page %d (supported: 128/32/16)",
+              cfg->head_dim, cfg->group_size, cfg->page_size);
+    return UQ_ERR_UNSUPPORTED;
+  }
+  if (cfg->num_q_heads / cfg->num_kv_heads > 16) {
+    set_error("unsupported GQA group %d (> 16)", cfg->num_q_heads / cfg->num_kv_heads);
+    return UQ_ERR_UNSUPPORTED;
+  }
+  return UQ_OK;
+}
+
+int32_t check_cuda(cudaError_t e, const char* what) {
+  if (e == cudaSuccess) return UQ_OK;
+  set_error("%s: %s", what, cudaGetErrorString(e));
+  return UQ_ERR_CUDA;
+}
+
+}  // namespace uq
+
+extern "C" const char* uq_last_error_string(void) { return uq::g_err; }
+
+extern "C" size_t uq_cache_record_bytes(const uq_config* cfg) {
+  if (uq::check_config(cfg) != UQ_OK) return 0;
+  return (size_t)cfg->page_size * (size_t)(cfg->head_dim / 2 + cfg->head_dim / cfg->group_size) * 2;
+}
+
+extern "C" int32_t uq_suggest_num_splits(const uq_config* cfg, int32_t batch, int32_t avg_seq_len) {
+  if (uq::check_config(cfg) != UQ_OK || batch <= 0) return 1;
+  int dev = 0, sms = 148;
+  if (cudaGetDevice(&dev) == cudaSuccess) {
+    int v = 0;
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) sms = v;
+  }
+  // Aim at ~4 waves of 3 resident CTAs per SM, but keep >= 64 pages (1024 tokens) per split.
+  const int64_t items = (int64_t)batch * cfg->num_kv_heads;
+  const int64_t want = (int64_t)sms * 3 * 4;
+  int64_t s = (want + items - 1) / items;
+  const int64_t pages = (avg_seq_len + cfg->page_size - 1) / cfg->page_size;
+  const int64_t max_s = pages / 64 > 0 ? pages / 64 : 1;
+  if (s > max_s) s = max_s;
+  if (s < 1) s = 1;
+  if (s > 256) s = 256;
+  return (int32_t)s;
+}

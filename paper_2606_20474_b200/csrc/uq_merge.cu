@@ -1,0 +1,73 @@
+// uq_merge.cu — merge of split-K partials (flash-decoding reduction; not in the paper, exact
+// reassociation of the softmax in Alg. 1 l.8; format in include/uq.h).
+//
+// One warp per (sequence, query head); a lane owns 4 of the 128 output channels (one 16-byte
+// load per split, coalesced 512 B per warp).  HBM-bound: reads S*(512+8) B, writes 256 B per row.
+#include <cuda_bf16.h>
+
+#include "uq_common.cuh"
+
+namespace uq {
+namespace {
+
+__global__ void __launch_bounds__(128)
+merge_kernel(const float* __restrict__ acc, const float* __restrict__ ml, int rows, int S,
+             __nv_bfloat16* __restrict__ out) {
+  const int lane = threadIdx.x & 31;
+  const int row = blockIdx.x * 4 + (threadIdx.x >> 5);
+  if (row >= rows) return;
+  const float2* ml2 = reinterpret_cast<const float2*>(ml) + (long long)row * S;
+  // pass 1: M = max over non-empty splits (lanes stride over splits, then warp max)
+  float M = -INFINITY;
+  for (int s = lane; s < S; s += 32) {
+    const float2 v = ml2[s];
+    if (v.y > 0.0f) M = fmaxf(M, v.x);
+  }
+#pragma unroll
+  for (int o = 16; o; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+  float4 num = make_float4(0.f, 0.f, 0.f, 0.f);
+  float den = 0.f;
+  if (M > -INFINITY) {
+    const float4* a4 = reinterpret_cast<const float4*>(acc) + (long long)row * S * 32 + lane;
+    for (int s = 0; s < S; ++s) {
+      const float2 v = ml2[s];
+      if (!(v.y > 0.0f)) continue;
+      const float w = __expf(v.x - M);
+      const float4 a = a4[(long long)s * 32];
+      num.x = fmaf(w, a.x, num.x);
+      num.y = fmaf(w, a.y, num.y);
+      num.z = fmaf(w, a.z, num.z);
+      num.w = fmaf(w, a.w, num.w);
+      den = fmaf(w, v.y, den);
+    }
+  }
+  const float inv = den > 0.f ? 1.0f / den : 0.f;
+  __nv_bfloat162 lo = __floats2bfloat162_rn(num.x * inv, num.y * inv);
+  __nv_bfloat162 hi = __floats2bfloat162_rn(num.z * inv, num.w * inv);
+  uint2 packed;
+  packed.x = *reinterpret_cast<uint32_t*>(&lo);
+  packed.y = *reinterpret_cast<uint32_t*>(&hi);
+  *reinterpret_cast<uint2*>(out + (long long)row * kHeadDim + 4 * lane) = packed;
+}
+
+}  // namespace
+}  // namespace uq
+
+extern "C" int32_t uq_merge_splits(const uq_config* cfg, const float* partial_acc, const float* partial_ml,
+                                   int32_t batch, int32_t num_splits, void* out_bf16, void* stream) {
+  using namespace uq;
+  int32_t st = check_config(cfg);
+  if (st != UQ_OK) return st;
+  if (batch <= 0 || num_splits <= 0 || !partial_acc || !partial_ml || !out_bf16) {
+    set_error("merge: NULL pointer or non-positive batch/num_splits");
+    return UQ_ERR_INVALID_ARG;
+  }
+  if (((uintptr_t)partial_acc & 15u) || ((uintptr_t)partial_ml & 7u) || ((uintptr_t)out_bf16 & 7u)) {
+    set_error("merge: misaligned pointer (partial_acc 16 B, partial_ml 8 B, out 8 B)");
+    return UQ_ERR_INVALID_ARG;
+  }
+  const int rows = batch * cfg->num_q_heads;
+  merge_kernel<<<(rows + 3) / 4, 128, 0, (cudaStream_t)stream>>>(partial_acc, partial_ml, rows, num_splits,
+                                                              (__nv_bfloat16*)out_bf16);
+  return check_cuda(cudaGetLastError(), "uq_merge_splits launch");
+}

@@ -1,0 +1,72 @@
+"""CPU-side checks of the boundary: libuq.so builds for sm_100a, loads without a GPU, exports
+every symbol include/uq.h declares, and validates arguments on the host (no compute calls)."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2606_20474_b200 as uq
+from paper_2606_20474_b200 import binding, build
+from tests import uq_layout
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return binding._load()
+
+
+def test_exports_every_declared_symbol(lib):
+    hdr = open(os.path.join(ROOT, "include", "uq.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(uq_[a-z_0-9]+)\s*\(", hdr))
+    assert {"uq_rotate_quantize_append", "uq_decode_attention", "uq_merge_splits"} <= declared
+    for name in declared:
+        assert hasattr(lib, name), f"{name} declared in uq.h but not exported"
+
+
+def test_record_bytes_is_4_25_bits_per_element(lib):
+    cfg = uq.UQConfig(64, 4)
+    assert uq.cache_record_bytes(cfg) == uq.RECORD_BYTES == 2176
+    assert 2176 * 8 / (16 * 128 * 2) == 4.25
+    count = uq_layout.used_byte_mask()
+    assert np.all(count[:1024] == 1) and np.all(count[1024:2048] == 2) and np.all(count[2048:] == 1)
+
+
+def test_host_side_validation(lib):
+    c = uq.UQConfig(64, 4).c()
+    f = lib.uq_merge_splits
+    assert f(None, None, None, 1, 1, None, None) == 1      # UQ_ERR_INVALID_ARG: NULL config
+    assert b"NULL" in lib.uq_last_error_string()
+    bad = uq.UQConfig(64, 5).c()
+    assert f(ctypes.byref(bad), None, None, 1, 1, None, None) == 1
+    bad = uq.UQConfig(64, 4, head_dim=64).c()
+    assert f(ctypes.byref(bad), None, None, 1, 1, None, None) == 2   # UQ_ERR_UNSUPPORTED
+    bad = uq.UQConfig(64, 2).c()                           # GQA group 32
+    assert f(ctypes.byref(bad), None, None, 1, 1, None, None) == 2
+    assert f(ctypes.byref(c), None, None, 1, 1, None, None) == 1     # NULL buffers
+    assert lib.uq_decode_attention(ctypes.byref(c), None, None, 1, None, 1, None, 1, 1, None, None, None) == 1
+    assert lib.uq_rotate_quantize_append(ctypes.byref(c), None, None, None, None, None, 1, 1, 4, None, 1,
+                                         None, None, None) == 1
+    assert uq.cache_record_bytes(uq.UQConfig(64, 4, page_size=32)) == 0
+
+
+def test_binding_refuses_cpu_tensors(lib):
+    import torch
+    cfg = uq.UQConfig(8, 1)
+    out = torch.zeros((1, 8, 128), dtype=torch.bfloat16)
+    with pytest.raises(uq.UQError):
+        uq.merge_splits(cfg, torch.zeros((1, 8, 1, 128)), torch.zeros((1, 8, 1, 2)), out)
+
+
+def test_product_package_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2606_20474_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for fn in files:
+            if fn.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, fn)).read()
+                assert "import oracle" not in src and "from oracle" not in src and "uq_oracle" not in src, fn

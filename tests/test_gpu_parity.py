@@ -1,0 +1,202 @@
+"""Parity of the CUDA path (through the C ABI / Python binding) with the float64 oracle.
+Codes, scale bytes and q_fp8: bit-exact.  Attention outputs: |gpu - ref| <= 2e-3 + 1e-2 |ref|
+(BASELINE.json north_star).  All inputs are seeded and synthetic (workloads.py)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2606_20474_b200 as uq
+from paper_2606_20474_b200 import workloads as W
+from tests import harness as H
+from tests import uq_layout
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+
+def _full_check(wl, splits_list, sample_seqs=None, check_cache=True):
+    cfg = H.cfg_of(wl)
+    cache, bt = H.fill_cache(cfg, wl, DEV)
+    q = W.gen_q(wl, DEV)
+    qb = H.bits(q)
+    seqs = range(wl.batch) if sample_seqs is None else sample_seqs
+    arrays = {b: H.oracle_sequence_cache(wl, b, int(wl.ctx_lens[b]), DEV) for b in seqs}
+    if check_cache:
+        for b in seqs:
+            H.compare_cache(cache, wl, b, int(wl.ctx_lens[b]), arrays[b])
+    worst = 0.0
+    for S in splits_list:
+        out, q_fp8, _ = H.run_decode(cfg, cache, bt, wl.ctx_lens, q, S)
+        out = out.float().cpu().numpy().astype(np.float64)
+        for b in seqs:
+            ref, q8 = H.oracle_out(wl, b, int(wl.ctx_lens[b]), qb[b], arrays[b])
+            assert np.array_equal(q_fp8[b].cpu().numpy(), q8), f"q_fp8 differs for seq {b}"
+            worst = max(worst, H.check_out(out[b], ref, f"{wl.name} seq {b} S={S}"))
+    return worst
+
+
+def test_cfg1_tiny_whole_cache_bit_exact_and_decode():
+    wl = W.make_config(1, peaked_frac=0.25)
+    _full_check(wl, [1, 4, 7])
+
+
+@pytest.mark.parametrize("hq,hkv", [(8, 8), (12, 2), (16, 2), (32, 2), (5, 1)])
+def test_ragged_batch_all_gqa_groups(hq, hkv):
+    # empty, 1-token, ragged tails, several pages; GQA groups 1, 6, 8, 16, 5
+    wl = W.make_custom("ragged", 11, [0, 1, 17, 203, 1000, 16, 31, 32], hq, hkv,
+                       outlier_channels=3, outlier_gain=8.0, peaked_frac=0.3)
+    _full_check(wl, [1, 3, 64])
+
+
+def test_zero_length_rows_are_zero():
+    wl = W.make_custom("empty", 12, [0, 0, 5], 8, 2)
+    cfg = H.cfg_of(wl)
+    cache, bt = H.fill_cache(cfg, wl, DEV)
+    out, _, _ = H.run_decode(cfg, cache, bt, wl.ctx_lens, W.gen_q(wl, DEV), 2)
+    assert torch.all(out[:2] == 0)
+
+
+def test_incremental_appends_match_bulk_and_oracle():
+    """Tokens arriving one at a time / in odd-sized pieces (V-code bytes shared by token pairs,
+    page boundaries) give the same cache image as the oracle's encoding."""
+    wl = W.make_custom("incr", 13, [75, 40, 1], 8, 2, extra_tokens=0)
+    cfg = H.cfg_of(wl)
+    cache = uq.alloc_cache(cfg, wl.num_pages, DEV)
+    cache.fill_(0xA5)                                   # stale garbage must be overwritten
+    bt = torch.from_numpy(wl.block_tables).to(DEV)
+    full = [W.gen_kv(wl, b, 0, int(wl.ctx_lens[b]), DEV) for b in range(wl.batch)]
+    pos = np.zeros(wl.batch, np.int32)
+    pieces = [3, 1, 1, 14, 2, 1, 33, 1, 100]
+    for n in pieces:
+        counts = np.minimum(n, wl.ctx_lens - pos).astype(np.int32)
+        if counts.sum() == 0:
+            break
+        k = torch.cat([full[b][0][pos[b]:pos[b] + counts[b]] for b in range(wl.batch)])
+        v = torch.cat([full[b][1][pos[b]:pos[b] + counts[b]] for b in range(wl.batch)])
+        H.append_tokens(cfg, cache, bt, pos, counts, k, v)
+        pos = pos + counts
+    torch.cuda.synchronize()
+    assert np.array_equal(pos, wl.ctx_lens)
+    for b in range(wl.batch):
+        arrays = H.oracle_sequence_cache(wl, b, int(wl.ctx_lens[b]), DEV)
+        H.compare_cache(cache, wl, b, int(wl.ctx_lens[b]), arrays)
+    # and decode over the (partly garbage-filled last) pages stays in tolerance
+    q = W.gen_q(wl, DEV)
+    out, _, _ = H.run_decode(cfg, cache, bt, wl.ctx_lens, q, 2)
+    for b in range(wl.batch):
+        ref, _ = H.oracle_out(wl, b, int(wl.ctx_lens[b]), H.bits(q)[b])
+        H.check_out(out[b].float().cpu().numpy().astype(np.float64), ref, f"incr seq {b}")
+
+
+def test_shared_prefix_steps_cfg4_scaled():
+    """Config 4 shape at 1/64 scale: shared prefix pages named by every block table, then three
+    timed-style steps (append 1 token per sequence, decode, merge)."""
+    wl = W.make_config(4, scale=1 / 64, peaked_frac=0.05)
+    cfg = H.cfg_of(wl)
+    cache, bt = H.fill_cache(cfg, wl, DEV)
+    S = 3
+    bufs = uq.StepBuffers(cfg, wl.batch, S, DEV)
+    lens = wl.ctx_lens.copy()
+    cu = torch.arange(wl.batch + 1, dtype=torch.int32, device=DEV)
+    appended_k, appended_v = [], []
+    for step in range(3):
+        q = W.gen_q(wl, DEV, step)
+        k_new, v_new = W.gen_new_kv(wl, step, DEV)
+        appended_k.append(k_new); appended_v.append(v_new)
+        before = torch.from_numpy(lens).to(DEV)
+        after = torch.from_numpy(lens + 1).to(DEV)
+        out = uq.decode_step(cfg, bufs, q, k_new, v_new, cu, before, after, bt, cache)
+        torch.cuda.synchronize()
+        lens = lens + 1
+        out = out.float().cpu().numpy().astype(np.float64)
+        for b in (0, wl.batch // 2, wl.batch - 1):
+            L0 = int(wl.ctx_lens[b])
+            k0, v0 = W.seq_kv(wl, b, L0, DEV)
+            k = torch.cat([k0] + [a[b:b + 1] for a in appended_k])
+            v = torch.cat([v0] + [a[b:b + 1] for a in appended_v])
+            arrays = oracle.encode_kv(H.bits(k), H.bits(v))
+            H.compare_cache(cache, wl, b, int(lens[b]), arrays)
+            ref, q8 = H.oracle_out(wl, b, int(lens[b]), H.bits(q)[b], arrays)
+            assert np.array_equal(bufs.q_fp8[b].cpu().numpy(), q8)
+            H.check_out(out[b], ref, f"cfg4 step {step} seq {b}")
+
+
+@pytest.mark.parametrize("idx,scale", [(2, 1 / 16), (3, 1 / 16), (5, 1 / 32)])
+def test_scaled_configs(idx, scale):
+    wl = W.make_config(idx, scale=scale, peaked_frac=0.05)
+    S = uq.suggest_num_splits(H.cfg_of(wl), wl.batch, int(wl.ctx_lens.mean()))
+    _full_check(wl, sorted({1, S}), sample_seqs=list(range(min(wl.batch, 3))))
+
+
+def test_merge_on_hand_made_partials():
+    rng = np.random.default_rng(21)
+    B, Hq, S, d = 3, 8, 5, 128
+    cfg = uq.UQConfig(Hq, 2)
+    acc = rng.standard_normal((B, Hq, S, d)).astype(np.float32)
+    m = (rng.standard_normal((B, Hq, S)) * 20).astype(np.float32)
+    l = rng.uniform(0.5, 50, (B, Hq, S)).astype(np.float32)
+    m[0, 0, 1] = -np.inf; l[0, 0, 1] = 0                 # an empty split
+    m[1, :, :] = -np.inf; l[1, :, :] = 0                 # a sequence of length 0
+    ml = np.stack([m, l], axis=-1)
+    out = torch.empty((B, Hq, d), dtype=torch.bfloat16, device=DEV)
+    uq.merge_splits(cfg, torch.from_numpy(acc).to(DEV), torch.from_numpy(ml).to(DEV), out)
+    torch.cuda.synchronize()
+    out = out.float().cpu().numpy().astype(np.float64)
+    a64, m64, l64 = acc.astype(np.float64), m.astype(np.float64), l.astype(np.float64)
+    with np.errstate(invalid="ignore"):
+        M = m64.max(axis=-1, keepdims=True)
+        w = np.where(l64 > 0, np.exp(m64 - M), 0.0)
+        den = (w * l64).sum(-1)
+        ref = (w[..., None] * a64).sum(-2) / np.where(den > 0, den, 1)[..., None]
+    ref[1] = 0
+    assert np.all(out[1] == 0)
+    assert np.allclose(out, ref, atol=1e-3 + 8e-3 * np.abs(ref).max(), rtol=8e-3)
+    assert np.abs(out - ref).max() <= 2 ** -8 * np.abs(ref).max() + 1e-6   # bf16 rounding only
+
+
+def test_wide_scale_spread_and_zero_vectors():
+    """V group scales spread over > 15 binades inside one page, all-zero K/V tokens, and huge K."""
+    wl = W.make_custom("spread", 14, [64], 16, 1)
+    cfg = H.cfg_of(wl)
+    k, v = W.gen_kv(wl, 0, 0, 64, DEV)
+    v = v.float()
+    v[0:4] *= 2.0 ** 12
+    v[4:8, :, 32:64] *= 2.0 ** -20
+    v[8] = 0
+    k = k.float(); k[8] = 0; k[9] *= 300.0
+    k, v = k.to(torch.bfloat16), v.to(torch.bfloat16)
+    cache = uq.alloc_cache(cfg, wl.num_pages, DEV)
+    bt = torch.from_numpy(wl.block_tables).to(DEV)
+    H.append_tokens(cfg, cache, bt, np.zeros(1, np.int32), np.array([64], np.int32), k, v)
+    arrays = oracle.encode_kv(H.bits(k), H.bits(v))
+    H.compare_cache(cache, wl, 0, 64, arrays)
+    q = W.gen_q(wl, DEV) * 0.05                            # diffuse attention: every token counts
+    out, _, _ = H.run_decode(cfg, cache, bt, wl.ctx_lens, q.to(torch.bfloat16), 1)
+    ref, _ = H.oracle_out(wl, 0, 64, H.bits(q.to(torch.bfloat16))[0], arrays)
+    got = out[0].float().cpu().numpy().astype(np.float64)
+    # tolerance relative to the dominant magnitude: rows hold values ~2^12
+    err = np.abs(got - ref)
+    assert np.all(err <= 2e-3 + 1e-2 * np.abs(ref) + 2.0 ** -14 * np.abs(ref).max()), err.max()
+
+
+def test_permuting_physical_pages_leaves_output_unchanged():
+    wl_a = W.make_custom("perm", 15, [300, 77], 8, 1, permute=False)
+    wl_b = W.make_custom("perm", 15, [300, 77], 8, 1, permute=True)
+    outs = []
+    for wl in (wl_a, wl_b):
+        cfg = H.cfg_of(wl)
+        cache, bt = H.fill_cache(cfg, wl, DEV)
+        out, _, _ = H.run_decode(cfg, cache, bt, wl.ctx_lens, W.gen_q(wl, DEV), 2)
+        outs.append(out)
+    assert not np.array_equal(wl_a.block_tables, wl_b.block_tables)
+    assert torch.equal(outs[0], outs[1])
+
+
+def test_full_size_cfg2_in_bench_launch_configuration_sampled():
+    """BASELINE.json config 2 at full size (32 x 32,768 tokens, 64/4 heads), decoded with the
+    num_splits bench.py uses; sampled sequences are checked row by row against the oracle."""
+    wl = W.make_config(2)
+    cfg = H.cfg_of(wl)
+    S = uq.suggest_num_splits(cfg, wl.batch, int(wl.ctx_lens.mean()))
+    _full_check(wl, [S], sample_seqs=[0, 17, 31], check_cache=True)
