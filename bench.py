@@ -1,0 +1,452 @@
+#!/usr/bin/env python
+"""bench.py — throughput of UltraQuant's hot path on B200 (driver contract: see README/DESIGN.md).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 2|3|5|1]
+
+One STEP = one pass of the whole hot path over one decode batch:
+  uq_rotate_quantize_append  (1 new K/V token per sequence: rotate, scale, encode, paged store;
+                              plus the step's queries: rotate + FP8 cast)
+  uq_decode_attention        (paged split-K FP8 x FP4 attention over the whole context)
+  uq_merge_splits            (split partials -> bf16 output)
+Workload (default): BASELINE.json configs[1] — Qwen3-235B-shaped layer, 64 Q / 4 KV heads,
+head_dim 128, batch 32, every sequence at 32,768 tokens, page_size 16, random block tables,
+K,V bf16 ~ N(0,1) with 3 K channels x8 (seed 1).  The cache is prefilled to 32,767 tokens per
+sequence through uq_rotate_quantize_append; every timed step appends token 32,768 (into the
+same slot each step, so the context stays at exactly 32,768) and decodes over 32,768 tokens.
+
+Metric = BASELINE.json's "decode-attention HBM GB/s": algorithmic bytes the step must move
+(136 B per (token, kv_head) of K+V codes and scales, block tables, Q, O, split partials, the
+appended rows — SURVEY.md §8(d)) divided by the device time of the step.  us/step and the
+fractions of the nominal 8 TB/s and of the measured copy peak ride along in the same line.
+
+--impl reference times the float64 CPU oracle (oracle/) on the same metric and config; it and
+the cpu_baseline leg are the only places this file touches oracle/.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+import torch
+
+METRIC = "decode_attention_hbm_gbps"
+UNIT = "GB/s"
+NOMINAL_HBM_GBS = 8000.0          # BASELINE.json north_star: "the B200's ~8 TB/s peak"
+FALLBACK_HBM_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md fallback
+
+# dram__bytes_read.sum + dram__bytes_write.sum per decode_kernel launch from the committed
+# `ncu --set full` capture of this command (profiles/), keyed by config; None = not captured.
+NCU_TRAFFIC_BYTES = {}
+
+
+# ----------------------------------------------------------------------------- helpers
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy read+write)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s; MEASURED_PEAKS.json absent)"
+
+
+def _workload(idx: int, rank: int):
+    import dataclasses
+
+    from paper_2606_20474_b200 import workloads as W
+    wl = W.make_config(idx, peaked_frac=0.0)
+    if rank:
+        wl = dataclasses.replace(wl, seed=wl.seed + 1000 * rank)   # other values, same structure
+    return wl
+
+
+def step_bytes(wl, num_splits: int, ctx_after: np.ndarray, new_per_seq: int):
+    """Algorithmic bytes of one step; returns (total, decode_kernel_only)."""
+    d, Hq, Hkv, B = wl.head_dim, wl.num_q_heads, wl.num_kv_heads, wl.batch
+    per_tok = 2 * (d // 2 + d // 32)                                 # 136 B
+    tokens = int(ctx_after.astype(np.int64).sum())
+    pages = int(((ctx_after.astype(np.int64) + wl.page_size - 1) // wl.page_size).sum())
+    kv = tokens * Hkv * per_tok
+    bt = 4 * pages
+    q8 = B * Hq * d
+    partials = B * Hq * num_splits * (4 * d + 8)
+    decode = kv + bt + q8 + partials                                 # decode kernel: read KV, tables, Q; write partials
+    merge = partials + B * Hq * d * 2                                # read partials, write bf16 O
+    n_new = B * new_per_seq
+    append = n_new * Hkv * (2 * d * 2 + per_tok) + B * Hq * (2 * d + d)   # read bf16 K,V rows + Q; write records + q_fp8
+    return decode + merge + append, decode
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed regions run."""
+
+    def __init__(self, index: int, period_s: float = 0.02):
+        super().__init__(daemon=True)
+        self.period = period_s
+        self.samples = []            # (busy flag, sm_mhz, reasons bitmask)
+        self.busy = False
+        self._stop_evt = threading.Event()
+        self.ok = False
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:     # no NVML: the line says so instead of inventing clocks
+            self.err = repr(e)
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        while not self._stop_evt.is_set():
+            try:
+                mhz = int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                reasons = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                self.samples.append((self.busy, mhz, reasons))
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+
+    def summary(self):
+        if not self.ok:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml_unavailable"]}
+        nv = self.nv
+        busy = [s for s in self.samples if s[0]] or self.samples
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake_slowdown",
+        }
+        seen = set()
+        for _, _, r in busy:
+            for bit, nm in names.items():
+                if r & bit:
+                    seen.add(nm)
+        return {"sm_mhz": (statistics.median([s[1] for s in busy]) if busy else None),
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(seen), "samples": len(busy)}
+
+
+# ----------------------------------------------------------------------------- our arm
+def fill_cache(uq, W, cfg, wl, lens, device, chunk_tokens=1 << 16):
+    """Prefill through uq_rotate_quantize_append (bulk appends); shared prefix written once."""
+    cache = uq.alloc_cache(cfg, wl.num_pages, device)
+    bt_dev = torch.from_numpy(wl.block_tables).to(device)
+    B = wl.batch
+
+    def put(b_gen, b_tab, start, n_total):
+        done = 0
+        while done < n_total:
+            n = min(chunk_tokens, n_total - done)
+            k, v = W.gen_kv(wl, b_gen, done, done + n, device)
+            before = np.zeros(B, np.int32); before[b_tab] = start + done
+            cu = np.zeros(B + 1, np.int32); cu[b_tab + 1:] = n
+            uq.rotate_quantize_append(cfg, k, v, torch.from_numpy(cu).to(device),
+                                      torch.from_numpy(before).to(device), bt_dev, cache)
+            done += n
+
+    if wl.prefix_len:
+        put(-1, 0, 0, wl.prefix_len)
+    for b in range(B):
+        put(b, b, wl.prefix_len, int(lens[b]) - wl.prefix_len)
+    torch.cuda.synchronize()
+    return cache, bt_dev
+
+
+def run_ours(args, rank, world, local_rank):
+    import paper_2606_20474_b200 as uq
+    from paper_2606_20474_b200 import workloads as W
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the hot path has no CPU fallback")
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    wl = _workload(args.config, rank)
+    cfg = uq.UQConfig(num_q_heads=wl.num_q_heads, num_kv_heads=wl.num_kv_heads)
+    B, Hq, Hkv, d = wl.batch, wl.num_q_heads, wl.num_kv_heads, wl.head_dim
+
+    # context AFTER the step's append = the config's lengths; the cache holds one token less
+    ctx_after = wl.ctx_lens.astype(np.int32)
+    ctx_before = ctx_after - 1
+    cache, bt_dev = fill_cache(uq, W, cfg, wl, ctx_before, dev)
+    S = args.splits or uq.suggest_num_splits(cfg, B, int(ctx_after.mean()))
+    bufs = uq.StepBuffers(cfg, B, S, dev)
+
+    # a small ring of per-step inputs (different values each step)
+    n_in = 4
+    qs = [W.gen_q(wl, dev, step=i) for i in range(n_in)]
+    wl1 = wl if wl.new_tokens == 1 else __import__("dataclasses").replace(wl, new_tokens=1)
+    kvs = [W.gen_new_kv(wl1, i, dev) for i in range(n_in)]
+    cu_dev = torch.arange(B + 1, dtype=torch.int32, device=dev)
+    before_dev = torch.from_numpy(ctx_before).to(dev)
+    after_dev = torch.from_numpy(ctx_after).to(dev)
+    stream = torch.cuda.current_stream()
+
+    def step(i):
+        k_new, v_new = kvs[i % n_in]
+        return uq.decode_step(cfg, bufs, qs[i % n_in], k_new, v_new, cu_dev, before_dev, after_dev,
+                              bt_dev, cache, stream=stream)
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+
+    # ---- device-resident timing: W warm-up, then exactly K steps between two events
+    for i in range(max(args.warmup, 3)):
+        step(i)
+    barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    dec_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+              for _ in range(args.steps)]
+    sampler.busy = True
+    ev0.record(stream)
+    for i in range(args.steps):
+        k_new, v_new = kvs[i % n_in]
+        uq.rotate_quantize_append(cfg, k_new, v_new, cu_dev, before_dev, bt_dev, cache,
+                                  q=qs[i % n_in], q_fp8=bufs.q_fp8, stream=stream)
+        dec_ev[i][0].record(stream)
+        uq.decode_attention(cfg, bufs.q_fp8, cache, bt_dev, after_dev, S, bufs.partial_acc,
+                            bufs.partial_ml, stream=stream)
+        dec_ev[i][1].record(stream)
+        uq.merge_splits(cfg, bufs.partial_acc, bufs.partial_ml, bufs.out, stream=stream)
+    ev1.record(stream)
+    barrier()
+    sampler.busy = False
+    ms_total = ev0.elapsed_time(ev1)
+    dec_ms = [a.elapsed_time(b) for a, b in dec_ev]
+
+    # ---- end-to-end through the public host-buffer API: H2D of the step's inputs, D2H of O
+    host = {
+        "q": [q.cpu().pin_memory() for q in qs],
+        "k": [kv[0].cpu().pin_memory() for kv in kvs],
+        "v": [kv[1].cpu().pin_memory() for kv in kvs],
+        "cu": cu_dev.cpu().pin_memory(), "before": before_dev.cpu().pin_memory(),
+        "after": after_dev.cpu().pin_memory(), "bt": bt_dev.cpu().pin_memory(),
+        "out": torch.empty((B, Hq, d), dtype=torch.bfloat16).pin_memory(),
+    }
+    dev_in = {"q": torch.empty_like(qs[0]), "k_new": torch.empty_like(kvs[0][0]),
+              "v_new": torch.empty_like(kvs[0][1]), "cu_new": torch.empty_like(cu_dev),
+              "seq_lens_before": torch.empty_like(before_dev), "seq_lens_after": torch.empty_like(after_dev),
+              "block_tables": torch.empty_like(bt_dev)}
+
+    def step_host(i):
+        j = i % n_in
+        uq.decode_step_host(cfg, bufs, dev_in, host["q"][j], host["k"][j], host["v"][j], host["cu"],
+                            host["before"], host["after"], host["bt"], cache, host["out"], stream=stream)
+        stream.synchronize()           # the caller reads O before it can issue the next step
+
+    h2d = sum(t.numel() * t.element_size() for t in (host["q"][0], host["k"][0], host["v"][0], host["cu"],
+                                                     host["before"], host["after"], host["bt"]))
+    d2h = host["out"].numel() * host["out"].element_size()
+    for i in range(max(args.warmup, 3)):
+        step_host(i)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler.busy = True
+    e0.record(stream)
+    for i in range(args.steps):
+        step_host(i)
+    e1.record(stream)
+    barrier()
+    sampler.busy = False
+    ms_e2e = e0.elapsed_time(e1)
+    sampler.stop()
+
+    # ---- reduce over ranks: max time, summed bytes
+    total_b, decode_b = step_bytes(wl, S, ctx_after, 1)
+    t = torch.tensor([ms_total, ms_e2e, statistics.fmean(dec_ms)], dtype=torch.float64, device=dev)
+    if world > 1:
+        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+    ms_total, ms_e2e, dec_ms_mean = (float(x) for x in t.cpu())
+    ms_step = ms_total / args.steps
+    value = world * total_b / (ms_step * 1e-3) / 1e9
+    e2e_value = world * total_b / (ms_e2e / args.steps * 1e-3) / 1e9
+    peak, peak_src = _peaks()
+    achieved = decode_b / (dec_ms_mean * 1e-3) / 1e9
+    line = {
+        "metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": round(ms_step, 5),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "fp8xfp4->f32",
+        "data": "synthetic", "impl": "ours",
+        "config": {"workload": f"BASELINE.json configs[{args.config - 1}] {wl.name}: batch {B}, "
+                               f"{Hq} Q / {Hkv} KV heads, head_dim {d}, ctx {int(ctx_after.min())}"
+                               f"..{int(ctx_after.max())} tokens, page_size {wl.page_size}, random block tables; "
+                               "step = append 1 token/seq + rotate/FP8 Q + split-K decode + merge",
+                   "batch_per_gpu": B, "tokens_per_gpu": int(ctx_after.astype(np.int64).sum()),
+                   "num_splits": S, "parallelism": f"replica x{world} (sequences sharded, no collective)",
+                   "l2": f"KV working set {wl.kv_bytes_per_step() / 1e6:.0f} MB per step >> 126 MB L2 (no flush needed)"},
+        "us_per_step": round(ms_step * 1e3, 2),
+        "decode_kernel_us": round(dec_ms_mean * 1e3, 2),
+        "bytes_per_step": total_b,
+        "frac_of_nominal_8TBs": round(value / world / NOMINAL_HBM_GBS, 4),
+        "frac_of_measured_peak": round(value / world / peak, 4),
+        "e2e": {"value": round(e2e_value, 1), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                "d2h_bytes_per_step": int(d2h), "us_per_step": round(ms_e2e / args.steps * 1e3, 2),
+                "note": "host pinned Q/K_new/V_new/lens/block tables -> device, O -> host, sync every step; "
+                        "the FP4 cache is resident state"},
+        "gpu_launches": 3 * args.steps,
+        "clocks": sampler.summary(),
+        "roofline": {"bound": "hbm", "kernel": "uq::decode_kernel", "achieved": round(achieved, 1),
+                     "peak": peak, "unit": "GB/s", "frac": round(achieved / peak, 4),
+                     "frac_of_nominal_8TBs": round(achieved / NOMINAL_HBM_GBS, 4),
+                     "traffic": NCU_TRAFFIC_BYTES.get(args.config), "algorithmic_bytes": decode_b,
+                     "peak_source": peak_src,
+                     "timing": "CUDA events around every uq_decode_attention launch inside the timed region, mean"},
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(args.config, budget_s=args.cpu_budget)
+    return line
+
+
+# ----------------------------------------------------------------------------- oracle legs
+def _oracle_sample(idx: int, n_seq: int, length: int):
+    """Oracle inputs for the first n_seq sequences of config idx truncated to `length` tokens:
+    logical cache arrays of the context minus one token, the step's new K/V row and query."""
+    import dataclasses
+
+    import oracle
+    from paper_2606_20474_b200 import workloads as W     # input generator only (no arithmetic)
+    wl = _workload(idx, 0)
+    wl1 = wl if wl.new_tokens == 1 else dataclasses.replace(wl, new_tokens=1)
+    q = W.gen_q(wl, "cpu", step=0).view(torch.uint16).numpy()
+    k_new, v_new = W.gen_new_kv(wl1, 0, "cpu")
+    k_new, v_new = k_new.view(torch.uint16).numpy(), v_new.view(torch.uint16).numpy()
+    seqs = []
+    for b in range(n_seq):
+        L = min(int(wl.ctx_lens[b]), length)
+        k, v = W.seq_kv(wl, b, L - 1, "cpu")
+        arrays = oracle.encode_kv(k.view(torch.uint16).numpy(), v.view(torch.uint16).numpy())
+        seqs.append((L, arrays))
+    return wl, q, k_new, v_new, seqs
+
+
+def _oracle_step(oracle, wl, q, k_new, v_new, seqs):
+    """One hot-path step on the CPU oracle for the sample: append 1 token, encode Q, attend."""
+    nbytes = 0
+    per_tok = 2 * (wl.head_dim // 2 + wl.head_dim // 32)
+    for b, (L, arrays) in enumerate(seqs):
+        new = oracle.encode_kv(k_new[b:b + 1], v_new[b:b + 1])
+        full = [np.concatenate([a, n], axis=0) for a, n in zip(arrays, new)]
+        q8 = oracle.encode_q(q[b])
+        oracle.attention(q8, *full, wl.num_q_heads, wl.num_kv_heads)
+        nbytes += L * wl.num_kv_heads * per_tok + 4 * ((L + 15) // 16) + wl.num_q_heads * wl.head_dim * 3
+    return nbytes
+
+
+def cpu_baseline(idx: int, budget_s: float = 15.0):
+    import oracle
+    oracle.build()
+    cores = oracle.num_threads()
+    # size the sample: one short probe, then whole sequences up to the budget
+    wl, q, k_new, v_new, seqs = _oracle_sample(idx, 1, 2048)
+    t0 = time.perf_counter(); _oracle_step(oracle, wl, q, k_new, v_new, seqs); probe = time.perf_counter() - t0
+    tok_per_s = 2048 / max(probe, 1e-6)
+    full_len = int(wl.ctx_lens[0])
+    want_tokens = max(2048, int(tok_per_s * budget_s))
+    n_seq = max(1, min(wl.batch, want_tokens // full_len))
+    length = full_len if want_tokens >= full_len else (want_tokens // 16) * 16
+    wl, q, k_new, v_new, seqs = _oracle_sample(idx, n_seq, length)
+    t0 = time.perf_counter()
+    nbytes = _oracle_step(oracle, wl, q, k_new, v_new, seqs)
+    dt = time.perf_counter() - t0
+    return {"value": round(nbytes / dt / 1e9, 5), "unit": UNIT, "cores": cores, "kind": "oracle",
+            "seconds": round(dt, 3),
+            "sample": f"{n_seq} of {wl.batch} sequences of config {idx}, {seqs[0][0]} tokens each "
+                      f"(append 1 token + Q encode + float64 attention, all {wl.num_q_heads} heads)"}
+
+
+def run_reference(args):
+    """The reference arm for this tier is the oracle as it stands, on the host cores."""
+    import oracle
+    oracle.build()
+    cores = oracle.num_threads()
+    W_, K_ = max(args.warmup, 0), args.steps
+    wl, q, k_new, v_new, seqs = _oracle_sample(args.config, 1, 1024)
+    t0 = time.perf_counter(); _oracle_step(oracle, wl, q, k_new, v_new, seqs); probe = time.perf_counter() - t0
+    tok_per_s = 1024 / max(probe, 1e-6)
+    per_step_s = max(0.05, min(10.0, args.ref_budget / max(1, W_ + K_)))
+    full_len = int(wl.ctx_lens[0])
+    length = int(min(full_len, max(256, (int(tok_per_s * per_step_s) // 16) * 16)))
+    wl, q, k_new, v_new, seqs = _oracle_sample(args.config, 1, length)
+    for _ in range(W_):
+        _oracle_step(oracle, wl, q, k_new, v_new, seqs)
+    t0 = time.perf_counter()
+    nbytes = 0
+    for _ in range(K_):
+        nbytes += _oracle_step(oracle, wl, q, k_new, v_new, seqs)
+    dt = time.perf_counter() - t0
+    value = nbytes / dt / 1e9
+    sample = (f"per step: 1 of {wl.batch} sequences of config {args.config} truncated to {seqs[0][0]} tokens "
+              f"(append 1 token + Q encode + float64 attention, all {wl.num_q_heads} heads)")
+    return {"metric": METRIC, "value": round(value, 5), "unit": UNIT, "n_gpus": args.gpus, "steps": K_,
+            "warmup": W_, "ms_per_step": round(dt / K_ * 1e3, 3), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "reference",
+            "config": {"workload": f"BASELINE.json configs[{args.config - 1}] {wl.name} (bounded sample: {sample})"},
+            "cpu_baseline": {"value": round(value, 5), "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": round(value, 5), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+
+
+# ----------------------------------------------------------------------------- main
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 5],
+                    help="BASELINE.json config number (1-based); 2 is the one the metric is quoted on")
+    ap.add_argument("--splits", type=int, default=0, help="num_splits override (0 = uq_suggest_num_splits)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
+    ap.add_argument("--ref-budget", type=float, default=90.0, help="seconds for the whole --impl reference run")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        if rank == 0:
+            print(json.dumps(run_reference(args)), flush=True)
+        return 0
+
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        torch.cuda.set_device(local_rank)
+        torch.distributed.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    try:
+        line = run_ours(args, rank, world, local_rank)
+        if rank == 0:
+            print(json.dumps(line), flush=True)
+    finally:
+        if world > 1:
+            torch.distributed.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
