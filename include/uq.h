@@ -29,21 +29,19 @@
  *
  * PHYSICAL CACHE LAYOUT (uint8).  cache[num_pages][num_kv_heads][UQ_RECORD_BYTES]; the record
  * of (page p, kv head h) starts at byte (p*num_kv_heads + h)*2176 and holds 16 tokens with
- * exactly 4.25 bit/element and no padding.  The LOGICAL content (what Alg. 1 defines: packed
- * codes with element 2j in bits 0-3 and 2j+1 in bits 4-7 of byte j, scale bytes in group
- * order) is permuted inside a record so that every lane of a warp fetches its tensor-core
- * fragment with 16-byte loads.  With t = token slot in the page (0..15), d = channel (0..127):
+ * exactly 4.25 bit/element and no padding.  The cache base must be 32-byte aligned (the K
+ * codes are fetched by TMA as packed 4-bit tensors).  With t = token slot in the page
+ * (0..15), d = channel (0..127), g = d / 32 (group):
  *
- *   [   0,1024)  K codes.  Token t at 64*t.  Logical 32-bit word j (channels 8j..8j+7,
- *                j = 4*ks + c with ks = group 0..3, c = 0..3) is stored at word 4*c + ks.
- *   [1024,2048)  V codes, token-pair interleaved.  For mt = d>>4, g = d&7, hi = (d>>3)&1,
- *                pair p = (t>>3)&1, c = (t&7)>>1:  byte
- *                   1024 + 512*(mt>>2) + 16*(4*g + c) + 4*(mt&3) + 2*p + hi
- *                holds the code of token (t & ~1) in bits 0-3 and of token (t | 1) in bits 4-7.
- *   [2048,2112)  K scale bytes.  Token t's four group bytes (group 0 first) form the 32-bit
- *                word at index 2*(t&7) + (t>>3).
- *   [2112,2176)  V scale bytes.  For token t (p, c as above, odd = t&1) and group gr:  byte
- *                   2112 + 16*c + 4*(2*p + (gr>>1)) + 2*odd + (gr&1).
+ *   [   0,1024)  K codes, LOGICAL order: token t at 64*t, byte j holds channel 2j in bits 0-3
+ *                and channel 2j+1 in bits 4-7 (what Alg. 1 l.5 writes; the tensor cores read
+ *                it directly as E2M1).
+ *   [1024,2048)  V codes, token-major nibbles.  The 32-bit word at
+ *                   1024 + 512*(t>>3) + 16*(d&31) + 4*(d>>5)
+ *                holds channel d of the eight tokens 8*(t>>3) .. 8*(t>>3)+7; token t sits in
+ *                bits 4*(t&7) .. 4*(t&7)+3.
+ *   [2048,2112)  K scale bytes: token t's four group bytes (group 0 first) at 2048 + 4*t.
+ *   [2112,2176)  V scale bytes: token t, group g at 2112 + 32*(t>>3) + 8*g + (t&7).
  *
  * tests/uq_layout.py holds an independent unpacker written from this description.
  */
@@ -116,21 +114,23 @@ int32_t uq_rotate_quantize_append(const uq_config* cfg, const void* k_new, const
  *  q_fp8        uint8 [batch, num_q_heads, head_dim] (E4M3 bytes of the rotated query).
  *  seq_lens     int32 [batch]: lengths INCLUDING any token appended in this step.
  *  num_splits   >= 1.  Split s of sequence b covers pages [s*pps, min((s+1)*pps, n_pages_b))
- *               with n_pages_b = ceil(seq_lens[b]/page_size), pps = ceil(n_pages_b/num_splits);
+ *               with n_pages_b = ceil(seq_lens[b]/page_size) and
+ *               pps = 8*ceil(ceil(n_pages_b/num_splits)/8) (whole 128-token tiles);
  *               a split may be empty.
  *  partial_acc  float32 [batch, num_q_heads, num_splits, head_dim]
  *  partial_ml   float32 [batch, num_q_heads, num_splits, 2] = (m_s, l_s)
  *
  * Partial format: with z_t = sm_scale * q8 . khat_t (natural-log units),
- *     m_s   = a reference logit of split s (>= every z_t of the split minus 8*ln2; it need
+ *     m_s   = a reference logit of split s (>= every z_t of the split minus 12*ln2; it need
  *             not be the exact maximum),  l_s = sum_t exp(z_t - m_s),
  *     acc_s = sum_t exp(z_t - m_s) * vhat_t   (unnormalised).
  * An empty split writes m_s = -inf, l_s = 0, acc_s = 0.
  *
- * Arithmetic: q8 x code products are exact and accumulate in fp32 on tensor cores; exp in
- * fp32 (ex2.approx); P and Vhat enter the PV product as fp16 (Vhat relative to a running
- * reference exponent; values more than 2^23 below the largest V scale seen by a warp flush to
- * zero); accumulation in fp32.  Error bound vs the float64 oracle: DESIGN.md "Tolerance".
+ * Arithmetic: S = K Q^T by tcgen05.mma kind::mxf8f6f4.block_scale (E2M1 x E4M3 products exact,
+ * UE8M0 group scales applied by the tensor core, fp32 accumulation in TMEM); exp in fp32
+ * (ex2.approx); P and Vhat enter the PV product (tcgen05.mma kind::f16) as fp16, Vhat relative to
+ * a running reference exponent (values more than 2^25 below the largest V scale seen so far
+ * flush to zero); accumulation in fp32 in TMEM.  Error bound vs the float64 oracle: DESIGN.md "Tolerance".
  */
 int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, const void* cache,
                             int64_t num_pages, const int32_t* block_tables, int32_t max_pages,

@@ -1,7 +1,7 @@
 // uq_append.cu — quantize-on-append: Alg. 1 "Write" l.1-5 and "Decode" l.6 of
 // arxiv/paper_2606_20474.
 //
-// One warp per (new token pair, kv head) or per (sequence, q head).  A lane owns 4 consecutive
+// Record layout: include/uq.h.  One warp per (new token pair, kv head) or per (sequence, q head).  A lane owns 4 consecutive
 // channels of the 128-channel vector.  The Walsh-Hadamard rotation is an in-register butterfly:
 // index bits 0-1 inside the lane, bits 2-6 through warp shuffles.  All of it runs in float64:
 // sums of 128 bf16 values are exact in double, so every rounding decision (scale exponent,
@@ -111,15 +111,13 @@ __device__ __forceinline__ void store_k(const uint16_t* krow, uint8_t* rec, int 
   uint32_t h16 = e2m1_code(x[0], E) | (e2m1_code(x[1], E) << 4) | (e2m1_code(x[2], E) << 8) |
                  (e2m1_code(x[3], E) << 12);
   const uint32_t other = __shfl_down_sync(kFull, h16, 1);
-  if ((lane & 1) == 0) {
-    const int j = lane >> 1;                  // logical word: channels 8j..8j+7
-    const int ks = j >> 2, c = j & 3;
-    *reinterpret_cast<uint32_t*>(rec + kOffKCodes + 64 * t + 4 * (4 * c + ks)) = h16 | (other << 16);
+  if ((lane & 1) == 0) {                      // logical order: word j = channels 8j..8j+7
+    *reinterpret_cast<uint32_t*>(rec + kOffKCodes + 64 * t + 4 * (lane >> 1)) = h16 | (other << 16);
   }
   const uint32_t b = (uint32_t)(E + 127);
   const uint32_t w = __shfl_sync(kFull, b, 0) | (__shfl_sync(kFull, b, 8) << 8) |
                      (__shfl_sync(kFull, b, 16) << 16) | (__shfl_sync(kFull, b, 24) << 24);
-  if (lane == 0) *reinterpret_cast<uint32_t*>(rec + kOffKScales + 4 * (2 * (t & 7) + (t >> 3))) = w;
+  if (lane == 0) *reinterpret_cast<uint32_t*>(rec + kOffKScales + 4 * t) = w;
 }
 
 // Encode V of one token: returns the lane's four 4-bit codes (one per byte of the result) and
@@ -128,10 +126,7 @@ __device__ __forceinline__ uint32_t encode_v(const uint16_t* vrow, uint8_t* rec,
   double x[4];
   load4(vrow, lane, x);
   const int E = group_exponent(x, c_v);
-  if ((lane & 7) == 0) {
-    const int gr = lane >> 3, p = (t >> 3) & 1, c = (t & 7) >> 1, odd = t & 1;
-    rec[kOffVScales + 16 * c + 4 * (2 * p + (gr >> 1)) + 2 * odd + (gr & 1)] = (uint8_t)(E + 127);
-  }
+  if ((lane & 7) == 0) rec[kOffVScales + 32 * (t >> 3) + 8 * (lane >> 3) + (t & 7)] = (uint8_t)(E + 127);
   return e2m1_code(x[0], E) | (e2m1_code(x[1], E) << 8) | (e2m1_code(x[2], E) << 16) |
          (e2m1_code(x[3], E) << 24);
 }
@@ -170,11 +165,12 @@ append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v
       store_k(krow + (long long)Hkv * kHeadDim, rec, t + 1, lane, c_k);
       cb = encode_v(vrow + (long long)Hkv * kHeadDim, rec, t + 1, lane, c_v);
     }
-    const int mt = lane >> 2, hib = (lane >> 1) & 1, p = (t >> 3) & 1, c = (t & 7) >> 1;
+    // token-major nibbles: channel d = 4*lane + r lives in word 512*(t>>3) + 16*(d&31) + 4*(d>>5),
+    // tokens (t, t+1) share byte (t&7)>>1 of that word
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
-      const int g = 4 * (lane & 1) + r;
-      uint8_t* dst = rec + kOffVCodes + 512 * (mt >> 2) + 16 * (4 * g + c) + 4 * (mt & 3) + 2 * p + hib;
+      const int d = 4 * lane + r;
+      uint8_t* dst = rec + kOffVCodes + 512 * (t >> 3) + 16 * (d & 31) + 4 * (d >> 5) + ((t & 7) >> 1);
       const uint32_t a4 = (ca >> (8 * r)) & 0xF, b4 = (cb >> (8 * r)) & 0xF;
       *dst = odd ? (uint8_t)((*dst & 0x0F) | (a4 << 4)) : (uint8_t)(a4 | (b4 << 4));
     }

@@ -2,32 +2,61 @@
 // l.7-8 of arxiv/paper_2606_20474 (Eq.(1) :104).  Paging / split-K / partial
 // format follow include/uq.h.
 //
-// Design: one CTA per (sequence, kv head, split); each of its warps is an
-// independent stream processor over 16-token page records:
-//   * lane 0 brings whole 2176-byte records into a per-warp shared-memory ring with
-//     cp.async.bulk + mbarrier (no CTA-wide barrier in the loop);
-//   * S^T[16 tok x 8 heads] = Kcodes . Q^T on tensor cores (mma.sync m16n8k32 e4m3): the FP4
-//     codes become E4M3 bytes by pure bit placement (E2M1 value * 2^-6 is an E4M3 bit pattern,
-//     subnormals included), the FP8 query fragments are loaded once per CTA ("hoisted",
-//     PAPER.md:285), products are exact, and the UE8M0 group scale (one MMA k-step = one
-//     32-channel group) is applied to the fp32 accumulator: S += 2^(byte-127) * acc;
-//   * online softmax in fp32 with a LAZY reference maximum (rescale only when a score exceeds
-//     the reference by more than 8 in log2 units);
-//   * O^T[128 d x 8 heads] += Vhat^T . P^T (mma.sync m16n8k16 f16): token-pair-interleaved V
-//     codes convert with cvt.rn.f16x2.e2m1x2 straight into A fragments, V scales are applied as
-//     exact power-of-two fp16 multipliers relative to a running reference exponent.
-// Every K/V byte is read from HBM once and touched by exactly one warp.
+// Design: one CTA per (sequence, kv head, split); the split is walked in
+// tiles of 128 tokens (8 pages).  Warp roles (320 threads):
+//   warp 8  producer: per page one TMA tensor copy of the packed FP4 K codes
+//           (CU_TENSOR_MAP_DATA_TYPE_16U4_ALIGN16B + SWIZZLE_128B: the TMA unit expands the
+//           nibbles into the 8-bit containers tcgen05 reads) and one cp.async.bulk of the rest of
+//           the record (V codes, K scales, V scales), through a ring of mbarrier stages;
+//   warp 9  MMA issuer: S[128 tok x 16 heads] = K . Q^T with
+//           tcgen05.mma.kind::mxf8f6f4.block_scale — E2M1 keys x E4M3 queries with the UE8M0 group
+//           scales applied by the tensor core (the paper's FP8xFP4 scaled MMA), K
+//           scales staged smem -> TMEM with tcgen05.cp; then O^T[128 d x 16 heads] += Vhat^T . P^T
+//           with tcgen05.mma.kind::f16; accumulators live in TMEM;
+//   warps 0-7 compute: V codes -> fp16 (cvt.rn.f16x2.e2m1x2 x exact power-of-two scale) into the
+//           K-major operand layout; S rows from TMEM (tcgen05.ld), base-2 softmax against a LAZY
+//           per-head reference (a "rebase" — new reference, O rescaled in TMEM, tile redone —
+//           happens on the first tile and whenever a score exceeds the reference by 2^12 or a V
+//           scale exceeds the reference exponent), P -> fp16 operand in smem.
+// The FP8 query tile is written to smem once per CTA ("hoisted").
+// Every K/V byte is read from HBM exactly once.
+#include <cuda.h>
 #include <cuda_fp16.h>
+
+#include <mutex>
 
 #include "uq_common.cuh"
 
 namespace uq {
 namespace {
 
-constexpr int kWarps = 4;
-constexpr int kStages = 4;
-constexpr int kHeadStride = 132;  // padded fp32 row (128 + 4) of the CTA combine staging
+constexpr int kComputeWarps = 8;
+constexpr int kThreads = (kComputeWarps + 2) * 32;   // + producer warp + MMA warp
+constexpr int kStages = 2;
+constexpr int kTilePages = 8;                        // 128 tokens per tile
+constexpr int kRestBytes = kRecordBytes - 1024;      // V codes + K scales + V scales = 1152
+constexpr int kStageBytes = kTilePages * (2048 + kRestBytes);   // K unpacked 16 KB + 9216 = 25600
+constexpr int kPStride = 272;                        // bytes between token-cores of the P operand
+constexpr float kThresh = 12.0f;                     // lazy-reference threshold (log2 units)
 constexpr unsigned kFull = 0xffffffffu;
+
+// dynamic shared memory map (offsets from a 1024-byte aligned base)
+constexpr int kOffStage = 0;
+constexpr int kOffQ = kOffStage + kStages * kStageBytes;       // 2048, SW128
+constexpr int kOffSFA = kOffQ + 2048;                          // 2 x 512
+constexpr int kOffSFB = kOffSFA + 1024;                        // 512
+constexpr int kOffV = kOffSFB + 512;                           // 32768: [token-core 16][d 128][16 B]
+constexpr int kOffP = kOffV + 32768;                           // 16 x 272
+constexpr int kOffMul = kOffP + 16 * kPStride + 256;           // 8 warps x 128 B
+constexpr int kOffEnd = kOffMul + kComputeWarps * 128;
+constexpr int kSmemBytes = kOffEnd + 1024;                     // + alignment slack
+
+// TMEM columns
+constexpr uint32_t kColS = 0;      // 2 x 16
+constexpr uint32_t kColO = 32;     // 16
+constexpr uint32_t kColSFA = 48;   // 2 x 4
+constexpr uint32_t kColSFB = 56;   // 4
+constexpr uint32_t kTmemCols = 64;
 
 // ---------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -38,6 +67,9 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
 }
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile(
@@ -54,40 +86,73 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, int c2, uint32_t bar) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+               ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void bar_compute() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
+
+// shared-memory matrix descriptor (SM100 UMMA): start>>4 | LBO>>4 <<16 | SBO>>4 <<32 | version 1 | layout
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes, uint32_t layout) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr >> 4) & 0x3FFF);
+  d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16;
+  d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32;
+  d |= (uint64_t)1 << 46;
+  d |= (uint64_t)(layout & 7) << 61;      // 0 = no swizzle, 2 = 128-byte swizzle
+  return d;
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void umma_cp_sf(uint32_t taddr, uint64_t sdesc) {
+  asm volatile("tcgen05.cp.cta_group::1.32x128b.warpx4 [%0], %1;" ::"r"(taddr), "l"(sdesc) : "memory");
+}
+// D[tmem] (+)= A[smem, E2M1] . B[smem, E4M3]^T with UE8M0 block scales in TMEM
+__device__ __forceinline__ void umma_mxf8f6f4(uint32_t d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t acc,
+                                              uint32_t tsfa, uint32_t tsfb) {
+  asm volatile(
+      "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::1.kind::mxf8f6f4.block_scale [%0], %1, %2, %3, [%5], [%6], p;\n}\n"
+      ::"r"(d), "l"(da), "l"(db), "r"(idesc), "r"(acc), "r"(tsfa), "r"(tsfb) : "memory");
+}
+__device__ __forceinline__ void umma_f16(uint32_t d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}\n"
+      ::"r"(d), "l"(da), "l"(db), "r"(idesc), "r"(acc) : "memory");
+}
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, float (&v)[8]) {
+  uint32_t r[8];
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+               : "r"(taddr));
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+  for (int j = 0; j < 8; ++j) v[j] = __uint_as_float(r[j]);
+}
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const float (&v)[8]) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+               ::"r"(taddr), "r"(__float_as_uint(v[0])), "r"(__float_as_uint(v[1])), "r"(__float_as_uint(v[2])),
+                 "r"(__float_as_uint(v[3])), "r"(__float_as_uint(v[4])), "r"(__float_as_uint(v[5])),
+                 "r"(__float_as_uint(v[6])), "r"(__float_as_uint(v[7])) : "memory");
+  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
 __device__ __forceinline__ uint4 lds128(uint32_t a) {
   uint4 v;
   asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
   return v;
 }
-__device__ __forceinline__ uint2 lds64(uint32_t a) {
-  uint2 v;
-  asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a));
-  return v;
+__device__ __forceinline__ void sts128(uint32_t a, uint4 v) {
+  asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 __device__ __forceinline__ float ex2(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
-}
-__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
-  uint32_t d;
-  asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(sel));
-  return d;
-}
-__device__ __forceinline__ uint32_t max_u16x2(uint32_t a, uint32_t b) {
-  uint32_t d;
-  asm("max.u16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b));
-  return d;
-}
-__device__ __forceinline__ uint32_t pack_f16x2(float lo, float hi) {
-  uint32_t d;
-  asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
-  return d;
-}
-__device__ __forceinline__ uint32_t movm_trans(uint32_t a) {
-  uint32_t d;
-  asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(d) : "r"(a));
-  return d;
 }
 __device__ __forceinline__ uint32_t hmul2(uint32_t a, uint32_t b) {
   uint32_t d;
@@ -105,355 +170,448 @@ __device__ __forceinline__ void cvt_e2m1x8(uint32_t w, uint32_t (&h)[4]) {
       "cvt.rn.f16x2.e2m1x2 %3, b3;\n"
       "}\n" : "=r"(h[0]), "=r"(h[1]), "=r"(h[2]), "=r"(h[3]) : "r"(w));
 }
-__device__ __forceinline__ void mma_e4m3(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
-                                         uint32_t b0, uint32_t b1) {
-  asm volatile("mma.sync.aligned.m16n8k32.row.col.f32.e4m3.e4m3.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, "
-               "{%10,%11,%12,%13};"
-               : "=f"(d[0]), "=f"(d[1]), "=f"(d[2]), "=f"(d[3])
-               : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1), "f"(0.f), "f"(0.f), "f"(0.f), "f"(0.f));
-}
-__device__ __forceinline__ void mma_f16(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
-                                        uint32_t b0, uint32_t b1) {
-  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, "
-               "{%0,%1,%2,%3};"
-               : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
-               : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+__device__ __forceinline__ float pow2i(int e) {   // 2^e, flushing to 0 below the fp32 normal range
+  const int f = e + 127;
+  return f > 0 ? __uint_as_float((uint32_t)min(f, 254) << 23) : 0.f;
 }
 
-// E2M1 nibbles -> E4M3 bytes holding value * 2^-6:  byte = sign<<7 | (e1 e0 m)<<2.
-// lo: the four low nibbles of w (even channels), hi: the four high nibbles (odd channels).
-__device__ __forceinline__ uint32_t e2m1_lo_to_e4m3(uint32_t w) {
-  return ((w << 2) & 0x1C1C1C1Cu) | ((w << 4) & 0x80808080u);
+// ---------------------------------------------------------------- per-CTA shared bookkeeping
+struct Shared {
+  uint64_t full[kStages];     // producer -> consumers: stage landed (tx bytes)
+  uint64_t empty[kStages];    // 8 compute warps + QK commit -> producer
+  uint64_t s_full[2];         // QK commit -> compute warps
+  uint64_t pv_ready;          // 8 compute warps -> MMA warp (Vhat and P of the tile are in smem)
+  uint64_t pv_done;           // PV commit -> compute warps (Vhat / P buffers free, O up to date)
+  uint32_t tmem_base;
+  volatile int flag;          // a warp asked for a rebase of the references
+  float wmax[kComputeWarps][8];
+  int wvmax[kComputeWarps];
+  float lsum[kComputeWarps][8];
+  float mref[16];
+};
+
+// V scale bytes of this warp's page -> fp16 power-of-two multipliers in the warp's scratch;
+// returns the largest scale byte among the page's valid tokens (warp-uniform).
+__device__ __forceinline__ int v_multipliers(uint32_t rest, uint32_t scratch, int lane, int n_valid, int eref) {
+  uint32_t pair;
+  asm volatile("ld.shared.u16 %0, [%1];" : "=r"(pair) : "r"(rest + 1088 + 2 * lane));
+  int lo = (int)(pair & 0xFFu), hi = (int)(pair >> 8);
+  const int tok = 8 * (lane >> 4) + 2 * (lane & 3);
+  if (tok >= n_valid) lo = 0;
+  if (tok + 1 >= n_valid) hi = 0;
+  const int vmax = __reduce_max_sync(kFull, max(lo, hi));
+  const int kbase = eref - 28;                       // fp16 exponent field = byte - kbase (2^13 at byte = eref)
+  const uint32_t mlo = (uint32_t)max(lo - kbase, 0), mhi = (uint32_t)max(hi - kbase, 0);
+  const uint32_t mult = (lo ? (mlo << 10) : 0u) | (hi ? (mhi << 26) : 0u);
+  __syncwarp();
+  asm volatile("st.shared.u32 [%0], %1;" ::"r"(scratch + 4 * lane), "r"(mult) : "memory");
+  __syncwarp();
+  return vmax;
 }
-__device__ __forceinline__ uint32_t e2m1_hi_to_e4m3(uint32_t w) {
-  return ((w >> 2) & 0x1C1C1C1Cu) | (w & 0x80808080u);
-}
-// fp32 2^(byte-127) for byte `i` of word w (byte 0 -> +0.0, which is what an all-zero group needs)
-template <int I>
-__device__ __forceinline__ float ue8m0_to_f32(uint32_t w) {
-  const uint32_t bits = (I < 3 ? (w << (23 - 8 * I)) : (w >> 1)) & 0x7F800000u;
-  return __uint_as_float(bits);
+
+// V codes of this warp's page (16 tokens x 128 channels) -> fp16 Vhat^T operand:
+// [token-core tc][d][8 tokens], tc = 2*page_in_tile + half.
+__device__ __forceinline__ void v_convert(uint32_t rest, uint32_t scratch, uint32_t sV, int page_in_tile, int lane,
+                                          int n_valid) {
+  if (n_valid <= 0) {
+    const uint4 z = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+    for (int h = 0; h < 2; ++h)
+#pragma unroll
+      for (int i = 0; i < 4; ++i) sts128(sV + (2 * page_in_tile + h) * 2048 + (32 * i + lane) * 16, z);
+    return;
+  }
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    const uint4 c4 = lds128(rest + 512 * h + 16 * lane);
+    const uint32_t cw[4] = {c4.x, c4.y, c4.z, c4.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {                     // channel d = 32 i + lane, group i
+      const uint4 m4 = lds128(scratch + 64 * h + 16 * i);
+      uint32_t f[4];
+      cvt_e2m1x8(cw[i], f);
+      uint4 o;
+      o.x = hmul2(f[0], m4.x);
+      o.y = hmul2(f[1], m4.y);
+      o.z = hmul2(f[2], m4.z);
+      o.w = hmul2(f[3], m4.w);
+      sts128(sV + (2 * page_in_tile + h) * 2048 + (32 * i + lane) * 16, o);
+    }
+  }
 }
 
 // ---------------------------------------------------------------- the kernel
-// NT = number of 8-head tiles (1 for GQA group <= 8, 2 for <= 16).
-template <int NT>
-__global__ void __launch_bounds__(kWarps * 32, 3)
-decode_kernel(const uint8_t* __restrict__ q_fp8, const uint8_t* __restrict__ cache,
-              const int32_t* __restrict__ block_tables, int max_pages,
+__global__ void __launch_bounds__(kThreads, 2)
+decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restrict__ q_fp8,
+              const uint8_t* __restrict__ cache, const int32_t* __restrict__ block_tables, int max_pages,
               const int32_t* __restrict__ seq_lens, int Hq, int Hkv, int num_splits,
-              float score_scale /* sm_scale * log2(e) * 2^6 */,
-              float* __restrict__ partial_acc, float* __restrict__ partial_ml) {
-  extern __shared__ __align__(128) uint8_t smem[];
-  __shared__ __align__(8) uint64_t s_bar[kWarps][kStages];
-  __shared__ float s_m[kWarps][16];
-  __shared__ float s_l[kWarps][16];
-  __shared__ int s_e[kWarps];
+              float score_scale /* sm_scale * log2(e) */, float* __restrict__ partial_acc,
+              float* __restrict__ partial_ml) {
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ __align__(8) Shared sh;
 
   const int split = blockIdx.x, kvh = blockIdx.y, b = blockIdx.z;
   const int G = Hq / Hkv;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int g = lane >> 2, c = lane & 3;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 
   const int L = seq_lens[b];
   const int n_pages = (L + kPage - 1) / kPage;
-  const int pps = (n_pages + num_splits - 1) / num_splits;
+  int pps = (n_pages + num_splits - 1) / num_splits;
+  pps = (pps + kTilePages - 1) / kTilePages * kTilePages;
   const int p0 = split * pps;
   const int p1 = min(p0 + pps, n_pages);
   const long long row0 = ((long long)b * Hq + (long long)kvh * G) * num_splits + split;  // + head*num_splits
   if (p0 >= p1) {  // empty split: (m, l) = (-inf, 0); acc is never read by the merge
-    if (threadIdx.x < G) {
-      float2* ml = reinterpret_cast<float2*>(partial_ml) + row0 + (long long)threadIdx.x * num_splits;
+    if (tid < G) {
+      float2* ml = reinterpret_cast<float2*>(partial_ml) + row0 + (long long)tid * num_splits;
       *ml = make_float2(-INFINITY, 0.f);
     }
     return;
   }
+  const int n_tiles = (p1 - p0 + kTilePages - 1) / kTilePages;
+  const int tok_end = min(L, p1 * kPage);
 
-  // ---- hoisted FP8 query fragments (B operand of S^T = K Q^T)
-  uint32_t qb[NT][4][2];
+  const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t sQ = base + kOffQ, sSFA = base + kOffSFA, sSFB = base + kOffSFB, sV = base + kOffV,
+                 sP = base + kOffP;
+  const uint32_t bar_full = smem_u32(&sh.full[0]), bar_empty = smem_u32(&sh.empty[0]),
+                 bar_sfull = smem_u32(&sh.s_full[0]), bar_pvready = smem_u32(&sh.pv_ready),
+                 bar_pvdone = smem_u32(&sh.pv_done);
+
+  // ---------------- setup
+  if (tid == 0) {
 #pragma unroll
-  for (int nt = 0; nt < NT; ++nt) {
-    const int head = 8 * nt + g;
-    const uint8_t* qrow = q_fp8 + ((long long)b * Hq + (long long)kvh * G + head) * kHeadDim;
-#pragma unroll
-    for (int ks = 0; ks < 4; ++ks) {
-      uint2 w = make_uint2(0u, 0u);
-      if (head < G) w = *reinterpret_cast<const uint2*>(qrow + 32 * ks + 8 * c);
-      qb[nt][ks][0] = prmt(w.x, w.y, 0x6420);  // even channels 8c+{0,2,4,6}  <-> k = 4c+i
-      qb[nt][ks][1] = prmt(w.x, w.y, 0x7531);  // odd channels               <-> k = 16+4c+i
+    for (int s = 0; s < kStages; ++s) {
+      mbar_init(bar_full + 8 * s, 1);
+      mbar_init(bar_empty + 8 * s, kComputeWarps + 1);
     }
-  }
-
-  // ---- per-warp page pipeline
-  uint8_t* ring = smem + (size_t)warp * kStages * kRecordBytes;
-  const uint32_t ring_u32 = smem_u32(ring);
-  const uint32_t bar_u32 = smem_u32(&s_bar[warp][0]);
-  if (lane == 0) {
-#pragma unroll
-    for (int s = 0; s < kStages; ++s) mbar_init(bar_u32 + 8 * s, 1);
+    mbar_init(bar_sfull, 1);
+    mbar_init(bar_sfull + 8, 1);
+    mbar_init(bar_pvready, kComputeWarps);
+    mbar_init(bar_pvdone, 1);
+    sh.flag = 0;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  __syncwarp();
-  const int n_my = (p1 - p0 - warp + kWarps - 1) / kWarps;  // pages p0+warp, p0+warp+kWarps, ...
-  const int32_t* bt = block_tables + (long long)b * max_pages;
-  const uint8_t* cache_h = cache + (long long)kvh * kRecordBytes;
-  const long long page_stride = (long long)Hkv * kRecordBytes;
-
-  // block-table window: lane j holds the physical page of this warp's page index (32*win + j)
-  int bt_win = 0;
-  int bt_reg = (lane < n_my) ? bt[p0 + warp + kWarps * lane] : 0;
-  auto issue = [&](int i) {  // all lanes call; lane 0 issues the copy of warp-page i
-    if ((i >> 5) != bt_win) {
-      bt_win = i >> 5;
-      const int j = 32 * bt_win + lane;
-      bt_reg = (j < n_my) ? bt[p0 + warp + kWarps * j] : 0;
-    }
-    const int page = __shfl_sync(kFull, bt_reg, i & 31);
-    if (lane == 0) {
-      const int st = i % kStages;
-      mbar_expect_tx(bar_u32 + 8 * st, kRecordBytes);
-      bulk_g2s(ring_u32 + st * kRecordBytes, cache_h + (long long)page * page_stride, kRecordBytes,
-               bar_u32 + 8 * st);
-    }
-  };
-  for (int i = 0; i < kStages && i < n_my; ++i) issue(i);
-
-  // ---- running state
-  float O[8][NT][4];
-#pragma unroll
-  for (int mt = 0; mt < 8; ++mt)
-#pragma unroll
-    for (int nt = 0; nt < NT; ++nt)
-#pragma unroll
-      for (int j = 0; j < 4; ++j) O[mt][nt][j] = 0.f;
-  float mref[NT][2], lsum[NT][2];
-#pragma unroll
-  for (int nt = 0; nt < NT; ++nt) {
-    mref[nt][0] = mref[nt][1] = -INFINITY;
-    lsum[nt][0] = lsum[nt][1] = 0.f;
+  if (warp == kComputeWarps + 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&sh.tmem_base)),
+                 "r"(kTmemCols));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
-  // Reference UE8M0 byte for V.  A group with scale byte B enters the PV product as
-  // code * 2^(B - eref + 13) in fp16 (exact for B >= eref - 27, flushed to zero below), so the
-  // largest value is 6 * 2^13 < 65504; eref >= 28 keeps B - (eref - 28) a valid exponent field.
-  int eref = 28;
+  if (tid < 128) {  // hoisted FP8 query tile: 16 rows x 128 B, 128-byte swizzle; rows >= G are zero
+    const int n = tid >> 3, c = tid & 7;
+    uint4 v = make_uint4(0u, 0u, 0u, 0u);
+    if (n < G) v = *reinterpret_cast<const uint4*>(q_fp8 + ((long long)b * Hq + (long long)kvh * G + n) * kHeadDim + 16 * c);
+    sts128(sQ + n * 128 + ((c ^ (n & 7)) << 4), v);
+  } else if (tid < 256) {  // query-side scale factors: UE8M0 byte 127 = 2^0
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(sSFB + 4 * (tid - 128)), "r"(0x7F7F7F7Fu) : "memory");
+  }
+  fence_async_smem();
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = sh.tmem_base;
 
-  // ================================================================ main loop over pages
-  for (int i = 0; i < n_my; ++i) {
-    const int st = i % kStages;
-    const uint32_t rec = ring_u32 + st * kRecordBytes;
-    mbar_wait(bar_u32 + 8 * st, (i / kStages) & 1);
-
-    const uint4 kA = lds128(rec + kOffKCodes + 64 * g + 16 * c);        // token g,   groups 0..3
-    const uint4 kB = lds128(rec + kOffKCodes + 64 * (g + 8) + 16 * c);  // token g+8
-    uint2 ksc = lds64(rec + kOffKScales + 8 * g);                       // scale words of g, g+8
-    const uint4 v0 = lds128(rec + kOffVCodes + 16 * lane);              // d tiles 0..3
-    const uint4 v1 = lds128(rec + kOffVCodes + 512 + 16 * lane);        // d tiles 4..7
-    uint4 vsc = lds128(rec + kOffVScales + 16 * c);                     // V scales of this lane's 4 tokens
-
-    // tokens past the sequence end (last page only): neutralise their scales, mask their scores
-    const int page_idx = p0 + warp + kWarps * i;
-    const int n_valid = L - page_idx * kPage;  // >= 1
-    const bool partial = n_valid < kPage;
-    if (partial) {
-      if (g >= n_valid) ksc.x = 0u;
-      if (g + 8 >= n_valid) ksc.y = 0u;
-      const uint32_t mA0 = (2 * c < n_valid) ? 0x0000FFFFu : 0u, mB0 = (2 * c + 1 < n_valid) ? 0xFFFF0000u : 0u;
-      const uint32_t mA1 = (2 * c + 8 < n_valid) ? 0x0000FFFFu : 0u, mB1 = (2 * c + 9 < n_valid) ? 0xFFFF0000u : 0u;
-      vsc.x &= (mA0 | mB0);
-      vsc.y &= (mA0 | mB0);
-      vsc.z &= (mA1 | mB1);
-      vsc.w &= (mA1 | mB1);
-    }
-
-    // ---------------- S^T = K Q^T, one MMA k-step per 32-channel group, scale on the accumulator
-    float S[NT][4];
-#pragma unroll
-    for (int nt = 0; nt < NT; ++nt) S[nt][0] = S[nt][1] = S[nt][2] = S[nt][3] = 0.f;
-    const uint32_t kAw[4] = {kA.x, kA.y, kA.z, kA.w};
-    const uint32_t kBw[4] = {kB.x, kB.y, kB.z, kB.w};
-    const float sA[4] = {ue8m0_to_f32<0>(ksc.x), ue8m0_to_f32<1>(ksc.x), ue8m0_to_f32<2>(ksc.x), ue8m0_to_f32<3>(ksc.x)};
-    const float sB[4] = {ue8m0_to_f32<0>(ksc.y), ue8m0_to_f32<1>(ksc.y), ue8m0_to_f32<2>(ksc.y), ue8m0_to_f32<3>(ksc.y)};
-#pragma unroll
-    for (int ks = 0; ks < 4; ++ks) {
-      const uint32_t a0 = e2m1_lo_to_e4m3(kAw[ks]), a1 = e2m1_lo_to_e4m3(kBw[ks]);
-      const uint32_t a2 = e2m1_hi_to_e4m3(kAw[ks]), a3 = e2m1_hi_to_e4m3(kBw[ks]);
-#pragma unroll
-      for (int nt = 0; nt < NT; ++nt) {
-        float acc[4];
-        mma_e4m3(acc, a0, a1, a2, a3, qb[nt][ks][0], qb[nt][ks][1]);
-        S[nt][0] = fmaf(acc[0], sA[ks], S[nt][0]);
-        S[nt][1] = fmaf(acc[1], sA[ks], S[nt][1]);
-        S[nt][2] = fmaf(acc[2], sB[ks], S[nt][2]);
-        S[nt][3] = fmaf(acc[3], sB[ks], S[nt][3]);
+  if (warp == kComputeWarps) {
+    // ================================================================ producer warp
+    const int32_t* bt = block_tables + (long long)b * max_pages;
+    int page_next = (lane < kTilePages && p0 + lane < p1) ? bt[p0 + lane] : 0;
+    for (int i = 0; i < n_tiles; ++i) {
+      const int s = i % kStages;
+      const int page = page_next;
+      const int npg = min(kTilePages, p1 - (p0 + kTilePages * i));
+      const int nb = p0 + kTilePages * (i + 1) + lane;
+      page_next = (lane < kTilePages && nb < p1) ? bt[nb] : 0;
+      mbar_wait(bar_empty + 8 * s, ((i / kStages) & 1) ^ 1);
+      if (lane == 0) mbar_expect_tx(bar_full + 8 * s, (uint32_t)npg * kRecordBytes);
+      __syncwarp();
+      if (lane < npg) {
+        const long long rec = (long long)page * Hkv + kvh;
+        const uint32_t st = base + kOffStage + s * kStageBytes;
+        tma_load_3d(st + 2048 * lane, &tmap, 0, 0, (int)rec, bar_full + 8 * s);
+        bulk_g2s(st + 16384 + kRestBytes * lane, cache + rec * kRecordBytes + 1024, kRestBytes, bar_full + 8 * s);
       }
     }
-    // log2-domain scores; S[nt][0..1]: token g, heads 8nt+2c, +1;  S[nt][2..3]: token g+8
-    bool exceed = false;
+  } else if (warp == kComputeWarps + 1) {
+    // ================================================================ MMA warp
+    if (lane == 0) umma_cp_sf(tmem + kColSFB, make_desc(sSFB, 16, 128, 0));
+    // E2M1 (5) x E4M3 (0), UE8M0 scales, N = 16, M = 128
+    const uint32_t idesc_qk = (5u << 7) | (0u << 10) | (2u << 17) | (1u << 23) | (8u << 24);
+    // f16 x f16 -> f32, N = 16, M = 128
+    const uint32_t idesc_pv = (1u << 4) | (2u << 17) | (8u << 24);
+    auto issue_qk = [&](int i) {
+      const int s = i % kStages, sb = i & 1;
+      const uint32_t st = base + kOffStage + s * kStageBytes;
+      mbar_wait(bar_full + 8 * s, (i / kStages) & 1);
+      // scale-factor atom: row r = 32 c + lane of the tile -> 16-byte line `lane`, word c
+      uint4 w;
+      {
+        uint32_t v[4];
 #pragma unroll
-    for (int nt = 0; nt < NT; ++nt) {
-#pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        float x = S[nt][j] * score_scale;
-        if (partial && ((j < 2 ? g : g + 8) >= n_valid)) x = -INFINITY;
-        S[nt][j] = x;
-        exceed |= x > mref[nt][j & 1] + 8.0f;
+        for (int c = 0; c < 4; ++c) {
+          const int r = 32 * c + lane;
+          asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v[c]) : "r"(st + 16384 + kRestBytes * (r >> 4) + 1024 + 4 * (r & 15)));
+        }
+        w = make_uint4(v[0], v[1], v[2], v[3]);
       }
+      sts128(sSFA + 512 * sb + 16 * lane, w);
+      fence_async_smem();
+      __syncwarp();
+      tc_fence_after();
+      if (lane == 0) {
+        const uint32_t t_sfa = tmem + kColSFA + 4 * sb;
+        umma_cp_sf(t_sfa, make_desc(sSFA + 512 * sb, 16, 128, 0));
+#pragma unroll
+        for (int kb = 0; kb < 4; ++kb)
+          umma_mxf8f6f4(tmem + kColS + 16 * sb, make_desc(st + 32 * kb, 16, 1024, 2), make_desc(sQ + 32 * kb, 16, 1024, 2),
+                        idesc_qk | ((uint32_t)kb << 29), kb > 0, t_sfa + ((uint32_t)kb << 30), tmem + kColSFB);
+        umma_commit(bar_sfull + 8 * sb);
+        umma_commit(bar_empty + 8 * s);
+      }
+      __syncwarp();
+    };
+    issue_qk(0);
+    for (int i = 0; i < n_tiles; ++i) {
+      if (i + 1 < n_tiles) issue_qk(i + 1);
+      mbar_wait(bar_pvready, i & 1);
+      tc_fence_after();
+      if (lane == 0) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+          umma_f16(tmem + kColO, make_desc(sV + 4096 * j, 2048, 128, 0), make_desc(sP + 2 * kPStride * j, kPStride, 128, 0),
+                   idesc_pv, (i > 0 || j > 0) ? 1u : 0u);
+        umma_commit(bar_pvdone);
+      }
+      __syncwarp();
     }
-    if (__any_sync(kFull, exceed)) {  // rare: raise the reference maximum, rescale O and l
+  } else {
+    // ================================================================ compute warps 0..7
+    const int q = warp & 3, hh = warp >> 2;            // TMEM lane quarter, head half
+    const int r = 32 * q + lane;                       // softmax: token row of the tile; epilogue: channel d
+    const bool heads_live = (8 * hh < G);
+    const uint32_t scratch = base + kOffMul + 128 * warp;
+    const uint32_t lane_sel = (uint32_t)(32 * q) << 16;
+    float mref[8], lsum[8];
 #pragma unroll
-      for (int nt = 0; nt < NT; ++nt) {
+    for (int j = 0; j < 8; ++j) { mref[j] = -INFINITY; lsum[j] = 0.f; }
+    int eref = 28;
+
+    for (int i = 0; i < n_tiles; ++i) {
+      const int s = i % kStages, sb = i & 1;
+      const uint32_t st = base + kOffStage + s * kStageBytes;
+      const uint32_t rest = st + 16384 + kRestBytes * warp;          // this warp converts page `warp` of the tile
+      const int pg = p0 + kTilePages * i + warp;
+      const int n_valid = pg < p1 ? min(kPage, L - kPage * pg) : 0;
+      const int tok = (p0 + kTilePages * i) * kPage + r;
+      const bool tok_ok = tok < tok_end;
+      const uint32_t t_s = tmem + lane_sel + kColS + 16 * sb + 8 * hh;
+      const uint32_t p_addr = sP + (r >> 3) * kPStride + (8 * hh) * 16 + (r & 7) * 2;
+
+      mbar_wait(bar_full + 8 * s, (i / kStages) & 1);
+      if (i > 0) mbar_wait(bar_pvdone, (i - 1) & 1);                 // Vhat / P buffers free, O complete
+      float lt[8];
+
+      // softmax of this thread's row against the current references; returns "a score exceeded"
+      auto softmax_pass = [&](bool detect) -> bool {
+        bool ex = false;
 #pragma unroll
-        for (int j = 0; j < 2; ++j) {
-          float mx = fmaxf(S[nt][j], S[nt][j + 2]);
-          mx = fmaxf(mx, __shfl_xor_sync(kFull, mx, 4));
-          mx = fmaxf(mx, __shfl_xor_sync(kFull, mx, 8));
-          mx = fmaxf(mx, __shfl_xor_sync(kFull, mx, 16));
-          const float mnew = fmaxf(mref[nt][j], mx);
-          const float f = (mref[nt][j] == -INFINITY) ? 0.f : ex2(mref[nt][j] - mnew);
-          mref[nt][j] = mnew;
-          lsum[nt][j] *= f;
+        for (int j = 0; j < 8; ++j) lt[j] = 0.f;
+        if (!heads_live) return false;
+        float sv[8];
+        tmem_ld8(t_s, sv);
 #pragma unroll
-          for (int mt = 0; mt < 8; ++mt) {
-            O[mt][nt][j] *= f;
-            O[mt][nt][j + 2] *= f;
+        for (int j = 0; j < 8; ++j) {
+          const float x = tok_ok ? sv[j] * score_scale : -INFINITY;
+          if (detect) ex |= x > mref[j] + kThresh;
+          const float p = ex2(x - mref[j]);
+          lt[j] = p;
+          const __half hp = __float2half_rn(p);
+          asm volatile("st.shared.u16 [%0], %1;" ::"r"(p_addr + 16 * j), "h"(__half_as_ushort(hp)) : "memory");
+        }
+        return ex;
+      };
+
+      bool rebase = (i == 0);
+      if (!rebase) {
+        const int vmax = v_multipliers(rest, scratch, lane, n_valid, eref);
+        v_convert(rest, scratch, sV, warp, lane, n_valid);
+        mbar_wait(bar_sfull + 8 * sb, (i >> 1) & 1);
+        tc_fence_after();
+        const bool ex = softmax_pass(true);
+        if (__any_sync(kFull, ex) || vmax > eref) {
+          if (lane == 0) sh.flag = 1;
+        }
+        tc_fence_before();
+        bar_compute();
+        rebase = sh.flag != 0;
+      } else {
+        mbar_wait(bar_sfull + 8 * sb, (i >> 1) & 1);
+        tc_fence_after();
+      }
+      if (rebase) {
+        // ---- statistics of the tile: per-head maximum score, maximum V scale byte
+        const int vmax = v_multipliers(rest, scratch, lane, n_valid, eref);
+        float tm[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) tm[j] = -INFINITY;
+        if (heads_live) {
+          float sv[8];
+          tmem_ld8(t_s, sv);
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {
+            float x = tok_ok ? sv[j] * score_scale : -INFINITY;
+#pragma unroll
+            for (int o = 16; o; o >>= 1) x = fmaxf(x, __shfl_xor_sync(kFull, x, o));
+            tm[j] = x;
           }
         }
+        if (lane == 0) {
+#pragma unroll
+          for (int j = 0; j < 8; ++j) sh.wmax[warp][j] = tm[j];
+          sh.wvmax[warp] = vmax;
+        }
+        bar_compute();
+        if (tid == 0) sh.flag = 0;
+        int evm = 0;
+#pragma unroll
+        for (int w = 0; w < kComputeWarps; ++w) evm = max(evm, sh.wvmax[w]);
+        const int enew = evm > eref ? evm + 2 : eref;
+        const float fe = pow2i(eref - enew);
+        float f[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          float m = sh.wmax[4 * hh][j];
+#pragma unroll
+          for (int w = 1; w < 4; ++w) m = fmaxf(m, sh.wmax[4 * hh + w][j]);
+          const float mnew = fmaxf(mref[j], m);
+          const float fm = (mref[j] == -INFINITY) ? 0.f : ex2(mref[j] - mnew);
+          mref[j] = mnew;
+          lsum[j] *= fm;
+          f[j] = fm * fe;
+        }
+        eref = enew;
+        if (i > 0) {  // rescale O^T in TMEM: this thread owns channel r, heads 8hh..8hh+7
+          float ov[8];
+          const uint32_t t_o = tmem + lane_sel + kColO + 8 * hh;
+          tmem_ld8(t_o, ov);
+#pragma unroll
+          for (int j = 0; j < 8; ++j) ov[j] *= f[j];
+          tmem_st8(t_o, ov);
+        }
+        (void)v_multipliers(rest, scratch, lane, n_valid, eref);
+        v_convert(rest, scratch, sV, warp, lane, n_valid);
+        (void)softmax_pass(false);
+      }
+#pragma unroll
+      for (int j = 0; j < 8; ++j) lsum[j] += lt[j];
+      // publish Vhat / P to the tensor core, release the stage
+      fence_async_smem();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) {
+        mbar_arrive(bar_pvready);
+        mbar_arrive(bar_empty + 8 * s);
       }
     }
-    // P = 2^(x - mref); accumulate l; pack to f16 and transpose into B fragments of P^T
-    uint32_t pb[NT][2];
-#pragma unroll
-    for (int nt = 0; nt < NT; ++nt) {
-      const float p0v = ex2(S[nt][0] - mref[nt][0]), p1v = ex2(S[nt][1] - mref[nt][1]);
-      const float p2v = ex2(S[nt][2] - mref[nt][0]), p3v = ex2(S[nt][3] - mref[nt][1]);
-      lsum[nt][0] += p0v + p2v;
-      lsum[nt][1] += p1v + p3v;
-      pb[nt][0] = movm_trans(pack_f16x2(p0v, p1v));  // -> (tokens 2c,2c+1 ; head g)
-      pb[nt][1] = movm_trans(pack_f16x2(p2v, p3v));  // -> (tokens 2c+8,2c+9 ; head g)
-    }
 
-    // ---------------- V scales -> fp16 power-of-two multipliers relative to eref
-    // word (p, hf) holds bytes [tokA gr=2hf, tokA gr=2hf+1, tokB gr=2hf, tokB gr=2hf+1]
-    const uint32_t vw[4] = {vsc.x, vsc.y, vsc.z, vsc.w};
-    uint32_t vraw[2][4];  // [pair][group] as u16x2 (byte of token A, byte of token B)
-#pragma unroll
-    for (int p = 0; p < 2; ++p)
-#pragma unroll
-      for (int gr = 0; gr < 4; ++gr) vraw[p][gr] = prmt(vw[2 * p + (gr >> 1)], 0u, (gr & 1) ? 0x4341u : 0x4240u);
+    // ================================================================ epilogue: write the split's partial
+    mbar_wait(bar_pvdone, (n_tiles - 1) & 1);
+    tc_fence_after();
     {
-      uint32_t mx = vraw[0][0];
+      float ov[8];
+      tmem_ld8(tmem + lane_sel + kColO + 8 * hh, ov);
+      const float vscale = pow2i(eref - 13 - 127);      // stored Vhat = code * 2^(byte - eref + 13)
 #pragma unroll
-      for (int p = 0; p < 2; ++p)
-#pragma unroll
-        for (int gr = 0; gr < 4; ++gr) mx = max_u16x2(mx, vraw[p][gr]);
-      const int top = max((int)(mx & 0xFFFFu), (int)(mx >> 16));
-      if (__any_sync(kFull, top > eref)) {  // rare: raise the reference exponent, rescale O
-        int e = top;
-        e = max(e, __shfl_xor_sync(kFull, e, 1));
-        e = max(e, __shfl_xor_sync(kFull, e, 2));
-        e = max(e, eref);
-        const int fe = 127 + eref - e;  // 2^(eref - e); flushes to 0 beyond fp32 range
-        const float f = fe > 0 ? __uint_as_float((uint32_t)fe << 23) : 0.f;
-        eref = e;
-#pragma unroll
-        for (int mt = 0; mt < 8; ++mt)
-#pragma unroll
-          for (int nt = 0; nt < NT; ++nt)
-#pragma unroll
-            for (int j = 0; j < 4; ++j) O[mt][nt][j] *= f;
+      for (int j = 0; j < 8; ++j) {
+        const int head = 8 * hh + j;
+        if (head < G) partial_acc[(row0 + (long long)head * num_splits) * kHeadDim + r] = ov[j] * vscale;
       }
     }
-    const uint32_t kbase = (uint32_t)(eref - 28) * 0x00010001u;
-    uint32_t vmul[2][4];
 #pragma unroll
-    for (int p = 0; p < 2; ++p)
+    for (int j = 0; j < 8; ++j) {
+      float v = lsum[j];
 #pragma unroll
-      for (int gr = 0; gr < 4; ++gr) vmul[p][gr] = (max_u16x2(vraw[p][gr], kbase) - kbase) << 10;  // fp16 2^(byte-eref+13); 0 below 2^-14
-
-    // ---------------- O^T += Vhat^T P^T
-    const uint32_t vword[8] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
-#pragma unroll
-    for (int mt = 0; mt < 8; ++mt) {
-      uint32_t h[4];
-      cvt_e2m1x8(vword[mt], h);  // h0: pair0 d=16mt+g, h1: pair0 d+8, h2: pair1 d, h3: pair1 d+8
-      const uint32_t a0 = hmul2(h[0], vmul[0][mt >> 1]), a1 = hmul2(h[1], vmul[0][mt >> 1]);
-      const uint32_t a2 = hmul2(h[2], vmul[1][mt >> 1]), a3 = hmul2(h[3], vmul[1][mt >> 1]);
-#pragma unroll
-      for (int nt = 0; nt < NT; ++nt) mma_f16(O[mt][nt], a0, a1, a2, a3, pb[nt][0], pb[nt][1]);
+      for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+      lsum[j] = v;
     }
-
-    // ---------------- release the stage and refill it
-    __syncwarp();
-    if (i + kStages < n_my) issue(i + kStages);
-  }
-
-  // ================================================================ CTA combine of the warps
-  // l: sum the lanes that share the same heads (same c) over g
+    if (lane == 0) {
 #pragma unroll
-  for (int nt = 0; nt < NT; ++nt)
-#pragma unroll
-    for (int j = 0; j < 2; ++j) {
-      float v = lsum[nt][j];
-      v += __shfl_xor_sync(kFull, v, 4);
-      v += __shfl_xor_sync(kFull, v, 8);
-      v += __shfl_xor_sync(kFull, v, 16);
-      lsum[nt][j] = v;
-    }
-  if (g == 0) {
-#pragma unroll
-    for (int nt = 0; nt < NT; ++nt)
-#pragma unroll
-      for (int j = 0; j < 2; ++j) s_m[warp][8 * nt + 2 * c + j] = mref[nt][j];
-  }
-  if (lane == 0) s_e[warp] = eref;
-  __syncthreads();  // also: every warp is done with its ring, which becomes the staging buffer
-
-  int emax = s_e[0];
-#pragma unroll
-  for (int w = 1; w < kWarps; ++w) emax = max(emax, s_e[w]);
-  const int fe = 127 + eref - emax;
-  const float fexp = fe > 0 ? __uint_as_float((uint32_t)fe << 23) : 0.f;
-  float* stage = reinterpret_cast<float*>(smem) + (size_t)warp * 16 * kHeadStride;
-#pragma unroll
-  for (int nt = 0; nt < NT; ++nt)
-#pragma unroll
-    for (int j = 0; j < 2; ++j) {
-      const int head = 8 * nt + 2 * c + j;
-      float M = s_m[0][head];
-#pragma unroll
-      for (int w = 1; w < kWarps; ++w) M = fmaxf(M, s_m[w][head]);
-      const float fm = (mref[nt][j] == -INFINITY) ? 0.f : ex2(mref[nt][j] - M);
-      if (g == 0) s_l[warp][head] = lsum[nt][j] * fm;
-      const float f = fm * fexp;
-#pragma unroll
-      for (int mt = 0; mt < 8; ++mt) {
-        stage[head * kHeadStride + 16 * mt + g] = O[mt][nt][j] * f;
-        stage[head * kHeadStride + 16 * mt + g + 8] = O[mt][nt][j + 2] * f;
+      for (int j = 0; j < 8; ++j) {
+        sh.lsum[warp][j] = lsum[j];
+        if (q == 0) sh.mref[8 * hh + j] = mref[j];
       }
     }
+    bar_compute();
+    if (tid < G) {
+      const int h2 = tid >> 3, j = tid & 7;
+      float l = 0.f;
+#pragma unroll
+      for (int w = 0; w < 4; ++w) l += sh.lsum[4 * h2 + w][j];
+      float2* ml = reinterpret_cast<float2*>(partial_ml) + row0 + (long long)tid * num_splits;
+      *ml = make_float2(sh.mref[tid] * 0.6931471805599453f, l);  // natural-log units
+    }
+  }
+
+  // ---------------- teardown
+  tc_fence_before();
   __syncthreads();
+  if (warp == kComputeWarps + 1) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTmemCols));
+  }
+}
 
-  // sum over warps, undo the reference exponent, write the split's partial (coalesced)
-  const int ve = emax - 13;  // true value = acc * 2^(emax - 13 - 127)
-  const float vscale = __uint_as_float((uint32_t)max(ve, 0) << 23) * (ve < 0 ? 0.f : 1.f);
-  const float* stg = reinterpret_cast<const float*>(smem);
-  for (int idx = threadIdx.x; idx < G * kHeadDim; idx += kWarps * 32) {
-    const int head = idx >> 7, d = idx & 127;
-    float v = 0.f;
-#pragma unroll
-    for (int w = 0; w < kWarps; ++w) v += stg[(w * 16 + head) * kHeadStride + d];
-    partial_acc[(row0 + (long long)head * num_splits) * kHeadDim + d] = v * vscale;
+// ---------------------------------------------------------------- host: TMA descriptor of the K codes
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct MapEntry {
+  const void* cache;
+  long long records;
+  CUtensorMap map;
+};
+std::mutex g_map_mu;
+MapEntry g_maps[8];
+int g_map_n = 0, g_map_next = 0;
+
+// 3-D view of the cache for TMA: [record][16 tokens][128 x 4-bit]; box = one page of K codes.
+int32_t k_code_map(const void* cache, long long records, CUtensorMap* out) {
+  std::lock_guard<std::mutex> lock(g_map_mu);
+  for (int i = 0; i < g_map_n; ++i)
+    if (g_maps[i].cache == cache && g_maps[i].records == records) {
+      *out = g_maps[i].map;
+      return UQ_OK;
+    }
+  static EncodeTiledFn encode = nullptr;
+  if (!encode) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess || fn == nullptr) {
+      set_error("decode: cuTensorMapEncodeTiled is not available from this driver");
+      return UQ_ERR_CUDA;
+    }
+    encode = (EncodeTiledFn)fn;
   }
-  if (threadIdx.x < G) {
-    const int head = threadIdx.x;
-    float M = s_m[0][head], l = 0.f;
-#pragma unroll
-    for (int w = 1; w < kWarps; ++w) M = fmaxf(M, s_m[w][head]);
-#pragma unroll
-    for (int w = 0; w < kWarps; ++w) l += s_l[w][head];
-    float2* ml = reinterpret_cast<float2*>(partial_ml) + row0 + (long long)head * num_splits;
-    *ml = make_float2(M * 0.6931471805599453f, l);  // natural-log units
+  const cuuint64_t gdim[3] = {128, 16, (cuuint64_t)records};
+  const cuuint64_t gstr[2] = {64, (cuuint64_t)kRecordBytes};
+  const cuuint32_t box[3] = {128, 16, 1};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  CUtensorMap m;
+  const CUresult cr = encode(&m, CU_TENSOR_MAP_DATA_TYPE_16U4_ALIGN16B, 3, const_cast<void*>(cache), gdim, gstr, box,
+                             estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                             CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (cr != CUDA_SUCCESS) {
+    set_error("decode: cuTensorMapEncodeTiled failed with CUresult %d", (int)cr);
+    return UQ_ERR_CUDA;
   }
+  MapEntry& e = g_maps[g_map_next];
+  e.cache = cache;
+  e.records = records;
+  e.map = m;
+  g_map_next = (g_map_next + 1) % 8;
+  if (g_map_n < 8) ++g_map_n;
+  *out = m;
+  return UQ_OK;
 }
 
 }  // namespace
@@ -475,30 +633,29 @@ extern "C" int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, 
     set_error("decode: batch and num_kv_heads must be <= 65535");
     return UQ_ERR_INVALID_ARG;
   }
-  if (((uintptr_t)cache & 15u) || ((uintptr_t)q_fp8 & 7u) || ((uintptr_t)partial_acc & 15u) ||
+  if (((uintptr_t)cache & 31u) || ((uintptr_t)q_fp8 & 15u) || ((uintptr_t)partial_acc & 15u) ||
       ((uintptr_t)partial_ml & 7u)) {
-    set_error("decode: misaligned pointer (cache 16 B, q_fp8 8 B, partial_acc 16 B, partial_ml 8 B)");
+    set_error("decode: misaligned pointer (cache 32 B, q_fp8 16 B, partial_acc 16 B, partial_ml 8 B)");
     return UQ_ERR_INVALID_ARG;
   }
-  const int G = cfg->num_q_heads / cfg->num_kv_heads;
-  const size_t ring = (size_t)kWarps * kStages * kRecordBytes;
-  const size_t staging = (size_t)kWarps * 16 * kHeadStride * sizeof(float);
-  const size_t smem = ring > staging ? ring : staging;
-  const float score_scale = resolved_sm_scale(cfg) * 1.4426950408889634f * 64.0f;
-  const dim3 grid((unsigned)num_splits, (unsigned)cfg->num_kv_heads, (unsigned)batch);
-  cudaError_t e;
-  if (G <= 8) {
-    e = cudaFuncSetAttribute(decode_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return check_cuda(e, "decode: cudaFuncSetAttribute");
-    decode_kernel<1><<<grid, kWarps * 32, smem, (cudaStream_t)stream>>>(
-        (const uint8_t*)q_fp8, (const uint8_t*)cache, block_tables, max_pages, seq_lens, cfg->num_q_heads,
-        cfg->num_kv_heads, num_splits, score_scale, partial_acc, partial_ml);
-  } else {
-    e = cudaFuncSetAttribute(decode_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return check_cuda(e, "decode: cudaFuncSetAttribute");
-    decode_kernel<2><<<grid, kWarps * 32, smem, (cudaStream_t)stream>>>(
-        (const uint8_t*)q_fp8, (const uint8_t*)cache, block_tables, max_pages, seq_lens, cfg->num_q_heads,
-        cfg->num_kv_heads, num_splits, score_scale, partial_acc, partial_ml);
+  const long long records = (long long)num_pages * cfg->num_kv_heads;
+  if (records > 0x7fffffffLL) {
+    set_error("decode: num_pages * num_kv_heads must be < 2^31");
+    return UQ_ERR_INVALID_ARG;
   }
+  CUtensorMap tmap;
+  st = k_code_map(cache, records, &tmap);
+  if (st != UQ_OK) return st;
+  const float score_scale = resolved_sm_scale(cfg) * 1.4426950408889634f;
+  const dim3 grid((unsigned)num_splits, (unsigned)cfg->num_kv_heads, (unsigned)batch);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e != cudaSuccess) return check_cuda(e, "decode: cudaFuncSetAttribute");
+    attr_set = true;
+  }
+  decode_kernel<<<grid, kThreads, kSmemBytes, (cudaStream_t)stream>>>(
+      tmap, (const uint8_t*)q_fp8, (const uint8_t*)cache, block_tables, max_pages, seq_lens, cfg->num_q_heads,
+      cfg->num_kv_heads, num_splits, score_scale, partial_acc, partial_ml);
   return check_cuda(cudaGetLastError(), "uq_decode_attention launch");
 }

@@ -173,11 +173,18 @@ def test_wide_scale_spread_and_zero_vectors():
     H.compare_cache(cache, wl, 0, 64, arrays)
     q = W.gen_q(wl, DEV) * 0.05                            # diffuse attention: every token counts
     out, _, _ = H.run_decode(cfg, cache, bt, wl.ctx_lens, q.to(torch.bfloat16), 1)
-    ref, _ = H.oracle_out(wl, 0, 64, H.bits(q.to(torch.bfloat16))[0], arrays)
+    qb16 = q.to(torch.bfloat16)
+    q8 = oracle.encode_q(H.bits(qb16)[0])
+    ref, probs = oracle.attention(q8, *arrays, wl.num_q_heads, wl.num_kv_heads, None, return_probs=True)
     got = out[0].float().cpu().numpy().astype(np.float64)
-    # tolerance relative to the dominant magnitude: rows hold values ~2^12
+    # V is scaled by 2^12 here, so terms of magnitude ~300 cancel in some outputs.  P enters the PV
+    # product as fp16 (relative rounding 2^-11 per term), hence the bound
+    # carries 2^-10 * sum_t p_t |vhat_t| next to the north-star terms.
+    vhat = np.abs(oracle.dequantize(arrays[2], arrays[3])[:, 0, :])          # [L, d]
+    mass = probs @ vhat                                                       # [Hq, d]
     err = np.abs(got - ref)
-    assert np.all(err <= 2e-3 + 1e-2 * np.abs(ref) + 2.0 ** -14 * np.abs(ref).max()), err.max()
+    bound = 2e-3 + 1e-2 * np.abs(ref) + 2.0 ** -10 * mass
+    assert np.all(err <= bound), float((err / bound).max())
 
 
 def test_permuting_physical_pages_leaves_output_unchanged():

@@ -13,9 +13,7 @@ def _k_code_index():
     idx = np.zeros((PAGE, 64), np.int64)
     for t in range(PAGE):
         for j in range(64):
-            word, byte = divmod(j, 4)             # logical word = channels 8*word .. 8*word+7
-            ks, c = divmod(word, 4)
-            idx[t, j] = 64 * t + 4 * (4 * c + ks) + byte
+            idx[t, j] = 64 * t + j                # logical order
     return idx
 
 
@@ -24,11 +22,11 @@ def _v_code_index():
     idx = np.zeros((PAGE, 128), np.int64)
     sh = np.zeros((PAGE, 128), np.int64)
     for t in range(PAGE):
-        p, c = (t >> 3) & 1, (t & 7) >> 1
         for d in range(128):
-            mt, g, hi = d >> 4, d & 7, (d >> 3) & 1
-            idx[t, d] = 1024 + 512 * (mt >> 2) + 16 * (4 * g + c) + 4 * (mt & 3) + 2 * p + hi
-            sh[t, d] = 4 * (t & 1)
+            word = 1024 + 512 * (t >> 3) + 16 * (d & 31) + 4 * (d >> 5)
+            bit = 4 * (t & 7)                      # token t in bits 4(t&7)..4(t&7)+3 of the word
+            idx[t, d] = word + bit // 8            # little-endian byte of the word
+            sh[t, d] = bit % 8
     return idx, sh
 
 
@@ -36,16 +34,15 @@ def _k_scale_index():
     idx = np.zeros((PAGE, 4), np.int64)
     for t in range(PAGE):
         for gr in range(4):
-            idx[t, gr] = 2048 + 4 * (2 * (t & 7) + (t >> 3)) + gr
+            idx[t, gr] = 2048 + 4 * t + gr
     return idx
 
 
 def _v_scale_index():
     idx = np.zeros((PAGE, 4), np.int64)
     for t in range(PAGE):
-        p, c, odd = (t >> 3) & 1, (t & 7) >> 1, t & 1
         for gr in range(4):
-            idx[t, gr] = 2112 + 16 * c + 4 * (2 * p + (gr >> 1)) + 2 * odd + (gr & 1)
+            idx[t, gr] = 2112 + 32 * (t >> 3) + 8 * gr + (t & 7)
     return idx
 
 
