@@ -13,11 +13,12 @@
 //           scales applied by the tensor core (the paper's FP8xFP4 scaled MMA), K
 //           scales staged smem -> TMEM with tcgen05.cp; then O^T[128 d x 16 heads] += Vhat^T . P^T
 //           with tcgen05.mma.kind::f16; accumulators live in TMEM;
-//   warps 0-7 compute: V codes -> fp16 (cvt.rn.f16x2.e2m1x2 x exact power-of-two scale) into the
-//           K-major operand layout; S rows from TMEM (tcgen05.ld), base-2 softmax against a LAZY
-//           per-head reference (a "rebase" — new reference, O rescaled in TMEM, tile redone —
-//           happens on the first tile and whenever a score exceeds the reference by 2^12 or a V
-//           scale exceeds the reference exponent), P -> fp16 operand in smem.
+//   warps 0-7 compute: S rows from TMEM (tcgen05.ld), base-2 softmax against a LAZY per-head
+//           reference (a "rebase" — new reference, O rescaled in TMEM, tile's P redone — happens on
+//           the first tile and whenever a score exceeds the reference by 2^12 or a V scale exceeds
+//           the reference exponent), P -> fp16 operand in smem (double-buffered); then V codes ->
+//           fp16 (cvt.rn.f16x2.e2m1x2 x exact power-of-two scale) into the K-major operand layout
+//           (one page per warp); the PV MMAs of a tile run under the softmax of the next one.
 // The FP8 query tile is written to smem once per CTA ("hoisted").
 // Every K/V byte is read from HBM exactly once.
 #include <cuda.h>
@@ -32,11 +33,17 @@ namespace {
 
 constexpr int kComputeWarps = 8;
 constexpr int kThreads = (kComputeWarps + 2) * 32;   // + producer warp + MMA warp
-constexpr int kStages = 2;
+#ifndef UQ_STAGES
+#define UQ_STAGES 2
+#endif
+#ifndef UQ_CTAS_PER_SM
+#define UQ_CTAS_PER_SM 2
+#endif
+constexpr int kStages = UQ_STAGES;
 constexpr int kTilePages = 8;                        // 128 tokens per tile
 constexpr int kRestBytes = kRecordBytes - 1024;      // V codes + K scales + V scales = 1152
 constexpr int kStageBytes = kTilePages * (2048 + kRestBytes);   // K unpacked 16 KB + 9216 = 25600
-constexpr int kPStride = 272;                        // bytes between token-cores of the P operand
+constexpr int kPBytes = 4096;                        // one P operand buffer: [token-core 16][head-core 2][8 tok][8 heads] f16
 constexpr float kThresh = 12.0f;                     // lazy-reference threshold (log2 units)
 constexpr unsigned kFull = 0xffffffffu;
 
@@ -46,8 +53,8 @@ constexpr int kOffQ = kOffStage + kStages * kStageBytes;       // 2048, SW128
 constexpr int kOffSFA = kOffQ + 2048;                          // 2 x 512
 constexpr int kOffSFB = kOffSFA + 1024;                        // 512
 constexpr int kOffV = kOffSFB + 512;                           // 32768: [token-core 16][d 128][16 B]
-constexpr int kOffP = kOffV + 32768;                           // 16 x 272
-constexpr int kOffMul = kOffP + 16 * kPStride + 256;           // 8 warps x 128 B
+constexpr int kOffP = kOffV + 32768;                           // 2 x 4096 (double-buffered)
+constexpr int kOffMul = kOffP + 2 * kPBytes;                   // 8 warps x 128 B
 constexpr int kOffEnd = kOffMul + kComputeWarps * 128;
 constexpr int kSmemBytes = kOffEnd + 1024;                     // + alignment slack
 
@@ -82,6 +89,12 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "DONE_%=:\n"
       "}\n" ::"r"(bar), "r"(parity) : "memory");
 }
+__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {   // one non-blocking probe
+  uint32_t ok;
+  asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
+               : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+  return ok != 0;
+}
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
@@ -94,6 +107,13 @@ __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.a
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void bar_compute() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
+// barrier over the 256 compute threads that also ORs a predicate across them
+__device__ __forceinline__ bool bar_compute_or(bool pred) {
+  uint32_t r;
+  asm volatile("{\n.reg .pred p, q;\nsetp.ne.b32 q, %1, 0;\nbar.red.or.pred p, 1, 256, q;\nselp.u32 %0, 1, 0, p;\n}\n"
+               : "=r"(r) : "r"((uint32_t)pred) : "memory");
+  return r != 0;
+}
 
 // shared-memory matrix descriptor (SM100 UMMA): start>>4 | LBO>>4 <<16 | SBO>>4 <<32 | version 1 | layout
 __device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes, uint32_t layout) {
@@ -180,47 +200,39 @@ struct Shared {
   uint64_t full[kStages];     // producer -> consumers: stage landed (tx bytes)
   uint64_t empty[kStages];    // 8 compute warps + QK commit -> producer
   uint64_t s_full[2];         // QK commit -> compute warps
-  uint64_t pv_ready;          // 8 compute warps -> MMA warp (Vhat and P of the tile are in smem)
-  uint64_t pv_done;           // PV commit -> compute warps (Vhat / P buffers free, O up to date)
+  uint64_t ready;             // 8 compute warps -> MMA warp: P and Vhat of the tile are in smem
+  uint64_t done;              // PV commit -> compute warps (Vhat free, O up to date)
   uint32_t tmem_base;
-  volatile int flag;          // a warp asked for a rebase of the references
   float wmax[kComputeWarps][8];
   int wvmax[kComputeWarps];
   float lsum[kComputeWarps][8];
   float mref[16];
 };
 
-// V scale bytes of this warp's page -> fp16 power-of-two multipliers in the warp's scratch;
-// returns the largest scale byte among the page's valid tokens (warp-uniform).
+// V scale bytes of this warp's page -> fp16 power-of-two multipliers (one f16x2 per token pair
+// and group) in the warp's scratch; returns the largest scale byte among the page's valid tokens
+// (warp-uniform).  rest = the page's [V codes | K scales | V scales] block in the stage.
+template <bool kPartial>
 __device__ __forceinline__ int v_multipliers(uint32_t rest, uint32_t scratch, int lane, int n_valid, int eref) {
   uint32_t pair;
   asm volatile("ld.shared.u16 %0, [%1];" : "=r"(pair) : "r"(rest + 1088 + 2 * lane));
   int lo = (int)(pair & 0xFFu), hi = (int)(pair >> 8);
-  const int tok = 8 * (lane >> 4) + 2 * (lane & 3);
-  if (tok >= n_valid) lo = 0;
-  if (tok + 1 >= n_valid) hi = 0;
+  if (kPartial) {
+    const int tok = 8 * (lane >> 4) + 2 * (lane & 3);
+    if (tok >= n_valid) lo = 0;
+    if (tok + 1 >= n_valid) hi = 0;
+  }
   const int vmax = __reduce_max_sync(kFull, max(lo, hi));
   const int kbase = eref - 28;                       // fp16 exponent field = byte - kbase (2^13 at byte = eref)
-  const uint32_t mlo = (uint32_t)max(lo - kbase, 0), mhi = (uint32_t)max(hi - kbase, 0);
-  const uint32_t mult = (lo ? (mlo << 10) : 0u) | (hi ? (mhi << 26) : 0u);
-  __syncwarp();
-  asm volatile("st.shared.u32 [%0], %1;" ::"r"(scratch + 4 * lane), "r"(mult) : "memory");
+  const uint32_t mlo = (uint32_t)max(lo - kbase, 0), mhi = (uint32_t)max(hi - kbase, 0);   // byte 0 -> multiplier 0
+  asm volatile("st.shared.u32 [%0], %1;" ::"r"(scratch + 4 * lane), "r"((mlo << 10) | (mhi << 26)) : "memory");
   __syncwarp();
   return vmax;
 }
 
-// V codes of this warp's page (16 tokens x 128 channels) -> fp16 Vhat^T operand:
-// [token-core tc][d][8 tokens], tc = 2*page_in_tile + half.
-__device__ __forceinline__ void v_convert(uint32_t rest, uint32_t scratch, uint32_t sV, int page_in_tile, int lane,
-                                          int n_valid) {
-  if (n_valid <= 0) {
-    const uint4 z = make_uint4(0u, 0u, 0u, 0u);
-#pragma unroll
-    for (int h = 0; h < 2; ++h)
-#pragma unroll
-      for (int i = 0; i < 4; ++i) sts128(sV + (2 * page_in_tile + h) * 2048 + (32 * i + lane) * 16, z);
-    return;
-  }
+// V codes of this warp's page (16 tokens x 128 channels) -> fp16 Vhat^T operand
+// [token-core][d][8 tokens]; v_dst = the page's two token-cores (2 x 2048 B).
+__device__ __forceinline__ void v_convert(uint32_t rest, uint32_t scratch, uint32_t v_dst, int lane) {
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
     const uint4 c4 = lds128(rest + 512 * h + 16 * lane);
@@ -235,13 +247,14 @@ __device__ __forceinline__ void v_convert(uint32_t rest, uint32_t scratch, uint3
       o.y = hmul2(f[1], m4.y);
       o.z = hmul2(f[2], m4.z);
       o.w = hmul2(f[3], m4.w);
-      sts128(sV + (2 * page_in_tile + h) * 2048 + (32 * i + lane) * 16, o);
+      sts128(v_dst + 2048 * h + (32 * i + lane) * 16, o);
     }
   }
+  __syncwarp();
 }
 
 // ---------------------------------------------------------------- the kernel
-__global__ void __launch_bounds__(kThreads, 2)
+__global__ void __launch_bounds__(kThreads, UQ_CTAS_PER_SM)
 decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restrict__ q_fp8,
               const uint8_t* __restrict__ cache, const int32_t* __restrict__ block_tables, int max_pages,
               const int32_t* __restrict__ seq_lens, int Hq, int Hkv, int num_splits,
@@ -275,8 +288,8 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
   const uint32_t sQ = base + kOffQ, sSFA = base + kOffSFA, sSFB = base + kOffSFB, sV = base + kOffV,
                  sP = base + kOffP;
   const uint32_t bar_full = smem_u32(&sh.full[0]), bar_empty = smem_u32(&sh.empty[0]),
-                 bar_sfull = smem_u32(&sh.s_full[0]), bar_pvready = smem_u32(&sh.pv_ready),
-                 bar_pvdone = smem_u32(&sh.pv_done);
+                 bar_sfull = smem_u32(&sh.s_full[0]), bar_ready = smem_u32(&sh.ready),
+                 bar_done = smem_u32(&sh.done);
 
   // ---------------- setup
   if (tid == 0) {
@@ -287,9 +300,8 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
     }
     mbar_init(bar_sfull, 1);
     mbar_init(bar_sfull + 8, 1);
-    mbar_init(bar_pvready, kComputeWarps);
-    mbar_init(bar_pvdone, 1);
-    sh.flag = 0;
+    mbar_init(bar_ready, kComputeWarps);
+    mbar_init(bar_done, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == kComputeWarps + 1) {
@@ -336,24 +348,20 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
     if (lane == 0) umma_cp_sf(tmem + kColSFB, make_desc(sSFB, 16, 128, 0));
     // E2M1 (5) x E4M3 (0), UE8M0 scales, N = 16, M = 128
     const uint32_t idesc_qk = (5u << 7) | (0u << 10) | (2u << 17) | (1u << 23) | (8u << 24);
-    // f16 x f16 -> f32, N = 16, M = 128
-    const uint32_t idesc_pv = (1u << 4) | (2u << 17) | (8u << 24);
+    // f16 x f16 -> f32, B (= P) MN-major, N = 16, M = 128
+    const uint32_t idesc_pv = (1u << 4) | (1u << 16) | (2u << 17) | (8u << 24);
     auto issue_qk = [&](int i) {
       const int s = i % kStages, sb = i & 1;
       const uint32_t st = base + kOffStage + s * kStageBytes;
       mbar_wait(bar_full + 8 * s, (i / kStages) & 1);
       // scale-factor atom: row r = 32 c + lane of the tile -> 16-byte line `lane`, word c
-      uint4 w;
-      {
-        uint32_t v[4];
+      uint32_t v[4];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-          const int r = 32 * c + lane;
-          asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v[c]) : "r"(st + 16384 + kRestBytes * (r >> 4) + 1024 + 4 * (r & 15)));
-        }
-        w = make_uint4(v[0], v[1], v[2], v[3]);
+      for (int c = 0; c < 4; ++c) {
+        const int r = 32 * c + lane;
+        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v[c]) : "r"(st + 16384 + kRestBytes * (r >> 4) + 1024 + 4 * (r & 15)));
       }
-      sts128(sSFA + 512 * sb + 16 * lane, w);
+      sts128(sSFA + 512 * sb + 16 * lane, make_uint4(v[0], v[1], v[2], v[3]));
       fence_async_smem();
       __syncwarp();
       tc_fence_after();
@@ -371,17 +379,27 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
     };
     issue_qk(0);
     for (int i = 0; i < n_tiles; ++i) {
-      if (i + 1 < n_tiles) issue_qk(i + 1);
-      mbar_wait(bar_pvready, i & 1);
+      // QK of the next tile goes first if its bytes have landed; PV of this tile as soon as it is ready
+      bool qk_done = (i + 1 >= n_tiles);
+      for (;;) {
+        if (!qk_done && __any_sync(kFull, mbar_test(bar_full + 8 * ((i + 1) % kStages), ((i + 1) / kStages) & 1))) {
+          issue_qk(i + 1);
+          qk_done = true;
+        }
+        if (__any_sync(kFull, mbar_test(bar_ready, i & 1))) break;
+      }
+      mbar_wait(bar_ready, i & 1);
       tc_fence_after();
       if (lane == 0) {
+        const uint32_t pbuf = sP + kPBytes * (i & 1);
 #pragma unroll
-        for (int j = 0; j < 8; ++j)
-          umma_f16(tmem + kColO, make_desc(sV + 4096 * j, 2048, 128, 0), make_desc(sP + 2 * kPStride * j, kPStride, 128, 0),
+        for (int j = 0; j < 8; ++j)                    // 16 tokens per MMA = token-cores 2j, 2j+1
+          umma_f16(tmem + kColO, make_desc(sV + 4096 * j, 2048, 128, 0), make_desc(pbuf + 512 * j, 256, 128, 0),
                    idesc_pv, (i > 0 || j > 0) ? 1u : 0u);
-        umma_commit(bar_pvdone);
+        umma_commit(bar_done);
       }
       __syncwarp();
+      if (!qk_done) issue_qk(i + 1);
     }
   } else {
     // ================================================================ compute warps 0..7
@@ -390,6 +408,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
     const bool heads_live = (8 * hh < G);
     const uint32_t scratch = base + kOffMul + 128 * warp;
     const uint32_t lane_sel = (uint32_t)(32 * q) << 16;
+    const uint32_t v_dst = sV + warp * 4096;           // this warp converts page `warp` of every tile
     float mref[8], lsum[8];
 #pragma unroll
     for (int j = 0; j < 8; ++j) { mref[j] = -INFINITY; lsum[j] = 0.f; }
@@ -397,59 +416,56 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
 
     for (int i = 0; i < n_tiles; ++i) {
       const int s = i % kStages, sb = i & 1;
-      const uint32_t st = base + kOffStage + s * kStageBytes;
-      const uint32_t rest = st + 16384 + kRestBytes * warp;          // this warp converts page `warp` of the tile
-      const int pg = p0 + kTilePages * i + warp;
-      const int n_valid = pg < p1 ? min(kPage, L - kPage * pg) : 0;
-      const int tok = (p0 + kTilePages * i) * kPage + r;
-      const bool tok_ok = tok < tok_end;
+      const uint32_t rest = base + kOffStage + s * kStageBytes + 16384 + kRestBytes * warp;
+      const int pg0 = p0 + kTilePages * i;                           // first page of the tile
+      const bool tile_partial = (pg0 + kTilePages) * kPage > tok_end;
+      const bool tok_ok = pg0 * kPage + r < tok_end;
+      const int n_valid = tile_partial ? (pg0 + warp < p1 ? min(kPage, L - kPage * (pg0 + warp)) : 0) : kPage;
       const uint32_t t_s = tmem + lane_sel + kColS + 16 * sb + 8 * hh;
-      const uint32_t p_addr = sP + (r >> 3) * kPStride + (8 * hh) * 16 + (r & 7) * 2;
+      const uint32_t p_addr = sP + kPBytes * sb + (r >> 3) * 256 + hh * 128 + (r & 7) * 16;
 
-      mbar_wait(bar_full + 8 * s, (i / kStages) & 1);
-      if (i > 0) mbar_wait(bar_pvdone, (i - 1) & 1);                 // Vhat / P buffers free, O complete
+      mbar_wait(bar_sfull + 8 * sb, (i >> 1) & 1);                   // S of the tile is in TMEM
+      tc_fence_after();
+      mbar_wait(bar_full + 8 * s, (i / kStages) & 1);                // (already complete) acquire the TMA bytes
+
       float lt[8];
-
-      // softmax of this thread's row against the current references; returns "a score exceeded"
-      auto softmax_pass = [&](bool detect) -> bool {
-        bool ex = false;
+      // softmax of this thread's row against the current references -> P (fp16, MN-major operand)
+      auto softmax_pass = [&]() -> bool {
 #pragma unroll
         for (int j = 0; j < 8; ++j) lt[j] = 0.f;
         if (!heads_live) return false;
-        float sv[8];
-        tmem_ld8(t_s, sv);
+        float t[8];
+        tmem_ld8(t_s, t);
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const float x = tok_ok ? sv[j] * score_scale : -INFINITY;
-          if (detect) ex |= x > mref[j] + kThresh;
-          const float p = ex2(x - mref[j]);
-          lt[j] = p;
-          const __half hp = __float2half_rn(p);
-          asm volatile("st.shared.u16 [%0], %1;" ::"r"(p_addr + 16 * j), "h"(__half_as_ushort(hp)) : "memory");
+        for (int j = 0; j < 8; ++j) t[j] = fmaf(t[j], score_scale, -mref[j]);
+        if (tile_partial) {
+#pragma unroll
+          for (int j = 0; j < 8; ++j) t[j] = tok_ok ? t[j] : -INFINITY;
         }
-        return ex;
+        const float tmax = fmaxf(fmaxf(fmaxf(t[0], t[1]), fmaxf(t[2], t[3])), fmaxf(fmaxf(t[4], t[5]), fmaxf(t[6], t[7])));
+#pragma unroll
+        for (int j = 0; j < 8; ++j) lt[j] = ex2(t[j]);
+        uint4 o;
+        asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.x) : "f"(lt[1]), "f"(lt[0]));
+        asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.y) : "f"(lt[3]), "f"(lt[2]));
+        asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.z) : "f"(lt[5]), "f"(lt[4]));
+        asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.w) : "f"(lt[7]), "f"(lt[6]));
+        sts128(p_addr, o);
+        return tmax > kThresh;
       };
 
       bool rebase = (i == 0);
+      int vmax = 0;
       if (!rebase) {
-        const int vmax = v_multipliers(rest, scratch, lane, n_valid, eref);
-        v_convert(rest, scratch, sV, warp, lane, n_valid);
-        mbar_wait(bar_sfull + 8 * sb, (i >> 1) & 1);
-        tc_fence_after();
-        const bool ex = softmax_pass(true);
-        if (__any_sync(kFull, ex) || vmax > eref) {
-          if (lane == 0) sh.flag = 1;
-        }
+        const bool ex = softmax_pass();
+        vmax = tile_partial ? v_multipliers<true>(rest, scratch, lane, n_valid, eref)
+                            : v_multipliers<false>(rest, scratch, lane, n_valid, eref);
         tc_fence_before();
-        bar_compute();
-        rebase = sh.flag != 0;
-      } else {
-        mbar_wait(bar_sfull + 8 * sb, (i >> 1) & 1);
-        tc_fence_after();
+        rebase = bar_compute_or(ex || vmax > eref);
       }
       if (rebase) {
         // ---- statistics of the tile: per-head maximum score, maximum V scale byte
-        const int vmax = v_multipliers(rest, scratch, lane, n_valid, eref);
+        vmax = v_multipliers<true>(rest, scratch, lane, n_valid, eref);
         float tm[8];
 #pragma unroll
         for (int j = 0; j < 8; ++j) tm[j] = -INFINITY;
@@ -469,8 +485,8 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
           for (int j = 0; j < 8; ++j) sh.wmax[warp][j] = tm[j];
           sh.wvmax[warp] = vmax;
         }
+        tc_fence_before();
         bar_compute();
-        if (tid == 0) sh.flag = 0;
         int evm = 0;
 #pragma unroll
         for (int w = 0; w < kComputeWarps; ++w) evm = max(evm, sh.wvmax[w]);
@@ -489,32 +505,43 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
           f[j] = fm * fe;
         }
         eref = enew;
-        if (i > 0) {  // rescale O^T in TMEM: this thread owns channel r, heads 8hh..8hh+7
+        if (i > 0) {  // every PV issued so far has to be in O before it is rescaled
+          mbar_wait(bar_done, (i - 1) & 1);
+          tc_fence_after();
           float ov[8];
-          const uint32_t t_o = tmem + lane_sel + kColO + 8 * hh;
+          const uint32_t t_o = tmem + lane_sel + kColO + 8 * hh;   // channel r, heads 8hh..8hh+7
           tmem_ld8(t_o, ov);
 #pragma unroll
           for (int j = 0; j < 8; ++j) ov[j] *= f[j];
           tmem_st8(t_o, ov);
         }
-        (void)v_multipliers(rest, scratch, lane, n_valid, eref);
-        v_convert(rest, scratch, sV, warp, lane, n_valid);
-        (void)softmax_pass(false);
+        (void)softmax_pass();
+        (void)v_multipliers<true>(rest, scratch, lane, n_valid, eref);
+        bar_compute();                                  // wmax / wvmax may be rewritten only after every warp read them
       }
 #pragma unroll
       for (int j = 0; j < 8; ++j) lsum[j] += lt[j];
-      // publish Vhat / P to the tensor core, release the stage
+
+      // ---- V codes of page `warp` -> Vhat^T (the PV MMAs of the previous tile ran under the softmax above)
+      if (i > 0) mbar_wait(bar_done, (i - 1) & 1);
+      if (n_valid > 0) {
+        v_convert(rest, scratch, v_dst, lane);
+      } else {
+        const uint4 z = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) sts128(v_dst + 512 * k + 16 * lane, z);
+      }
       fence_async_smem();
       tc_fence_before();
       __syncwarp();
       if (lane == 0) {
-        mbar_arrive(bar_pvready);
+        mbar_arrive(bar_ready);
         mbar_arrive(bar_empty + 8 * s);
       }
     }
 
     // ================================================================ epilogue: write the split's partial
-    mbar_wait(bar_pvdone, (n_tiles - 1) & 1);
+    mbar_wait(bar_done, (n_tiles - 1) & 1);
     tc_fence_after();
     {
       float ov[8];
