@@ -37,7 +37,7 @@
  *                and channel 2j+1 in bits 4-7 (what Alg. 1 l.5 writes; the tensor cores read
  *                it directly as E2M1).
  *   [1024,2048)  V codes, token-major nibbles.  The 32-bit word at
- *                   1024 + 512*(t>>3) + 16*(d&31) + 4*(d>>5)
+ *                   1024 + 512*(t>>3) + 128*(d>>5) + 4*(d&31)
  *                holds channel d of the eight tokens 8*(t>>3) .. 8*(t>>3)+7; token t sits in
  *                bits 4*(t&7) .. 4*(t&7)+3.
  *   [2048,2112)  K scale bytes: token t's four group bytes (group 0 first) at 2048 + 4*t.

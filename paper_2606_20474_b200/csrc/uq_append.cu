@@ -165,12 +165,12 @@ append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v
       store_k(krow + (long long)Hkv * kHeadDim, rec, t + 1, lane, c_k);
       cb = encode_v(vrow + (long long)Hkv * kHeadDim, rec, t + 1, lane, c_v);
     }
-    // token-major nibbles: channel d = 4*lane + r lives in word 512*(t>>3) + 16*(d&31) + 4*(d>>5),
+    // token-major nibbles: channel d = 4*lane + r lives in word 512*(t>>3) + 128*(d>>5) + 4*(d&31),
     // tokens (t, t+1) share byte (t&7)>>1 of that word
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
       const int d = 4 * lane + r;
-      uint8_t* dst = rec + kOffVCodes + 512 * (t >> 3) + 16 * (d & 31) + 4 * (d >> 5) + ((t & 7) >> 1);
+      uint8_t* dst = rec + kOffVCodes + 512 * (t >> 3) + 128 * (d >> 5) + 4 * (d & 31) + ((t & 7) >> 1);
       const uint32_t a4 = (ca >> (8 * r)) & 0xF, b4 = (cb >> (8 * r)) & 0xF;
       *dst = odd ? (uint8_t)((*dst & 0x0F) | (a4 << 4)) : (uint8_t)(a4 | (b4 << 4));
     }

@@ -12,13 +12,15 @@
 //           tcgen05.mma.kind::mxf8f6f4.block_scale — E2M1 keys x E4M3 queries with the UE8M0 group
 //           scales applied by the tensor core (the paper's FP8xFP4 scaled MMA), K
 //           scales staged smem -> TMEM with tcgen05.cp; then O^T[128 d x 16 heads] += Vhat^T . P^T
-//           with tcgen05.mma.kind::f16; accumulators live in TMEM;
+//           with tcgen05.mma.kind::f16 (A = Vhat^T from TMEM, B = P from smem); accumulators in TMEM;
 //   warps 0-7 compute: S rows from TMEM (tcgen05.ld), base-2 softmax against a LAZY per-head
 //           reference (a "rebase" — new reference, O rescaled in TMEM, tile's P redone — happens on
 //           the first tile and whenever a score exceeds the reference by 2^12 or a V scale exceeds
 //           the reference exponent), P -> fp16 operand in smem (double-buffered); then V codes ->
-//           fp16 (cvt.rn.f16x2.e2m1x2 x exact power-of-two scale) into the K-major operand layout
-//           (one page per warp); the PV MMAs of a tile run under the softmax of the next one.
+//           fp16 (cvt.rn.f16x2.e2m1x2 x exact power-of-two scale) written with tcgen05.st straight
+//           into TMEM, where the PV MMA reads it as its A operand (no shared-memory round trip:
+//           the kernel is shared-memory-bandwidth sensitive); the PV MMAs of a tile run under the
+//           softmax of the next one.
 // The FP8 query tile is written to smem once per CTA ("hoisted").
 // Every K/V byte is read from HBM exactly once.
 #include <cuda.h>
@@ -34,7 +36,7 @@ namespace {
 constexpr int kComputeWarps = 8;
 constexpr int kThreads = (kComputeWarps + 2) * 32;   // + producer warp + MMA warp
 #ifndef UQ_STAGES
-#define UQ_STAGES 2
+#define UQ_STAGES 3
 #endif
 #ifndef UQ_CTAS_PER_SM
 #define UQ_CTAS_PER_SM 2
@@ -52,8 +54,7 @@ constexpr int kOffStage = 0;
 constexpr int kOffQ = kOffStage + kStages * kStageBytes;       // 2048, SW128
 constexpr int kOffSFA = kOffQ + 2048;                          // 2 x 512
 constexpr int kOffSFB = kOffSFA + 1024;                        // 512
-constexpr int kOffV = kOffSFB + 512;                           // 32768: [token-core 16][d 128][16 B]
-constexpr int kOffP = kOffV + 32768;                           // 2 x 4096 (double-buffered)
+constexpr int kOffP = kOffSFB + 512;                           // 2 x 4096 (double-buffered)
 constexpr int kOffMul = kOffP + 2 * kPBytes;                   // 8 warps x 128 B
 constexpr int kOffEnd = kOffMul + kComputeWarps * 128;
 constexpr int kSmemBytes = kOffEnd + 1024;                     // + alignment slack
@@ -63,7 +64,8 @@ constexpr uint32_t kColS = 0;      // 2 x 16
 constexpr uint32_t kColO = 32;     // 16
 constexpr uint32_t kColSFA = 48;   // 2 x 4
 constexpr uint32_t kColSFB = 56;   // 4
-constexpr uint32_t kTmemCols = 64;
+constexpr uint32_t kColV = 64;     // 64: Vhat^T operand, lane = channel d, column c = tokens 2c, 2c+1 (f16x2)
+constexpr uint32_t kTmemCols = 128;
 
 // ---------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -161,6 +163,22 @@ __device__ __forceinline__ void tmem_st8(uint32_t taddr, const float (&v)[8]) {
                  "r"(__float_as_uint(v[6])), "r"(__float_as_uint(v[7])) : "memory");
   asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"
+      "%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"
+      ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]),
+        "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]), "r"(v[16]), "r"(v[17]),
+        "r"(v[18]), "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]), "r"(v[24]), "r"(v[25]), "r"(v[26]),
+        "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31]) : "memory");
+  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void umma_f16_ts(uint32_t d, uint32_t ta, uint64_t db, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n}\n"
+      ::"r"(d), "r"(ta), "l"(db), "r"(idesc), "r"(acc) : "memory");
+}
 __device__ __forceinline__ uint4 lds128(uint32_t a) {
   uint4 v;
   asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
@@ -209,18 +227,21 @@ struct Shared {
   float mref[16];
 };
 
-// V scale bytes of this warp's page -> fp16 power-of-two multipliers (one f16x2 per token pair
-// and group) in the warp's scratch; returns the largest scale byte among the page's valid tokens
-// (warp-uniform).  rest = the page's [V codes | K scales | V scales] block in the stage.
+// This warp's share of the tile's V: channel group g (= its TMEM lane quarter), tokens
+// 64*hf .. 64*hf+63 (pages 4*hf .. 4*hf+3 of the tile).  rest0 = [V codes | K scales | V scales]
+// block of page 4*hf in the stage.
+// Step 1: the 64 scale bytes -> 32 fp16 power-of-two multipliers (one f16x2 per token pair) in the
+// warp's scratch; returns the largest scale byte among the valid tokens (warp-uniform).
 template <bool kPartial>
-__device__ __forceinline__ int v_multipliers(uint32_t rest, uint32_t scratch, int lane, int n_valid, int eref) {
+__device__ __forceinline__ int v_multipliers(uint32_t rest0, uint32_t scratch, int lane, int g, int tok_left, int eref) {
+  const int pl = lane >> 3, hk = (lane >> 2) & 1, bp = lane & 3;     // page, half of the page, token pair
   uint32_t pair;
-  asm volatile("ld.shared.u16 %0, [%1];" : "=r"(pair) : "r"(rest + 1088 + 2 * lane));
+  asm volatile("ld.shared.u16 %0, [%1];" : "=r"(pair) : "r"(rest0 + kRestBytes * pl + 1088 + 32 * hk + 8 * g + 2 * bp));
   int lo = (int)(pair & 0xFFu), hi = (int)(pair >> 8);
-  if (kPartial) {
-    const int tok = 8 * (lane >> 4) + 2 * (lane & 3);
-    if (tok >= n_valid) lo = 0;
-    if (tok + 1 >= n_valid) hi = 0;
+  if (kPartial) {                                    // tok_left = valid tokens from the first token of this warp's range
+    const int tok = 16 * pl + 8 * hk + 2 * bp;
+    if (tok >= tok_left) lo = 0;
+    if (tok + 1 >= tok_left) hi = 0;
   }
   const int vmax = __reduce_max_sync(kFull, max(lo, hi));
   const int kbase = eref - 28;                       // fp16 exponent field = byte - kbase (2^13 at byte = eref)
@@ -230,26 +251,23 @@ __device__ __forceinline__ int v_multipliers(uint32_t rest, uint32_t scratch, in
   return vmax;
 }
 
-// V codes of this warp's page (16 tokens x 128 channels) -> fp16 Vhat^T operand
-// [token-core][d][8 tokens]; v_dst = the page's two token-cores (2 x 2048 B).
-__device__ __forceinline__ void v_convert(uint32_t rest, uint32_t scratch, uint32_t v_dst, int lane) {
+// Step 2: 64 tokens of channel d = 32 g + lane -> fp16 x multiplier -> TMEM (A operand of the PV
+// MMA: lane = channel, column c = tokens 2c, 2c+1).
+__device__ __forceinline__ void v_convert(uint32_t rest0, uint32_t scratch, uint32_t t_dst, int lane, int g) {
+  uint32_t o[32];
 #pragma unroll
-  for (int h = 0; h < 2; ++h) {
-    const uint4 c4 = lds128(rest + 512 * h + 16 * lane);
-    const uint32_t cw[4] = {c4.x, c4.y, c4.z, c4.w};
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {                     // channel d = 32 i + lane, group i
-      const uint4 m4 = lds128(scratch + 64 * h + 16 * i);
-      uint32_t f[4];
-      cvt_e2m1x8(cw[i], f);
-      uint4 o;
-      o.x = hmul2(f[0], m4.x);
-      o.y = hmul2(f[1], m4.y);
-      o.z = hmul2(f[2], m4.z);
-      o.w = hmul2(f[3], m4.w);
-      sts128(v_dst + 2048 * h + (32 * i + lane) * 16, o);
-    }
+  for (int k = 0; k < 8; ++k) {                      // token-core k: page k>>1, half k&1 -> 8 tokens
+    uint32_t cw;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(cw) : "r"(rest0 + kRestBytes * (k >> 1) + 512 * (k & 1) + 128 * g + 4 * lane));
+    const uint4 m4 = lds128(scratch + 16 * k);
+    uint32_t f[4];
+    cvt_e2m1x8(cw, f);
+    o[4 * k + 0] = hmul2(f[0], m4.x);
+    o[4 * k + 1] = hmul2(f[1], m4.y);
+    o[4 * k + 2] = hmul2(f[2], m4.z);
+    o[4 * k + 3] = hmul2(f[3], m4.w);
   }
+  tmem_st32(t_dst, o);
   __syncwarp();
 }
 
@@ -285,8 +303,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
   const int tok_end = min(L, p1 * kPage);
 
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t sQ = base + kOffQ, sSFA = base + kOffSFA, sSFB = base + kOffSFB, sV = base + kOffV,
-                 sP = base + kOffP;
+  const uint32_t sQ = base + kOffQ, sSFA = base + kOffSFA, sSFB = base + kOffSFB, sP = base + kOffP;
   const uint32_t bar_full = smem_u32(&sh.full[0]), bar_empty = smem_u32(&sh.empty[0]),
                  bar_sfull = smem_u32(&sh.s_full[0]), bar_ready = smem_u32(&sh.ready),
                  bar_done = smem_u32(&sh.done);
@@ -393,9 +410,9 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
       if (lane == 0) {
         const uint32_t pbuf = sP + kPBytes * (i & 1);
 #pragma unroll
-        for (int j = 0; j < 8; ++j)                    // 16 tokens per MMA = token-cores 2j, 2j+1
-          umma_f16(tmem + kColO, make_desc(sV + 4096 * j, 2048, 128, 0), make_desc(pbuf + 512 * j, 256, 128, 0),
-                   idesc_pv, (i > 0 || j > 0) ? 1u : 0u);
+        for (int j = 0; j < 8; ++j)                    // 16 tokens per MMA = 8 columns of Vhat^T
+          umma_f16_ts(tmem + kColO, tmem + kColV + 8 * j, make_desc(pbuf + 512 * j, 256, 128, 0), idesc_pv,
+                      (i > 0 || j > 0) ? 1u : 0u);
         umma_commit(bar_done);
       }
       __syncwarp();
@@ -408,7 +425,8 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
     const bool heads_live = (8 * hh < G);
     const uint32_t scratch = base + kOffMul + 128 * warp;
     const uint32_t lane_sel = (uint32_t)(32 * q) << 16;
-    const uint32_t v_dst = sV + warp * 4096;           // this warp converts page `warp` of every tile
+    const int g = q, hf = hh;                          // V conversion: channel group (= lane quarter), token half of the tile
+    const uint32_t t_v = tmem + lane_sel + kColV + 32 * hf;
     float mref[8], lsum[8];
 #pragma unroll
     for (int j = 0; j < 8; ++j) { mref[j] = -INFINITY; lsum[j] = 0.f; }
@@ -416,11 +434,11 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
 
     for (int i = 0; i < n_tiles; ++i) {
       const int s = i % kStages, sb = i & 1;
-      const uint32_t rest = base + kOffStage + s * kStageBytes + 16384 + kRestBytes * warp;
+      const uint32_t rest0 = base + kOffStage + s * kStageBytes + 16384 + kRestBytes * (4 * hf);
       const int pg0 = p0 + kTilePages * i;                           // first page of the tile
       const bool tile_partial = (pg0 + kTilePages) * kPage > tok_end;
       const bool tok_ok = pg0 * kPage + r < tok_end;
-      const int n_valid = tile_partial ? (pg0 + warp < p1 ? min(kPage, L - kPage * (pg0 + warp)) : 0) : kPage;
+      const int tok_left = tok_end - (pg0 * kPage + 64 * hf);      // valid tokens in this warp's 64-token half
       const uint32_t t_s = tmem + lane_sel + kColS + 16 * sb + 8 * hh;
       const uint32_t p_addr = sP + kPBytes * sb + (r >> 3) * 256 + hh * 128 + (r & 7) * 16;
 
@@ -458,14 +476,14 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
       int vmax = 0;
       if (!rebase) {
         const bool ex = softmax_pass();
-        vmax = tile_partial ? v_multipliers<true>(rest, scratch, lane, n_valid, eref)
-                            : v_multipliers<false>(rest, scratch, lane, n_valid, eref);
+        vmax = tile_partial ? v_multipliers<true>(rest0, scratch, lane, g, tok_left, eref)
+                            : v_multipliers<false>(rest0, scratch, lane, g, tok_left, eref);
         tc_fence_before();
         rebase = bar_compute_or(ex || vmax > eref);
       }
       if (rebase) {
         // ---- statistics of the tile: per-head maximum score, maximum V scale byte
-        vmax = v_multipliers<true>(rest, scratch, lane, n_valid, eref);
+        vmax = v_multipliers<true>(rest0, scratch, lane, g, tok_left, eref);
         float tm[8];
 #pragma unroll
         for (int j = 0; j < 8; ++j) tm[j] = -INFINITY;
@@ -516,21 +534,18 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
           tmem_st8(t_o, ov);
         }
         (void)softmax_pass();
-        (void)v_multipliers<true>(rest, scratch, lane, n_valid, eref);
+        (void)v_multipliers<true>(rest0, scratch, lane, g, tok_left, eref);
         bar_compute();                                  // wmax / wvmax may be rewritten only after every warp read them
       }
 #pragma unroll
       for (int j = 0; j < 8; ++j) lsum[j] += lt[j];
 
-      // ---- V codes of page `warp` -> Vhat^T (the PV MMAs of the previous tile ran under the softmax above)
-      if (i > 0) mbar_wait(bar_done, (i - 1) & 1);
-      if (n_valid > 0) {
-        v_convert(rest, scratch, v_dst, lane);
-      } else {
-        const uint4 z = make_uint4(0u, 0u, 0u, 0u);
-#pragma unroll
-        for (int k = 0; k < 8; ++k) sts128(v_dst + 512 * k + 16 * lane, z);
+      // ---- V codes -> Vhat^T in TMEM (the PV MMAs of the previous tile ran under the softmax above)
+      if (i > 0) {
+        mbar_wait(bar_done, (i - 1) & 1);
+        tc_fence_after();
       }
+      v_convert(rest0, scratch, t_v, lane, g);
       fence_async_smem();
       tc_fence_before();
       __syncwarp();

@@ -23,7 +23,7 @@ def _v_code_index():
     sh = np.zeros((PAGE, 128), np.int64)
     for t in range(PAGE):
         for d in range(128):
-            word = 1024 + 512 * (t >> 3) + 16 * (d & 31) + 4 * (d >> 5)
+            word = 1024 + 512 * (t >> 3) + 128 * (d >> 5) + 4 * (d & 31)
             bit = 4 * (t & 7)                      # token t in bits 4(t&7)..4(t&7)+3 of the word
             idx[t, d] = word + bit // 8            # little-endian byte of the word
             sh[t, d] = bit % 8
