@@ -4,16 +4,19 @@
 //
 // Design: one CTA per (sequence, kv head, split); the split is walked in
 // tiles of 128 tokens (8 pages).  Warp roles (320 threads):
-//   warp 8  producer: per page one TMA tensor copy of the packed FP4 K codes
+//   producer: per page one TMA tensor copy of the packed FP4 K codes
 //           (CU_TENSOR_MAP_DATA_TYPE_16U4_ALIGN16B + SWIZZLE_128B: the TMA unit expands the
 //           nibbles into the 8-bit containers tcgen05 reads) and one cp.async.bulk of the rest of
-//           the record (V codes, K scales, V scales), through a ring of mbarrier stages;
-//   warp 9  MMA issuer: S[128 tok x 16 heads] = K . Q^T with
+//           the record (V codes, K scales, V scales), into a ring of mbarrier stages; compute warp
+//           w issues the copies of page w of every tile (an async-copy instruction occupies its
+//           issuing warp for ~55 cycles, so a single producer warp would cap the stream);
+//   warp 0  QK issuer: S[128 tok x 16 heads] = K . Q^T with
 //           tcgen05.mma.kind::mxf8f6f4.block_scale — E2M1 keys x E4M3 queries with the UE8M0 group
 //           scales applied by the tensor core (the paper's FP8xFP4 scaled MMA), K
-//           scales staged smem -> TMEM with tcgen05.cp; then O^T[128 d x 16 heads] += Vhat^T . P^T
+//           scales staged smem -> TMEM with tcgen05.cp;
+//   warp 1  PV issuer: O^T[128 d x 16 heads] += Vhat^T . P^T
 //           with tcgen05.mma.kind::f16 (A = Vhat^T from TMEM, B = P from smem); accumulators in TMEM;
-//   warps 0-7 compute: S rows from TMEM (tcgen05.ld), base-2 softmax against a LAZY per-head
+//   warps 2-9 compute: S rows from TMEM (tcgen05.ld), base-2 softmax against a LAZY per-head
 //           reference (a "rebase" — new reference, O rescaled in TMEM, tile's P redone — happens on
 //           the first tile and whenever a score exceeds the reference by 2^12 or a V scale exceeds
 //           the reference exponent), P -> fp16 operand in smem (double-buffered); then V codes ->
@@ -64,8 +67,8 @@ constexpr uint32_t kColS = 0;      // 2 x 16
 constexpr uint32_t kColO = 32;     // 16
 constexpr uint32_t kColSFA = 48;   // 2 x 4
 constexpr uint32_t kColSFB = 56;   // 4
-constexpr uint32_t kColV = 64;     // 64: Vhat^T operand, lane = channel d, column c = tokens 2c, 2c+1 (f16x2)
-constexpr uint32_t kTmemCols = 128;
+constexpr uint32_t kColV = 64;     // 2 x 64: Vhat^T operand, lane = channel d, column c = tokens 2c, 2c+1 (f16x2)
+constexpr uint32_t kTmemCols = 256;
 
 // ---------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -80,7 +83,24 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+// A thread suspended in a plain mbarrier.try_wait was observed (clock64 trace) to sleep ~2.5k cycles
+// past a tcgen05.commit arrival before it resumed, and a pure test_wait spin steals issue slots from
+// the working warps; so waits use try_wait with a short suspend-time hint.
+#ifndef UQ_WAIT_NS
+#define UQ_WAIT_NS -1
+#endif
+__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {   // one non-blocking probe
+  uint32_t ok;
+  asm volatile("{\n.reg .pred p;\nmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
+               : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+  return ok != 0;
+}
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+#if UQ_WAIT_NS > 0
+  while (!mbar_test(bar, parity)) asm volatile("nanosleep.u32 %0;" ::"r"((uint32_t)UQ_WAIT_NS));
+#elif UQ_WAIT_NS == 0
+  while (!mbar_test(bar, parity)) {}
+#else
   asm volatile(
       "{\n"
       ".reg .pred p;\n"
@@ -90,20 +110,35 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "bra WAIT_%=;\n"
       "DONE_%=:\n"
       "}\n" ::"r"(bar), "r"(parity) : "memory");
+#endif
 }
-__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {   // one non-blocking probe
-  uint32_t ok;
-  asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
-               : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-  return ok != 0;
+#ifndef UQ_SPIN_NS
+#define UQ_SPIN_NS 32
+#endif
+__device__ __forceinline__ void spin_pause() {
+#if UQ_SPIN_NS > 0
+  asm volatile("nanosleep.u32 %0;" ::"r"((uint32_t)UQ_SPIN_NS));
+#endif
 }
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+__device__ __forceinline__ void mbar_wait_spin(uint32_t bar, uint32_t parity) {   // for the single-warp issuers
+  while (!mbar_test(bar, parity)) spin_pause();
 }
-__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, int c2, uint32_t bar) {
-  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-               ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
+// The KV stream is read once: L2 evict-first keeps it from flushing everything else (the kernel's own
+// instructions included) out of L2.
+__device__ __forceinline__ uint64_t l2_evict_first_policy() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint64_t pol) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, int c2, uint32_t bar,
+                                            uint64_t pol) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
+               " [%0], [%1, {%2, %3, %4}], [%5], %6;"
+               ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "l"(pol) : "memory");
 }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -213,13 +248,21 @@ __device__ __forceinline__ float pow2i(int e) {   // 2^e, flushing to 0 below th
   return f > 0 ? __uint_as_float((uint32_t)min(f, 254) << 23) : 0.f;
 }
 
+#ifdef UQ_TRACE   // debug builds only: clock timeline of one CTA, buffered in smem (see uq_debug_trace below)
+__device__ long long g_trace[10][4096];
+__device__ int g_trace_n[10];
+#define TRACE(role, tag, tile) do { if (trace_on && lane == 0 && tr_n < 160) { tr_buf[role][tr_n] = make_uint2(((uint32_t)(tag) << 16) | (uint32_t)(tile), (uint32_t)clock64()); ++tr_n; } } while (0)
+#else
+#define TRACE(role, tag, tile) do {} while (0)
+#endif
+
 // ---------------------------------------------------------------- per-CTA shared bookkeeping
 struct Shared {
-  uint64_t full[kStages];     // producer -> consumers: stage landed (tx bytes)
-  uint64_t empty[kStages];    // 8 compute warps + QK commit -> producer
+  uint64_t full[kStages];     // 8 compute warps (expect_tx, one page each) + TMA bytes -> QK warp, compute warps
   uint64_t s_full[2];         // QK commit -> compute warps
-  uint64_t ready;             // 8 compute warps -> MMA warp: P and Vhat of the tile are in smem
-  uint64_t done;              // PV commit -> compute warps (Vhat free, O up to date)
+  uint64_t s_free[2];         // 8 compute warps -> QK warp: S buffer read, may be overwritten
+  uint64_t ready;             // 8 compute warps -> PV warp: P (smem) and Vhat (TMEM) of the tile are written
+  uint64_t done[2];           // PV commit of tile i -> done[i&1]: P / Vhat buffer i&1 free, O up to date
   uint32_t tmem_base;
   float wmax[kComputeWarps][8];
   int wvmax[kComputeWarps];
@@ -284,6 +327,11 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
   const int split = blockIdx.x, kvh = blockIdx.y, b = blockIdx.z;
   const int G = Hq / Hkv;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+#ifdef UQ_TRACE
+  const bool trace_on = (split == 2 && kvh == 1 && b == 7);
+  __shared__ uint2 tr_buf[10][160];
+  int tr_n = 0;
+#endif
 
   const int L = seq_lens[b];
   const int n_pages = (L + kPage - 1) / kPage;
@@ -304,24 +352,26 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
 
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = base + kOffQ, sSFA = base + kOffSFA, sSFB = base + kOffSFB, sP = base + kOffP;
-  const uint32_t bar_full = smem_u32(&sh.full[0]), bar_empty = smem_u32(&sh.empty[0]),
-                 bar_sfull = smem_u32(&sh.s_full[0]), bar_ready = smem_u32(&sh.ready),
-                 bar_done = smem_u32(&sh.done);
+  const uint32_t bar_full = smem_u32(&sh.full[0]),
+                 bar_sfull = smem_u32(&sh.s_full[0]), bar_sfree = smem_u32(&sh.s_free[0]),
+                 bar_ready = smem_u32(&sh.ready), bar_done = smem_u32(&sh.done[0]);
 
   // ---------------- setup
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < kStages; ++s) {
-      mbar_init(bar_full + 8 * s, 1);
-      mbar_init(bar_empty + 8 * s, kComputeWarps + 1);
+      mbar_init(bar_full + 8 * s, kComputeWarps);
     }
-    mbar_init(bar_sfull, 1);
-    mbar_init(bar_sfull + 8, 1);
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      mbar_init(bar_sfull + 8 * h, 1);
+      mbar_init(bar_sfree + 8 * h, kComputeWarps);
+      mbar_init(bar_done + 8 * h, 1);
+    }
     mbar_init(bar_ready, kComputeWarps);
-    mbar_init(bar_done, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == kComputeWarps + 1) {
+  if (warp == 1) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&sh.tmem_base)),
                  "r"(kTmemCols));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
@@ -340,37 +390,18 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
   tc_fence_after();
   const uint32_t tmem = sh.tmem_base;
 
-  if (warp == kComputeWarps) {
-    // ================================================================ producer warp
-    const int32_t* bt = block_tables + (long long)b * max_pages;
-    int page_next = (lane < kTilePages && p0 + lane < p1) ? bt[p0 + lane] : 0;
-    for (int i = 0; i < n_tiles; ++i) {
-      const int s = i % kStages;
-      const int page = page_next;
-      const int npg = min(kTilePages, p1 - (p0 + kTilePages * i));
-      const int nb = p0 + kTilePages * (i + 1) + lane;
-      page_next = (lane < kTilePages && nb < p1) ? bt[nb] : 0;
-      mbar_wait(bar_empty + 8 * s, ((i / kStages) & 1) ^ 1);
-      if (lane == 0) mbar_expect_tx(bar_full + 8 * s, (uint32_t)npg * kRecordBytes);
-      __syncwarp();
-      if (lane < npg) {
-        const long long rec = (long long)page * Hkv + kvh;
-        const uint32_t st = base + kOffStage + s * kStageBytes;
-        tma_load_3d(st + 2048 * lane, &tmap, 0, 0, (int)rec, bar_full + 8 * s);
-        bulk_g2s(st + 16384 + kRestBytes * lane, cache + rec * kRecordBytes + 1024, kRestBytes, bar_full + 8 * s);
-      }
-    }
-  } else if (warp == kComputeWarps + 1) {
-    // ================================================================ MMA warp
+  if (warp == 0) {
+    // ================================================================ QK warp
+    // S(i)[128 tok x 16 heads] = K(i) . Q^T as soon as the tile's bytes have landed and the S buffer
+    // (read by the softmax of tile i-2) is free.
+    const uint32_t idesc_qk = (5u << 7) | (0u << 10) | (2u << 17) | (1u << 23) | (8u << 24);   // E2M1 x E4M3, UE8M0, N=16, M=128
     if (lane == 0) umma_cp_sf(tmem + kColSFB, make_desc(sSFB, 16, 128, 0));
-    // E2M1 (5) x E4M3 (0), UE8M0 scales, N = 16, M = 128
-    const uint32_t idesc_qk = (5u << 7) | (0u << 10) | (2u << 17) | (1u << 23) | (8u << 24);
-    // f16 x f16 -> f32, B (= P) MN-major, N = 16, M = 128
-    const uint32_t idesc_pv = (1u << 4) | (1u << 16) | (2u << 17) | (8u << 24);
-    auto issue_qk = [&](int i) {
+    for (int i = 0; i < n_tiles; ++i) {
       const int s = i % kStages, sb = i & 1;
-      const uint32_t st = base + kOffStage + s * kStageBytes;
+      if (i >= 2) mbar_wait(bar_sfree + 8 * sb, ((i >> 1) - 1) & 1);
       mbar_wait(bar_full + 8 * s, (i / kStages) & 1);
+      TRACE(0, 3, i);
+      const uint32_t st = base + kOffStage + s * kStageBytes;
       // scale-factor atom: row r = 32 c + lane of the tile -> 16-byte line `lane`, word c
       uint32_t v[4];
 #pragma unroll
@@ -390,40 +421,38 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
           umma_mxf8f6f4(tmem + kColS + 16 * sb, make_desc(st + 32 * kb, 16, 1024, 2), make_desc(sQ + 32 * kb, 16, 1024, 2),
                         idesc_qk | ((uint32_t)kb << 29), kb > 0, t_sfa + ((uint32_t)kb << 30), tmem + kColSFB);
         umma_commit(bar_sfull + 8 * sb);
-        umma_commit(bar_empty + 8 * s);
       }
       __syncwarp();
-    };
-    issue_qk(0);
+      TRACE(0, 4, i);
+    }
+  } else if (warp == 1) {
+    // ================================================================ PV warp
+    // O^T[128 d x 16 heads] += Vhat^T (TMEM, buffer i&1) . P^T (smem, buffer i&1); f16 x f16 -> f32, B MN-major
+    const uint32_t idesc_pv = (1u << 4) | (1u << 16) | (2u << 17) | (8u << 24);
     for (int i = 0; i < n_tiles; ++i) {
-      // QK of the next tile goes first if its bytes have landed; PV of this tile as soon as it is ready
-      bool qk_done = (i + 1 >= n_tiles);
-      for (;;) {
-        if (!qk_done && __any_sync(kFull, mbar_test(bar_full + 8 * ((i + 1) % kStages), ((i + 1) / kStages) & 1))) {
-          issue_qk(i + 1);
-          qk_done = true;
-        }
-        if (__any_sync(kFull, mbar_test(bar_ready, i & 1))) break;
-      }
       mbar_wait(bar_ready, i & 1);
+      TRACE(1, 3, i);
       tc_fence_after();
       if (lane == 0) {
-        const uint32_t pbuf = sP + kPBytes * (i & 1);
+        const uint32_t pbuf = sP + kPBytes * (i & 1), vbuf = tmem + kColV + 64 * (i & 1);
 #pragma unroll
         for (int j = 0; j < 8; ++j)                    // 16 tokens per MMA = 8 columns of Vhat^T
-          umma_f16_ts(tmem + kColO, tmem + kColV + 8 * j, make_desc(pbuf + 512 * j, 256, 128, 0), idesc_pv,
+          umma_f16_ts(tmem + kColO, vbuf + 8 * j, make_desc(pbuf + 512 * j, 256, 128, 0), idesc_pv,
                       (i > 0 || j > 0) ? 1u : 0u);
-        umma_commit(bar_done);
+        umma_commit(bar_done + 8 * (i & 1));
       }
       __syncwarp();
-      if (!qk_done) issue_qk(i + 1);
+      TRACE(1, 4, i);
     }
   } else {
-    // ================================================================ compute warps 0..7
-    const int q = warp & 3, hh = warp >> 2;            // TMEM lane quarter, head half
+    // ================================================================ compute warps (warp ids 2..9)
+    // The two issuer warps poll mbarriers; they sit on the lowest warp ids so that the scheduler's
+    // highest-warp-id-first arbitration favours the compute warps.
+    const int cw = warp - 2;                           // 0..7
+    const int q = warp & 3, hh = cw >> 2;              // TMEM lane quarter (hardware: warp id % 4), head half
     const int r = 32 * q + lane;                       // softmax: token row of the tile; epilogue: channel d
     const bool heads_live = (8 * hh < G);
-    const uint32_t scratch = base + kOffMul + 128 * warp;
+    const uint32_t scratch = base + kOffMul + 128 * cw;
     const uint32_t lane_sel = (uint32_t)(32 * q) << 16;
     const int g = q, hf = hh;                          // V conversion: channel group (= lane quarter), token half of the tile
     const uint32_t t_v = tmem + lane_sel + kColV + 32 * hf;
@@ -431,6 +460,31 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
 #pragma unroll
     for (int j = 0; j < 8; ++j) { mref[j] = -INFINITY; lsum[j] = 0.f; }
     int eref = 28;
+
+    // Every compute warp is the TMA producer of page `cw` of each tile (an async-copy instruction
+    // costs its issuing warp ~55 cycles, so the 16 copies of a tile are spread over the 8 warps).
+    const int32_t* bt = block_tables + (long long)b * max_pages;
+    const uint64_t pol = l2_evict_first_policy();
+    auto bt_entry = [&](int tile) -> int {             // physical page of this warp's page of `tile` (lane 0)
+      const int pg = p0 + kTilePages * tile + cw;
+      return (lane == 0 && tile < n_tiles && pg < p1) ? bt[pg] : -1;
+    };
+    auto load_page = [&](int tile, int page) {         // lane 0: arrive on full[stage] and start the two copies
+      if (lane == 0 && tile < n_tiles) {
+        const int s = tile % kStages;
+        if (page >= 0) {
+          const long long rec = (long long)page * Hkv + kvh;
+          const uint32_t st = base + kOffStage + s * kStageBytes;
+          mbar_expect_tx(bar_full + 8 * s, kRecordBytes);
+          tma_load_3d(st + 2048 * cw, &tmap, 0, 0, (int)rec, bar_full + 8 * s, pol);
+          bulk_g2s(st + 16384 + kRestBytes * cw, cache + rec * kRecordBytes + 1024, kRestBytes, bar_full + 8 * s, pol);
+        } else {
+          mbar_arrive(bar_full + 8 * s);               // page beyond the split: nothing to load
+        }
+      }
+    };
+#pragma unroll
+    for (int t = 0; t < kStages; ++t) load_page(t, bt_entry(t));
 
     for (int i = 0; i < n_tiles; ++i) {
       const int s = i % kStages, sb = i & 1;
@@ -442,9 +496,16 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
       const uint32_t t_s = tmem + lane_sel + kColS + 16 * sb + 8 * hh;
       const uint32_t p_addr = sP + kPBytes * sb + (r >> 3) * 256 + hh * 128 + (r & 7) * 16;
 
+      TRACE(2 + cw, 1, i);
+      const int page_ahead = bt_entry(i + kStages - 1);              // for the refill below (latency hidden by the softmax)
       mbar_wait(bar_sfull + 8 * sb, (i >> 1) & 1);                   // S of the tile is in TMEM
+      TRACE(2 + cw, 2, i);
       tc_fence_after();
       mbar_wait(bar_full + 8 * s, (i / kStages) & 1);                // (already complete) acquire the TMA bytes
+      if (i >= 2) {                                                  // P / Vhat buffers i&1 were read by PV(i-2)
+        mbar_wait(bar_done + 8 * sb, ((i - 2) >> 1) & 1);
+        tc_fence_after();
+      }
 
       float lt[8];
       // softmax of this thread's row against the current references -> P (fp16, MN-major operand)
@@ -479,9 +540,11 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
         vmax = tile_partial ? v_multipliers<true>(rest0, scratch, lane, g, tok_left, eref)
                             : v_multipliers<false>(rest0, scratch, lane, g, tok_left, eref);
         tc_fence_before();
+        TRACE(2 + cw, 3, i);
         rebase = bar_compute_or(ex || vmax > eref);
+        TRACE(2 + cw, 4, i);
       }
-      if (rebase) {
+      if (__builtin_expect(rebase, 0)) {
         // ---- statistics of the tile: per-head maximum score, maximum V scale byte
         vmax = v_multipliers<true>(rest0, scratch, lane, g, tok_left, eref);
         float tm[8];
@@ -500,8 +563,8 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
         }
         if (lane == 0) {
 #pragma unroll
-          for (int j = 0; j < 8; ++j) sh.wmax[warp][j] = tm[j];
-          sh.wvmax[warp] = vmax;
+          for (int j = 0; j < 8; ++j) sh.wmax[cw][j] = tm[j];
+          sh.wvmax[cw] = vmax;
         }
         tc_fence_before();
         bar_compute();
@@ -524,7 +587,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
         }
         eref = enew;
         if (i > 0) {  // every PV issued so far has to be in O before it is rescaled
-          mbar_wait(bar_done, (i - 1) & 1);
+          mbar_wait(bar_done + 8 * ((i - 1) & 1), ((i - 1) >> 1) & 1);
           tc_fence_after();
           float ov[8];
           const uint32_t t_o = tmem + lane_sel + kColO + 8 * hh;   // channel r, heads 8hh..8hh+7
@@ -540,23 +603,27 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
 #pragma unroll
       for (int j = 0; j < 8; ++j) lsum[j] += lt[j];
 
-      // ---- V codes -> Vhat^T in TMEM (the PV MMAs of the previous tile ran under the softmax above)
-      if (i > 0) {
-        mbar_wait(bar_done, (i - 1) & 1);
-        tc_fence_after();
-      }
-      v_convert(rest0, scratch, t_v, lane, g);
+      // ---- every compute warp is past the barrier above, so all of them finished tile i-1 and QK(i-1)
+      //      completed: the stage of tile i-1 is free -> refill it with tile i-1+kStages
+      if (i >= 1) load_page(i + kStages - 1, page_ahead);
+
+      // ---- S has been read: the QK warp may overwrite this S buffer (tile i+2)
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar_sfree + 8 * sb);
+
+      // ---- V codes -> Vhat^T in TMEM buffer i&1
+      TRACE(2 + cw, 5, i);
+      v_convert(rest0, scratch, t_v + 64 * sb, lane, g);
+      TRACE(2 + cw, 6, i);
       fence_async_smem();
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) {
-        mbar_arrive(bar_ready);
-        mbar_arrive(bar_empty + 8 * s);
-      }
+      if (lane == 0) mbar_arrive(bar_ready);
     }
 
     // ================================================================ epilogue: write the split's partial
-    mbar_wait(bar_done, (n_tiles - 1) & 1);
+    mbar_wait(bar_done + 8 * ((n_tiles - 1) & 1), ((n_tiles - 1) >> 1) & 1);
     tc_fence_after();
     {
       float ov[8];
@@ -578,25 +645,34 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
     if (lane == 0) {
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
-        sh.lsum[warp][j] = lsum[j];
+        sh.lsum[cw][j] = lsum[j];
         if (q == 0) sh.mref[8 * hh + j] = mref[j];
       }
     }
     bar_compute();
-    if (tid < G) {
-      const int h2 = tid >> 3, j = tid & 7;
+    const int head = tid - 64;                         // first compute threads: one per query head
+    if (head < G) {
+      const int h2 = head >> 3, j = head & 7;
       float l = 0.f;
 #pragma unroll
       for (int w = 0; w < 4; ++w) l += sh.lsum[4 * h2 + w][j];
-      float2* ml = reinterpret_cast<float2*>(partial_ml) + row0 + (long long)tid * num_splits;
-      *ml = make_float2(sh.mref[tid] * 0.6931471805599453f, l);  // natural-log units
+      float2* ml = reinterpret_cast<float2*>(partial_ml) + row0 + (long long)head * num_splits;
+      *ml = make_float2(sh.mref[head] * 0.6931471805599453f, l);  // natural-log units
     }
   }
 
   // ---------------- teardown
+#ifdef UQ_TRACE
+  if (trace_on && lane == 0) {
+    const int role = warp;
+    for (int k = 0; k < tr_n; ++k)
+      g_trace[role][k] = ((long long)(tr_buf[role][k].x >> 16) << 56) | ((long long)(tr_buf[role][k].x & 0xFFFF) << 40) | tr_buf[role][k].y;
+    g_trace_n[role] = tr_n;
+  }
+#endif
   tc_fence_before();
   __syncthreads();
-  if (warp == kComputeWarps + 1) {
+  if (warp == 1) {
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTmemCols));
   }
 }
@@ -658,6 +734,17 @@ int32_t k_code_map(const void* cache, long long records, CUtensorMap* out) {
 
 }  // namespace
 }  // namespace uq
+
+#ifdef UQ_TRACE
+extern "C" int32_t uq_debug_trace(long long* out /* host [10][4096] */, int* n /* host [10] */) {
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(out, uq::g_trace, sizeof(long long) * 10 * 4096);
+  cudaMemcpyFromSymbol(n, uq::g_trace_n, sizeof(int) * 10);
+  int z[10] = {0};
+  cudaMemcpyToSymbol(uq::g_trace_n, z, sizeof(z));
+  return 0;
+}
+#endif
 
 extern "C" int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, const void* cache,
                                        int64_t num_pages, const int32_t* block_tables, int32_t max_pages,
