@@ -36,8 +36,8 @@
 namespace uq {
 namespace {
 
-constexpr int kComputeWarps = 8;
-constexpr int kThreads = (kComputeWarps + 2) * 32;   // + producer warp + MMA warp
+constexpr int kComputeWarps = 8;                     // two per TMEM lane quarter
+constexpr int kThreads = (kComputeWarps + 2) * 32;   // + QK issuer warp + PV issuer warp
 #ifndef UQ_STAGES
 #define UQ_STAGES 3
 #endif
@@ -67,8 +67,12 @@ constexpr uint32_t kColS = 0;      // 2 x 16
 constexpr uint32_t kColO = 32;     // 16
 constexpr uint32_t kColSFA = 48;   // 2 x 4
 constexpr uint32_t kColSFB = 56;   // 4
-constexpr uint32_t kColV = 64;     // 2 x 64: Vhat^T operand, lane = channel d, column c = tokens 2c, 2c+1 (f16x2)
-constexpr uint32_t kTmemCols = 256;
+#ifndef UQ_VBUFS
+#define UQ_VBUFS 2
+#endif
+constexpr int kVBufs = UQ_VBUFS;   // Vhat^T buffers in TMEM
+constexpr uint32_t kColV = 64;     // kVBufs x 64: Vhat^T operand, lane = channel d, column c = tokens 2c, 2c+1 (f16x2)
+constexpr uint32_t kTmemCols = kVBufs == 1 ? 128 : 256;
 
 // ---------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -360,7 +364,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < kStages; ++s) {
-      mbar_init(bar_full + 8 * s, kComputeWarps);
+      mbar_init(bar_full + 8 * s, kTilePages);        // one arrival per page (its loader lane)
     }
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
@@ -381,8 +385,9 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
     uint4 v = make_uint4(0u, 0u, 0u, 0u);
     if (n < G) v = *reinterpret_cast<const uint4*>(q_fp8 + ((long long)b * Hq + (long long)kvh * G + n) * kHeadDim + 16 * c);
     sts128(sQ + n * 128 + ((c ^ (n & 7)) << 4), v);
-  } else if (tid < 256) {  // query-side scale factors: UE8M0 byte 127 = 2^0
-    asm volatile("st.shared.u32 [%0], %1;" ::"r"(sSFB + 4 * (tid - 128)), "r"(0x7F7F7F7Fu) : "memory");
+  }
+  if (tid < 128) {  // query-side scale factors: UE8M0 byte 127 = 2^0
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(sSFB + 4 * tid), "r"(0x7F7F7F7Fu) : "memory");
   }
   fence_async_smem();
   tc_fence_before();
@@ -434,7 +439,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
       TRACE(1, 3, i);
       tc_fence_after();
       if (lane == 0) {
-        const uint32_t pbuf = sP + kPBytes * (i & 1), vbuf = tmem + kColV + 64 * (i & 1);
+        const uint32_t pbuf = sP + kPBytes * (i & 1), vbuf = tmem + kColV + 64 * ((i & 1) % kVBufs);
 #pragma unroll
         for (int j = 0; j < 8; ++j)                    // 16 tokens per MMA = 8 columns of Vhat^T
           umma_f16_ts(tmem + kColO, vbuf + 8 * j, make_desc(pbuf + 512 * j, 256, 128, 0), idesc_pv,
@@ -463,31 +468,32 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
 
     // Every compute warp is the TMA producer of page `cw` of each tile (an async-copy instruction
     // costs its issuing warp ~55 cycles, so the 16 copies of a tile are spread over the 8 warps).
-    const int32_t* bt = block_tables + (long long)b * max_pages;
     const uint64_t pol = l2_evict_first_policy();
+    const int32_t* bt_mine = block_tables + (long long)b * max_pages + p0 + cw;
+    const uint8_t* cache_kvh = cache + (long long)kvh * kRecordBytes;
+    const long long page_stride = (long long)Hkv * kRecordBytes;
     auto bt_entry = [&](int tile) -> int {             // physical page of this warp's page of `tile` (lane 0)
-      const int pg = p0 + kTilePages * tile + cw;
-      return (lane == 0 && tile < n_tiles && pg < p1) ? bt[pg] : -1;
+      return (lane == 0 && tile < n_tiles && p0 + kTilePages * tile + cw < p1) ? bt_mine[kTilePages * tile] : -1;
     };
-    auto load_page = [&](int tile, int page) {         // lane 0: arrive on full[stage] and start the two copies
+    auto load_page = [&](int tile, int page, int s) {  // lane 0: arrive on full[s] and start the two copies
       if (lane == 0 && tile < n_tiles) {
-        const int s = tile % kStages;
         if (page >= 0) {
-          const long long rec = (long long)page * Hkv + kvh;
           const uint32_t st = base + kOffStage + s * kStageBytes;
           mbar_expect_tx(bar_full + 8 * s, kRecordBytes);
-          tma_load_3d(st + 2048 * cw, &tmap, 0, 0, (int)rec, bar_full + 8 * s, pol);
-          bulk_g2s(st + 16384 + kRestBytes * cw, cache + rec * kRecordBytes + 1024, kRestBytes, bar_full + 8 * s, pol);
+          tma_load_3d(st + 2048 * cw, &tmap, 0, 0, page * Hkv + kvh, bar_full + 8 * s, pol);
+          bulk_g2s(st + 16384 + kRestBytes * cw, cache_kvh + page * page_stride + 1024, kRestBytes, bar_full + 8 * s, pol);
         } else {
           mbar_arrive(bar_full + 8 * s);               // page beyond the split: nothing to load
         }
       }
     };
 #pragma unroll
-    for (int t = 0; t < kStages; ++t) load_page(t, bt_entry(t));
+    for (int t = 0; t < kStages; ++t) load_page(t, bt_entry(t), t);
 
+    int s = 0, ph_full = 0;                            // stage of tile i, parity of i / kStages
+    int s_prev = kStages - 1;                          // stage of tile i-1 (refilled with tile i-1+kStages)
     for (int i = 0; i < n_tiles; ++i) {
-      const int s = i % kStages, sb = i & 1;
+      const int sb = i & 1, ph2 = (i >> 1) & 1;
       const uint32_t rest0 = base + kOffStage + s * kStageBytes + 16384 + kRestBytes * (4 * hf);
       const int pg0 = p0 + kTilePages * i;                           // first page of the tile
       const bool tile_partial = (pg0 + kTilePages) * kPage > tok_end;
@@ -498,12 +504,12 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
 
       TRACE(2 + cw, 1, i);
       const int page_ahead = bt_entry(i + kStages - 1);              // for the refill below (latency hidden by the softmax)
-      mbar_wait(bar_sfull + 8 * sb, (i >> 1) & 1);                   // S of the tile is in TMEM
+      mbar_wait(bar_sfull + 8 * sb, ph2);                            // S of the tile is in TMEM
       TRACE(2 + cw, 2, i);
       tc_fence_after();
-      mbar_wait(bar_full + 8 * s, (i / kStages) & 1);                // (already complete) acquire the TMA bytes
+      mbar_wait(bar_full + 8 * s, ph_full);                          // (already complete) acquire the TMA bytes
       if (i >= 2) {                                                  // P / Vhat buffers i&1 were read by PV(i-2)
-        mbar_wait(bar_done + 8 * sb, ((i - 2) >> 1) & 1);
+        mbar_wait(bar_done + 8 * sb, ph2 ^ 1);
         tc_fence_after();
       }
 
@@ -605,7 +611,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
 
       // ---- every compute warp is past the barrier above, so all of them finished tile i-1 and QK(i-1)
       //      completed: the stage of tile i-1 is free -> refill it with tile i-1+kStages
-      if (i >= 1) load_page(i + kStages - 1, page_ahead);
+      if (i >= 1) load_page(i + kStages - 1, page_ahead, s_prev);
 
       // ---- S has been read: the QK warp may overwrite this S buffer (tile i+2)
       tc_fence_before();
@@ -620,6 +626,9 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(bar_ready);
+
+      s_prev = s;
+      if (++s == kStages) { s = 0; ph_full ^= 1; }
     }
 
     // ================================================================ epilogue: write the split's partial
