@@ -46,7 +46,7 @@ FALLBACK_HBM_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md fallbac
 
 # dram__bytes_read.sum + dram__bytes_write.sum per decode_kernel launch from the committed
 # `ncu --set full` capture of this command (profiles/), keyed by config; None = not captured.
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {2: 570_994_688 + 7_573_248}   # profiles/r01_v7_decode_cfg2.md
 
 
 # ----------------------------------------------------------------------------- helpers
@@ -87,10 +87,24 @@ def step_bytes(wl, num_splits: int, ctx_after: np.ndarray, new_per_seq: int):
     return decode + merge + append, decode
 
 
+def max_over_ranks(values, world: int, device="cpu"):
+    """MAX over ranks of a list of per-rank timings (the contract's "max over ranks"); the data path
+    itself has no collective.  Works with any initialised backend (NCCL on GPUs, gloo in the CPU test)."""
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if world > 1:
+        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+    return [float(x) for x in t.cpu()]
+
+
+def whole_job_value(bytes_per_rank: int, world: int, ms_per_step: float) -> float:
+    """Aggregate GB/s of `world` replicas that each move bytes_per_rank per step (weak scaling)."""
+    return world * bytes_per_rank / (ms_per_step * 1e-3) / 1e9
+
+
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML while the timed regions run."""
 
-    def __init__(self, index: int, period_s: float = 0.02):
+    def __init__(self, index: int, period_s: float = 0.005):
         super().__init__(daemon=True)
         self.period = period_s
         self.samples = []            # (busy flag, sm_mhz, reasons bitmask)
@@ -276,13 +290,10 @@ def run_ours(args, rank, world, local_rank):
 
     # ---- reduce over ranks: max time, summed bytes
     total_b, decode_b = step_bytes(wl, S, ctx_after, 1)
-    t = torch.tensor([ms_total, ms_e2e, statistics.fmean(dec_ms)], dtype=torch.float64, device=dev)
-    if world > 1:
-        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-    ms_total, ms_e2e, dec_ms_mean = (float(x) for x in t.cpu())
+    ms_total, ms_e2e, dec_ms_mean = max_over_ranks([ms_total, ms_e2e, statistics.fmean(dec_ms)], world, dev)
     ms_step = ms_total / args.steps
-    value = world * total_b / (ms_step * 1e-3) / 1e9
-    e2e_value = world * total_b / (ms_e2e / args.steps * 1e-3) / 1e9
+    value = whole_job_value(total_b, world, ms_step)
+    e2e_value = whole_job_value(total_b, world, ms_e2e / args.steps)
     peak, peak_src = _peaks()
     achieved = decode_b / (dec_ms_mean * 1e-3) / 1e9
     line = {
