@@ -101,7 +101,10 @@ def oracle_out(wl, b, length, q_bits_b: np.ndarray, cache_arrays=None, device="c
 
 def compare_cache(cache: torch.Tensor, wl, b: int, length: int, arrays):
     """Bit-exact comparison of the device cache image with the oracle's logical arrays."""
-    got = uq_layout.gather_sequence(cache.cpu().numpy(), wl.block_tables[b], length)
+    n_pages = -(-length // wl.page_size)
+    idx = torch.from_numpy(wl.block_tables[b][:n_pages].astype(np.int64)).to(cache.device)
+    recs = cache.index_select(0, idx).cpu().numpy()                # only this sequence's pages leave the device
+    got = uq_layout.gather_sequence(recs, np.arange(n_pages), length)
     for name, g_, o_ in zip(("k_codes", "k_scales", "v_codes", "v_scales"), got, arrays):
         o_ = o_[:length]
         assert g_.shape == o_.shape, (name, g_.shape, o_.shape)

@@ -207,3 +207,46 @@ def test_full_size_cfg2_in_bench_launch_configuration_sampled():
     cfg = H.cfg_of(wl)
     S = uq.suggest_num_splits(cfg, wl.batch, int(wl.ctx_lens.mean()))
     _full_check(wl, [S], sample_seqs=[0, 17, 31], check_cache=True)
+
+
+@pytest.mark.parametrize("idx,seqs", [(3, "extremes"), (5, [3])])
+def test_full_size_configs_3_and_5_sampled(idx, seqs):
+    """BASELINE.json configs 3 (64 ragged sequences of 16k-64k tokens, 48/8 heads, GQA 6) and 5
+    (8 x 262,144 tokens) at FULL size with the split count bench.py would use; the cache image and
+    the decode output of the sampled sequences are checked against the oracle."""
+    wl = W.make_config(idx)
+    if seqs == "extremes":
+        seqs = [int(np.argmin(wl.ctx_lens)), int(np.argmax(wl.ctx_lens))]
+    cfg = H.cfg_of(wl)
+    S = uq.suggest_num_splits(cfg, wl.batch, int(wl.ctx_lens.mean()))
+    _full_check(wl, [S], sample_seqs=seqs, check_cache=True)
+
+
+def test_full_size_cfg4_shared_prefix_step_sampled():
+    """BASELINE.json config 4 at FULL size: 256 sequences share a 30,000-token prefix (the same
+    physical pages in every block table) and have log-normal private suffixes; one timed-style step
+    (append 1 token per sequence, decode, merge); two sampled sequences against the oracle."""
+    wl = W.make_config(4)
+    cfg = H.cfg_of(wl)
+    cache, bt = H.fill_cache(cfg, wl, DEV)
+    S = uq.suggest_num_splits(cfg, wl.batch, int(wl.ctx_lens.mean()))
+    bufs = uq.StepBuffers(cfg, wl.batch, S, DEV)
+    q = W.gen_q(wl, DEV, 0)
+    k_new, v_new = W.gen_new_kv(wl, 0, DEV)
+    cu = torch.arange(wl.batch + 1, dtype=torch.int32, device=DEV)
+    before = torch.from_numpy(wl.ctx_lens).to(DEV)
+    after = torch.from_numpy(wl.ctx_lens + 1).to(DEV)
+    out = uq.decode_step(cfg, bufs, q, k_new, v_new, cu, before, after, bt, cache)
+    torch.cuda.synchronize()
+    out = out.float().cpu().numpy().astype(np.float64)
+    order = np.argsort(wl.ctx_lens)
+    for b in (int(order[0]), int(order[len(order) // 2])):          # shortest and median sequence
+        L0 = int(wl.ctx_lens[b])
+        k0, v0 = W.seq_kv(wl, b, L0, DEV)
+        k = torch.cat([k0, k_new[b:b + 1]])
+        v = torch.cat([v0, v_new[b:b + 1]])
+        arrays = oracle.encode_kv(H.bits(k), H.bits(v))
+        H.compare_cache(cache, wl, b, L0 + 1, arrays)
+        ref, q8 = H.oracle_out(wl, b, L0 + 1, H.bits(q)[b], arrays)
+        assert np.array_equal(bufs.q_fp8[b].cpu().numpy(), q8)
+        H.check_out(out[b], ref, f"cfg4 full seq {b}")
