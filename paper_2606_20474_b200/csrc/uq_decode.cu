@@ -3,20 +3,20 @@
 // format follow include/uq.h.
 //
 // Design: one CTA per (sequence, kv head, split); the split is walked in
-// tiles of 128 tokens (8 pages).  Warp roles (320 threads):
-//   producer: per page one TMA tensor copy of the packed FP4 K codes
+// tiles of 128 tokens (8 pages).  Warp roles (352 threads).  Every async instruction (TMA copy,
+// tcgen05.mma / cp / commit) occupies its issuing warp for ~55 cycles (measured), so the 16 copies and
+// 12 MMAs of a tile are spread over three issuer warps:
+//   warp 2  TMA producer: per page one TMA tensor copy of the packed FP4 K codes
 //           (CU_TENSOR_MAP_DATA_TYPE_16U4_ALIGN16B + SWIZZLE_128B: the TMA unit expands the
 //           nibbles into the 8-bit containers tcgen05 reads) and one cp.async.bulk of the rest of
-//           the record (V codes, K scales, V scales), into a ring of mbarrier stages; compute warp
-//           w issues the copies of page w of every tile (an async-copy instruction occupies its
-//           issuing warp for ~55 cycles, so a single producer warp would cap the stream);
+//           the record (V codes, K scales, V scales), into a 3-stage mbarrier ring, L2 evict-first;
 //   warp 0  QK issuer: S[128 tok x 16 heads] = K . Q^T with
 //           tcgen05.mma.kind::mxf8f6f4.block_scale — E2M1 keys x E4M3 queries with the UE8M0 group
 //           scales applied by the tensor core (the paper's FP8xFP4 scaled MMA), K
 //           scales staged smem -> TMEM with tcgen05.cp;
 //   warp 1  PV issuer: O^T[128 d x 16 heads] += Vhat^T . P^T
 //           with tcgen05.mma.kind::f16 (A = Vhat^T from TMEM, B = P from smem); accumulators in TMEM;
-//   warps 2-9 compute: S rows from TMEM (tcgen05.ld), base-2 softmax against a LAZY per-head
+//   warps 3-10 compute: S rows from TMEM (tcgen05.ld), base-2 softmax against a LAZY per-head
 //           reference (a "rebase" — new reference, O rescaled in TMEM, tile's P redone — happens on
 //           the first tile and whenever a score exceeds the reference by 2^12 or a V scale exceeds
 //           the reference exponent), P -> fp16 operand in smem (double-buffered); then V codes ->
@@ -37,7 +37,8 @@ namespace uq {
 namespace {
 
 constexpr int kComputeWarps = 8;                     // two per TMEM lane quarter
-constexpr int kThreads = (kComputeWarps + 2) * 32;   // + QK issuer warp + PV issuer warp
+constexpr int kIssuerWarps = 3;                      // QK issuer, PV issuer, TMA producer
+constexpr int kThreads = (kComputeWarps + kIssuerWarps) * 32;
 #ifndef UQ_STAGES
 #define UQ_STAGES 3
 #endif
@@ -262,7 +263,8 @@ __device__ int g_trace_n[10];
 
 // ---------------------------------------------------------------- per-CTA shared bookkeeping
 struct Shared {
-  uint64_t full[kStages];     // 8 compute warps (expect_tx, one page each) + TMA bytes -> QK warp, compute warps
+  uint64_t full[kStages];     // producer (expect_tx) + TMA bytes -> QK warp, compute warps
+  uint64_t empty[kStages];    // 8 compute warps + QK commit -> producer
   uint64_t s_full[2];         // QK commit -> compute warps
   uint64_t s_free[2];         // 8 compute warps -> QK warp: S buffer read, may be overwritten
   uint64_t ready;             // 8 compute warps -> PV warp: P (smem) and Vhat (TMEM) of the tile are written
@@ -356,7 +358,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
 
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = base + kOffQ, sSFA = base + kOffSFA, sSFB = base + kOffSFB, sP = base + kOffP;
-  const uint32_t bar_full = smem_u32(&sh.full[0]),
+  const uint32_t bar_full = smem_u32(&sh.full[0]), bar_empty = smem_u32(&sh.empty[0]),
                  bar_sfull = smem_u32(&sh.s_full[0]), bar_sfree = smem_u32(&sh.s_free[0]),
                  bar_ready = smem_u32(&sh.ready), bar_done = smem_u32(&sh.done[0]);
 
@@ -364,7 +366,8 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < kStages; ++s) {
-      mbar_init(bar_full + 8 * s, kTilePages);        // one arrival per page (its loader lane)
+      mbar_init(bar_full + 8 * s, 1);
+      mbar_init(bar_empty + 8 * s, kComputeWarps + 1);
     }
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
@@ -426,6 +429,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
           umma_mxf8f6f4(tmem + kColS + 16 * sb, make_desc(st + 32 * kb, 16, 1024, 2), make_desc(sQ + 32 * kb, 16, 1024, 2),
                         idesc_qk | ((uint32_t)kb << 29), kb > 0, t_sfa + ((uint32_t)kb << 30), tmem + kColSFB);
         umma_commit(bar_sfull + 8 * sb);
+        umma_commit(bar_empty + 8 * s);
       }
       __syncwarp();
       TRACE(0, 4, i);
@@ -449,11 +453,35 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
       __syncwarp();
       TRACE(1, 4, i);
     }
+  } else if (warp == 2) {
+    // ================================================================ TMA producer warp
+    // Lanes 0..7 each issue the two copies of one page of the tile (the copies of a warp serialise at
+    // ~55 cycles each: ~900 cycles per tile, well inside the CTA's tile period).
+    const int32_t* bt = block_tables + (long long)b * max_pages;
+    const uint64_t pol = l2_evict_first_policy();
+    int page_next = (lane < kTilePages && p0 + lane < p1) ? bt[p0 + lane] : 0;
+    int s = 0, ph = 1;                                 // stage, parity to wait for on empty[s]
+    for (int i = 0; i < n_tiles; ++i) {
+      const int page = page_next;
+      const int npg = min(kTilePages, p1 - (p0 + kTilePages * i));
+      const int nb = p0 + kTilePages * (i + 1) + lane;
+      page_next = (lane < kTilePages && nb < p1) ? bt[nb] : 0;
+      mbar_wait(bar_empty + 8 * s, ph);
+      if (lane == 0) mbar_expect_tx(bar_full + 8 * s, (uint32_t)npg * kRecordBytes);
+      __syncwarp();
+      if (lane < npg) {
+        const uint32_t st = base + kOffStage + s * kStageBytes;
+        tma_load_3d(st + 2048 * lane, &tmap, 0, 0, page * Hkv + kvh, bar_full + 8 * s, pol);
+        bulk_g2s(st + 16384 + kRestBytes * lane, cache + ((long long)page * Hkv + kvh) * kRecordBytes + 1024, kRestBytes,
+                 bar_full + 8 * s, pol);
+      }
+      if (++s == kStages) { s = 0; ph ^= 1; }
+    }
   } else {
-    // ================================================================ compute warps (warp ids 2..9)
-    // The two issuer warps poll mbarriers; they sit on the lowest warp ids so that the scheduler's
-    // highest-warp-id-first arbitration favours the compute warps.
-    const int cw = warp - 2;                           // 0..7
+    // ================================================================ compute warps (warp ids 3..10)
+    // The three issuer warps sit on the lowest warp ids so that the scheduler's highest-warp-id-first
+    // arbitration favours the compute warps.
+    const int cw = warp - kIssuerWarps;                // 0..7
     const int q = warp & 3, hh = cw >> 2;              // TMEM lane quarter (hardware: warp id % 4), head half
     const int r = 32 * q + lane;                       // softmax: token row of the tile; epilogue: channel d
     const bool heads_live = (8 * hh < G);
@@ -466,32 +494,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
     for (int j = 0; j < 8; ++j) { mref[j] = -INFINITY; lsum[j] = 0.f; }
     int eref = 28;
 
-    // Every compute warp is the TMA producer of page `cw` of each tile (an async-copy instruction
-    // costs its issuing warp ~55 cycles, so the 16 copies of a tile are spread over the 8 warps).
-    const uint64_t pol = l2_evict_first_policy();
-    const int32_t* bt_mine = block_tables + (long long)b * max_pages + p0 + cw;
-    const uint8_t* cache_kvh = cache + (long long)kvh * kRecordBytes;
-    const long long page_stride = (long long)Hkv * kRecordBytes;
-    auto bt_entry = [&](int tile) -> int {             // physical page of this warp's page of `tile` (lane 0)
-      return (lane == 0 && tile < n_tiles && p0 + kTilePages * tile + cw < p1) ? bt_mine[kTilePages * tile] : -1;
-    };
-    auto load_page = [&](int tile, int page, int s) {  // lane 0: arrive on full[s] and start the two copies
-      if (lane == 0 && tile < n_tiles) {
-        if (page >= 0) {
-          const uint32_t st = base + kOffStage + s * kStageBytes;
-          mbar_expect_tx(bar_full + 8 * s, kRecordBytes);
-          tma_load_3d(st + 2048 * cw, &tmap, 0, 0, page * Hkv + kvh, bar_full + 8 * s, pol);
-          bulk_g2s(st + 16384 + kRestBytes * cw, cache_kvh + page * page_stride + 1024, kRestBytes, bar_full + 8 * s, pol);
-        } else {
-          mbar_arrive(bar_full + 8 * s);               // page beyond the split: nothing to load
-        }
-      }
-    };
-#pragma unroll
-    for (int t = 0; t < kStages; ++t) load_page(t, bt_entry(t), t);
-
     int s = 0, ph_full = 0;                            // stage of tile i, parity of i / kStages
-    int s_prev = kStages - 1;                          // stage of tile i-1 (refilled with tile i-1+kStages)
     for (int i = 0; i < n_tiles; ++i) {
       const int sb = i & 1, ph2 = (i >> 1) & 1;
       const uint32_t rest0 = base + kOffStage + s * kStageBytes + 16384 + kRestBytes * (4 * hf);
@@ -503,7 +506,6 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
       const uint32_t p_addr = sP + kPBytes * sb + (r >> 3) * 256 + hh * 128 + (r & 7) * 16;
 
       TRACE(2 + cw, 1, i);
-      const int page_ahead = bt_entry(i + kStages - 1);              // for the refill below (latency hidden by the softmax)
       mbar_wait(bar_sfull + 8 * sb, ph2);                            // S of the tile is in TMEM
       TRACE(2 + cw, 2, i);
       tc_fence_after();
@@ -609,10 +611,6 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
 #pragma unroll
       for (int j = 0; j < 8; ++j) lsum[j] += lt[j];
 
-      // ---- every compute warp is past the barrier above, so all of them finished tile i-1 and QK(i-1)
-      //      completed: the stage of tile i-1 is free -> refill it with tile i-1+kStages
-      if (i >= 1) load_page(i + kStages - 1, page_ahead, s_prev);
-
       // ---- S has been read: the QK warp may overwrite this S buffer (tile i+2)
       tc_fence_before();
       __syncwarp();
@@ -625,9 +623,11 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
       fence_async_smem();
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(bar_ready);
+      if (lane == 0) {
+        mbar_arrive(bar_ready);
+        mbar_arrive(bar_empty + 8 * s);                // this warp is done with the stage's V codes and scales
+      }
 
-      s_prev = s;
       if (++s == kStages) { s = 0; ph_full ^= 1; }
     }
 
@@ -659,7 +659,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
       }
     }
     bar_compute();
-    const int head = tid - 64;                         // first compute threads: one per query head
+    const int head = tid - 32 * kIssuerWarps;          // first compute threads: one per query head
     if (head < G) {
       const int h2 = head >> 3, j = head & 7;
       float l = 0.f;
