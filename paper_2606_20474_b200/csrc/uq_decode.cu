@@ -317,7 +317,6 @@ __device__ __forceinline__ void v_convert(uint32_t rest0, uint32_t scratch, uint
     o[4 * k + 3] = hmul2(f[3], m4.w);
   }
   tmem_st32(t_dst, o);
-  __syncwarp();
 }
 
 // ---------------------------------------------------------------- the kernel
@@ -406,7 +405,10 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
     if (lane == 0) umma_cp_sf(tmem + kColSFB, make_desc(sSFB, 16, 128, 0));
     for (int i = 0; i < n_tiles; ++i) {
       const int s = i % kStages, sb = i & 1;
-      if (i >= 2) mbar_wait(bar_sfree + 8 * sb, ((i >> 1) - 1) & 1);
+      if (i >= 2) {
+        mbar_wait(bar_sfree + 8 * sb, ((i >> 1) - 1) & 1);   // softmax(i-2) has read this S buffer
+        mbar_wait(bar_done + 8 * sb, ((i >> 1) - 1) & 1);    // PV(i-2) has read the P / Vhat buffers i&1: the
+      }                                                      // compute warps take s_full(i) as that guarantee too
       mbar_wait(bar_full + 8 * s, (i / kStages) & 1);
       TRACE(0, 3, i);
       const uint32_t st = base + kOffStage + s * kStageBytes;
@@ -509,11 +511,8 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
       mbar_wait(bar_sfull + 8 * sb, ph2);                            // S of the tile is in TMEM
       TRACE(2 + cw, 2, i);
       tc_fence_after();
-      mbar_wait(bar_full + 8 * s, ph_full);                          // (already complete) acquire the TMA bytes
-      if (i >= 2) {                                                  // P / Vhat buffers i&1 were read by PV(i-2)
-        mbar_wait(bar_done + 8 * sb, ph2 ^ 1);
-        tc_fence_after();
-      }
+      (void)mbar_test(bar_full + 8 * s, ph_full);                    // complete (QK(i) consumed it): acquire the TMA bytes
+      // PV(i-2) is complete as well (the QK warp waited for it before S(i)): P / Vhat buffers i&1 are free
 
       float lt[8];
       // softmax of this thread's row against the current references -> P (fp16, MN-major operand)
