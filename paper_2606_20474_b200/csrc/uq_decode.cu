@@ -213,6 +213,13 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32
         "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31]) : "memory");
   asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
+__device__ __forceinline__ void tmem_st16_nowait(uint32_t taddr, const uint32_t (&v)[16]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+      ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]),
+        "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void umma_f16_ts(uint32_t d, uint32_t ta, uint64_t db, uint32_t idesc, uint32_t acc) {
   asm volatile(
       "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
@@ -303,20 +310,25 @@ __device__ __forceinline__ int v_multipliers(uint32_t rest0, uint32_t scratch, i
 // Step 2: 64 tokens of channel d = 32 g + lane -> fp16 x multiplier -> TMEM (A operand of the PV
 // MMA: lane = channel, column c = tokens 2c, 2c+1).
 __device__ __forceinline__ void v_convert(uint32_t rest0, uint32_t scratch, uint32_t t_dst, int lane, int g) {
-  uint32_t o[32];
 #pragma unroll
-  for (int k = 0; k < 8; ++k) {                      // token-core k: page k>>1, half k&1 -> 8 tokens
-    uint32_t cw;
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(cw) : "r"(rest0 + kRestBytes * (k >> 1) + 512 * (k & 1) + 128 * g + 4 * lane));
-    const uint4 m4 = lds128(scratch + 16 * k);
-    uint32_t f[4];
-    cvt_e2m1x8(cw, f);
-    o[4 * k + 0] = hmul2(f[0], m4.x);
-    o[4 * k + 1] = hmul2(f[1], m4.y);
-    o[4 * k + 2] = hmul2(f[2], m4.z);
-    o[4 * k + 3] = hmul2(f[3], m4.w);
+  for (int h = 0; h < 2; ++h) {                      // 32 tokens (16 TMEM columns) at a time
+    uint32_t o[16];
+#pragma unroll
+    for (int kk = 0; kk < 4; ++kk) {                 // token-core k: page k>>1, half k&1 -> 8 tokens
+      const int k = 4 * h + kk;
+      uint32_t cw;
+      asm volatile("ld.shared.u32 %0, [%1];" : "=r"(cw) : "r"(rest0 + kRestBytes * (k >> 1) + 512 * (k & 1) + 128 * g + 4 * lane));
+      const uint4 m4 = lds128(scratch + 16 * k);
+      uint32_t f[4];
+      cvt_e2m1x8(cw, f);
+      o[4 * kk + 0] = hmul2(f[0], m4.x);
+      o[4 * kk + 1] = hmul2(f[1], m4.y);
+      o[4 * kk + 2] = hmul2(f[2], m4.z);
+      o[4 * kk + 3] = hmul2(f[3], m4.w);
+    }
+    tmem_st16_nowait(t_dst + 16 * h, o);
   }
-  tmem_st32(t_dst, o);
+  tmem_wait_st();
 }
 
 // ---------------------------------------------------------------- the kernel
