@@ -24,7 +24,8 @@
  *  - Arguments are validated on the host only.  Block-table entries outside [0, num_pages),
  *    seq_lens beyond max_pages*page_size, NaN/Inf inputs: undefined behaviour.
  *  - Supported geometry in this version: head_dim = 128, group_size = 32, page_size = 16,
- *    num_q_heads / num_kv_heads in 1..16 (UQ_ERR_UNSUPPORTED otherwise).
+ *    num_q_heads / num_kv_heads in 1..16, batch <= 2048 for uq_decode_attention
+ *    (UQ_ERR_UNSUPPORTED otherwise).
  *  - GQA map: query head h reads KV head h / (num_q_heads/num_kv_heads).
  *
  * PHYSICAL CACHE LAYOUT (uint8).  cache[num_pages][num_kv_heads][UQ_RECORD_BYTES]; the record
@@ -113,10 +114,16 @@ int32_t uq_rotate_quantize_append(const uq_config* cfg, const void* k_new, const
  *
  *  q_fp8        uint8 [batch, num_q_heads, head_dim] (E4M3 bytes of the rotated query).
  *  seq_lens     int32 [batch]: lengths INCLUDING any token appended in this step.
- *  num_splits   >= 1.  Split s of sequence b covers pages [s*pps, min((s+1)*pps, n_pages_b))
- *               with n_pages_b = ceil(seq_lens[b]/page_size) and
- *               pps = 8*ceil(ceil(n_pages_b/num_splits)/8) (whole 128-token tiles);
- *               a split may be empty.
+ *  num_splits   >= 1: the number of partial SLOTS per (sequence, query head).  The kernel cuts the
+ *               128-token tiles of all (sequence, kv head) items of the call, taken one item after
+ *               the other, into equal contiguous ranges, one per resident CTA (the same HBM traffic
+ *               per CTA whatever the sequence lengths are); a range may end inside an item, and the
+ *               CTAs that share an item fill consecutive slots of it, starting at slot 0.  Ranges are
+ *               made longer when needed so that no item spans more than num_splits of them; slots
+ *               an item does not use are written as empty.  With num_splits = 1 every item is
+ *               processed whole by one CTA.  Which tokens a slot covers is therefore an
+ *               implementation detail; uq_merge_splits needs only the format below.
+ *               batch <= 2048 per call.
  *  partial_acc  float32 [batch, num_q_heads, num_splits, head_dim]
  *  partial_ml   float32 [batch, num_q_heads, num_splits, 2] = (m_s, l_s)
  *
@@ -146,8 +153,8 @@ int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, const void*
 int32_t uq_merge_splits(const uq_config* cfg, const float* partial_acc, const float* partial_ml,
                         int32_t batch, int32_t num_splits, void* out_bf16, void* stream);
 
-/* Host.  A num_splits that gives uq_decode_attention about `waves` full waves of CTAs on the
- * current device for `batch` sequences of about `avg_seq_len` tokens (never below 1). */
+/* Host.  A num_splits (slot count) that lets uq_decode_attention balance `batch` sequences of about
+ * `avg_seq_len` tokens over the current device with room for sequences twice that long (never below 1). */
 int32_t uq_suggest_num_splits(const uq_config* cfg, int32_t batch, int32_t avg_seq_len);
 
 #ifdef __cplusplus

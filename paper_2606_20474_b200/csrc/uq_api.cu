@@ -71,25 +71,18 @@ extern "C" int32_t uq_suggest_num_splits(const uq_config* cfg, int32_t batch, in
     int v = 0;
     if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) sms = v;
   }
-  // The decode kernel runs 2 CTAs per SM, each walking its split in 128-token tiles with a fixed
-  // cost of about 2 tiles (setup, first-tile rebase, epilogue).  Pick the split count that best
-  // fills whole waves of CTAs while keeping splits long.
+  // uq_decode_attention gives every resident CTA (2 per SM) one equal range of 128-token tiles; an item
+  // (sequence, kv head) of T tiles then spans about T / range + 1 CTAs = slots.  Leave room for sequences
+  // twice the average length.
   const int64_t items = (int64_t)batch * cfg->num_kv_heads;
   const int64_t slots = (int64_t)sms * 2;
   const int64_t pages = (avg_seq_len + cfg->page_size - 1) / cfg->page_size;
   const int64_t tiles = (pages + 7) / 8 > 0 ? (pages + 7) / 8 : 1;
-  int64_t s = 1;
-  double best = -1.0;
-  for (int64_t c = 1; c <= 128 && c <= tiles; ++c) {
-    const int64_t t = (tiles + c - 1) / c;                 // tiles per split
-    const int64_t used = (tiles + t - 1) / t;              // non-empty splits
-    const double waves = (double)(items * used) / (double)slots;
-    const double whole = waves <= 1.0 ? 1.0 : (double)(int64_t)(waves + 0.999999);
-    const double score = (waves / whole) * ((double)t / (double)(t + 2));
-    if (score > best + 1e-9) {
-      best = score;
-      s = c;
-    }
-  }
+  int64_t range = (items * tiles + slots - 1) / slots;
+  if (range < 1) range = 1;
+  int64_t s = (2 * tiles + range - 1) / range + 1;
+  if (s > tiles + 1) s = tiles + 1;
+  if (s < 2) s = 2;
+  if (s > 64) s = 64;
   return (int32_t)s;
 }

@@ -52,11 +52,12 @@ constexpr int kStageBytes = kTilePages * (2048 + kRestBytes);   // K unpacked 16
 constexpr int kPBytes = 4096;                        // one P operand buffer: [token-core 16][head-core 2][8 tok][8 heads] f16
 constexpr float kThresh = 12.0f;                     // lazy-reference threshold (log2 units)
 constexpr unsigned kFull = 0xffffffffu;
+constexpr int kMaxBatch = 2048;                      // sequences per call (tile prefix sums live in shared memory)
 
 // dynamic shared memory map (offsets from a 1024-byte aligned base)
 constexpr int kOffStage = 0;
-constexpr int kOffQ = kOffStage + kStages * kStageBytes;       // 2048, SW128
-constexpr int kOffSFA = kOffQ + 2048;                          // 2 x 512
+constexpr int kOffQ = kOffStage + kStages * kStageBytes;       // 2 x 2048, SW128 (one per unit in flight)
+constexpr int kOffSFA = kOffQ + 4096;                          // 2 x 512
 constexpr int kOffSFB = kOffSFA + 1024;                        // 512
 constexpr int kOffP = kOffSFB + 512;                           // 2 x 4096 (double-buffered)
 constexpr int kOffMul = kOffP + 2 * kPBytes;                   // 8 warps x 128 B
@@ -144,6 +145,10 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tm,
   asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
                " [%0], [%1, {%2, %3, %4}], [%5], %6;"
                ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, uint32_t bar) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+               ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(bar) : "memory");
 }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -260,14 +265,6 @@ __device__ __forceinline__ float pow2i(int e) {   // 2^e, flushing to 0 below th
   return f > 0 ? __uint_as_float((uint32_t)min(f, 254) << 23) : 0.f;
 }
 
-#ifdef UQ_TRACE   // debug builds only: clock timeline of one CTA, buffered in smem (see uq_debug_trace below)
-__device__ long long g_trace[10][4096];
-__device__ int g_trace_n[10];
-#define TRACE(role, tag, tile) do { if (trace_on && lane == 0 && tr_n < 160) { tr_buf[role][tr_n] = make_uint2(((uint32_t)(tag) << 16) | (uint32_t)(tile), (uint32_t)clock64()); ++tr_n; } } while (0)
-#else
-#define TRACE(role, tag, tile) do {} while (0)
-#endif
-
 // ---------------------------------------------------------------- per-CTA shared bookkeeping
 struct Shared {
   uint64_t full[kStages];     // producer (expect_tx) + TMA bytes -> QK warp, compute warps
@@ -276,11 +273,14 @@ struct Shared {
   uint64_t s_free[2];         // 8 compute warps -> QK warp: S buffer read, may be overwritten
   uint64_t ready;             // 8 compute warps -> PV warp: P (smem) and Vhat (TMEM) of the tile are written
   uint64_t done[2];           // PV commit of tile i -> done[i&1]: P / Vhat buffer i&1 free, O up to date
+  uint64_t q_full[2];         // TMA: the FP8 query tile of a work unit landed (buffer = unit ordinal & 1)
   uint32_t tmem_base;
   float wmax[kComputeWarps][8];
   int wvmax[kComputeWarps];
   float lsum[kComputeWarps][8];
   float mref[16];
+  int total_tiles, max_tiles;  // sum (x kv heads) and max over sequences of the tiles per (sequence, kv head)
+  int pre[kMaxBatch + 1];      // pre[b] = tiles of sequences 0..b-1 (per kv head)
 };
 
 // This warp's share of the tile's V: channel group g (= its TMEM lane quarter), tokens
@@ -331,47 +331,108 @@ __device__ __forceinline__ void v_convert(uint32_t rest0, uint32_t scratch, uint
   tmem_wait_st();
 }
 
+// ---------------------------------------------------------------- work schedule
+// The tiles (128 tokens) of all (sequence, kv head) items form one sequence, item after item.  With
+// num_splits >= 2 every CTA of the grid takes one contiguous range of `tpc` tiles of it (balanced: the
+// same amount of HBM traffic per CTA whatever the lengths are); a range may end inside an item and
+// start inside the next one, so a CTA works through a few UNITS (item, tile range), keeping its TMA /
+// MMA pipelines running across unit boundaries.  The CTAs that share an item write consecutive partial
+// slots of it; tpc is raised if needed so that no item spans more than num_splits CTAs.  With
+// num_splits == 1 a unit is a whole item and CTA c takes items c, c + gridDim.x, ...
+struct Unit {
+  int b, kvh, p0, p1, n_tiles, tok_end, L;
+  int slots_used;                                      // > 0 on the unit holding the item's last tile: slots the item uses
+  long long row0;                                      // partial row of head 0 in this unit's slot: + head * num_splits
+};
+struct Cursor {
+  int b, kvh, t, g, g1, it;                            // balanced: position (b, kvh, tile t), global tile g, range end g1; items: it
+};
+
+struct Sched {
+  const int32_t* seq_lens;
+  const int* pre;                                      // shared: pre[b] = tiles of sequences < b (per kv head)
+  int B, Hq, Hkv, G, S, tpc, total;
+  __device__ __forceinline__ int tiles(int b) const { return pre[b + 1] - pre[b]; }
+
+  __device__ void start(Cursor& c) const {
+    if (S == 1) { c.it = blockIdx.x; return; }
+    c.g = min((int)blockIdx.x * tpc, total);
+    c.g1 = min(c.g + tpc, total);
+    if (c.g >= c.g1) return;
+    int lo = 0, hi = B;                                // largest b with Hkv * pre[b] <= g (and tiles(b) > 0 follows)
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (Hkv * pre[mid] <= c.g) lo = mid; else hi = mid;
+    }
+    c.b = lo;
+    const int off = c.g - Hkv * pre[lo], tb = tiles(lo);
+    c.kvh = off / tb;
+    c.t = off - c.kvh * tb;
+  }
+  // next unit of this CTA, false when there is none
+  __device__ bool next(Cursor& c, Unit& u) const {
+    int t0, t1, tb;
+    if (S == 1) {
+      for (;; c.it += gridDim.x) {
+        if (c.it >= B * Hkv) return false;
+        u.b = c.it / Hkv;
+        tb = tiles(u.b);
+        if (tb > 0) break;
+      }
+      u.kvh = c.it - u.b * Hkv;
+      c.it += gridDim.x;
+      t0 = 0; t1 = tb;
+      u.slots_used = 1;
+      u.row0 = ((long long)u.b * Hq + (long long)u.kvh * G) * S;
+    } else {
+      if (c.g >= c.g1) return false;
+      u.b = c.b; u.kvh = c.kvh;
+      tb = tiles(c.b);
+      t0 = c.t;
+      t1 = min(tb, t0 + (c.g1 - c.g));
+      const int item_start = c.g - t0;                 // global tile index of the item's first tile
+      const int slot = (int)blockIdx.x - item_start / tpc;
+      u.slots_used = (t1 == tb) ? slot + 1 : 0;
+      u.row0 = ((long long)u.b * Hq + (long long)u.kvh * G) * S + slot;
+      c.g += t1 - t0;
+      c.t = t1;
+      if (t1 == tb) {                                  // on to the next item with tiles
+        c.t = 0;
+        if (++c.kvh == Hkv) {
+          c.kvh = 0;
+          do { ++c.b; } while (c.b < B && tiles(c.b) == 0);
+        }
+      }
+    }
+    u.L = seq_lens[u.b];
+    const int n_pages = (u.L + kPage - 1) / kPage;
+    u.p0 = kTilePages * t0;
+    u.p1 = min(kTilePages * t1, n_pages);
+    u.n_tiles = t1 - t0;
+    u.tok_end = min(u.L, u.p1 * kPage);
+    return true;
+  }
+};
+
 // ---------------------------------------------------------------- the kernel
 __global__ void __launch_bounds__(kThreads, UQ_CTAS_PER_SM)
-decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restrict__ q_fp8,
+decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_q,
               const uint8_t* __restrict__ cache, const int32_t* __restrict__ block_tables, int max_pages,
-              const int32_t* __restrict__ seq_lens, int Hq, int Hkv, int num_splits,
+              const int32_t* __restrict__ seq_lens, int batch, int Hq, int Hkv, int num_splits,
               float score_scale /* sm_scale * log2(e) */, float* __restrict__ partial_acc,
               float* __restrict__ partial_ml) {
   extern __shared__ uint8_t smem_raw[];
   __shared__ __align__(8) Shared sh;
 
-  const int split = blockIdx.x, kvh = blockIdx.y, b = blockIdx.z;
   const int G = Hq / Hkv;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-#ifdef UQ_TRACE
-  const bool trace_on = (split == 2 && kvh == 1 && b == 7);
-  __shared__ uint2 tr_buf[10][160];
-  int tr_n = 0;
-#endif
-
-  const int L = seq_lens[b];
-  const int n_pages = (L + kPage - 1) / kPage;
-  int pps = (n_pages + num_splits - 1) / num_splits;
-  pps = (pps + kTilePages - 1) / kTilePages * kTilePages;
-  const int p0 = split * pps;
-  const int p1 = min(p0 + pps, n_pages);
-  const long long row0 = ((long long)b * Hq + (long long)kvh * G) * num_splits + split;  // + head*num_splits
-  if (p0 >= p1) {  // empty split: (m, l) = (-inf, 0); acc is never read by the merge
-    if (tid < G) {
-      float2* ml = reinterpret_cast<float2*>(partial_ml) + row0 + (long long)tid * num_splits;
-      *ml = make_float2(-INFINITY, 0.f);
-    }
-    return;
-  }
-  const int n_tiles = (p1 - p0 + kTilePages - 1) / kTilePages;
-  const int tok_end = min(L, p1 * kPage);
 
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = base + kOffQ, sSFA = base + kOffSFA, sSFB = base + kOffSFB, sP = base + kOffP;
   const uint32_t bar_full = smem_u32(&sh.full[0]), bar_empty = smem_u32(&sh.empty[0]),
                  bar_sfull = smem_u32(&sh.s_full[0]), bar_sfree = smem_u32(&sh.s_free[0]),
-                 bar_ready = smem_u32(&sh.ready), bar_done = smem_u32(&sh.done[0]);
+                 bar_ready = smem_u32(&sh.ready), bar_done = smem_u32(&sh.done[0]),
+                 bar_qfull = smem_u32(&sh.q_full[0]);
 
   // ---------------- setup
   if (tid == 0) {
@@ -385,6 +446,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
       mbar_init(bar_sfull + 8 * h, 1);
       mbar_init(bar_sfree + 8 * h, kComputeWarps);
       mbar_init(bar_done + 8 * h, 1);
+      mbar_init(bar_qfull + 8 * h, 1);
     }
     mbar_init(bar_ready, kComputeWarps);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -394,14 +456,32 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
                  "r"(kTmemCols));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
-  if (tid < 128) {  // hoisted FP8 query tile: 16 rows x 128 B, 128-byte swizzle; rows >= G are zero
-    const int n = tid >> 3, c = tid & 7;
-    uint4 v = make_uint4(0u, 0u, 0u, 0u);
-    if (n < G) v = *reinterpret_cast<const uint4*>(q_fp8 + ((long long)b * Hq + (long long)kvh * G + n) * kHeadDim + 16 * c);
-    sts128(sQ + n * 128 + ((c ^ (n & 7)) << 4), v);
-  }
   if (tid < 128) {  // query-side scale factors: UE8M0 byte 127 = 2^0
     asm volatile("st.shared.u32 [%0], %1;" ::"r"(sSFB + 4 * tid), "r"(0x7F7F7F7Fu) : "memory");
+  }
+  // tiles per sequence -> inclusive prefix sums in shared memory (every CTA computes the same schedule)
+  for (int b = tid; b < batch; b += kThreads) {
+    const int L = seq_lens[b];
+    sh.pre[b + 1] = ((L + kPage - 1) / kPage + kTilePages - 1) / kTilePages;
+  }
+  if (tid == 0) sh.pre[0] = 0;
+  __syncthreads();
+  if (warp == 0) {                                     // warp scan over chunks of 32 with a running carry
+    int carry = 0, mx = 0;
+    for (int b0 = 0; b0 < batch; b0 += 32) {
+      const int b = b0 + lane;
+      const int v = b < batch ? sh.pre[b + 1] : 0;
+      int x = v;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int y = __shfl_up_sync(kFull, x, o);
+        if (lane >= o) x += y;
+      }
+      if (b < batch) sh.pre[b + 1] = carry + x;
+      carry += __shfl_sync(kFull, x, 31);
+      mx = max(mx, __reduce_max_sync(kFull, v));
+    }
+    if (lane == 0) { sh.total_tiles = carry * Hkv; sh.max_tiles = mx; }
   }
   fence_async_smem();
   tc_fence_before();
@@ -409,93 +489,139 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
   tc_fence_after();
   const uint32_t tmem = sh.tmem_base;
 
+  Sched sc;
+  sc.seq_lens = seq_lens; sc.pre = sh.pre; sc.B = batch; sc.Hq = Hq; sc.Hkv = Hkv; sc.G = G; sc.S = num_splits;
+  sc.total = sh.total_tiles;
+  sc.tpc = 1;
+  if (num_splits > 1) {
+    const int even = (sc.total + (int)gridDim.x - 1) / (int)gridDim.x;
+    const int fit = (sh.max_tiles + num_splits - 2) / (num_splits - 1);   // an item spans at most num_splits ranges
+    sc.tpc = max(1, max(even, fit));
+  }
+
   if (warp == 0) {
     // ================================================================ QK warp
-    // S(i)[128 tok x 16 heads] = K(i) . Q^T as soon as the tile's bytes have landed and the S buffer
-    // (read by the softmax of tile i-2) is free.
+    // Per unit: the FP8 query tile (16 rows x 128 B, 128-byte swizzle) arrives by TMA into Q buffer
+    // (unit ordinal & 1) — "hoisted", once per unit; rows past the unit's G heads belong to
+    // the next kv head (or are zero past the tensor end) and only feed score columns nobody reads.
+    // Per tile: S(gt)[128 tok x 16 heads] = K . Q^T once the tile's bytes have landed, the S buffer was read
+    // by the softmax of global tile gt-2 and PV(gt-2) has read the P / Vhat buffers gt&1.
     const uint32_t idesc_qk = (5u << 7) | (0u << 10) | (2u << 17) | (1u << 23) | (8u << 24);   // E2M1 x E4M3, UE8M0, N=16, M=128
     if (lane == 0) umma_cp_sf(tmem + kColSFB, make_desc(sSFB, 16, 128, 0));
-    for (int i = 0; i < n_tiles; ++i) {
-      const int s = i % kStages, sb = i & 1;
-      if (i >= 2) {
-        mbar_wait(bar_sfree + 8 * sb, ((i >> 1) - 1) & 1);   // softmax(i-2) has read this S buffer
-        mbar_wait(bar_done + 8 * sb, ((i >> 1) - 1) & 1);    // PV(i-2) has read the P / Vhat buffers i&1: the
-      }                                                      // compute warps take s_full(i) as that guarantee too
-      mbar_wait(bar_full + 8 * s, (i / kStages) & 1);
-      TRACE(0, 3, i);
-      const uint32_t st = base + kOffStage + s * kStageBytes;
-      // scale-factor atom: row r = 32 c + lane of the tile -> 16-byte line `lane`, word c
-      uint32_t v[4];
-#pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        const int r = 32 * c + lane;
-        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v[c]) : "r"(st + 16384 + kRestBytes * (r >> 4) + 1024 + 4 * (r & 15)));
-      }
-      sts128(sSFA + 512 * sb + 16 * lane, make_uint4(v[0], v[1], v[2], v[3]));
-      fence_async_smem();
-      __syncwarp();
-      tc_fence_after();
+    auto load_q = [&](const Unit& un, int k) {         // lane 0: Q tile of unit ordinal k
       if (lane == 0) {
-        const uint32_t t_sfa = tmem + kColSFA + 4 * sb;
-        umma_cp_sf(t_sfa, make_desc(sSFA + 512 * sb, 16, 128, 0));
-#pragma unroll
-        for (int kb = 0; kb < 4; ++kb)
-          umma_mxf8f6f4(tmem + kColS + 16 * sb, make_desc(st + 32 * kb, 16, 1024, 2), make_desc(sQ + 32 * kb, 16, 1024, 2),
-                        idesc_qk | ((uint32_t)kb << 29), kb > 0, t_sfa + ((uint32_t)kb << 30), tmem + kColSFB);
-        umma_commit(bar_sfull + 8 * sb);
-        umma_commit(bar_empty + 8 * s);
+        mbar_expect_tx(bar_qfull + 8 * (k & 1), 2048);
+        tma_load_2d(sQ + 2048 * (k & 1), &tmap_q, 0, un.b * Hq + un.kvh * G, bar_qfull + 8 * (k & 1));
       }
-      __syncwarp();
-      TRACE(0, 4, i);
+    };
+    Cursor cur, cur_nx;
+    sc.start(cur);
+    cur_nx = cur;
+    Unit un, nx;
+    bool have_nx = sc.next(cur_nx, nx);                // nx runs one unit ahead of un
+    int gt = 0, s = 0, ph_full = 0;                    // global tile counter, its stage and full-barrier parity
+    int k = 0, k_q = -1;                               // ordinal of the current unit; last ordinal whose Q load was issued
+    while (have_nx) {
+      un = nx;
+      have_nx = sc.next(cur_nx, nx);
+      for (int i = 0; i < un.n_tiles; ++i) {
+        const int sb = gt & 1;
+        if (gt >= 2) {
+          mbar_wait(bar_sfree + 8 * sb, ((gt >> 1) - 1) & 1);
+          mbar_wait(bar_done + 8 * sb, ((gt >> 1) - 1) & 1);
+        }
+        // here every QK up to global tile gt-2 has completed (its S was read): at i == 0 the Q buffer of
+        // unit k-2 (= buffer k & 1), at i == 1 that of unit k-1 (= buffer (k+1) & 1) may be refilled
+        if (i == 0 && k_q < k) { load_q(un, k); k_q = k; }
+        if (i == 1 && have_nx) { load_q(nx, k + 1); k_q = k + 1; }
+        if (i == 0) mbar_wait(bar_qfull + 8 * (k & 1), (k >> 1) & 1);
+        mbar_wait(bar_full + 8 * s, ph_full);
+        const uint32_t st = base + kOffStage + s * kStageBytes;
+        // scale-factor atom: row r = 32 c + lane of the tile -> 16-byte line `lane`, word c
+        uint32_t v[4];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          const int r = 32 * c + lane;
+          asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v[c]) : "r"(st + 16384 + kRestBytes * (r >> 4) + 1024 + 4 * (r & 15)));
+        }
+        sts128(sSFA + 512 * sb + 16 * lane, make_uint4(v[0], v[1], v[2], v[3]));
+        fence_async_smem();
+        __syncwarp();
+        tc_fence_after();
+        if (lane == 0) {
+          const uint32_t t_sfa = tmem + kColSFA + 4 * sb, qb = sQ + 2048 * (k & 1);
+          umma_cp_sf(t_sfa, make_desc(sSFA + 512 * sb, 16, 128, 0));
+#pragma unroll
+          for (int kb = 0; kb < 4; ++kb)
+            umma_mxf8f6f4(tmem + kColS + 16 * sb, make_desc(st + 32 * kb, 16, 1024, 2), make_desc(qb + 32 * kb, 16, 1024, 2),
+                          idesc_qk | ((uint32_t)kb << 29), kb > 0, t_sfa + ((uint32_t)kb << 30), tmem + kColSFB);
+          umma_commit(bar_sfull + 8 * sb);
+          umma_commit(bar_empty + 8 * s);
+        }
+        __syncwarp();
+        ++gt;
+        if (++s == kStages) { s = 0; ph_full ^= 1; }
+      }
+      ++k;
     }
   } else if (warp == 1) {
     // ================================================================ PV warp
-    // O^T[128 d x 16 heads] += Vhat^T (TMEM, buffer i&1) . P^T (smem, buffer i&1); f16 x f16 -> f32, B MN-major
+    // O^T[128 d x 16 heads] += Vhat^T (TMEM, buffer gt&1) . P^T (smem, buffer gt&1); f16 x f16 -> f32, B MN-major
     const uint32_t idesc_pv = (1u << 4) | (1u << 16) | (2u << 17) | (8u << 24);
-    for (int i = 0; i < n_tiles; ++i) {
-      mbar_wait(bar_ready, i & 1);
-      TRACE(1, 3, i);
-      tc_fence_after();
-      if (lane == 0) {
-        const uint32_t pbuf = sP + kPBytes * (i & 1), vbuf = tmem + kColV + 64 * ((i & 1) % kVBufs);
+    Cursor cur;
+    sc.start(cur);
+    Unit un;
+    int gt = 0;
+    while (sc.next(cur, un)) {
+      for (int i = 0; i < un.n_tiles; ++i, ++gt) {
+        mbar_wait(bar_ready, gt & 1);
+        tc_fence_after();
+        if (lane == 0) {
+          const uint32_t pbuf = sP + kPBytes * (gt & 1), vbuf = tmem + kColV + 64 * ((gt & 1) % kVBufs);
 #pragma unroll
-        for (int j = 0; j < 8; ++j)                    // 16 tokens per MMA = 8 columns of Vhat^T
-          umma_f16_ts(tmem + kColO, vbuf + 8 * j, make_desc(pbuf + 512 * j, 256, 128, 0), idesc_pv,
-                      (i > 0 || j > 0) ? 1u : 0u);
-        umma_commit(bar_done + 8 * (i & 1));
+          for (int j = 0; j < 8; ++j)                    // 16 tokens per MMA = 8 columns of Vhat^T
+            umma_f16_ts(tmem + kColO, vbuf + 8 * j, make_desc(pbuf + 512 * j, 256, 128, 0), idesc_pv,
+                        (i > 0 || j > 0) ? 1u : 0u);
+          umma_commit(bar_done + 8 * (gt & 1));
+        }
+        __syncwarp();
       }
-      __syncwarp();
-      TRACE(1, 4, i);
     }
   } else if (warp == 2) {
     // ================================================================ TMA producer warp
     // Lanes 0..7 each issue the two copies of one page of the tile (the copies of a warp serialise at
-    // ~55 cycles each: ~900 cycles per tile, well inside the CTA's tile period).
-    const int32_t* bt = block_tables + (long long)b * max_pages;
+    // ~55 cycles each: ~900 cycles per tile, inside the CTA's tile period); the ring runs across units.
     const uint64_t pol = l2_evict_first_policy();
-    int page_next = (lane < kTilePages && p0 + lane < p1) ? bt[p0 + lane] : 0;
+    Cursor cur;
+    sc.start(cur);
+    Unit un;
     int s = 0, ph = 1;                                 // stage, parity to wait for on empty[s]
-    for (int i = 0; i < n_tiles; ++i) {
-      const int page = page_next;
-      const int npg = min(kTilePages, p1 - (p0 + kTilePages * i));
-      const int nb = p0 + kTilePages * (i + 1) + lane;
-      page_next = (lane < kTilePages && nb < p1) ? bt[nb] : 0;
-      mbar_wait(bar_empty + 8 * s, ph);
-      if (lane == 0) mbar_expect_tx(bar_full + 8 * s, (uint32_t)npg * kRecordBytes);
-      __syncwarp();
-      if (lane < npg) {
-        const uint32_t st = base + kOffStage + s * kStageBytes;
-        tma_load_3d(st + 2048 * lane, &tmap, 0, 0, page * Hkv + kvh, bar_full + 8 * s, pol);
-        bulk_g2s(st + 16384 + kRestBytes * lane, cache + ((long long)page * Hkv + kvh) * kRecordBytes + 1024, kRestBytes,
-                 bar_full + 8 * s, pol);
+    while (sc.next(cur, un)) {
+      const int32_t* bt = block_tables + (long long)un.b * max_pages + un.p0 + lane;
+      int page_next = (lane < kTilePages && un.p0 + lane < un.p1) ? bt[0] : 0;
+      for (int i = 0; i < un.n_tiles; ++i) {
+        const int page = page_next;
+        const int npg = min(kTilePages, un.p1 - (un.p0 + kTilePages * i));
+        const int nb = un.p0 + kTilePages * (i + 1) + lane;
+        page_next = (lane < kTilePages && nb < un.p1) ? bt[kTilePages * (i + 1)] : 0;
+        mbar_wait(bar_empty + 8 * s, ph);
+        if (lane == 0) mbar_expect_tx(bar_full + 8 * s, (uint32_t)npg * kRecordBytes);
+        __syncwarp();
+        if (lane < npg) {
+          const uint32_t st = base + kOffStage + s * kStageBytes;
+          tma_load_3d(st + 2048 * lane, &tmap, 0, 0, page * Hkv + un.kvh, bar_full + 8 * s, pol);
+          bulk_g2s(st + 16384 + kRestBytes * lane, cache + ((long long)page * Hkv + un.kvh) * kRecordBytes + 1024, kRestBytes,
+                   bar_full + 8 * s, pol);
+        }
+        if (++s == kStages) { s = 0; ph ^= 1; }
       }
-      if (++s == kStages) { s = 0; ph ^= 1; }
     }
   } else {
     // ================================================================ compute warps (warp ids 3..10)
     // The three issuer warps sit on the lowest warp ids so that the scheduler's highest-warp-id-first
     // arbitration favours the compute warps.
     const int cw = warp - kIssuerWarps;                // 0..7
+    const int ctid = tid - 32 * kIssuerWarps;          // 0..255
     const int q = warp & 3, hh = cw >> 2;              // TMEM lane quarter (hardware: warp id % 4), head half
     const int r = 32 * q + lane;                       // softmax: token row of the tile; epilogue: channel d
     const bool heads_live = (8 * hh < G);
@@ -503,193 +629,204 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restric
     const uint32_t lane_sel = (uint32_t)(32 * q) << 16;
     const int g = q, hf = hh;                          // V conversion: channel group (= lane quarter), token half of the tile
     const uint32_t t_v = tmem + lane_sel + kColV + 32 * hf;
-    float mref[8], lsum[8];
-#pragma unroll
-    for (int j = 0; j < 8; ++j) { mref[j] = -INFINITY; lsum[j] = 0.f; }
-    int eref = 28;
+    float2* const ml_out = reinterpret_cast<float2*>(partial_ml);
 
-    int s = 0, ph_full = 0;                            // stage of tile i, parity of i / kStages
-    for (int i = 0; i < n_tiles; ++i) {
-      const int sb = i & 1, ph2 = (i >> 1) & 1;
-      const uint32_t rest0 = base + kOffStage + s * kStageBytes + 16384 + kRestBytes * (4 * hf);
-      const int pg0 = p0 + kTilePages * i;                           // first page of the tile
-      const bool tile_partial = (pg0 + kTilePages) * kPage > tok_end;
-      const bool tok_ok = pg0 * kPage + r < tok_end;
-      const int tok_left = tok_end - (pg0 * kPage + 64 * hf);      // valid tokens in this warp's 64-token half
-      const uint32_t t_s = tmem + lane_sel + kColS + 16 * sb + 8 * hh;
-      const uint32_t p_addr = sP + kPBytes * sb + (r >> 3) * 256 + hh * 128 + (r & 7) * 16;
-
-      TRACE(2 + cw, 1, i);
-      mbar_wait(bar_sfull + 8 * sb, ph2);                            // S of the tile is in TMEM
-      TRACE(2 + cw, 2, i);
-      tc_fence_after();
-      (void)mbar_test(bar_full + 8 * s, ph_full);                    // complete (QK(i) consumed it): acquire the TMA bytes
-      // PV(i-2) is complete as well (the QK warp waited for it before S(i)): P / Vhat buffers i&1 are free
-
-      float lt[8];
-      // softmax of this thread's row against the current references -> P (fp16, MN-major operand)
-      auto softmax_pass = [&]() -> bool {
-#pragma unroll
-        for (int j = 0; j < 8; ++j) lt[j] = 0.f;
-        if (!heads_live) return false;
-        float t[8];
-        tmem_ld8(t_s, t);
-#pragma unroll
-        for (int j = 0; j < 8; ++j) t[j] = fmaf(t[j], score_scale, -mref[j]);
-        if (tile_partial) {
-#pragma unroll
-          for (int j = 0; j < 8; ++j) t[j] = tok_ok ? t[j] : -INFINITY;
-        }
-        const float tmax = fmaxf(fmaxf(fmaxf(t[0], t[1]), fmaxf(t[2], t[3])), fmaxf(fmaxf(t[4], t[5]), fmaxf(t[6], t[7])));
-#pragma unroll
-        for (int j = 0; j < 8; ++j) lt[j] = ex2(t[j]);
-        uint4 o;
-        asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.x) : "f"(lt[1]), "f"(lt[0]));
-        asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.y) : "f"(lt[3]), "f"(lt[2]));
-        asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.z) : "f"(lt[5]), "f"(lt[4]));
-        asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.w) : "f"(lt[7]), "f"(lt[6]));
-        sts128(p_addr, o);
-        return tmax > kThresh;
-      };
-
-      bool rebase = (i == 0);
-      int vmax = 0;
-      if (!rebase) {
-        const bool ex = softmax_pass();
-        vmax = tile_partial ? v_multipliers<true>(rest0, scratch, lane, g, tok_left, eref)
-                            : v_multipliers<false>(rest0, scratch, lane, g, tok_left, eref);
-        tc_fence_before();
-        TRACE(2 + cw, 3, i);
-        rebase = bar_compute_or(ex || vmax > eref);
-        TRACE(2 + cw, 4, i);
+    // items without any token: all their slots are empty, (m, l) = (-inf, 0)
+    for (int it = blockIdx.x; it < batch * Hkv; it += gridDim.x) {
+      const int b = it / Hkv;
+      if (sc.tiles(b) == 0) {
+        const long long row = ((long long)b * Hq + (long long)(it - b * Hkv) * G) * num_splits;
+        for (int e = ctid; e < G * num_splits; e += 32 * kComputeWarps) ml_out[row + e] = make_float2(-INFINITY, 0.f);
       }
-      if (__builtin_expect(rebase, 0)) {
-        // ---- statistics of the tile: per-head maximum score, maximum V scale byte
-        vmax = v_multipliers<true>(rest0, scratch, lane, g, tok_left, eref);
-        float tm[8];
+    }
+
+    Cursor cur;
+    sc.start(cur);
+    Unit un;
+    int gt = 0, s = 0, ph_full = 0;                    // global tile counter, its stage and full-barrier parity
+    while (sc.next(cur, un)) {
+      float mref[8], lsum[8];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) tm[j] = -INFINITY;
-        if (heads_live) {
-          float sv[8];
-          tmem_ld8(t_s, sv);
+      for (int j = 0; j < 8; ++j) { mref[j] = -INFINITY; lsum[j] = 0.f; }
+      int eref = 28;
+
+      for (int i = 0; i < un.n_tiles; ++i) {
+        const int sb = gt & 1, ph2 = (gt >> 1) & 1;
+        const uint32_t rest0 = base + kOffStage + s * kStageBytes + 16384 + kRestBytes * (4 * hf);
+        const int pg0 = un.p0 + kTilePages * i;                        // first page of the tile
+        const bool tile_partial = (pg0 + kTilePages) * kPage > un.tok_end;
+        const bool tok_ok = pg0 * kPage + r < un.tok_end;
+        const int tok_left = un.tok_end - (pg0 * kPage + 64 * hf);   // valid tokens in this warp's 64-token half
+        const uint32_t t_s = tmem + lane_sel + kColS + 16 * sb + 8 * hh;
+        const uint32_t p_addr = sP + kPBytes * sb + (r >> 3) * 256 + hh * 128 + (r & 7) * 16;
+
+        mbar_wait(bar_sfull + 8 * sb, ph2);                            // S of the tile is in TMEM
+        tc_fence_after();
+        (void)mbar_test(bar_full + 8 * s, ph_full);                    // complete (QK consumed it): acquire the TMA bytes
+        // PV(gt-2) is complete as well (the QK warp waited for it before S(gt)): P / Vhat buffers gt&1 are free
+
+        float lt[8];
+        // softmax of this thread's row against the current references -> P (fp16, MN-major operand)
+        auto softmax_pass = [&]() -> bool {
+#pragma unroll
+          for (int j = 0; j < 8; ++j) lt[j] = 0.f;
+          if (!heads_live) return false;
+          float t[8];
+          tmem_ld8(t_s, t);
+#pragma unroll
+          for (int j = 0; j < 8; ++j) t[j] = fmaf(t[j], score_scale, -mref[j]);
+          if (tile_partial) {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) t[j] = tok_ok ? t[j] : -INFINITY;
+          }
+          const float tmax = fmaxf(fmaxf(fmaxf(t[0], t[1]), fmaxf(t[2], t[3])), fmaxf(fmaxf(t[4], t[5]), fmaxf(t[6], t[7])));
+#pragma unroll
+          for (int j = 0; j < 8; ++j) lt[j] = ex2(t[j]);
+          uint4 o;
+          asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.x) : "f"(lt[1]), "f"(lt[0]));
+          asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.y) : "f"(lt[3]), "f"(lt[2]));
+          asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.z) : "f"(lt[5]), "f"(lt[4]));
+          asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.w) : "f"(lt[7]), "f"(lt[6]));
+          sts128(p_addr, o);
+          return tmax > kThresh;
+        };
+
+        bool rebase = (i == 0);
+        int vmax = 0;
+        if (!rebase) {
+          const bool ex = softmax_pass();
+          vmax = tile_partial ? v_multipliers<true>(rest0, scratch, lane, g, tok_left, eref)
+                              : v_multipliers<false>(rest0, scratch, lane, g, tok_left, eref);
+          tc_fence_before();
+          rebase = bar_compute_or(ex || vmax > eref);
+        }
+        if (__builtin_expect(rebase, 0)) {
+          // ---- statistics of the tile: per-head maximum score, maximum V scale byte
+          vmax = v_multipliers<true>(rest0, scratch, lane, g, tok_left, eref);
+          float tm[8];
+#pragma unroll
+          for (int j = 0; j < 8; ++j) tm[j] = -INFINITY;
+          if (heads_live) {
+            float sv[8];
+            tmem_ld8(t_s, sv);
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              float x = tok_ok ? sv[j] * score_scale : -INFINITY;
+#pragma unroll
+              for (int o = 16; o; o >>= 1) x = fmaxf(x, __shfl_xor_sync(kFull, x, o));
+              tm[j] = x;
+            }
+          }
+          if (lane == 0) {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) sh.wmax[cw][j] = tm[j];
+            sh.wvmax[cw] = vmax;
+          }
+          tc_fence_before();
+          bar_compute();
+          int evm = 0;
+#pragma unroll
+          for (int w = 0; w < kComputeWarps; ++w) evm = max(evm, sh.wvmax[w]);
+          const int enew = evm > eref ? evm + 2 : eref;
+          const float fe = pow2i(eref - enew);
+          float f[8];
 #pragma unroll
           for (int j = 0; j < 8; ++j) {
-            float x = tok_ok ? sv[j] * score_scale : -INFINITY;
+            float m = sh.wmax[4 * hh][j];
 #pragma unroll
-            for (int o = 16; o; o >>= 1) x = fmaxf(x, __shfl_xor_sync(kFull, x, o));
-            tm[j] = x;
+            for (int w = 1; w < 4; ++w) m = fmaxf(m, sh.wmax[4 * hh + w][j]);
+            const float mnew = fmaxf(mref[j], m);
+            const float fm = (mref[j] == -INFINITY) ? 0.f : ex2(mref[j] - mnew);
+            mref[j] = mnew;
+            lsum[j] *= fm;
+            f[j] = fm * fe;
           }
-        }
-        if (lane == 0) {
+          eref = enew;
+          if (i > 0) {  // every PV of this unit issued so far has to be in O before it is rescaled
+            mbar_wait(bar_done + 8 * (sb ^ 1), ((gt - 1) >> 1) & 1);
+            tc_fence_after();
+            float ov[8];
+            const uint32_t t_o = tmem + lane_sel + kColO + 8 * hh;   // channel r, heads 8hh..8hh+7
+            tmem_ld8(t_o, ov);
 #pragma unroll
-          for (int j = 0; j < 8; ++j) sh.wmax[cw][j] = tm[j];
-          sh.wvmax[cw] = vmax;
+            for (int j = 0; j < 8; ++j) ov[j] *= f[j];
+            tmem_st8(t_o, ov);
+          }
+          (void)softmax_pass();
+          (void)v_multipliers<true>(rest0, scratch, lane, g, tok_left, eref);
+          bar_compute();                                // wmax / wvmax may be rewritten only after every warp read them
         }
+#pragma unroll
+        for (int j = 0; j < 8; ++j) lsum[j] += lt[j];
+
+        // ---- S has been read: the QK warp may overwrite this S buffer (global tile gt+2)
         tc_fence_before();
-        bar_compute();
-        int evm = 0;
-#pragma unroll
-        for (int w = 0; w < kComputeWarps; ++w) evm = max(evm, sh.wvmax[w]);
-        const int enew = evm > eref ? evm + 2 : eref;
-        const float fe = pow2i(eref - enew);
-        float f[8];
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_sfree + 8 * sb);
+
+        // ---- V codes -> Vhat^T in TMEM buffer gt&1
+        v_convert(rest0, scratch, t_v + 64 * (sb % kVBufs), lane, g);
+        fence_async_smem();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) {
+          mbar_arrive(bar_ready);
+          mbar_arrive(bar_empty + 8 * s);              // this warp is done with the stage's V codes and scales
+        }
+
+        ++gt;
+        if (++s == kStages) { s = 0; ph_full ^= 1; }
+      }
+
+      // ================================================================ the unit's partial
+      mbar_wait(bar_done + 8 * ((gt - 1) & 1), ((gt - 1) >> 1) & 1);
+      tc_fence_after();
+      {
+        float ov[8];
+        tmem_ld8(tmem + lane_sel + kColO + 8 * hh, ov);
+        const float vscale = pow2i(eref - 13 - 127);    // stored Vhat = code * 2^(byte - eref + 13)
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
-          float m = sh.wmax[4 * hh][j];
-#pragma unroll
-          for (int w = 1; w < 4; ++w) m = fmaxf(m, sh.wmax[4 * hh + w][j]);
-          const float mnew = fmaxf(mref[j], m);
-          const float fm = (mref[j] == -INFINITY) ? 0.f : ex2(mref[j] - mnew);
-          mref[j] = mnew;
-          lsum[j] *= fm;
-          f[j] = fm * fe;
+          const int head = 8 * hh + j;
+          if (head < G) partial_acc[(un.row0 + (long long)head * num_splits) * kHeadDim + r] = ov[j] * vscale;
         }
-        eref = enew;
-        if (i > 0) {  // every PV issued so far has to be in O before it is rescaled
-          mbar_wait(bar_done + 8 * ((i - 1) & 1), ((i - 1) >> 1) & 1);
-          tc_fence_after();
-          float ov[8];
-          const uint32_t t_o = tmem + lane_sel + kColO + 8 * hh;   // channel r, heads 8hh..8hh+7
-          tmem_ld8(t_o, ov);
-#pragma unroll
-          for (int j = 0; j < 8; ++j) ov[j] *= f[j];
-          tmem_st8(t_o, ov);
-        }
-        (void)softmax_pass();
-        (void)v_multipliers<true>(rest0, scratch, lane, g, tok_left, eref);
-        bar_compute();                                  // wmax / wvmax may be rewritten only after every warp read them
       }
 #pragma unroll
-      for (int j = 0; j < 8; ++j) lsum[j] += lt[j];
-
-      // ---- S has been read: the QK warp may overwrite this S buffer (tile i+2)
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(bar_sfree + 8 * sb);
-
-      // ---- V codes -> Vhat^T in TMEM buffer i&1
-      TRACE(2 + cw, 5, i);
-      v_convert(rest0, scratch, t_v + 64 * sb, lane, g);
-      TRACE(2 + cw, 6, i);
-      fence_async_smem();
-      tc_fence_before();
-      __syncwarp();
+      for (int j = 0; j < 8; ++j) {
+        float v = lsum[j];
+#pragma unroll
+        for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+        lsum[j] = v;
+      }
       if (lane == 0) {
-        mbar_arrive(bar_ready);
-        mbar_arrive(bar_empty + 8 * s);                // this warp is done with the stage's V codes and scales
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          sh.lsum[cw][j] = lsum[j];
+          if (q == 0) sh.mref[8 * hh + j] = mref[j];
+        }
       }
-
-      if (++s == kStages) { s = 0; ph_full ^= 1; }
-    }
-
-    // ================================================================ epilogue: write the split's partial
-    mbar_wait(bar_done + 8 * ((n_tiles - 1) & 1), ((n_tiles - 1) >> 1) & 1);
-    tc_fence_after();
-    {
-      float ov[8];
-      tmem_ld8(tmem + lane_sel + kColO + 8 * hh, ov);
-      const float vscale = pow2i(eref - 13 - 127);      // stored Vhat = code * 2^(byte - eref + 13)
+      tc_fence_before();
+      bar_compute();
+      if (ctid < G) {                                  // one thread per query head
+        const int h2 = ctid >> 3, j = ctid & 7;
+        float l = 0.f;
 #pragma unroll
-      for (int j = 0; j < 8; ++j) {
-        const int head = 8 * hh + j;
-        if (head < G) partial_acc[(row0 + (long long)head * num_splits) * kHeadDim + r] = ov[j] * vscale;
+        for (int w = 0; w < 4; ++w) l += sh.lsum[4 * h2 + w][j];
+        ml_out[un.row0 + (long long)ctid * num_splits] = make_float2(sh.mref[ctid] * 0.6931471805599453f, l);   // natural log
       }
-    }
-#pragma unroll
-    for (int j = 0; j < 8; ++j) {
-      float v = lsum[j];
-#pragma unroll
-      for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
-      lsum[j] = v;
-    }
-    if (lane == 0) {
-#pragma unroll
-      for (int j = 0; j < 8; ++j) {
-        sh.lsum[cw][j] = lsum[j];
-        if (q == 0) sh.mref[8 * hh + j] = mref[j];
+      if (un.slots_used > 0) {                         // item finished: its remaining slots are empty
+        const long long row_item = un.row0 - (un.slots_used - 1);
+        const int n_empty = num_splits - un.slots_used;
+        for (int e = ctid; e < G * n_empty; e += 32 * kComputeWarps) {
+          const int head = e / n_empty, sl = un.slots_used + (e - head * n_empty);
+          ml_out[row_item + (long long)head * num_splits + sl] = make_float2(-INFINITY, 0.f);
+        }
       }
-    }
-    bar_compute();
-    const int head = tid - 32 * kIssuerWarps;          // first compute threads: one per query head
-    if (head < G) {
-      const int h2 = head >> 3, j = head & 7;
-      float l = 0.f;
-#pragma unroll
-      for (int w = 0; w < 4; ++w) l += sh.lsum[4 * h2 + w][j];
-      float2* ml = reinterpret_cast<float2*>(partial_ml) + row0 + (long long)head * num_splits;
-      *ml = make_float2(sh.mref[head] * 0.6931471805599453f, l);  // natural-log units
+      bar_compute();                                    // sh.lsum / sh.mref are reused by the next unit
     }
   }
 
   // ---------------- teardown
-#ifdef UQ_TRACE
-  if (trace_on && lane == 0) {
-    const int role = warp;
-    for (int k = 0; k < tr_n; ++k)
-      g_trace[role][k] = ((long long)(tr_buf[role][k].x >> 16) << 56) | ((long long)(tr_buf[role][k].x & 0xFFFF) << 40) | tr_buf[role][k].y;
-    g_trace_n[role] = tr_n;
-  }
-#endif
   tc_fence_before();
   __syncthreads();
   if (warp == 1) {
@@ -752,19 +889,37 @@ int32_t k_code_map(const void* cache, long long records, CUtensorMap* out) {
   return UQ_OK;
 }
 
+// 2-D view of q_fp8 for TMA: [batch * Hq rows][128 bytes]; box = 16 rows (the heads of one kv head, padded).
+int32_t q_map(const void* q_fp8, long long rows, CUtensorMap* out) {
+  std::lock_guard<std::mutex> lock(g_map_mu);
+  static EncodeTiledFn encode = nullptr;
+  if (!encode) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess || fn == nullptr) {
+      set_error("decode: cuTensorMapEncodeTiled is not available from this driver");
+      return UQ_ERR_CUDA;
+    }
+    encode = (EncodeTiledFn)fn;
+  }
+  const cuuint64_t gdim[2] = {128, (cuuint64_t)rows};
+  const cuuint64_t gstr[1] = {128};
+  const cuuint32_t box[2] = {128, 16};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult cr = encode(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(q_fp8), gdim, gstr, box, estr,
+                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (cr != CUDA_SUCCESS) {
+    set_error("decode: cuTensorMapEncodeTiled (q_fp8) failed with CUresult %d", (int)cr);
+    return UQ_ERR_CUDA;
+  }
+  return UQ_OK;
+}
+
 }  // namespace
 }  // namespace uq
 
-#ifdef UQ_TRACE
-extern "C" int32_t uq_debug_trace(long long* out /* host [10][4096] */, int* n /* host [10] */) {
-  cudaDeviceSynchronize();
-  cudaMemcpyFromSymbol(out, uq::g_trace, sizeof(long long) * 10 * 4096);
-  cudaMemcpyFromSymbol(n, uq::g_trace_n, sizeof(int) * 10);
-  int z[10] = {0};
-  cudaMemcpyToSymbol(uq::g_trace_n, z, sizeof(z));
-  return 0;
-}
-#endif
 
 extern "C" int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, const void* cache,
                                        int64_t num_pages, const int32_t* block_tables, int32_t max_pages,
@@ -776,10 +931,6 @@ extern "C" int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, 
   if (!q_fp8 || !cache || !block_tables || !seq_lens || !partial_acc || !partial_ml || batch <= 0 ||
       num_splits <= 0 || max_pages <= 0 || num_pages <= 0) {
     set_error("decode: NULL pointer or non-positive size");
-    return UQ_ERR_INVALID_ARG;
-  }
-  if (batch > 65535 || cfg->num_kv_heads > 65535) {
-    set_error("decode: batch and num_kv_heads must be <= 65535");
     return UQ_ERR_INVALID_ARG;
   }
   if (((uintptr_t)cache & 31u) || ((uintptr_t)q_fp8 & 15u) || ((uintptr_t)partial_acc & 15u) ||
@@ -795,8 +946,25 @@ extern "C" int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, 
   CUtensorMap tmap;
   st = k_code_map(cache, records, &tmap);
   if (st != UQ_OK) return st;
+  CUtensorMap tmap_q;
+  st = q_map(q_fp8, (long long)batch * cfg->num_q_heads, &tmap_q);
+  if (st != UQ_OK) return st;
   const float score_scale = resolved_sm_scale(cfg) * 1.4426950408889634f;
-  const dim3 grid((unsigned)num_splits, (unsigned)cfg->num_kv_heads, (unsigned)batch);
+  if (batch > kMaxBatch) {
+    set_error("decode: batch %d exceeds the supported maximum of %d sequences per call", batch, kMaxBatch);
+    return UQ_ERR_UNSUPPORTED;
+  }
+  static int sm_count = 0;
+  if (sm_count == 0) {
+    int dev = 0, v = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) sm_count = v;
+    else sm_count = 148;
+  }
+  const long long slots = (long long)sm_count * UQ_CTAS_PER_SM;
+  const long long items = (long long)batch * cfg->num_kv_heads;
+  // num_splits == 1: a CTA per item (round-robin beyond the resident set); otherwise one balanced tile range per CTA
+  const dim3 grid((unsigned)((num_splits == 1 && items < slots) ? items : slots));
   static bool attr_set = false;
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
@@ -804,7 +972,7 @@ extern "C" int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, 
     attr_set = true;
   }
   decode_kernel<<<grid, kThreads, kSmemBytes, (cudaStream_t)stream>>>(
-      tmap, (const uint8_t*)q_fp8, (const uint8_t*)cache, block_tables, max_pages, seq_lens, cfg->num_q_heads,
+      tmap, tmap_q, (const uint8_t*)cache, block_tables, max_pages, seq_lens, batch, cfg->num_q_heads,
       cfg->num_kv_heads, num_splits, score_scale, partial_acc, partial_ml);
   return check_cuda(cudaGetLastError(), "uq_decode_attention launch");
 }
