@@ -2,8 +2,10 @@
 // l.7-8 of arxiv/paper_2606_20474 (Eq.(1) :104).  Paging / split-K / partial
 // format follow include/uq.h.
 //
-// Design: one CTA per (sequence, kv head, split); the split is walked in
-// tiles of 128 tokens (8 pages).  Warp roles (352 threads).  Every async instruction (TMA copy,
+// Design: the 128-token tiles (8 pages) of all (sequence, kv head) items form one
+// sequence that is cut into equal contiguous ranges, one per resident CTA (one wave, 2 CTAs per SM); a
+// range is walked as units (item, tile range), each unit writing one partial slot of its item.
+// Warp roles (352 threads).  Every async instruction (TMA copy,
 // tcgen05.mma / cp / commit) occupies its issuing warp for ~55 cycles (measured), so the 16 copies and
 // 12 MMAs of a tile are spread over three issuer warps:
 //   warp 2  TMA producer: per page one TMA tensor copy of the packed FP4 K codes
@@ -24,7 +26,7 @@
 //           into TMEM, where the PV MMA reads it as its A operand (no shared-memory round trip:
 //           the kernel is shared-memory-bandwidth sensitive); the PV MMAs of a tile run under the
 //           softmax of the next one.
-// The FP8 query tile is written to smem once per CTA ("hoisted").
+// The FP8 query tile is copied to smem by TMA once per unit ("hoisted").
 // Every K/V byte is read from HBM exactly once.
 #include <cuda.h>
 #include <cuda_fp16.h>
