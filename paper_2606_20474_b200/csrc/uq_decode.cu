@@ -32,13 +32,15 @@
 #include <cuda_fp16.h>
 
 #include <mutex>
+#include <type_traits>
 
 #include "uq_common.cuh"
 
 namespace uq {
 namespace {
 
-constexpr int kComputeWarps = 8;                     // two per TMEM lane quarter
+constexpr int kComputeWarps = 8;                     // two per TMEM lane quarter: one softmax warp, one V warp
+constexpr int kSoftmaxWarps = 4;
 constexpr int kIssuerWarps = 3;                      // QK issuer, PV issuer, TMA producer
 constexpr int kThreads = (kComputeWarps + kIssuerWarps) * 32;
 #ifndef UQ_STAGES
@@ -62,7 +64,7 @@ constexpr int kOffQ = kOffStage + kStages * kStageBytes;       // 2 x 2048, SW12
 constexpr int kOffSFA = kOffQ + 4096;                          // 2 x 512
 constexpr int kOffSFB = kOffSFA + 1024;                        // 512
 constexpr int kOffP = kOffSFB + 512;                           // 2 x 4096 (double-buffered)
-constexpr int kOffMul = kOffP + 2 * kPBytes;                   // 8 warps x 128 B
+constexpr int kOffMul = kOffP + 2 * kPBytes;                   // 4 V warps x 256 B of fp16 multipliers
 constexpr int kOffEnd = kOffMul + kComputeWarps * 128;
 constexpr int kSmemBytes = kOffEnd + 1024;                     // + alignment slack
 
@@ -155,11 +157,11 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm,
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void bar_compute() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
-// barrier over the 256 compute threads that also ORs a predicate across them
-__device__ __forceinline__ bool bar_compute_or(bool pred) {
+__device__ __forceinline__ void bar_softmax() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
+// barrier over the 128 softmax threads that also ORs a predicate across them
+__device__ __forceinline__ bool bar_softmax_or(bool pred) {
   uint32_t r;
-  asm volatile("{\n.reg .pred p, q;\nsetp.ne.b32 q, %1, 0;\nbar.red.or.pred p, 1, 256, q;\nselp.u32 %0, 1, 0, p;\n}\n"
+  asm volatile("{\n.reg .pred p, q;\nsetp.ne.b32 q, %1, 0;\nbar.red.or.pred p, 1, 128, q;\nselp.u32 %0, 1, 0, p;\n}\n"
                : "=r"(r) : "r"((uint32_t)pred) : "memory");
   return r != 0;
 }
@@ -194,30 +196,38 @@ __device__ __forceinline__ void umma_f16(uint32_t d, uint64_t da, uint64_t db, u
       "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}\n"
       ::"r"(d), "l"(da), "l"(db), "r"(idesc), "r"(acc) : "memory");
 }
-__device__ __forceinline__ void tmem_ld8(uint32_t taddr, float (&v)[8]) {
-  uint32_t r[8];
-  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
-               : "r"(taddr));
+// N consecutive 32-bit columns of this thread's TMEM lane <-> registers (N = 8 or 16), complete on return
+template <int N>
+__device__ __forceinline__ void tmem_ld(uint32_t taddr, float (&v)[N]) {
+  static_assert(N == 8 || N == 16, "tmem_ld: 8 or 16 columns");
+  uint32_t r[N];
+  if constexpr (N == 8) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "r"(taddr));
+  } else {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+                   "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+                 : "r"(taddr));
+  }
   asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
-  for (int j = 0; j < 8; ++j) v[j] = __uint_as_float(r[j]);
+  for (int j = 0; j < N; ++j) v[j] = __uint_as_float(r[j]);
 }
-__device__ __forceinline__ void tmem_st8(uint32_t taddr, const float (&v)[8]) {
+template <int N>
+__device__ __forceinline__ void tmem_st(uint32_t taddr, const float (&v)[N]) {
+  static_assert(N == 8 || N == 16, "tmem_st: 8 or 16 columns");
   asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
                ::"r"(taddr), "r"(__float_as_uint(v[0])), "r"(__float_as_uint(v[1])), "r"(__float_as_uint(v[2])),
                  "r"(__float_as_uint(v[3])), "r"(__float_as_uint(v[4])), "r"(__float_as_uint(v[5])),
                  "r"(__float_as_uint(v[6])), "r"(__float_as_uint(v[7])) : "memory");
-  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32]) {
-  asm volatile(
-      "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"
-      "%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"
-      ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]),
-        "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]), "r"(v[16]), "r"(v[17]),
-        "r"(v[18]), "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]), "r"(v[24]), "r"(v[25]), "r"(v[26]),
-        "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31]) : "memory");
+  if constexpr (N == 16) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                 ::"r"(taddr + 8), "r"(__float_as_uint(v[8])), "r"(__float_as_uint(v[9])), "r"(__float_as_uint(v[10])),
+                   "r"(__float_as_uint(v[11])), "r"(__float_as_uint(v[12])), "r"(__float_as_uint(v[13])),
+                   "r"(__float_as_uint(v[14])), "r"(__float_as_uint(v[15])) : "memory");
+  }
   asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
 __device__ __forceinline__ void tmem_st16_nowait(uint32_t taddr, const uint32_t (&v)[16]) {
@@ -271,67 +281,19 @@ __device__ __forceinline__ float pow2i(int e) {   // 2^e, flushing to 0 below th
 struct Shared {
   uint64_t full[kStages];     // producer (expect_tx) + TMA bytes -> QK warp, compute warps
   uint64_t empty[kStages];    // 8 compute warps + QK commit -> producer
-  uint64_t s_full[2];         // QK commit -> compute warps
+  uint64_t s_full[2];         // QK(gt) commit + PV(gt-2) commit -> compute warps: S is there, P / Vhat buffers are free
   uint64_t s_free[2];         // 8 compute warps -> QK warp: S buffer read, may be overwritten
-  uint64_t ready;             // 8 compute warps -> PV warp: P (smem) and Vhat (TMEM) of the tile are written
+  uint64_t ready[2];          // 4 softmax + 4 V warps -> PV warp: P (smem) and Vhat (TMEM) buffer gt&1 are written
+                              // (two barriers: a V warp may be one tile ahead of the softmax warps)
   uint64_t done[2];           // PV commit of tile i -> done[i&1]: P / Vhat buffer i&1 free, O up to date
   uint64_t q_full[2];         // TMA: the FP8 query tile of a work unit landed (buffer = unit ordinal & 1)
   uint32_t tmem_base;
-  float wmax[kComputeWarps][8];
-  int wvmax[kComputeWarps];
-  float lsum[kComputeWarps][8];
+  float wmax[kSoftmaxWarps][16];
+  float lsum[kSoftmaxWarps][16];
   float mref[16];
   int total_tiles, max_tiles;  // sum (x kv heads) and max over sequences of the tiles per (sequence, kv head)
   int pre[kMaxBatch + 1];      // pre[b] = tiles of sequences 0..b-1 (per kv head)
 };
-
-// This warp's share of the tile's V: channel group g (= its TMEM lane quarter), tokens
-// 64*hf .. 64*hf+63 (pages 4*hf .. 4*hf+3 of the tile).  rest0 = [V codes | K scales | V scales]
-// block of page 4*hf in the stage.
-// Step 1: the 64 scale bytes -> 32 fp16 power-of-two multipliers (one f16x2 per token pair) in the
-// warp's scratch; returns the largest scale byte among the valid tokens (warp-uniform).
-template <bool kPartial>
-__device__ __forceinline__ int v_multipliers(uint32_t rest0, uint32_t scratch, int lane, int g, int tok_left, int eref) {
-  const int pl = lane >> 3, hk = (lane >> 2) & 1, bp = lane & 3;     // page, half of the page, token pair
-  uint32_t pair;
-  asm volatile("ld.shared.u16 %0, [%1];" : "=r"(pair) : "r"(rest0 + kRestBytes * pl + 1088 + 32 * hk + 8 * g + 2 * bp));
-  int lo = (int)(pair & 0xFFu), hi = (int)(pair >> 8);
-  if (kPartial) {                                    // tok_left = valid tokens from the first token of this warp's range
-    const int tok = 16 * pl + 8 * hk + 2 * bp;
-    if (tok >= tok_left) lo = 0;
-    if (tok + 1 >= tok_left) hi = 0;
-  }
-  const int vmax = __reduce_max_sync(kFull, max(lo, hi));
-  const int kbase = eref - 28;                       // fp16 exponent field = byte - kbase (2^13 at byte = eref)
-  const uint32_t mlo = (uint32_t)max(lo - kbase, 0), mhi = (uint32_t)max(hi - kbase, 0);   // byte 0 -> multiplier 0
-  asm volatile("st.shared.u32 [%0], %1;" ::"r"(scratch + 4 * lane), "r"((mlo << 10) | (mhi << 26)) : "memory");
-  __syncwarp();
-  return vmax;
-}
-
-// Step 2: 64 tokens of channel d = 32 g + lane -> fp16 x multiplier -> TMEM (A operand of the PV
-// MMA: lane = channel, column c = tokens 2c, 2c+1).
-__device__ __forceinline__ void v_convert(uint32_t rest0, uint32_t scratch, uint32_t t_dst, int lane, int g) {
-#pragma unroll
-  for (int h = 0; h < 2; ++h) {                      // 32 tokens (16 TMEM columns) at a time
-    uint32_t o[16];
-#pragma unroll
-    for (int kk = 0; kk < 4; ++kk) {                 // token-core k: page k>>1, half k&1 -> 8 tokens
-      const int k = 4 * h + kk;
-      uint32_t cw;
-      asm volatile("ld.shared.u32 %0, [%1];" : "=r"(cw) : "r"(rest0 + kRestBytes * (k >> 1) + 512 * (k & 1) + 128 * g + 4 * lane));
-      const uint4 m4 = lds128(scratch + 16 * k);
-      uint32_t f[4];
-      cvt_e2m1x8(cw, f);
-      o[4 * kk + 0] = hmul2(f[0], m4.x);
-      o[4 * kk + 1] = hmul2(f[1], m4.y);
-      o[4 * kk + 2] = hmul2(f[2], m4.z);
-      o[4 * kk + 3] = hmul2(f[3], m4.w);
-    }
-    tmem_st16_nowait(t_dst + 16 * h, o);
-  }
-  tmem_wait_st();
-}
 
 // ---------------------------------------------------------------- work schedule
 // The tiles (128 tokens) of all (sequence, kv head) items form one sequence, item after item.  With
@@ -433,7 +395,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
   const uint32_t sQ = base + kOffQ, sSFA = base + kOffSFA, sSFB = base + kOffSFB, sP = base + kOffP;
   const uint32_t bar_full = smem_u32(&sh.full[0]), bar_empty = smem_u32(&sh.empty[0]),
                  bar_sfull = smem_u32(&sh.s_full[0]), bar_sfree = smem_u32(&sh.s_free[0]),
-                 bar_ready = smem_u32(&sh.ready), bar_done = smem_u32(&sh.done[0]),
+                 bar_ready = smem_u32(&sh.ready[0]), bar_done = smem_u32(&sh.done[0]),
                  bar_qfull = smem_u32(&sh.q_full[0]);
 
   // ---------------- setup
@@ -441,16 +403,18 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
 #pragma unroll
     for (int s = 0; s < kStages; ++s) {
       mbar_init(bar_full + 8 * s, 1);
-      mbar_init(bar_empty + 8 * s, kComputeWarps + 1);
+      mbar_init(bar_empty + 8 * s, (kComputeWarps - kSoftmaxWarps) + 1);
     }
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
-      mbar_init(bar_sfull + 8 * h, 1);
-      mbar_init(bar_sfree + 8 * h, kComputeWarps);
+      mbar_init(bar_sfull + 8 * h, 2);
+      mbar_init(bar_sfree + 8 * h, kSoftmaxWarps);
       mbar_init(bar_done + 8 * h, 1);
       mbar_init(bar_qfull + 8 * h, 1);
+      mbar_init(bar_ready + 8 * h, kComputeWarps);
     }
-    mbar_init(bar_ready, kComputeWarps);
+#pragma unroll
+    for (int h = 0; h < 2; ++h) mbar_arrive(bar_sfull + 8 * h);   // global tiles 0 and 1 have no PV(gt-2)
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {
@@ -507,7 +471,8 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     // (unit ordinal & 1) — "hoisted", once per unit; rows past the unit's G heads belong to
     // the next kv head (or are zero past the tensor end) and only feed score columns nobody reads.
     // Per tile: S(gt)[128 tok x 16 heads] = K . Q^T once the tile's bytes have landed, the S buffer was read
-    // by the softmax of global tile gt-2 and PV(gt-2) has read the P / Vhat buffers gt&1.
+    // by the softmax of global tile gt-2.  (PV(gt-2), which frees the P / Vhat buffers gt&1, is the second
+    // arrival of s_full: it is not on this warp's path.)
     const uint32_t idesc_qk = (5u << 7) | (0u << 10) | (2u << 17) | (1u << 23) | (8u << 24);   // E2M1 x E4M3, UE8M0, N=16, M=128
     if (lane == 0) umma_cp_sf(tmem + kColSFB, make_desc(sSFB, 16, 128, 0));
     auto load_q = [&](const Unit& un, int k) {         // lane 0: Q tile of unit ordinal k
@@ -528,10 +493,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
       have_nx = sc.next(cur_nx, nx);
       for (int i = 0; i < un.n_tiles; ++i) {
         const int sb = gt & 1;
-        if (gt >= 2) {
-          mbar_wait(bar_sfree + 8 * sb, ((gt >> 1) - 1) & 1);
-          mbar_wait(bar_done + 8 * sb, ((gt >> 1) - 1) & 1);
-        }
+        if (gt >= 2) mbar_wait(bar_sfree + 8 * sb, ((gt >> 1) - 1) & 1);
         // here every QK up to global tile gt-2 has completed (its S was read): at i == 0 the Q buffer of
         // unit k-2 (= buffer k & 1), at i == 1 that of unit k-1 (= buffer (k+1) & 1) may be refilled
         if (i == 0 && k_q < k) { load_q(un, k); k_q = k; }
@@ -576,7 +538,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     int gt = 0;
     while (sc.next(cur, un)) {
       for (int i = 0; i < un.n_tiles; ++i, ++gt) {
-        mbar_wait(bar_ready, gt & 1);
+        mbar_wait(bar_ready + 8 * (gt & 1), (gt >> 1) & 1);
         tc_fence_after();
         if (lane == 0) {
           const uint32_t pbuf = sP + kPBytes * (gt & 1), vbuf = tmem + kColV + 64 * ((gt & 1) % kVBufs);
@@ -585,6 +547,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
             umma_f16_ts(tmem + kColO, vbuf + 8 * j, make_desc(pbuf + 512 * j, 256, 128, 0), idesc_pv,
                         (i > 0 || j > 0) ? 1u : 0u);
           umma_commit(bar_done + 8 * (gt & 1));
+          umma_commit(bar_sfull + 8 * (gt & 1));       // second arrival of S(gt+2)'s phase: P / Vhat buffers gt&1 are free
         }
         __syncwarp();
       }
@@ -620,211 +583,287 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     }
   } else {
     // ================================================================ compute warps (warp ids 3..10)
-    // The three issuer warps sit on the lowest warp ids so that the scheduler's highest-warp-id-first
-    // arbitration favours the compute warps.
+    // Two role-pure groups of four warps, one warp of each per TMEM lane quarter (hardware: warp id % 4):
+    //   softmax warps (3..6):  thread = token row of the tile, all query heads of the kv head;
+    //   V warps (7..10):       thread = channel d, all 128 tokens of the tile.
+    // A V warp needs the tile's bytes but not its scores, so it may run ahead of the softmax warps; the
+    // two groups meet only at the `ready` barrier of the PV warp.  The issuer warps sit on the lowest
+    // warp ids so that the scheduler's highest-warp-id-first arbitration favours the compute warps.
     const int cw = warp - kIssuerWarps;                // 0..7
-    const int ctid = tid - 32 * kIssuerWarps;          // 0..255
-    const int q = warp & 3, hh = cw >> 2;              // TMEM lane quarter (hardware: warp id % 4), head half
-    const int r = 32 * q + lane;                       // softmax: token row of the tile; epilogue: channel d
-    const bool heads_live = (8 * hh < G);
-    const uint32_t scratch = base + kOffMul + 128 * cw;
+    const int q = warp & 3;                            // TMEM lane quarter
     const uint32_t lane_sel = (uint32_t)(32 * q) << 16;
-    const int g = q, hf = hh;                          // V conversion: channel group (= lane quarter), token half of the tile
-    const uint32_t t_v = tmem + lane_sel + kColV + 32 * hf;
-    float2* const ml_out = reinterpret_cast<float2*>(partial_ml);
+    const int r = 32 * q + lane;                       // softmax: token row of the tile; V warps: channel d
 
-    // items without any token: all their slots are empty, (m, l) = (-inf, 0)
-    for (int it = blockIdx.x; it < batch * Hkv; it += gridDim.x) {
-      const int b = it / Hkv;
-      if (sc.tiles(b) == 0) {
-        const long long row = ((long long)b * Hq + (long long)(it - b * Hkv) * G) * num_splits;
-        for (int e = ctid; e < G * num_splits; e += 32 * kComputeWarps) ml_out[row + e] = make_float2(-INFINITY, 0.f);
-      }
-    }
+    if (cw < kSoftmaxWarps) {
+      // ============================================================== softmax warps
+      const int atid = tid - 32 * kIssuerWarps;        // 0..127
+      float2* const ml_out = reinterpret_cast<float2*>(partial_ml);
 
-    Cursor cur;
-    sc.start(cur);
-    Unit un;
-    int gt = 0, s = 0, ph_full = 0;                    // global tile counter, its stage and full-barrier parity
-    while (sc.next(cur, un)) {
-      float mref[8], lsum[8];
-#pragma unroll
-      for (int j = 0; j < 8; ++j) { mref[j] = -INFINITY; lsum[j] = 0.f; }
-      int eref = 28;
-
-      for (int i = 0; i < un.n_tiles; ++i) {
-        const int sb = gt & 1, ph2 = (gt >> 1) & 1;
-        const uint32_t rest0 = base + kOffStage + s * kStageBytes + 16384 + kRestBytes * (4 * hf);
-        const int pg0 = un.p0 + kTilePages * i;                        // first page of the tile
-        const bool tile_partial = (pg0 + kTilePages) * kPage > un.tok_end;
-        const bool tok_ok = pg0 * kPage + r < un.tok_end;
-        const int tok_left = un.tok_end - (pg0 * kPage + 64 * hf);   // valid tokens in this warp's 64-token half
-        const uint32_t t_s = tmem + lane_sel + kColS + 16 * sb + 8 * hh;
-        const uint32_t p_addr = sP + kPBytes * sb + (r >> 3) * 256 + hh * 128 + (r & 7) * 16;
-
-        mbar_wait(bar_sfull + 8 * sb, ph2);                            // S of the tile is in TMEM
-        tc_fence_after();
-        (void)mbar_test(bar_full + 8 * s, ph_full);                    // complete (QK consumed it): acquire the TMA bytes
-        // PV(gt-2) is complete as well (the QK warp waited for it before S(gt)): P / Vhat buffers gt&1 are free
-
-        float lt[8];
-        // softmax of this thread's row against the current references -> P (fp16, MN-major operand)
-        auto softmax_pass = [&]() -> bool {
-#pragma unroll
-          for (int j = 0; j < 8; ++j) lt[j] = 0.f;
-          if (!heads_live) return false;
-          float t[8];
-          tmem_ld8(t_s, t);
-#pragma unroll
-          for (int j = 0; j < 8; ++j) t[j] = fmaf(t[j], score_scale, -mref[j]);
-          if (tile_partial) {
-#pragma unroll
-            for (int j = 0; j < 8; ++j) t[j] = tok_ok ? t[j] : -INFINITY;
-          }
-          const float tmax = fmaxf(fmaxf(fmaxf(t[0], t[1]), fmaxf(t[2], t[3])), fmaxf(fmaxf(t[4], t[5]), fmaxf(t[6], t[7])));
-#pragma unroll
-          for (int j = 0; j < 8; ++j) lt[j] = ex2(t[j]);
-          uint4 o;
-          asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.x) : "f"(lt[1]), "f"(lt[0]));
-          asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.y) : "f"(lt[3]), "f"(lt[2]));
-          asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.z) : "f"(lt[5]), "f"(lt[4]));
-          asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.w) : "f"(lt[7]), "f"(lt[6]));
-          sts128(p_addr, o);
-          return tmax > kThresh;
-        };
-
-        bool rebase = (i == 0);
-        int vmax = 0;
-        if (!rebase) {
-          const bool ex = softmax_pass();
-          vmax = tile_partial ? v_multipliers<true>(rest0, scratch, lane, g, tok_left, eref)
-                              : v_multipliers<false>(rest0, scratch, lane, g, tok_left, eref);
-          tc_fence_before();
-          rebase = bar_compute_or(ex || vmax > eref);
+      // items without any token: all their slots are empty, (m, l) = (-inf, 0)
+      for (int it = blockIdx.x; it < batch * Hkv; it += gridDim.x) {
+        const int b = it / Hkv;
+        if (sc.tiles(b) == 0) {
+          const long long row = ((long long)b * Hq + (long long)(it - b * Hkv) * G) * num_splits;
+          for (int e = atid; e < G * num_splits; e += 32 * kSoftmaxWarps) ml_out[row + e] = make_float2(-INFINITY, 0.f);
         }
-        if (__builtin_expect(rebase, 0)) {
-          // ---- statistics of the tile: per-head maximum score, maximum V scale byte
-          vmax = v_multipliers<true>(rest0, scratch, lane, g, tok_left, eref);
-          float tm[8];
+      }
+
+      auto run = [&](auto nh_tag) {
+        constexpr int NH = decltype(nh_tag)::value;    // head columns this thread handles: 8 (G <= 8) or 16
+        Cursor cur;
+        sc.start(cur);
+        Unit un;
+        int gt = 0;                                    // global tile counter
+        const uint32_t p_row = sP + (r >> 3) * 256 + (r & 7) * 16;
+        while (sc.next(cur, un)) {
+          float mref[NH], lsum[NH];
 #pragma unroll
-          for (int j = 0; j < 8; ++j) tm[j] = -INFINITY;
-          if (heads_live) {
-            float sv[8];
-            tmem_ld8(t_s, sv);
+          for (int j = 0; j < NH; ++j) { mref[j] = -INFINITY; lsum[j] = 0.f; }
+          int rem = un.tok_end - un.p0 * kPage;        // valid tokens from the first row of the tile on
+
+          for (int i = 0; i < un.n_tiles; ++i, rem -= kTilePages * kPage) {
+            const int sb = gt & 1, ph2 = (gt >> 1) & 1;
+            const bool tile_partial = rem < kTilePages * kPage;
+            const bool tok_ok = r < rem;
+            const uint32_t t_s = tmem + lane_sel + kColS + 16 * sb;
+            const uint32_t p_addr = p_row + kPBytes * sb;
+
+            mbar_wait(bar_sfull + 8 * sb, ph2);        // S(gt) is in TMEM and PV(gt-2) has read P buffer gt&1
+            tc_fence_after();
+
+            float lt[NH];
+            // softmax of this thread's row against the current references -> P (fp16, MN-major operand)
+            auto softmax_pass = [&]() -> bool {
+              float t[NH];
+              tmem_ld<NH>(t_s, t);
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-              float x = tok_ok ? sv[j] * score_scale : -INFINITY;
+              for (int j = 0; j < NH; ++j) t[j] = fmaf(t[j], score_scale, -mref[j]);
+              if (tile_partial) {
 #pragma unroll
-              for (int o = 16; o; o >>= 1) x = fmaxf(x, __shfl_xor_sync(kFull, x, o));
-              tm[j] = x;
+                for (int j = 0; j < NH; ++j) t[j] = tok_ok ? t[j] : -INFINITY;
+              }
+              float tmax = t[0];
+#pragma unroll
+              for (int j = 1; j < NH; ++j) tmax = fmaxf(tmax, t[j]);
+#pragma unroll
+              for (int j = 0; j < NH; ++j) lt[j] = ex2(t[j]);
+#pragma unroll
+              for (int c = 0; c < NH / 8; ++c) {
+                uint4 o;
+                asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.x) : "f"(lt[8 * c + 1]), "f"(lt[8 * c + 0]));
+                asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.y) : "f"(lt[8 * c + 3]), "f"(lt[8 * c + 2]));
+                asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.z) : "f"(lt[8 * c + 5]), "f"(lt[8 * c + 4]));
+                asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.w) : "f"(lt[8 * c + 7]), "f"(lt[8 * c + 6]));
+                sts128(p_addr + 128 * c, o);
+              }
+              return tmax > kThresh;
+            };
+
+            bool rebase = (i == 0);
+            if (!rebase) {
+              const bool ex = softmax_pass();
+              rebase = bar_softmax_or(ex);
             }
+            if (__builtin_expect(rebase, 0)) {
+              // ---- per-head maximum score of the tile -> new references; O and l rescaled
+              float tm[NH];
+              {
+                float sv[NH];
+                tmem_ld<NH>(t_s, sv);
+#pragma unroll
+                for (int j = 0; j < NH; ++j) {
+                  float x = tok_ok ? sv[j] * score_scale : -INFINITY;
+#pragma unroll
+                  for (int o = 16; o; o >>= 1) x = fmaxf(x, __shfl_xor_sync(kFull, x, o));
+                  tm[j] = x;
+                }
+              }
+              if (lane == 0) {
+#pragma unroll
+                for (int j = 0; j < NH; ++j) sh.wmax[cw][j] = tm[j];
+              }
+              tc_fence_before();
+              bar_softmax();
+              float f[NH];
+#pragma unroll
+              for (int j = 0; j < NH; ++j) {
+                float m = sh.wmax[0][j];
+#pragma unroll
+                for (int w = 1; w < kSoftmaxWarps; ++w) m = fmaxf(m, sh.wmax[w][j]);
+                const float mnew = fmaxf(mref[j], m);
+                const float fm = (mref[j] == -INFINITY) ? 0.f : ex2(mref[j] - mnew);
+                mref[j] = mnew;
+                lsum[j] *= fm;
+                f[j] = fm;
+              }
+              if (i > 0) {  // every PV of this unit issued so far has to be in O before it is rescaled
+                mbar_wait(bar_done + 8 * (sb ^ 1), ((gt - 1) >> 1) & 1);
+                tc_fence_after();
+                float ov[NH];
+                const uint32_t t_o = tmem + lane_sel + kColO;      // channel r, heads 0..NH-1
+                tmem_ld<NH>(t_o, ov);
+#pragma unroll
+                for (int j = 0; j < NH; ++j) ov[j] *= f[j];
+                tmem_st<NH>(t_o, ov);
+              }
+              (void)softmax_pass();
+              bar_softmax();                            // wmax may be rewritten only after every warp read it
+            }
+#pragma unroll
+            for (int j = 0; j < NH; ++j) lsum[j] += lt[j];
+
+            // ---- S has been read (QK may overwrite the buffer), P is written, O is consistent with mref
+            fence_async_smem();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) {
+              mbar_arrive(bar_sfree + 8 * sb);
+              mbar_arrive(bar_ready + 8 * sb);
+            }
+            ++gt;
+          }
+
+          // ============================================================ the unit's (m, l)
+#pragma unroll
+          for (int j = 0; j < NH; ++j) {
+            float v = lsum[j];
+#pragma unroll
+            for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+            lsum[j] = v;
           }
           if (lane == 0) {
 #pragma unroll
-            for (int j = 0; j < 8; ++j) sh.wmax[cw][j] = tm[j];
-            sh.wvmax[cw] = vmax;
+            for (int j = 0; j < NH; ++j) {
+              sh.lsum[cw][j] = lsum[j];
+              if (cw == 0) sh.mref[j] = mref[j];
+            }
           }
-          tc_fence_before();
-          bar_compute();
-          int evm = 0;
+          bar_softmax();
+          if (atid < G) {                              // one thread per query head
+            float l = 0.f;
 #pragma unroll
-          for (int w = 0; w < kComputeWarps; ++w) evm = max(evm, sh.wvmax[w]);
-          const int enew = evm > eref ? evm + 2 : eref;
-          const float fe = pow2i(eref - enew);
-          float f[8];
-#pragma unroll
-          for (int j = 0; j < 8; ++j) {
-            float m = sh.wmax[4 * hh][j];
-#pragma unroll
-            for (int w = 1; w < 4; ++w) m = fmaxf(m, sh.wmax[4 * hh + w][j]);
-            const float mnew = fmaxf(mref[j], m);
-            const float fm = (mref[j] == -INFINITY) ? 0.f : ex2(mref[j] - mnew);
-            mref[j] = mnew;
-            lsum[j] *= fm;
-            f[j] = fm * fe;
+            for (int w = 0; w < kSoftmaxWarps; ++w) l += sh.lsum[w][atid];
+            ml_out[un.row0 + (long long)atid * num_splits] = make_float2(sh.mref[atid] * 0.6931471805599453f, l);   // natural log
           }
-          eref = enew;
-          if (i > 0) {  // every PV of this unit issued so far has to be in O before it is rescaled
-            mbar_wait(bar_done + 8 * (sb ^ 1), ((gt - 1) >> 1) & 1);
+          if (un.slots_used > 0) {                     // item finished: its remaining slots are empty
+            const long long row_item = un.row0 - (un.slots_used - 1);
+            const int n_empty = num_splits - un.slots_used;
+            for (int e = atid; e < G * n_empty; e += 32 * kSoftmaxWarps) {
+              const int head = e / n_empty, sl = un.slots_used + (e - head * n_empty);
+              ml_out[row_item + (long long)head * num_splits + sl] = make_float2(-INFINITY, 0.f);
+            }
+          }
+          bar_softmax();                                // sh.lsum / sh.mref are reused by the next unit
+        }
+      };
+      if (G > 8) run(std::integral_constant<int, 16>{});
+      else run(std::integral_constant<int, 8>{});
+    } else {
+      // ============================================================== V warps
+      // Warp of lane quarter q converts channel group g = q (channels 32 q .. 32 q + 31 = one UE8M0 scale
+      // group of V): its reference exponent eref is its own, so the four V warps never have to agree on
+      // anything.  Stored Vhat = code * 2^(byte - eref + 13) in fp16, written straight into TMEM.
+      const int g = q;
+      const uint32_t scratch = base + kOffMul + 256 * (cw - kSoftmaxWarps);
+      const uint32_t t_o = tmem + lane_sel + kColO;    // channel r, heads 0..15
+      Cursor cur;
+      sc.start(cur);
+      Unit un;
+      int gt = 0, s = 0, ph_full = 0;                  // global tile counter, its stage and full-barrier parity
+      while (sc.next(cur, un)) {
+        int eref = 28;
+        int rem = un.tok_end - un.p0 * kPage;          // valid tokens from the first token of the tile on
+
+        for (int i = 0; i < un.n_tiles; ++i, rem -= kTilePages * kPage) {
+          const int sb = gt & 1;
+          const uint32_t rest = base + kOffStage + s * kStageBytes + 16384;   // [V codes | K scales | V scales] of page 0
+          mbar_wait(bar_full + 8 * s, ph_full);        // the tile's bytes have landed
+
+          // ---- the tile's 128 scale bytes of group g: lane <-> tokens 4 lane .. 4 lane + 3
+          uint32_t sw;
+          asm volatile("ld.shared.u32 %0, [%1];" : "=r"(sw)
+                       : "r"(rest + kRestBytes * (lane >> 2) + 1088 + 32 * ((lane >> 1) & 1) + 8 * g + 4 * (lane & 1)));
+          if (rem < kTilePages * kPage) {              // bytes of tokens past the end (stale shared memory) -> 0
+            const int nv = rem - 4 * lane;             // valid tokens among this lane's four
+            sw = nv >= 4 ? sw : (nv <= 0 ? 0u : (sw & (0xFFFFFFFFu >> (8 * (4 - nv)))));
+          }
+          const uint32_t mx2 = __vmaxu4(sw, sw >> 16);
+          const int vmax = __reduce_max_sync(kFull, (int)(__vmaxu4(mx2, mx2 >> 8) & 0xFFu));
+          if (__builtin_expect(vmax > eref, 0)) {      // warp-uniform
+            const int enew = vmax + 2;
+            if (i > 0) {
+              // O rows of this lane quarter change unit: after the softmax warps are through with the tile
+              // (their own rescale of O included) and every PV issued so far has landed
+              mbar_wait(bar_sfree + 8 * sb, (gt >> 1) & 1);
+              mbar_wait(bar_done + 8 * (sb ^ 1), ((gt - 1) >> 1) & 1);
+              tc_fence_after();
+              float ov[16];
+              tmem_ld<16>(t_o, ov);
+              const float fe = pow2i(eref - enew);
+#pragma unroll
+              for (int j = 0; j < 16; ++j) ov[j] *= fe;
+              tmem_st<16>(t_o, ov);
+            }
+            eref = enew;
+          }
+          {   // four fp16 power-of-two multipliers (two f16x2: token pairs 2 lane, 2 lane + 1); byte 0 -> 0
+            const int kbase = eref - 28;               // fp16 exponent field = byte - kbase (2^13 at byte = eref)
+            const uint32_t e0 = (uint32_t)max((int)(sw & 0xFFu) - kbase, 0), e1 = (uint32_t)max((int)((sw >> 8) & 0xFFu) - kbase, 0),
+                           e2 = (uint32_t)max((int)((sw >> 16) & 0xFFu) - kbase, 0), e3 = (uint32_t)max((int)(sw >> 24) - kbase, 0);
+            asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(scratch + 8 * lane), "r"((e0 << 10) | (e1 << 26)),
+                         "r"((e2 << 10) | (e3 << 26)) : "memory");
+          }
+          __syncwarp();
+
+          if (gt >= 2) {                               // PV(gt-2) has read Vhat buffer gt&1
+            mbar_wait(bar_done + 8 * sb, ((gt >> 1) - 1) & 1);
             tc_fence_after();
-            float ov[8];
-            const uint32_t t_o = tmem + lane_sel + kColO + 8 * hh;   // channel r, heads 8hh..8hh+7
-            tmem_ld8(t_o, ov);
-#pragma unroll
-            for (int j = 0; j < 8; ++j) ov[j] *= f[j];
-            tmem_st8(t_o, ov);
           }
-          (void)softmax_pass();
-          (void)v_multipliers<true>(rest0, scratch, lane, g, tok_left, eref);
-          bar_compute();                                // wmax / wvmax may be rewritten only after every warp read them
-        }
+          // ---- V codes -> Vhat^T in TMEM buffer gt&1: lane = channel, column c = tokens 2c, 2c+1
+          const uint32_t t_v = tmem + lane_sel + kColV + 64 * sb;
+          const uint32_t code0 = rest + 128 * g + 4 * lane;
 #pragma unroll
-        for (int j = 0; j < 8; ++j) lsum[j] += lt[j];
+          for (int h = 0; h < 4; ++h) {                // 32 tokens (16 TMEM columns) at a time
+            uint32_t o[16];
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk) {           // token octet k: page k>>1, half k&1
+              const int k = 4 * h + kk;
+              uint32_t cwd;
+              asm volatile("ld.shared.u32 %0, [%1];" : "=r"(cwd) : "r"(code0 + kRestBytes * (k >> 1) + 512 * (k & 1)));
+              const uint4 m4 = lds128(scratch + 16 * k);
+              uint32_t f[4];
+              cvt_e2m1x8(cwd, f);
+              o[4 * kk + 0] = hmul2(f[0], m4.x);
+              o[4 * kk + 1] = hmul2(f[1], m4.y);
+              o[4 * kk + 2] = hmul2(f[2], m4.z);
+              o[4 * kk + 3] = hmul2(f[3], m4.w);
+            }
+            tmem_st16_nowait(t_v + 16 * h, o);
+          }
+          tmem_wait_st();
+          tc_fence_before();
+          __syncwarp();                                 // also: every lane has read the scratch of this tile
+          if (lane == 0) {
+            mbar_arrive(bar_ready + 8 * sb);
+            mbar_arrive(bar_empty + 8 * s);            // this warp is done with the stage's V codes and scales
+          }
+          ++gt;
+          if (++s == kStages) { s = 0; ph_full ^= 1; }
+        }
 
-        // ---- S has been read: the QK warp may overwrite this S buffer (global tile gt+2)
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(bar_sfree + 8 * sb);
-
-        // ---- V codes -> Vhat^T in TMEM buffer gt&1
-        v_convert(rest0, scratch, t_v + 64 * (sb % kVBufs), lane, g);
-        fence_async_smem();
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) {
-          mbar_arrive(bar_ready);
-          mbar_arrive(bar_empty + 8 * s);              // this warp is done with the stage's V codes and scales
+        // ============================================================== the unit's accumulator
+        mbar_wait(bar_done + 8 * ((gt - 1) & 1), ((gt - 1) >> 1) & 1);
+        tc_fence_after();
+        {
+          float ov[16];
+          tmem_ld<16>(t_o, ov);
+          const float vscale = pow2i(eref - 13 - 127);  // stored Vhat = code * 2^(byte - eref + 13)
+#pragma unroll
+          for (int j = 0; j < 16; ++j)
+            if (j < G) partial_acc[(un.row0 + (long long)j * num_splits) * kHeadDim + r] = ov[j] * vscale;
         }
-
-        ++gt;
-        if (++s == kStages) { s = 0; ph_full ^= 1; }
+        tc_fence_before();                              // the next unit's first PV overwrites O
       }
-
-      // ================================================================ the unit's partial
-      mbar_wait(bar_done + 8 * ((gt - 1) & 1), ((gt - 1) >> 1) & 1);
-      tc_fence_after();
-      {
-        float ov[8];
-        tmem_ld8(tmem + lane_sel + kColO + 8 * hh, ov);
-        const float vscale = pow2i(eref - 13 - 127);    // stored Vhat = code * 2^(byte - eref + 13)
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const int head = 8 * hh + j;
-          if (head < G) partial_acc[(un.row0 + (long long)head * num_splits) * kHeadDim + r] = ov[j] * vscale;
-        }
-      }
-#pragma unroll
-      for (int j = 0; j < 8; ++j) {
-        float v = lsum[j];
-#pragma unroll
-        for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
-        lsum[j] = v;
-      }
-      if (lane == 0) {
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          sh.lsum[cw][j] = lsum[j];
-          if (q == 0) sh.mref[8 * hh + j] = mref[j];
-        }
-      }
-      tc_fence_before();
-      bar_compute();
-      if (ctid < G) {                                  // one thread per query head
-        const int h2 = ctid >> 3, j = ctid & 7;
-        float l = 0.f;
-#pragma unroll
-        for (int w = 0; w < 4; ++w) l += sh.lsum[4 * h2 + w][j];
-        ml_out[un.row0 + (long long)ctid * num_splits] = make_float2(sh.mref[ctid] * 0.6931471805599453f, l);   // natural log
-      }
-      if (un.slots_used > 0) {                         // item finished: its remaining slots are empty
-        const long long row_item = un.row0 - (un.slots_used - 1);
-        const int n_empty = num_splits - un.slots_used;
-        for (int e = ctid; e < G * n_empty; e += 32 * kComputeWarps) {
-          const int head = e / n_empty, sl = un.slots_used + (e - head * n_empty);
-          ml_out[row_item + (long long)head * num_splits + sl] = make_float2(-INFINITY, 0.f);
-        }
-      }
-      bar_compute();                                    // sh.lsum / sh.mref are reused by the next unit
     }
   }
 
