@@ -41,26 +41,35 @@ namespace {
 
 constexpr int kComputeWarps = 8;                     // two per TMEM lane quarter: one softmax warp, one V warp
 constexpr int kSoftmaxWarps = 4;
-constexpr int kIssuerWarps = 3;                      // QK issuer, PV issuer, TMA producer
-constexpr int kThreads = (kComputeWarps + kIssuerWarps) * 32;
-#ifndef UQ_STAGES
-#define UQ_STAGES 3
+constexpr int kIssuerWarps = 4;                      // QK issuer, PV issuer, K producer, V producer
+constexpr int kThreads = (kComputeWarps + kIssuerWarps) * 32;   // 12 warps: registers are allocated per 4 warps anyway
+#ifndef UQ_KSTAGES
+#define UQ_KSTAGES 3
+#endif
+#ifndef UQ_VSTAGES
+#define UQ_VSTAGES 4
 #endif
 #ifndef UQ_CTAS_PER_SM
 #define UQ_CTAS_PER_SM 2
 #endif
-constexpr int kStages = UQ_STAGES;
+// Two rings: the K codes of a tile (16 KB once the TMA unit has expanded the nibbles) are needed by the QK
+// MMA only and leave early; the rest of the records (V codes, K scales, V scales: 9 KB) stays until the V
+// warps have converted it.  Separate rings let the small one run deep (bytes in flight hide HBM latency).
+constexpr int kKStages = UQ_KSTAGES;
+constexpr int kVStages = UQ_VSTAGES;
 constexpr int kTilePages = 8;                        // 128 tokens per tile
 constexpr int kRestBytes = kRecordBytes - 1024;      // V codes + K scales + V scales = 1152
-constexpr int kStageBytes = kTilePages * (2048 + kRestBytes);   // K unpacked 16 KB + 9216 = 25600
+constexpr int kKStageBytes = kTilePages * 2048;      // K codes, one byte per code: 16384
+constexpr int kVStageBytes = kTilePages * kRestBytes;   // 9216
 constexpr int kPBytes = 4096;                        // one P operand buffer: [token-core 16][head-core 2][8 tok][8 heads] f16
 constexpr float kThresh = 12.0f;                     // lazy-reference threshold (log2 units)
 constexpr unsigned kFull = 0xffffffffu;
 constexpr int kMaxBatch = 2048;                      // sequences per call (tile prefix sums live in shared memory)
 
 // dynamic shared memory map (offsets from a 1024-byte aligned base)
-constexpr int kOffStage = 0;
-constexpr int kOffQ = kOffStage + kStages * kStageBytes;       // 2 x 2048, SW128 (one per unit in flight)
+constexpr int kOffK = 0;                                       // kKStages x 16384, SW128
+constexpr int kOffV = kOffK + kKStages * kKStageBytes;         // kVStages x 9216
+constexpr int kOffQ = kOffV + kVStages * kVStageBytes;         // 2 x 2048, SW128 (one per unit in flight)
 constexpr int kOffSFA = kOffQ + 4096;                          // 2 x 512
 constexpr int kOffSFB = kOffSFA + 1024;                        // 512
 constexpr int kOffP = kOffSFB + 512;                           // 2 x 4096 (double-buffered)
@@ -122,6 +131,22 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "}\n" ::"r"(bar), "r"(parity) : "memory");
 #endif
 }
+// try_wait with a suspend-time hint (ns): for waiters that are known to wait long (the softmax warps wait
+// for the V warps most of the time) — fewer wake-ups, fewer issue slots taken from the working warps
+__device__ __forceinline__ void mbar_wait_hint(uint32_t bar, uint32_t parity, uint32_t ns) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(bar), "r"(parity), "r"(ns) : "memory");
+}
+#ifndef UQ_A_WAIT_NS
+#define UQ_A_WAIT_NS 0
+#endif
 #ifndef UQ_SPIN_NS
 #define UQ_SPIN_NS 32
 #endif
@@ -279,8 +304,10 @@ __device__ __forceinline__ float pow2i(int e) {   // 2^e, flushing to 0 below th
 
 // ---------------------------------------------------------------- per-CTA shared bookkeeping
 struct Shared {
-  uint64_t full[kStages];     // producer (expect_tx) + TMA bytes -> QK warp, compute warps
-  uint64_t empty[kStages];    // 8 compute warps + QK commit -> producer
+  uint64_t full_k[kKStages];  // K producer (expect_tx) + TMA bytes -> QK warp
+  uint64_t empty_k[kKStages]; // QK commit -> K producer
+  uint64_t full_v[kVStages];  // V producer (expect_tx) + bulk-copy bytes -> QK warp (K scales), V warps
+  uint64_t empty_v[kVStages]; // 4 V warps + QK warp -> V producer
   uint64_t s_full[2];         // QK(gt) commit + PV(gt-2) commit -> compute warps: S is there, P / Vhat buffers are free
   uint64_t s_free[2];         // 8 compute warps -> QK warp: S buffer read, may be overwritten
   uint64_t ready[2];          // 4 softmax + 4 V warps -> PV warp: P (smem) and Vhat (TMEM) buffer gt&1 are written
@@ -393,7 +420,8 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
 
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = base + kOffQ, sSFA = base + kOffSFA, sSFB = base + kOffSFB, sP = base + kOffP;
-  const uint32_t bar_full = smem_u32(&sh.full[0]), bar_empty = smem_u32(&sh.empty[0]),
+  const uint32_t bar_fullk = smem_u32(&sh.full_k[0]), bar_emptyk = smem_u32(&sh.empty_k[0]),
+                 bar_fullv = smem_u32(&sh.full_v[0]), bar_emptyv = smem_u32(&sh.empty_v[0]),
                  bar_sfull = smem_u32(&sh.s_full[0]), bar_sfree = smem_u32(&sh.s_free[0]),
                  bar_ready = smem_u32(&sh.ready[0]), bar_done = smem_u32(&sh.done[0]),
                  bar_qfull = smem_u32(&sh.q_full[0]);
@@ -401,9 +429,14 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
   // ---------------- setup
   if (tid == 0) {
 #pragma unroll
-    for (int s = 0; s < kStages; ++s) {
-      mbar_init(bar_full + 8 * s, 1);
-      mbar_init(bar_empty + 8 * s, (kComputeWarps - kSoftmaxWarps) + 1);
+    for (int s = 0; s < kKStages; ++s) {
+      mbar_init(bar_fullk + 8 * s, 1);
+      mbar_init(bar_emptyk + 8 * s, 1);
+    }
+#pragma unroll
+    for (int s = 0; s < kVStages; ++s) {
+      mbar_init(bar_fullv + 8 * s, 1);
+      mbar_init(bar_emptyv + 8 * s, (kComputeWarps - kSoftmaxWarps) + 1);
     }
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
@@ -486,7 +519,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     cur_nx = cur;
     Unit un, nx;
     bool have_nx = sc.next(cur_nx, nx);                // nx runs one unit ahead of un
-    int gt = 0, s = 0, ph_full = 0;                    // global tile counter, its stage and full-barrier parity
+    int gt = 0, sk = 0, phk = 0, sv = 0, phv = 0;      // global tile counter; its K / V stage and full-barrier parity
     int k = 0, k_q = -1;                               // ordinal of the current unit; last ordinal whose Q load was issued
     while (have_nx) {
       un = nx;
@@ -499,18 +532,20 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
         if (i == 0 && k_q < k) { load_q(un, k); k_q = k; }
         if (i == 1 && have_nx) { load_q(nx, k + 1); k_q = k + 1; }
         if (i == 0) mbar_wait(bar_qfull + 8 * (k & 1), (k >> 1) & 1);
-        mbar_wait(bar_full + 8 * s, ph_full);
-        const uint32_t st = base + kOffStage + s * kStageBytes;
+        mbar_wait(bar_fullv + 8 * sv, phv);
+        const uint32_t st = base + kOffK + sk * kKStageBytes, rest = base + kOffV + sv * kVStageBytes;
         // scale-factor atom: row r = 32 c + lane of the tile -> 16-byte line `lane`, word c
         uint32_t v[4];
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
           const int r = 32 * c + lane;
-          asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v[c]) : "r"(st + 16384 + kRestBytes * (r >> 4) + 1024 + 4 * (r & 15)));
+          asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v[c]) : "r"(rest + kRestBytes * (r >> 4) + 1024 + 4 * (r & 15)));
         }
         sts128(sSFA + 512 * sb + 16 * lane, make_uint4(v[0], v[1], v[2], v[3]));
         fence_async_smem();
         __syncwarp();
+        if (lane == 0) mbar_arrive(bar_emptyv + 8 * sv);   // the K scales are copied: this warp is done with the V stage
+        mbar_wait(bar_fullk + 8 * sk, phk);
         tc_fence_after();
         if (lane == 0) {
           const uint32_t t_sfa = tmem + kColSFA + 4 * sb, qb = sQ + 2048 * (k & 1);
@@ -520,11 +555,12 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
             umma_mxf8f6f4(tmem + kColS + 16 * sb, make_desc(st + 32 * kb, 16, 1024, 2), make_desc(qb + 32 * kb, 16, 1024, 2),
                           idesc_qk | ((uint32_t)kb << 29), kb > 0, t_sfa + ((uint32_t)kb << 30), tmem + kColSFB);
           umma_commit(bar_sfull + 8 * sb);
-          umma_commit(bar_empty + 8 * s);
+          umma_commit(bar_emptyk + 8 * sk);
         }
         __syncwarp();
         ++gt;
-        if (++s == kStages) { s = 0; ph_full ^= 1; }
+        if (++sk == kKStages) { sk = 0; phk ^= 1; }
+        if (++sv == kVStages) { sv = 0; phv ^= 1; }
       }
       ++k;
     }
@@ -552,10 +588,16 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
         __syncwarp();
       }
     }
-  } else if (warp == 2) {
-    // ================================================================ TMA producer warp
-    // Lanes 0..7 each issue the two copies of one page of the tile (the copies of a warp serialise at
-    // ~55 cycles each: ~900 cycles per tile, inside the CTA's tile period); the ring runs across units.
+  } else if (warp == 2 || warp == 3) {
+    // ================================================================ producer warps
+    // Warp 2 streams the K codes (one TMA tensor copy per page: the TMA unit expands the packed nibbles to
+    // one byte per code), warp 3 the rest of the records (one 1152-byte bulk copy per page), each into its own
+    // ring and at its own pace.  Lanes 0..7 issue one page each (the copies of a warp serialise at ~55 cycles:
+    // ~450 cycles per tile and warp); the rings run across units.
+    const bool is_k = (warp == 2);
+    const int n_stages = is_k ? kKStages : kVStages;
+    const uint32_t bar_e = is_k ? bar_emptyk : bar_emptyv, bar_f = is_k ? bar_fullk : bar_fullv;
+    const uint32_t page_tx = is_k ? 1024u : (uint32_t)kRestBytes;
     const uint64_t pol = l2_evict_first_policy();
     Cursor cur;
     sc.start(cur);
@@ -569,23 +611,24 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
         const int npg = min(kTilePages, un.p1 - (un.p0 + kTilePages * i));
         const int nb = un.p0 + kTilePages * (i + 1) + lane;
         page_next = (lane < kTilePages && nb < un.p1) ? bt[kTilePages * (i + 1)] : 0;
-        mbar_wait(bar_empty + 8 * s, ph);
-        if (lane == 0) mbar_expect_tx(bar_full + 8 * s, (uint32_t)npg * kRecordBytes);
+        mbar_wait(bar_e + 8 * s, ph);
+        if (lane == 0) mbar_expect_tx(bar_f + 8 * s, (uint32_t)npg * page_tx);
         __syncwarp();
         if (lane < npg) {
-          const uint32_t st = base + kOffStage + s * kStageBytes;
-          tma_load_3d(st + 2048 * lane, &tmap, 0, 0, page * Hkv + un.kvh, bar_full + 8 * s, pol);
-          bulk_g2s(st + 16384 + kRestBytes * lane, cache + ((long long)page * Hkv + un.kvh) * kRecordBytes + 1024, kRestBytes,
-                   bar_full + 8 * s, pol);
+          if (is_k)
+            tma_load_3d(base + kOffK + s * kKStageBytes + 2048 * lane, &tmap, 0, 0, page * Hkv + un.kvh, bar_f + 8 * s, pol);
+          else
+            bulk_g2s(base + kOffV + s * kVStageBytes + kRestBytes * lane,
+                     cache + ((long long)page * Hkv + un.kvh) * kRecordBytes + 1024, kRestBytes, bar_f + 8 * s, pol);
         }
-        if (++s == kStages) { s = 0; ph ^= 1; }
+        if (++s == n_stages) { s = 0; ph ^= 1; }
       }
     }
   } else {
-    // ================================================================ compute warps (warp ids 3..10)
+    // ================================================================ compute warps (warp ids 4..11)
     // Two role-pure groups of four warps, one warp of each per TMEM lane quarter (hardware: warp id % 4):
-    //   softmax warps (3..6):  thread = token row of the tile, all query heads of the kv head;
-    //   V warps (7..10):       thread = channel d, all 128 tokens of the tile.
+    //   softmax warps (4..7):  thread = token row of the tile, all query heads of the kv head;
+    //   V warps (8..11):       thread = channel d, all 128 tokens of the tile.
     // A V warp needs the tile's bytes but not its scores, so it may run ahead of the softmax warps; the
     // two groups meet only at the `ready` barrier of the PV warp.  The issuer warps sit on the lowest
     // warp ids so that the scheduler's highest-warp-id-first arbitration favours the compute warps.
@@ -628,7 +671,11 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
             const uint32_t t_s = tmem + lane_sel + kColS + 16 * sb;
             const uint32_t p_addr = p_row + kPBytes * sb;
 
+#if UQ_A_WAIT_NS > 0
+            mbar_wait_hint(bar_sfull + 8 * sb, ph2, UQ_A_WAIT_NS);
+#else
             mbar_wait(bar_sfull + 8 * sb, ph2);        // S(gt) is in TMEM and PV(gt-2) has read P buffer gt&1
+#endif
             tc_fence_after();
 
             float lt[NH];
@@ -769,15 +816,15 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
       Cursor cur;
       sc.start(cur);
       Unit un;
-      int gt = 0, s = 0, ph_full = 0;                  // global tile counter, its stage and full-barrier parity
+      int gt = 0, s = 0, ph_full = 0;                  // global tile counter, its V stage and full-barrier parity
       while (sc.next(cur, un)) {
         int eref = 28;
         int rem = un.tok_end - un.p0 * kPage;          // valid tokens from the first token of the tile on
 
         for (int i = 0; i < un.n_tiles; ++i, rem -= kTilePages * kPage) {
           const int sb = gt & 1;
-          const uint32_t rest = base + kOffStage + s * kStageBytes + 16384;   // [V codes | K scales | V scales] of page 0
-          mbar_wait(bar_full + 8 * s, ph_full);        // the tile's bytes have landed
+          const uint32_t rest = base + kOffV + s * kVStageBytes;   // [V codes | K scales | V scales] of page 0
+          mbar_wait(bar_fullv + 8 * s, ph_full);       // the tile's bytes have landed
 
           // ---- the tile's 128 scale bytes of group g: lane <-> tokens 4 lane .. 4 lane + 3
           uint32_t sw;
@@ -845,10 +892,10 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
           __syncwarp();                                 // also: every lane has read the scratch of this tile
           if (lane == 0) {
             mbar_arrive(bar_ready + 8 * sb);
-            mbar_arrive(bar_empty + 8 * s);            // this warp is done with the stage's V codes and scales
+            mbar_arrive(bar_emptyv + 8 * s);           // this warp is done with the stage's V codes and scales
           }
           ++gt;
-          if (++s == kStages) { s = 0; ph_full ^= 1; }
+          if (++s == kVStages) { s = 0; ph_full ^= 1; }
         }
 
         // ============================================================== the unit's accumulator
