@@ -594,6 +594,10 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     // one byte per code), warp 3 the rest of the records (one 1152-byte bulk copy per page), each into its own
     // ring and at its own pace.  Lanes 0..7 issue one page each (the copies of a warp serialise at ~55 cycles:
     // ~450 cycles per tile and warp); the rings run across units.
+    // (Measured: issuing a tile's copies, or its MMAs, back to back from one elected thread — elect.sync, which
+    // lets ptxas drop the dozen instructions it wraps around every uniform-operand instruction behind
+    // `lane == 0` — is SLOWER, 123-142 us against 119.7 us on config 2: an async instruction that finds its
+    // unit busy holds the scheduler's dispatch port; the filler instructions space the issues out for free.)
     const bool is_k = (warp == 2);
     const int n_stages = is_k ? kKStages : kVStages;
     const uint32_t bar_e = is_k ? bar_emptyk : bar_emptyv, bar_f = is_k ? bar_fullk : bar_fullv;
