@@ -179,6 +179,16 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm,
   asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
                ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(bar) : "memory");
 }
+// One lane of the (converged) warp.  With elect.sync ptxas knows that a single thread runs the guarded block and
+// feeds the uniform-register operands of UTCQMMA / UTMALDG with one R2UR each; behind `lane == 0` it wraps every
+// such instruction in an elect-and-broadcast loop of a dozen instructions.  Measured on config 2: for the QK warp
+// (the busiest issuer: its serial per-tile instruction stream bounded the tile period) this is 119 -> 109.5 us;
+// for the PV warp and the producers the same change is SLOWER (124-132 us), so those keep `lane == 0`.
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n.reg .pred p;\nelect.sync _|p, 0xffffffff;\nselp.u32 %0, 1, 0, p;\n}\n" : "=r"(pred));
+  return pred != 0;
+}
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -417,6 +427,15 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
 
   const int G = Hq / Hkv;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+#ifndef UQ_ISSUERS_HIGH
+#define UQ_ISSUERS_HIGH 1
+#endif
+  // role 0 QK issuer, 1 PV issuer, 2 K producer, 3 V producer, 4..7 softmax warps, 8..11 V warps
+#if UQ_ISSUERS_HIGH
+  const int role = warp < kComputeWarps ? warp + kIssuerWarps : warp - kComputeWarps;
+#else
+  const int role = warp;
+#endif
 
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = base + kOffQ, sSFA = base + kOffSFA, sSFB = base + kOffSFB, sP = base + kOffP;
@@ -450,7 +469,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     for (int h = 0; h < 2; ++h) mbar_arrive(bar_sfull + 8 * h);   // global tiles 0 and 1 have no PV(gt-2)
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == 1) {
+  if (role == 1) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&sh.tmem_base)),
                  "r"(kTmemCols));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
@@ -498,7 +517,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     sc.tpc = max(1, max(even, fit));
   }
 
-  if (warp == 0) {
+  if (role == 0) {
     // ================================================================ QK warp
     // Per unit: the FP8 query tile (16 rows x 128 B, 128-byte swizzle) arrives by TMA into Q buffer
     // (unit ordinal & 1) — "hoisted", once per unit; rows past the unit's G heads belong to
@@ -507,9 +526,9 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     // by the softmax of global tile gt-2.  (PV(gt-2), which frees the P / Vhat buffers gt&1, is the second
     // arrival of s_full: it is not on this warp's path.)
     const uint32_t idesc_qk = (5u << 7) | (0u << 10) | (2u << 17) | (1u << 23) | (8u << 24);   // E2M1 x E4M3, UE8M0, N=16, M=128
-    if (lane == 0) umma_cp_sf(tmem + kColSFB, make_desc(sSFB, 16, 128, 0));
+    if (elect_one()) umma_cp_sf(tmem + kColSFB, make_desc(sSFB, 16, 128, 0));
     auto load_q = [&](const Unit& un, int k) {         // lane 0: Q tile of unit ordinal k
-      if (lane == 0) {
+      if (elect_one()) {
         mbar_expect_tx(bar_qfull + 8 * (k & 1), 2048);
         tma_load_2d(sQ + 2048 * (k & 1), &tmap_q, 0, un.b * Hq + un.kvh * G, bar_qfull + 8 * (k & 1));
       }
@@ -547,7 +566,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
         if (lane == 0) mbar_arrive(bar_emptyv + 8 * sv);   // the K scales are copied: this warp is done with the V stage
         mbar_wait(bar_fullk + 8 * sk, phk);
         tc_fence_after();
-        if (lane == 0) {
+        if (elect_one()) {
           const uint32_t t_sfa = tmem + kColSFA + 4 * sb, qb = sQ + 2048 * (k & 1);
           umma_cp_sf(t_sfa, make_desc(sSFA + 512 * sb, 16, 128, 0));
 #pragma unroll
@@ -564,7 +583,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
       }
       ++k;
     }
-  } else if (warp == 1) {
+  } else if (role == 1) {
     // ================================================================ PV warp
     // O^T[128 d x 16 heads] += Vhat^T (TMEM, buffer gt&1) . P^T (smem, buffer gt&1); f16 x f16 -> f32, B MN-major
     const uint32_t idesc_pv = (1u << 4) | (1u << 16) | (2u << 17) | (8u << 24);
@@ -588,17 +607,15 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
         __syncwarp();
       }
     }
-  } else if (warp == 2 || warp == 3) {
+  } else if (role == 2 || role == 3) {
     // ================================================================ producer warps
     // Warp 2 streams the K codes (one TMA tensor copy per page: the TMA unit expands the packed nibbles to
     // one byte per code), warp 3 the rest of the records (one 1152-byte bulk copy per page), each into its own
     // ring and at its own pace.  Lanes 0..7 issue one page each (the copies of a warp serialise at ~55 cycles:
     // ~450 cycles per tile and warp); the rings run across units.
-    // (Measured: issuing a tile's copies, or its MMAs, back to back from one elected thread — elect.sync, which
-    // lets ptxas drop the dozen instructions it wraps around every uniform-operand instruction behind
-    // `lane == 0` — is SLOWER, 123-142 us against 119.7 us on config 2: an async instruction that finds its
-    // unit busy holds the scheduler's dispatch port; the filler instructions space the issues out for free.)
-    const bool is_k = (warp == 2);
+    // (Measured: issuing a tile's eight copies back to back from one elected thread is slower, 131.7 us against
+    // 119.7 us on config 2, than one copy per lane — see elect_one().)
+    const bool is_k = (role == 2);
     const int n_stages = is_k ? kKStages : kVStages;
     const uint32_t bar_e = is_k ? bar_emptyk : bar_emptyv, bar_f = is_k ? bar_fullk : bar_fullv;
     const uint32_t page_tx = is_k ? 1024u : (uint32_t)kRestBytes;
@@ -636,14 +653,14 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     // A V warp needs the tile's bytes but not its scores, so it may run ahead of the softmax warps; the
     // two groups meet only at the `ready` barrier of the PV warp.  The issuer warps sit on the lowest
     // warp ids so that the scheduler's highest-warp-id-first arbitration favours the compute warps.
-    const int cw = warp - kIssuerWarps;                // 0..7
+    const int cw = role - kIssuerWarps;                // 0..7
     const int q = warp & 3;                            // TMEM lane quarter
     const uint32_t lane_sel = (uint32_t)(32 * q) << 16;
     const int r = 32 * q + lane;                       // softmax: token row of the tile; V warps: channel d
 
     if (cw < kSoftmaxWarps) {
       // ============================================================== softmax warps
-      const int atid = tid - 32 * kIssuerWarps;        // 0..127
+      const int atid = 32 * cw + lane;                 // 0..127
       float2* const ml_out = reinterpret_cast<float2*>(partial_ml);
 
       // items without any token: all their slots are empty, (m, l) = (-inf, 0)
@@ -675,7 +692,9 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
             const uint32_t t_s = tmem + lane_sel + kColS + 16 * sb;
             const uint32_t p_addr = p_row + kPBytes * sb;
 
-#if UQ_A_WAIT_NS > 0
+#if defined(UQ_A_SLEEP_NS)
+            while (!mbar_test(bar_sfull + 8 * sb, ph2)) asm volatile("nanosleep.u32 %0;" ::"r"((uint32_t)UQ_A_SLEEP_NS));
+#elif UQ_A_WAIT_NS > 0
             mbar_wait_hint(bar_sfull + 8 * sb, ph2, UQ_A_WAIT_NS);
 #else
             mbar_wait(bar_sfull + 8 * sb, ph2);        // S(gt) is in TMEM and PV(gt-2) has read P buffer gt&1
@@ -921,7 +940,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
   // ---------------- teardown
   tc_fence_before();
   __syncthreads();
-  if (warp == 1) {
+  if (role == 1) {
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTmemCols));
   }
 }
