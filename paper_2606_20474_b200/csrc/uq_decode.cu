@@ -318,7 +318,7 @@ struct Shared {
   uint64_t empty_k[kKStages]; // QK commit -> K producer
   uint64_t full_v[kVStages];  // V producer (expect_tx) + bulk-copy bytes -> QK warp (K scales), V warps
   uint64_t empty_v[kVStages]; // 4 V warps + QK warp -> V producer
-  uint64_t s_full[2];         // QK(gt) commit + PV(gt-2) commit -> compute warps: S is there, P / Vhat buffers are free
+  uint64_t s_full[2];         // QK commit -> softmax warps: S(gt) is in TMEM buffer gt&1
   uint64_t s_free[2];         // 8 compute warps -> QK warp: S buffer read, may be overwritten
   uint64_t ready[2];          // 4 softmax + 4 V warps -> PV warp: P (smem) and Vhat (TMEM) buffer gt&1 are written
                               // (two barriers: a V warp may be one tile ahead of the softmax warps)
@@ -459,14 +459,12 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     }
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
-      mbar_init(bar_sfull + 8 * h, 2);
+      mbar_init(bar_sfull + 8 * h, 1);
       mbar_init(bar_sfree + 8 * h, kSoftmaxWarps);
       mbar_init(bar_done + 8 * h, 1);
       mbar_init(bar_qfull + 8 * h, 1);
       mbar_init(bar_ready + 8 * h, kComputeWarps);
     }
-#pragma unroll
-    for (int h = 0; h < 2; ++h) mbar_arrive(bar_sfull + 8 * h);   // global tiles 0 and 1 have no PV(gt-2)
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (role == 1) {
@@ -523,8 +521,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     // (unit ordinal & 1) — "hoisted", once per unit; rows past the unit's G heads belong to
     // the next kv head (or are zero past the tensor end) and only feed score columns nobody reads.
     // Per tile: S(gt)[128 tok x 16 heads] = K . Q^T once the tile's bytes have landed, the S buffer was read
-    // by the softmax of global tile gt-2.  (PV(gt-2), which frees the P / Vhat buffers gt&1, is the second
-    // arrival of s_full: it is not on this warp's path.)
+    // by the softmax of global tile gt-2.
     const uint32_t idesc_qk = (5u << 7) | (0u << 10) | (2u << 17) | (1u << 23) | (8u << 24);   // E2M1 x E4M3, UE8M0, N=16, M=128
     if (elect_one()) umma_cp_sf(tmem + kColSFB, make_desc(sSFB, 16, 128, 0));
     auto load_q = [&](const Unit& un, int k) {         // lane 0: Q tile of unit ordinal k
@@ -602,7 +599,6 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
             umma_f16_ts(tmem + kColO, vbuf + 8 * j, make_desc(pbuf + 512 * j, 256, 128, 0), idesc_pv,
                         (i > 0 || j > 0) ? 1u : 0u);
           umma_commit(bar_done + 8 * (gt & 1));
-          umma_commit(bar_sfull + 8 * (gt & 1));       // second arrival of S(gt+2)'s phase: P / Vhat buffers gt&1 are free
         }
         __syncwarp();
       }
@@ -697,8 +693,10 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
 #elif UQ_A_WAIT_NS > 0
             mbar_wait_hint(bar_sfull + 8 * sb, ph2, UQ_A_WAIT_NS);
 #else
-            mbar_wait(bar_sfull + 8 * sb, ph2);        // S(gt) is in TMEM and PV(gt-2) has read P buffer gt&1
+            mbar_wait(bar_sfull + 8 * sb, ph2);        // S(gt) is in TMEM
 #endif
+            if (gt >= 2) mbar_wait(bar_done + 8 * sb, ph2 ^ 1);   // PV(gt-2) has read P buffer gt&1 (the PV warp commits
+                                                                   // once per tile: its issue stream bounds the tile period)
             tc_fence_after();
 
             float lt[NH];
@@ -857,10 +855,9 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
             const int nv = rem - 4 * lane;             // valid tokens among this lane's four
             sw = nv >= 4 ? sw : (nv <= 0 ? 0u : (sw & (0xFFFFFFFFu >> (8 * (4 - nv)))));
           }
-          const uint32_t mx2 = __vmaxu4(sw, sw >> 16);
-          const int vmax = __reduce_max_sync(kFull, (int)(__vmaxu4(mx2, mx2 >> 8) & 0xFFu));
-          if (__builtin_expect(vmax > eref, 0)) {      // warp-uniform
-            const int enew = vmax + 2;
+          const int b0 = (int)(sw & 0xFFu), b1 = (int)((sw >> 8) & 0xFFu), b2 = (int)((sw >> 16) & 0xFFu), b3 = (int)(sw >> 24);
+          if (__builtin_expect(__any_sync(kFull, max(max(b0, b1), max(b2, b3)) > eref), 0)) {   // warp-uniform
+            const int enew = __reduce_max_sync(kFull, max(max(b0, b1), max(b2, b3))) + 2;
             if (i > 0) {
               // O rows of this lane quarter change unit: after the softmax warps are through with the tile
               // (their own rescale of O included) and every PV issued so far has landed
@@ -878,8 +875,8 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
           }
           {   // four fp16 power-of-two multipliers (two f16x2: token pairs 2 lane, 2 lane + 1); byte 0 -> 0
             const int kbase = eref - 28;               // fp16 exponent field = byte - kbase (2^13 at byte = eref)
-            const uint32_t e0 = (uint32_t)max((int)(sw & 0xFFu) - kbase, 0), e1 = (uint32_t)max((int)((sw >> 8) & 0xFFu) - kbase, 0),
-                           e2 = (uint32_t)max((int)((sw >> 16) & 0xFFu) - kbase, 0), e3 = (uint32_t)max((int)(sw >> 24) - kbase, 0);
+            const uint32_t e0 = (uint32_t)max(b0 - kbase, 0), e1 = (uint32_t)max(b1 - kbase, 0),
+                           e2 = (uint32_t)max(b2 - kbase, 0), e3 = (uint32_t)max(b3 - kbase, 0);
             asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(scratch + 8 * lane), "r"((e0 << 10) | (e1 << 26)),
                          "r"((e2 << 10) | (e3 << 26)) : "memory");
           }
