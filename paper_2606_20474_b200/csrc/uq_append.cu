@@ -137,6 +137,8 @@ append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v
               const int32_t* __restrict__ block_tables, int max_pages, int batch, int total_new,
               int Hq, int Hkv, uint8_t* __restrict__ cache, const uint16_t* __restrict__ q,
               uint8_t* __restrict__ q_fp8, double c_k, double c_v) {
+  pdl_launch_dependents();
+  pdl_wait();                                          // inputs and cache may come from the kernel before this one
   const int lane = threadIdx.x & 31;
   const long long unit = (long long)blockIdx.x * 4 + (threadIdx.x >> 5);
   const long long kv_units = (long long)total_new * Hkv;
@@ -224,9 +226,10 @@ extern "C" int32_t uq_rotate_quantize_append(const uq_config* cfg, const void* k
     set_error("append: too many work units");
     return UQ_ERR_INVALID_ARG;
   }
-  append_kernel<<<(unsigned)blocks, 128, 0, (cudaStream_t)stream>>>(
-      (const uint16_t*)k_new, (const uint16_t*)v_new, cu_new, seq_lens, block_tables, max_pages,
-      batch, total_new, cfg->num_q_heads, cfg->num_kv_heads, (uint8_t*)cache, (const uint16_t*)q,
-      (uint8_t*)q_fp8, (double)cfg->c_k, (double)cfg->c_v);
-  return check_cuda(cudaGetLastError(), "uq_rotate_quantize_append launch");
+  return check_cuda(launch_pdl(append_kernel, dim3((unsigned)blocks), dim3(128), 0, (cudaStream_t)stream,
+                               (const uint16_t*)k_new, (const uint16_t*)v_new, cu_new, seq_lens, block_tables,
+                               (int)max_pages, (int)batch, (int)total_new, (int)cfg->num_q_heads,
+                               (int)cfg->num_kv_heads, (uint8_t*)cache, (const uint16_t*)q, (uint8_t*)q_fp8,
+                               (double)cfg->c_k, (double)cfg->c_v),
+                    "uq_rotate_quantize_append launch");
 }

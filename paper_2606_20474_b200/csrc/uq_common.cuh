@@ -23,6 +23,32 @@ void set_error(const char* fmt, ...);
 int32_t check_config(const uq_config* cfg);  // UQ_OK / UQ_ERR_*; sets the error string
 int32_t check_cuda(cudaError_t e, const char* what);
 
+// Programmatic dependent launch.  The three kernels of a decode step (append -> decode -> merge) are short and
+// run back to back on one stream: each is launched with programmatic stream serialization, announces right
+// away that its dependents may be launched (their CTAs become resident and run their own prologue as resources
+// allow), and waits for the grid before it in the stream — complete, memory visible — before it touches
+// global memory that grid may have written.  Behind a kernel that is not part of the scheme (or a copy) the
+// launch is ordered as usual.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+#endif
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream,
+                              Args&&... args) {
+  cudaLaunchConfig_t lc = {};
+  lc.gridDim = grid;
+  lc.blockDim = block;
+  lc.dynamicSmemBytes = smem;
+  lc.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  lc.attrs = attr;
+  lc.numAttrs = 1;
+  return cudaLaunchKernelEx(&lc, kernel, KArgs(args)...);
+}
+
 inline float resolved_sm_scale(const uq_config* cfg) {
   return cfg->sm_scale != 0.0f ? cfg->sm_scale : 0.08838834764831845f;  // 1/sqrt(128)
 }

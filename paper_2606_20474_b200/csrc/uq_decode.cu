@@ -475,6 +475,10 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
   if (tid < 128) {  // query-side scale factors: UE8M0 byte 127 = 2^0
     asm volatile("st.shared.u32 [%0], %1;" ::"r"(sSFB + 4 * tid), "r"(0x7F7F7F7Fu) : "memory");
   }
+  // Barriers, TMEM and scale constants are set up under the tail of the kernel before this one in the stream;
+  // everything below reads global memory it may have written (programmatic dependent launch, uq_common.cuh).
+  pdl_launch_dependents();
+  pdl_wait();
   // tiles per sequence -> inclusive prefix sums in shared memory (every CTA computes the same schedule)
   for (int b = tid; b < batch; b += kThreads) {
     const int L = seq_lens[b];
@@ -1079,8 +1083,9 @@ extern "C" int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, 
     if (e != cudaSuccess) return check_cuda(e, "decode: cudaFuncSetAttribute");
     attr_set = true;
   }
-  decode_kernel<<<grid, kThreads, kSmemBytes, (cudaStream_t)stream>>>(
-      tmap, tmap_q, (const uint8_t*)cache, block_tables, max_pages, seq_lens, batch, cfg->num_q_heads,
-      cfg->num_kv_heads, num_splits, score_scale, partial_acc, partial_ml);
-  return check_cuda(cudaGetLastError(), "uq_decode_attention launch");
+  return check_cuda(launch_pdl(decode_kernel, grid, dim3(kThreads), (size_t)kSmemBytes, (cudaStream_t)stream, tmap, tmap_q,
+                               (const uint8_t*)cache, block_tables, (int)max_pages, seq_lens, (int)batch,
+                               (int)cfg->num_q_heads, (int)cfg->num_kv_heads, (int)num_splits, score_scale, partial_acc,
+                               partial_ml),
+                    "uq_decode_attention launch");
 }

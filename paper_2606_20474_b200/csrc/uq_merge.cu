@@ -13,6 +13,8 @@ namespace {
 __global__ void __launch_bounds__(128)
 merge_kernel(const float* __restrict__ acc, const float* __restrict__ ml, int rows, int S,
              __nv_bfloat16* __restrict__ out) {
+  pdl_launch_dependents();
+  pdl_wait();                                          // the partials come from the kernel before this one
   const int lane = threadIdx.x & 31;
   const int row = blockIdx.x * 4 + (threadIdx.x >> 5);
   if (row >= rows) return;
@@ -67,7 +69,7 @@ extern "C" int32_t uq_merge_splits(const uq_config* cfg, const float* partial_ac
     return UQ_ERR_INVALID_ARG;
   }
   const int rows = batch * cfg->num_q_heads;
-  merge_kernel<<<(rows + 3) / 4, 128, 0, (cudaStream_t)stream>>>(partial_acc, partial_ml, rows, num_splits,
-                                                              (__nv_bfloat16*)out_bf16);
-  return check_cuda(cudaGetLastError(), "uq_merge_splits launch");
+  return check_cuda(launch_pdl(merge_kernel, dim3((rows + 3) / 4), dim3(128), 0, (cudaStream_t)stream, partial_acc,
+                               partial_ml, rows, (int)num_splits, (__nv_bfloat16*)out_bf16),
+                    "uq_merge_splits launch");
 }
