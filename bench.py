@@ -46,7 +46,7 @@ FALLBACK_HBM_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md fallbac
 
 # dram__bytes_read.sum + dram__bytes_write.sum per decode_kernel launch from the committed
 # `ncu --set full` capture of this command (profiles/), keyed by config; None = not captured.
-NCU_TRAFFIC_BYTES = {2: 571_058_432 + 4_535_552}   # profiles/r01_v10_decode_cfg2.md
+NCU_TRAFFIC_BYTES = {2: 571_075_072 + 5_741_056}   # dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01_v14_decode_cfg2.md
 
 
 # ----------------------------------------------------------------------------- helpers

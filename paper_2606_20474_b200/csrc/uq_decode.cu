@@ -5,27 +5,24 @@
 // Design: the 128-token tiles (8 pages) of all (sequence, kv head) items form one
 // sequence that is cut into equal contiguous ranges, one per resident CTA (one wave, 2 CTAs per SM); a
 // range is walked as units (item, tile range), each unit writing one partial slot of its item.
-// Warp roles (352 threads).  Every async instruction (TMA copy,
-// tcgen05.mma / cp / commit) occupies its issuing warp for ~55 cycles (measured), so the 16 copies and
-// 12 MMAs of a tile are spread over three issuer warps:
-//   warp 2  TMA producer: per page one TMA tensor copy of the packed FP4 K codes
-//           (CU_TENSOR_MAP_DATA_TYPE_16U4_ALIGN16B + SWIZZLE_128B: the TMA unit expands the
-//           nibbles into the 8-bit containers tcgen05 reads) and one cp.async.bulk of the rest of
-//           the record (V codes, K scales, V scales), into a 3-stage mbarrier ring, L2 evict-first;
-//   warp 0  QK issuer: S[128 tok x 16 heads] = K . Q^T with
-//           tcgen05.mma.kind::mxf8f6f4.block_scale — E2M1 keys x E4M3 queries with the UE8M0 group
-//           scales applied by the tensor core (the paper's FP8xFP4 scaled MMA), K
-//           scales staged smem -> TMEM with tcgen05.cp;
-//   warp 1  PV issuer: O^T[128 d x 16 heads] += Vhat^T . P^T
-//           with tcgen05.mma.kind::f16 (A = Vhat^T from TMEM, B = P from smem); accumulators in TMEM;
-//   warps 3-10 compute: S rows from TMEM (tcgen05.ld), base-2 softmax against a LAZY per-head
-//           reference (a "rebase" — new reference, O rescaled in TMEM, tile's P redone — happens on
-//           the first tile and whenever a score exceeds the reference by 2^12 or a V scale exceeds
-//           the reference exponent), P -> fp16 operand in smem (double-buffered); then V codes ->
-//           fp16 (cvt.rn.f16x2.e2m1x2 x exact power-of-two scale) written with tcgen05.st straight
-//           into TMEM, where the PV MMA reads it as its A operand (no shared-memory round trip:
-//           the kernel is shared-memory-bandwidth sensitive); the PV MMAs of a tile run under the
-//           softmax of the next one.
+// Warp roles (384 threads = 12 warps, one role each; the tile period is set by the longest serial instruction
+// stream of the CTA, so the roles are cut to keep every stream short):
+//   K producer   per page one TMA tensor copy of the packed FP4 K codes (CU_TENSOR_MAP_DATA_TYPE_16U4_ALIGN16B +
+//                SWIZZLE_128B: the TMA unit lays the nibbles out in the 8-bit containers tcgen05 reads) into a
+//                3-stage ring; L2 evict-first;
+//   V producer   per page one cp.async.bulk of the rest of the record (V codes, K scales, V scales) into a
+//                4-stage ring of its own;
+//   QK issuer    S[128 tok x 16 heads] = K . Q^T with tcgen05.mma.kind::mxf8f6f4.block_scale — E2M1 keys x E4M3
+//                queries with the UE8M0 group scales applied by the tensor core (the paper's FP8xFP4 scaled MMA,
+//                PAPER.md:281), K scales staged smem -> TMEM with tcgen05.cp; S double-buffered in TMEM;
+//   PV issuer    O^T[128 d x 16 heads] += Vhat^T . P^T with tcgen05.mma.kind::f16 (A = Vhat^T from TMEM, B = P from
+//                smem); accumulators in TMEM;
+//   4 softmax warps   thread = token row: S from TMEM (tcgen05.ld), base-2 softmax against a LAZY per-head
+//                reference (a "rebase" — new reference, O rescaled in TMEM, tile's P redone — happens on the first
+//                tile and whenever a score exceeds the reference by 2^12), P -> fp16 operand in smem;
+//   4 V warps    thread = channel: V codes -> fp16 (cvt.rn.f16x2.e2m1x2 x exact power-of-two scale against the
+//                warp's own reference exponent: its 32 channels are one scale group) written with tcgen05.st
+//                straight into TMEM, where the PV MMA reads it as its A operand (no shared-memory round trip).
 // The FP8 query tile is copied to smem by TMA once per unit ("hoisted").
 // Every K/V byte is read from HBM exactly once.
 #include <cuda.h>
