@@ -11,6 +11,7 @@ from .binding import (  # noqa: F401
     UQError,
     RECORD_BYTES,
     StepBuffers,
+    HostStage,
     alloc_cache,
     cache_record_bytes,
     decode_attention,

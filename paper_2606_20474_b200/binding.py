@@ -182,23 +182,52 @@ def decode_step(cfg: UQConfig, bufs: StepBuffers, q, k_new, v_new, cu_new, seq_l
     return bufs.out
 
 
-def decode_step_host(cfg: UQConfig, bufs: StepBuffers, dev_in: dict, q_host, k_new_host, v_new_host,
-                     cu_new_host, seq_lens_before_host, seq_lens_after_host, block_tables_host,
-                     cache, out_host, stream=None) -> torch.Tensor:
-    """The same step with HOST (pinned) inputs and output: the step's query, new K/V rows,
-    lengths and block tables are copied host->device, the attention output device->host.  The
-    KV cache itself is the resident state and stays in HBM.  dev_in holds preallocated device
-    tensors with keys q, k_new, v_new, cu_new, seq_lens_before, seq_lens_after, block_tables."""
-    dev_in["q"].copy_(q_host, non_blocking=True)
-    if k_new_host.shape[0] > 0:
-        dev_in["k_new"].copy_(k_new_host, non_blocking=True)
-        dev_in["v_new"].copy_(v_new_host, non_blocking=True)
-    dev_in["cu_new"].copy_(cu_new_host, non_blocking=True)
-    dev_in["seq_lens_before"].copy_(seq_lens_before_host, non_blocking=True)
-    dev_in["seq_lens_after"].copy_(seq_lens_after_host, non_blocking=True)
-    dev_in["block_tables"].copy_(block_tables_host, non_blocking=True)
-    out = decode_step(cfg, bufs, dev_in["q"], dev_in["k_new"], dev_in["v_new"], dev_in["cu_new"],
-                      dev_in["seq_lens_before"], dev_in["seq_lens_after"], dev_in["block_tables"],
-                      cache, stream=stream)
+class HostStage:
+    """A step's inputs laid back to back in ONE pinned host block with a device block of the same layout, so
+    that they cross PCIe in a single copy: q bf16 [batch, Hq, d], k_new / v_new bf16 [total_new, Hkv, d],
+    cu_new i32 [batch + 1], seq_lens_before / seq_lens_after i32 [batch], block_tables i32 [batch, max_pages].
+    The caller writes the host views (`.h[name]`), `upload()` enqueues the copy, the kernels read `.d[name]`."""
+
+    FIELDS = ("q", "k_new", "v_new", "cu_new", "seq_lens_before", "seq_lens_after", "block_tables")
+
+    def __init__(self, cfg: UQConfig, batch: int, total_new: int, max_pages: int, device="cuda"):
+        d = cfg.head_dim
+        spec = {
+            "q": ((batch, cfg.num_q_heads, d), torch.bfloat16),
+            "k_new": ((total_new, cfg.num_kv_heads, d), torch.bfloat16),
+            "v_new": ((total_new, cfg.num_kv_heads, d), torch.bfloat16),
+            "cu_new": ((batch + 1,), torch.int32),
+            "seq_lens_before": ((batch,), torch.int32),
+            "seq_lens_after": ((batch,), torch.int32),
+            "block_tables": ((batch, max_pages), torch.int32),
+        }
+        offs, total = {}, 0
+        for name in self.FIELDS:
+            shape, dtype = spec[name]
+            n = int(torch.tensor(shape).prod().item()) * torch.empty((), dtype=dtype).element_size()
+            offs[name] = (total, n)
+            total = (total + n + 255) // 256 * 256          # every field 256-byte aligned (the kernels ask for 16)
+        self.nbytes = total
+        self.host = torch.empty(total, dtype=torch.uint8)
+        if torch.device(device).type == "cuda":
+            self.host = self.host.pin_memory()
+        self.dev = torch.empty(total, dtype=torch.uint8, device=device)
+
+        def views(block):
+            return {name: block[o:o + n].view(spec[name][1]).view(spec[name][0]) for name, (o, n) in offs.items()}
+        self.h, self.d = views(self.host), views(self.dev)
+
+    def upload(self):
+        self.dev.copy_(self.host, non_blocking=True)        # on the current stream
+
+
+def decode_step_host(cfg: UQConfig, bufs: StepBuffers, stage: HostStage, cache, out_host, stream=None) -> torch.Tensor:
+    """The step with HOST (pinned) inputs and output: the step's query, new K/V rows, lengths and block tables
+    (stage.h, filled by the caller) are copied host->device in one copy, the attention output device->host.
+    The KV cache itself is the resident state and stays in HBM."""
+    stage.upload()
+    dv = stage.d
+    out = decode_step(cfg, bufs, dv["q"], dv["k_new"], dv["v_new"], dv["cu_new"], dv["seq_lens_before"],
+                      dv["seq_lens_after"], dv["block_tables"], cache, stream=stream)
     out_host.copy_(out, non_blocking=True)
     return out_host

@@ -70,3 +70,28 @@ def test_product_package_never_imports_the_oracle():
             if fn.endswith((".py", ".cu", ".cuh", ".h")):
                 src = open(os.path.join(dirpath, fn)).read()
                 assert "import oracle" not in src and "from oracle" not in src and "uq_oracle" not in src, fn
+
+
+def test_host_stage_layout_one_block():
+    """HostStage: the seven step inputs are disjoint, 256-byte aligned views of one host block and of
+    one device block with the same layout (here the 'device' block is a CPU tensor: layout only)."""
+    import torch
+    cfg = uq.UQConfig(8, 2)
+    st = uq.HostStage(cfg, batch=3, total_new=5, max_pages=7, device="cpu")
+    assert tuple(st.h["q"].shape) == (3, 8, 128) and st.h["q"].dtype == torch.bfloat16
+    assert tuple(st.h["k_new"].shape) == (5, 2, 128) and tuple(st.h["block_tables"].shape) == (3, 7)
+    base_h, base_d = st.host.data_ptr(), st.dev.data_ptr()
+    spans = []
+    for name in uq.HostStage.FIELDS:
+        h, d = st.h[name], st.d[name]
+        off = h.data_ptr() - base_h
+        assert off == d.data_ptr() - base_d and off % 256 == 0
+        assert h.shape == d.shape and h.dtype == d.dtype
+        spans.append((off, off + h.numel() * h.element_size()))
+    spans.sort()
+    assert all(a1 <= b0 for (_, a1), (b0, _) in zip(spans, spans[1:])) and spans[-1][1] <= st.nbytes
+    for i, name in enumerate(uq.HostStage.FIELDS):
+        st.h[name].view(torch.uint8).fill_(i + 1)
+    st.upload()
+    for i, name in enumerate(uq.HostStage.FIELDS):
+        assert bool((st.d[name].view(torch.uint8) == i + 1).all())
