@@ -250,3 +250,40 @@ def test_full_size_cfg4_shared_prefix_step_sampled():
         ref, q8 = H.oracle_out(wl, b, L0 + 1, H.bits(q)[b], arrays)
         assert np.array_equal(bufs.q_fp8[b].cpu().numpy(), q8)
         H.check_out(out[b], ref, f"cfg4 full seq {b}")
+
+
+def test_host_staged_step_equals_device_step_and_oracle():
+    """decode_step_host (one staged H2D copy, programmatic launch chain append -> decode -> merge, D2H of O) gives
+    bit-for-bit the output of decode_step on device-resident inputs, over several consecutive steps that cross
+    a page boundary, and that output is within tolerance of the oracle on the grown context."""
+    steps = 3
+    wl = W.make_custom("staged", 21, [47, 200, 16], 16, 2, extra_tokens=steps)
+    cfg = H.cfg_of(wl)
+    B = wl.batch
+    lens0 = (wl.ctx_lens - steps).astype(np.int32)
+    caches = []
+    for _ in range(2):
+        cache, bt = H.fill_cache(cfg, wl, DEV, lens=lens0)
+        caches.append(cache)
+    bufs = [uq.StepBuffers(cfg, B, 3, DEV) for _ in range(2)]
+    cu = torch.arange(B + 1, dtype=torch.int32, device=DEV)
+    stage = uq.HostStage(cfg, B, B, int(bt.shape[1]), DEV)
+    out_host = torch.empty((B, wl.num_q_heads, 128), dtype=torch.bfloat16).pin_memory()
+    for s in range(steps):
+        before = lens0 + s
+        q = W.gen_q(wl, DEV, step=s)
+        k = torch.cat([W.gen_kv(wl, b, int(before[b]), int(before[b]) + 1, DEV)[0] for b in range(B)])
+        v = torch.cat([W.gen_kv(wl, b, int(before[b]), int(before[b]) + 1, DEV)[1] for b in range(B)])
+        before_d = torch.from_numpy(before).to(DEV)
+        after_d = torch.from_numpy(before + 1).to(DEV)
+        ref_out = uq.decode_step(cfg, bufs[0], q, k, v, cu, before_d, after_d, bt, caches[0]).clone()
+        stage.h["q"].copy_(q.cpu()); stage.h["k_new"].copy_(k.cpu()); stage.h["v_new"].copy_(v.cpu())
+        stage.h["cu_new"].copy_(cu.cpu()); stage.h["seq_lens_before"].copy_(before_d.cpu())
+        stage.h["seq_lens_after"].copy_(after_d.cpu()); stage.h["block_tables"].copy_(bt.cpu())
+        uq.decode_step_host(cfg, bufs[1], stage, caches[1], out_host)
+        torch.cuda.synchronize()
+        assert torch.equal(out_host.view(torch.int16), ref_out.cpu().view(torch.int16)), f"step {s}"
+    assert torch.equal(caches[0], caches[1])
+    for b in range(B):
+        ref, _ = H.oracle_out(wl, b, int(wl.ctx_lens[b]), H.bits(q)[b])
+        H.check_out(out_host[b].float().numpy().astype(np.float64), ref, f"staged seq {b}")
