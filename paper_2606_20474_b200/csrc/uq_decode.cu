@@ -288,6 +288,22 @@ __device__ __forceinline__ float ex2(float x) {
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
+// packed fp32 pairs (FFMA2 / FADD2): d = a * s + c and d = a + b on two lanes at once
+__device__ __forceinline__ void ffma2(float& d0, float& d1, float a0, float a1, float s, float c0, float c1) {
+  uint64_t av, sv, cv, dv;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(av) : "f"(a0), "f"(a1));
+  asm("mov.b64 %0, {%1, %2};" : "=l"(sv) : "f"(s), "f"(s));
+  asm("mov.b64 %0, {%1, %2};" : "=l"(cv) : "f"(c0), "f"(c1));
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(dv) : "l"(av), "l"(sv), "l"(cv));
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(d0), "=f"(d1) : "l"(dv));
+}
+__device__ __forceinline__ void fadd2(float& d0, float& d1, float a0, float a1, float b0, float b1) {
+  uint64_t av, bv, dv;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(av) : "f"(a0), "f"(a1));
+  asm("mov.b64 %0, {%1, %2};" : "=l"(bv) : "f"(b0), "f"(b1));
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(dv) : "l"(av), "l"(bv));
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(d0), "=f"(d1) : "l"(dv));
+}
 __device__ __forceinline__ uint32_t hmul2(uint32_t a, uint32_t b) {
   uint32_t d;
   asm("mul.rn.f16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b));
@@ -677,9 +693,9 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
         int gt = 0;                                    // global tile counter
         const uint32_t p_row = sP + (r >> 3) * 256 + (r & 7) * 16;
         while (sc.next(cur, un)) {
-          float mref[NH], lsum[NH];
+          float nmref[NH], lsum[NH];                   // nmref = minus the per-head reference logit
 #pragma unroll
-          for (int j = 0; j < NH; ++j) { mref[j] = -INFINITY; lsum[j] = 0.f; }
+          for (int j = 0; j < NH; ++j) { nmref[j] = INFINITY; lsum[j] = 0.f; }
           int rem = un.tok_end - un.p0 * kPage;        // valid tokens from the first row of the tile on
 
           for (int i = 0; i < un.n_tiles; ++i, rem -= kTilePages * kPage) {
@@ -706,7 +722,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
               float t[NH];
               tmem_ld<NH>(t_s, t);
 #pragma unroll
-              for (int j = 0; j < NH; ++j) t[j] = fmaf(t[j], score_scale, -mref[j]);
+              for (int j = 0; j < NH; j += 2) ffma2(t[j], t[j + 1], t[j], t[j + 1], score_scale, nmref[j], nmref[j + 1]);
               if (tile_partial) {
 #pragma unroll
                 for (int j = 0; j < NH; ++j) t[j] = tok_ok ? t[j] : -INFINITY;
@@ -759,9 +775,9 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
                 float m = sh.wmax[0][j];
 #pragma unroll
                 for (int w = 1; w < kSoftmaxWarps; ++w) m = fmaxf(m, sh.wmax[w][j]);
-                const float mnew = fmaxf(mref[j], m);
-                const float fm = (mref[j] == -INFINITY) ? 0.f : ex2(mref[j] - mnew);
-                mref[j] = mnew;
+                const float mold = -nmref[j], mnew = fmaxf(mold, m);
+                const float fm = (mold == -INFINITY) ? 0.f : ex2(mold - mnew);
+                nmref[j] = -mnew;
                 lsum[j] *= fm;
                 f[j] = fm;
               }
@@ -779,7 +795,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
               bar_softmax();                            // wmax may be rewritten only after every warp read it
             }
 #pragma unroll
-            for (int j = 0; j < NH; ++j) lsum[j] += lt[j];
+            for (int j = 0; j < NH; j += 2) fadd2(lsum[j], lsum[j + 1], lsum[j], lsum[j + 1], lt[j], lt[j + 1]);
 
             // ---- S has been read (QK may overwrite the buffer), P is written, O is consistent with mref
             fence_async_smem();
@@ -804,7 +820,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
 #pragma unroll
             for (int j = 0; j < NH; ++j) {
               sh.lsum[cw][j] = lsum[j];
-              if (cw == 0) sh.mref[j] = mref[j];
+              if (cw == 0) sh.mref[j] = -nmref[j];
             }
           }
           bar_softmax();
