@@ -144,12 +144,17 @@ append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v
   const long long kv_units = (long long)total_new * Hkv;
   if (unit < kv_units) {
     const int n = (int)(unit / Hkv), h = (int)(unit % Hkv);
-    int lo = 0, hi = batch;                   // largest b with cu_new[b] <= n
-    while (hi - lo > 1) {
-      const int mid = (lo + hi) >> 1;
-      if (cu_new[mid] <= n) lo = mid; else hi = mid;
+    // largest b with cu_new[b] <= n: first the guess for evenly spread tokens (the decode step appends one
+    // token per sequence) checked with two independent loads, else a binary search (log2(batch) dependent loads)
+    int b = (int)(((long long)n * batch) / total_new);
+    if (!(cu_new[b] <= n && n < cu_new[b + 1])) {
+      int lo = 0, hi = batch;
+      while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (cu_new[mid] <= n) lo = mid; else hi = mid;
+      }
+      b = lo;
     }
-    const int b = lo;
     const int j = n - cu_new[b];
     const int pos = seq_lens[b] + j;
     const bool odd = pos & 1;

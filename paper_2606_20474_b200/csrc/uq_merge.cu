@@ -31,16 +31,27 @@ merge_kernel(const float* __restrict__ acc, const float* __restrict__ ml, int ro
   float den = 0.f;
   if (M > -INFINITY) {
     const float4* a4 = reinterpret_cast<const float4*>(acc) + (long long)row * S * 32 + lane;
-    for (int s = 0; s < S; ++s) {
-      const float2 v = ml2[s];
-      if (!(v.y > 0.0f)) continue;
-      const float w = __expf(v.x - M);
-      const float4 a = a4[(long long)s * 32];
-      num.x = fmaf(w, a.x, num.x);
-      num.y = fmaf(w, a.y, num.y);
-      num.z = fmaf(w, a.z, num.z);
-      num.w = fmaf(w, a.w, num.w);
-      den = fmaf(w, v.y, den);
+    // eight slots at a time, all loads issued before the first use (the kernel is latency-bound: one pass of
+    // dependent loads instead of one per slot)
+    for (int s0 = 0; s0 < S; s0 += 8) {
+      float2 v[8];
+      float4 a[8];
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const bool in = s0 + k < S;
+        v[k] = in ? ml2[s0 + k] : make_float2(0.f, 0.f);
+        a[k] = in ? a4[(long long)(s0 + k) * 32] : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        if (!(v[k].y > 0.0f)) continue;                // empty slot (or past the last one)
+        const float w = __expf(v[k].x - M);
+        num.x = fmaf(w, a[k].x, num.x);
+        num.y = fmaf(w, a[k].y, num.y);
+        num.z = fmaf(w, a[k].z, num.z);
+        num.w = fmaf(w, a[k].w, num.w);
+        den = fmaf(w, v[k].y, den);
+      }
     }
   }
   const float inv = den > 0.f ? 1.0f / den : 0.f;
