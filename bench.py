@@ -46,7 +46,7 @@ FALLBACK_HBM_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md fallbac
 
 # dram__bytes_read.sum + dram__bytes_write.sum per decode_kernel launch from the committed
 # `ncu --set full` capture of this command (profiles/), keyed by config; None = not captured.
-NCU_TRAFFIC_BYTES = {2: 571_075_072 + 5_741_056}   # dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01_v14_decode_cfg2.md
+NCU_TRAFFIC_BYTES = {2: 571_073_792 + 4_757_760}   # dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01_v16_decode_cfg2.md
 
 
 # ----------------------------------------------------------------------------- helpers
@@ -243,9 +243,11 @@ def run_ours(args, rank, world, local_rank):
     # ---- the same K steps once more with an event on both sides of every decode launch (the dominant kernel's
     # duration for the roofline; an event between two launches ends their programmatic overlap, so this pass
     # is not the one `value` is taken from)
+    # (at most 50 steps: on the long configs a second full-length pass runs into sw_power_cap and times the cap)
+    n_inst = min(args.steps, 50)
     dec_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-              for _ in range(args.steps)]
-    for i in range(args.steps):
+              for _ in range(n_inst)]
+    for i in range(n_inst):
         k_new, v_new = kvs[i % n_in]
         uq.rotate_quantize_append(cfg, k_new, v_new, cu_dev, before_dev, bt_dev, cache,
                                   q=qs[i % n_in], q_fp8=bufs.q_fp8, stream=stream)
@@ -327,7 +329,7 @@ def run_ours(args, rank, world, local_rank):
                      "traffic": NCU_TRAFFIC_BYTES.get(args.config), "algorithmic_bytes": decode_b,
                      "peak_source": peak_src,
                      "timing": "CUDA events around every uq_decode_attention launch, mean over a second pass of the same K steps "
-                               "(events between launches would end the programmatic overlap of the timed pass)"},
+                               "(at most 50; events between launches would end the programmatic overlap of the timed pass)"},
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(args.config, budget_s=args.cpu_budget)
