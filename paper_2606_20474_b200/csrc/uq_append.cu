@@ -102,14 +102,127 @@ __device__ __forceinline__ void load4(const uint16_t* row, int lane, double (&x)
   x[3] = bf16_bits_to_double(raw.y >> 16);
 }
 
+// ---------------------------------------------------------------- float32 fast path
+// The float64 path above takes every rounding decision on exact sums.  The fast path computes the same vector in
+// float32 with a proven error bound and accepts a decision only if the whole error interval falls on one side of
+// every rounding boundary (the decision functions are monotone, so equal results at both ends of the interval
+// mean the exact value gives that result too); otherwise the warp redoes the vector in float64.  Results are
+// therefore identical to the float64 path bit for bit — only the time differs.
+//
+// Error bound of the rotated value z_i (float32) against the oracle's y_i (float64, exact sums): seven levels of
+// float32 additions give |sum - exact| <= ((1+u)^7 - 1) S with u = 2^-24 and S = sum_i |x_i|; the float32 constant
+// 2^-3.5 and the final product add 2u|y| <= 2u S: |z_i - y_i| <= 9.0001 u kappa S < 4.75e-8 S.  kBound leaves 5 %
+// for the float32 evaluation of S and of the bound itself.
+constexpr float kBound = 5.0e-8f;
+
+__device__ __forceinline__ void load4f(const uint16_t* row, int lane, float (&x)[4]) {
+  const uint2 raw = *reinterpret_cast<const uint2*>(row + 4 * lane);
+  x[0] = __uint_as_float(raw.x << 16);
+  x[1] = __uint_as_float(raw.x & 0xFFFF0000u);
+  x[2] = __uint_as_float(raw.y << 16);
+  x[3] = __uint_as_float(raw.y & 0xFFFF0000u);
+}
+
+// four values -> four E2M1 codes (hardware conversion: round to nearest, ties to the even code, saturating),
+// code i in bits 4i..4i+3; "-0" (only the sign bit set) is mapped to +0 as in the float64 path
+__device__ __forceinline__ uint32_t e2m1x4(float r0, float r1, float r2, float r3) {
+  uint32_t n;
+  asm("{\n.reg .b8 t0, t1;\n.reg .b16 h;\n"
+      "cvt.rn.satfinite.e2m1x2.f32 t0, %2, %1;\n"
+      "cvt.rn.satfinite.e2m1x2.f32 t1, %4, %3;\n"
+      "mov.b16 h, {t0, t1};\ncvt.u32.u16 %0, h;\n}\n" : "=r"(n) : "f"(r0), "f"(r1), "f"(r2), "f"(r3));
+  const uint32_t t = n & 0x7777u;
+  const uint32_t nz = ((t + 0x7777u) | t) & 0x8888u;       // bit 3 of a nibble set iff its magnitude is not 0
+  return n & (0x7777u | nz);
+}
+
+// round(log2 t) for a positive normal float t by integer arithmetic on its bits: the exponent, plus one if the
+// significand is at least sqrt(2) (0x3504F3 = float32 significand bits of sqrt(2), rounded down).  Monotone in t.
+__device__ __forceinline__ int round_log2_f32(float t) {
+  return (int)((__float_as_uint(t) + (0x800000u - 0x3504F3u)) >> 23) - 127;
+}
+// E = round(log2(c m)) for m known to +-radius: both ends of the error interval of t = c m — widened by 3.4 u t
+// for the float32 product and the float32 sqrt(2) — must give the same exponent; false otherwise.
+__device__ __forceinline__ bool scale_exponent_f32(float c, float m, float radius, int& E) {
+  const float t = __fmul_rn(c, m);
+  const float d = __fmaf_rn(t, 2.0e-7f, __fmul_rn(__fmul_rn(c, radius), 1.0001f));
+  const float lo = t - d, hi = t + d;
+  E = round_log2_f32(hi);
+  return (lo > 1e-30f) && (hi < 1e30f) && (round_log2_f32(lo) == E);
+}
+
+// 2^-E as a float (|E| <= 100 is checked by the callers)
+__device__ __forceinline__ float pow2_neg(int E) { return __uint_as_float((uint32_t)(127 - E) << 23); }
+
+// K of one token, float32: codes (as store_k packs them) and scale exponent; false if any decision is unsafe.
+__device__ __forceinline__ bool encode_k_fast(const uint16_t* krow, int lane, double c_k, uint32_t& h16, int& E) {
+  float x[4];
+  load4f(krow, lane, x);
+  float S = (fabsf(x[0]) + fabsf(x[1])) + (fabsf(x[2]) + fabsf(x[3]));
+#pragma unroll
+  for (int k = 1; k < 32; k <<= 1) S += __shfl_xor_sync(kFull, S, k);
+  // butterflies: index bits 0-1 inside the lane, bits 2-6 through shuffles
+  const float a0 = x[0] + x[1], a1 = x[0] - x[1], a2 = x[2] + x[3], a3 = x[2] - x[3];
+  x[0] = a0 + a2; x[2] = a0 - a2; x[1] = a1 + a3; x[3] = a1 - a3;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    const float sgn = ((lane >> k) & 1) ? -1.0f : 1.0f;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      const float other = __shfl_xor_sync(kFull, x[r], 1 << k);
+      x[r] = __fmaf_rn(x[r], sgn, other);               // exact product: one rounding, as an addition
+    }
+  }
+  const float kappa = 0x1.6a09e6p-4f;                     // float32 nearest to 2^-3.5
+#pragma unroll
+  for (int r = 0; r < 4; ++r) x[r] = __fmul_rn(x[r], kappa);
+  const float eps = __fmul_rn(S, kBound);
+  bool ok = (S > 1e-30f) && (S < 1e30f);                  // no underflow / overflow / NaN games on the fast path
+  // ---- scale exponent of the group (8 lanes x 4 channels)
+  float m = fmaxf(fmaxf(fabsf(x[0]), fabsf(x[1])), fmaxf(fabsf(x[2]), fabsf(x[3])));
+#pragma unroll
+  for (int s = 1; s <= 4; s <<= 1) m = fmaxf(m, __shfl_xor_sync(kFull, m, s));
+  ok = scale_exponent_f32((float)c_k, m, eps, E) && ok && (E >= -100) && (E <= 100);
+  // ---- codes: the error interval of every element must round to one code
+  const float sc = pow2_neg(ok ? E : 0);
+  const float er = __fmaf_rn(__fmul_rn(eps, sc), 1.0001f, 1.2e-6f);   // + the rounding of the two additions below
+  float r[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) r[i] = __fmul_rn(x[i], sc);  // exact (power of two)
+  const uint32_t lo = e2m1x4(r[0] - er, r[1] - er, r[2] - er, r[3] - er);
+  const uint32_t hi = e2m1x4(r[0] + er, r[1] + er, r[2] + er, r[3] + er);
+  h16 = lo;
+  return ok && (lo == hi);
+}
+
+// V of one token, float32: exact (no rotation: the bf16 values themselves are scaled by a power of two); only the
+// scale exponent needs the float64 product c * m.  Returns the codes as encode_v does; false -> use encode_v.
+__device__ __forceinline__ bool encode_v_fast(const uint16_t* vrow, int lane, double c_v, uint32_t& codes, int& E) {
+  float x[4];
+  load4f(vrow, lane, x);
+  float m = fmaxf(fmaxf(fabsf(x[0]), fabsf(x[1])), fmaxf(fabsf(x[2]), fabsf(x[3])));
+#pragma unroll
+  for (int s = 1; s <= 4; s <<= 1) m = fmaxf(m, __shfl_xor_sync(kFull, m, s));
+  const bool zero = (m == 0.0f);                           // an all-zero group: E = -127, codes 0 (as scale_exponent)
+  const bool ok = zero || (scale_exponent_f32((float)c_v, m, 0.0f, E) && (E >= -100) && (E <= 100));
+  const float sc = pow2_neg((ok && !zero) ? E : 0);
+  const uint32_t h = e2m1x4(__fmul_rn(x[0], sc), __fmul_rn(x[1], sc), __fmul_rn(x[2], sc), __fmul_rn(x[3], sc));
+  codes = zero ? 0u : ((h & 0xFu) | ((h & 0xF0u) << 4) | ((h & 0xF00u) << 8) | ((h & 0xF000u) << 12));
+  if (zero) E = -127;
+  return ok;
+}
+
 // Encode + store K of one token: codes into the word-permuted K block, scale word.
 __device__ __forceinline__ void store_k(const uint16_t* krow, uint8_t* rec, int t, int lane, double c_k) {
-  double x[4];
-  load4(krow, lane, x);
-  wht128(x, lane);
-  const int E = group_exponent(x, c_k);
-  uint32_t h16 = e2m1_code(x[0], E) | (e2m1_code(x[1], E) << 4) | (e2m1_code(x[2], E) << 8) |
-                 (e2m1_code(x[3], E) << 12);
+  uint32_t h16;
+  int E;
+  if (!__all_sync(kFull, encode_k_fast(krow, lane, c_k, h16, E))) {   // float64 when any decision was too close
+    double x[4];
+    load4(krow, lane, x);
+    wht128(x, lane);
+    E = group_exponent(x, c_k);
+    h16 = e2m1_code(x[0], E) | (e2m1_code(x[1], E) << 4) | (e2m1_code(x[2], E) << 8) | (e2m1_code(x[3], E) << 12);
+  }
   const uint32_t other = __shfl_down_sync(kFull, h16, 1);
   if ((lane & 1) == 0) {                      // logical order: word j = channels 8j..8j+7
     *reinterpret_cast<uint32_t*>(rec + kOffKCodes + 64 * t + 4 * (lane >> 1)) = h16 | (other << 16);
@@ -123,12 +236,16 @@ __device__ __forceinline__ void store_k(const uint16_t* krow, uint8_t* rec, int 
 // Encode V of one token: returns the lane's four 4-bit codes (one per byte of the result) and
 // stores the token's scale bytes.
 __device__ __forceinline__ uint32_t encode_v(const uint16_t* vrow, uint8_t* rec, int t, int lane, double c_v) {
-  double x[4];
-  load4(vrow, lane, x);
-  const int E = group_exponent(x, c_v);
+  uint32_t codes;
+  int E;
+  if (!__all_sync(kFull, encode_v_fast(vrow, lane, c_v, codes, E))) {
+    double x[4];
+    load4(vrow, lane, x);
+    E = group_exponent(x, c_v);
+    codes = e2m1_code(x[0], E) | (e2m1_code(x[1], E) << 8) | (e2m1_code(x[2], E) << 16) | (e2m1_code(x[3], E) << 24);
+  }
   if ((lane & 7) == 0) rec[kOffVScales + 32 * (t >> 3) + 8 * (lane >> 3) + (t & 7)] = (uint8_t)(E + 127);
-  return e2m1_code(x[0], E) | (e2m1_code(x[1], E) << 8) | (e2m1_code(x[2], E) << 16) |
-         (e2m1_code(x[3], E) << 24);
+  return codes;
 }
 
 __global__ void __launch_bounds__(128)
@@ -140,20 +257,31 @@ append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v
   pdl_launch_dependents();
   pdl_wait();                                          // inputs and cache may come from the kernel before this one
   const int lane = threadIdx.x & 31;
-  const long long unit = (long long)blockIdx.x * 4 + (threadIdx.x >> 5);
-  const long long kv_units = (long long)total_new * Hkv;
-  if (unit < kv_units) {
-    const int n = (int)(unit / Hkv), h = (int)(unit % Hkv);
+  // grid: y < Hkv -> K/V of kv head y, token row 4 x + warp;  y >= Hkv -> query rows (no division anywhere)
+  if ((int)blockIdx.y < Hkv) {
+    const int n = (int)blockIdx.x * 4 + (int)(threadIdx.x >> 5), h = (int)blockIdx.y;
+    if (n >= total_new) return;
     // largest b with cu_new[b] <= n: first the guess for evenly spread tokens (the decode step appends one
-    // token per sequence) checked with two independent loads, else a binary search (log2(batch) dependent loads)
-    int b = (int)(((long long)n * batch) / total_new);
+    // token per sequence) checked with two independent loads; else a two-level search by the whole warp (32
+    // entries per level, one load per lane and a ballot), or a binary search beyond 1024 sequences
+    int b = (total_new == batch) ? n : 0;
     if (!(cu_new[b] <= n && n < cu_new[b + 1])) {
-      int lo = 0, hi = batch;
-      while (hi - lo > 1) {
-        const int mid = (lo + hi) >> 1;
-        if (cu_new[mid] <= n) lo = mid; else hi = mid;
+      if (batch <= 1024) {
+        const int step = (batch + 31) >> 5;             // entries per first-level block
+        const int i1 = min((lane + 1) * step, batch);
+        const int blk = __popc(__ballot_sync(kFull, cu_new[i1] <= n && i1 < batch));   // blocks wholly <= n
+        const int base = min(blk * step, batch - 1);
+        const int i2 = min(base + lane, batch - 1);
+        const unsigned le = __ballot_sync(kFull, lane < step && base + lane < batch && cu_new[i2] <= n);
+        b = base + (31 - __clz((int)(le | 1u)));        // cu_new[base] <= n always holds
+      } else {
+        int lo = 0, hi = batch;
+        while (hi - lo > 1) {
+          const int mid = (lo + hi) >> 1;
+          if (cu_new[mid] <= n) lo = mid; else hi = mid;
+        }
+        b = lo;
       }
-      b = lo;
     }
     const int j = n - cu_new[b];
     const int pos = seq_lens[b] + j;
@@ -183,7 +311,7 @@ append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v
     }
     return;
   }
-  const long long qu = unit - kv_units;
+  const long long qu = ((long long)((int)blockIdx.y - Hkv) * gridDim.x + blockIdx.x) * 4 + (threadIdx.x >> 5);
   if (q != nullptr && qu < (long long)batch * Hq) {
     double x[4];
     load4(q + qu * kHeadDim, lane, x);
@@ -223,15 +351,19 @@ extern "C" int32_t uq_rotate_quantize_append(const uq_config* cfg, const void* k
     set_error("append: misaligned pointer (k/v/q 8 B, cache 16 B, q_fp8 4 B)");
     return UQ_ERR_INVALID_ARG;
   }
-  const long long units = (long long)total_new * cfg->num_kv_heads +
-                          (q ? (long long)batch * cfg->num_q_heads : 0);
-  if (units == 0) return UQ_OK;
-  const long long blocks = (units + 3) / 4;
-  if (blocks > 0x7fffffffLL) {
+  const long long q_rows = q ? (long long)batch * cfg->num_q_heads : 0;
+  if (total_new == 0 && q_rows == 0) return UQ_OK;
+  // grid.x: blocks of 4 token rows (K/V part, grid.y = kv head) — widened if the query rows would need more than
+  // 60000 further grid rows; grid.y beyond the kv heads: query rows, 4 * grid.x per grid row
+  long long gx = ((long long)total_new + 3) / 4;
+  gx = gx > (q_rows + 4 * 60000LL - 1) / (4 * 60000LL) ? gx : (q_rows + 4 * 60000LL - 1) / (4 * 60000LL);
+  if (gx < 1) gx = 1;
+  const long long gy = cfg->num_kv_heads + (q_rows + 4 * gx - 1) / (4 * gx);
+  if (gx > 0x7fffffffLL || gy > 65535) {
     set_error("append: too many work units");
     return UQ_ERR_INVALID_ARG;
   }
-  return check_cuda(launch_pdl(append_kernel, dim3((unsigned)blocks), dim3(128), 0, (cudaStream_t)stream,
+  return check_cuda(launch_pdl(append_kernel, dim3((unsigned)gx, (unsigned)gy), dim3(128), 0, (cudaStream_t)stream,
                                (const uint16_t*)k_new, (const uint16_t*)v_new, cu_new, seq_lens, block_tables,
                                (int)max_pages, (int)batch, (int)total_new, (int)cfg->num_q_heads,
                                (int)cfg->num_kv_heads, (uint8_t*)cache, (const uint16_t*)q, (uint8_t*)q_fp8,
