@@ -287,3 +287,42 @@ def test_host_staged_step_equals_device_step_and_oracle():
     for b in range(B):
         ref, _ = H.oracle_out(wl, b, int(wl.ctx_lens[b]), H.bits(q)[b])
         H.check_out(out_host[b].float().numpy().astype(np.float64), ref, f"staged seq {b}")
+
+
+def test_append_on_rounding_boundaries_is_bit_exact():
+    """The append kernel's float32 fast path must hand every close call to float64: V elements exactly on the
+    E2M1 ties (0.25, 0.75, 1.25, 1.75, 2.5, 3.5, 5 times the group scale), group maxima on both sides of the
+    scale-exponent thresholds 2^(k-1/2)/c (nextafter in bf16), constant and one-hot K rows (rotated vectors with
+    127 exact zeros / 128 equal magnitudes), huge and tiny magnitudes — all compared bit for bit with the oracle."""
+    L = 192
+    wl = W.make_custom("bound", 31, [L], 8, 2)
+    cfg = H.cfg_of(wl)
+    g = torch.Generator(device="cpu"); g.manual_seed(1234)
+    k = torch.randn((L, 2, 128), generator=g)
+    v = torch.randn((L, 2, 128), generator=g)
+    ties = torch.tensor([0.25, 0.75, 1.25, 1.75, 2.5, 3.5, 5.0, 6.0, 0.5, 1.0, 1.5, 2.0, 3.0, 4.0, 0.0, -0.25])
+    for t in range(0, 64):                                  # V: group max 6 * 2^e -> E = e; the rest sits on ties
+        e = (t % 23) - 11
+        row = ties[torch.randint(0, 16, (2, 128), generator=g)] * (1.0 if t % 2 else -1.0)
+        row[:, ::32] = 6.0                                 # one maximum per 32-group
+        v[t] = row * 2.0 ** e
+    thr = [2.0 ** (kk - 0.5) / 0.15600000321865082 for kk in range(-6, 7)]
+    for t in range(64, 96):                                 # V: group maxima right below / above a scale threshold
+        x = torch.tensor(thr[t % len(thr)], dtype=torch.float32).to(torch.bfloat16)
+        nb = (x.view(torch.int16) + (1 if t % 2 else -1)).view(torch.bfloat16)
+        row = torch.rand((2, 128), generator=g) * float(x) * 0.9
+        row[:, ::32] = float(nb) if t % 3 else float(x)
+        v[t] = row
+    k[96] = 0.75                                            # constant rows: one nonzero rotated value, 127 zeros
+    k[97] = -3.0
+    k[98] = 0; k[98, :, 5] = 2.0                            # one-hot rows: 128 equal magnitudes
+    k[99] = 0; k[99, :, 127] = -1.0 / 3.0
+    k[100] *= 1e20; k[101] *= 1e-20; v[100] *= 1e25; v[101] *= 1e-25
+    k[102] = 0; v[102] = 0
+    k, v = k.to(torch.bfloat16).to(DEV), v.to(torch.bfloat16).to(DEV)
+    cache = uq.alloc_cache(cfg, wl.num_pages, DEV)
+    bt = torch.from_numpy(wl.block_tables).to(DEV)
+    H.append_tokens(cfg, cache, bt, np.zeros(1, np.int32), np.array([L], np.int32), k, v)
+    torch.cuda.synchronize()
+    arrays = oracle.encode_kv(H.bits(k), H.bits(v))
+    H.compare_cache(cache, wl, 0, L, arrays)
