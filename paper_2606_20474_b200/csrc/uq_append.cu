@@ -154,10 +154,10 @@ __device__ __forceinline__ bool scale_exponent_f32(float c, float m, float radiu
 // 2^-E as a float (|E| <= 100 is checked by the callers)
 __device__ __forceinline__ float pow2_neg(int E) { return __uint_as_float((uint32_t)(127 - E) << 23); }
 
-// K of one token, float32: codes (as store_k packs them) and scale exponent; false if any decision is unsafe.
-__device__ __forceinline__ bool encode_k_fast(const uint16_t* krow, int lane, double c_k, uint32_t& h16, int& E) {
-  float x[4];
-  load4f(krow, lane, x);
+// y = H_128 x * 2^-3.5 in float32 for the lane's 4 channels; eps = bound of |x[i] - exact|; false if the vector is
+// outside the range the bound was derived for (underflow / overflow / NaN: float64 takes those).
+__device__ __forceinline__ bool wht128_f32(const uint16_t* row, int lane, float (&x)[4], float& eps) {
+  load4f(row, lane, x);
   float S = (fabsf(x[0]) + fabsf(x[1])) + (fabsf(x[2]) + fabsf(x[3]));
 #pragma unroll
   for (int k = 1; k < 32; k <<= 1) S += __shfl_xor_sync(kFull, S, k);
@@ -176,8 +176,44 @@ __device__ __forceinline__ bool encode_k_fast(const uint16_t* krow, int lane, do
   const float kappa = 0x1.6a09e6p-4f;                     // float32 nearest to 2^-3.5
 #pragma unroll
   for (int r = 0; r < 4; ++r) x[r] = __fmul_rn(x[r], kappa);
-  const float eps = __fmul_rn(S, kBound);
-  bool ok = (S > 1e-30f) && (S < 1e30f);                  // no underflow / overflow / NaN games on the fast path
+  eps = __fmul_rn(S, kBound);
+  return (S > 1e-30f) && (S < 1e30f);                     // no underflow / overflow / NaN games on the fast path
+}
+
+// four values -> four OCP E4M3 bytes (hardware conversion: round to nearest even, saturating to +-448), value i in
+// byte i; "-0" is mapped to +0 as in the float64 path
+__device__ __forceinline__ uint32_t e4m3x4(float r0, float r1, float r2, float r3) {
+  uint32_t n;
+  asm("{\n.reg .b16 h0, h1;\n"
+      "cvt.rn.satfinite.e4m3x2.f32 h0, %2, %1;\n"
+      "cvt.rn.satfinite.e4m3x2.f32 h1, %4, %3;\n"
+      "mov.b32 %0, {h0, h1};\n}\n" : "=r"(n) : "f"(r0), "f"(r1), "f"(r2), "f"(r3));
+  const uint32_t t = n & 0x7F7F7F7Fu;
+  const uint32_t nz = ((t + 0x7F7F7F7Fu) | t) & 0x80808080u;   // bit 7 of a byte set iff its magnitude is not 0
+  return n & (0x7F7F7F7Fu | nz);
+}
+
+// Query row, float32: the four E4M3 bytes of the lane; false if any element's error interval straddles a rounding
+// boundary of E4M3 (the conversion is monotone).
+__device__ __forceinline__ bool encode_q_fast(const uint16_t* qrow, int lane, uint32_t& w) {
+  float x[4], eps;
+  const bool ok = wht128_f32(qrow, lane, x, eps);
+  const float er = __fmaf_rn(eps, 1.0001f, 1e-37f);       // the two additions below round: widen by their ulp as well
+  float lo[4], hi[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const float slack = __fmaf_rn(fabsf(x[i]), 1.2e-7f, er);
+    lo[i] = x[i] - slack;
+    hi[i] = x[i] + slack;
+  }
+  w = e4m3x4(lo[0], lo[1], lo[2], lo[3]);
+  return ok && (w == e4m3x4(hi[0], hi[1], hi[2], hi[3]));
+}
+
+// K of one token, float32: codes (as store_k packs them) and scale exponent; false if any decision is unsafe.
+__device__ __forceinline__ bool encode_k_fast(const uint16_t* krow, int lane, double c_k, uint32_t& h16, int& E) {
+  float x[4], eps;
+  bool ok = wht128_f32(krow, lane, x, eps);
   // ---- scale exponent of the group (8 lanes x 4 channels)
   float m = fmaxf(fmaxf(fabsf(x[0]), fabsf(x[1])), fmaxf(fabsf(x[2]), fabsf(x[3])));
 #pragma unroll
@@ -313,11 +349,13 @@ append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v
   }
   const long long qu = ((long long)((int)blockIdx.y - Hkv) * gridDim.x + blockIdx.x) * 4 + (threadIdx.x >> 5);
   if (q != nullptr && qu < (long long)batch * Hq) {
-    double x[4];
-    load4(q + qu * kHeadDim, lane, x);
-    wht128(x, lane);
-    const uint32_t w = e4m3_byte(x[0]) | (e4m3_byte(x[1]) << 8) | (e4m3_byte(x[2]) << 16) |
-                       (e4m3_byte(x[3]) << 24);
+    uint32_t w;
+    if (!__all_sync(kFull, encode_q_fast(q + qu * kHeadDim, lane, w))) {   // float64 when any byte was too close
+      double x[4];
+      load4(q + qu * kHeadDim, lane, x);
+      wht128(x, lane);
+      w = e4m3_byte(x[0]) | (e4m3_byte(x[1]) << 8) | (e4m3_byte(x[2]) << 16) | (e4m3_byte(x[3]) << 24);
+    }
     *reinterpret_cast<uint32_t*>(q_fp8 + qu * kHeadDim + 4 * lane) = w;
   }
 }

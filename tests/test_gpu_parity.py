@@ -326,3 +326,10 @@ def test_append_on_rounding_boundaries_is_bit_exact():
     torch.cuda.synchronize()
     arrays = oracle.encode_kv(H.bits(k), H.bits(v))
     H.compare_cache(cache, wl, 0, L, arrays)
+    # query rows: constant, one-hot, huge, tiny, zero, and random ones -> q_fp8 bytes against the oracle
+    q = torch.randn((1, 8, 128), generator=g)
+    q[0, 0] = 0.75; q[0, 1] = 0; q[0, 1, 17] = -2.0; q[0, 2] *= 1e20; q[0, 3] *= 1e-20; q[0, 4] = 0
+    q[0, 5] = 448.0 / 11.313708498984761                    # rotated value 448-ish: the saturation boundary
+    q = q.to(torch.bfloat16).to(DEV)
+    _, q_fp8, _ = H.run_decode(cfg, cache, bt, wl.ctx_lens, q, 1)
+    assert np.array_equal(q_fp8[0].cpu().numpy(), oracle.encode_q(H.bits(q)[0]))
