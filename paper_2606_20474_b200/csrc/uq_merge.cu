@@ -19,38 +19,64 @@ merge_kernel(const float* __restrict__ acc, const float* __restrict__ ml, int ro
   const int row = blockIdx.x * 4 + (threadIdx.x >> 5);
   if (row >= rows) return;
   const float2* ml2 = reinterpret_cast<const float2*>(ml) + (long long)row * S;
-  // pass 1: M = max over non-empty splits (lanes stride over splits, then warp max)
-  float M = -INFINITY;
-  for (int s = lane; s < S; s += 32) {
-    const float2 v = ml2[s];
-    if (v.y > 0.0f) M = fmaxf(M, v.x);
-  }
-#pragma unroll
-  for (int o = 16; o; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+  const float4* a4 = reinterpret_cast<const float4*>(acc) + (long long)row * S * 32 + lane;
   float4 num = make_float4(0.f, 0.f, 0.f, 0.f);
   float den = 0.f;
-  if (M > -INFINITY) {
-    const float4* a4 = reinterpret_cast<const float4*>(acc) + (long long)row * S * 32 + lane;
-    // eight slots at a time, all loads issued before the first use (the kernel is latency-bound: one pass of
-    // dependent loads instead of one per slot)
-    for (int s0 = 0; s0 < S; s0 += 8) {
-      float2 v[8];
-      float4 a[8];
+  if (S <= 8) {
+    // the usual case, one round of loads: every lane reads all (m, l) pairs (broadcast) and its 16 bytes of every
+    // accumulator before anything is used; the maximum needs no exchange between lanes
+    float2 v[8];
+    float4 a[8];
 #pragma unroll
-      for (int k = 0; k < 8; ++k) {
-        const bool in = s0 + k < S;
-        v[k] = in ? ml2[s0 + k] : make_float2(0.f, 0.f);
-        a[k] = in ? a4[(long long)(s0 + k) * 32] : make_float4(0.f, 0.f, 0.f, 0.f);
-      }
+    for (int k = 0; k < 8; ++k) {
+      const bool in = k < S;
+      v[k] = in ? ml2[k] : make_float2(0.f, 0.f);
+      a[k] = in ? a4[(long long)k * 32] : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    float M = -INFINITY;
 #pragma unroll
-      for (int k = 0; k < 8; ++k) {
-        if (!(v[k].y > 0.0f)) continue;                // empty slot (or past the last one)
-        const float w = __expf(v[k].x - M);
-        num.x = fmaf(w, a[k].x, num.x);
-        num.y = fmaf(w, a[k].y, num.y);
-        num.z = fmaf(w, a[k].z, num.z);
-        num.w = fmaf(w, a[k].w, num.w);
-        den = fmaf(w, v[k].y, den);
+    for (int k = 0; k < 8; ++k)
+      if (v[k].y > 0.0f) M = fmaxf(M, v[k].x);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      if (!(v[k].y > 0.0f)) continue;                  // empty slot (or past the last one)
+      const float w = __expf(v[k].x - M);
+      num.x = fmaf(w, a[k].x, num.x);
+      num.y = fmaf(w, a[k].y, num.y);
+      num.z = fmaf(w, a[k].z, num.z);
+      num.w = fmaf(w, a[k].w, num.w);
+      den = fmaf(w, v[k].y, den);
+    }
+  } else {
+    // pass 1: M = max over non-empty splits (lanes stride over splits, then warp max)
+    float M = -INFINITY;
+    for (int s = lane; s < S; s += 32) {
+      const float2 v = ml2[s];
+      if (v.y > 0.0f) M = fmaxf(M, v.x);
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+    if (M > -INFINITY) {
+      // eight slots at a time, all loads issued before the first use (the kernel is latency-bound)
+      for (int s0 = 0; s0 < S; s0 += 8) {
+        float2 v[8];
+        float4 a[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const bool in = s0 + k < S;
+          v[k] = in ? ml2[s0 + k] : make_float2(0.f, 0.f);
+          a[k] = in ? a4[(long long)(s0 + k) * 32] : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          if (!(v[k].y > 0.0f)) continue;              // empty slot (or past the last one)
+          const float w = __expf(v[k].x - M);
+          num.x = fmaf(w, a[k].x, num.x);
+          num.y = fmaf(w, a[k].y, num.y);
+          num.z = fmaf(w, a[k].z, num.z);
+          num.w = fmaf(w, a[k].w, num.w);
+          den = fmaf(w, v[k].y, den);
+        }
       }
     }
   }
