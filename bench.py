@@ -426,6 +426,51 @@ def run_reference(args):
             "gpu_launches": 0}
 
 
+# ----------------------------------------------------------------------------- bulk append
+def run_bulk_append(args):
+    """Not the headline metric: prefill-sized quantize-on-append of one sequence of the chosen config (32,768
+    new tokens x Hkv heads per call by default), algorithmic bytes = 2 * 256 B read + 136 B written per
+    (token, kv head), CUDA events over K calls."""
+    import paper_2606_20474_b200 as uq
+    from paper_2606_20474_b200 import workloads as W
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the hot path has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    wl = _workload(args.config, 0)
+    cfg = uq.UQConfig(num_q_heads=wl.num_q_heads, num_kv_heads=wl.num_kv_heads)
+    n = min(args.bulk_append, int(wl.ctx_lens[0]))
+    cache = uq.alloc_cache(cfg, wl.num_pages, dev)
+    bt = torch.from_numpy(wl.block_tables).to(dev)
+    k, v = W.gen_kv(wl, 0, 0, n, dev)
+    before = torch.zeros(wl.batch, dtype=torch.int32, device=dev)
+    cu = np.zeros(wl.batch + 1, np.int32); cu[1:] = n
+    cu = torch.from_numpy(cu).to(dev)
+    stream = torch.cuda.current_stream()
+    for _ in range(max(args.warmup, 3)):
+        uq.rotate_quantize_append(cfg, k, v, cu, before, bt, cache, stream=stream)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        uq.rotate_quantize_append(cfg, k, v, cu, before, bt, cache, stream=stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    nbytes = n * wl.num_kv_heads * (2 * 2 * wl.head_dim + 136)
+    peak, peak_src = _peaks()
+    gbs = nbytes / (ms * 1e-3) / 1e9
+    return {"metric": "bulk_append_hbm_gbps", "value": round(gbs, 1), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": round(ms, 5), "higher_is_better": True, "dtype": "f32/f64->fp4",
+            "data": "synthetic", "impl": "ours",
+            "config": {"workload": f"bulk quantize-on-append, {n} tokens x {wl.num_kv_heads} kv heads of {wl.name} per call "
+                                   f"(source rows {2 * n * wl.num_kv_heads * 256 / 1e6:.1f} MB > L2 only beyond 246k tokens: "
+                                   "reads may hit L2 between calls)"},
+            "bytes_per_step": nbytes, "gpu_launches": args.steps,
+            "roofline": {"bound": "hbm", "kernel": "uq::append_kernel", "achieved": round(gbs, 1), "peak": peak,
+                         "unit": "GB/s", "frac": round(gbs / peak, 4), "traffic": None, "peak_source": peak_src}}
+
+
 # ----------------------------------------------------------------------------- main
 def main():
     ap = argparse.ArgumentParser()
@@ -437,6 +482,8 @@ def main():
                     help="BASELINE.json config number (1-based); 2 is the one the metric is quoted on")
     ap.add_argument("--splits", type=int, default=0, help="num_splits override (0 = uq_suggest_num_splits)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--bulk-append", type=int, default=0, metavar="TOKENS",
+                    help="instead of the decode step, time bulk quantize-on-append of TOKENS new tokens per call")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--ref-budget", type=float, default=90.0, help="seconds for the whole --impl reference run")
     args = ap.parse_args()
@@ -445,6 +492,10 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
 
+    if args.bulk_append > 0:
+        if rank == 0:
+            print(json.dumps(run_bulk_append(args)), flush=True)
+        return 0
     if args.impl == "reference":
         if rank == 0:
             print(json.dumps(run_reference(args)), flush=True)
