@@ -333,3 +333,71 @@ def test_append_on_rounding_boundaries_is_bit_exact():
     q = q.to(torch.bfloat16).to(DEV)
     _, q_fp8, _ = H.run_decode(cfg, cache, bt, wl.ctx_lens, q, 1)
     assert np.array_equal(q_fp8[0].cpu().numpy(), oracle.encode_q(H.bits(q)[0]))
+
+
+def test_random_small_configs():
+    """Seeded sweep over head geometries, batch sizes (up to more items than resident CTAs), length mixes (empty,
+    one token, tile multiples +-1, ragged) and slot counts 1..6: cache image bit-exact, outputs in tolerance."""
+    rng = np.random.default_rng(7)
+    heads = [(8, 8), (8, 1), (16, 1), (12, 2), (32, 2), (6, 1), (10, 2), (64, 4), (48, 8)]
+    for case in range(24):
+        hq, hkv = heads[rng.integers(len(heads))]
+        kind = int(rng.integers(6))
+        B = int(rng.integers(1, 7)) if kind < 4 else int(rng.integers(40, 130))
+        if kind == 0: lens = rng.integers(0, 40, B)
+        elif kind == 1: lens = rng.integers(100, 700, B)
+        elif kind == 2: lens = rng.integers(0, 3000, B)
+        elif kind == 3: lens = np.array([int(rng.integers(1, 5)) * 128 + int(rng.integers(-1, 2)) for _ in range(B)])
+        else: lens = rng.integers(0, 260, B)
+        if lens.sum() == 0: lens[0] = 1
+        S = int(rng.integers(1, 7))
+        wl = W.make_custom(f"rnd{case}", 1000 + case, [int(x) for x in lens], hq, hkv,
+                           peaked_frac=float(rng.choice([0.0, 0.3])))
+        cfg = H.cfg_of(wl)
+        cache, bt = H.fill_cache(cfg, wl, DEV)
+        q = W.gen_q(wl, DEV)
+        out, q_fp8, _ = H.run_decode(cfg, cache, bt, wl.ctx_lens, q, S)
+        out = out.float().cpu().numpy().astype(np.float64)
+        for b in rng.choice(B, min(B, 6), replace=False):
+            L = int(wl.ctx_lens[b])
+            if L == 0:
+                assert np.all(out[b] == 0), f"case {case} seq {b}: an empty sequence gives zeros"
+                continue
+            arrays = H.oracle_sequence_cache(wl, int(b), L, DEV)
+            H.compare_cache(cache, wl, int(b), L, arrays)
+            ref, q8 = H.oracle_out(wl, int(b), L, H.bits(q)[b], arrays)
+            assert np.array_equal(q_fp8[b].cpu().numpy(), q8)
+            H.check_out(out[b], ref, f"case {case} {hq}/{hkv} B={B} S={S} seq {b} len {L}")
+
+
+@pytest.mark.parametrize("B", [33, 700, 1025, 1500])
+def test_random_multi_sequence_appends(B):
+    """Several sequences per append call with irregular counts (zeros included) over consecutive calls: the guess,
+    the two-level warp search (batch <= 1024) and the binary search (beyond) of cu_new all land every token in its
+    slot — cache image of sampled sequences bit-exact against the oracle."""
+    rng = np.random.default_rng(B)
+    lens = rng.integers(0, 50, B)
+    lens[rng.integers(0, B, B // 3)] = 0
+    wl = W.make_custom(f"ma{B}", 2000 + B, [int(x) for x in lens], 8, 2)
+    cfg = H.cfg_of(wl)
+    cache = uq.alloc_cache(cfg, wl.num_pages, DEV)
+    cache.fill_(0x5A)
+    bt = torch.from_numpy(wl.block_tables).to(DEV)
+    full, pos = {}, np.zeros(B, np.int32)
+    while (pos < wl.ctx_lens).any():
+        counts = np.minimum(rng.integers(0, 20, B), wl.ctx_lens - pos).astype(np.int32)
+        if counts.sum() == 0:
+            continue
+        ks, vs = [], []
+        for b in np.nonzero(counts)[0]:
+            if b not in full:
+                full[b] = W.gen_kv(wl, int(b), 0, int(wl.ctx_lens[b]), DEV)
+            ks.append(full[b][0][pos[b]:pos[b] + counts[b]])
+            vs.append(full[b][1][pos[b]:pos[b] + counts[b]])
+        H.append_tokens(cfg, cache, bt, pos, counts, torch.cat(ks), torch.cat(vs))
+        pos = pos + counts
+    torch.cuda.synchronize()
+    for b in rng.choice(B, 10, replace=False):
+        L = int(wl.ctx_lens[b])
+        if L:
+            H.compare_cache(cache, wl, int(b), L, H.oracle_sequence_cache(wl, int(b), L, DEV))
