@@ -98,7 +98,9 @@ size_t uq_cache_record_bytes(const uq_config* cfg);
  *
  * Every rounding decision (scale exponent, E2M1 code, E4M3 byte) is taken on float64 values of
  * the exactly-computed rotation (reading G1), so codes, scale bytes and q_fp8 are
- * bit-identical to the float64 oracle.  Tokens of one sequence that share a V-code byte (slots
+ * bit-identical to the float64 oracle.  (A float32 fast path computes the same vector with a proven error bound
+ * and accepts a decision only if the whole error interval lies on one side of every rounding boundary; any other
+ * vector is redone in float64: the bytes written are those of the float64 path.)  Tokens of one sequence that share a V-code byte (slots
  * 2i, 2i+1) may arrive in one call or in successive calls on the same stream; two concurrent
  * calls must not append to the same page.  Appending to a page shared by several block tables
  * is the caller's error.
