@@ -1,7 +1,7 @@
 // uq_append.cu — quantize-on-append: Alg. 1 "Write" l.1-5 and "Decode" l.6 of
 // arxiv/paper_2606_20474.
 //
-// Record layout: include/uq.h.  One warp per (new token pair, kv head) or per (sequence, q head).  A lane owns 4 consecutive
+// Record layout: include/uq.h.  One warp per (aligned octet of token positions, kv head) or per (sequence, q head).  A lane owns 4 consecutive
 // channels of the 128-channel vector.  The Walsh-Hadamard rotation is an in-register butterfly:
 // index bits 0-1 inside the lane, bits 2-6 through warp shuffles.  All of it runs in float64:
 // sums of 128 bf16 values are exact in double, so every rounding decision (scale exponent,
@@ -293,57 +293,64 @@ append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v
   pdl_launch_dependents();
   pdl_wait();                                          // inputs and cache may come from the kernel before this one
   const int lane = threadIdx.x & 31;
-  // grid: y < Hkv -> K/V of kv head y, token row 4 x + warp;  y >= Hkv -> query rows (no division anywhere)
+  // grid: y < Hkv -> K/V of kv head y, unit 4 x + warp;  y >= Hkv -> query rows.
+  // A K/V unit is one aligned octet of token positions (8 k .. 8 k + 7) of one sequence: its V codes are 128
+  // whole 32-bit words (one per channel, a nibble per token) = 512 contiguous bytes of the record, written with one
+  // 16-byte store per lane; the tokens of the octet that are not part of this call keep their nibbles.  The
+  // position of a sequence's first new token is device data, so units are dealt out by an upper bound that needs
+  // cu_new only: sequence b owns units off(b) .. off(b+1)-1 with off(b) = (cu_new[b] >> 3) + 2 b (its tokens touch at
+  // most (count >> 3) + 2 octets); surplus units exit.
   if ((int)blockIdx.y < Hkv) {
-    const int n = (int)blockIdx.x * 4 + (int)(threadIdx.x >> 5), h = (int)blockIdx.y;
-    if (n >= total_new) return;
-    // largest b with cu_new[b] <= n: first the guess for evenly spread tokens (the decode step appends one
-    // token per sequence) checked with two independent loads; else a two-level search by the whole warp (32
-    // entries per level, one load per lane and a ballot), or a binary search beyond 1024 sequences
-    int b = (total_new == batch) ? n : 0;
-    if (!(cu_new[b] <= n && n < cu_new[b + 1])) {
+    const int u = (int)blockIdx.x * 4 + (int)(threadIdx.x >> 5), h = (int)blockIdx.y;
+    const int n_units = (total_new >> 3) + 2 * batch;
+    if (total_new == 0 || u >= n_units) return;
+    auto off = [&](int i) { return (cu_new[i] >> 3) + 2 * i; };
+    // largest b < batch with off(b) <= u: a guess for evenly spread tokens checked with two independent loads; else
+    // a two-level search by the whole warp (32 entries per level, one load per lane and a ballot), or a binary
+    // search beyond 1024 sequences
+    int b = max(0, min((int)((float)u * (float)batch / (float)n_units), batch - 1));   // only a guess: verified next
+    if (!(off(b) <= u && u < off(b + 1))) {
       if (batch <= 1024) {
         const int step = (batch + 31) >> 5;             // entries per first-level block
         const int i1 = min((lane + 1) * step, batch);
-        const int blk = __popc(__ballot_sync(kFull, cu_new[i1] <= n && i1 < batch));   // blocks wholly <= n
+        const int blk = __popc(__ballot_sync(kFull, off(i1) <= u && i1 < batch));   // blocks wholly <= u
         const int base = min(blk * step, batch - 1);
         const int i2 = min(base + lane, batch - 1);
-        const unsigned le = __ballot_sync(kFull, lane < step && base + lane < batch && cu_new[i2] <= n);
-        b = base + (31 - __clz((int)(le | 1u)));        // cu_new[base] <= n always holds
+        const unsigned le = __ballot_sync(kFull, lane < step && base + lane < batch && off(i2) <= u);
+        b = base + (31 - __clz((int)(le | 1u)));        // off(base) <= u always holds
       } else {
         int lo = 0, hi = batch;
         while (hi - lo > 1) {
           const int mid = (lo + hi) >> 1;
-          if (cu_new[mid] <= n) lo = mid; else hi = mid;
+          if (off(mid) <= u) lo = mid; else hi = mid;
         }
         b = lo;
       }
     }
-    const int j = n - cu_new[b];
-    const int pos = seq_lens[b] + j;
-    const bool odd = pos & 1;
-    if (odd && j > 0) return;                 // handled by the warp of the even partner
-    const bool has_b = !odd && (n + 1 < cu_new[b + 1]);
-    const int page = block_tables[(long long)b * max_pages + (pos >> 4)];
-    const int t = pos & 15;
+    const int c0 = cu_new[b], cnt = cu_new[b + 1] - c0, p0 = seq_lens[b];
+    const int q0 = ((p0 >> 3) + (u - off(b))) << 3;     // first position of this unit's octet
+    const int t_lo = max(p0, q0), t_hi = min(p0 + cnt, q0 + 8);   // the call's positions inside the octet
+    if (t_lo >= t_hi) return;
+    const int page = block_tables[(long long)b * max_pages + (q0 >> 4)];
     uint8_t* rec = cache + ((long long)page * Hkv + h) * kRecordBytes;
-    const uint16_t* krow = k_new + ((long long)n * Hkv + h) * kHeadDim;
-    const uint16_t* vrow = v_new + ((long long)n * Hkv + h) * kHeadDim;
-    store_k(krow, rec, t, lane, c_k);
-    const uint32_t ca = encode_v(vrow, rec, t, lane, c_v);
-    uint32_t cb = 0;
-    if (has_b) {
-      store_k(krow + (long long)Hkv * kHeadDim, rec, t + 1, lane, c_k);
-      cb = encode_v(vrow + (long long)Hkv * kHeadDim, rec, t + 1, lane, c_v);
-    }
-    // token-major nibbles: channel d = 4*lane + r lives in word 512*(t>>3) + 128*(d>>5) + 4*(d&31),
-    // tokens (t, t+1) share byte (t&7)>>1 of that word
+    uint32_t vw[4] = {0u, 0u, 0u, 0u};                  // V code words of channels 4 lane .. 4 lane + 3
+    for (int pos = t_lo; pos < t_hi; ++pos) {
+      const long long row = ((long long)(c0 + (pos - p0)) * Hkv + h) * kHeadDim;
+      store_k(k_new + row, rec, pos & 15, lane, c_k);
+      const uint32_t c = encode_v(v_new + row, rec, pos & 15, lane, c_v);
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {
-      const int d = 4 * lane + r;
-      uint8_t* dst = rec + kOffVCodes + 512 * (t >> 3) + 128 * (d >> 5) + 4 * (d & 31) + ((t & 7) >> 1);
-      const uint32_t a4 = (ca >> (8 * r)) & 0xF, b4 = (cb >> (8 * r)) & 0xF;
-      *dst = odd ? (uint8_t)((*dst & 0x0F) | (a4 << 4)) : (uint8_t)(a4 | (b4 << 4));
+      for (int r = 0; r < 4; ++r) vw[r] |= ((c >> (8 * r)) & 0xFu) << (4 * (pos & 7));
+    }
+    // token-major nibbles: channel d lives in word 512*(t>>3) + 4 d of the V codes, token t in nibble t & 7
+    uint4* dst = reinterpret_cast<uint4*>(rec + kOffVCodes + 512 * ((q0 >> 3) & 1) + 16 * lane);
+    if (t_hi - t_lo == 8) {
+      *dst = make_uint4(vw[0], vw[1], vw[2], vw[3]);
+    } else {                                            // keep the nibbles of the other tokens of the octet
+      const uint32_t below_hi = (t_hi - q0 == 8) ? 0xFFFFFFFFu : ((1u << (4 * (t_hi - q0))) - 1u);
+      const uint32_t m = below_hi & ~((1u << (4 * (t_lo - q0))) - 1u);
+      const uint4 old = *dst;
+      *dst = make_uint4((old.x & ~m) | (vw[0] & m), (old.y & ~m) | (vw[1] & m), (old.z & ~m) | (vw[2] & m),
+                        (old.w & ~m) | (vw[3] & m));
     }
     return;
   }
@@ -391,9 +398,9 @@ extern "C" int32_t uq_rotate_quantize_append(const uq_config* cfg, const void* k
   }
   const long long q_rows = q ? (long long)batch * cfg->num_q_heads : 0;
   if (total_new == 0 && q_rows == 0) return UQ_OK;
-  // grid.x: blocks of 4 token rows (K/V part, grid.y = kv head) — widened if the query rows would need more than
-  // 60000 further grid rows; grid.y beyond the kv heads: query rows, 4 * grid.x per grid row
-  long long gx = ((long long)total_new + 3) / 4;
+  // grid.x: blocks of 4 K/V units (one aligned octet of positions each; grid.y = kv head) — widened if the query
+  // rows would need more than 60000 further grid rows; grid.y beyond the kv heads: query rows, 4 * grid.x per row
+  long long gx = total_new > 0 ? (((long long)(total_new >> 3) + 2LL * batch) + 3) / 4 : 0;
   gx = gx > (q_rows + 4 * 60000LL - 1) / (4 * 60000LL) ? gx : (q_rows + 4 * 60000LL - 1) / (4 * 60000LL);
   if (gx < 1) gx = 1;
   const long long gy = cfg->num_kv_heads + (q_rows + 4 * gx - 1) / (4 * gx);
