@@ -331,8 +331,18 @@ append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v
     const int q0 = ((p0 >> 3) + (u - off(b))) << 3;     // first position of this unit's octet
     const int t_lo = max(p0, q0), t_hi = min(p0 + cnt, q0 + 8);   // the call's positions inside the octet
     if (t_lo >= t_hi) return;
+    {   // the first token's rows on their way while the page is looked up (a decode step is a chain of latencies)
+      const long long row0 = ((long long)(c0 + (t_lo - p0)) * Hkv + h) * kHeadDim + 4 * lane;
+      asm volatile("prefetch.global.L1 [%0];" ::"l"(k_new + row0));
+      asm volatile("prefetch.global.L1 [%0];" ::"l"(v_new + row0));
+    }
     const int page = block_tables[(long long)b * max_pages + (q0 >> 4)];
     uint8_t* rec = cache + ((long long)page * Hkv + h) * kRecordBytes;
+    // token-major nibbles: channel d lives in word 512*(t>>3) + 4 d of the V codes, token t in nibble t & 7
+    uint4* dst = reinterpret_cast<uint4*>(rec + kOffVCodes + 512 * ((q0 >> 3) & 1) + 16 * lane);
+    const bool whole = (t_hi - t_lo == 8);
+    uint4 old = make_uint4(0u, 0u, 0u, 0u);
+    if (!whole) old = *dst;                             // the other tokens' nibbles: loaded under the encoding below
     uint32_t vw[4] = {0u, 0u, 0u, 0u};                  // V code words of channels 4 lane .. 4 lane + 3
     for (int pos = t_lo; pos < t_hi; ++pos) {
       const long long row = ((long long)(c0 + (pos - p0)) * Hkv + h) * kHeadDim;
@@ -341,14 +351,11 @@ append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v
 #pragma unroll
       for (int r = 0; r < 4; ++r) vw[r] |= ((c >> (8 * r)) & 0xFu) << (4 * (pos & 7));
     }
-    // token-major nibbles: channel d lives in word 512*(t>>3) + 4 d of the V codes, token t in nibble t & 7
-    uint4* dst = reinterpret_cast<uint4*>(rec + kOffVCodes + 512 * ((q0 >> 3) & 1) + 16 * lane);
-    if (t_hi - t_lo == 8) {
+    if (whole) {
       *dst = make_uint4(vw[0], vw[1], vw[2], vw[3]);
     } else {                                            // keep the nibbles of the other tokens of the octet
       const uint32_t below_hi = (t_hi - q0 == 8) ? 0xFFFFFFFFu : ((1u << (4 * (t_hi - q0))) - 1u);
       const uint32_t m = below_hi & ~((1u << (4 * (t_lo - q0))) - 1u);
-      const uint4 old = *dst;
       *dst = make_uint4((old.x & ~m) | (vw[0] & m), (old.y & ~m) | (vw[1] & m), (old.z & ~m) | (vw[2] & m),
                         (old.w & ~m) | (vw[3] & m));
     }
