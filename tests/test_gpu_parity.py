@@ -401,3 +401,36 @@ def test_random_multi_sequence_appends(B):
         L = int(wl.ctx_lens[b])
         if L:
             H.compare_cache(cache, wl, int(b), L, H.oracle_sequence_cache(wl, int(b), L, DEV))
+
+
+def test_custom_constants_sm_scale_and_c():
+    """Non-default uq_config values reach the kernels: softmax scale 0.05 (instead of 1/sqrt(d)) and the paper's
+    power-of-two-rule constant c = 0.195 for K and V — cache bit-exact, outputs in tolerance."""
+    wl = W.make_custom("consts", 41, [333, 40], 16, 2, peaked_frac=0.3)
+    cfg = H.cfg_of(wl, sm_scale=0.05, c_k=0.195, c_v=0.195)
+    cache, bt = H.fill_cache(cfg, wl, DEV)
+    q = W.gen_q(wl, DEV)
+    out, q_fp8, _ = H.run_decode(cfg, cache, bt, wl.ctx_lens, q, 3)
+    for b in range(wl.batch):
+        L = int(wl.ctx_lens[b])
+        arrays = H.oracle_sequence_cache(wl, b, L, DEV, c_k=0.195, c_v=0.195)
+        H.compare_cache(cache, wl, b, L, arrays)
+        ref, q8 = H.oracle_out(wl, b, L, H.bits(q)[b], arrays, sm_scale=0.05)
+        assert np.array_equal(q_fp8[b].cpu().numpy(), q8)
+        H.check_out(out[b].float().cpu().numpy().astype(np.float64), ref, f"consts seq {b}")
+
+
+def test_decode_refuses_more_than_2048_sequences():
+    """include/uq.h: at most 2048 sequences per uq_decode_attention call (the tile prefix sums live in shared
+    memory); a larger batch is refused on the host with UQ_ERR_INVALID_ARG / UQ_ERR_UNSUPPORTED and nothing is launched."""
+    cfg = uq.UQConfig(num_q_heads=8, num_kv_heads=1)
+    B = 2049
+    cache = uq.alloc_cache(cfg, 4, DEV)
+    bt = torch.zeros((B, 1), dtype=torch.int32, device=DEV)
+    lens = torch.ones(B, dtype=torch.int32, device=DEV)
+    q8 = torch.zeros((B, 8, 128), dtype=torch.uint8, device=DEV)
+    acc = torch.zeros((B, 8, 2, 128), dtype=torch.float32, device=DEV)
+    ml = torch.zeros((B, 8, 2, 2), dtype=torch.float32, device=DEV)
+    with pytest.raises(uq.UQError, match="2048"):
+        uq.decode_attention(cfg, q8, cache, bt, lens, 2, acc, ml)
+    torch.cuda.synchronize()
