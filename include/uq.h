@@ -64,6 +64,10 @@ extern "C" {
 
 #define UQ_RECORD_BYTES 2176  /* 16 tokens * (64 + 4 + 64 + 4) bytes */
 
+/* uq_config.flags: keep uq_rotate_quantize_append on the one-warp-per-octet kernel even for prefill-sized calls
+ * (the bytes written do not depend on it; tests use it to cover both kernels on the same inputs). */
+#define UQ_FLAG_NO_BULK_APPEND 1u
+
 typedef struct {
   int32_t num_q_heads;   /* e.g. 64 */
   int32_t num_kv_heads;  /* e.g. 4  */
@@ -73,7 +77,7 @@ typedef struct {
   float c_k;             /* global constant c for keys   (0.156f); used as (double)c_k */
   float c_v;             /* global constant c for values (0.156f; same rule, reading G3) */
   float sm_scale;        /* softmax scale; 0 => 1/sqrt(head_dim) */
-  uint32_t flags;        /* reserved, must be 0 */
+  uint32_t flags;        /* UQ_FLAG_* bits; unknown bits are an error */
 } uq_config;
 
 /* Host.  Static, thread-local description of the last error returned on this thread. */
@@ -95,6 +99,11 @@ size_t uq_cache_record_bytes(const uq_config* cfg);
  *  q             bf16 [batch, num_q_heads, head_dim] or NULL.  If given, q_fp8 (uint8, same
  *                shape) receives cast_fp8_e4m3(R*q): OCP E4M3, round-to-nearest-even,
  *                saturating at +-448, zero stored as 0x00.
+ *
+ * Two kernels, one result: calls with on average >= 64 new tokens per sequence (and >= 1024 in all, k_new / v_new
+ * 16-byte aligned) take the bulk kernel (one warp per aligned block of 32 positions, rows staged in shared memory,
+ * the rotation done in registers with one token per lane); all other calls, and the heads / tails of a bulk
+ * call's ranges, one warp per aligned octet of positions.
  *
  * Every rounding decision (scale exponent, E2M1 code, E4M3 byte) is taken on float64 values of
  * the exactly-computed rotation (reading G1), so codes, scale bytes and q_fp8 are

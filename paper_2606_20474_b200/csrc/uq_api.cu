@@ -33,8 +33,8 @@ int32_t check_config(const uq_config* cfg) {
     set_error("uq_config: c_k and c_v must be positive");
     return UQ_ERR_INVALID_ARG;
   }
-  if (cfg->flags != 0) {
-    set_error("uq_config: flags must be 0");
+  if ((cfg->flags & ~(uint32_t)UQ_FLAG_NO_BULK_APPEND) != 0) {
+    set_error("uq_config: unknown bit in flags");
     return UQ_ERR_INVALID_ARG;
   }
   if (cfg->head_dim != kHeadDim || cfg->group_size != kGroup || cfg->page_size != kPage) {

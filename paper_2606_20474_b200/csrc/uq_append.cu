@@ -284,6 +284,80 @@ __device__ __forceinline__ uint32_t encode_v(const uint16_t* vrow, uint8_t* rec,
   return codes;
 }
 
+// Sequence b owns the work units off(b) .. off(b+1)-1 with off(b) = (cu_new[b] >> SHIFT) + 2 b (its new tokens touch
+// at most (count >> SHIFT) + 2 aligned blocks of 2^SHIFT positions).  Returns the largest b < batch with off(b) <= u:
+// a guess for evenly spread tokens checked with two independent loads; else a two-level search by the whole warp
+// (32 entries per level, one load per lane and a ballot), or a binary search beyond 1024 sequences.
+template <int SHIFT>
+__device__ __forceinline__ int find_sequence(const int32_t* __restrict__ cu_new, int batch, int u, int n_units, int lane) {
+  auto off = [&](int i) { return (cu_new[i] >> SHIFT) + 2 * i; };
+  int b = max(0, min((int)((float)u * (float)batch / (float)n_units), batch - 1));   // only a guess: verified next
+  if (!(off(b) <= u && u < off(b + 1))) {
+    if (batch <= 1024) {
+      const int step = (batch + 31) >> 5;             // entries per first-level block
+      const int i1 = min((lane + 1) * step, batch);
+      const int blk = __popc(__ballot_sync(kFull, off(i1) <= u && i1 < batch));   // blocks wholly <= u
+      const int base = min(blk * step, batch - 1);
+      const int i2 = min(base + lane, batch - 1);
+      const unsigned le = __ballot_sync(kFull, lane < step && base + lane < batch && off(i2) <= u);
+      b = base + (31 - __clz((int)(le | 1u)));        // off(base) <= u always holds
+    } else {
+      int lo = 0, hi = batch;
+      while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (off(mid) <= u) lo = mid; else hi = mid;
+      }
+      b = lo;
+    }
+  }
+  return b;
+}
+
+// One warp: K and V of the call's positions t_lo .. t_hi-1 inside the aligned octet q0 .. q0+7 of a sequence whose
+// first new token (row c0 of k_new / v_new) lands at position p0.  An octet's V codes are 128 whole 32-bit words (one
+// per channel, a nibble per token) = 512 contiguous bytes of the record, written with one 16-byte store per lane; the
+// tokens of the octet that are not part of the range keep their nibbles (masked merge).
+__device__ __forceinline__ void append_octet(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v_new,
+                                             uint8_t* rec, int c0, int p0, int q0, int t_lo, int t_hi, int h, int Hkv,
+                                             int lane, double c_k, double c_v) {
+  // token-major nibbles: channel d lives in word 512*(t>>3) + 4 d of the V codes, token t in nibble t & 7
+  uint4* dst = reinterpret_cast<uint4*>(rec + kOffVCodes + 512 * ((q0 >> 3) & 1) + 16 * lane);
+  const bool whole = (t_hi - t_lo == 8);
+  uint4 old = make_uint4(0u, 0u, 0u, 0u);
+  if (!whole) old = *dst;                             // the other tokens' nibbles: loaded under the encoding below
+  uint32_t vw[4] = {0u, 0u, 0u, 0u};                  // V code words of channels 4 lane .. 4 lane + 3
+  for (int pos = t_lo; pos < t_hi; ++pos) {
+    const long long row = ((long long)(c0 + (pos - p0)) * Hkv + h) * kHeadDim;
+    store_k(k_new + row, rec, pos & 15, lane, c_k);
+    const uint32_t c = encode_v(v_new + row, rec, pos & 15, lane, c_v);
+#pragma unroll
+    for (int r = 0; r < 4; ++r) vw[r] |= ((c >> (8 * r)) & 0xFu) << (4 * (pos & 7));
+  }
+  if (whole) {
+    *dst = make_uint4(vw[0], vw[1], vw[2], vw[3]);
+  } else {                                            // keep the nibbles of the other tokens of the octet
+    const uint32_t below_hi = (t_hi - q0 == 8) ? 0xFFFFFFFFu : ((1u << (4 * (t_hi - q0))) - 1u);
+    const uint32_t m = below_hi & ~((1u << (4 * (t_lo - q0))) - 1u);
+    *dst = make_uint4((old.x & ~m) | (vw[0] & m), (old.y & ~m) | (vw[1] & m), (old.z & ~m) | (vw[2] & m),
+                      (old.w & ~m) | (vw[3] & m));
+  }
+}
+
+// V of the single position pos (octet q0) redone in float64 by the warp: the token's nibbles are merged into the
+// words the octet already holds.
+__device__ __forceinline__ void append_octet_v(const uint16_t* __restrict__ v_new, uint8_t* rec, int c0, int p0, int q0,
+                                               int pos, int h, int Hkv, int lane, double c_v) {
+  uint4* dst = reinterpret_cast<uint4*>(rec + kOffVCodes + 512 * ((q0 >> 3) & 1) + 16 * lane);
+  const uint4 old = *dst;
+  const long long row = ((long long)(c0 + (pos - p0)) * Hkv + h) * kHeadDim;
+  const uint32_t c = encode_v(v_new + row, rec, pos & 15, lane, c_v);
+  const uint32_t m = 0xFu << (4 * (pos & 7));
+  uint32_t vw[4];
+#pragma unroll
+  for (int r = 0; r < 4; ++r) vw[r] = ((c >> (8 * r)) & 0xFu) << (4 * (pos & 7));
+  *dst = make_uint4((old.x & ~m) | vw[0], (old.y & ~m) | vw[1], (old.z & ~m) | vw[2], (old.w & ~m) | vw[3]);
+}
+
 __global__ void __launch_bounds__(128)
 append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v_new,
               const int32_t* __restrict__ cu_new, const int32_t* __restrict__ seq_lens,
@@ -304,31 +378,9 @@ append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v
     const int u = (int)blockIdx.x * 4 + (int)(threadIdx.x >> 5), h = (int)blockIdx.y;
     const int n_units = (total_new >> 3) + 2 * batch;
     if (total_new == 0 || u >= n_units) return;
-    auto off = [&](int i) { return (cu_new[i] >> 3) + 2 * i; };
-    // largest b < batch with off(b) <= u: a guess for evenly spread tokens checked with two independent loads; else
-    // a two-level search by the whole warp (32 entries per level, one load per lane and a ballot), or a binary
-    // search beyond 1024 sequences
-    int b = max(0, min((int)((float)u * (float)batch / (float)n_units), batch - 1));   // only a guess: verified next
-    if (!(off(b) <= u && u < off(b + 1))) {
-      if (batch <= 1024) {
-        const int step = (batch + 31) >> 5;             // entries per first-level block
-        const int i1 = min((lane + 1) * step, batch);
-        const int blk = __popc(__ballot_sync(kFull, off(i1) <= u && i1 < batch));   // blocks wholly <= u
-        const int base = min(blk * step, batch - 1);
-        const int i2 = min(base + lane, batch - 1);
-        const unsigned le = __ballot_sync(kFull, lane < step && base + lane < batch && off(i2) <= u);
-        b = base + (31 - __clz((int)(le | 1u)));        // off(base) <= u always holds
-      } else {
-        int lo = 0, hi = batch;
-        while (hi - lo > 1) {
-          const int mid = (lo + hi) >> 1;
-          if (off(mid) <= u) lo = mid; else hi = mid;
-        }
-        b = lo;
-      }
-    }
+    const int b = find_sequence<3>(cu_new, batch, u, n_units, lane);
     const int c0 = cu_new[b], cnt = cu_new[b + 1] - c0, p0 = seq_lens[b];
-    const int q0 = ((p0 >> 3) + (u - off(b))) << 3;     // first position of this unit's octet
+    const int q0 = ((p0 >> 3) + (u - ((c0 >> 3) + 2 * b))) << 3;     // first position of this unit's octet
     const int t_lo = max(p0, q0), t_hi = min(p0 + cnt, q0 + 8);   // the call's positions inside the octet
     if (t_lo >= t_hi) return;
     {   // the first token's rows on their way while the page is looked up (a decode step is a chain of latencies)
@@ -338,27 +390,7 @@ append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v
     }
     const int page = block_tables[(long long)b * max_pages + (q0 >> 4)];
     uint8_t* rec = cache + ((long long)page * Hkv + h) * kRecordBytes;
-    // token-major nibbles: channel d lives in word 512*(t>>3) + 4 d of the V codes, token t in nibble t & 7
-    uint4* dst = reinterpret_cast<uint4*>(rec + kOffVCodes + 512 * ((q0 >> 3) & 1) + 16 * lane);
-    const bool whole = (t_hi - t_lo == 8);
-    uint4 old = make_uint4(0u, 0u, 0u, 0u);
-    if (!whole) old = *dst;                             // the other tokens' nibbles: loaded under the encoding below
-    uint32_t vw[4] = {0u, 0u, 0u, 0u};                  // V code words of channels 4 lane .. 4 lane + 3
-    for (int pos = t_lo; pos < t_hi; ++pos) {
-      const long long row = ((long long)(c0 + (pos - p0)) * Hkv + h) * kHeadDim;
-      store_k(k_new + row, rec, pos & 15, lane, c_k);
-      const uint32_t c = encode_v(v_new + row, rec, pos & 15, lane, c_v);
-#pragma unroll
-      for (int r = 0; r < 4; ++r) vw[r] |= ((c >> (8 * r)) & 0xFu) << (4 * (pos & 7));
-    }
-    if (whole) {
-      *dst = make_uint4(vw[0], vw[1], vw[2], vw[3]);
-    } else {                                            // keep the nibbles of the other tokens of the octet
-      const uint32_t below_hi = (t_hi - q0 == 8) ? 0xFFFFFFFFu : ((1u << (4 * (t_hi - q0))) - 1u);
-      const uint32_t m = below_hi & ~((1u << (4 * (t_lo - q0))) - 1u);
-      *dst = make_uint4((old.x & ~m) | (vw[0] & m), (old.y & ~m) | (vw[1] & m), (old.z & ~m) | (vw[2] & m),
-                        (old.w & ~m) | (vw[3] & m));
-    }
+    append_octet(k_new, v_new, rec, c0, p0, q0, t_lo, t_hi, h, Hkv, lane, c_k, c_v);
     return;
   }
   const long long qu = ((long long)((int)blockIdx.y - Hkv) * gridDim.x + blockIdx.x) * 4 + (threadIdx.x >> 5);
@@ -371,6 +403,258 @@ append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v
       w = e4m3_byte(x[0]) | (e4m3_byte(x[1]) << 8) | (e4m3_byte(x[2]) << 16) | (e4m3_byte(x[3]) << 24);
     }
     *reinterpret_cast<uint32_t*>(q_fp8 + qu * kHeadDim + 4 * lane) = w;
+  }
+}
+
+// ---------------------------------------------------------------- bulk (prefill-sized) append
+// SURVEY 8(f) rank 1.  The kernel above spends a warp on every vector: 326 warp instructions per (token, kv head),
+// a third of them shuffles and lane bookkeeping.  Here a warp takes an aligned block of 32 positions (two pages) of
+// one kv head, stages its K and V rows in shared memory with one bulk copy per row (32 x 256 B each, issued by the
+// lanes, completion on an mbarrier) and works in two thread mappings:
+//   K      lane = token: the whole 128-channel vector in registers, the Walsh-Hadamard butterfly is 7 x 64
+//          in-register add/sub pairs (no shuffle), the same float32 error-interval test as the fast path above decides
+//          every scale exponent and code, 64 B of codes and one scale word are stored per lane;
+//   V      pass 1, lane = token: group maxima by packed 16-bit integer maxima of the bf16 magnitudes -> scale exponent,
+//          scale bytes, and the power-of-two multipliers left in shared memory;
+//          pass 2, lane = 4 channels: eight tokens of a channel make one 32-bit word of the token-major layout
+//          (four cvt.e2m1x2 per word), one 16-byte store per lane and octet.
+// A vector whose interval test fails (0.45 % of N(0,1) keys) is redone by the whole warp with store_k / append_octet
+// (float64), after the fast lanes have stored; a block that the call covers only partly goes through append_octet
+// octet by octet.  The bytes written are those of the kernel above in every case.
+constexpr int kBulkWarps = 4;
+constexpr int kRowStride = 272;                        // 256 B row + 16 B: a lane reading its own row with 16-byte loads
+                                                       // is bank-conflict free (17 x 16 B: odd stride in 16-byte units)
+constexpr int kBulkBuf = 32 * kRowStride;              // 8704
+constexpr int kBulkWarpBytes = 2 * kBulkBuf + 512;     // K rows, V rows, V multipliers [32 tokens][4 groups] f32
+constexpr int kBulkSmem = kBulkWarps * kBulkWarpBytes; // 71,680
+
+// eight values -> eight E2M1 codes, value i in bits 4i..4i+3; "-0" -> +0
+__device__ __forceinline__ uint32_t e2m1x8(float r0, float r1, float r2, float r3, float r4, float r5, float r6, float r7) {
+  uint32_t n;
+  asm("{\n.reg .b8 t0, t1, t2, t3;\n"
+      "cvt.rn.satfinite.e2m1x2.f32 t0, %2, %1;\n"
+      "cvt.rn.satfinite.e2m1x2.f32 t1, %4, %3;\n"
+      "cvt.rn.satfinite.e2m1x2.f32 t2, %6, %5;\n"
+      "cvt.rn.satfinite.e2m1x2.f32 t3, %8, %7;\n"
+      "mov.b32 %0, {t0, t1, t2, t3};\n}\n"
+      : "=r"(n) : "f"(r0), "f"(r1), "f"(r2), "f"(r3), "f"(r4), "f"(r5), "f"(r6), "f"(r7));
+  const uint32_t t = n & 0x77777777u;
+  const uint32_t nz = ((t + 0x77777777u) | t) & 0x88888888u;   // bit 3 of a nibble set iff its magnitude is not 0
+  return n & (0x77777777u | nz);
+}
+
+// one butterfly level over the 128 values of a thread: index bit log2(H)
+template <int H>
+__device__ __forceinline__ void wht_level(float (&x)[128]) {
+#pragma unroll
+  for (int k = 0; k < 64; ++k) {
+    const int j = ((k / H) * 2 * H) + (k % H);
+    const float a = x[j], b = x[j + H];
+    x[j] = __fadd_rn(a, b);
+    x[j + H] = __fsub_rn(a, b);
+  }
+}
+
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// K of the lane's token from its shared-memory row: 16 code words, 4 scale bytes; false if any decision is unsafe.
+__device__ __forceinline__ bool bulk_encode_k(uint32_t row, float c_k, uint32_t (&codes)[16], uint32_t& scale_word) {
+  float x[128];
+#pragma unroll
+  for (int j = 0; j < 16; ++j) {
+    uint4 w;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "r"(row + 16 * j));
+    x[8 * j + 0] = __uint_as_float(w.x << 16); x[8 * j + 1] = __uint_as_float(w.x & 0xFFFF0000u);
+    x[8 * j + 2] = __uint_as_float(w.y << 16); x[8 * j + 3] = __uint_as_float(w.y & 0xFFFF0000u);
+    x[8 * j + 4] = __uint_as_float(w.z << 16); x[8 * j + 5] = __uint_as_float(w.z & 0xFFFF0000u);
+    x[8 * j + 6] = __uint_as_float(w.w << 16); x[8 * j + 7] = __uint_as_float(w.w & 0xFFFF0000u);
+  }
+  float S = 0.f;                                         // sum |x_i|: four chains
+  {
+    float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+#pragma unroll
+    for (int i = 0; i < 128; i += 4) {
+      s0 += fabsf(x[i]); s1 += fabsf(x[i + 1]); s2 += fabsf(x[i + 2]); s3 += fabsf(x[i + 3]);
+    }
+    S = (s0 + s1) + (s2 + s3);
+  }
+  // butterfly: seven levels, one rounding per output and level (the bound kBound is for exactly this)
+  wht_level<1>(x); wht_level<2>(x); wht_level<4>(x); wht_level<8>(x); wht_level<16>(x); wht_level<32>(x); wht_level<64>(x);
+  const float kappa = 0x1.6a09e6p-4f;                    // float32 nearest to 2^-3.5
+  const float eps = __fmul_rn(S, kBound);
+  bool ok = (S > 1e-30f) && (S < 1e30f);
+  scale_word = 0u;
+#pragma unroll
+  for (int g = 0; g < 4; ++g) {
+    float m = 0.f;
+#pragma unroll
+    for (int i = 0; i < 32; ++i) m = fmaxf(m, fabsf(x[32 * g + i]));
+    m = __fmul_rn(m, kappa);                             // = max |fl(kappa x_i)|: rounding is monotone
+    int E;
+    const bool okg = scale_exponent_f32(c_k, m, eps, E) && (E >= -100) && (E <= 100);
+    ok = ok && okg;
+    if (!okg) E = 0;
+    scale_word |= (uint32_t)(E + 127) << (8 * g);
+    const float sc = pow2_neg(E);
+    const float ksc = __fmul_rn(kappa, sc);              // exact: fl(x kappa) 2^-E = fl(x (kappa 2^-E))
+    const float er = __fmaf_rn(__fmul_rn(eps, sc), 1.0001f, 1.2e-6f);   // + the rounding of the two additions below
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      float r[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) r[i] = __fmul_rn(x[32 * g + 8 * w + i], ksc);
+      const uint32_t lo = e2m1x8(r[0] - er, r[1] - er, r[2] - er, r[3] - er, r[4] - er, r[5] - er, r[6] - er, r[7] - er);
+      const uint32_t hi = e2m1x8(r[0] + er, r[1] + er, r[2] + er, r[3] + er, r[4] + er, r[5] + er, r[6] + er, r[7] + er);
+      ok = ok && (lo == hi);
+      codes[4 * g + w] = lo;
+    }
+  }
+  return ok;
+}
+
+__global__ void __launch_bounds__(32 * kBulkWarps, 3)
+append_bulk_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v_new,
+                   const int32_t* __restrict__ cu_new, const int32_t* __restrict__ seq_lens,
+                   const int32_t* __restrict__ block_tables, int max_pages, int batch, int total_new, int Hkv,
+                   uint8_t* __restrict__ cache, double c_k, double c_v) {
+  extern __shared__ __align__(16) uint8_t bulk_smem[];
+  __shared__ __align__(8) uint64_t bars[kBulkWarps][2];
+  pdl_launch_dependents();
+  pdl_wait();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int u = (int)blockIdx.x * kBulkWarps + warp, h = (int)blockIdx.y;
+  const int n_units = (total_new >> 5) + 2 * batch;
+  if (u >= n_units) return;                            // warps are independent: no CTA-wide barrier below
+  const int b = find_sequence<5>(cu_new, batch, u, n_units, lane);
+  const int c0 = cu_new[b], cnt = cu_new[b + 1] - c0, p0 = seq_lens[b];
+  const int q0 = ((p0 >> 5) + (u - ((c0 >> 5) + 2 * b))) << 5;      // first position of this unit's block of 32
+  const int t_lo = max(p0, q0), t_hi = min(p0 + cnt, q0 + 32);      // the call's positions inside the block
+  if (t_lo >= t_hi) return;
+  const int32_t* bt = block_tables + (long long)b * max_pages + (q0 >> 4);
+
+  if (t_hi - t_lo < 32) {                              // head / tail of a sequence's range: octet by octet
+    for (int o = 0; o < 4; ++o) {
+      const int qo = q0 + 8 * o, lo = max(t_lo, qo), hi = min(t_hi, qo + 8);
+      if (lo >= hi) continue;
+      uint8_t* rec = cache + ((long long)bt[o >> 1] * Hkv + h) * kRecordBytes;
+      append_octet(k_new, v_new, rec, c0, p0, qo, lo, hi, h, Hkv, lane, c_k, c_v);
+      __syncwarp();
+    }
+    return;
+  }
+
+  // ---------------- whole block: rows -> shared memory
+  uint8_t* const wbase = bulk_smem + warp * kBulkWarpBytes;
+  const uint32_t sK = smem_addr(wbase), sV = sK + kBulkBuf, sM = sV + kBulkBuf;
+  const uint32_t barK = smem_addr(&bars[warp][0]), barV = barK + 8;
+  if (lane == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(barK));
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(barV));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(barK), "r"(32 * 256) : "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(barV), "r"(32 * 256) : "memory");
+  }
+  __syncwarp();
+  const long long row = ((long long)(c0 + (q0 - p0) + lane) * Hkv + h) * kHeadDim;   // this lane's token
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], 256, [%2];"
+               ::"r"(sK + kRowStride * lane), "l"(k_new + row), "r"(barK) : "memory");
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], 256, [%2];"
+               ::"r"(sV + kRowStride * lane), "l"(v_new + row), "r"(barV) : "memory");
+  const int page = bt[lane >> 4];                      // lanes 0-15: first page of the block, 16-31: second
+  uint8_t* const rec = cache + ((long long)page * Hkv + h) * kRecordBytes;
+  const int t = lane & 15;                             // this lane's slot in its page
+  auto wait = [](uint32_t bar) {
+    asm volatile("{\n.reg .pred p;\nW_%=:\nmbarrier.try_wait.parity.shared::cta.b64 p, [%0], 0;\n@p bra D_%=;\nbra W_%=;\nD_%=:\n}\n"
+                 ::"r"(bar) : "memory");
+  };
+
+  // ---------------- K: lane = token
+  wait(barK);
+  unsigned bad_k;
+  {
+    uint32_t codes[16], scale_word;
+    const bool ok = bulk_encode_k(sK + kRowStride * lane, (float)c_k, codes, scale_word);
+    if (ok) {
+      uint4* dst = reinterpret_cast<uint4*>(rec + kOffKCodes + 64 * t);
+#pragma unroll
+      for (int j = 0; j < 4; ++j) dst[j] = make_uint4(codes[4 * j], codes[4 * j + 1], codes[4 * j + 2], codes[4 * j + 3]);
+      *reinterpret_cast<uint32_t*>(rec + kOffKScales + 4 * t) = scale_word;
+    }
+    bad_k = __ballot_sync(kFull, !ok);
+  }
+
+  // ---------------- V pass 1: lane = token
+  wait(barV);
+  unsigned bad_v;
+  {
+    const uint32_t vrow = sV + kRowStride * lane;
+    bool ok = true;
+    float mult[4];
+#pragma unroll
+    for (int g = 0; g < 4; ++g) {
+      uint32_t mx = 0u;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        uint4 w;
+        asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "r"(vrow + 64 * g + 16 * j));
+        mx = __vmaxu2(mx, __vmaxu2(__vmaxu2(w.x & 0x7FFF7FFFu, w.y & 0x7FFF7FFFu), __vmaxu2(w.z & 0x7FFF7FFFu, w.w & 0x7FFF7FFFu)));
+      }
+      const float m = __uint_as_float(max(mx >> 16, mx & 0xFFFFu) << 16);   // bf16 magnitudes order like their bits
+      int E = -127;
+      const bool zero = (m == 0.0f);
+      const bool okg = zero || (scale_exponent_f32((float)c_v, m, 0.0f, E) && (E >= -100) && (E <= 100));
+      ok = ok && okg;
+      mult[g] = (okg && !zero) ? pow2_neg(E) : 1.0f;
+      if (zero) E = -127;
+      if (okg) rec[kOffVScales + 32 * (t >> 3) + 8 * g + (t & 7)] = (uint8_t)(E + 127);
+    }
+    asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(sM + 16 * lane), "f"(mult[0]), "f"(mult[1]), "f"(mult[2]), "f"(mult[3]) : "memory");
+    bad_v = __ballot_sync(kFull, !ok);
+  }
+  __syncwarp();
+
+  // ---------------- V pass 2: lane = channels 4 lane .. 4 lane + 3 (group lane >> 3), an octet of tokens per word
+#pragma unroll 1
+  for (int o = 0; o < 4; ++o) {
+    float r[4][8];
+#pragma unroll
+    for (int tt = 0; tt < 8; ++tt) {
+      uint32_t w0, w1;
+      float mu;
+      asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(w0), "=r"(w1) : "r"(sV + kRowStride * (8 * o + tt) + 8 * lane));
+      asm volatile("ld.shared.f32 %0, [%1];" : "=f"(mu) : "r"(sM + 16 * (8 * o + tt) + 4 * (lane >> 3)));
+      r[0][tt] = __fmul_rn(__uint_as_float(w0 << 16), mu);
+      r[1][tt] = __fmul_rn(__uint_as_float(w0 & 0xFFFF0000u), mu);
+      r[2][tt] = __fmul_rn(__uint_as_float(w1 << 16), mu);
+      r[3][tt] = __fmul_rn(__uint_as_float(w1 & 0xFFFF0000u), mu);
+    }
+    uint32_t vw[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+      vw[c] = e2m1x8(r[c][0], r[c][1], r[c][2], r[c][3], r[c][4], r[c][5], r[c][6], r[c][7]);
+    const int pg = __shfl_sync(kFull, page, 16 * (o >> 1));
+    uint8_t* const rec_o = cache + ((long long)pg * Hkv + h) * kRecordBytes;
+    *reinterpret_cast<uint4*>(rec_o + kOffVCodes + 512 * (o & 1) + 16 * lane) = make_uint4(vw[0], vw[1], vw[2], vw[3]);
+  }
+
+  // ---------------- vectors the float32 intervals could not decide: the whole warp, float64
+  if (bad_k | bad_v) {
+    __syncwarp();
+    while (bad_k) {
+      const int tk = __ffs(bad_k) - 1;
+      bad_k &= bad_k - 1;
+      const int pg = __shfl_sync(kFull, page, tk);
+      const long long rw = ((long long)(c0 + (q0 - p0) + tk) * Hkv + h) * kHeadDim;
+      store_k(k_new + rw, cache + ((long long)pg * Hkv + h) * kRecordBytes, tk & 15, lane, c_k);
+    }
+    while (bad_v) {
+      const int tv = __ffs(bad_v) - 1;
+      bad_v &= bad_v - 1;
+      const int pg = __shfl_sync(kFull, page, tv);
+      const int pos = q0 + tv;
+      append_octet_v(v_new, cache + ((long long)pg * Hkv + h) * kRecordBytes, c0, p0, pos & ~7, pos, h, Hkv, lane, c_v);
+      __syncwarp();
+    }
   }
 }
 
@@ -405,6 +689,30 @@ extern "C" int32_t uq_rotate_quantize_append(const uq_config* cfg, const void* k
   }
   const long long q_rows = q ? (long long)batch * cfg->num_q_heads : 0;
   if (total_new == 0 && q_rows == 0) return UQ_OK;
+  // Prefill-sized calls (on average 64 or more new tokens per sequence): K/V through append_bulk_kernel, one warp per
+  // aligned block of 32 positions; the kernel below then only encodes the query rows.  Same bytes either way.
+  if (total_new >= 1024 && (long long)total_new >= 64LL * batch && !(((uintptr_t)k_new | (uintptr_t)v_new) & 15u) &&
+      !(cfg->flags & UQ_FLAG_NO_BULK_APPEND)) {
+    static bool attr_set = false;
+    if (!attr_set) {
+      cudaError_t e = cudaFuncSetAttribute(append_bulk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kBulkSmem);
+      if (e != cudaSuccess) return check_cuda(e, "append: cudaFuncSetAttribute");
+      attr_set = true;
+    }
+    const long long n_units = (long long)(total_new >> 5) + 2LL * batch;
+    const long long bx = (n_units + kBulkWarps - 1) / kBulkWarps;
+    if (bx > 0x7fffffffLL) {
+      set_error("append: too many work units");
+      return UQ_ERR_INVALID_ARG;
+    }
+    st = check_cuda(launch_pdl(append_bulk_kernel, dim3((unsigned)bx, (unsigned)cfg->num_kv_heads), dim3(32 * kBulkWarps),
+                               (size_t)kBulkSmem, (cudaStream_t)stream, (const uint16_t*)k_new, (const uint16_t*)v_new,
+                               cu_new, seq_lens, block_tables, (int)max_pages, (int)batch, (int)total_new,
+                               (int)cfg->num_kv_heads, (uint8_t*)cache, (double)cfg->c_k, (double)cfg->c_v),
+                    "uq_rotate_quantize_append (bulk) launch");
+    if (st != UQ_OK || q_rows == 0) return st;
+    total_new = 0;                                     // the query rows are left
+  }
   // grid.x: blocks of 4 K/V units (one aligned octet of positions each; grid.y = kv head) — widened if the query
   // rows would need more than 60000 further grid rows; grid.y beyond the kv heads: query rows, 4 * grid.x per row
   long long gx = total_new > 0 ? (((long long)(total_new >> 3) + 2LL * batch) + 3) / 4 : 0;

@@ -335,6 +335,93 @@ def test_append_on_rounding_boundaries_is_bit_exact():
     assert np.array_equal(q_fp8[0].cpu().numpy(), oracle.encode_q(H.bits(q)[0]))
 
 
+def _boundary_rows(L, g):
+    """K / V rows of test_append_on_rounding_boundaries_is_bit_exact (first 103 rows special, the rest N(0,1))."""
+    k = torch.randn((L, 2, 128), generator=g)
+    v = torch.randn((L, 2, 128), generator=g)
+    ties = torch.tensor([0.25, 0.75, 1.25, 1.75, 2.5, 3.5, 5.0, 6.0, 0.5, 1.0, 1.5, 2.0, 3.0, 4.0, 0.0, -0.25])
+    for t in range(0, 64):
+        e = (t % 23) - 11
+        row = ties[torch.randint(0, 16, (2, 128), generator=g)] * (1.0 if t % 2 else -1.0)
+        row[:, ::32] = 6.0
+        v[t] = row * 2.0 ** e
+    thr = [2.0 ** (kk - 0.5) / 0.15600000321865082 for kk in range(-6, 7)]
+    for t in range(64, 96):
+        x = torch.tensor(thr[t % len(thr)], dtype=torch.float32).to(torch.bfloat16)
+        nb = (x.view(torch.int16) + (1 if t % 2 else -1)).view(torch.bfloat16)
+        row = torch.rand((2, 128), generator=g) * float(x) * 0.9
+        row[:, ::32] = float(nb) if t % 3 else float(x)
+        v[t] = row
+    k[96] = 0.75
+    k[97] = -3.0
+    k[98] = 0; k[98, :, 5] = 2.0
+    k[99] = 0; k[99, :, 127] = -1.0 / 3.0
+    k[100] *= 1e20; k[101] *= 1e-20; v[100] *= 1e25; v[101] *= 1e-25
+    k[102] = 0; v[102] = 0
+    return k, v
+
+
+@pytest.mark.parametrize("start", [0, 5, 37])
+def test_bulk_append_kernel_on_rounding_boundaries_and_ragged_ends(start):
+    """The bulk append kernel (one warp per aligned block of 32 positions, prefill-sized calls): the same boundary
+    rows as above, spread over whole blocks and the partly covered head / tail blocks of the range (the sequence
+    starts at position `start`, so rows land in different lanes, octets and pages) — bit for bit the oracle's
+    image, and byte-identical to the per-octet kernel (UQ_FLAG_NO_BULK_APPEND) on the same input."""
+    L = 1500
+    wl = W.make_custom("bulkbound", 77 + start, [start + L], 8, 2)
+    g = torch.Generator(device="cpu"); g.manual_seed(4321 + start)
+    k, v = _boundary_rows(L, g)
+    perm = torch.randperm(L, generator=g)                   # the special rows anywhere in the range
+    k, v = k[perm], v[perm]
+    k0, v0 = torch.randn((start, 2, 128), generator=g), torch.randn((start, 2, 128), generator=g)
+    k, v = torch.cat([k0, k]).to(torch.bfloat16).to(DEV), torch.cat([v0, v]).to(torch.bfloat16).to(DEV)
+    bt = torch.from_numpy(wl.block_tables).to(DEV)
+    images = []
+    for flags in (0, 1):
+        cfg = H.cfg_of(wl, flags=flags)
+        cache = uq.alloc_cache(cfg, wl.num_pages, DEV)
+        cache.fill_(0x3C)
+        if start:
+            H.append_tokens(cfg, cache, bt, np.zeros(1, np.int32), np.array([start], np.int32), k[:start], v[:start])
+        H.append_tokens(cfg, cache, bt, np.array([start], np.int32), np.array([L], np.int32), k[start:], v[start:])
+        torch.cuda.synchronize()
+        H.compare_cache(cache, wl, 0, start + L, oracle.encode_kv(H.bits(k), H.bits(v)))
+        images.append(cache.clone())
+    n_rec = -(-(start + L) // 16)
+    idx = torch.from_numpy(wl.block_tables[0][:n_rec - 1].astype(np.int64)).to(DEV)   # whole pages: every byte defined
+    assert torch.equal(images[0].index_select(0, idx), images[1].index_select(0, idx))
+
+
+def test_bulk_append_many_sequences_irregular_counts():
+    """A prefill-sized call over 24 sequences with irregular starts and counts (zero counts, counts below one
+    block, ranges that start and end inside a block): every token of sampled sequences in its slot, bit-exact."""
+    B = 24
+    rng = np.random.default_rng(99)
+    starts = rng.integers(0, 70, B).astype(np.int32)
+    counts = rng.integers(0, 400, B).astype(np.int32)
+    counts[[3, 11]] = 0
+    counts[[5, 17]] = [7, 33]
+    wl = W.make_custom("bulkmulti", 4242, [int(x) for x in starts + counts], 8, 2)
+    cfg = H.cfg_of(wl)
+    assert counts.sum() >= max(1024, 64 * B)                # the call takes the bulk kernel
+    cache = uq.alloc_cache(cfg, wl.num_pages, DEV)
+    cache.fill_(0xC3)
+    bt = torch.from_numpy(wl.block_tables).to(DEV)
+    full = [W.gen_kv(wl, b, 0, int(wl.ctx_lens[b]), DEV) for b in range(B)]
+    if starts.sum():
+        H.append_tokens(cfg, cache, bt, np.zeros(B, np.int32), starts,
+                        torch.cat([full[b][0][:starts[b]] for b in range(B)]),
+                        torch.cat([full[b][1][:starts[b]] for b in range(B)]))
+    H.append_tokens(cfg, cache, bt, starts, counts,
+                    torch.cat([full[b][0][starts[b]:] for b in range(B)]),
+                    torch.cat([full[b][1][starts[b]:] for b in range(B)]))
+    torch.cuda.synchronize()
+    for b in range(B):
+        L = int(wl.ctx_lens[b])
+        if L:
+            H.compare_cache(cache, wl, b, L, H.oracle_sequence_cache(wl, b, L, DEV))
+
+
 def test_random_small_configs():
     """Seeded sweep over head geometries, batch sizes (up to more items than resident CTAs), length mixes (empty,
     one token, tile multiples +-1, ragged) and slot counts 1..6: cache image bit-exact, outputs in tolerance."""
