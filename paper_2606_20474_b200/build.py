@@ -9,6 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libuq.so")
 SOURCES = ["uq_api.cu", "uq_append.cu", "uq_decode.cu", "uq_merge.cu"]
+PTXAS_FLAGS = {"uq_decode.cu": ["-Xptxas", "-O1"], "uq_merge.cu": ["-Xptxas", "-O1"]}
 
 
 def _stale() -> bool:
@@ -24,17 +25,27 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not (force or _stale()):
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    # ptxas -O1: measured, not assumed — the decode kernel is bound by the serial instruction streams of twelve
-    # warps sharing four schedulers, and the -O3 schedule of the same SASS-level work is 2 % slower on config 2
-    # (104.7 us against 102.6 us); the append and merge kernels do not care.
-    cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-           "-shared", "-Xcompiler", "-fPIC", "-Xptxas", "-O1"] + (["-Xptxas", "-v"] if verbose else []) + \
-          ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    if verbose or res.returncode != 0:
-        sys.stderr.write(res.stdout + res.stderr)
+    # ptxas -O1 for the decode kernel only: measured, not assumed — it is bound by the serial instruction streams of
+    # twelve warps sharing four schedulers, and the -O3 schedule of the same SASS-level work is 2 % slower on config 2
+    # (104.7 us against 102.6 us).  The append kernels are long straight-line arithmetic and want the -O3 scheduler.
+    common = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+              "-Xcompiler", "-fPIC"] + (["-Xptxas", "-v"] if verbose else [])
+    objs = []
+    for src in SOURCES:
+        obj = os.path.join(HERE, src.replace(".cu", ".o"))
+        cmd = common + PTXAS_FLAGS.get(src, []) + ["-c", "-o", obj, os.path.join(CSRC, src)]
+        res = subprocess.run(cmd, capture_output=True, text=True)
+        if verbose or res.returncode != 0:
+            sys.stderr.write(res.stdout + res.stderr)
+        if res.returncode != 0:
+            raise RuntimeError(f"nvcc failed compiling {src}")
+        objs.append(obj)
+    res = subprocess.run([nvcc, "-shared", "-o", LIB] + objs, capture_output=True, text=True)
+    for obj in objs:
+        os.remove(obj)
     if res.returncode != 0:
-        raise RuntimeError("nvcc failed building libuq.so")
+        sys.stderr.write(res.stdout + res.stderr)
+        raise RuntimeError("nvcc failed linking libuq.so")
     return LIB
 
 

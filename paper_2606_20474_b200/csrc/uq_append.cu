@@ -7,6 +7,8 @@
 // sums of 128 bf16 values are exact in double, so every rounding decision (scale exponent,
 // E2M1 level, E4M3 byte) is taken on the same real numbers the float64 oracle sees
 // (reading G1).  __dadd_rn/__dmul_rn keep the compiler from contracting into FMAs.
+#include <cuda.h>
+
 #include "uq_common.cuh"
 
 namespace uq {
@@ -409,8 +411,8 @@ append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v
 // ---------------------------------------------------------------- bulk (prefill-sized) append
 // SURVEY 8(f) rank 1.  The kernel above spends a warp on every vector: 326 warp instructions per (token, kv head),
 // a third of them shuffles and lane bookkeeping.  Here a warp takes an aligned block of 32 positions (two pages) of
-// one kv head, stages its K and V rows in shared memory with one bulk copy per row (32 x 256 B each, issued by the
-// lanes, completion on an mbarrier) and works in two thread mappings:
+// one kv head, stages its K and V rows in shared memory with four TMA tensor copies (k_new / v_new seen as
+// [rows][kv heads x 128] bf16, box 32 rows x 64 channels, completion on an mbarrier) and works in two thread mappings:
 //   K      lane = token: the whole 128-channel vector in registers, the Walsh-Hadamard butterfly is 7 x 64
 //          in-register add/sub pairs (no shuffle), the same float32 error-interval test as the fast path above decides
 //          every scale exponent and code, 64 B of codes and one scale word are stored per lane;
@@ -422,13 +424,14 @@ append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v
 // (float64), after the fast lanes have stored; a block that the call covers only partly goes through append_octet
 // octet by octet.  The bytes written are those of the kernel above in every case.
 constexpr int kBulkWarps = 4;
-constexpr int kRowStride = 272;                        // 256 B row + 16 B: a lane reading its own row with 16-byte loads
-                                                       // is bank-conflict free (17 x 16 B: odd stride in 16-byte units)
-constexpr int kBulkBuf = 32 * kRowStride;              // 8704
-constexpr int kBulkWarpBytes = 2 * kBulkBuf + 512;     // K rows, V rows, V multipliers [32 tokens][4 groups] f32
-constexpr int kBulkSmem = kBulkWarps * kBulkWarpBytes; // 71,680
+// Shared memory per warp: the K and the V rows of its 32 tokens as two channel halves each — a TMA tensor tile of
+// [32 tokens][64 channels] bf16 = 32 rows of 128 B with the 128-byte swizzle (16-byte chunk c of row r sits at chunk
+// c ^ (r & 7)), so a lane reading its own row with 16-byte loads is bank-conflict free — and 32 x 4 V multipliers.
+constexpr int kBulkHalf = 32 * 128;                    // 4096
+constexpr int kBulkTiles = 4 * kBulkHalf;              // K lo, K hi, V lo, V hi: 16,384 per warp
+constexpr int kBulkSmem = kBulkWarps * (kBulkTiles + 512) + 1024;   // + alignment slack (the swizzle atom is 1024 B)
 
-// eight values -> eight E2M1 codes, value i in bits 4i..4i+3; "-0" -> +0
+// eight values -> eight E2M1 codes, value i in bits 4i..4i+3 (raw hardware result: may hold "-0")
 __device__ __forceinline__ uint32_t e2m1x8(float r0, float r1, float r2, float r3, float r4, float r5, float r6, float r7) {
   uint32_t n;
   asm("{\n.reg .b8 t0, t1, t2, t3;\n"
@@ -438,6 +441,9 @@ __device__ __forceinline__ uint32_t e2m1x8(float r0, float r1, float r2, float r
       "cvt.rn.satfinite.e2m1x2.f32 t3, %8, %7;\n"
       "mov.b32 %0, {t0, t1, t2, t3};\n}\n"
       : "=r"(n) : "f"(r0), "f"(r1), "f"(r2), "f"(r3), "f"(r4), "f"(r5), "f"(r6), "f"(r7));
+  return n;
+}
+__device__ __forceinline__ uint32_t canon_e2m1x8(uint32_t n) {   // "-0" (only the sign bit of a nibble set) -> +0
   const uint32_t t = n & 0x77777777u;
   const uint32_t nz = ((t + 0x77777777u) | t) & 0x88888888u;   // bit 3 of a nibble set iff its magnitude is not 0
   return n & (0x77777777u | nz);
@@ -458,12 +464,14 @@ __device__ __forceinline__ void wht_level(float (&x)[128]) {
 __device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 // K of the lane's token from its shared-memory row: 16 code words, 4 scale bytes; false if any decision is unsafe.
-__device__ __forceinline__ bool bulk_encode_k(uint32_t row, float c_k, uint32_t (&codes)[16], uint32_t& scale_word) {
+__device__ __forceinline__ bool bulk_encode_k(uint32_t tile, int lane, float c_k, uint32_t (&codes)[16], uint32_t& scale_word) {
   float x[128];
+  const uint32_t row = tile + 128 * lane, sw = (uint32_t)(lane & 7);
 #pragma unroll
   for (int j = 0; j < 16; ++j) {
     uint4 w;
-    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "r"(row + 16 * j));
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w)
+                 : "r"(row + kBulkHalf * (j >> 3) + ((((uint32_t)j & 7u) ^ sw) << 4)));
     x[8 * j + 0] = __uint_as_float(w.x << 16); x[8 * j + 1] = __uint_as_float(w.x & 0xFFFF0000u);
     x[8 * j + 2] = __uint_as_float(w.y << 16); x[8 * j + 3] = __uint_as_float(w.y & 0xFFFF0000u);
     x[8 * j + 4] = __uint_as_float(w.z << 16); x[8 * j + 5] = __uint_as_float(w.z & 0xFFFF0000u);
@@ -505,15 +513,16 @@ __device__ __forceinline__ bool bulk_encode_k(uint32_t row, float c_k, uint32_t 
       for (int i = 0; i < 8; ++i) r[i] = __fmul_rn(x[32 * g + 8 * w + i], ksc);
       const uint32_t lo = e2m1x8(r[0] - er, r[1] - er, r[2] - er, r[3] - er, r[4] - er, r[5] - er, r[6] - er, r[7] - er);
       const uint32_t hi = e2m1x8(r[0] + er, r[1] + er, r[2] + er, r[3] + er, r[4] + er, r[5] + er, r[6] + er, r[7] + er);
-      ok = ok && (lo == hi);
-      codes[4 * g + w] = lo;
+      ok = ok && (lo == hi);                           // raw codes: an interval over 0 counts as undecided too
+      codes[4 * g + w] = canon_e2m1x8(lo);
     }
   }
   return ok;
 }
 
 __global__ void __launch_bounds__(32 * kBulkWarps, 3)
-append_bulk_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v_new,
+append_bulk_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_constant__ CUtensorMap tmap_v,
+                   const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v_new,
                    const int32_t* __restrict__ cu_new, const int32_t* __restrict__ seq_lens,
                    const int32_t* __restrict__ block_tables, int max_pages, int batch, int total_new, int Hkv,
                    uint8_t* __restrict__ cache, double c_k, double c_v) {
@@ -544,22 +553,28 @@ append_bulk_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restric
   }
 
   // ---------------- whole block: rows -> shared memory
-  uint8_t* const wbase = bulk_smem + warp * kBulkWarpBytes;
-  const uint32_t sK = smem_addr(wbase), sV = sK + kBulkBuf, sM = sV + kBulkBuf;
+  const uint32_t sbase = (smem_addr(bulk_smem) + 1023u) & ~1023u;
+  const uint32_t sK = sbase + warp * kBulkTiles, sV = sK + 2 * kBulkHalf, sM = sbase + kBulkWarps * kBulkTiles + 512 * warp;
   const uint32_t barK = smem_addr(&bars[warp][0]), barV = barK + 8;
   if (lane == 0) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(barK));
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(barV));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(barK), "r"(32 * 256) : "memory");
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(barV), "r"(32 * 256) : "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(barK), "r"(2 * kBulkHalf) : "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(barV), "r"(2 * kBulkHalf) : "memory");
+    const int row0 = c0 + (q0 - p0);                   // k_new / v_new row of the block's first token
+#pragma unroll
+    for (int hf = 0; hf < 2; ++hf) {
+      asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                   ::"r"(sK + kBulkHalf * hf), "l"(&tmap_k), "r"(h * kHeadDim + 64 * hf), "r"(row0), "r"(barK) : "memory");
+    }
+#pragma unroll
+    for (int hf = 0; hf < 2; ++hf) {
+      asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                   ::"r"(sV + kBulkHalf * hf), "l"(&tmap_v), "r"(h * kHeadDim + 64 * hf), "r"(row0), "r"(barV) : "memory");
+    }
   }
   __syncwarp();
-  const long long row = ((long long)(c0 + (q0 - p0) + lane) * Hkv + h) * kHeadDim;   // this lane's token
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], 256, [%2];"
-               ::"r"(sK + kRowStride * lane), "l"(k_new + row), "r"(barK) : "memory");
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], 256, [%2];"
-               ::"r"(sV + kRowStride * lane), "l"(v_new + row), "r"(barV) : "memory");
   const int page = bt[lane >> 4];                      // lanes 0-15: first page of the block, 16-31: second
   uint8_t* const rec = cache + ((long long)page * Hkv + h) * kRecordBytes;
   const int t = lane & 15;                             // this lane's slot in its page
@@ -573,7 +588,7 @@ append_bulk_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restric
   unsigned bad_k;
   {
     uint32_t codes[16], scale_word;
-    const bool ok = bulk_encode_k(sK + kRowStride * lane, (float)c_k, codes, scale_word);
+    const bool ok = bulk_encode_k(sK, lane, (float)c_k, codes, scale_word);
     if (ok) {
       uint4* dst = reinterpret_cast<uint4*>(rec + kOffKCodes + 64 * t);
 #pragma unroll
@@ -587,7 +602,7 @@ append_bulk_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restric
   wait(barV);
   unsigned bad_v;
   {
-    const uint32_t vrow = sV + kRowStride * lane;
+    const uint32_t vrow = sV + 128 * lane, sw = (uint32_t)(lane & 7);
     bool ok = true;
     float mult[4];
 #pragma unroll
@@ -596,7 +611,7 @@ append_bulk_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restric
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
         uint4 w;
-        asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "r"(vrow + 64 * g + 16 * j));
+        asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "r"(vrow + kBulkHalf * (g >> 1) + ((((uint32_t)(4 * (g & 1) + j)) ^ sw) << 4)));
         mx = __vmaxu2(mx, __vmaxu2(__vmaxu2(w.x & 0x7FFF7FFFu, w.y & 0x7FFF7FFFu), __vmaxu2(w.z & 0x7FFF7FFFu, w.w & 0x7FFF7FFFu)));
       }
       const float m = __uint_as_float(max(mx >> 16, mx & 0xFFFFu) << 16);   // bf16 magnitudes order like their bits
@@ -614,6 +629,7 @@ append_bulk_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restric
   __syncwarp();
 
   // ---------------- V pass 2: lane = channels 4 lane .. 4 lane + 3 (group lane >> 3), an octet of tokens per word
+  const uint32_t vsrc = sV + kBulkHalf * (lane >> 4) + 8 * (lane & 1), vchunk = (uint32_t)((lane & 15) >> 1);
 #pragma unroll 1
   for (int o = 0; o < 4; ++o) {
     float r[4][8];
@@ -621,7 +637,8 @@ append_bulk_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restric
     for (int tt = 0; tt < 8; ++tt) {
       uint32_t w0, w1;
       float mu;
-      asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(w0), "=r"(w1) : "r"(sV + kRowStride * (8 * o + tt) + 8 * lane));
+      asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(w0), "=r"(w1)
+                   : "r"(vsrc + 128 * (8 * o + tt) + ((vchunk ^ (uint32_t)tt) << 4)));   // row & 7 = tt
       asm volatile("ld.shared.f32 %0, [%1];" : "=f"(mu) : "r"(sM + 16 * (8 * o + tt) + 4 * (lane >> 3)));
       r[0][tt] = __fmul_rn(__uint_as_float(w0 << 16), mu);
       r[1][tt] = __fmul_rn(__uint_as_float(w0 & 0xFFFF0000u), mu);
@@ -631,7 +648,7 @@ append_bulk_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restric
     uint32_t vw[4];
 #pragma unroll
     for (int c = 0; c < 4; ++c)
-      vw[c] = e2m1x8(r[c][0], r[c][1], r[c][2], r[c][3], r[c][4], r[c][5], r[c][6], r[c][7]);
+      vw[c] = canon_e2m1x8(e2m1x8(r[c][0], r[c][1], r[c][2], r[c][3], r[c][4], r[c][5], r[c][6], r[c][7]));
     const int pg = __shfl_sync(kFull, page, 16 * (o >> 1));
     uint8_t* const rec_o = cache + ((long long)pg * Hkv + h) * kRecordBytes;
     *reinterpret_cast<uint4*>(rec_o + kOffVCodes + 512 * (o & 1) + 16 * lane) = make_uint4(vw[0], vw[1], vw[2], vw[3]);
@@ -656,6 +673,37 @@ append_bulk_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restric
       __syncwarp();
     }
   }
+}
+
+// 2-D TMA view of k_new / v_new: [rows][kv heads x 128] bf16; box = 32 rows x 64 channels (128 B: the widest row the
+// 128-byte swizzle takes), so a block's K (or V) rows of one kv head are two tensor copies.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+int32_t rows_map(const void* rows, long long n_rows, int Hkv, CUtensorMap* out) {
+  static EncodeTiledFn encode = nullptr;               // set once; racing first calls store the same pointer
+  if (!encode) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess || fn == nullptr) {
+      set_error("append: cuTensorMapEncodeTiled is not available from this driver");
+      return UQ_ERR_CUDA;
+    }
+    encode = (EncodeTiledFn)fn;
+  }
+  const cuuint64_t gdim[2] = {(cuuint64_t)Hkv * kHeadDim, (cuuint64_t)n_rows};
+  const cuuint64_t gstr[1] = {(cuuint64_t)Hkv * kHeadDim * 2};
+  const cuuint32_t box[2] = {64, 32};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult cr = encode(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(rows), gdim, gstr, box, estr,
+                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (cr != CUDA_SUCCESS) {
+    set_error("append: cuTensorMapEncodeTiled failed with CUresult %d", (int)cr);
+    return UQ_ERR_CUDA;
+  }
+  return UQ_OK;
 }
 
 }  // namespace
@@ -699,6 +747,10 @@ extern "C" int32_t uq_rotate_quantize_append(const uq_config* cfg, const void* k
       if (e != cudaSuccess) return check_cuda(e, "append: cudaFuncSetAttribute");
       attr_set = true;
     }
+    CUtensorMap tmap_k, tmap_v;
+    st = rows_map(k_new, total_new, cfg->num_kv_heads, &tmap_k);
+    if (st == UQ_OK) st = rows_map(v_new, total_new, cfg->num_kv_heads, &tmap_v);
+    if (st != UQ_OK) return st;
     const long long n_units = (long long)(total_new >> 5) + 2LL * batch;
     const long long bx = (n_units + kBulkWarps - 1) / kBulkWarps;
     if (bx > 0x7fffffffLL) {
@@ -706,8 +758,8 @@ extern "C" int32_t uq_rotate_quantize_append(const uq_config* cfg, const void* k
       return UQ_ERR_INVALID_ARG;
     }
     st = check_cuda(launch_pdl(append_bulk_kernel, dim3((unsigned)bx, (unsigned)cfg->num_kv_heads), dim3(32 * kBulkWarps),
-                               (size_t)kBulkSmem, (cudaStream_t)stream, (const uint16_t*)k_new, (const uint16_t*)v_new,
-                               cu_new, seq_lens, block_tables, (int)max_pages, (int)batch, (int)total_new,
+                               (size_t)kBulkSmem, (cudaStream_t)stream, tmap_k, tmap_v, (const uint16_t*)k_new,
+                               (const uint16_t*)v_new, cu_new, seq_lens, block_tables, (int)max_pages, (int)batch, (int)total_new,
                                (int)cfg->num_kv_heads, (uint8_t*)cache, (double)cfg->c_k, (double)cfg->c_v),
                     "uq_rotate_quantize_append (bulk) launch");
     if (st != UQ_OK || q_rows == 0) return st;
