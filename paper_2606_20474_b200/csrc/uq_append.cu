@@ -449,15 +449,39 @@ __device__ __forceinline__ uint32_t canon_e2m1x8(uint32_t n) {   // "-0" (only t
   return n & (0x77777777u | nz);
 }
 
-// one butterfly level over the 128 values of a thread: index bit log2(H)
-template <int H>
-__device__ __forceinline__ void wht_level(float (&x)[128]) {
+// Packed float32 pairs (one instruction, two IEEE results: each half rounds exactly as the scalar operation does).
+__device__ __forceinline__ uint64_t pack2(float a, float b) {
+  uint64_t v;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(a), "f"(b));
+  return v;
+}
+__device__ __forceinline__ void unpack2(uint64_t v, float& a, float& b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ uint64_t mul2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+
+// one butterfly level over the 64 pairs {x[2i], x[2i+1]} of a thread: element index bit log2(2 HP).  a - b is
+// fma(b, -1, a): the product is exact, so it rounds once, like the subtraction.
+template <int HP>
+__device__ __forceinline__ void wht_level2(uint64_t (&p)[64], uint64_t minus1) {
 #pragma unroll
-  for (int k = 0; k < 64; ++k) {
-    const int j = ((k / H) * 2 * H) + (k % H);
-    const float a = x[j], b = x[j + H];
-    x[j] = __fadd_rn(a, b);
-    x[j + H] = __fsub_rn(a, b);
+  for (int k = 0; k < 32; ++k) {
+    const int j = ((k / HP) * 2 * HP) + (k % HP);
+    const uint64_t a = p[j], b = p[j + HP];
+    p[j] = add2(a, b);
+    p[j + HP] = fma2(b, minus1, a);
   }
 }
 
@@ -465,29 +489,27 @@ __device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)
 
 // K of the lane's token from its shared-memory row: 16 code words, 4 scale bytes; false if any decision is unsafe.
 __device__ __forceinline__ bool bulk_encode_k(uint32_t tile, int lane, float c_k, uint32_t (&codes)[16], uint32_t& scale_word) {
-  float x[128];
+  uint64_t p[64];                                        // p[i] = {x[2i], x[2i+1]}
   const uint32_t row = tile + 128 * lane, sw = (uint32_t)(lane & 7);
+  float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;          // sum |x_i|: four chains
 #pragma unroll
   for (int j = 0; j < 16; ++j) {
     uint4 w;
     asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w)
                  : "r"(row + kBulkHalf * (j >> 3) + ((((uint32_t)j & 7u) ^ sw) << 4)));
-    x[8 * j + 0] = __uint_as_float(w.x << 16); x[8 * j + 1] = __uint_as_float(w.x & 0xFFFF0000u);
-    x[8 * j + 2] = __uint_as_float(w.y << 16); x[8 * j + 3] = __uint_as_float(w.y & 0xFFFF0000u);
-    x[8 * j + 4] = __uint_as_float(w.z << 16); x[8 * j + 5] = __uint_as_float(w.z & 0xFFFF0000u);
-    x[8 * j + 6] = __uint_as_float(w.w << 16); x[8 * j + 7] = __uint_as_float(w.w & 0xFFFF0000u);
-  }
-  float S = 0.f;                                         // sum |x_i|: four chains
-  {
-    float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+    const uint32_t ww[4] = {w.x, w.y, w.z, w.w};
 #pragma unroll
-    for (int i = 0; i < 128; i += 4) {
-      s0 += fabsf(x[i]); s1 += fabsf(x[i + 1]); s2 += fabsf(x[i + 2]); s3 += fabsf(x[i + 3]);
+    for (int i = 0; i < 4; ++i) {                        // first butterfly level (index bit 0) while unpacking
+      const float a = __uint_as_float(ww[i] << 16), b = __uint_as_float(ww[i] & 0xFFFF0000u);
+      if (i & 1) { s2 += fabsf(a); s3 += fabsf(b); } else { s0 += fabsf(a); s1 += fabsf(b); }
+      p[4 * j + i] = pack2(__fadd_rn(a, b), __fsub_rn(a, b));
     }
-    S = (s0 + s1) + (s2 + s3);
   }
-  // butterfly: seven levels, one rounding per output and level (the bound kBound is for exactly this)
-  wht_level<1>(x); wht_level<2>(x); wht_level<4>(x); wht_level<8>(x); wht_level<16>(x); wht_level<32>(x); wht_level<64>(x);
+  const float S = (s0 + s1) + (s2 + s3);
+  // the other six levels, one rounding per output and level (the bound kBound is for exactly this)
+  const uint64_t minus1 = pack2(-1.0f, -1.0f);
+  wht_level2<1>(p, minus1); wht_level2<2>(p, minus1); wht_level2<4>(p, minus1);
+  wht_level2<8>(p, minus1); wht_level2<16>(p, minus1); wht_level2<32>(p, minus1);
   const float kappa = 0x1.6a09e6p-4f;                    // float32 nearest to 2^-3.5
   const float eps = __fmul_rn(S, kBound);
   bool ok = (S > 1e-30f) && (S < 1e30f);
@@ -496,7 +518,11 @@ __device__ __forceinline__ bool bulk_encode_k(uint32_t tile, int lane, float c_k
   for (int g = 0; g < 4; ++g) {
     float m = 0.f;
 #pragma unroll
-    for (int i = 0; i < 32; ++i) m = fmaxf(m, fabsf(x[32 * g + i]));
+    for (int i = 0; i < 16; ++i) {
+      float a, b;
+      unpack2(p[16 * g + i], a, b);
+      m = fmaxf(m, fmaxf(fabsf(a), fabsf(b)));
+    }
     m = __fmul_rn(m, kappa);                             // = max |fl(kappa x_i)|: rounding is monotone
     int E;
     const bool okg = scale_exponent_f32(c_k, m, eps, E) && (E >= -100) && (E <= 100);
@@ -506,15 +532,20 @@ __device__ __forceinline__ bool bulk_encode_k(uint32_t tile, int lane, float c_k
     const float sc = pow2_neg(E);
     const float ksc = __fmul_rn(kappa, sc);              // exact: fl(x kappa) 2^-E = fl(x (kappa 2^-E))
     const float er = __fmaf_rn(__fmul_rn(eps, sc), 1.0001f, 1.2e-6f);   // + the rounding of the two additions below
+    const uint64_t ksc2 = pack2(ksc, ksc), per = pack2(er, er), mer = pack2(-er, -er);
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
-      float r[8];
+      float lo[8], hi[8];
 #pragma unroll
-      for (int i = 0; i < 8; ++i) r[i] = __fmul_rn(x[32 * g + 8 * w + i], ksc);
-      const uint32_t lo = e2m1x8(r[0] - er, r[1] - er, r[2] - er, r[3] - er, r[4] - er, r[5] - er, r[6] - er, r[7] - er);
-      const uint32_t hi = e2m1x8(r[0] + er, r[1] + er, r[2] + er, r[3] + er, r[4] + er, r[5] + er, r[6] + er, r[7] + er);
-      ok = ok && (lo == hi);                           // raw codes: an interval over 0 counts as undecided too
-      codes[4 * g + w] = canon_e2m1x8(lo);
+      for (int i = 0; i < 4; ++i) {
+        const uint64_t r = mul2(p[16 * g + 4 * w + i], ksc2);
+        unpack2(add2(r, mer), lo[2 * i], lo[2 * i + 1]);
+        unpack2(add2(r, per), hi[2 * i], hi[2 * i + 1]);
+      }
+      const uint32_t cl = e2m1x8(lo[0], lo[1], lo[2], lo[3], lo[4], lo[5], lo[6], lo[7]);
+      const uint32_t ch = e2m1x8(hi[0], hi[1], hi[2], hi[3], hi[4], hi[5], hi[6], hi[7]);
+      ok = ok && (cl == ch);                           // raw codes: an interval over 0 counts as undecided too
+      codes[4 * g + w] = canon_e2m1x8(cl);
     }
   }
   return ok;
