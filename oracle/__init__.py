@@ -71,6 +71,9 @@ def _load():
     lib.uqo_attention_dense.restype = None
     lib.uqo_attention_dense.argtypes = [f64p, f64p, f64p, ctypes.c_int64, ctypes.c_int,
                                         ctypes.c_int, ctypes.c_int, ctypes.c_double, f64p]
+    lib.uqo_calib_sq_err.restype = None
+    lib.uqo_calib_sq_err.argtypes = [u16p, ctypes.c_int64, ctypes.c_int, ctypes.c_int,
+                                     ctypes.POINTER(ctypes.c_float), ctypes.c_int, ctypes.c_int, f64p, f64p]
     lib.uqo_num_threads.restype = ctypes.c_int
     lib.uqo_set_num_threads.argtypes = [ctypes.c_int]
     _lib = lib
@@ -166,6 +169,21 @@ def encode_kv(k_bits, v_bits, c_k: float = 0.156, c_v: float = 0.156):
                           _ptr(vc, ctypes.c_uint8), _ptr(vs, ctypes.c_uint8))
     return (kc.reshape(lead + (d // 2,)), ks.reshape(lead + (d // 32,)),
             vc.reshape(lead + (d // 2,)), vs.reshape(lead + (d // 32,)))
+
+
+def calib_sq_err(x_bits, c_grid, rotate: bool = True, pow2: bool = True):
+    """Objective of Eq.(2) on a grid of constants: x_bits uint16 bf16 patterns [n, d], c_grid
+    float32 [n_c].  Returns (sq_err float64 [n_c], sq_norm float): sums over all elements of (z - zhat)^2 and
+    z^2, z rotated if `rotate`; pow2 selects the deployed power-of-two scale (Alg. 1 l.3) against s = c*m."""
+    x_bits = _c(x_bits, np.uint16)
+    c_grid = _c(c_grid, np.float32)
+    n, d = x_bits.shape
+    sq_err = np.zeros(c_grid.shape[0], np.float64)
+    sq_norm = np.zeros(1, np.float64)
+    _load().uqo_calib_sq_err(_ptr(x_bits, ctypes.c_uint16), n, d, int(bool(rotate)), _ptr(c_grid, ctypes.c_float),
+                             c_grid.shape[0], int(bool(pow2)), _ptr(sq_err, ctypes.c_double),
+                             _ptr(sq_norm, ctypes.c_double))
+    return sq_err, float(sq_norm[0])
 
 
 def encode_q(q_bits) -> np.ndarray:

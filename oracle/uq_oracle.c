@@ -19,7 +19,9 @@
  * Pins (tests/test_oracle_pins.py): Hadamard orthogonality and Kronecker
  * structure, decode table vs Eq.(1), exact round trip, brute-force nearest
  * level, scale thresholds, statistical fingerprints, the paper's two constants
- * (0.156 / 0.195), library E2M1/E4M3 casts, softmax closed forms, torch SDPA.
+ * (0.156 / 0.195), library E2M1/E4M3 casts, softmax closed forms, torch SDPA; the Eq.(2)
+ * objective (O11) against an independent numpy quantiser, exactly representable inputs
+ * (zero error), the rotation's norm invariance and the paper's ordering of c (P11).
  * Parity unpinned: the attention *output values* for concrete inputs (the paper
  * prints no worked example) — pinned only through the closed forms above.
  */
@@ -155,6 +157,66 @@ void uqo_encode_kv(const uint16_t* k_bf16, const uint16_t* v_bf16, int64_t n_vec
     free(x);
     free(y);
   }
+}
+
+/* ---- O11: the objective of Eq.(2) on a grid of constants: for every c_j,
+ *     sq_err[j] = sum over all elements z of (z - zhat_j(z))^2,   sq_norm = sum z^2,
+ * with z the rotated vector (rotate != 0: Alg. 1 l.1) or the vector itself, m the absmax of
+ * z's 32-channel group and
+ *   pow2 == 0: s = c_j*m, the scale of Eq.(2) as printed; zhat = s * q(z/s), q = nearest level
+ *              of F (the ladder of O5 applied to r = |z|/s);
+ *   pow2 != 0: s = 2^E, E = round(log2(c_j*m)) (O4): the quantiser Alg. 1 deploys
+ *              (l.3-5, :253-255) followed by Eq.(1); zhat = dequant(encode(z, E), E).
+ * c_j is a float (as uq_config.c_k) used as (double)c_j.  A group with m = 0 contributes 0.
+ * E[.] of Eq.(2) is sq_err / (n_vec*d); its argmin over j is the calibrated constant (:128).
+ * Plain loops, vector after vector, one double accumulator per c_j. */
+static int uqo_mag_of_ratio(double r) {
+  return (r > 0.25) + (r >= 0.75) + (r > 1.25) + (r >= 1.75) + (r > 2.5) + (r >= 3.5) + (r > 5.0);
+}
+
+void uqo_calib_sq_err(const uint16_t* x_bf16, int64_t n_vec, int d, int rotate, const float* c_grid,
+                      int n_c, int pow2, double* sq_err /*[n_c]*/, double* sq_norm /*[1]*/) {
+  static const double F[8] = {0.0, 0.5, 1.0, 1.5, 2.0, 3.0, 4.0, 6.0};
+  double* x = (double*)malloc(sizeof(double) * (size_t)d);
+  double* y = (double*)malloc(sizeof(double) * (size_t)d);
+  for (int j = 0; j < n_c; ++j) sq_err[j] = 0.0;
+  *sq_norm = 0.0;
+  for (int64_t n = 0; n < n_vec; ++n) {
+    for (int i = 0; i < d; ++i) x[i] = uqo_bf16_to_double(x_bf16[n * d + i]);
+    if (rotate) uqo_hadamard(x, d, y);
+    else memcpy(y, x, sizeof(double) * (size_t)d);
+    for (int i = 0; i < d; ++i) *sq_norm += y[i] * y[i];
+    for (int g = 0; g < d / UQ_GROUP; ++g) {
+      const double* yg = y + g * UQ_GROUP;
+      double m = 0.0;
+      for (int i = 0; i < UQ_GROUP; ++i) {
+        double a = fabs(yg[i]);
+        if (a > m) m = a;
+      }
+      for (int j = 0; j < n_c; ++j) {
+        const double c = (double)c_grid[j];
+        if (pow2) {
+          int E = uqo_scale_exponent(c, m);
+          for (int i = 0; i < UQ_GROUP; ++i) {
+            double zh = uqo_dequant(uqo_e2m1_encode(yg[i], E), (uint8_t)(E + 127));
+            double e = yg[i] - zh;
+            sq_err[j] += e * e;
+          }
+        } else {
+          double s = c * m;
+          if (!(s > 0.0)) continue;
+          for (int i = 0; i < UQ_GROUP; ++i) {
+            double lev = F[uqo_mag_of_ratio(fabs(yg[i]) / s)];
+            double zh = (yg[i] < 0.0 ? -lev : lev) * s;
+            double e = yg[i] - zh;
+            sq_err[j] += e * e;
+          }
+        }
+      }
+    }
+  }
+  free(x);
+  free(y);
 }
 
 /* ---- O7: cast_fp8_e4m3 (Alg. 1 l.6).  OCP E4M3 "FN": bias 7, normals

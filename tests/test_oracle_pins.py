@@ -223,6 +223,60 @@ def test_p7_c_equal_one_uses_no_shrinkage():
     assert codes.max() <= 3                              # nothing above 1.5 grid units is used
 
 
+# ----------------------------------------------------------------------------- P11 the Eq.(2) objective (O11)
+def _bf16_bits(a):
+    return (torch.from_numpy(np.asarray(a, np.float32)).to(torch.bfloat16).view(torch.uint16).numpy())
+
+
+@pytest.mark.parametrize("pow2", [False, True])
+def test_p11_objective_equals_an_independent_numpy_quantiser(pow2):
+    """oracle.calib_sq_err without rotation against _mse_for_c above (argmin over the level set, numpy log2 /
+    rint for the exponent): the same mean squared error for every c of a grid (a tie between two levels costs
+    the same whichever is taken)."""
+    rng = np.random.default_rng(21)
+    bits = _bf16_bits(rng.standard_normal((400, 128)) * np.exp(rng.standard_normal((400, 1))))
+    y = oracle.bf16_to_double(bits)
+    cs = np.array([0.1, 0.14, 0.156, 0.17, 0.195, 0.25, 0.4, 1.0], np.float32)
+    sq, nrm = oracle.calib_sq_err(bits, cs, rotate=False, pow2=pow2)
+    assert nrm == pytest.approx(float((y ** 2).sum()), rel=1e-13)
+    for j, c in enumerate(cs):
+        ref = _mse_for_c(y.reshape(-1, 32), float(c), pow2) * y.size
+        assert sq[j] == pytest.approx(ref, rel=1e-10), (pow2, c)
+
+
+def test_p11_exactly_representable_inputs_have_zero_error_and_rotation_keeps_the_norm():
+    rng = np.random.default_rng(22)
+    lev = np.array(LEVELS + [-v for v in LEVELS[1:]])
+    e = rng.integers(-6, 7, (64, 4))
+    x = lev[rng.integers(0, 15, (64, 4, 32))] * 2.0 ** e[..., None]
+    x[:, :, 0] = 6.0 * 2.0 ** e                              # group max 6 * 2^e: E = e at c = 0.156 (0.936 * 2^e)
+    bits = _bf16_bits(x.reshape(64, 128))
+    sq, nrm = oracle.calib_sq_err(bits, np.array([0.156], np.float32), rotate=False, pow2=True)
+    assert sq[0] == 0.0 and nrm == float((x ** 2).sum())
+    # rotation: H/sqrt(d) is orthogonal, so sum z^2 is the same with and without it
+    g = _bf16_bits(rng.standard_normal((50, 128)))
+    _, n0 = oracle.calib_sq_err(g, np.array([0.156], np.float32), rotate=False)
+    _, n1 = oracle.calib_sq_err(g, np.array([0.156], np.float32), rotate=True)
+    assert n1 == pytest.approx(n0, rel=1e-13)
+
+
+def test_p11_paper_ordering_of_the_constants_on_rotated_vectors():
+    """PAPER.md:128, :333 and Table 5: on rotated keys the MSE optimum of Eq.(2) is 0.156, the power-of-two
+    optimum 0.195, and c = 1.0 is far worse than either — here on rotated unit-sphere-like vectors (Fig. 2)."""
+    g = _golden()
+    rng = np.random.default_rng(23)
+    x = rng.standard_normal((3000, 128))
+    x[:, rng.choice(128, 3, replace=False)] *= 8.0           # outlier channels: the rotation spreads them
+    bits = _bf16_bits(x)
+    cs = np.arange(0.10, 0.32, 0.004).astype(np.float32)
+    cont, _ = oracle.calib_sq_err(bits, cs, rotate=True, pow2=False)
+    p2, _ = oracle.calib_sq_err(bits, cs, rotate=True, pow2=True)
+    assert abs(float(cs[int(np.argmin(cont))]) - float(g["c_default"])) < 0.02
+    assert abs(float(cs[int(np.argmin(p2))]) - float(g["c_power_of_two_optimal"])) < 0.02
+    three, _ = oracle.calib_sq_err(bits, np.array([0.156, 0.195, 1.0], np.float32), rotate=True, pow2=False)
+    assert three[0] < three[1] < three[2] and three[2] > 5 * three[0]
+
+
 # ----------------------------------------------------------------------------- P8 library casts
 @pytest.fixture(scope="module")
 def libcasts():
