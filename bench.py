@@ -494,6 +494,53 @@ def run_bulk_append(args):
                          "algorithmic_bytes": nbytes, "peak_source": peak_src}}
 
 
+# ----------------------------------------------------------------------------- calibration
+def run_calibrate(args):
+    """Not the headline metric: uq_calibrate_c (Eq.(2)) over VECTORS synthetic keys of the chosen config
+    and the 56 constants 0.100 .. 0.320 in steps of 0.004, power-of-two scale; CUDA events over K calls.  Bound: the
+    float64 pipe.  Counted float64 operations per (vector, constant): 128 elements x (7 ladder compares + 2 products
+    + 2 additions) = 1408, plus per vector and pass of 8 constants the rotation (7 x 128 additions + 128 products)
+    and the group maxima (128 compares): 1152 / 8 = 144 per (vector, constant).  Peak: 64 float64 lanes per SM x
+    SM count x the SM clock (one operation per lane and cycle)."""
+    import paper_2606_20474_b200 as uq
+    from paper_2606_20474_b200 import workloads as W
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the hot path has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    wl = _workload(args.config, 0)
+    cfg = uq.UQConfig(num_q_heads=wl.num_q_heads, num_kv_heads=wl.num_kv_heads)
+    n_tok = max(1, min(args.calibrate // wl.num_kv_heads, int(wl.ctx_lens[0])))
+    k, _ = W.gen_kv(wl, 0, 0, n_tok, dev)
+    x = k.reshape(-1, wl.head_dim).contiguous()
+    cs = torch.arange(0.100, 0.322, 0.004, dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream()
+    for _ in range(max(args.warmup, 3)):
+        sq, nrm = uq.calibrate_c(cfg, x, cs, rotate=True, pow2_scale=True, stream=stream)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        sq, nrm = uq.calibrate_c(cfg, x, cs, rotate=True, pow2_scale=True, stream=stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    evals = x.shape[0] * cs.shape[0]
+    ops = evals * (1408 + 144)
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    peak = 64 * sms * 1.965e9 / 1e12
+    best = float(cs[int(torch.argmin(sq).item())])
+    return {"metric": "calibrate_vector_constant_evals_per_s", "value": round(evals / (ms * 1e-3) / 1e9, 3), "unit": "G/s",
+            "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": round(ms, 5),
+            "higher_is_better": True, "dtype": "f64", "data": "synthetic", "impl": "ours",
+            "config": {"workload": f"uq_calibrate_c: {x.shape[0]} rotated key vectors of {wl.name} x {cs.shape[0]} "
+                                   "constants (0.100 .. 0.320), power-of-two scale"},
+            "argmin_c": round(best, 3), "rel_mse_at_argmin": float(sq.min().item() / nrm.item()), "gpu_launches": args.steps,
+            "roofline": {"bound": "alu", "kernel": "uq::calib_kernel", "achieved": round(ops / (ms * 1e-3) / 1e12, 3),
+                         "peak": round(peak, 2), "unit": "Tfp64op/s", "frac": round(ops / (ms * 1e-3) / 1e12 / peak, 4),
+                         "traffic": None, "peak_source": "64 float64 lanes per SM x SMs x 1.965 GHz (DESIGN.md 5.4)"}}
+
+
 # ----------------------------------------------------------------------------- main
 def main():
     ap = argparse.ArgumentParser()
@@ -509,6 +556,8 @@ def main():
                     help="with --bulk-append: sequences that receive TOKENS new tokens each in one call")
     ap.add_argument("--bulk-append", type=int, default=0, metavar="TOKENS",
                     help="instead of the decode step, time bulk quantize-on-append of TOKENS new tokens per call")
+    ap.add_argument("--calibrate", type=int, default=0, metavar="VECTORS",
+                    help="instead of the decode step, time uq_calibrate_c over VECTORS key vectors and 56 constants")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--ref-budget", type=float, default=90.0, help="seconds for the whole --impl reference run")
     args = ap.parse_args()
@@ -520,6 +569,10 @@ def main():
     if args.bulk_append > 0:
         if rank == 0:
             print(json.dumps(run_bulk_append(args)), flush=True)
+        return 0
+    if args.calibrate > 0:
+        if rank == 0:
+            print(json.dumps(run_calibrate(args)), flush=True)
         return 0
     if args.impl == "reference":
         if rank == 0:

@@ -14,6 +14,7 @@ from .binding import (  # noqa: F401
     HostStage,
     alloc_cache,
     cache_record_bytes,
+    calibrate_c,
     decode_attention,
     decode_step,
     decode_step_host,

@@ -521,3 +521,31 @@ def test_decode_refuses_more_than_2048_sequences():
     with pytest.raises(uq.UQError, match="2048"):
         uq.decode_attention(cfg, q8, cache, bt, lens, 2, acc, ml)
     torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("rotate,pow2", [(True, True), (True, False), (False, True), (False, False)])
+def test_calibrate_c_matches_the_oracle_objective(rotate, pow2):
+    """uq_calibrate_c (Eq.(2)) against oracle.calib_sq_err on keys with outlier
+    channels, scale spread over vectors, all-zero vectors and groups: every sum within 1e-11 relative (the float64
+    additions are ordered differently), the same argmin, and — on the rotated keys — the paper's constants."""
+    g = torch.Generator(device="cpu"); g.manual_seed(77)
+    n = 3001                                               # not a multiple of the warps of a CTA
+    x = torch.randn((n, 128), generator=g) * torch.exp(0.7 * torch.randn((n, 1), generator=g))
+    x[:, [3, 40, 97]] *= 9.0
+    x[5] = 0; x[6, 32:64] = 0; x[7] = 2.0 ** -120; x[8] = 3.0e30
+    x = x.to(torch.bfloat16)
+    cs = np.concatenate([np.arange(0.10, 0.30, 0.0125), [0.156, 0.195, 1.0, 0.5]]).astype(np.float32)   # 20: 8 + 8 + 4
+    cfg = uq.UQConfig(num_q_heads=8, num_kv_heads=1)
+    sq, nrm = uq.calibrate_c(cfg, x.to(DEV), torch.from_numpy(cs).to(DEV), rotate=rotate, pow2_scale=pow2)
+    torch.cuda.synchronize()
+    sq, nrm = sq.cpu().numpy(), float(nrm.cpu()[0])
+    ref, ref_nrm = oracle.calib_sq_err(H.bits(x), cs, rotate=rotate, pow2=pow2)
+    assert nrm == pytest.approx(ref_nrm, rel=1e-11)
+    np.testing.assert_allclose(sq, ref, rtol=1e-11, atol=0)
+    assert int(np.argmin(sq)) == int(np.argmin(ref))
+    if rotate:
+        # without the rows of extreme magnitude (they dominate the sums) the rotated keys behave like the paper's:
+        # continuous optimum near 0.156 (:128), power-of-two optimum near 0.195 (:333)
+        sq2, _ = uq.calibrate_c(cfg, x[9:].contiguous().to(DEV), torch.from_numpy(cs).to(DEV), rotate=True, pow2_scale=pow2)
+        best = float(cs[int(torch.argmin(sq2[:16]).item())])
+        assert abs(best - (0.195 if pow2 else 0.156)) < 0.03
