@@ -101,8 +101,8 @@ size_t uq_cache_record_bytes(const uq_config* cfg);
  *                saturating at +-448, zero stored as 0x00.
  *
  * Two kernels, one result: calls with on average >= 64 new tokens per sequence (and >= 1024 in all, k_new / v_new
- * 16-byte aligned) take the bulk kernel (one warp per aligned block of 32 positions, rows staged in shared memory,
- * the rotation done in registers with one token per lane); all other calls, and the heads / tails of a bulk
+ * 16-byte aligned) take the bulk kernel (one warp per page, rows staged in shared memory by TMA, the rotation
+ * done in registers with two lanes per token); all other calls, and the partly covered first / last page of a bulk
  * call's ranges, one warp per aligned octet of positions.
  *
  * Every rounding decision (scale exponent, E2M1 code, E4M3 byte) is taken on float64 values of

@@ -321,26 +321,34 @@ append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v
 
 // ---------------------------------------------------------------- bulk (prefill-sized) append
 // SURVEY 8(f) rank 1.  The kernel above spends a warp on every vector: 326 warp instructions per (token, kv head),
-// a third of them shuffles and lane bookkeeping.  Here a warp takes an aligned block of 32 positions (two pages) of
-// one kv head, stages its K and V rows in shared memory with four TMA tensor copies (k_new / v_new seen as
-// [rows][kv heads x 128] bf16, box 32 rows x 64 channels, completion on an mbarrier) and works in two thread mappings:
-//   K      lane = token: the whole 128-channel vector in registers, the Walsh-Hadamard butterfly is 7 x 64
-//          in-register add/sub pairs (no shuffle), the same float32 error-interval test as the fast path above decides
-//          every scale exponent and code, 64 B of codes and one scale word are stored per lane;
-//   V      pass 1, lane = token: group maxima by packed 16-bit integer maxima of the bf16 magnitudes -> scale exponent,
-//          scale bytes, and the power-of-two multipliers left in shared memory;
+// a third of them shuffles and lane bookkeeping.  Here a warp takes one page (16 aligned positions) of one kv head,
+// stages its K and V rows in shared memory with four TMA tensor copies (k_new / v_new seen as
+// [rows][kv heads x 128] bf16, box 16 rows x 64 channels, completion on an mbarrier) and works in two thread mappings:
+//   K      lanes t and t + 16 = token t, 64 channels (two whole scale groups) each: the butterfly level between the
+//          two halves is a shuffle of the packed bf16 words, the other six are in-register add/sub pairs on packed
+//          float32 pairs; the same float32 error-interval test as the fast path above decides every scale exponent
+//          and code; 32 B of codes and two scale bytes are stored per lane;
+//   V      pass 1, lane = (token, channel half): group maxima by packed 16-bit integer maxima of the bf16
+//          magnitudes -> scale exponent, scale bytes, and the power-of-two multipliers left in shared memory;
 //          pass 2, lane = 4 channels: eight tokens of a channel make one 32-bit word of the token-major layout
 //          (four cvt.e2m1x2 per word), one 16-byte store per lane and octet.
-// A vector whose interval test fails (0.45 % of N(0,1) keys) is redone by the whole warp with store_k / append_octet
-// (float64), after the fast lanes have stored; a block that the call covers only partly goes through append_octet
-// octet by octet.  The bytes written are those of the kernel above in every case.
+// A vector whose interval test fails (0.45 % of N(0,1) keys) is redone by the whole warp with store_k /
+// append_octet_v (float64), after the fast lanes have stored; a page that the call covers only partly goes through
+// append_octet octet by octet.  The bytes written are those of the kernel above in every case.
+// (First version: a block of 32 positions per warp, lane = token with all 128 channels in registers — 78 instead
+// of 96 instructions per vector but 168 registers, 11 warps per SM; this one runs 20 warps per SM and is 2-8 %
+// faster, profiles/r01_append_bulk_cfg2.md.)
 constexpr int kBulkWarps = 4;
-// Shared memory per warp: the K and the V rows of its 32 tokens as two channel halves each — a TMA tensor tile of
-// [32 tokens][64 channels] bf16 = 32 rows of 128 B with the 128-byte swizzle (16-byte chunk c of row r sits at chunk
-// c ^ (r & 7)), so a lane reading its own row with 16-byte loads is bank-conflict free — and 32 x 4 V multipliers.
-constexpr int kBulkHalf = 32 * 128;                    // 4096
-constexpr int kBulkTiles = 4 * kBulkHalf;              // K lo, K hi, V lo, V hi: 16,384 per warp
-constexpr int kBulkSmem = kBulkWarps * (kBulkTiles + 512) + 1024;   // + alignment slack (the swizzle atom is 1024 B)
+#ifndef UQ_BULK_CTAS
+#define UQ_BULK_CTAS 5
+#endif
+// Shared memory per warp: the K and the V rows of its 16 tokens (one page) as two channel halves each — a TMA tensor
+// tile of [16 tokens][64 channels] bf16 = 16 rows of 128 B with the 128-byte swizzle (16-byte chunk c of row r sits
+// at chunk c ^ (r & 7)), so a lane reading its own row with 16-byte loads is bank-conflict free — and 16 x 4 V
+// multipliers.
+constexpr int kBulkHalf = 16 * 128;                    // 2048
+constexpr int kBulkTiles = 4 * kBulkHalf;              // K lo, K hi, V lo, V hi: 8192 per warp
+constexpr int kBulkSmem = kBulkWarps * (kBulkTiles + 256) + 1024;   // + alignment slack (the swizzle atom is 1024 B)
 
 // eight values -> eight E2M1 codes, value i in bits 4i..4i+3 (raw hardware result: may hold "-0")
 __device__ __forceinline__ uint32_t e2m1x8(float r0, float r1, float r2, float r3, float r4, float r5, float r6, float r7) {
@@ -383,12 +391,12 @@ __device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
   return d;
 }
 
-// one butterfly level over the 64 pairs {x[2i], x[2i+1]} of a thread: element index bit log2(2 HP).  a - b is
-// fma(b, -1, a): the product is exact, so it rounds once, like the subtraction.
+// one butterfly level over the 32 pairs {x[2i], x[2i+1]} of a lane (64 channels): element index bit log2(2 HP).
+// a - b is fma(b, -1, a): the product is exact, so it rounds once, like the subtraction.
 template <int HP>
-__device__ __forceinline__ void wht_level2(uint64_t (&p)[64], uint64_t minus1) {
+__device__ __forceinline__ void wht_level2(uint64_t (&p)[32], uint64_t minus1) {
 #pragma unroll
-  for (int k = 0; k < 32; ++k) {
+  for (int k = 0; k < 16; ++k) {
     const int j = ((k / HP) * 2 * HP) + (k % HP);
     const uint64_t a = p[j], b = p[j + HP];
     p[j] = add2(a, b);
@@ -398,35 +406,44 @@ __device__ __forceinline__ void wht_level2(uint64_t (&p)[64], uint64_t minus1) {
 
 __device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
-// K of the lane's token from its shared-memory row: 16 code words, 4 scale bytes; false if any decision is unsafe.
-__device__ __forceinline__ bool bulk_encode_k(uint32_t tile, int lane, float c_k, uint32_t (&codes)[16], uint32_t& scale_word) {
-  uint64_t p[64];                                        // p[i] = {x[2i], x[2i+1]}
-  const uint32_t row = tile + 128 * lane, sw = (uint32_t)(lane & 7);
-  float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;          // sum |x_i|: four chains
+// K of one token by the two lanes t and t + 16: lane t + 16 hf holds channels 64 hf .. 64 hf + 63 (row t of channel
+// half hf of the tile, two whole scale groups).  Returns the lane's 8 code words and 2 scale bytes; false if any of
+// ITS decisions is unsafe.
+__device__ __forceinline__ bool bulk_encode_k(uint32_t tile, int lane, float c_k, uint32_t (&codes)[8], uint32_t& scale_half) {
+  const int t = lane & 15, hf = lane >> 4;
+  const uint32_t row = tile + kBulkHalf * hf + 128 * t, sw = (uint32_t)(t & 7);
+  uint32_t mine[32];
 #pragma unroll
-  for (int j = 0; j < 16; ++j) {
-    uint4 w;
-    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w)
-                 : "r"(row + kBulkHalf * (j >> 3) + ((((uint32_t)j & 7u) ^ sw) << 4)));
-    const uint32_t ww[4] = {w.x, w.y, w.z, w.w};
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {                        // first butterfly level (index bit 0) while unpacking
-      const float a = __uint_as_float(ww[i] << 16), b = __uint_as_float(ww[i] & 0xFFFF0000u);
-      if (i & 1) { s2 += fabsf(a); s3 += fabsf(b); } else { s0 += fabsf(a); s1 += fabsf(b); }
-      p[4 * j + i] = pack2(__fadd_rn(a, b), __fsub_rn(a, b));
-    }
+  for (int j = 0; j < 8; ++j) {
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(mine[4 * j]), "=r"(mine[4 * j + 1]), "=r"(mine[4 * j + 2]),
+                 "=r"(mine[4 * j + 3]) : "r"(row + ((((uint32_t)j) ^ sw) << 4)));
   }
-  const float S = (s0 + s1) + (s2 + s3);
-  // the other six levels, one rounding per output and level (the bound kBound is for exactly this)
+  // index bit 6 (the other channel half lives in lane ^ 16) on the packed bf16 words, then index bit 0 while
+  // unpacking: x = lower half + upper half in lanes 0-15, lower - upper in lanes 16-31
+  uint64_t p[32];                                        // p[i] = {x[2i], x[2i+1]} of this lane's 64 channels
+  const float sgn = hf ? -1.0f : 1.0f;
+  float s0 = 0.f, s1 = 0.f;                              // sum |x_i| over this lane's inputs: two chains
+#pragma unroll
+  for (int i = 0; i < 32; ++i) {
+    const uint32_t oth = __shfl_xor_sync(kFull, mine[i], 16);
+    const float ma = __uint_as_float(mine[i] << 16), mb = __uint_as_float(mine[i] & 0xFFFF0000u);
+    const float oa = __uint_as_float(oth << 16), ob = __uint_as_float(oth & 0xFFFF0000u);
+    s0 += fabsf(ma); s1 += fabsf(mb);
+    const float a = __fmaf_rn(ma, sgn, oa), b = __fmaf_rn(mb, sgn, ob);   // exact product: one rounding each
+    p[i] = pack2(__fadd_rn(a, b), __fsub_rn(a, b));
+  }
+  float S = s0 + s1;
+  S += __shfl_xor_sync(kFull, S, 16);                    // the token's 128 inputs
+  // the other five levels, one rounding per output and level (the bound kBound is for exactly this: seven levels)
   const uint64_t minus1 = pack2(-1.0f, -1.0f);
-  wht_level2<1>(p, minus1); wht_level2<2>(p, minus1); wht_level2<4>(p, minus1);
-  wht_level2<8>(p, minus1); wht_level2<16>(p, minus1); wht_level2<32>(p, minus1);
+  wht_level2<1>(p, minus1); wht_level2<2>(p, minus1); wht_level2<4>(p, minus1); wht_level2<8>(p, minus1);
+  wht_level2<16>(p, minus1);
   const float kappa = 0x1.6a09e6p-4f;                    // float32 nearest to 2^-3.5
   const float eps = __fmul_rn(S, kBound);
   bool ok = (S > 1e-30f) && (S < 1e30f);
-  scale_word = 0u;
+  scale_half = 0u;
 #pragma unroll
-  for (int g = 0; g < 4; ++g) {
+  for (int g = 0; g < 2; ++g) {
     float m = 0.f;
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
@@ -439,7 +456,7 @@ __device__ __forceinline__ bool bulk_encode_k(uint32_t tile, int lane, float c_k
     const bool okg = scale_exponent_f32(c_k, m, eps, E) && (E >= -100) && (E <= 100);
     ok = ok && okg;
     if (!okg) E = 0;
-    scale_word |= (uint32_t)(E + 127) << (8 * g);
+    scale_half |= (uint32_t)(E + 127) << (8 * g);
     const float sc = pow2_neg(E);
     const float ksc = __fmul_rn(kappa, sc);              // exact: fl(x kappa) 2^-E = fl(x (kappa 2^-E))
     const float er = __fmaf_rn(__fmul_rn(eps, sc), 1.0001f, 1.2e-6f);   // + the rounding of the two additions below
@@ -462,7 +479,7 @@ __device__ __forceinline__ bool bulk_encode_k(uint32_t tile, int lane, float c_k
   return ok;
 }
 
-__global__ void __launch_bounds__(32 * kBulkWarps, 3)
+__global__ void __launch_bounds__(32 * kBulkWarps, UQ_BULK_CTAS)
 append_bulk_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_constant__ CUtensorMap tmap_v,
                    const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v_new,
                    const int32_t* __restrict__ cu_new, const int32_t* __restrict__ seq_lens,
@@ -474,37 +491,26 @@ append_bulk_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_cons
   pdl_wait();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int u = (int)blockIdx.x * kBulkWarps + warp, h = (int)blockIdx.y;
-  const int n_units = (total_new >> 5) + 2 * batch;
+  const int n_units = (total_new >> 4) + 2 * batch;
   if (u >= n_units) return;                            // warps are independent: no CTA-wide barrier below
-  const int b = find_sequence<5>(cu_new, batch, u, n_units, lane);
+  const int b = find_sequence<4>(cu_new, batch, u, n_units, lane);
   const int c0 = cu_new[b], cnt = cu_new[b + 1] - c0, p0 = seq_lens[b];
-  const int q0 = ((p0 >> 5) + (u - ((c0 >> 5) + 2 * b))) << 5;      // first position of this unit's block of 32
-  const int t_lo = max(p0, q0), t_hi = min(p0 + cnt, q0 + 32);      // the call's positions inside the block
+  const int q0 = ((p0 >> 4) + (u - ((c0 >> 4) + 2 * b))) << 4;      // first position of this unit's page
+  const int t_lo = max(p0, q0), t_hi = min(p0 + cnt, q0 + 16);      // the call's positions inside the page
   if (t_lo >= t_hi) return;
-  const int32_t* bt = block_tables + (long long)b * max_pages + (q0 >> 4);
+  const bool whole = (t_hi - t_lo == 16);
 
-  if (t_hi - t_lo < 32) {                              // head / tail of a sequence's range: octet by octet
-    for (int o = 0; o < 4; ++o) {
-      const int qo = q0 + 8 * o, lo = max(t_lo, qo), hi = min(t_hi, qo + 8);
-      if (lo >= hi) continue;
-      uint8_t* rec = cache + ((long long)bt[o >> 1] * Hkv + h) * kRecordBytes;
-      append_octet(k_new, v_new, rec, c0, p0, qo, lo, hi, h, Hkv, lane, c_k, c_v);
-      __syncwarp();
-    }
-    return;
-  }
-
-  // ---------------- whole block: rows -> shared memory
+  // ---------------- whole page: rows -> shared memory (issued before the page lookup)
   const uint32_t sbase = (smem_addr(bulk_smem) + 1023u) & ~1023u;
-  const uint32_t sK = sbase + warp * kBulkTiles, sV = sK + 2 * kBulkHalf, sM = sbase + kBulkWarps * kBulkTiles + 512 * warp;
+  const uint32_t sK = sbase + warp * kBulkTiles, sV = sK + 2 * kBulkHalf, sM = sbase + kBulkWarps * kBulkTiles + 256 * warp;
   const uint32_t barK = smem_addr(&bars[warp][0]), barV = barK + 8;
-  if (lane == 0) {
+  if (whole && lane == 0) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(barK));
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(barV));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(barK), "r"(2 * kBulkHalf) : "memory");
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(barV), "r"(2 * kBulkHalf) : "memory");
-    const int row0 = c0 + (q0 - p0);                   // k_new / v_new row of the block's first token
+    const int row0 = c0 + (q0 - p0);                   // k_new / v_new row of the page's first token
 #pragma unroll
     for (int hf = 0; hf < 2; ++hf) {
       asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
@@ -517,43 +523,57 @@ append_bulk_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_cons
     }
   }
   __syncwarp();
-  const int page = bt[lane >> 4];                      // lanes 0-15: first page of the block, 16-31: second
+  const int page = block_tables[(long long)b * max_pages + (q0 >> 4)];
   uint8_t* const rec = cache + ((long long)page * Hkv + h) * kRecordBytes;
-  const int t = lane & 15;                             // this lane's slot in its page
+
+  if (!whole) {                                        // head / tail of a sequence's range: octet by octet
+    for (int o = 0; o < 2; ++o) {
+      const int qo = q0 + 8 * o, lo = max(t_lo, qo), hi = min(t_hi, qo + 8);
+      if (lo >= hi) continue;
+      append_octet(k_new, v_new, rec, c0, p0, qo, lo, hi, h, Hkv, lane, c_k, c_v);
+      __syncwarp();
+    }
+    return;
+  }
+
+  const int t = lane & 15, hf = lane >> 4;             // this lane's token slot and channel half
   auto wait = [](uint32_t bar) {
     asm volatile("{\n.reg .pred p;\nW_%=:\nmbarrier.try_wait.parity.shared::cta.b64 p, [%0], 0;\n@p bra D_%=;\nbra W_%=;\nD_%=:\n}\n"
                  ::"r"(bar) : "memory");
   };
 
-  // ---------------- K: lane = token
+  // ---------------- K: lanes t and t + 16 = token t
   wait(barK);
   unsigned bad_k;
   {
-    uint32_t codes[16], scale_word;
-    const bool ok = bulk_encode_k(sK, lane, (float)c_k, codes, scale_word);
-    if (ok) {
-      uint4* dst = reinterpret_cast<uint4*>(rec + kOffKCodes + 64 * t);
-#pragma unroll
-      for (int j = 0; j < 4; ++j) dst[j] = make_uint4(codes[4 * j], codes[4 * j + 1], codes[4 * j + 2], codes[4 * j + 3]);
-      *reinterpret_cast<uint32_t*>(rec + kOffKScales + 4 * t) = scale_word;
-    }
+    uint32_t codes[8], scale_half;
+    const bool ok = bulk_encode_k(sK, lane, (float)c_k, codes, scale_half);
     bad_k = __ballot_sync(kFull, !ok);
+    bad_k = (bad_k | (bad_k >> 16)) & 0xFFFFu;         // tokens with an undecided half
+    if (!((bad_k >> t) & 1u)) {
+      uint4* dst = reinterpret_cast<uint4*>(rec + kOffKCodes + 64 * t + 32 * hf);
+      dst[0] = make_uint4(codes[0], codes[1], codes[2], codes[3]);
+      dst[1] = make_uint4(codes[4], codes[5], codes[6], codes[7]);
+      *reinterpret_cast<uint16_t*>(rec + kOffKScales + 4 * t + 2 * hf) = (uint16_t)scale_half;
+    }
   }
 
-  // ---------------- V pass 1: lane = token
+  // ---------------- V pass 1: lane = (token, channel half): two groups
   wait(barV);
   unsigned bad_v;
   {
-    const uint32_t vrow = sV + 128 * lane, sw = (uint32_t)(lane & 7);
+    const uint32_t vrow = sV + kBulkHalf * hf + 128 * t, sw = (uint32_t)(t & 7);
     bool ok = true;
-    float mult[4];
+    float mult[2];
+    uint32_t bytes = 0u;
 #pragma unroll
-    for (int g = 0; g < 4; ++g) {
+    for (int gg = 0; gg < 2; ++gg) {
       uint32_t mx = 0u;
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
         uint4 w;
-        asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "r"(vrow + kBulkHalf * (g >> 1) + ((((uint32_t)(4 * (g & 1) + j)) ^ sw) << 4)));
+        asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w)
+                     : "r"(vrow + ((((uint32_t)(4 * gg + j)) ^ sw) << 4)));
         mx = __vmaxu2(mx, __vmaxu2(__vmaxu2(w.x & 0x7FFF7FFFu, w.y & 0x7FFF7FFFu), __vmaxu2(w.z & 0x7FFF7FFFu, w.w & 0x7FFF7FFFu)));
       }
       const float m = __uint_as_float(max(mx >> 16, mx & 0xFFFFu) << 16);   // bf16 magnitudes order like their bits
@@ -561,19 +581,25 @@ append_bulk_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_cons
       const bool zero = (m == 0.0f);
       const bool okg = zero || (scale_exponent_f32((float)c_v, m, 0.0f, E) && (E >= -100) && (E <= 100));
       ok = ok && okg;
-      mult[g] = (okg && !zero) ? pow2_neg(E) : 1.0f;
-      if (zero) E = -127;
-      if (okg) rec[kOffVScales + 32 * (t >> 3) + 8 * g + (t & 7)] = (uint8_t)(E + 127);
+      mult[gg] = (okg && !zero) ? pow2_neg(E) : 1.0f;
+      if (zero || !okg) E = -127;
+      bytes |= (uint32_t)(E + 127) << (8 * gg);
     }
-    asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(sM + 16 * lane), "f"(mult[0]), "f"(mult[1]), "f"(mult[2]), "f"(mult[3]) : "memory");
+    asm volatile("st.shared.v2.f32 [%0], {%1,%2};" ::"r"(sM + 16 * t + 8 * hf), "f"(mult[0]), "f"(mult[1]) : "memory");
     bad_v = __ballot_sync(kFull, !ok);
+    bad_v = (bad_v | (bad_v >> 16)) & 0xFFFFu;
+    if (!((bad_v >> t) & 1u)) {                          // group g = 2 hf + gg of token t: byte 32 (t >> 3) + 8 g + (t & 7)
+      uint8_t* sb = rec + kOffVScales + 32 * (t >> 3) + 16 * hf + (t & 7);
+      sb[0] = (uint8_t)(bytes & 0xFFu);
+      sb[8] = (uint8_t)(bytes >> 8);
+    }
   }
   __syncwarp();
 
   // ---------------- V pass 2: lane = channels 4 lane .. 4 lane + 3 (group lane >> 3), an octet of tokens per word
   const uint32_t vsrc = sV + kBulkHalf * (lane >> 4) + 8 * (lane & 1), vchunk = (uint32_t)((lane & 15) >> 1);
-#pragma unroll 1
-  for (int o = 0; o < 4; ++o) {
+#pragma unroll
+  for (int o = 0; o < 2; ++o) {
     float r[4][8];
 #pragma unroll
     for (int tt = 0; tt < 8; ++tt) {
@@ -591,9 +617,7 @@ append_bulk_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_cons
 #pragma unroll
     for (int c = 0; c < 4; ++c)
       vw[c] = canon_e2m1x8(e2m1x8(r[c][0], r[c][1], r[c][2], r[c][3], r[c][4], r[c][5], r[c][6], r[c][7]));
-    const int pg = __shfl_sync(kFull, page, 16 * (o >> 1));
-    uint8_t* const rec_o = cache + ((long long)pg * Hkv + h) * kRecordBytes;
-    *reinterpret_cast<uint4*>(rec_o + kOffVCodes + 512 * (o & 1) + 16 * lane) = make_uint4(vw[0], vw[1], vw[2], vw[3]);
+    *reinterpret_cast<uint4*>(rec + kOffVCodes + 512 * o + 16 * lane) = make_uint4(vw[0], vw[1], vw[2], vw[3]);
   }
 
   // ---------------- vectors the float32 intervals could not decide: the whole warp, float64
@@ -602,23 +626,21 @@ append_bulk_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_cons
     while (bad_k) {
       const int tk = __ffs(bad_k) - 1;
       bad_k &= bad_k - 1;
-      const int pg = __shfl_sync(kFull, page, tk);
       const long long rw = ((long long)(c0 + (q0 - p0) + tk) * Hkv + h) * kHeadDim;
-      store_k(k_new + rw, cache + ((long long)pg * Hkv + h) * kRecordBytes, tk & 15, lane, c_k);
+      store_k(k_new + rw, rec, tk, lane, c_k);
     }
     while (bad_v) {
       const int tv = __ffs(bad_v) - 1;
       bad_v &= bad_v - 1;
-      const int pg = __shfl_sync(kFull, page, tv);
       const int pos = q0 + tv;
-      append_octet_v(v_new, cache + ((long long)pg * Hkv + h) * kRecordBytes, c0, p0, pos & ~7, pos, h, Hkv, lane, c_v);
+      append_octet_v(v_new, rec, c0, p0, pos & ~7, pos, h, Hkv, lane, c_v);
       __syncwarp();
     }
   }
 }
 
-// 2-D TMA view of k_new / v_new: [rows][kv heads x 128] bf16; box = 32 rows x 64 channels (128 B: the widest row the
-// 128-byte swizzle takes), so a block's K (or V) rows of one kv head are two tensor copies.
+// 2-D TMA view of k_new / v_new: [rows][kv heads x 128] bf16; box = 16 rows x 64 channels (128 B: the widest row the
+// 128-byte swizzle takes), so a page's K (or V) rows of one kv head are two tensor copies.
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -636,7 +658,7 @@ int32_t rows_map(const void* rows, long long n_rows, int Hkv, CUtensorMap* out) 
   }
   const cuuint64_t gdim[2] = {(cuuint64_t)Hkv * kHeadDim, (cuuint64_t)n_rows};
   const cuuint64_t gstr[1] = {(cuuint64_t)Hkv * kHeadDim * 2};
-  const cuuint32_t box[2] = {64, 32};
+  const cuuint32_t box[2] = {64, 16};
   const cuuint32_t estr[2] = {1, 1};
   const CUresult cr = encode(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(rows), gdim, gstr, box, estr,
                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -680,7 +702,7 @@ extern "C" int32_t uq_rotate_quantize_append(const uq_config* cfg, const void* k
   const long long q_rows = q ? (long long)batch * cfg->num_q_heads : 0;
   if (total_new == 0 && q_rows == 0) return UQ_OK;
   // Prefill-sized calls (on average 64 or more new tokens per sequence): K/V through append_bulk_kernel, one warp per
-  // aligned block of 32 positions; the kernel below then only encodes the query rows.  Same bytes either way.
+  // page; the kernel below then only encodes the query rows.  Same bytes either way.
   if (total_new >= 1024 && (long long)total_new >= 64LL * batch && !(((uintptr_t)k_new | (uintptr_t)v_new) & 15u) &&
       !(cfg->flags & UQ_FLAG_NO_BULK_APPEND)) {
     static bool attr_set = false;
@@ -693,7 +715,7 @@ extern "C" int32_t uq_rotate_quantize_append(const uq_config* cfg, const void* k
     st = rows_map(k_new, total_new, cfg->num_kv_heads, &tmap_k);
     if (st == UQ_OK) st = rows_map(v_new, total_new, cfg->num_kv_heads, &tmap_v);
     if (st != UQ_OK) return st;
-    const long long n_units = (long long)(total_new >> 5) + 2LL * batch;
+    const long long n_units = (long long)(total_new >> 4) + 2LL * batch;
     const long long bx = (n_units + kBulkWarps - 1) / kBulkWarps;
     if (bx > 0x7fffffffLL) {
       set_error("append: too many work units");
