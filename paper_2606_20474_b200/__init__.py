@@ -12,6 +12,7 @@ from .binding import (  # noqa: F401
     RECORD_BYTES,
     StepBuffers,
     HostStage,
+    HostStepGraph,
     alloc_cache,
     cache_record_bytes,
     calibrate_c,

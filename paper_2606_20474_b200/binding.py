@@ -249,3 +249,22 @@ def decode_step_host(cfg: UQConfig, bufs: StepBuffers, stage: HostStage, cache, 
                       dv["seq_lens_after"], dv["block_tables"], cache, stream=stream)
     out_host.copy_(out, non_blocking=True)
     return out_host
+
+
+class HostStepGraph:
+    """decode_step_host captured once as a CUDA graph — the host->device copy of the staged inputs, the three kernels
+    (their programmatic-launch edges are kept by the capture) and the device->host copy of O — so that a step costs
+    the host one graph launch.  All addresses are those of `stage`, `bufs`, `cache` and `out_host`: the caller
+    rewrites `stage.h[...]` between launches.  `launch()` enqueues on the current stream."""
+
+    def __init__(self, cfg: UQConfig, bufs: StepBuffers, stage: HostStage, cache, out_host):
+        decode_step_host(cfg, bufs, stage, cache, out_host)          # first-call set-up happens outside the capture
+        torch.cuda.current_stream().synchronize()
+        self.graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(self.graph):                           # torch's capture stream becomes the current one
+            decode_step_host(cfg, bufs, stage, cache, out_host)
+        self.out_host = out_host
+
+    def launch(self) -> torch.Tensor:
+        self.graph.replay()
+        return self.out_host

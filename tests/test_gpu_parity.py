@@ -262,13 +262,17 @@ def test_host_staged_step_equals_device_step_and_oracle():
     B = wl.batch
     lens0 = (wl.ctx_lens - steps).astype(np.int32)
     caches = []
-    for _ in range(2):
+    for _ in range(3):
         cache, bt = H.fill_cache(cfg, wl, DEV, lens=lens0)
         caches.append(cache)
-    bufs = [uq.StepBuffers(cfg, B, 3, DEV) for _ in range(2)]
+    bufs = [uq.StepBuffers(cfg, B, 3, DEV) for _ in range(3)]
     cu = torch.arange(B + 1, dtype=torch.int32, device=DEV)
     stage = uq.HostStage(cfg, B, B, int(bt.shape[1]), DEV)
     out_host = torch.empty((B, wl.num_q_heads, 128), dtype=torch.bfloat16).pin_memory()
+    # the same step as a CUDA graph (HostStepGraph) on a third cache: its own staging block and output
+    stage_g = uq.HostStage(cfg, B, B, int(bt.shape[1]), DEV)
+    out_host_g = torch.empty((B, wl.num_q_heads, 128), dtype=torch.bfloat16).pin_memory()
+    graph = None
     for s in range(steps):
         before = lens0 + s
         q = W.gen_q(wl, DEV, step=s)
@@ -283,7 +287,16 @@ def test_host_staged_step_equals_device_step_and_oracle():
         uq.decode_step_host(cfg, bufs[1], stage, caches[1], out_host)
         torch.cuda.synchronize()
         assert torch.equal(out_host.view(torch.int16), ref_out.cpu().view(torch.int16)), f"step {s}"
+        for name in uq.HostStage.FIELDS:
+            stage_g.h[name].copy_(stage.h[name])
+        if graph is None:                                   # captured with the first step's inputs in the block
+            graph = uq.HostStepGraph(cfg, bufs[2], stage_g, caches[2], out_host_g)
+        out_host_g.zero_()
+        graph.launch()
+        torch.cuda.synchronize()
+        assert torch.equal(out_host_g.view(torch.int16), ref_out.cpu().view(torch.int16)), f"graph step {s}"
     assert torch.equal(caches[0], caches[1])
+    assert torch.equal(caches[0], caches[2])
     for b in range(B):
         ref, _ = H.oracle_out(wl, b, int(wl.ctx_lens[b]), H.bits(q)[b])
         H.check_out(out_host[b].float().numpy().astype(np.float64), ref, f"staged seq {b}")
