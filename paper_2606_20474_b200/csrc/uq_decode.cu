@@ -99,24 +99,10 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-// A thread suspended in a plain mbarrier.try_wait was observed (clock64 trace) to sleep ~2.5k cycles
-// past a tcgen05.commit arrival before it resumed, and a pure test_wait spin steals issue slots from
-// the working warps; so waits use try_wait with a short suspend-time hint.
-#ifndef UQ_WAIT_NS
-#define UQ_WAIT_NS -1
-#endif
-__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {   // one non-blocking probe
-  uint32_t ok;
-  asm volatile("{\n.reg .pred p;\nmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
-               : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-  return ok != 0;
-}
+// Waits are a plain mbarrier.try_wait loop (the hardware suspends the thread for a bounded time per probe).
+// Measured and dropped on config 2: test_wait spin loops (157-161 us: the spin steals issue slots from the working
+// warps), nanosleep polling and suspend-time hints in the softmax warps (no change).
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-#if UQ_WAIT_NS > 0
-  while (!mbar_test(bar, parity)) asm volatile("nanosleep.u32 %0;" ::"r"((uint32_t)UQ_WAIT_NS));
-#elif UQ_WAIT_NS == 0
-  while (!mbar_test(bar, parity)) {}
-#else
   asm volatile(
       "{\n"
       ".reg .pred p;\n"
@@ -126,34 +112,6 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "bra WAIT_%=;\n"
       "DONE_%=:\n"
       "}\n" ::"r"(bar), "r"(parity) : "memory");
-#endif
-}
-// try_wait with a suspend-time hint (ns): for waiters that are known to wait long (the softmax warps wait
-// for the V warps most of the time) — fewer wake-ups, fewer issue slots taken from the working warps
-__device__ __forceinline__ void mbar_wait_hint(uint32_t bar, uint32_t parity, uint32_t ns) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "WAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
-      "@p bra DONE_%=;\n"
-      "bra WAIT_%=;\n"
-      "DONE_%=:\n"
-      "}\n" ::"r"(bar), "r"(parity), "r"(ns) : "memory");
-}
-#ifndef UQ_A_WAIT_NS
-#define UQ_A_WAIT_NS 0
-#endif
-#ifndef UQ_SPIN_NS
-#define UQ_SPIN_NS 32
-#endif
-__device__ __forceinline__ void spin_pause() {
-#if UQ_SPIN_NS > 0
-  asm volatile("nanosleep.u32 %0;" ::"r"((uint32_t)UQ_SPIN_NS));
-#endif
-}
-__device__ __forceinline__ void mbar_wait_spin(uint32_t bar, uint32_t parity) {   // for the single-warp issuers
-  while (!mbar_test(bar, parity)) spin_pause();
 }
 // The KV stream is read once: L2 evict-first keeps it from flushing everything else (the kernel's own
 // instructions included) out of L2.
@@ -221,12 +179,6 @@ __device__ __forceinline__ void umma_mxf8f6f4(uint32_t d, uint64_t da, uint64_t 
       "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
       "tcgen05.mma.cta_group::1.kind::mxf8f6f4.block_scale [%0], %1, %2, %3, [%5], [%6], p;\n}\n"
       ::"r"(d), "l"(da), "l"(db), "r"(idesc), "r"(acc), "r"(tsfa), "r"(tsfb) : "memory");
-}
-__device__ __forceinline__ void umma_f16(uint32_t d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t acc) {
-  asm volatile(
-      "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}\n"
-      ::"r"(d), "l"(da), "l"(db), "r"(idesc), "r"(acc) : "memory");
 }
 // N consecutive 32-bit columns of this thread's TMEM lane <-> registers (N = 8 or 16), complete on return
 template <int N>
@@ -705,13 +657,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
             const uint32_t t_s = tmem + lane_sel + kColS + 16 * sb;
             const uint32_t p_addr = p_row + kPBytes * sb;
 
-#if defined(UQ_A_SLEEP_NS)
-            while (!mbar_test(bar_sfull + 8 * sb, ph2)) asm volatile("nanosleep.u32 %0;" ::"r"((uint32_t)UQ_A_SLEEP_NS));
-#elif UQ_A_WAIT_NS > 0
-            mbar_wait_hint(bar_sfull + 8 * sb, ph2, UQ_A_WAIT_NS);
-#else
             mbar_wait(bar_sfull + 8 * sb, ph2);        // S(gt) is in TMEM
-#endif
             if (gt >= 2) mbar_wait(bar_done + 8 * sb, ph2 ^ 1);   // PV(gt-2) has read P buffer gt&1 (the PV warp commits
                                                                    // once per tile: its issue stream bounds the tile period)
             tc_fence_after();
