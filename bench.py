@@ -494,7 +494,7 @@ def run_bulk_append(args):
             "roofline": {"bound": "hbm", "kernel": "uq::append_bulk_kernel", "achieved": round(gbs, 1), "peak": peak,
                          "unit": "GB/s", "frac": round(gbs / peak, 4),
                          # dram__bytes_read.sum + write.sum of the ncu capture in profiles/r01_append_bulk_cfg2.md
-                         "traffic": 662710272 if (args.config, n, nseq) == (2, 32768, 8) else None,
+                         "traffic": 662109440 if (args.config, n, nseq) == (2, 32768, 8) else None,
                          "algorithmic_bytes": nbytes, "peak_source": peak_src}}
 
 

@@ -324,9 +324,9 @@ append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v
 // a third of them shuffles and lane bookkeeping.  Here a warp takes one page (16 aligned positions) of one kv head,
 // stages its K and V rows in shared memory with four TMA tensor copies (k_new / v_new seen as
 // [rows][kv heads x 128] bf16, box 16 rows x 64 channels, completion on an mbarrier) and works in two thread mappings:
-//   K      lanes t and t + 16 = token t, 64 channels (two whole scale groups) each: the butterfly level between the
-//          two halves is a shuffle of the packed bf16 words, the other six are in-register add/sub pairs on packed
-//          float32 pairs; the same float32 error-interval test as the fast path above decides every scale exponent
+//   K      lanes t and t + 16 = token t, 64 channels (two whole scale groups) each: six butterfly levels are
+//          in-register add/sub pairs (five of them on packed float32 pairs), the level between the two halves is a
+//          shuffle of those pairs; the same float32 error-interval test as the fast path above decides every scale exponent
 //          and code; 32 B of codes and two scale bytes are stored per lane;
 //   V      pass 1, lane = (token, channel half): group maxima by packed 16-bit integer maxima of the bf16
 //          magnitudes -> scale exponent, scale bytes, and the power-of-two multipliers left in shared memory;
@@ -336,7 +336,7 @@ append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v
 // append_octet_v (float64), after the fast lanes have stored; a page that the call covers only partly goes through
 // append_octet octet by octet.  The bytes written are those of the kernel above in every case.
 // (First version: a block of 32 positions per warp, lane = token with all 128 channels in registers — 78 instead
-// of 96 instructions per vector but 168 registers, 11 warps per SM; this one runs 20 warps per SM and is 2-8 %
+// of 90 instructions per vector but 168 registers, 11 warps per SM; this one runs 20 warps per SM and is 2-8 %
 // faster, profiles/r01_append_bulk_cfg2.md.)
 constexpr int kBulkWarps = 4;
 #ifndef UQ_BULK_CTAS
@@ -418,26 +418,32 @@ __device__ __forceinline__ bool bulk_encode_k(uint32_t tile, int lane, float c_k
     asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(mine[4 * j]), "=r"(mine[4 * j + 1]), "=r"(mine[4 * j + 2]),
                  "=r"(mine[4 * j + 3]) : "r"(row + ((((uint32_t)j) ^ sw) << 4)));
   }
-  // index bit 6 (the other channel half lives in lane ^ 16) on the packed bf16 words, then index bit 0 while
-  // unpacking: x = lower half + upper half in lanes 0-15, lower - upper in lanes 16-31
+  // index bit 0 while unpacking, bits 1-5 on packed pairs in the lane, bit 6 (the other channel half lives in lane ^ 16)
+  // last: x = lower + upper in lanes 0-15, lower - upper in lanes 16-31.  One rounding per output and level in any
+  // order of the levels (the bound kBound is for exactly this: seven levels).
   uint64_t p[32];                                        // p[i] = {x[2i], x[2i+1]} of this lane's 64 channels
-  const float sgn = hf ? -1.0f : 1.0f;
   float s0 = 0.f, s1 = 0.f;                              // sum |x_i| over this lane's inputs: two chains
 #pragma unroll
   for (int i = 0; i < 32; ++i) {
-    const uint32_t oth = __shfl_xor_sync(kFull, mine[i], 16);
-    const float ma = __uint_as_float(mine[i] << 16), mb = __uint_as_float(mine[i] & 0xFFFF0000u);
-    const float oa = __uint_as_float(oth << 16), ob = __uint_as_float(oth & 0xFFFF0000u);
-    s0 += fabsf(ma); s1 += fabsf(mb);
-    const float a = __fmaf_rn(ma, sgn, oa), b = __fmaf_rn(mb, sgn, ob);   // exact product: one rounding each
+    const float a = __uint_as_float(mine[i] << 16), b = __uint_as_float(mine[i] & 0xFFFF0000u);
+    s0 += fabsf(a); s1 += fabsf(b);
     p[i] = pack2(__fadd_rn(a, b), __fsub_rn(a, b));
   }
   float S = s0 + s1;
   S += __shfl_xor_sync(kFull, S, 16);                    // the token's 128 inputs
-  // the other five levels, one rounding per output and level (the bound kBound is for exactly this: seven levels)
   const uint64_t minus1 = pack2(-1.0f, -1.0f);
   wht_level2<1>(p, minus1); wht_level2<2>(p, minus1); wht_level2<4>(p, minus1); wht_level2<8>(p, minus1);
   wht_level2<16>(p, minus1);
+  {
+    const float sgn = hf ? -1.0f : 1.0f;
+    const uint64_t sgn2 = pack2(sgn, sgn);
+#pragma unroll
+    for (int i = 0; i < 32; ++i) {
+      const uint32_t lo = (uint32_t)p[i], hi = (uint32_t)(p[i] >> 32);
+      const uint64_t oth = (uint64_t)__shfl_xor_sync(kFull, lo, 16) | ((uint64_t)__shfl_xor_sync(kFull, hi, 16) << 32);
+      p[i] = fma2(p[i], sgn2, oth);                      // exact product: one rounding
+    }
+  }
   const float kappa = 0x1.6a09e6p-4f;                    // float32 nearest to 2^-3.5
   const float eps = __fmul_rn(S, kBound);
   bool ok = (S > 1e-30f) && (S < 1e30f);
