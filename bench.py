@@ -214,7 +214,15 @@ def run_ours(args, rank, world, local_rank):
     after_dev = torch.from_numpy(ctx_after).to(dev)
     stream = torch.cuda.current_stream()
 
+    # one CUDA graph per entry of the input ring (uq.StepGraph: the step's three kernels, one launch for the host)
+    step_graphs = None
+    if args.graph:
+        step_graphs = [uq.StepGraph(cfg, bufs, qs[j], kvs[j][0], kvs[j][1], cu_dev, before_dev, after_dev, bt_dev, cache)
+                       for j in range(n_in)]
+
     def step(i):
+        if step_graphs is not None:
+            return step_graphs[i % n_in].launch()
         k_new, v_new = kvs[i % n_in]
         return uq.decode_step(cfg, bufs, qs[i % n_in], k_new, v_new, cu_dev, before_dev, after_dev,
                               bt_dev, cache, stream=stream)
@@ -556,6 +564,8 @@ def main():
                     help="BASELINE.json config number (1-based); 2 is the one the metric is quoted on")
     ap.add_argument("--splits", type=int, default=0, help="num_splits override (0 = uq_suggest_num_splits)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--graph", type=int, default=0, choices=[0, 1],
+                    help="1: the timed steps are launches of uq.StepGraph (one CUDA graph per step)")
     ap.add_argument("--bulk-seqs", type=int, default=1, metavar="S",
                     help="with --bulk-append: sequences that receive TOKENS new tokens each in one call")
     ap.add_argument("--bulk-append", type=int, default=0, metavar="TOKENS",

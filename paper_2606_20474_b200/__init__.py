@@ -11,6 +11,7 @@ from .binding import (  # noqa: F401
     UQError,
     RECORD_BYTES,
     StepBuffers,
+    StepGraph,
     HostStage,
     HostStepGraph,
     alloc_cache,

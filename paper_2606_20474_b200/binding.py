@@ -251,6 +251,27 @@ def decode_step_host(cfg: UQConfig, bufs: StepBuffers, stage: HostStage, cache, 
     return out_host
 
 
+class StepGraph:
+    """decode_step on device-resident inputs captured once as a CUDA graph (the three kernels with their
+    programmatic-launch edges): a step costs the host one graph launch — what matters when the step is short
+    (config 1: three launches from Python take longer than the kernels).  All addresses are those of the tensors
+    given here: the caller rewrites them in place between launches.  The constructor runs the step once."""
+
+    def __init__(self, cfg: UQConfig, bufs: StepBuffers, q, k_new, v_new, cu_new, seq_lens_before, seq_lens_after,
+                 block_tables, cache):
+        args = (cfg, bufs, q, k_new, v_new, cu_new, seq_lens_before, seq_lens_after, block_tables, cache)
+        decode_step(*args)                                           # first-call set-up happens outside the capture
+        torch.cuda.current_stream().synchronize()
+        self.graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(self.graph):
+            decode_step(*args)
+        self.out = bufs.out
+
+    def launch(self) -> torch.Tensor:
+        self.graph.replay()
+        return self.out
+
+
 class HostStepGraph:
     """decode_step_host captured once as a CUDA graph — the host->device copy of the staged inputs, the three kernels
     (their programmatic-launch edges are kept by the capture) and the device->host copy of O — so that a step costs

@@ -336,7 +336,7 @@ append_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v
 // append_octet_v (float64), after the fast lanes have stored; a page that the call covers only partly goes through
 // append_octet octet by octet.  The bytes written are those of the kernel above in every case.
 // (First version: a block of 32 positions per warp, lane = token with all 128 channels in registers — 78 instead
-// of 90 instructions per vector but 168 registers, 11 warps per SM; this one runs 20 warps per SM and is 2-8 %
+// of 90 instructions per vector but 168 registers, 11 warps per SM; this one runs 20 warps per SM and is 6-10 %
 // faster, profiles/r01_append_bulk_cfg2.md.)
 constexpr int kBulkWarps = 4;
 #ifndef UQ_BULK_CTAS

@@ -302,6 +302,40 @@ def test_host_staged_step_equals_device_step_and_oracle():
         H.check_out(out_host[b].float().numpy().astype(np.float64), ref, f"staged seq {b}")
 
 
+def test_step_graph_equals_direct_calls():
+    """uq.StepGraph (decode_step captured as a CUDA graph, inputs rewritten in place between launches) gives the
+    direct calls' output bit for bit over consecutive steps, and the same cache image."""
+    steps = 3
+    wl = W.make_custom("sgraph", 23, [130, 31, 64, 1000], 16, 2, extra_tokens=steps)
+    cfg = H.cfg_of(wl)
+    B = wl.batch
+    lens0 = (wl.ctx_lens - steps).astype(np.int32)
+    (cache_a, bt), (cache_b, _) = H.fill_cache(cfg, wl, DEV, lens=lens0), H.fill_cache(cfg, wl, DEV, lens=lens0)
+    bufs_a, bufs_b = uq.StepBuffers(cfg, B, 3, DEV), uq.StepBuffers(cfg, B, 3, DEV)
+    cu = torch.arange(B + 1, dtype=torch.int32, device=DEV)
+    q_g = torch.empty((B, wl.num_q_heads, 128), dtype=torch.bfloat16, device=DEV)
+    k_g = torch.empty((B, wl.num_kv_heads, 128), dtype=torch.bfloat16, device=DEV)
+    v_g = torch.empty_like(k_g)
+    before_g = torch.empty(B, dtype=torch.int32, device=DEV)
+    after_g = torch.empty(B, dtype=torch.int32, device=DEV)
+    graph = None
+    for s_ in range(steps):
+        before = lens0 + s_
+        q = W.gen_q(wl, DEV, step=s_)
+        k = torch.cat([W.gen_kv(wl, b, int(before[b]), int(before[b]) + 1, DEV)[0] for b in range(B)])
+        v = torch.cat([W.gen_kv(wl, b, int(before[b]), int(before[b]) + 1, DEV)[1] for b in range(B)])
+        before_d, after_d = torch.from_numpy(before).to(DEV), torch.from_numpy(before + 1).to(DEV)
+        ref = uq.decode_step(cfg, bufs_a, q, k, v, cu, before_d, after_d, bt, cache_a).clone()
+        q_g.copy_(q); k_g.copy_(k); v_g.copy_(v); before_g.copy_(before_d); after_g.copy_(after_d)
+        if graph is None:
+            graph = uq.StepGraph(cfg, bufs_b, q_g, k_g, v_g, cu, before_g, after_g, bt, cache_b)
+        bufs_b.out.zero_()
+        out = graph.launch()
+        torch.cuda.synchronize()
+        assert torch.equal(out.view(torch.int16), ref.view(torch.int16)), f"step {s_}"
+    assert torch.equal(cache_a, cache_b)
+
+
 def test_append_on_rounding_boundaries_is_bit_exact():
     """The append kernel's float32 fast path must hand every close call to float64: V elements exactly on the
     E2M1 ties (0.25, 0.75, 1.25, 1.75, 2.5, 3.5, 5 times the group scale), group maxima on both sides of the
