@@ -73,7 +73,8 @@ def _load():
                                         ctypes.c_int, ctypes.c_int, ctypes.c_double, f64p]
     lib.uqo_calib_sq_err.restype = None
     lib.uqo_calib_sq_err.argtypes = [u16p, ctypes.c_int64, ctypes.c_int, ctypes.c_int,
-                                     ctypes.POINTER(ctypes.c_float), ctypes.c_int, ctypes.c_int, f64p, f64p]
+                                     ctypes.POINTER(ctypes.c_float), ctypes.c_int, ctypes.c_int,
+                                     ctypes.POINTER(ctypes.c_float), f64p, f64p]
     lib.uqo_num_threads.restype = ctypes.c_int
     lib.uqo_set_num_threads.argtypes = [ctypes.c_int]
     _lib = lib
@@ -171,18 +172,21 @@ def encode_kv(k_bits, v_bits, c_k: float = 0.156, c_v: float = 0.156):
             vc.reshape(lead + (d // 2,)), vs.reshape(lead + (d // 32,)))
 
 
-def calib_sq_err(x_bits, c_grid, rotate: bool = True, pow2: bool = True):
+def calib_sq_err(x_bits, c_grid, rotate: bool = True, pow2: bool = True, scale_mode: int | None = None, levels=None):
     """Objective of Eq.(2) on a grid of constants: x_bits uint16 bf16 patterns [n, d], c_grid
     float32 [n_c].  Returns (sq_err float64 [n_c], sq_norm float): sums over all elements of (z - zhat)^2 and
-    z^2, z rotated if `rotate`; pow2 selects the deployed power-of-two scale (Alg. 1 l.3) against s = c*m."""
+    z^2, z rotated if `rotate`.  scale_mode 0: s = c*m; 1: the deployed power-of-two scale (Alg. 1 l.3); 2: s = c
+    (no absmax); default 1 if pow2 else 0.  levels: None (E2M1) or 8 ascending magnitudes of another codebook."""
     x_bits = _c(x_bits, np.uint16)
     c_grid = _c(c_grid, np.float32)
     n, d = x_bits.shape
+    mode = (1 if pow2 else 0) if scale_mode is None else int(scale_mode)
+    lev = None if levels is None else _c(levels, np.float32)
     sq_err = np.zeros(c_grid.shape[0], np.float64)
     sq_norm = np.zeros(1, np.float64)
     _load().uqo_calib_sq_err(_ptr(x_bits, ctypes.c_uint16), n, d, int(bool(rotate)), _ptr(c_grid, ctypes.c_float),
-                             c_grid.shape[0], int(bool(pow2)), _ptr(sq_err, ctypes.c_double),
-                             _ptr(sq_norm, ctypes.c_double))
+                             c_grid.shape[0], mode, None if lev is None else _ptr(lev, ctypes.c_float),
+                             _ptr(sq_err, ctypes.c_double), _ptr(sq_norm, ctypes.c_double))
     return sq_err, float(sq_norm[0])
 
 

@@ -163,11 +163,16 @@ void uqo_encode_kv(const uint16_t* k_bf16, const uint16_t* v_bf16, int64_t n_vec
  *     sq_err[j] = sum over all elements z of (z - zhat_j(z))^2,   sq_norm = sum z^2,
  * with z the rotated vector (rotate != 0: Alg. 1 l.1) or the vector itself, m the absmax of
  * z's 32-channel group and
- *   pow2 == 0: s = c_j*m, the scale of Eq.(2) as printed; zhat = s * q(z/s), q = nearest level
- *              of F (the ladder of O5 applied to r = |z|/s);
- *   pow2 != 0: s = 2^E, E = round(log2(c_j*m)) (O4): the quantiser Alg. 1 deploys
- *              (l.3-5, :253-255) followed by Eq.(1); zhat = dequant(encode(z, E), E).
- * c_j is a float (as uq_config.c_k) used as (double)c_j.  A group with m = 0 contributes 0.
+ *   scale_mode 0: s = c_j*m, the scale of Eq.(2) as printed; zhat = s * q(z/s), q = nearest level;
+ *   scale_mode 1: s = 2^E, E = round(log2(c_j*m)) (O4): the quantiser Alg. 1 deploys
+ *                 (l.3-5, :253-255) followed by Eq.(1); zhat = dequant(encode(z, E), E);
+ *   scale_mode 2: s = c_j, no absmax: a fixed grid for vectors of known norm (the per-token
+ *                 l2-norm schemes the paper compares with, :116-120 and Fig. 2).
+ * Levels: levels == NULL -> F = {0,.5,1,1.5,2,3,4,6} with the tie rule of O5 (the only choice
+ * for scale_mode 1); else 8 ascending magnitudes L_0..L_7 of a symmetric 15/16-level codebook
+ * (uniform INT4: 0..7; Lloyd-Max centroids: Fig. 2a), q(r) = the L_i nearest to r, a tie going
+ * to the smaller one (the squared error of a tie does not depend on the choice).
+ * c_j is a float (as uq_config.c_k) used as (double)c_j.  A group with s = 0 contributes 0.
  * E[.] of Eq.(2) is sq_err / (n_vec*d); its argmin over j is the calibrated constant (:128).
  * Plain loops, vector after vector, one double accumulator per c_j. */
 static int uqo_mag_of_ratio(double r) {
@@ -175,8 +180,10 @@ static int uqo_mag_of_ratio(double r) {
 }
 
 void uqo_calib_sq_err(const uint16_t* x_bf16, int64_t n_vec, int d, int rotate, const float* c_grid,
-                      int n_c, int pow2, double* sq_err /*[n_c]*/, double* sq_norm /*[1]*/) {
-  static const double F[8] = {0.0, 0.5, 1.0, 1.5, 2.0, 3.0, 4.0, 6.0};
+                      int n_c, int scale_mode, const float* levels /*[8] or NULL*/,
+                      double* sq_err /*[n_c]*/, double* sq_norm /*[1]*/) {
+  double F[8] = {0.0, 0.5, 1.0, 1.5, 2.0, 3.0, 4.0, 6.0};
+  if (levels) for (int i = 0; i < 8; ++i) F[i] = (double)levels[i];
   double* x = (double*)malloc(sizeof(double) * (size_t)d);
   double* y = (double*)malloc(sizeof(double) * (size_t)d);
   for (int j = 0; j < n_c; ++j) sq_err[j] = 0.0;
@@ -195,7 +202,7 @@ void uqo_calib_sq_err(const uint16_t* x_bf16, int64_t n_vec, int d, int rotate, 
       }
       for (int j = 0; j < n_c; ++j) {
         const double c = (double)c_grid[j];
-        if (pow2) {
+        if (scale_mode == 1) {
           int E = uqo_scale_exponent(c, m);
           for (int i = 0; i < UQ_GROUP; ++i) {
             double zh = uqo_dequant(uqo_e2m1_encode(yg[i], E), (uint8_t)(E + 127));
@@ -203,11 +210,18 @@ void uqo_calib_sq_err(const uint16_t* x_bf16, int64_t n_vec, int d, int rotate, 
             sq_err[j] += e * e;
           }
         } else {
-          double s = c * m;
+          double s = (scale_mode == 2) ? c : c * m;
           if (!(s > 0.0)) continue;
           for (int i = 0; i < UQ_GROUP; ++i) {
-            double lev = F[uqo_mag_of_ratio(fabs(yg[i]) / s)];
-            double zh = (yg[i] < 0.0 ? -lev : lev) * s;
+            double r = fabs(yg[i]) / s;
+            int mag;
+            if (levels) {
+              mag = 0;
+              for (int k = 0; k < 7; ++k) mag += (r > 0.5 * (F[k] + F[k + 1]));
+            } else {
+              mag = uqo_mag_of_ratio(r);
+            }
+            double zh = (yg[i] < 0.0 ? -F[mag] : F[mag]) * s;
             double e = yg[i] - zh;
             sq_err[j] += e * e;
           }

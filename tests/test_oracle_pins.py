@@ -277,6 +277,49 @@ def test_p11_paper_ordering_of_the_constants_on_rotated_vectors():
     assert three[0] < three[1] < three[2] and three[2] > 5 * three[0]
 
 
+def _lloyd_max_gaussian_magnitudes():
+    """Lloyd's algorithm for a 16-level quantiser of N(0,1) (the published fixed-point iteration: thresholds =
+    midpoints, centroids = conditional means), run here on the closed-form Gaussian integrals; returns the 8
+    positive centroids."""
+    from scipy.stats import norm
+    c = np.linspace(0.1, 2.5, 8)
+    for _ in range(500):
+        t = np.concatenate([[0.0], 0.5 * (c[:-1] + c[1:]), [np.inf]])
+        c = (norm.pdf(t[:-1]) - norm.pdf(t[1:])) / (norm.cdf(t[1:]) - norm.cdf(t[:-1]))
+    return c
+
+
+def test_p11_other_codebooks_and_the_fixed_scale():
+    """scale_mode 2 (s = c, no absmax) and `levels` against numpy restatements, on the distribution of Fig. 2
+    (PAPER.md:118-120): coordinates of random unit vectors, d = 64, 128, 256.  The analytical Lloyd-Max codebook at
+    the fixed scale 1/sqrt(d) has a lower MSE than absmax-scaled FP4 at any of the paper's constants (Fig. 2b: "FP4
+    has higher MSE than analytical Lloyd-Max"), and c = 0.156 beats c = 1.0 by a wide margin (Table 5)."""
+    lm = _lloyd_max_gaussian_magnitudes()
+    assert lm[0] == pytest.approx(0.1284, abs=2e-3) and lm[-1] == pytest.approx(2.7326, abs=2e-3)   # textbook table
+    rng = np.random.default_rng(31)
+    for d in (64, 128, 256):
+        u = rng.standard_normal((512 * 128 // d, d))
+        u /= np.linalg.norm(u, axis=1, keepdims=True)
+        bits = _bf16_bits(u.reshape(-1, 128))
+        y = oracle.bf16_to_double(bits)
+        one = lambda c, mode, lev=None: oracle.calib_sq_err(bits, np.array([c], np.float32), rotate=False,
+                                                            scale_mode=mode, levels=lev)[0][0] / y.size
+        mse_lm = one(d ** -0.5, 2, lm)
+        mse_opt, mse_195, mse_one = one(0.156, 0), one(0.195, 0), one(1.0, 0)
+        mse_int4 = one(1.0 / 7.0, 0, np.arange(8.0))
+        assert mse_lm < min(mse_opt, mse_195, mse_one)
+        assert mse_opt < mse_195 < mse_one and mse_one > 5 * mse_opt
+        # numpy restatements: the fixed-scale Lloyd-Max quantiser, and absmax INT4 (grid m/7 * {-7..7})
+        s = np.float64(np.float32(d ** -0.5))
+        lev = np.concatenate([-lm[::-1], lm]).astype(np.float32).astype(np.float64)
+        q = lev[np.abs(y[..., None] / s - lev).argmin(axis=-1)]
+        assert mse_lm == pytest.approx(np.mean((y - s * q) ** 2), rel=1e-10)
+        yg = y.reshape(-1, 32)
+        sg = np.float64(np.float32(1.0 / 7.0)) * np.abs(yg).max(axis=1, keepdims=True)
+        qi = np.clip(np.floor(np.abs(yg) / sg + 0.5), 0, 7) * np.sign(yg)
+        assert mse_int4 == pytest.approx(np.mean((yg - sg * qi) ** 2), rel=1e-9)
+
+
 # ----------------------------------------------------------------------------- P8 library casts
 @pytest.fixture(scope="module")
 def libcasts():
