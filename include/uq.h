@@ -170,9 +170,13 @@ int32_t uq_merge_splits(const uq_config* cfg, const float* partial_acc, const fl
  *     sq_err[j] = sum over all elements z of (z - zhat_j(z))^2,        sq_norm[0] = sum z^2,
  * z = the rotated vector H x / sqrt(head_dim) if rotate != 0 (keys, Alg. 1 l.1), else x itself (values); m = the
  * absmax of z's 32-channel group;
- *     pow2_scale == 0:  zhat = s * q(z / s) with s = c_j * m and q the nearest level of F   (Eq.(2) as printed);
- *     pow2_scale != 0:  zhat = Eq.(1) of the code Alg. 1 l.3-5 stores: s = 2^round(log2(c_j * m)) (the deployed
- *                       quantiser; ties and clamping as in uq_rotate_quantize_append).
+ *     scale_mode 0:  zhat = s * q(z / s) with s = c_j * m and q the nearest level               (Eq.(2) as printed);
+ *     scale_mode 1:  zhat = Eq.(1) of the code Alg. 1 l.3-5 stores: s = 2^round(log2(c_j * m)) (the deployed
+ *                    quantiser; ties and clamping as in uq_rotate_quantize_append; E2M1 levels only);
+ *     scale_mode 2:  s = c_j, no absmax: a fixed grid for vectors of known norm (the per-token-norm schemes the
+ *                    paper compares with, Fig. 2).
+ *  levels   NULL: F = {0,.5,1,1.5,2,3,4,6} (E2M1); else float32 [8] (device), ascending magnitudes of another
+ *           symmetric codebook (uniform INT4: 0..7; Lloyd-Max centroids), nearest level, a tie to the smaller one.
  * E[.] of Eq.(2) is sq_err[j] / (n_vec * head_dim); the calibrated constant is the c_j with the smallest sq_err[j].
  *  x        bf16 [n_vec, head_dim], 8-byte aligned.     c_grid  float32 [n_c] (device), used as (double)c_j.
  *  sq_err   float64 [n_c], sq_norm float64 [1] (device): zeroed on the stream, then accumulated.
@@ -181,8 +185,8 @@ int32_t uq_merge_splits(const uq_config* cfg, const float* partial_acc, const fl
  * the additions (relative difference ~1e-13) and may differ in the last bits from run to run.
  */
 int32_t uq_calibrate_c(const uq_config* cfg, const void* x, int64_t n_vec, int32_t rotate,
-                       const float* c_grid, int32_t n_c, int32_t pow2_scale, double* sq_err,
-                       double* sq_norm, void* stream);
+                       const float* c_grid, int32_t n_c, int32_t scale_mode, const float* levels,
+                       double* sq_err, double* sq_norm, void* stream);
 
 /* Host.  A num_splits (slot count) that lets uq_decode_attention balance `batch` sequences of about
  * `avg_seq_len` tokens over the current device with room for sequences twice that long (never below 1). */

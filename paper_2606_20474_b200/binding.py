@@ -68,7 +68,7 @@ def _load():
     lib.uq_merge_splits.restype = i32
     lib.uq_merge_splits.argtypes = [cfgp, vp, vp, i32, i32, vp, vp]
     lib.uq_calibrate_c.restype = i32
-    lib.uq_calibrate_c.argtypes = [cfgp, vp, i64, i32, vp, i32, i32, vp, vp, vp]
+    lib.uq_calibrate_c.argtypes = [cfgp, vp, i64, i32, vp, i32, i32, vp, vp, vp, vp]
     lib.uq_suggest_num_splits.restype = i32
     lib.uq_suggest_num_splits.argtypes = [cfgp, i32, i32]
     _lib = lib
@@ -133,18 +133,26 @@ def rotate_quantize_append(cfg: UQConfig, k_new, v_new, cu_new, seq_lens, block_
     _check(st, "uq_rotate_quantize_append")
 
 
-def calibrate_c(cfg: UQConfig, x, c_grid, rotate: bool = True, pow2_scale: bool = True, stream=None):
-    """uq_calibrate_c (Eq.(2)).  x bf16 [n, head_dim], c_grid float32 [n_c] (CUDA tensors).  Returns
-    (sq_err float64 [n_c], sq_norm float64 [1]) on the device; the calibrated constant is c_grid[sq_err.argmin()]."""
+def calibrate_c(cfg: UQConfig, x, c_grid, rotate: bool = True, pow2_scale: bool = True, scale_mode=None, levels=None,
+                stream=None):
+    """uq_calibrate_c (Eq.(2)).  x bf16 [n, head_dim], c_grid float32 [n_c] (CUDA tensors); scale_mode
+    0 (s = c m), 1 (the deployed power of two) or 2 (s = c), default 1 if pow2_scale else 0; levels None (E2M1) or
+    float32 [8] on the device.  Returns (sq_err float64 [n_c], sq_norm float64 [1]) on the device; the calibrated
+    constant is c_grid[sq_err.argmin()]."""
     lib = _load()
     _dev(x, torch.bfloat16, "x"); _dev(c_grid, torch.float32, "c_grid")
+    if levels is not None:
+        _dev(levels, torch.float32, "levels")
+        if levels.numel() != 8:
+            raise UQError("levels must hold 8 magnitudes")
     if x.dim() != 2 or x.shape[1] != cfg.head_dim:
         raise UQError(f"x must be [n, {cfg.head_dim}], got {tuple(x.shape)}")
+    mode = (1 if pow2_scale else 0) if scale_mode is None else int(scale_mode)
     sq_err = torch.empty(c_grid.shape[0], dtype=torch.float64, device=x.device)
     sq_norm = torch.empty(1, dtype=torch.float64, device=x.device)
     c = cfg.c()
     st = lib.uq_calibrate_c(ctypes.byref(c), _p(x), x.shape[0], int(bool(rotate)), _p(c_grid), c_grid.shape[0],
-                            int(bool(pow2_scale)), _p(sq_err), _p(sq_norm), _stream(stream))
+                            mode, _p(levels), _p(sq_err), _p(sq_norm), _stream(stream))
     _check(st, "uq_calibrate_c")
     return sq_err, sq_norm
 

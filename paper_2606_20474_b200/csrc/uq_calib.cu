@@ -27,8 +27,16 @@ __device__ __forceinline__ double warp_sum(double v) {
 
 __global__ void __launch_bounds__(32 * kCalibWarps)
 calib_kernel(const uint16_t* __restrict__ x, long long n_vec, int rotate, const float* __restrict__ c_grid, int n_c,
-             int pow2, double* __restrict__ sq_err, double* __restrict__ sq_norm) {
+             int scale_mode, const float* __restrict__ levels, double* __restrict__ sq_err, double* __restrict__ sq_norm) {
   const int lane = threadIdx.x & 31;
+  // a codebook other than E2M1: its 8 magnitudes and the 7 midpoints between them (a tie goes to the smaller level)
+  double lv[8], th[7];
+  if (levels != nullptr) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) lv[i] = (double)levels[i];
+#pragma unroll
+    for (int i = 0; i < 7; ++i) th[i] = __dmul_rn(0.5, __dadd_rn(lv[i], lv[i + 1]));
+  }
   const long long w0 = (long long)blockIdx.x * kCalibWarps + (threadIdx.x >> 5), nw = (long long)gridDim.x * kCalibWarps;
   for (int j0 = 0; j0 < n_c; j0 += kChunk) {
     double c[kChunk], acc[kChunk], nrm = 0.0;
@@ -50,7 +58,7 @@ calib_kernel(const uint16_t* __restrict__ x, long long n_vec, int rotate, const 
       for (int s = 1; s <= 4; s <<= 1) m = fmax(m, __shfl_xor_sync(kFull, m, s));
 #pragma unroll
       for (int j = 0; j < kChunk; ++j) {
-        if (pow2) {                                    // Alg. 1 l.3-5 and Eq.(1): the deployed quantiser
+        if (scale_mode == 1) {                         // Alg. 1 l.3-5 and Eq.(1): the deployed quantiser
           const int E = scale_exponent(c[j], m);
           const double s = __longlong_as_double((long long)(1023 + E) << 52);   // 2^E, |E| <= 127
 #pragma unroll
@@ -60,14 +68,21 @@ calib_kernel(const uint16_t* __restrict__ x, long long n_vec, int rotate, const 
             const double e = __dadd_rn(y[r], -__dmul_rn((code & 8u) ? -lev : lev, s));
             acc[j] = __dadd_rn(acc[j], __dmul_rn(e, e));
           }
-        } else {                                       // Eq.(2) as printed: s = c m
-          const double s = __dmul_rn(c[j], m);
+        } else {                                       // Eq.(2) as printed: s = c m; or the fixed scale s = c
+          const double s = (scale_mode == 2) ? c[j] : __dmul_rn(c[j], m);
           if (s > 0.0) {
 #pragma unroll
             for (int r = 0; r < 4; ++r) {
               const double q = __ddiv_rn(fabs(y[r]), s);
-              const uint32_t mag = (q > 0.25) + (q >= 0.75) + (q > 1.25) + (q >= 1.75) + (q > 2.5) + (q >= 3.5) + (q > 5.0);
-              const double lev = e2m1_level_of(mag);
+              double lev;
+              if (levels != nullptr) {
+                lev = lv[0];
+#pragma unroll
+                for (int i = 0; i < 7; ++i) lev = (q > th[i]) ? lv[i + 1] : lev;
+              } else {
+                const uint32_t mag = (q > 0.25) + (q >= 0.75) + (q > 1.25) + (q >= 1.75) + (q > 2.5) + (q >= 3.5) + (q > 5.0);
+                lev = e2m1_level_of(mag);
+              }
               const double e = __dadd_rn(y[r], -__dmul_rn(y[r] < 0.0 ? -lev : lev, s));
               acc[j] = __dadd_rn(acc[j], __dmul_rn(e, e));
             }
@@ -91,13 +106,17 @@ calib_kernel(const uint16_t* __restrict__ x, long long n_vec, int rotate, const 
 }  // namespace uq
 
 extern "C" int32_t uq_calibrate_c(const uq_config* cfg, const void* x, int64_t n_vec, int32_t rotate,
-                                  const float* c_grid, int32_t n_c, int32_t pow2_scale, double* sq_err,
-                                  double* sq_norm, void* stream) {
+                                  const float* c_grid, int32_t n_c, int32_t scale_mode, const float* levels,
+                                  double* sq_err, double* sq_norm, void* stream) {
   using namespace uq;
   int32_t st = check_config(cfg);
   if (st != UQ_OK) return st;
   if (!x || !c_grid || !sq_err || !sq_norm || n_vec <= 0 || n_c <= 0) {
     set_error("calibrate: NULL pointer or non-positive size");
+    return UQ_ERR_INVALID_ARG;
+  }
+  if (scale_mode < 0 || scale_mode > 2 || (scale_mode == 1 && levels != nullptr)) {
+    set_error("calibrate: scale_mode must be 0, 1 or 2, and the power-of-two scale (1) takes the E2M1 levels only");
     return UQ_ERR_INVALID_ARG;
   }
   if (((uintptr_t)x & 7u) || ((uintptr_t)sq_err & 7u) || ((uintptr_t)sq_norm & 7u) || ((uintptr_t)c_grid & 3u)) {
@@ -118,6 +137,6 @@ extern "C" int32_t uq_calibrate_c(const uq_config* cfg, const void* x, int64_t n
   long long blocks = (n_vec + kCalibWarps - 1) / kCalibWarps;
   if (blocks > 8LL * sm_count) blocks = 8LL * sm_count;   // a multiple of the SM count; warps stride over the vectors
   calib_kernel<<<(unsigned)blocks, 32 * kCalibWarps, 0, s>>>((const uint16_t*)x, (long long)n_vec, (int)rotate, c_grid,
-                                                             (int)n_c, (int)pow2_scale, sq_err, sq_norm);
+                                                             (int)n_c, (int)scale_mode, levels, sq_err, sq_norm);
   return check_cuda(cudaGetLastError(), "uq_calibrate_c launch");
 }

@@ -596,3 +596,23 @@ def test_calibrate_c_matches_the_oracle_objective(rotate, pow2):
         sq2, _ = uq.calibrate_c(cfg, x[9:].contiguous().to(DEV), torch.from_numpy(cs).to(DEV), rotate=True, pow2_scale=pow2)
         best = float(cs[int(torch.argmin(sq2[:16]).item())])
         assert abs(best - (0.195 if pow2 else 0.156)) < 0.03
+
+
+def test_calibrate_c_other_codebooks_and_fixed_scale():
+    """uq_calibrate_c with a codebook other than E2M1 (uniform INT4 magnitudes 0..7 on the absmax scale; 8 Lloyd-Max-
+    like magnitudes on a fixed scale, scale_mode 2) against the oracle, on coordinates of random unit vectors
+    (the distribution of Fig. 2)."""
+    g = torch.Generator(device="cpu"); g.manual_seed(5)
+    u = torch.randn((2048, 128), generator=g)
+    u = (u / u.norm(dim=1, keepdim=True)).to(torch.bfloat16)
+    cfg = uq.UQConfig(num_q_heads=8, num_kv_heads=1)
+    lm = np.array([0.1284, 0.3881, 0.6568, 0.9424, 1.2562, 1.6181, 2.0690, 2.7326], np.float32)
+    cases = [(0, np.arange(8, dtype=np.float32), np.array([1 / 7, 0.12, 0.2], np.float32)),
+             (2, lm, np.array([128 ** -0.5, 0.07, 0.1], np.float32)),
+             (2, None, np.array([0.02, 0.05], np.float32))]
+    for mode, lev, cs in cases:
+        sq, nrm = uq.calibrate_c(cfg, u.to(DEV), torch.from_numpy(cs).to(DEV), rotate=False, scale_mode=mode,
+                                 levels=None if lev is None else torch.from_numpy(lev).to(DEV))
+        ref, ref_nrm = oracle.calib_sq_err(H.bits(u), cs, rotate=False, scale_mode=mode, levels=lev)
+        np.testing.assert_allclose(sq.cpu().numpy(), ref, rtol=1e-11, atol=0)
+        assert float(nrm.cpu()[0]) == pytest.approx(ref_nrm, rel=1e-11)
