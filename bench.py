@@ -409,7 +409,27 @@ def cpu_baseline(idx: int, budget_s: float = 15.0):
     return {"value": round(nbytes / dt / 1e9, 5), "unit": UNIT, "cores": cores, "kind": "oracle",
             "seconds": round(dt, 3),
             "sample": f"{n_seq} of {wl.batch} sequences of config {idx}, {seqs[0][0]} tokens each "
-                      f"(append 1 token + Q encode + float64 attention, all {wl.num_q_heads} heads)"}
+                      f"(append 1 token + Q encode + float64 attention, all {wl.num_q_heads} heads)",
+            "quant_error_vs_bf16": _quant_error_context(oracle, idx)}
+
+
+def _quant_error_context(oracle, idx: int, length: int = 4096):
+    """Context only (north_star): the method's own error — the oracle's attention over the FP4 / FP8-quantised
+    values against float64 attention over the unquantised bf16 Q, K, V — on sequence 0 truncated to `length` tokens."""
+    from paper_2606_20474_b200 import workloads as W     # input generator only (no arithmetic)
+    wl = _workload(idx, 0)
+    L = min(int(wl.ctx_lens[0]), length)
+    k, v = W.seq_kv(wl, 0, L, "cpu")
+    q = W.gen_q(wl, "cpu", step=0)[0]
+    arrays = oracle.encode_kv(k.view(torch.uint16).numpy(), v.view(torch.uint16).numpy())
+    out_q = oracle.attention(oracle.encode_q(q.view(torch.uint16).numpy()), *arrays, wl.num_q_heads, wl.num_kv_heads)
+    out_d = oracle.attention_dense(q.double().numpy(), k.double().numpy(), v.double().numpy())
+    return {"rel_fro": round(float(np.linalg.norm(out_q - out_d) / np.linalg.norm(out_d)), 5),
+            "max_abs": round(float(np.abs(out_q - out_d).max()), 5),
+            "sample": f"sequence 0 of config {idx}, first {L} tokens, all {wl.num_q_heads} heads",
+            "note": "synthetic N(0,1) inputs: an output row is a near-uniform average of random values, so the relative "
+                    "figure is the quantisers' own noise (4-bit V: 0.125 relative RMS per element, plus the score "
+                    "noise of 4-bit K and FP8 Q) undamped by any signal; context, not a parity figure"}
 
 
 def run_reference(args):
