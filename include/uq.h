@@ -165,6 +165,27 @@ int32_t uq_merge_splits(const uq_config* cfg, const float* partial_acc, const fl
                         int32_t batch, int32_t num_splits, void* out_bf16, void* stream);
 
 /*
+ * Shared-prefix ("cascade") decode: the first prefix_len tokens of ALL `batch` sequences are the same physical pages
+ * (block_tables[b][p] is the same for every b and p < prefix_len / page_size: the caller's guarantee — the long
+ * shared prompt of the paper's agent workloads).  Computes the partials of exactly those tokens
+ * for every sequence, each 128-token tile staged, converted and multiplied once for two sequences at a time; the
+ * remaining tokens of a sequence go through uq_decode_attention with block_tables + prefix_len / page_size and
+ * seq_lens - prefix_len, and uq_merge_splits2 combines the two sets.
+ *  prefix_len   a positive multiple of 128, <= every sequence's length.      num_splits >= 2.
+ *  partial_acc / partial_ml: as for uq_decode_attention, [batch, num_q_heads, num_splits, ...].
+ * Arithmetic and error bound as uq_decode_attention.
+ */
+int32_t uq_decode_prefix_attention(const uq_config* cfg, const void* q_fp8, const void* cache,
+                                   int64_t num_pages, const int32_t* block_tables, int32_t max_pages,
+                                   int32_t batch, int32_t prefix_len, int32_t num_splits,
+                                   float* partial_acc, float* partial_ml, void* stream);
+
+/* uq_merge_splits over two sets of partials of the same rows (splits_a and splits_b slots per row). */
+int32_t uq_merge_splits2(const uq_config* cfg, const float* acc_a, const float* ml_a, int32_t splits_a,
+                         const float* acc_b, const float* ml_b, int32_t splits_b, int32_t batch,
+                         void* out_bf16, void* stream);
+
+/*
  * The objective of Eq.(2) on a grid of constants — "solved once, offline, on captured rotated key
  * activations" (:128).  For every c_j of the grid:
  *     sq_err[j] = sum over all elements z of (z - zhat_j(z))^2,        sq_norm[0] = sum z^2,

@@ -17,7 +17,9 @@ from .binding import (  # noqa: F401
     alloc_cache,
     cache_record_bytes,
     calibrate_c,
+    PrefixBuffers,
     decode_attention,
+    decode_attention_shared_prefix,
     decode_step,
     decode_step_host,
     last_error,

@@ -67,6 +67,10 @@ def _load():
     lib.uq_decode_attention.argtypes = [cfgp, vp, vp, i64, vp, i32, vp, i32, i32, vp, vp, vp]
     lib.uq_merge_splits.restype = i32
     lib.uq_merge_splits.argtypes = [cfgp, vp, vp, i32, i32, vp, vp]
+    lib.uq_decode_prefix_attention.restype = i32
+    lib.uq_decode_prefix_attention.argtypes = [cfgp, vp, vp, i64, vp, i32, i32, i32, i32, vp, vp, vp]
+    lib.uq_merge_splits2.restype = i32
+    lib.uq_merge_splits2.argtypes = [cfgp, vp, vp, i32, vp, vp, i32, i32, vp, vp]
     lib.uq_calibrate_c.restype = i32
     lib.uq_calibrate_c.argtypes = [cfgp, vp, i64, i32, vp, i32, i32, vp, vp, vp, vp]
     lib.uq_suggest_num_splits.restype = i32
@@ -180,6 +184,45 @@ def merge_splits(cfg: UQConfig, partial_acc, partial_ml, out, stream=None) -> No
     st = lib.uq_merge_splits(ctypes.byref(c), _p(partial_acc), _p(partial_ml), out.shape[0],
                              partial_ml.shape[2], _p(out), _stream(stream))
     _check(st, "uq_merge_splits")
+
+
+class PrefixBuffers:
+    """Device scratch of the shared-prefix decode: the prefix partials (a second set next to StepBuffers') and the
+    suffix lengths / block-table view the suffix call reads.  `suffix_lens` (int32 [batch], = seq_lens - prefix_len)
+    is the caller's to fill."""
+
+    def __init__(self, cfg: UQConfig, batch: int, prefix_splits: int, device="cuda"):
+        self.prefix_splits = prefix_splits
+        self.partial_acc = torch.empty((batch, cfg.num_q_heads, prefix_splits, cfg.head_dim), dtype=torch.float32, device=device)
+        self.partial_ml = torch.empty((batch, cfg.num_q_heads, prefix_splits, 2), dtype=torch.float32, device=device)
+        self.suffix_lens = torch.empty((batch,), dtype=torch.int32, device=device)
+
+
+def decode_attention_shared_prefix(cfg: UQConfig, bufs: "StepBuffers", pbufs: PrefixBuffers, cache, block_tables,
+                                   prefix_len: int, stream=None) -> torch.Tensor:
+    """Decode + merge for sequences that share their first prefix_len tokens (a multiple of 128; same pages in every
+    block table): uq_decode_prefix_attention over the prefix, uq_decode_attention over the private suffixes
+    (pbufs.suffix_lens, the block tables from page prefix_len / page_size on), uq_merge_splits2.  bufs.q_fp8 holds
+    the encoded queries.  Returns bufs.out."""
+    lib = _load()
+    _dev(cache, torch.uint8, "cache"); _dev(block_tables, torch.int32, "block_tables")
+    c = cfg.c()
+    batch, max_pages = block_tables.shape
+    pp = prefix_len // cfg.page_size
+    st = lib.uq_decode_prefix_attention(ctypes.byref(c), _p(bufs.q_fp8), _p(cache), cache.shape[0], _p(block_tables),
+                                        max_pages, batch, int(prefix_len), pbufs.prefix_splits, _p(pbufs.partial_acc),
+                                        _p(pbufs.partial_ml), _stream(stream))
+    _check(st, "uq_decode_prefix_attention")
+    bt_suffix = ctypes.c_void_p(block_tables.data_ptr() + 4 * pp)      # row stride stays max_pages
+    st = lib.uq_decode_attention(ctypes.byref(c), _p(bufs.q_fp8), _p(cache), cache.shape[0], bt_suffix, max_pages,
+                                 _p(pbufs.suffix_lens), batch, bufs.num_splits, _p(bufs.partial_acc),
+                                 _p(bufs.partial_ml), _stream(stream))
+    _check(st, "uq_decode_attention (suffix)")
+    st = lib.uq_merge_splits2(ctypes.byref(c), _p(pbufs.partial_acc), _p(pbufs.partial_ml), pbufs.prefix_splits,
+                              _p(bufs.partial_acc), _p(bufs.partial_ml), bufs.num_splits, batch, _p(bufs.out),
+                              _stream(stream))
+    _check(st, "uq_merge_splits2")
+    return bufs.out
 
 
 class StepBuffers:

@@ -49,6 +49,13 @@ inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, s
   return cudaLaunchKernelEx(&lc, kernel, KArgs(args)...);
 }
 
+// TMA descriptors of the decode kernels (uq_decode.cu): the K codes of the cache as a packed 4-bit tensor (cached
+// per cache pointer), and q_fp8 as [rows][128] bytes with a box of 16 rows.
+#ifdef CUDA_VERSION
+int32_t k_code_map(const void* cache, long long records, CUtensorMap* out);
+int32_t q_map(const void* q_fp8, long long rows, CUtensorMap* out);
+#endif
+
 inline float resolved_sm_scale(const uq_config* cfg) {
   return cfg->sm_scale != 0.0f ? cfg->sm_scale : 0.08838834764831845f;  // 1/sqrt(128)
 }

@@ -1,30 +1,13 @@
-// uq_decode.cu — paged split-K decode attention over the FP4+UE8M0 cache: Alg. 1 "Decode"
-// l.7-8 of arxiv/paper_2606_20474 (Eq.(1) :104).  Paging / split-K / partial
-// format follow include/uq.h.
-//
-// Design: the 128-token tiles (8 pages) of all (sequence, kv head) items form one
-// sequence that is cut into equal contiguous ranges, one per resident CTA (one wave, 2 CTAs per SM); a
-// range is walked as units (item, tile range), each unit writing one partial slot of its item.
-// Warp roles (384 threads = 12 warps, one role each; the tile period is set by the longest serial instruction
-// stream of the CTA, so the roles are cut to keep every stream short):
-//   K producer   per page one TMA tensor copy of the packed FP4 K codes (CU_TENSOR_MAP_DATA_TYPE_16U4_ALIGN16B +
-//                SWIZZLE_128B: the TMA unit lays the nibbles out in the 8-bit containers tcgen05 reads) into a
-//                3-stage ring; L2 evict-first;
-//   V producer   per page one cp.async.bulk of the rest of the record (V codes, K scales, V scales) into a
-//                4-stage ring of its own;
-//   QK issuer    S[128 tok x 16 heads] = K . Q^T with tcgen05.mma.kind::mxf8f6f4.block_scale — E2M1 keys x E4M3
-//                queries with the UE8M0 group scales applied by the tensor core (the paper's FP8xFP4 scaled MMA,
-//                PAPER.md:281), K scales staged smem -> TMEM with tcgen05.cp; S double-buffered in TMEM;
-//   PV issuer    O^T[128 d x 16 heads] += Vhat^T . P^T with tcgen05.mma.kind::f16 (A = Vhat^T from TMEM, B = P from
-//                smem); accumulators in TMEM;
-//   4 softmax warps   thread = token row: S from TMEM (tcgen05.ld), base-2 softmax against a LAZY per-head
-//                reference (a "rebase" — new reference, O rescaled in TMEM, tile's P redone — happens on the first
-//                tile and whenever a score exceeds the reference by 2^12), P -> fp16 operand in smem;
-//   4 V warps    thread = channel: V codes -> fp16 (cvt.rn.f16x2.e2m1x2 x exact power-of-two scale against the
-//                warp's own reference exponent: its 32 channels are one scale group) written with tcgen05.st
-//                straight into TMEM, where the PV MMA reads it as its A operand (no shared-memory round trip).
-// The FP8 query tile is copied to smem by TMA once per unit ("hoisted").
-// Every K/V byte is read from HBM exactly once.
+// uq_decode_prefix.cu — decode attention over a SHARED PREFIX ("cascade"): the first prefix_len
+// tokens of every sequence of the call are the same physical pages (the agent workloads of the paper share a long
+// prompt), so a 128-token tile of the prefix is staged, its V codes converted and its MMAs issued
+// once for kNS sequences at a time instead of once per sequence.  Same CTA design as uq_decode.cu (read that file
+// first): TMA K / V rings, tcgen05 block-scaled QK, softmax warps with lazy per-head references, V warps writing
+// Vhat^T to TMEM, PV from TMEM — with the score tile widened from 16 to 16 kNS columns (the query tiles of kNS
+// sequences side by side), kNS sets of references and running sums in the softmax warps, and one CTA per SM (the
+// registers and TMEM columns of two).  All items have the same length, so the schedule is plain arithmetic.
+// The partials have the format of include/uq.h; the private suffixes go through uq_decode_attention and both sets
+// are combined by uq_merge_splits2.
 #include <cuda.h>
 #include <cuda_fp16.h>
 
@@ -40,15 +23,17 @@ constexpr int kComputeWarps = 8;                     // two per TMEM lane quarte
 constexpr int kSoftmaxWarps = 4;
 constexpr int kIssuerWarps = 4;                      // QK issuer, PV issuer, K producer, V producer
 constexpr int kThreads = (kComputeWarps + kIssuerWarps) * 32;   // 12 warps: registers are allocated per 4 warps anyway
-#ifndef UQ_KSTAGES
-#define UQ_KSTAGES 3
+#ifndef UQ_PREFIX_NSEQ
+#define UQ_PREFIX_NSEQ 2
 #endif
-#ifndef UQ_VSTAGES
-#define UQ_VSTAGES 4
-#endif
-#ifndef UQ_CTAS_PER_SM
-#define UQ_CTAS_PER_SM 2
-#endif
+constexpr int kNS = UQ_PREFIX_NSEQ;                   // sequences per prefix tile
+constexpr int kNCols = 16 * kNS;                      // score columns: 16 head slots per sequence
+#undef UQ_KSTAGES
+#undef UQ_VSTAGES
+#undef UQ_CTAS_PER_SM
+#define UQ_KSTAGES 4
+#define UQ_VSTAGES 6
+#define UQ_CTAS_PER_SM 1
 // Two rings: the K codes of a tile (16 KB once the TMA unit has expanded the nibbles) are needed by the QK
 // MMA only and leave early; the rest of the records (V codes, K scales, V scales: 9 KB) stays until the V
 // warps have converted it.  Separate rings let the small one run deep (bytes in flight hide HBM latency).
@@ -58,16 +43,15 @@ constexpr int kTilePages = 8;                        // 128 tokens per tile
 constexpr int kRestBytes = kRecordBytes - 1024;      // V codes + K scales + V scales = 1152
 constexpr int kKStageBytes = kTilePages * 2048;      // K codes, one byte per code: 16384
 constexpr int kVStageBytes = kTilePages * kRestBytes;   // 9216
-constexpr int kPBytes = 4096;                        // one P operand buffer: [token-core 16][head-core 2][8 tok][8 heads] f16
+constexpr int kPBytes = 4096 * kNS;                  // one P operand buffer: [token-core 16][head-core 2 kNS][8 tok][8 heads] f16
 constexpr float kThresh = 12.0f;                     // lazy-reference threshold (log2 units)
 constexpr unsigned kFull = 0xffffffffu;
-constexpr int kMaxBatch = 2048;                      // sequences per call (tile prefix sums live in shared memory)
 
 // dynamic shared memory map (offsets from a 1024-byte aligned base)
 constexpr int kOffK = 0;                                       // kKStages x 16384, SW128
 constexpr int kOffV = kOffK + kKStages * kKStageBytes;         // kVStages x 9216
 constexpr int kOffQ = kOffV + kVStages * kVStageBytes;         // 2 x 2048, SW128 (one per unit in flight)
-constexpr int kOffSFA = kOffQ + 4096;                          // 2 x 512
+constexpr int kOffSFA = kOffQ + 4096 * kNS;                    // 2 x 512
 constexpr int kOffSFB = kOffSFA + 1024;                        // 512
 constexpr int kOffP = kOffSFB + 512;                           // 2 x 4096 (double-buffered)
 constexpr int kOffMul = kOffP + 2 * kPBytes;                   // 4 V warps x 256 B of fp16 multipliers
@@ -75,16 +59,17 @@ constexpr int kOffEnd = kOffMul + kComputeWarps * 128;
 constexpr int kSmemBytes = kOffEnd + 1024;                     // + alignment slack
 
 // TMEM columns
-constexpr uint32_t kColS = 0;      // 2 x 16
-constexpr uint32_t kColO = 32;     // 16
-constexpr uint32_t kColSFA = 48;   // 2 x 4
-constexpr uint32_t kColSFB = 56;   // 4
+constexpr uint32_t kColS = 0;                   // 2 x kNCols
+constexpr uint32_t kColO = 2 * kNCols;          // kNCols
+constexpr uint32_t kColSFA = 3 * kNCols;        // 2 x 4
+constexpr uint32_t kColSFB = 3 * kNCols + 8;    // 4
 #ifndef UQ_VBUFS
 #define UQ_VBUFS 2
 #endif
 constexpr int kVBufs = UQ_VBUFS;   // Vhat^T buffers in TMEM
-constexpr uint32_t kColV = 64;     // kVBufs x 64: Vhat^T operand, lane = channel d, column c = tokens 2c, 2c+1 (f16x2)
-constexpr uint32_t kTmemCols = kVBufs == 1 ? 128 : 256;
+constexpr uint32_t kColV = 256;    // kVBufs x 64: Vhat^T operand, lane = channel d, column c = tokens 2c, 2c+1 (f16x2)
+constexpr uint32_t kTmemCols = 512;
+static_assert(3 * kNCols + 12 <= 256, "score / accumulator / scale columns must stay below the Vhat buffers");
 
 // ---------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -293,98 +278,59 @@ struct Shared {
   float wmax[kSoftmaxWarps][16];
   float lsum[kSoftmaxWarps][16];
   float mref[16];
-  int total_tiles, max_tiles;  // sum (x kv heads) and max over sequences of the tiles per (sequence, kv head)
-  int pre[kMaxBatch + 1];      // pre[b] = tiles of sequences 0..b-1 (per kv head)
 };
 
 // ---------------------------------------------------------------- work schedule
-// The tiles (128 tokens) of all (sequence, kv head) items form one sequence, item after item.  With
-// num_splits >= 2 every CTA of the grid takes one contiguous range of `tpc` tiles of it (balanced: the
-// same amount of HBM traffic per CTA whatever the lengths are); a range may end inside an item and
-// start inside the next one, so a CTA works through a few UNITS (item, tile range), keeping its TMA /
-// MMA pipelines running across unit boundaries.  The CTAs that share an item write consecutive partial
-// slots of it; tpc is raised if needed so that no item spans more than num_splits CTAs.  With
-// num_splits == 1 a unit is a whole item and CTA c takes items c, c + gridDim.x, ...
+// Items = (group of kNS consecutive sequences, kv head), kv head fastest, every item PT = prefix_len / 128 tiles
+// long.  The tiles of all items form one sequence that is cut into equal contiguous ranges, one per CTA; a range may
+// end inside an item and start inside the next one, so a CTA works through a few UNITS (item, tile range).  The CTAs
+// that share an item write consecutive partial slots of it (the same slot for each of its sequences); tpc is raised
+// if needed so that no item spans more than num_splits CTAs.
 struct Unit {
-  int b, kvh, p0, p1, n_tiles, tok_end, L;
+  int b, kvh, p0, p1, n_tiles, tok_end;               // b: first sequence of the group
   int slots_used;                                      // > 0 on the unit holding the item's last tile: slots the item uses
-  long long row0;                                      // partial row of head 0 in this unit's slot: + head * num_splits
-};
+  long long row0;                                      // partial row of (sequence b, head 0) in this unit's slot:
+};                                                     // + head * num_splits, + hs * Hq * num_splits for sequence b + hs
 struct Cursor {
-  int b, kvh, t, g, g1, it;                            // balanced: position (b, kvh, tile t), global tile g, range end g1; items: it
+  int it, t, g, g1;                                    // item, tile inside it, global tile, range end
 };
 
 struct Sched {
-  const int32_t* seq_lens;
-  const int* pre;                                      // shared: pre[b] = tiles of sequences < b (per kv head)
-  int B, Hq, Hkv, G, S, tpc, total;
-  __device__ __forceinline__ int tiles(int b) const { return pre[b + 1] - pre[b]; }
+  int B, Hq, Hkv, G, S, tpc, total, PT;
 
   __device__ void start(Cursor& c) const {
-    if (S == 1) { c.it = blockIdx.x; return; }
     c.g = min((int)blockIdx.x * tpc, total);
     c.g1 = min(c.g + tpc, total);
-    if (c.g >= c.g1) return;
-    int lo = 0, hi = B;                                // largest b with Hkv * pre[b] <= g (and tiles(b) > 0 follows)
-    while (hi - lo > 1) {
-      const int mid = (lo + hi) >> 1;
-      if (Hkv * pre[mid] <= c.g) lo = mid; else hi = mid;
-    }
-    c.b = lo;
-    const int off = c.g - Hkv * pre[lo], tb = tiles(lo);
-    c.kvh = off / tb;
-    c.t = off - c.kvh * tb;
+    c.it = c.g / PT;
+    c.t = c.g - c.it * PT;
   }
   // next unit of this CTA, false when there is none
   __device__ bool next(Cursor& c, Unit& u) const {
-    int t0, t1, tb;
-    if (S == 1) {
-      for (;; c.it += gridDim.x) {
-        if (c.it >= B * Hkv) return false;
-        u.b = c.it / Hkv;
-        tb = tiles(u.b);
-        if (tb > 0) break;
-      }
-      u.kvh = c.it - u.b * Hkv;
-      c.it += gridDim.x;
-      t0 = 0; t1 = tb;
-      u.slots_used = 1;
-      u.row0 = ((long long)u.b * Hq + (long long)u.kvh * G) * S;
-    } else {
-      if (c.g >= c.g1) return false;
-      u.b = c.b; u.kvh = c.kvh;
-      tb = tiles(c.b);
-      t0 = c.t;
-      t1 = min(tb, t0 + (c.g1 - c.g));
-      const int item_start = c.g - t0;                 // global tile index of the item's first tile
-      const int slot = (int)blockIdx.x - item_start / tpc;
-      u.slots_used = (t1 == tb) ? slot + 1 : 0;
-      u.row0 = ((long long)u.b * Hq + (long long)u.kvh * G) * S + slot;
-      c.g += t1 - t0;
-      c.t = t1;
-      if (t1 == tb) {                                  // on to the next item with tiles
-        c.t = 0;
-        if (++c.kvh == Hkv) {
-          c.kvh = 0;
-          do { ++c.b; } while (c.b < B && tiles(c.b) == 0);
-        }
-      }
-    }
-    u.L = seq_lens[u.b];
-    const int n_pages = (u.L + kPage - 1) / kPage;
+    if (c.g >= c.g1) return false;
+    const int grp = c.it / Hkv;
+    u.kvh = c.it - grp * Hkv;
+    u.b = grp * kNS;
+    const int t0 = c.t, t1 = min(PT, t0 + (c.g1 - c.g));
+    const int item_start = c.g - t0;                   // global tile index of the item's first tile
+    const int slot = (int)blockIdx.x - item_start / tpc;
+    u.slots_used = (t1 == PT) ? slot + 1 : 0;
+    u.row0 = ((long long)u.b * Hq + (long long)u.kvh * G) * S + slot;
+    c.g += t1 - t0;
+    c.t = t1;
+    if (t1 == PT) { c.t = 0; ++c.it; }
     u.p0 = kTilePages * t0;
-    u.p1 = min(kTilePages * t1, n_pages);
+    u.p1 = kTilePages * t1;
     u.n_tiles = t1 - t0;
-    u.tok_end = min(u.L, u.p1 * kPage);
+    u.tok_end = u.p1 * kPage;
     return true;
   }
 };
 
 // ---------------------------------------------------------------- the kernel
 __global__ void __launch_bounds__(kThreads, UQ_CTAS_PER_SM)
-decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_q,
+decode_prefix_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_q,
               const uint8_t* __restrict__ cache, const int32_t* __restrict__ block_tables, int max_pages,
-              const int32_t* __restrict__ seq_lens, int batch, int Hq, int Hkv, int num_splits,
+              int prefix_tiles, int batch, int Hq, int Hkv, int num_splits,
               float score_scale /* sm_scale * log2(e) */, float* __restrict__ partial_acc,
               float* __restrict__ partial_ml) {
   extern __shared__ uint8_t smem_raw[];
@@ -444,30 +390,6 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
   // everything below reads global memory it may have written (programmatic dependent launch, uq_common.cuh).
   pdl_launch_dependents();
   pdl_wait();
-  // tiles per sequence -> inclusive prefix sums in shared memory (every CTA computes the same schedule)
-  for (int b = tid; b < batch; b += kThreads) {
-    const int L = seq_lens[b];
-    sh.pre[b + 1] = ((L + kPage - 1) / kPage + kTilePages - 1) / kTilePages;
-  }
-  if (tid == 0) sh.pre[0] = 0;
-  __syncthreads();
-  if (warp == 0) {                                     // warp scan over chunks of 32 with a running carry
-    int carry = 0, mx = 0;
-    for (int b0 = 0; b0 < batch; b0 += 32) {
-      const int b = b0 + lane;
-      const int v = b < batch ? sh.pre[b + 1] : 0;
-      int x = v;
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const int y = __shfl_up_sync(kFull, x, o);
-        if (lane >= o) x += y;
-      }
-      if (b < batch) sh.pre[b + 1] = carry + x;
-      carry += __shfl_sync(kFull, x, 31);
-      mx = max(mx, __reduce_max_sync(kFull, v));
-    }
-    if (lane == 0) { sh.total_tiles = carry * Hkv; sh.max_tiles = mx; }
-  }
   fence_async_smem();
   tc_fence_before();
   __syncthreads();
@@ -475,12 +397,11 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
   const uint32_t tmem = sh.tmem_base;
 
   Sched sc;
-  sc.seq_lens = seq_lens; sc.pre = sh.pre; sc.B = batch; sc.Hq = Hq; sc.Hkv = Hkv; sc.G = G; sc.S = num_splits;
-  sc.total = sh.total_tiles;
-  sc.tpc = 1;
-  if (num_splits > 1) {
+  sc.B = batch; sc.Hq = Hq; sc.Hkv = Hkv; sc.G = G; sc.S = num_splits; sc.PT = prefix_tiles;
+  sc.total = ((batch + kNS - 1) / kNS) * Hkv * prefix_tiles;
+  {
     const int even = (sc.total + (int)gridDim.x - 1) / (int)gridDim.x;
-    const int fit = (sh.max_tiles + num_splits - 2) / (num_splits - 1);   // an item spans at most num_splits ranges
+    const int fit = (prefix_tiles + num_splits - 2) / (num_splits - 1);   // an item spans at most num_splits ranges (>= 2)
     sc.tpc = max(1, max(even, fit));
   }
 
@@ -491,12 +412,14 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     // the next kv head (or are zero past the tensor end) and only feed score columns nobody reads.
     // Per tile: S(gt)[128 tok x 16 heads] = K . Q^T once the tile's bytes have landed, the S buffer was read
     // by the softmax of global tile gt-2.
-    const uint32_t idesc_qk = (5u << 7) | (0u << 10) | (2u << 17) | (1u << 23) | (8u << 24);   // E2M1 x E4M3, UE8M0, N=16, M=128
+    const uint32_t idesc_qk = (5u << 7) | (0u << 10) | ((uint32_t)(kNCols >> 3) << 17) | (1u << 23) | (8u << 24);   // E2M1 x E4M3, UE8M0, N=16 kNS, M=128
     if (elect_one()) umma_cp_sf(tmem + kColSFB, make_desc(sSFB, 16, 128, 0));
     auto load_q = [&](const Unit& un, int k) {         // lane 0: Q tile of unit ordinal k
       if (elect_one()) {
-        mbar_expect_tx(bar_qfull + 8 * (k & 1), 2048);
-        tma_load_2d(sQ + 2048 * (k & 1), &tmap_q, 0, un.b * Hq + un.kvh * G, bar_qfull + 8 * (k & 1));
+        mbar_expect_tx(bar_qfull + 8 * (k & 1), 2048 * kNS);
+#pragma unroll
+        for (int hs = 0; hs < kNS; ++hs)               // rows past the last sequence are zero-filled by the TMA unit
+          tma_load_2d(sQ + 2048 * kNS * (k & 1) + 2048 * hs, &tmap_q, 0, (un.b + hs) * Hq + un.kvh * G, bar_qfull + 8 * (k & 1));
       }
     };
     Cursor cur, cur_nx;
@@ -533,11 +456,11 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
         mbar_wait(bar_fullk + 8 * sk, phk);
         tc_fence_after();
         if (elect_one()) {
-          const uint32_t t_sfa = tmem + kColSFA + 4 * sb, qb = sQ + 2048 * (k & 1);
+          const uint32_t t_sfa = tmem + kColSFA + 4 * sb, qb = sQ + 2048 * kNS * (k & 1);
           umma_cp_sf(t_sfa, make_desc(sSFA + 512 * sb, 16, 128, 0));
 #pragma unroll
           for (int kb = 0; kb < 4; ++kb)
-            umma_mxf8f6f4(tmem + kColS + 16 * sb, make_desc(st + 32 * kb, 16, 1024, 2), make_desc(qb + 32 * kb, 16, 1024, 2),
+            umma_mxf8f6f4(tmem + kColS + kNCols * sb, make_desc(st + 32 * kb, 16, 1024, 2), make_desc(qb + 32 * kb, 16, 1024, 2),
                           idesc_qk | ((uint32_t)kb << 29), kb > 0, t_sfa + ((uint32_t)kb << 30), tmem + kColSFB);
           umma_commit(bar_sfull + 8 * sb);
           umma_commit(bar_emptyk + 8 * sk);
@@ -552,7 +475,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
   } else if (role == 1) {
     // ================================================================ PV warp
     // O^T[128 d x 16 heads] += Vhat^T (TMEM, buffer gt&1) . P^T (smem, buffer gt&1); f16 x f16 -> f32, B MN-major
-    const uint32_t idesc_pv = (1u << 4) | (1u << 16) | (2u << 17) | (8u << 24);
+    const uint32_t idesc_pv = (1u << 4) | (1u << 16) | ((uint32_t)(kNCols >> 3) << 17) | (8u << 24);
     Cursor cur;
     sc.start(cur);
     Unit un;
@@ -565,7 +488,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
           const uint32_t pbuf = sP + kPBytes * (gt & 1), vbuf = tmem + kColV + 64 * ((gt & 1) % kVBufs);
 #pragma unroll
           for (int j = 0; j < 8; ++j)                    // 16 tokens per MMA = 8 columns of Vhat^T
-            umma_f16_ts(tmem + kColO, vbuf + 8 * j, make_desc(pbuf + 512 * j, 256, 128, 0), idesc_pv,
+            umma_f16_ts(tmem + kColO, vbuf + 8 * j, make_desc(pbuf + 512 * kNS * j, 256 * kNS, 128, 0), idesc_pv,
                         (i > 0 || j > 0) ? 1u : 0u);
           umma_commit(bar_done + 8 * (gt & 1));
         }
@@ -627,123 +550,114 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
       // ============================================================== softmax warps
       const int atid = 32 * cw + lane;                 // 0..127
       float2* const ml_out = reinterpret_cast<float2*>(partial_ml);
-
-      // items without any token: all their slots are empty, (m, l) = (-inf, 0)
-      for (int it = blockIdx.x; it < batch * Hkv; it += gridDim.x) {
-        const int b = it / Hkv;
-        if (sc.tiles(b) == 0) {
-          const long long row = ((long long)b * Hq + (long long)(it - b * Hkv) * G) * num_splits;
-          for (int e = atid; e < G * num_splits; e += 32 * kSoftmaxWarps) ml_out[row + e] = make_float2(-INFINITY, 0.f);
-        }
-      }
+      const long long seq_rows = (long long)Hq * num_splits;   // partial rows of one sequence
 
       auto run = [&](auto nh_tag) {
-        constexpr int NH = decltype(nh_tag)::value;    // head columns this thread handles: 8 (G <= 8) or 16
+        constexpr int NH = decltype(nh_tag)::value;    // head columns per sequence this thread handles: 8 (G <= 8) or 16
         Cursor cur;
         sc.start(cur);
         Unit un;
         int gt = 0;                                    // global tile counter
-        const uint32_t p_row = sP + (r >> 3) * 256 + (r & 7) * 16;
+        const uint32_t p_row = sP + (r >> 3) * (256 * kNS) + (r & 7) * 16;
         while (sc.next(cur, un)) {
-          float nmref[NH], lsum[NH];                   // nmref = minus the per-head reference logit
+          float nmref[kNS][NH], lsum[kNS][NH];         // nmref = minus the per-head reference logit, per sequence
 #pragma unroll
-          for (int j = 0; j < NH; ++j) { nmref[j] = INFINITY; lsum[j] = 0.f; }
-          int rem = un.tok_end - un.p0 * kPage;        // valid tokens from the first row of the tile on
+          for (int hs = 0; hs < kNS; ++hs) {
+#pragma unroll
+            for (int j = 0; j < NH; ++j) { nmref[hs][j] = INFINITY; lsum[hs][j] = 0.f; }
+          }
 
-          for (int i = 0; i < un.n_tiles; ++i, rem -= kTilePages * kPage) {
+          for (int i = 0; i < un.n_tiles; ++i) {       // every tile of the prefix is whole: no token mask
             const int sb = gt & 1, ph2 = (gt >> 1) & 1;
-            const bool tile_partial = rem < kTilePages * kPage;
-            const bool tok_ok = r < rem;
-            const uint32_t t_s = tmem + lane_sel + kColS + 16 * sb;
-            const uint32_t p_addr = p_row + kPBytes * sb;
-
             mbar_wait(bar_sfull + 8 * sb, ph2);        // S(gt) is in TMEM
-            if (gt >= 2) mbar_wait(bar_done + 8 * sb, ph2 ^ 1);   // PV(gt-2) has read P buffer gt&1 (the PV warp commits
-                                                                   // once per tile: its issue stream bounds the tile period)
+            if (gt >= 2) mbar_wait(bar_done + 8 * sb, ph2 ^ 1);   // PV(gt-2) has read P buffer gt&1
             tc_fence_after();
 
-            float lt[NH];
-            // softmax of this thread's row against the current references -> P (fp16, MN-major operand)
-            auto softmax_pass = [&]() -> bool {
-              float t[NH];
-              tmem_ld<NH>(t_s, t);
 #pragma unroll
-              for (int j = 0; j < NH; j += 2) ffma2(t[j], t[j + 1], t[j], t[j + 1], score_scale, nmref[j], nmref[j + 1]);
-              if (tile_partial) {
+            for (int hs = 0; hs < kNS; ++hs) {         // the sequences of the group one after the other
+              const uint32_t t_s = tmem + lane_sel + kColS + kNCols * sb + 16 * hs;
+              const uint32_t p_addr = p_row + kPBytes * sb + 256 * hs;   // head-cores 2 hs, 2 hs + 1
+              float lt[NH];
+              // softmax of this thread's row against the current references -> P (fp16, MN-major operand)
+              auto softmax_pass = [&]() -> bool {
+                float t[NH];
+                tmem_ld<NH>(t_s, t);
 #pragma unroll
-                for (int j = 0; j < NH; ++j) t[j] = tok_ok ? t[j] : -INFINITY;
-              }
-              float tmax = t[0];
+                for (int j = 0; j < NH; j += 2)
+                  ffma2(t[j], t[j + 1], t[j], t[j + 1], score_scale, nmref[hs][j], nmref[hs][j + 1]);
+                float tmax = t[0];
 #pragma unroll
-              for (int j = 1; j < NH; ++j) tmax = fmaxf(tmax, t[j]);
+                for (int j = 1; j < NH; ++j) tmax = fmaxf(tmax, t[j]);
 #pragma unroll
-              for (int j = 0; j < NH; ++j) lt[j] = ex2(t[j]);
+                for (int j = 0; j < NH; ++j) lt[j] = ex2(t[j]);
 #pragma unroll
-              for (int c = 0; c < NH / 8; ++c) {
-                uint4 o;
-                asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.x) : "f"(lt[8 * c + 1]), "f"(lt[8 * c + 0]));
-                asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.y) : "f"(lt[8 * c + 3]), "f"(lt[8 * c + 2]));
-                asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.z) : "f"(lt[8 * c + 5]), "f"(lt[8 * c + 4]));
-                asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.w) : "f"(lt[8 * c + 7]), "f"(lt[8 * c + 6]));
-                sts128(p_addr + 128 * c, o);
-              }
-              return tmax > kThresh;
-            };
+                for (int c = 0; c < NH / 8; ++c) {
+                  uint4 o;
+                  asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.x) : "f"(lt[8 * c + 1]), "f"(lt[8 * c + 0]));
+                  asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.y) : "f"(lt[8 * c + 3]), "f"(lt[8 * c + 2]));
+                  asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.z) : "f"(lt[8 * c + 5]), "f"(lt[8 * c + 4]));
+                  asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o.w) : "f"(lt[8 * c + 7]), "f"(lt[8 * c + 6]));
+                  sts128(p_addr + 128 * c, o);
+                }
+                return tmax > kThresh;
+              };
 
-            bool rebase = (i == 0);
-            if (!rebase) {
-              const bool ex = softmax_pass();
-              rebase = bar_softmax_or(ex);
-            }
-            if (__builtin_expect(rebase, 0)) {
-              // ---- per-head maximum score of the tile -> new references; O and l rescaled
-              float tm[NH];
-              {
-                float sv[NH];
-                tmem_ld<NH>(t_s, sv);
+              bool rebase = (i == 0);
+              if (!rebase) {
+                const bool ex = softmax_pass();
+                rebase = bar_softmax_or(ex);
+              }
+              if (__builtin_expect(rebase, 0)) {
+                // ---- per-head maximum score of the tile -> new references; O and l of this sequence rescaled
+                float tm[NH];
+                {
+                  float sv[NH];
+                  tmem_ld<NH>(t_s, sv);
+#pragma unroll
+                  for (int j = 0; j < NH; ++j) {
+                    float x = sv[j] * score_scale;
+#pragma unroll
+                    for (int o = 16; o; o >>= 1) x = fmaxf(x, __shfl_xor_sync(kFull, x, o));
+                    tm[j] = x;
+                  }
+                }
+                if (lane == 0) {
+#pragma unroll
+                  for (int j = 0; j < NH; ++j) sh.wmax[cw][j] = tm[j];
+                }
+                tc_fence_before();
+                bar_softmax();
+                float f[NH];
 #pragma unroll
                 for (int j = 0; j < NH; ++j) {
-                  float x = tok_ok ? sv[j] * score_scale : -INFINITY;
+                  float m = sh.wmax[0][j];
 #pragma unroll
-                  for (int o = 16; o; o >>= 1) x = fmaxf(x, __shfl_xor_sync(kFull, x, o));
-                  tm[j] = x;
+                  for (int w = 1; w < kSoftmaxWarps; ++w) m = fmaxf(m, sh.wmax[w][j]);
+                  const float mold = -nmref[hs][j], mnew = fmaxf(mold, m);
+                  const float fm = (mold == -INFINITY) ? 0.f : ex2(mold - mnew);
+                  nmref[hs][j] = -mnew;
+                  lsum[hs][j] *= fm;
+                  f[j] = fm;
                 }
-              }
-              if (lane == 0) {
+                if (i > 0) {  // every PV of this unit issued so far has to be in O before it is rescaled
+                  mbar_wait(bar_done + 8 * (sb ^ 1), ((gt - 1) >> 1) & 1);
+                  tc_fence_after();
+                  float ov[NH];
+                  const uint32_t t_o = tmem + lane_sel + kColO + 16 * hs;   // channel r, heads of sequence hs
+                  tmem_ld<NH>(t_o, ov);
 #pragma unroll
-                for (int j = 0; j < NH; ++j) sh.wmax[cw][j] = tm[j];
+                  for (int j = 0; j < NH; ++j) ov[j] *= f[j];
+                  tmem_st<NH>(t_o, ov);
+                }
+                (void)softmax_pass();
+                bar_softmax();                          // wmax may be rewritten only after every warp read it
               }
-              tc_fence_before();
-              bar_softmax();
-              float f[NH];
 #pragma unroll
-              for (int j = 0; j < NH; ++j) {
-                float m = sh.wmax[0][j];
-#pragma unroll
-                for (int w = 1; w < kSoftmaxWarps; ++w) m = fmaxf(m, sh.wmax[w][j]);
-                const float mold = -nmref[j], mnew = fmaxf(mold, m);
-                const float fm = (mold == -INFINITY) ? 0.f : ex2(mold - mnew);
-                nmref[j] = -mnew;
-                lsum[j] *= fm;
-                f[j] = fm;
-              }
-              if (i > 0) {  // every PV of this unit issued so far has to be in O before it is rescaled
-                mbar_wait(bar_done + 8 * (sb ^ 1), ((gt - 1) >> 1) & 1);
-                tc_fence_after();
-                float ov[NH];
-                const uint32_t t_o = tmem + lane_sel + kColO;      // channel r, heads 0..NH-1
-                tmem_ld<NH>(t_o, ov);
-#pragma unroll
-                for (int j = 0; j < NH; ++j) ov[j] *= f[j];
-                tmem_st<NH>(t_o, ov);
-              }
-              (void)softmax_pass();
-              bar_softmax();                            // wmax may be rewritten only after every warp read it
+              for (int j = 0; j < NH; j += 2)
+                fadd2(lsum[hs][j], lsum[hs][j + 1], lsum[hs][j], lsum[hs][j + 1], lt[j], lt[j + 1]);
             }
-#pragma unroll
-            for (int j = 0; j < NH; j += 2) fadd2(lsum[j], lsum[j + 1], lsum[j], lsum[j + 1], lt[j], lt[j + 1]);
 
-            // ---- S has been read (QK may overwrite the buffer), P is written, O is consistent with mref
+            // ---- S has been read (QK may overwrite the buffer), P is written, O is consistent with the references
             fence_async_smem();
             tc_fence_before();
             __syncwarp();
@@ -754,37 +668,43 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
             ++gt;
           }
 
-          // ============================================================ the unit's (m, l)
+          // ============================================================ the unit's (m, l), sequence by sequence
 #pragma unroll
-          for (int j = 0; j < NH; ++j) {
-            float v = lsum[j];
-#pragma unroll
-            for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
-            lsum[j] = v;
-          }
-          if (lane == 0) {
+          for (int hs = 0; hs < kNS; ++hs) {
 #pragma unroll
             for (int j = 0; j < NH; ++j) {
-              sh.lsum[cw][j] = lsum[j];
-              if (cw == 0) sh.mref[j] = -nmref[j];
-            }
-          }
-          bar_softmax();
-          if (atid < G) {                              // one thread per query head
-            float l = 0.f;
+              float v = lsum[hs][j];
 #pragma unroll
-            for (int w = 0; w < kSoftmaxWarps; ++w) l += sh.lsum[w][atid];
-            ml_out[un.row0 + (long long)atid * num_splits] = make_float2(sh.mref[atid] * 0.6931471805599453f, l);   // natural log
-          }
-          if (un.slots_used > 0) {                     // item finished: its remaining slots are empty
-            const long long row_item = un.row0 - (un.slots_used - 1);
-            const int n_empty = num_splits - un.slots_used;
-            for (int e = atid; e < G * n_empty; e += 32 * kSoftmaxWarps) {
-              const int head = e / n_empty, sl = un.slots_used + (e - head * n_empty);
-              ml_out[row_item + (long long)head * num_splits + sl] = make_float2(-INFINITY, 0.f);
+              for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+              lsum[hs][j] = v;
             }
+            if (lane == 0) {
+#pragma unroll
+              for (int j = 0; j < NH; ++j) {
+                sh.lsum[cw][j] = lsum[hs][j];
+                if (cw == 0) sh.mref[j] = -nmref[hs][j];
+              }
+            }
+            bar_softmax();
+            if (un.b + hs < batch) {
+              const long long row0 = un.row0 + hs * seq_rows;
+              if (atid < G) {                            // one thread per query head
+                float l = 0.f;
+#pragma unroll
+                for (int w = 0; w < kSoftmaxWarps; ++w) l += sh.lsum[w][atid];
+                ml_out[row0 + (long long)atid * num_splits] = make_float2(sh.mref[atid] * 0.6931471805599453f, l);   // natural log
+              }
+              if (un.slots_used > 0) {                   // item finished: its remaining slots are empty
+                const long long row_item = row0 - (un.slots_used - 1);
+                const int n_empty = num_splits - un.slots_used;
+                for (int e = atid; e < G * n_empty; e += 32 * kSoftmaxWarps) {
+                  const int head = e / n_empty, sl = un.slots_used + (e - head * n_empty);
+                  ml_out[row_item + (long long)head * num_splits + sl] = make_float2(-INFINITY, 0.f);
+                }
+              }
+            }
+            bar_softmax();                              // sh.lsum / sh.mref are reused by the next sequence / unit
           }
-          bar_softmax();                                // sh.lsum / sh.mref are reused by the next unit
         }
       };
       if (G > 8) run(std::integral_constant<int, 16>{});
@@ -796,7 +716,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
       // anything.  Stored Vhat = code * 2^(byte - eref + 13) in fp16, written straight into TMEM.
       const int g = q;
       const uint32_t scratch = base + kOffMul + 256 * (cw - kSoftmaxWarps);
-      const uint32_t t_o = tmem + lane_sel + kColO;    // channel r, heads 0..15
+      const uint32_t t_o = tmem + lane_sel + kColO;    // channel r, heads 0..15 of sequence 0 of the group
       Cursor cur;
       sc.start(cur);
       Unit un;
@@ -827,12 +747,15 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
               mbar_wait(bar_sfree + 8 * sb, (gt >> 1) & 1);
               mbar_wait(bar_done + 8 * (sb ^ 1), ((gt - 1) >> 1) & 1);
               tc_fence_after();
-              float ov[16];
-              tmem_ld<16>(t_o, ov);
               const float fe = pow2i(eref - enew);
 #pragma unroll
-              for (int j = 0; j < 16; ++j) ov[j] *= fe;
-              tmem_st<16>(t_o, ov);
+              for (int hs = 0; hs < kNS; ++hs) {
+                float ov[16];
+                tmem_ld<16>(t_o + 16 * hs, ov);
+#pragma unroll
+                for (int j = 0; j < 16; ++j) ov[j] *= fe;
+                tmem_st<16>(t_o + 16 * hs, ov);
+              }
             }
             eref = enew;
           }
@@ -885,12 +808,18 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
         mbar_wait(bar_done + 8 * ((gt - 1) & 1), ((gt - 1) >> 1) & 1);
         tc_fence_after();
         {
-          float ov[16];
-          tmem_ld<16>(t_o, ov);
           const float vscale = pow2i(eref - 13 - 127);  // stored Vhat = code * 2^(byte - eref + 13)
 #pragma unroll
-          for (int j = 0; j < 16; ++j)
-            if (j < G) partial_acc[(un.row0 + (long long)j * num_splits) * kHeadDim + r] = ov[j] * vscale;
+          for (int hs = 0; hs < kNS; ++hs) {
+            float ov[16];
+            tmem_ld<16>(t_o + 16 * hs, ov);
+            if (un.b + hs < batch) {
+              const long long row0 = un.row0 + (long long)hs * Hq * num_splits;
+#pragma unroll
+              for (int j = 0; j < 16; ++j)
+                if (j < G) partial_acc[(row0 + (long long)j * num_splits) * kHeadDim + r] = ov[j] * vscale;
+            }
+          }
         }
         tc_fence_before();                              // the next unit's first PV overwrites O
       }
@@ -906,129 +835,44 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
 }
 
 }  // namespace
-
-// ---------------------------------------------------------------- host: TMA descriptors (shared with uq_decode_prefix.cu)
-namespace {
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-struct MapEntry {
-  const void* cache;
-  long long records;
-  CUtensorMap map;
-};
-std::mutex g_map_mu;
-MapEntry g_maps[8];
-int g_map_n = 0, g_map_next = 0;
-
-}  // namespace
-
-// 3-D view of the cache for TMA: [record][16 tokens][128 x 4-bit]; box = one page of K codes.
-int32_t k_code_map(const void* cache, long long records, CUtensorMap* out) {
-  std::lock_guard<std::mutex> lock(g_map_mu);
-  for (int i = 0; i < g_map_n; ++i)
-    if (g_maps[i].cache == cache && g_maps[i].records == records) {
-      *out = g_maps[i].map;
-      return UQ_OK;
-    }
-  static EncodeTiledFn encode = nullptr;
-  if (!encode) {
-    void* fn = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
-    if (e != cudaSuccess || fn == nullptr) {
-      set_error("decode: cuTensorMapEncodeTiled is not available from this driver");
-      return UQ_ERR_CUDA;
-    }
-    encode = (EncodeTiledFn)fn;
-  }
-  const cuuint64_t gdim[3] = {128, 16, (cuuint64_t)records};
-  const cuuint64_t gstr[2] = {64, (cuuint64_t)kRecordBytes};
-  const cuuint32_t box[3] = {128, 16, 1};
-  const cuuint32_t estr[3] = {1, 1, 1};
-  CUtensorMap m;
-  const CUresult cr = encode(&m, CU_TENSOR_MAP_DATA_TYPE_16U4_ALIGN16B, 3, const_cast<void*>(cache), gdim, gstr, box,
-                             estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
-                             CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (cr != CUDA_SUCCESS) {
-    set_error("decode: cuTensorMapEncodeTiled failed with CUresult %d", (int)cr);
-    return UQ_ERR_CUDA;
-  }
-  MapEntry& e = g_maps[g_map_next];
-  e.cache = cache;
-  e.records = records;
-  e.map = m;
-  g_map_next = (g_map_next + 1) % 8;
-  if (g_map_n < 8) ++g_map_n;
-  *out = m;
-  return UQ_OK;
-}
-
-// 2-D view of q_fp8 for TMA: [batch * Hq rows][128 bytes]; box = 16 rows (the heads of one kv head, padded).
-int32_t q_map(const void* q_fp8, long long rows, CUtensorMap* out) {
-  std::lock_guard<std::mutex> lock(g_map_mu);
-  static EncodeTiledFn encode = nullptr;
-  if (!encode) {
-    void* fn = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
-    if (e != cudaSuccess || fn == nullptr) {
-      set_error("decode: cuTensorMapEncodeTiled is not available from this driver");
-      return UQ_ERR_CUDA;
-    }
-    encode = (EncodeTiledFn)fn;
-  }
-  const cuuint64_t gdim[2] = {128, (cuuint64_t)rows};
-  const cuuint64_t gstr[1] = {128};
-  const cuuint32_t box[2] = {128, 16};
-  const cuuint32_t estr[2] = {1, 1};
-  const CUresult cr = encode(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(q_fp8), gdim, gstr, box, estr,
-                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
-                             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (cr != CUDA_SUCCESS) {
-    set_error("decode: cuTensorMapEncodeTiled (q_fp8) failed with CUresult %d", (int)cr);
-    return UQ_ERR_CUDA;
-  }
-  return UQ_OK;
-}
-
 }  // namespace uq
 
-
-extern "C" int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, const void* cache,
-                                       int64_t num_pages, const int32_t* block_tables, int32_t max_pages,
-                                       const int32_t* seq_lens, int32_t batch, int32_t num_splits,
-                                       float* partial_acc, float* partial_ml, void* stream) {
+extern "C" int32_t uq_decode_prefix_attention(const uq_config* cfg, const void* q_fp8, const void* cache,
+                                              int64_t num_pages, const int32_t* block_tables, int32_t max_pages,
+                                              int32_t batch, int32_t prefix_len, int32_t num_splits,
+                                              float* partial_acc, float* partial_ml, void* stream) {
   using namespace uq;
   int32_t st = check_config(cfg);
   if (st != UQ_OK) return st;
-  if (!q_fp8 || !cache || !block_tables || !seq_lens || !partial_acc || !partial_ml || batch <= 0 ||
-      num_splits <= 0 || max_pages <= 0 || num_pages <= 0) {
-    set_error("decode: NULL pointer or non-positive size");
+  if (!q_fp8 || !cache || !block_tables || !partial_acc || !partial_ml || batch <= 0 || max_pages <= 0 ||
+      num_pages <= 0) {
+    set_error("decode_prefix: NULL pointer or non-positive size");
+    return UQ_ERR_INVALID_ARG;
+  }
+  if (prefix_len <= 0 || prefix_len % 128 != 0 || prefix_len / kPage > max_pages) {
+    set_error("decode_prefix: prefix_len must be a positive multiple of 128 tokens within max_pages");
+    return UQ_ERR_INVALID_ARG;
+  }
+  if (num_splits < 2) {
+    set_error("decode_prefix: num_splits must be at least 2");
     return UQ_ERR_INVALID_ARG;
   }
   if (((uintptr_t)cache & 31u) || ((uintptr_t)q_fp8 & 15u) || ((uintptr_t)partial_acc & 15u) ||
       ((uintptr_t)partial_ml & 7u)) {
-    set_error("decode: misaligned pointer (cache 32 B, q_fp8 16 B, partial_acc 16 B, partial_ml 8 B)");
+    set_error("decode_prefix: misaligned pointer (cache 32 B, q_fp8 16 B, partial_acc 16 B, partial_ml 8 B)");
     return UQ_ERR_INVALID_ARG;
   }
   const long long records = (long long)num_pages * cfg->num_kv_heads;
   if (records > 0x7fffffffLL) {
-    set_error("decode: num_pages * num_kv_heads must be < 2^31");
+    set_error("decode_prefix: num_pages * num_kv_heads must be < 2^31");
     return UQ_ERR_INVALID_ARG;
   }
-  CUtensorMap tmap;
+  CUtensorMap tmap, tmap_q;
   st = k_code_map(cache, records, &tmap);
   if (st != UQ_OK) return st;
-  CUtensorMap tmap_q;
   st = q_map(q_fp8, (long long)batch * cfg->num_q_heads, &tmap_q);
   if (st != UQ_OK) return st;
   const float score_scale = resolved_sm_scale(cfg) * 1.4426950408889634f;
-  if (batch > kMaxBatch) {
-    set_error("decode: batch %d exceeds the supported maximum of %d sequences per call", batch, kMaxBatch);
-    return UQ_ERR_UNSUPPORTED;
-  }
   static int sm_count = 0;
   if (sm_count == 0) {
     int dev = 0, v = 0;
@@ -1036,19 +880,17 @@ extern "C" int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, 
         cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) sm_count = v;
     else sm_count = 148;
   }
-  const long long slots = (long long)sm_count * UQ_CTAS_PER_SM;
-  const long long items = (long long)batch * cfg->num_kv_heads;
-  // num_splits == 1: a CTA per item (round-robin beyond the resident set); otherwise one balanced tile range per CTA
-  const dim3 grid((unsigned)((num_splits == 1 && items < slots) ? items : slots));
+  const long long total = (long long)((batch + kNS - 1) / kNS) * cfg->num_kv_heads * (prefix_len / 128);
+  const dim3 grid((unsigned)(total < sm_count ? total : sm_count));   // one CTA per SM, one balanced tile range each
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
-    if (e != cudaSuccess) return check_cuda(e, "decode: cudaFuncSetAttribute");
+    cudaError_t e = cudaFuncSetAttribute(decode_prefix_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e != cudaSuccess) return check_cuda(e, "decode_prefix: cudaFuncSetAttribute");
     attr_set = true;
   }
-  return check_cuda(launch_pdl(decode_kernel, grid, dim3(kThreads), (size_t)kSmemBytes, (cudaStream_t)stream, tmap, tmap_q,
-                               (const uint8_t*)cache, block_tables, (int)max_pages, seq_lens, (int)batch,
-                               (int)cfg->num_q_heads, (int)cfg->num_kv_heads, (int)num_splits, score_scale, partial_acc,
-                               partial_ml),
-                    "uq_decode_attention launch");
+  return check_cuda(launch_pdl(decode_prefix_kernel, grid, dim3(kThreads), (size_t)kSmemBytes, (cudaStream_t)stream, tmap,
+                               tmap_q, (const uint8_t*)cache, block_tables, (int)max_pages, (int)(prefix_len / 128),
+                               (int)batch, (int)cfg->num_q_heads, (int)cfg->num_kv_heads, (int)num_splits, score_scale,
+                               partial_acc, partial_ml),
+                    "uq_decode_prefix_attention launch");
 }

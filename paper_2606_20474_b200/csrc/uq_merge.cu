@@ -89,6 +89,47 @@ merge_kernel(const float* __restrict__ acc, const float* __restrict__ ml, int ro
   *reinterpret_cast<uint2*>(out + (long long)row * kHeadDim + 4 * lane) = packed;
 }
 
+// Two sets of partials per row (shared-prefix decode: the prefix slots and the suffix slots live in separate
+// arrays).  One warp per row, a lane owns 4 channels; first the maximum over both sets, then the weighted sums.
+__global__ void __launch_bounds__(128)
+merge2_kernel(const float* __restrict__ acc_a, const float* __restrict__ ml_a, int Sa, const float* __restrict__ acc_b,
+              const float* __restrict__ ml_b, int Sb, int rows, __nv_bfloat16* __restrict__ out) {
+  pdl_launch_dependents();
+  pdl_wait();
+  const int lane = threadIdx.x & 31;
+  const int row = blockIdx.x * 4 + (threadIdx.x >> 5);
+  if (row >= rows) return;
+  const float2* mla = reinterpret_cast<const float2*>(ml_a) + (long long)row * Sa;
+  const float2* mlb = reinterpret_cast<const float2*>(ml_b) + (long long)row * Sb;
+  const float4* aa = reinterpret_cast<const float4*>(acc_a) + (long long)row * Sa * 32 + lane;
+  const float4* ab = reinterpret_cast<const float4*>(acc_b) + (long long)row * Sb * 32 + lane;
+  float M = -INFINITY;
+  for (int s = 0; s < Sa + Sb; ++s) {
+    const float2 v = s < Sa ? mla[s] : mlb[s - Sa];
+    if (v.y > 0.0f) M = fmaxf(M, v.x);
+  }
+  float4 num = make_float4(0.f, 0.f, 0.f, 0.f);
+  float den = 0.f;
+  for (int s = 0; s < Sa + Sb; ++s) {
+    const float2 v = s < Sa ? mla[s] : mlb[s - Sa];
+    if (!(v.y > 0.0f)) continue;                       // empty slot
+    const float4 a = s < Sa ? aa[(long long)s * 32] : ab[(long long)(s - Sa) * 32];
+    const float w = __expf(v.x - M);
+    num.x = fmaf(w, a.x, num.x);
+    num.y = fmaf(w, a.y, num.y);
+    num.z = fmaf(w, a.z, num.z);
+    num.w = fmaf(w, a.w, num.w);
+    den = fmaf(w, v.y, den);
+  }
+  const float inv = den > 0.f ? 1.0f / den : 0.f;
+  __nv_bfloat162 lo = __floats2bfloat162_rn(num.x * inv, num.y * inv);
+  __nv_bfloat162 hi = __floats2bfloat162_rn(num.z * inv, num.w * inv);
+  uint2 packed;
+  packed.x = *reinterpret_cast<uint32_t*>(&lo);
+  packed.y = *reinterpret_cast<uint32_t*>(&hi);
+  *reinterpret_cast<uint2*>(out + (long long)row * kHeadDim + 4 * lane) = packed;
+}
+
 }  // namespace
 }  // namespace uq
 
@@ -109,4 +150,24 @@ extern "C" int32_t uq_merge_splits(const uq_config* cfg, const float* partial_ac
   return check_cuda(launch_pdl(merge_kernel, dim3((rows + 3) / 4), dim3(128), 0, (cudaStream_t)stream, partial_acc,
                                partial_ml, rows, (int)num_splits, (__nv_bfloat16*)out_bf16),
                     "uq_merge_splits launch");
+}
+
+extern "C" int32_t uq_merge_splits2(const uq_config* cfg, const float* acc_a, const float* ml_a, int32_t splits_a,
+                                    const float* acc_b, const float* ml_b, int32_t splits_b, int32_t batch,
+                                    void* out_bf16, void* stream) {
+  using namespace uq;
+  int32_t st = check_config(cfg);
+  if (st != UQ_OK) return st;
+  if (batch <= 0 || splits_a <= 0 || splits_b <= 0 || !acc_a || !ml_a || !acc_b || !ml_b || !out_bf16) {
+    set_error("merge2: NULL pointer or non-positive batch/splits");
+    return UQ_ERR_INVALID_ARG;
+  }
+  if ((((uintptr_t)acc_a | (uintptr_t)acc_b) & 15u) || (((uintptr_t)ml_a | (uintptr_t)ml_b | (uintptr_t)out_bf16) & 7u)) {
+    set_error("merge2: misaligned pointer (partial_acc 16 B, partial_ml 8 B, out 8 B)");
+    return UQ_ERR_INVALID_ARG;
+  }
+  const int rows = batch * cfg->num_q_heads;
+  return check_cuda(launch_pdl(merge2_kernel, dim3((rows + 3) / 4), dim3(128), 0, (cudaStream_t)stream, acc_a, ml_a,
+                               (int)splits_a, acc_b, ml_b, (int)splits_b, rows, (__nv_bfloat16*)out_bf16),
+                    "uq_merge_splits2 launch");
 }

@@ -616,3 +616,36 @@ def test_calibrate_c_other_codebooks_and_fixed_scale():
         ref, ref_nrm = oracle.calib_sq_err(H.bits(u), cs, rotate=False, scale_mode=mode, levels=lev)
         np.testing.assert_allclose(sq.cpu().numpy(), ref, rtol=1e-11, atol=0)
         assert float(nrm.cpu()[0]) == pytest.approx(ref_nrm, rel=1e-11)
+
+
+@pytest.mark.parametrize("hq,hkv,lens,prefix,pfx_call,splits", [
+    (16, 2, [700, 512, 1300, 497, 900], 496, 384, (2, 3)),          # G = 8, odd batch: the last group has one sequence
+    (32, 2, [1500, 1500, 2100, 1281], 1280, 1280, (3, 2)),          # G = 16, a sequence with a 1-token suffix
+    (16, 1, [640, 640], 640, 640, (2, 2)),                           # no suffix at all: every suffix slot empty
+])
+def test_shared_prefix_decode_matches_the_oracle_and_the_plain_decode(hq, hkv, lens, prefix, pfx_call, splits):
+    """uq_decode_prefix_attention + suffix decode + uq_merge_splits2 on sequences whose block
+    tables name the same prefix pages: outputs within tolerance of the float64 oracle for every sequence, and within
+    twice that of the plain decode of the same cache (two roundings of the same quantities)."""
+    wl = W.make_custom("pfx", 300 + hq + len(lens), lens, hq, hkv, prefix_len=prefix, peaked_frac=0.05)
+    cfg = H.cfg_of(wl)
+    cache, bt = H.fill_cache(cfg, wl, DEV)
+    q = W.gen_q(wl, DEV)
+    plain, q_fp8, bufs = H.run_decode(cfg, cache, bt, wl.ctx_lens, q, 3)
+    B = wl.batch
+    sp, ss = splits
+    bufs2 = uq.StepBuffers(cfg, B, ss, DEV)
+    bufs2.q_fp8.copy_(q_fp8)
+    pb = uq.PrefixBuffers(cfg, B, sp, DEV)
+    pb.suffix_lens.copy_(torch.from_numpy((wl.ctx_lens - pfx_call).astype(np.int32)))
+    bufs2.partial_acc.fill_(float("nan")); pb.partial_acc.fill_(float("nan"))   # every slot has to be written
+    bufs2.partial_ml.fill_(float("nan")); pb.partial_ml.fill_(float("nan"))
+    out = uq.decode_attention_shared_prefix(cfg, bufs2, pb, cache, bt, pfx_call)
+    torch.cuda.synchronize()
+    out = out.float().cpu().numpy().astype(np.float64)
+    assert np.isfinite(out).all()
+    for b in range(B):
+        ref, _ = H.oracle_out(wl, b, int(wl.ctx_lens[b]), H.bits(q)[b])
+        H.check_out(out[b], ref, f"shared prefix seq {b}")
+    pl = plain.float().cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(out - pl) <= 2 * (H.ATOL + H.RTOL * np.abs(pl)))
