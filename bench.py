@@ -220,7 +220,22 @@ def run_ours(args, rank, world, local_rank):
         step_graphs = [uq.StepGraph(cfg, bufs, qs[j], kvs[j][0], kvs[j][1], cu_dev, before_dev, after_dev, bt_dev, cache)
                        for j in range(n_in)]
 
+    # --shared-prefix 1 (configs with a shared prefix): the prefix through uq_decode_prefix_attention (two sequences per
+    # prefix tile), the private suffixes through uq_decode_attention, uq_merge_splits2 over both sets of partials
+    pbufs, pfx = None, 0
+    if args.shared_prefix and wl.prefix_len >= 128:
+        pfx = (int(wl.prefix_len) // 128) * 128
+        pbufs = uq.PrefixBuffers(cfg, B, 2, dev)
+        pbufs.suffix_lens.copy_(torch.from_numpy((ctx_after - pfx).astype(np.int32)))
+        S_suffix = args.splits or uq.suggest_num_splits(cfg, B, max(1, int((ctx_after - pfx).mean())))
+        bufs_sp = uq.StepBuffers(cfg, B, S_suffix, dev)
+
     def step(i):
+        if pbufs is not None:
+            k_new, v_new = kvs[i % n_in]
+            uq.rotate_quantize_append(cfg, k_new, v_new, cu_dev, before_dev, bt_dev, cache, q=qs[i % n_in],
+                                      q_fp8=bufs_sp.q_fp8, stream=stream)
+            return uq.decode_attention_shared_prefix(cfg, bufs_sp, pbufs, cache, bt_dev, pfx, stream=stream)
         if step_graphs is not None:
             return step_graphs[i % n_in].launch()
         k_new, v_new = kvs[i % n_in]
@@ -331,7 +346,7 @@ def run_ours(args, rank, world, local_rank):
             "note": "bytes_per_step / value / roofline count LOGICAL bytes; the prefix pages are named by every block "
                     "table and read from HBM once per step (L2 serves the rest), so the fractions of the HBM peak can "
                     "exceed what HBM alone delivers",
-            "prefix_tokens": int(wl.prefix_len),
+            "prefix_tokens": int(wl.prefix_len), "shared_prefix_decode": bool(args.shared_prefix),
             "physical_kv_bytes_per_step": int((int(ctx_after.astype(np.int64).sum()) - (B - 1) * int(wl.prefix_len))
                                               * Hkv * 136)}} if wl.prefix_len else {}),
         "frac_of_nominal_8TBs": round(value / world / NOMINAL_HBM_GBS, 4),
@@ -584,6 +599,8 @@ def main():
                     help="BASELINE.json config number (1-based); 2 is the one the metric is quoted on")
     ap.add_argument("--splits", type=int, default=0, help="num_splits override (0 = uq_suggest_num_splits)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--shared-prefix", type=int, default=0, choices=[0, 1],
+                    help="1 (config 4): the timed step decodes the shared prefix with uq_decode_prefix_attention")
     ap.add_argument("--graph", type=int, default=0, choices=[0, 1],
                     help="1: the timed steps are launches of uq.StepGraph (one CUDA graph per step)")
     ap.add_argument("--bulk-seqs", type=int, default=1, metavar="S",

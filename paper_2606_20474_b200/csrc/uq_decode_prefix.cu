@@ -19,21 +19,36 @@
 namespace uq {
 namespace {
 
-constexpr int kComputeWarps = 8;                     // two per TMEM lane quarter: one softmax warp, one V warp
-constexpr int kSoftmaxWarps = 4;
+#ifndef UQ_PREFIX_GROUPS
+#define UQ_PREFIX_GROUPS 4
+#endif
+constexpr int kSoftGroups = UQ_PREFIX_GROUPS;        // softmax warp groups: each takes kNS / kSoftGroups of the sequences
+constexpr int kSoftmaxWarps = 4;                     // per group: one warp per TMEM lane quarter
+constexpr int kVWarps = 4;
+constexpr int kComputeWarps = kSoftGroups * kSoftmaxWarps + kVWarps;
 constexpr int kIssuerWarps = 4;                      // QK issuer, PV issuer, K producer, V producer
-constexpr int kThreads = (kComputeWarps + kIssuerWarps) * 32;   // 12 warps: registers are allocated per 4 warps anyway
+constexpr int kThreads = (kComputeWarps + kIssuerWarps) * 32;
 #ifndef UQ_PREFIX_NSEQ
-#define UQ_PREFIX_NSEQ 2
+#define UQ_PREFIX_NSEQ 4
 #endif
 constexpr int kNS = UQ_PREFIX_NSEQ;                   // sequences per prefix tile
 constexpr int kNCols = 16 * kNS;                      // score columns: 16 head slots per sequence
+constexpr int kSeqPerGroup = kNS / UQ_PREFIX_GROUPS;
+static_assert(kSeqPerGroup * UQ_PREFIX_GROUPS == kNS, "sequences per tile must divide over the softmax groups");
 #undef UQ_KSTAGES
 #undef UQ_VSTAGES
 #undef UQ_CTAS_PER_SM
+#ifndef UQ_PREFIX_CTAS
+#define UQ_PREFIX_CTAS 1
+#endif
+#if UQ_PREFIX_CTAS == 2
+#define UQ_KSTAGES 3
+#define UQ_VSTAGES 4
+#else
 #define UQ_KSTAGES 4
 #define UQ_VSTAGES 6
-#define UQ_CTAS_PER_SM 1
+#endif
+#define UQ_CTAS_PER_SM UQ_PREFIX_CTAS
 // Two rings: the K codes of a tile (16 KB once the TMA unit has expanded the nibbles) are needed by the QK
 // MMA only and leave early; the rest of the records (V codes, K scales, V scales: 9 KB) stays until the V
 // warps have converted it.  Separate rings let the small one run deep (bytes in flight hide HBM latency).
@@ -67,9 +82,9 @@ constexpr uint32_t kColSFB = 3 * kNCols + 8;    // 4
 #define UQ_VBUFS 2
 #endif
 constexpr int kVBufs = UQ_VBUFS;   // Vhat^T buffers in TMEM
-constexpr uint32_t kColV = 256;    // kVBufs x 64: Vhat^T operand, lane = channel d, column c = tokens 2c, 2c+1 (f16x2)
-constexpr uint32_t kTmemCols = 512;
-static_assert(3 * kNCols + 12 <= 256, "score / accumulator / scale columns must stay below the Vhat buffers");
+constexpr uint32_t kColV = UQ_PREFIX_CTAS == 2 ? 128 : 256;    // kVBufs x 64: Vhat^T operand, lane = channel d, column c = tokens 2c, 2c+1 (f16x2)
+constexpr uint32_t kTmemCols = UQ_PREFIX_CTAS == 2 ? 256 : 512;
+static_assert(3 * kNCols + 12 <= kColV, "score / accumulator / scale columns must stay below the Vhat buffers");
 
 // ---------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -132,12 +147,12 @@ __device__ __forceinline__ bool elect_one() {
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void bar_softmax() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
+__device__ __forceinline__ void bar_softmax(int id) { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
 // barrier over the 128 softmax threads that also ORs a predicate across them
-__device__ __forceinline__ bool bar_softmax_or(bool pred) {
+__device__ __forceinline__ bool bar_softmax_or(int id, bool pred) {
   uint32_t r;
-  asm volatile("{\n.reg .pred p, q;\nsetp.ne.b32 q, %1, 0;\nbar.red.or.pred p, 1, 128, q;\nselp.u32 %0, 1, 0, p;\n}\n"
-               : "=r"(r) : "r"((uint32_t)pred) : "memory");
+  asm volatile("{\n.reg .pred p, q;\nsetp.ne.b32 q, %1, 0;\nbar.red.or.pred p, %2, 128, q;\nselp.u32 %0, 1, 0, p;\n}\n"
+               : "=r"(r) : "r"((uint32_t)pred), "r"(id) : "memory");
   return r != 0;
 }
 
@@ -275,9 +290,9 @@ struct Shared {
   uint64_t done[2];           // PV commit of tile i -> done[i&1]: P / Vhat buffer i&1 free, O up to date
   uint64_t q_full[2];         // TMA: the FP8 query tile of a work unit landed (buffer = unit ordinal & 1)
   uint32_t tmem_base;
-  float wmax[kSoftmaxWarps][16];
-  float lsum[kSoftmaxWarps][16];
-  float mref[16];
+  float wmax[kSoftGroups][kSoftmaxWarps][16];
+  float lsum[kSoftGroups][kSoftmaxWarps][16];
+  float mref[kSoftGroups][16];
 };
 
 // ---------------------------------------------------------------- work schedule
@@ -366,12 +381,12 @@ decode_prefix_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
 #pragma unroll
     for (int s = 0; s < kVStages; ++s) {
       mbar_init(bar_fullv + 8 * s, 1);
-      mbar_init(bar_emptyv + 8 * s, (kComputeWarps - kSoftmaxWarps) + 1);
+      mbar_init(bar_emptyv + 8 * s, kVWarps + 1);
     }
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
       mbar_init(bar_sfull + 8 * h, 1);
-      mbar_init(bar_sfree + 8 * h, kSoftmaxWarps);
+      mbar_init(bar_sfree + 8 * h, kSoftGroups * kSoftmaxWarps);
       mbar_init(bar_done + 8 * h, 1);
       mbar_init(bar_qfull + 8 * h, 1);
       mbar_init(bar_ready + 8 * h, kComputeWarps);
@@ -546,9 +561,11 @@ decode_prefix_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
     const uint32_t lane_sel = (uint32_t)(32 * q) << 16;
     const int r = 32 * q + lane;                       // softmax: token row of the tile; V warps: channel d
 
-    if (cw < kSoftmaxWarps) {
+    if (cw < kSoftGroups * kSoftmaxWarps) {
       // ============================================================== softmax warps
-      const int atid = 32 * cw + lane;                 // 0..127
+      const int grp = cw >> 2, cwl = cw & 3;           // softmax group, warp inside it
+      const int bar_id = 1 + grp;                      // the group's named barrier
+      const int atid = 32 * cwl + lane;                // 0..127 inside the group
       float2* const ml_out = reinterpret_cast<float2*>(partial_ml);
       const long long seq_rows = (long long)Hq * num_splits;   // partial rows of one sequence
 
@@ -560,11 +577,11 @@ decode_prefix_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
         int gt = 0;                                    // global tile counter
         const uint32_t p_row = sP + (r >> 3) * (256 * kNS) + (r & 7) * 16;
         while (sc.next(cur, un)) {
-          float nmref[kNS][NH], lsum[kNS][NH];         // nmref = minus the per-head reference logit, per sequence
+          float nmref[kSeqPerGroup][NH], lsum[kSeqPerGroup][NH];         // nmref = minus the per-head reference logit, per sequence
 #pragma unroll
-          for (int hs = 0; hs < kNS; ++hs) {
+          for (int hq = 0; hq < kSeqPerGroup; ++hq) {
 #pragma unroll
-            for (int j = 0; j < NH; ++j) { nmref[hs][j] = INFINITY; lsum[hs][j] = 0.f; }
+            for (int j = 0; j < NH; ++j) { nmref[hq][j] = INFINITY; lsum[hq][j] = 0.f; }
           }
 
           for (int i = 0; i < un.n_tiles; ++i) {       // every tile of the prefix is whole: no token mask
@@ -574,7 +591,8 @@ decode_prefix_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
             tc_fence_after();
 
 #pragma unroll
-            for (int hs = 0; hs < kNS; ++hs) {         // the sequences of the group one after the other
+            for (int hq = 0; hq < kSeqPerGroup; ++hq) { // this warp group's sequences one after the other
+              const int hs = grp * kSeqPerGroup + hq;
               const uint32_t t_s = tmem + lane_sel + kColS + kNCols * sb + 16 * hs;
               const uint32_t p_addr = p_row + kPBytes * sb + 256 * hs;   // head-cores 2 hs, 2 hs + 1
               float lt[NH];
@@ -584,7 +602,7 @@ decode_prefix_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
                 tmem_ld<NH>(t_s, t);
 #pragma unroll
                 for (int j = 0; j < NH; j += 2)
-                  ffma2(t[j], t[j + 1], t[j], t[j + 1], score_scale, nmref[hs][j], nmref[hs][j + 1]);
+                  ffma2(t[j], t[j + 1], t[j], t[j + 1], score_scale, nmref[hq][j], nmref[hq][j + 1]);
                 float tmax = t[0];
 #pragma unroll
                 for (int j = 1; j < NH; ++j) tmax = fmaxf(tmax, t[j]);
@@ -605,7 +623,7 @@ decode_prefix_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
               bool rebase = (i == 0);
               if (!rebase) {
                 const bool ex = softmax_pass();
-                rebase = bar_softmax_or(ex);
+                rebase = bar_softmax_or(bar_id, ex);
               }
               if (__builtin_expect(rebase, 0)) {
                 // ---- per-head maximum score of the tile -> new references; O and l of this sequence rescaled
@@ -623,20 +641,20 @@ decode_prefix_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
                 }
                 if (lane == 0) {
 #pragma unroll
-                  for (int j = 0; j < NH; ++j) sh.wmax[cw][j] = tm[j];
+                  for (int j = 0; j < NH; ++j) sh.wmax[grp][cwl][j] = tm[j];
                 }
                 tc_fence_before();
-                bar_softmax();
+                bar_softmax(bar_id);
                 float f[NH];
 #pragma unroll
                 for (int j = 0; j < NH; ++j) {
-                  float m = sh.wmax[0][j];
+                  float m = sh.wmax[grp][0][j];
 #pragma unroll
-                  for (int w = 1; w < kSoftmaxWarps; ++w) m = fmaxf(m, sh.wmax[w][j]);
-                  const float mold = -nmref[hs][j], mnew = fmaxf(mold, m);
+                  for (int w = 1; w < kSoftmaxWarps; ++w) m = fmaxf(m, sh.wmax[grp][w][j]);
+                  const float mold = -nmref[hq][j], mnew = fmaxf(mold, m);
                   const float fm = (mold == -INFINITY) ? 0.f : ex2(mold - mnew);
-                  nmref[hs][j] = -mnew;
-                  lsum[hs][j] *= fm;
+                  nmref[hq][j] = -mnew;
+                  lsum[hq][j] *= fm;
                   f[j] = fm;
                 }
                 if (i > 0) {  // every PV of this unit issued so far has to be in O before it is rescaled
@@ -650,11 +668,11 @@ decode_prefix_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
                   tmem_st<NH>(t_o, ov);
                 }
                 (void)softmax_pass();
-                bar_softmax();                          // wmax may be rewritten only after every warp read it
+                bar_softmax(bar_id);                          // wmax may be rewritten only after every warp read it
               }
 #pragma unroll
               for (int j = 0; j < NH; j += 2)
-                fadd2(lsum[hs][j], lsum[hs][j + 1], lsum[hs][j], lsum[hs][j + 1], lt[j], lt[j + 1]);
+                fadd2(lsum[hq][j], lsum[hq][j + 1], lsum[hq][j], lsum[hq][j + 1], lt[j], lt[j + 1]);
             }
 
             // ---- S has been read (QK may overwrite the buffer), P is written, O is consistent with the references
@@ -670,29 +688,30 @@ decode_prefix_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
 
           // ============================================================ the unit's (m, l), sequence by sequence
 #pragma unroll
-          for (int hs = 0; hs < kNS; ++hs) {
+          for (int hq = 0; hq < kSeqPerGroup; ++hq) {
+            const int hs = grp * kSeqPerGroup + hq;
 #pragma unroll
             for (int j = 0; j < NH; ++j) {
-              float v = lsum[hs][j];
+              float v = lsum[hq][j];
 #pragma unroll
               for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
-              lsum[hs][j] = v;
+              lsum[hq][j] = v;
             }
             if (lane == 0) {
 #pragma unroll
               for (int j = 0; j < NH; ++j) {
-                sh.lsum[cw][j] = lsum[hs][j];
-                if (cw == 0) sh.mref[j] = -nmref[hs][j];
+                sh.lsum[grp][cwl][j] = lsum[hq][j];
+                if (cwl == 0) sh.mref[grp][j] = -nmref[hq][j];
               }
             }
-            bar_softmax();
+            bar_softmax(bar_id);
             if (un.b + hs < batch) {
               const long long row0 = un.row0 + hs * seq_rows;
               if (atid < G) {                            // one thread per query head
                 float l = 0.f;
 #pragma unroll
-                for (int w = 0; w < kSoftmaxWarps; ++w) l += sh.lsum[w][atid];
-                ml_out[row0 + (long long)atid * num_splits] = make_float2(sh.mref[atid] * 0.6931471805599453f, l);   // natural log
+                for (int w = 0; w < kSoftmaxWarps; ++w) l += sh.lsum[grp][w][atid];
+                ml_out[row0 + (long long)atid * num_splits] = make_float2(sh.mref[grp][atid] * 0.6931471805599453f, l);   // natural log
               }
               if (un.slots_used > 0) {                   // item finished: its remaining slots are empty
                 const long long row_item = row0 - (un.slots_used - 1);
@@ -703,7 +722,7 @@ decode_prefix_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
                 }
               }
             }
-            bar_softmax();                              // sh.lsum / sh.mref are reused by the next sequence / unit
+            bar_softmax(bar_id);                              // sh.lsum / sh.mref are reused by the next sequence / unit
           }
         }
       };
@@ -715,7 +734,7 @@ decode_prefix_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
       // group of V): its reference exponent eref is its own, so the four V warps never have to agree on
       // anything.  Stored Vhat = code * 2^(byte - eref + 13) in fp16, written straight into TMEM.
       const int g = q;
-      const uint32_t scratch = base + kOffMul + 256 * (cw - kSoftmaxWarps);
+      const uint32_t scratch = base + kOffMul + 256 * (cw - kSoftGroups * kSoftmaxWarps);
       const uint32_t t_o = tmem + lane_sel + kColO;    // channel r, heads 0..15 of sequence 0 of the group
       Cursor cur;
       sc.start(cur);
@@ -881,7 +900,8 @@ extern "C" int32_t uq_decode_prefix_attention(const uq_config* cfg, const void* 
     else sm_count = 148;
   }
   const long long total = (long long)((batch + kNS - 1) / kNS) * cfg->num_kv_heads * (prefix_len / 128);
-  const dim3 grid((unsigned)(total < sm_count ? total : sm_count));   // one CTA per SM, one balanced tile range each
+  const long long slots = (long long)sm_count * UQ_CTAS_PER_SM;
+  const dim3 grid((unsigned)(total < slots ? total : slots));   // one wave, one balanced tile range per CTA
   static bool attr_set = false;
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(decode_prefix_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
