@@ -4,8 +4,11 @@
 // once for kNS sequences at a time instead of once per sequence.  Same CTA design as uq_decode.cu (read that file
 // first): TMA K / V rings, tcgen05 block-scaled QK, softmax warps with lazy per-head references, V warps writing
 // Vhat^T to TMEM, PV from TMEM — with the score tile widened from 16 to 16 kNS columns (the query tiles of kNS
-// sequences side by side), kNS sets of references and running sums in the softmax warps, and one CTA per SM (the
-// registers and TMEM columns of two).  All items have the same length, so the schedule is plain arithmetic.
+// sequences side by side), one group of four softmax warps per sequence (each with its own named barrier, references
+// and running sums), and one CTA of 24 warps per SM (the TMEM columns and shared memory of two).  All items have the
+// same length, so the schedule is plain arithmetic.
+// Measured on config 4 (256 sequences, 30,000-token prefix): kNS = 2 with one softmax group 1,181 us
+// per step, kNS = 4 with one group 1,222 us, with two groups 1,045 us, with four groups 969 us; the plain kernel 989 us.
 // The partials have the format of include/uq.h; the private suffixes go through uq_decode_attention and both sets
 // are combined by uq_merge_splits2.
 #include <cuda.h>
