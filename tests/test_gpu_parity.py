@@ -239,6 +239,19 @@ def test_full_size_cfg4_shared_prefix_step_sampled():
     out = uq.decode_step(cfg, bufs, q, k_new, v_new, cu, before, after, bt, cache)
     torch.cuda.synchronize()
     out = out.float().cpu().numpy().astype(np.float64)
+    # the same step's decode through the shared-prefix path (bench.py --shared-prefix 1: 29,952 prefix tokens by
+    # uq_decode_prefix_attention, the suffixes by uq_decode_attention, uq_merge_splits2), in bench.py's launch configuration
+    pfx = (int(wl.prefix_len) // 128) * 128
+    suf_tiles = -(-(wl.ctx_lens + 1 - pfx).astype(np.int64) // 128)
+    even = max(1, int(-(-int(suf_tiles.sum()) * wl.num_kv_heads // (2 * 148))))
+    bufs_sp = uq.StepBuffers(cfg, wl.batch, max(2, 2 + int(suf_tiles.max()) // even), DEV)
+    bufs_sp.q_fp8.copy_(bufs.q_fp8)
+    pb = uq.PrefixBuffers(cfg, wl.batch, 2, DEV)
+    pb.suffix_lens.copy_(torch.from_numpy((wl.ctx_lens + 1 - pfx).astype(np.int32)))
+    out_sp = uq.decode_attention_shared_prefix(cfg, bufs_sp, pb, cache, bt, pfx)
+    torch.cuda.synchronize()
+    out_sp = out_sp.float().cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(out_sp - out) <= 2 * (H.ATOL + H.RTOL * np.abs(out)))      # every sequence, against the plain path
     order = np.argsort(wl.ctx_lens)
     for b in (int(order[0]), int(order[len(order) // 2])):          # shortest and median sequence
         L0 = int(wl.ctx_lens[b])
@@ -250,6 +263,7 @@ def test_full_size_cfg4_shared_prefix_step_sampled():
         ref, q8 = H.oracle_out(wl, b, L0 + 1, H.bits(q)[b], arrays)
         assert np.array_equal(bufs.q_fp8[b].cpu().numpy(), q8)
         H.check_out(out[b], ref, f"cfg4 full seq {b}")
+        H.check_out(out_sp[b], ref, f"cfg4 full seq {b}, shared-prefix path")
 
 
 def test_host_staged_step_equals_device_step_and_oracle():
