@@ -229,12 +229,9 @@ def run_ours(args, rank, world, local_rank):
         pbufs.suffix_lens.copy_(torch.from_numpy((ctx_after - pfx).astype(np.int32)))
         # slots of the suffix call: the suffix lengths are far more skewed than the whole lengths (config 4: mean 16.5k,
         # maximum 98k), and the balanced schedule lengthens every CTA's range until the longest item fits into S - 1
-        # of them — so S follows from the longest suffix, which the host knows
-        suf_tiles = -(-(ctx_after - pfx).astype(np.int64) // 128)
-        sms = torch.cuda.get_device_properties(dev).multi_processor_count
-        even = max(1, int(-(-int(suf_tiles.sum()) * Hkv // (2 * sms))))
-        S_suffix = args.splits or max(uq.suggest_num_splits(cfg, B, max(1, int((ctx_after - pfx).mean()))),
-                                      2 + int(suf_tiles.max()) // even)
+        # of them — so S follows from the longest suffix, which the host knows (uq_suggest_num_splits_max)
+        suf = (ctx_after - pfx).astype(np.int64)
+        S_suffix = args.splits or uq.suggest_num_splits_max(cfg, B, max(1, int(suf.mean())), int(suf.max()))
         bufs_sp = uq.StepBuffers(cfg, B, S_suffix, dev)
 
     def step(i):

@@ -213,6 +213,10 @@ int32_t uq_calibrate_c(const uq_config* cfg, const void* x, int64_t n_vec, int32
  * `avg_seq_len` tokens over the current device with room for sequences twice that long (never below 1). */
 int32_t uq_suggest_num_splits(const uq_config* cfg, int32_t batch, int32_t avg_seq_len);
 
+/* Host.  The same with the longest sequence of the call known: enough slots for it at the balanced range length
+ * (a skewed length mix — e.g. the private suffixes of a shared-prefix batch — otherwise stretches every CTA's range). */
+int32_t uq_suggest_num_splits_max(const uq_config* cfg, int32_t batch, int32_t avg_seq_len, int32_t max_seq_len);
+
 #ifdef __cplusplus
 }
 #endif

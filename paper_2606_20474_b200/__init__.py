@@ -27,4 +27,5 @@ from .binding import (  # noqa: F401
     merge_splits,
     rotate_quantize_append,
     suggest_num_splits,
+    suggest_num_splits_max,
 )

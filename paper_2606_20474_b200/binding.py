@@ -75,6 +75,8 @@ def _load():
     lib.uq_calibrate_c.argtypes = [cfgp, vp, i64, i32, vp, i32, i32, vp, vp, vp, vp]
     lib.uq_suggest_num_splits.restype = i32
     lib.uq_suggest_num_splits.argtypes = [cfgp, i32, i32]
+    lib.uq_suggest_num_splits_max.restype = i32
+    lib.uq_suggest_num_splits_max.argtypes = [cfgp, i32, i32, i32]
     _lib = lib
     return lib
 
@@ -113,6 +115,11 @@ def cache_record_bytes(cfg: UQConfig) -> int:
 def suggest_num_splits(cfg: UQConfig, batch: int, avg_seq_len: int) -> int:
     c = cfg.c()
     return int(_load().uq_suggest_num_splits(ctypes.byref(c), int(batch), int(avg_seq_len)))
+
+
+def suggest_num_splits_max(cfg: UQConfig, batch: int, avg_seq_len: int, max_seq_len: int) -> int:
+    c = cfg.c()
+    return int(_load().uq_suggest_num_splits_max(ctypes.byref(c), int(batch), int(avg_seq_len), int(max_seq_len)))
 
 
 def alloc_cache(cfg: UQConfig, num_pages: int, device="cuda") -> torch.Tensor:

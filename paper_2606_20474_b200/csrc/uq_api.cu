@@ -86,3 +86,25 @@ extern "C" int32_t uq_suggest_num_splits(const uq_config* cfg, int32_t batch, in
   if (s > 64) s = 64;
   return (int32_t)s;
 }
+
+extern "C" int32_t uq_suggest_num_splits_max(const uq_config* cfg, int32_t batch, int32_t avg_seq_len,
+                                             int32_t max_seq_len) {
+  // As above with the longest sequence known: the balanced schedule makes every range long enough for the longest
+  // item to fit into num_splits - 1 of them, so a skewed length mix (the private suffixes of a shared-prefix batch:
+  // mean 16k, maximum 98k tokens) needs max_tiles / range + 2 slots or every CTA's range is stretched.
+  const int32_t base = uq_suggest_num_splits(cfg, batch, avg_seq_len);
+  if (uq::check_config(cfg) != UQ_OK || batch <= 0 || max_seq_len <= avg_seq_len) return base;
+  int dev = 0, sms = 148;
+  if (cudaGetDevice(&dev) == cudaSuccess) {
+    int v = 0;
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) sms = v;
+  }
+  const int64_t tiles_avg = ((int64_t)avg_seq_len + 127) / 128 > 0 ? ((int64_t)avg_seq_len + 127) / 128 : 1;
+  const int64_t tiles_max = ((int64_t)max_seq_len + 127) / 128;
+  int64_t range = ((int64_t)batch * cfg->num_kv_heads * tiles_avg + 2 * sms - 1) / (2 * sms);
+  if (range < 1) range = 1;
+  int64_t s = tiles_max / range + 2;
+  if (s < base) s = base;
+  if (s > 64) s = 64;
+  return (int32_t)s;
+}

@@ -242,9 +242,8 @@ def test_full_size_cfg4_shared_prefix_step_sampled():
     # the same step's decode through the shared-prefix path (bench.py --shared-prefix 1: 29,952 prefix tokens by
     # uq_decode_prefix_attention, the suffixes by uq_decode_attention, uq_merge_splits2), in bench.py's launch configuration
     pfx = (int(wl.prefix_len) // 128) * 128
-    suf_tiles = -(-(wl.ctx_lens + 1 - pfx).astype(np.int64) // 128)
-    even = max(1, int(-(-int(suf_tiles.sum()) * wl.num_kv_heads // (2 * 148))))
-    bufs_sp = uq.StepBuffers(cfg, wl.batch, max(2, 2 + int(suf_tiles.max()) // even), DEV)
+    suf = (wl.ctx_lens + 1 - pfx).astype(np.int64)
+    bufs_sp = uq.StepBuffers(cfg, wl.batch, uq.suggest_num_splits_max(cfg, wl.batch, int(suf.mean()), int(suf.max())), DEV)
     bufs_sp.q_fp8.copy_(bufs.q_fp8)
     pb = uq.PrefixBuffers(cfg, wl.batch, 2, DEV)
     pb.suffix_lens.copy_(torch.from_numpy((wl.ctx_lens + 1 - pfx).astype(np.int32)))
