@@ -84,8 +84,9 @@ constexpr uint32_t kColSFB = 3 * kNCols + 8;    // 4
 #define UQ_VBUFS 2
 #endif
 constexpr int kVBufs = UQ_VBUFS;   // Vhat^T buffers in TMEM
-constexpr uint32_t kColV = UQ_PREFIX_CTAS == 2 ? 128 : 256;    // kVBufs x 64: Vhat^T operand, lane = channel d, column c = tokens 2c, 2c+1 (f16x2)
+constexpr uint32_t kColV = UQ_PREFIX_CTAS == 2 ? 128 : (3 * kNCols + 12 + 31) / 32 * 32;    // kVBufs x 64: Vhat^T operand, lane = channel d, column c = tokens 2c, 2c+1 (f16x2)
 constexpr uint32_t kTmemCols = UQ_PREFIX_CTAS == 2 ? 256 : 512;
+static_assert(kColV + 128 <= kTmemCols, "TMEM columns");
 static_assert(3 * kNCols + 12 <= kColV, "score / accumulator / scale columns must stay below the Vhat buffers");
 
 // ---------------------------------------------------------------- PTX wrappers
