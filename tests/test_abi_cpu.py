@@ -55,6 +55,22 @@ def test_host_side_validation(lib):
     assert uq.cache_record_bytes(uq.UQConfig(64, 4, page_size=32)) == 0
 
 
+def test_prefix_decode_and_calibrate_validate_on_the_host(lib):
+    c = uq.UQConfig(64, 4).c()
+    fake = ctypes.c_void_p(0x1000)                          # aligned, never dereferenced: validation comes first
+    f = lib.uq_decode_prefix_attention
+    assert f(ctypes.byref(c), None, None, 1, None, 1, 1, 128, 2, None, None, None) == 1
+    assert f(ctypes.byref(c), fake, fake, 64, fake, 64, 4, 100, 2, fake, fake, None) == 1    # prefix_len % 128
+    assert b"128" in lib.uq_last_error_string()
+    assert f(ctypes.byref(c), fake, fake, 64, fake, 4, 4, 128, 2, fake, fake, None) == 1     # prefix beyond max_pages
+    assert f(ctypes.byref(c), fake, fake, 64, fake, 64, 4, 128, 1, fake, fake, None) == 1    # num_splits < 2
+    g = lib.uq_calibrate_c
+    assert g(ctypes.byref(c), fake, 8, 1, fake, 4, 3, None, fake, fake, None) == 1           # scale_mode out of range
+    assert g(ctypes.byref(c), fake, 8, 1, fake, 4, 1, fake, fake, fake, None) == 1           # power-of-two scale + levels
+    assert lib.uq_merge_splits2(ctypes.byref(c), None, None, 2, None, None, 2, 1, None, None) == 1
+    assert uq.suggest_num_splits_max(uq.UQConfig(64, 4), 256, 16500, 98000) > uq.suggest_num_splits(uq.UQConfig(64, 4), 256, 16500)
+
+
 def test_binding_refuses_cpu_tensors(lib):
     import torch
     cfg = uq.UQConfig(8, 1)
