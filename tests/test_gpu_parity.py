@@ -635,6 +635,8 @@ def test_calibrate_c_other_codebooks_and_fixed_scale():
     (16, 2, [700, 512, 1300, 497, 900], 496, 384, (2, 3)),          # G = 8, odd batch: the last group has one sequence
     (32, 2, [1500, 1500, 2100, 1281], 1280, 1280, (3, 2)),          # G = 16, a sequence with a 1-token suffix
     (16, 1, [640, 640], 640, 640, (2, 2)),                           # no suffix at all: every suffix slot empty
+    (2, 2, [129], 128, 128, (2, 1)),                                 # one sequence, G = 1, a single prefix tile
+    (8, 2, [300 + 7 * i for i in range(37)], 256, 256, (4, 2)),      # 37 sequences (10 groups of 4, the last with 1), G = 4
 ])
 def test_shared_prefix_decode_matches_the_oracle_and_the_plain_decode(hq, hkv, lens, prefix, pfx_call, splits):
     """uq_decode_prefix_attention + suffix decode + uq_merge_splits2 on sequences whose block
