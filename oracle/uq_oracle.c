@@ -21,7 +21,11 @@
  * level, scale thresholds, statistical fingerprints, the paper's two constants
  * (0.156 / 0.195), library E2M1/E4M3 casts, softmax closed forms, torch SDPA; the Eq.(2)
  * objective (O11) against an independent numpy quantiser, exactly representable inputs
- * (zero error), the rotation's norm invariance and the paper's ordering of c (P11).
+ * (zero error), the rotation's norm invariance and the paper's ordering of c (P11);
+ * uqo_encode_q element for element against hadamard + e4m3_encode and against the library
+ * cast of an independently rotated query, on random / one-hot / saturating rows (P12);
+ * uqo_attention_dense against float64 SDPA and the L = 1 / equal-keys / dominant-key closed
+ * forms (P13).
  * Parity unpinned: the attention *output values* for concrete inputs (the paper
  * prints no worked example) — pinned only through the closed forms above.
  */

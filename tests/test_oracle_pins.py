@@ -468,3 +468,86 @@ def test_k_is_rotated_and_v_is_not():
             p, s = oracle.quantize_vector(y, float(np.float32(0.156)))
             assert np.array_equal(p, kc[t, h]) and np.array_equal(s, ks[t, h])
     assert kc.shape[-1] + ks.shape[-1] == 68 and vc.shape[-1] + vs.shape[-1] == 68
+
+
+# ----------------------------------------------------------------------------- P12 query encoder (Alg. 1 l.6)
+@pytest.mark.parametrize("d", [64, 128, 256])
+def test_p12_encode_q_is_e4m3_of_the_rotated_query_element_for_element(d):
+    """`encode_q` (Alg. 1 l.6: "Q <- R*Q; Q <- cast_fp8_e4m3(Q)") against its parts, each pinned on its own
+    (P1 the rotation, P8 the cast): byte i of row n == e4m3_encode(hadamard(bf16_to_double(row n))[i]), on random rows,
+    one-hot rows (every rotated element +-kappa*x: a missing rotation or a wrong kappa changes every byte), rows that
+    saturate (|Rq| > 448), rows with a single non-zero in the LAST channel (element order / transposed index), huge,
+    tiny and zero rows.  Then against the library cast (torch float8_e4m3fn, P8) of an independently rotated query
+    (numpy float64 matmul with the Sylvester matrix built here) wherever that cast is defined (|y| < 464)."""
+    rng = np.random.default_rng(120 + d)
+    rows = [rng.standard_normal(d) for _ in range(6)]
+    e = np.zeros(d); e[0] = 3.0; rows.append(e)                       # one-hot, first channel: all +3*kappa
+    e = np.zeros(d); e[d - 1] = -2.5; rows.append(e)                  # one-hot, last channel: signs follow popcount(i & (d-1))
+    e = np.zeros(d); e[5] = 1.0; e[d // 2 + 1] = -7.0; rows.append(e)
+    rows.append(np.full(d, 448.0 / math.sqrt(d) * 1.5))               # rotated element 0 = 672 > 448: saturates, the rest 0
+    rows.append(rng.standard_normal(d) * 300.0)                       # many elements beyond 448
+    rows.append(rng.standard_normal(d) * 1e-3)                        # subnormal E4M3 range
+    rows.append(rng.standard_normal(d) * 1e20)
+    rows.append(rng.standard_normal(d) * 1e-20)
+    rows.append(np.zeros(d))
+    x = torch.from_numpy(np.stack(rows).astype(np.float32)).to(torch.bfloat16)
+    bits = x.view(torch.uint16).numpy()
+    got = oracle.encode_q(bits)
+    assert got.shape == bits.shape and got.dtype == np.uint8
+    # (a) element for element against the pinned parts
+    for n in range(bits.shape[0]):
+        y = oracle.hadamard(oracle.bf16_to_double(bits[n]))
+        want = np.array([oracle.e4m3_encode(float(v)) for v in y], np.uint8)
+        assert np.array_equal(got[n], want), f"row {n}"
+    # (b) against an independent rotation + the library cast
+    i, j = np.meshgrid(np.arange(d), np.arange(d), indexing="ij")
+    H = 1.0 - 2.0 * (np.vectorize(lambda a: bin(a).count("1"))(i & j) & 1)
+    y_ind = (H @ x.double().numpy().T).T * (2.0 ** (-0.5 * math.log2(d)))
+    ok = np.abs(y_ind) < 448.0
+    lib = torch.from_numpy(y_ind).to(torch.float8_e4m3fn).view(torch.uint8).numpy()
+    lib = np.where((lib & 0x7F) == 0, 0, lib)                          # -0 is never stored (reading G7)
+    # y_ind carries float64 rounding of the kappa product only when d is an odd power of two; a value within 1e-12
+    # relative of an E4M3 rounding boundary could flip there, everything else must agree exactly
+    mism = (got != lib) & ok
+    assert mism.sum() == 0, f"{int(mism.sum())} bytes differ from the library cast"
+    sat = np.abs(y_ind) >= 448.0
+    assert np.all((got[sat] & 0x7F) == 0x7E)                           # saturation to +-448 (reading G9)
+    assert sat.sum() >= d // 4                                         # the saturating rows really saturate
+    # one-hot rows: every byte is the same magnitude, signs follow the Sylvester pattern of that column
+    mag = got[6] & 0x7F
+    assert len(set(mag.tolist())) == 1 and np.all(got[6] < 0x80)
+    pop = np.array([bin(a & (d - 1)).count("1") & 1 for a in range(d)])
+    assert np.array_equal(got[7] >> 7, 1 - pop)                        # x = -2.5 e_{d-1}: y_i = -2.5 kappa (-1)^popcount(i)
+
+
+# ----------------------------------------------------------------------------- P13 unquantised attention (context figure)
+def test_p13_attention_dense_against_sdpa_and_closed_forms():
+    """`attention_dense` (textbook softmax attention over unquantised doubles; feeds only the context figure
+    quant_error_vs_bf16) against torch float64 SDPA (library routine) with GQA, a non-default scale, and the closed
+    forms: L = 1 -> out = v_0; all keys equal -> the mean of v; one dominant key -> its value; L = 0 -> zeros."""
+    rng = np.random.default_rng(13)
+    Hq, Hkv, d, L = 12, 3, 64, 91
+    G = Hq // Hkv
+    q = rng.standard_normal((Hq, d)); k = rng.standard_normal((L, Hkv, d)); v = rng.standard_normal((L, Hkv, d))
+    for scale in (None, 0.3):
+        out = oracle.attention_dense(q, k, v, scale)
+        tq = torch.from_numpy(q)[None, :, None, :]
+        tk = torch.from_numpy(k).permute(1, 0, 2).repeat_interleave(G, dim=0)[None]
+        tv = torch.from_numpy(v).permute(1, 0, 2).repeat_interleave(G, dim=0)[None]
+        ref = torch.nn.functional.scaled_dot_product_attention(tq, tk, tv, scale=scale)[0, :, 0].numpy()
+        assert np.allclose(out, ref, atol=1e-13)
+        assert not np.allclose(out[0], ref[G], atol=1e-6)              # contiguous GQA groups, not interleaved
+    out1 = oracle.attention_dense(q, k[:1], v[:1])
+    for h in range(Hq):
+        assert np.array_equal(out1[h], v[0, h // G])
+    keq = np.repeat(k[:1], L, axis=0)
+    oeq = oracle.attention_dense(q, keq, v)
+    for h in range(Hq):
+        assert np.allclose(oeq[h], v[:, h // G].mean(axis=0), atol=1e-13)
+    kd = k.copy(); kd[17] = 0.0
+    qd = np.zeros((Hq, d)); qd[:, 3] = 1.0
+    kd[:, :, 3] = 0.0; kd[17, :, 3] = 4000.0                           # logit 4000/8 = 500 above all others
+    od = oracle.attention_dense(qd, kd, v)
+    for h in range(Hq):
+        assert np.allclose(od[h], v[17, h // G], atol=1e-13)
+    assert np.array_equal(oracle.attention_dense(q, k[:0], v[:0]), np.zeros((Hq, d)))
