@@ -22,7 +22,11 @@
  *  - Every function returns a status code; no C++ exception crosses the boundary.
  *    uq_last_error_string() (host, thread-local) describes the last failure.
  *  - Arguments are validated on the host only.  Block-table entries outside [0, num_pages),
- *    seq_lens beyond max_pages*page_size, NaN/Inf inputs: undefined behaviour.
+ *    seq_lens beyond max_pages*page_size, NaN/Inf inputs: undefined behaviour — unless
+ *    UQ_FLAG_DEBUG_CHECKS is set (below), which validates the tables on the device first.
+ *  - The library may be used on several devices of one process: a call runs on the CURRENT device
+ *    (cudaSetDevice), which must own every pointer passed; per-device state (SM count, shared-memory
+ *    opt-in of the kernels, TMA descriptors) is kept per device and guarded by mutexes.
  *  - Supported geometry in this version: head_dim = 128, group_size = 32, page_size = 16,
  *    num_q_heads / num_kv_heads in 1..16, batch <= 2048 for uq_decode_attention
  *    (UQ_ERR_UNSUPPORTED otherwise).
@@ -59,7 +63,7 @@ extern "C" {
 #define UQ_OK 0
 #define UQ_ERR_INVALID_ARG 1  /* null pointer, non-positive size, Hq % Hkv != 0, misaligned pointer */
 #define UQ_ERR_UNSUPPORTED 2  /* geometry outside the supported set above */
-#define UQ_ERR_WORKSPACE 3    /* reserved */
+#define UQ_ERR_WORKSPACE 3    /* reserved: no entry point takes a workspace (uq_decode_workspace_bytes reports 0) */
 #define UQ_ERR_CUDA 4         /* launch / driver error */
 
 #define UQ_RECORD_BYTES 2176  /* 16 tokens * (64 + 4 + 64 + 4) bytes */
@@ -67,6 +71,15 @@ extern "C" {
 /* uq_config.flags: keep uq_rotate_quantize_append on the one-warp-per-octet kernel even for prefill-sized calls
  * (the bytes written do not depend on it; tests use it to cover both kernels on the same inputs). */
 #define UQ_FLAG_NO_BULK_APPEND 1u
+/* uq_config.flags: debug mode.  uq_rotate_quantize_append, uq_decode_attention and uq_decode_prefix_attention first run a
+ * small kernel over exactly the table entries and lengths the call is going to use — decode: 0 <= seq_lens[b] <=
+ * max_pages*page_size and every entry of pages [0, ceil(seq_lens[b]/page_size)) inside [0, num_pages); append: cu_new
+ * starts at 0, ends at total_new and does not decrease, seq_lens[b] + count fits the table, the entries of the pages
+ * written are in range; shared prefix: the prefix entries are in range AND equal to sequence 0's — then copy a five-word
+ * report to the host and SYNCHRONISE the stream (the one exception to "never synchronises"; such a call cannot be captured
+ * into a CUDA graph).  On an offender the call returns UQ_ERR_INVALID_ARG, names the first one in uq_last_error_string()
+ * and launches nothing else.  Without the flag none of this runs. */
+#define UQ_FLAG_DEBUG_CHECKS 2u
 
 typedef struct {
   int32_t num_q_heads;   /* e.g. 64 */
@@ -85,6 +98,12 @@ const char* uq_last_error_string(void);
 
 /* Host.  Bytes of one (page, kv_head) record: page_size*(d/2 + d/32)*2 = 2176; 0 if unsupported. */
 size_t uq_cache_record_bytes(const uq_config* cfg);
+
+/* Host.  Device scratch uq_decode_attention / uq_decode_prefix_attention need beyond the caller's partial buffers for
+ * `batch` sequences and `num_splits` slots: *bytes = 0 in this version — the schedule (tile prefix sums of up to 2048
+ * sequences), the K / V rings, the operands and the accumulators live in shared memory and TMEM, which is why those
+ * entry points take no workspace argument.  Kept so that a caller sizing its arena does not have to know that. */
+int32_t uq_decode_workspace_bytes(const uq_config* cfg, int32_t batch, int32_t num_splits, size_t* bytes);
 
 /*
  * Alg. 1 "Write" l.1-5 and "Decode" l.6: quantize-on-append.
@@ -142,7 +161,9 @@ int32_t uq_rotate_quantize_append(const uq_config* cfg, const void* k_new, const
  *     m_s   = a reference logit of split s (>= every z_t of the split minus 12*ln2; it need
  *             not be the exact maximum),  l_s = sum_t exp(z_t - m_s),
  *     acc_s = sum_t exp(z_t - m_s) * vhat_t   (unnormalised).
- * An empty split writes m_s = -inf, l_s = 0, acc_s = 0.
+ * An empty split (a slot its item does not use, or any slot of a sequence of length 0) writes m_s = -inf, l_s = 0;
+ * its acc_s row is NOT written and must not be read: a merge skips every slot with l_s = 0 (uq_merge_splits does),
+ * it must not multiply a weight of 0 into the row (stale memory may hold NaN).
  *
  * Arithmetic: S = K Q^T by tcgen05.mma kind::mxf8f6f4.block_scale (E2M1 x E4M3 products exact,
  * UE8M0 group scales applied by the tensor core, fp32 accumulation in TMEM); exp in fp32

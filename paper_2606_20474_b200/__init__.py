@@ -22,6 +22,9 @@ from .binding import (  # noqa: F401
     decode_attention_shared_prefix,
     decode_step,
     decode_step_host,
+    decode_workspace_bytes,
+    FLAG_DEBUG_CHECKS,
+    FLAG_NO_BULK_APPEND,
     last_error,
     library_path,
     merge_splits,

@@ -73,6 +73,8 @@ def _load():
     lib.uq_merge_splits2.argtypes = [cfgp, vp, vp, i32, vp, vp, i32, i32, vp, vp]
     lib.uq_calibrate_c.restype = i32
     lib.uq_calibrate_c.argtypes = [cfgp, vp, i64, i32, vp, i32, i32, vp, vp, vp, vp]
+    lib.uq_decode_workspace_bytes.restype = i32
+    lib.uq_decode_workspace_bytes.argtypes = [cfgp, i32, i32, ctypes.POINTER(ctypes.c_size_t)]
     lib.uq_suggest_num_splits.restype = i32
     lib.uq_suggest_num_splits.argtypes = [cfgp, i32, i32]
     lib.uq_suggest_num_splits_max.restype = i32
@@ -110,6 +112,19 @@ def _dev(t: torch.Tensor, dtype, name: str) -> torch.Tensor:
 def cache_record_bytes(cfg: UQConfig) -> int:
     c = cfg.c()
     return int(_load().uq_cache_record_bytes(ctypes.byref(c)))
+
+
+FLAG_NO_BULK_APPEND = 1
+FLAG_DEBUG_CHECKS = 2
+
+
+def decode_workspace_bytes(cfg: UQConfig, batch: int, num_splits: int) -> int:
+    """uq_decode_workspace_bytes: device scratch the decode calls need beyond the partial buffers (0 in this version)."""
+    c = cfg.c()
+    n = ctypes.c_size_t(0)
+    _check(_load().uq_decode_workspace_bytes(ctypes.byref(c), int(batch), int(num_splits), ctypes.byref(n)),
+           "uq_decode_workspace_bytes")
+    return int(n.value)
 
 
 def suggest_num_splits(cfg: UQConfig, batch: int, avg_seq_len: int) -> int:

@@ -1,6 +1,8 @@
 // uq_api.cu — host-side plumbing of libuq.so: error string, config validation, small queries.
 #include <stdarg.h>
 
+#include <mutex>
+
 #include "uq_common.cuh"
 
 namespace uq {
@@ -33,7 +35,7 @@ int32_t check_config(const uq_config* cfg) {
     set_error("uq_config: c_k and c_v must be positive");
     return UQ_ERR_INVALID_ARG;
   }
-  if ((cfg->flags & ~(uint32_t)UQ_FLAG_NO_BULK_APPEND) != 0) {
+  if ((cfg->flags & ~(uint32_t)(UQ_FLAG_NO_BULK_APPEND | UQ_FLAG_DEBUG_CHECKS)) != 0) {
     set_error("uq_config: unknown bit in flags");
     return UQ_ERR_INVALID_ARG;
   }
@@ -55,6 +57,60 @@ int32_t check_cuda(cudaError_t e, const char* what) {
   return UQ_ERR_CUDA;
 }
 
+// ---------------------------------------------------------------- per-device host state
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex g_dev_mu;
+int g_sms[kMaxDevices];                                // 0 = not looked up yet
+struct OptIn { const void* kernel; int device; int bytes; };
+OptIn g_optin[256];
+int g_optin_n = 0;
+}  // namespace
+
+int32_t current_device_sms(int* sms) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return check_cuda(e, "cudaGetDevice");
+  std::lock_guard<std::mutex> lock(g_dev_mu);
+  if (dev >= 0 && dev < kMaxDevices && g_sms[dev] > 0) { *sms = g_sms[dev]; return UQ_OK; }
+  int v = 0;
+  e = cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
+  if (e != cudaSuccess || v <= 0) return check_cuda(e != cudaSuccess ? e : cudaErrorUnknown, "cudaDeviceGetAttribute(SM count)");
+  if (dev >= 0 && dev < kMaxDevices) g_sms[dev] = v;
+  *sms = v;
+  return UQ_OK;
+}
+
+int32_t opt_in_dynamic_smem(const void* kernel, int bytes, const char* what) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return check_cuda(e, "cudaGetDevice");
+  std::lock_guard<std::mutex> lock(g_dev_mu);
+  for (int i = 0; i < g_optin_n; ++i)
+    if (g_optin[i].kernel == kernel && g_optin[i].device == dev && g_optin[i].bytes >= bytes) return UQ_OK;
+  e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e != cudaSuccess) return check_cuda(e, what);
+  if (g_optin_n < 256) g_optin[g_optin_n++] = OptIn{kernel, dev, bytes};   // a full table only costs a repeated call
+  return UQ_OK;
+}
+
+EncodeTiledFn encode_tiled_fn() {
+  static std::mutex mu;
+  static EncodeTiledFn encode = nullptr;
+  std::lock_guard<std::mutex> lock(mu);
+  if (!encode) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess || fn == nullptr) {
+      set_error("cuTensorMapEncodeTiled is not available from this driver");
+      return nullptr;
+    }
+    encode = (EncodeTiledFn)fn;
+  }
+  return encode;
+}
+
 }  // namespace uq
 
 extern "C" const char* uq_last_error_string(void) { return uq::g_err; }
@@ -64,13 +120,23 @@ extern "C" size_t uq_cache_record_bytes(const uq_config* cfg) {
   return (size_t)cfg->page_size * (size_t)(cfg->head_dim / 2 + cfg->head_dim / cfg->group_size) * 2;
 }
 
+extern "C" int32_t uq_decode_workspace_bytes(const uq_config* cfg, int32_t batch, int32_t num_splits, size_t* bytes) {
+  const int32_t st = uq::check_config(cfg);
+  if (st != UQ_OK) return st;
+  if (batch <= 0 || num_splits <= 0 || bytes == nullptr) {
+    uq::set_error("uq_decode_workspace_bytes: non-positive size or NULL result pointer");
+    return UQ_ERR_INVALID_ARG;
+  }
+  // The decode kernels keep their schedule (tile prefix sums), their rings and their accumulators in shared memory and
+  // TMEM, and the split partials are the caller's buffers: no device scratch beyond them.
+  *bytes = 0;
+  return UQ_OK;
+}
+
 extern "C" int32_t uq_suggest_num_splits(const uq_config* cfg, int32_t batch, int32_t avg_seq_len) {
   if (uq::check_config(cfg) != UQ_OK || batch <= 0) return 1;
-  int dev = 0, sms = 148;
-  if (cudaGetDevice(&dev) == cudaSuccess) {
-    int v = 0;
-    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) sms = v;
-  }
+  int sms = 148;
+  if (uq::current_device_sms(&sms) != UQ_OK) sms = 148;   // no device (a host-only caller sizing buffers): B200's count
   // uq_decode_attention gives every resident CTA (2 per SM) one equal range of 128-token tiles; an item
   // (sequence, kv head) of T tiles then spans about T / range + 1 CTAs = slots.  Leave room for sequences
   // twice the average length.
@@ -94,11 +160,8 @@ extern "C" int32_t uq_suggest_num_splits_max(const uq_config* cfg, int32_t batch
   // mean 16k, maximum 98k tokens) needs max_tiles / range + 2 slots or every CTA's range is stretched.
   const int32_t base = uq_suggest_num_splits(cfg, batch, avg_seq_len);
   if (uq::check_config(cfg) != UQ_OK || batch <= 0 || max_seq_len <= avg_seq_len) return base;
-  int dev = 0, sms = 148;
-  if (cudaGetDevice(&dev) == cudaSuccess) {
-    int v = 0;
-    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) sms = v;
-  }
+  int sms = 148;
+  if (uq::current_device_sms(&sms) != UQ_OK) sms = 148;   // no device (a host-only caller sizing buffers): B200's count
   const int64_t tiles_avg = ((int64_t)avg_seq_len + 127) / 128 > 0 ? ((int64_t)avg_seq_len + 127) / 128 : 1;
   const int64_t tiles_max = ((int64_t)max_seq_len + 127) / 128;
   int64_t range = ((int64_t)batch * cfg->num_kv_heads * tiles_avg + 2 * sms - 1) / (2 * sms);

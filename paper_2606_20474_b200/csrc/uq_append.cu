@@ -647,21 +647,9 @@ append_bulk_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_cons
 
 // 2-D TMA view of k_new / v_new: [rows][kv heads x 128] bf16; box = 16 rows x 64 channels (128 B: the widest row the
 // 128-byte swizzle takes), so a page's K (or V) rows of one kv head are two tensor copies.
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 int32_t rows_map(const void* rows, long long n_rows, int Hkv, CUtensorMap* out) {
-  static EncodeTiledFn encode = nullptr;               // set once; racing first calls store the same pointer
-  if (!encode) {
-    void* fn = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
-    if (e != cudaSuccess || fn == nullptr) {
-      set_error("append: cuTensorMapEncodeTiled is not available from this driver");
-      return UQ_ERR_CUDA;
-    }
-    encode = (EncodeTiledFn)fn;
-  }
+  const EncodeTiledFn encode = encode_tiled_fn();
+  if (!encode) return UQ_ERR_CUDA;
   const cuuint64_t gdim[2] = {(cuuint64_t)Hkv * kHeadDim, (cuuint64_t)n_rows};
   const cuuint64_t gstr[1] = {(cuuint64_t)Hkv * kHeadDim * 2};
   const cuuint32_t box[2] = {64, 16};
@@ -707,16 +695,17 @@ extern "C" int32_t uq_rotate_quantize_append(const uq_config* cfg, const void* k
   }
   const long long q_rows = q ? (long long)batch * cfg->num_q_heads : 0;
   if (total_new == 0 && q_rows == 0) return UQ_OK;
+  if ((cfg->flags & UQ_FLAG_DEBUG_CHECKS) && total_new > 0) {
+    st = debug_check_tables("uq_rotate_quantize_append", block_tables, max_pages, batch, num_pages, seq_lens, cu_new,
+                            total_new, 0, cfg->page_size, 1, (cudaStream_t)stream);
+    if (st != UQ_OK) return st;
+  }
   // Prefill-sized calls (on average 64 or more new tokens per sequence): K/V through append_bulk_kernel, one warp per
   // page; the kernel below then only encodes the query rows.  Same bytes either way.
   if (total_new >= 1024 && (long long)total_new >= 64LL * batch && !(((uintptr_t)k_new | (uintptr_t)v_new) & 15u) &&
       !(cfg->flags & UQ_FLAG_NO_BULK_APPEND)) {
-    static bool attr_set = false;
-    if (!attr_set) {
-      cudaError_t e = cudaFuncSetAttribute(append_bulk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kBulkSmem);
-      if (e != cudaSuccess) return check_cuda(e, "append: cudaFuncSetAttribute");
-      attr_set = true;
-    }
+    st = opt_in_dynamic_smem((const void*)append_bulk_kernel, kBulkSmem, "append: cudaFuncSetAttribute");
+    if (st != UQ_OK) return st;
     CUtensorMap tmap_k, tmap_v;
     st = rows_map(k_new, total_new, cfg->num_kv_heads, &tmap_k);
     if (st == UQ_OK) st = rows_map(v_new, total_new, cfg->num_kv_heads, &tmap_v);

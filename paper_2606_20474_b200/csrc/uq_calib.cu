@@ -127,13 +127,9 @@ extern "C" int32_t uq_calibrate_c(const uq_config* cfg, const void* x, int64_t n
   cudaError_t e = cudaMemsetAsync(sq_err, 0, sizeof(double) * (size_t)n_c, s);
   if (e == cudaSuccess) e = cudaMemsetAsync(sq_norm, 0, sizeof(double), s);
   if (e != cudaSuccess) return check_cuda(e, "calibrate: cudaMemsetAsync");
-  static int sm_count = 0;
-  if (sm_count == 0) {
-    int dev = 0, v = 0;
-    if (cudaGetDevice(&dev) == cudaSuccess &&
-        cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) sm_count = v;
-    else sm_count = 148;
-  }
+  int sm_count = 0;
+  st = current_device_sms(&sm_count);
+  if (st != UQ_OK) return st;
   long long blocks = (n_vec + kCalibWarps - 1) / kCalibWarps;
   if (blocks > 8LL * sm_count) blocks = 8LL * sm_count;   // a multiple of the SM count; warps stride over the vectors
   calib_kernel<<<(unsigned)blocks, 32 * kCalibWarps, 0, s>>>((const uint16_t*)x, (long long)n_vec, (int)rotate, c_grid,

@@ -2,6 +2,7 @@
 // record-layout constants documented in include/uq.h.  CUDA path only; the oracle shares
 // nothing with this file.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stdio.h>
@@ -49,9 +50,26 @@ inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, s
   return cudaLaunchKernelEx(&lc, kernel, KArgs(args)...);
 }
 
-// TMA descriptors of the decode kernels (uq_decode.cu): the K codes of the cache as a packed 4-bit tensor (cached
-// per cache pointer), and q_fp8 as [rows][128] bytes with a box of 16 rows.
+// Per-DEVICE host state (uq_api.cu).  The library may be called on several devices of one process (the caller's
+// cudaSetDevice decides): the SM count sizes the one-wave grids, and the dynamic-shared-memory opt-in of a kernel is a
+// per-device function attribute.  Both are looked up for the current device under a mutex.
+int32_t current_device_sms(int* sms);                                   // UQ_OK / UQ_ERR_CUDA
+int32_t opt_in_dynamic_smem(const void* kernel, int bytes, const char* what);   // once per (kernel, device)
+
+// UQ_FLAG_DEBUG_CHECKS (uq_debug.cu): validates on the device the table entries / lengths a call is going to use and
+// synchronises the stream; mode 0 decode, 1 append, 2 shared prefix (fixed_pages entries equal to sequence 0's).
+int32_t debug_check_tables(const char* who, const int32_t* block_tables, int max_pages, int batch, long long num_pages,
+                           const int32_t* seq_lens, const int32_t* cu_new, int total_new, int fixed_pages, int page,
+                           int mode, cudaStream_t stream);
+
+// TMA descriptors.  cuTensorMapEncodeTiled is fetched once through the runtime (no link-time dependency on
+// libcuda); k_code_map: the K codes of the cache as a packed 4-bit tensor (descriptors cached per cache pointer);
+// q_map: q_fp8 as [rows][128] bytes with a box of 16 rows.
 #ifdef CUDA_VERSION
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn();                                        // nullptr (error string set) if unavailable
 int32_t k_code_map(const void* cache, long long records, CUtensorMap* out);
 int32_t q_map(const void* q_fp8, long long rows, CUtensorMap* out);
 #endif

@@ -16,7 +16,7 @@
 #include <mutex>
 #include <type_traits>
 
-#include "uq_common.cuh"
+#include "uq_tc.cuh"
 
 namespace uq {
 namespace {
@@ -62,7 +62,6 @@ constexpr int kKStageBytes = kTilePages * 2048;      // K codes, one byte per co
 constexpr int kVStageBytes = kTilePages * kRestBytes;   // 9216
 constexpr int kPBytes = 4096 * kNS;                  // one P operand buffer: [token-core 16][head-core 2 kNS][8 tok][8 heads] f16
 constexpr float kThresh = 12.0f;                     // lazy-reference threshold (log2 units)
-constexpr unsigned kFull = 0xffffffffu;
 
 // dynamic shared memory map (offsets from a 1024-byte aligned base)
 constexpr int kOffK = 0;                                       // kKStages x 16384, SW128
@@ -88,197 +87,6 @@ constexpr uint32_t kColV = UQ_PREFIX_CTAS == 2 ? 128 : (3 * kNCols + 12 + 31) / 
 constexpr uint32_t kTmemCols = UQ_PREFIX_CTAS == 2 ? 256 : 512;
 static_assert(kColV + 128 <= kTmemCols, "TMEM columns");
 static_assert(3 * kNCols + 12 <= kColV, "score / accumulator / scale columns must stay below the Vhat buffers");
-
-// ---------------------------------------------------------------- PTX wrappers
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-  return (uint32_t)__cvta_generic_to_shared(p);
-}
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-// Waits are a plain mbarrier.try_wait loop (the hardware suspends the thread for a bounded time per probe).
-// Measured and dropped on config 2: test_wait spin loops (157-161 us: the spin steals issue slots from the working
-// warps), nanosleep polling and suspend-time hints in the softmax warps (no change).
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "WAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra DONE_%=;\n"
-      "bra WAIT_%=;\n"
-      "DONE_%=:\n"
-      "}\n" ::"r"(bar), "r"(parity) : "memory");
-}
-// The KV stream is read once: L2 evict-first keeps it from flushing everything else (the kernel's own
-// instructions included) out of L2.
-__device__ __forceinline__ uint64_t l2_evict_first_policy() {
-  uint64_t p;
-  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
-  return p;
-}
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint64_t pol) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
-               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
-}
-__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, int c2, uint32_t bar,
-                                            uint64_t pol) {
-  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
-               " [%0], [%1, {%2, %3, %4}], [%5], %6;"
-               ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "l"(pol) : "memory");
-}
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, uint32_t bar) {
-  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-               ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(bar) : "memory");
-}
-// One lane of the (converged) warp.  With elect.sync ptxas knows that a single thread runs the guarded block and
-// feeds the uniform-register operands of UTCQMMA / UTMALDG with one R2UR each; behind `lane == 0` it wraps every
-// such instruction in an elect-and-broadcast loop of a dozen instructions.  Measured on config 2: for the QK warp
-// (the busiest issuer: its serial per-tile instruction stream bounded the tile period) this is 119 -> 109.5 us;
-// for the PV warp and the producers the same change is SLOWER (124-132 us), so those keep `lane == 0`.
-__device__ __forceinline__ bool elect_one() {
-  uint32_t pred;
-  asm volatile("{\n.reg .pred p;\nelect.sync _|p, 0xffffffff;\nselp.u32 %0, 1, 0, p;\n}\n" : "=r"(pred));
-  return pred != 0;
-}
-__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void bar_softmax(int id) { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
-// barrier over the 128 softmax threads that also ORs a predicate across them
-__device__ __forceinline__ bool bar_softmax_or(int id, bool pred) {
-  uint32_t r;
-  asm volatile("{\n.reg .pred p, q;\nsetp.ne.b32 q, %1, 0;\nbar.red.or.pred p, %2, 128, q;\nselp.u32 %0, 1, 0, p;\n}\n"
-               : "=r"(r) : "r"((uint32_t)pred), "r"(id) : "memory");
-  return r != 0;
-}
-
-// shared-memory matrix descriptor (SM100 UMMA): start>>4 | LBO>>4 <<16 | SBO>>4 <<32 | version 1 | layout
-__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes, uint32_t layout) {
-  uint64_t d = 0;
-  d |= (uint64_t)((saddr >> 4) & 0x3FFF);
-  d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16;
-  d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32;
-  d |= (uint64_t)1 << 46;
-  d |= (uint64_t)(layout & 7) << 61;      // 0 = no swizzle, 2 = 128-byte swizzle
-  return d;
-}
-__device__ __forceinline__ void umma_commit(uint32_t bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void umma_cp_sf(uint32_t taddr, uint64_t sdesc) {
-  asm volatile("tcgen05.cp.cta_group::1.32x128b.warpx4 [%0], %1;" ::"r"(taddr), "l"(sdesc) : "memory");
-}
-// D[tmem] (+)= A[smem, E2M1] . B[smem, E4M3]^T with UE8M0 block scales in TMEM
-__device__ __forceinline__ void umma_mxf8f6f4(uint32_t d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t acc,
-                                              uint32_t tsfa, uint32_t tsfb) {
-  asm volatile(
-      "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
-      "tcgen05.mma.cta_group::1.kind::mxf8f6f4.block_scale [%0], %1, %2, %3, [%5], [%6], p;\n}\n"
-      ::"r"(d), "l"(da), "l"(db), "r"(idesc), "r"(acc), "r"(tsfa), "r"(tsfb) : "memory");
-}
-// N consecutive 32-bit columns of this thread's TMEM lane <-> registers (N = 8 or 16), complete on return
-template <int N>
-__device__ __forceinline__ void tmem_ld(uint32_t taddr, float (&v)[N]) {
-  static_assert(N == 8 || N == 16, "tmem_ld: 8 or 16 columns");
-  uint32_t r[N];
-  if constexpr (N == 8) {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
-                 : "r"(taddr));
-  } else {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
-                   "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
-                 : "r"(taddr));
-  }
-  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-  for (int j = 0; j < N; ++j) v[j] = __uint_as_float(r[j]);
-}
-template <int N>
-__device__ __forceinline__ void tmem_st(uint32_t taddr, const float (&v)[N]) {
-  static_assert(N == 8 || N == 16, "tmem_st: 8 or 16 columns");
-  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
-               ::"r"(taddr), "r"(__float_as_uint(v[0])), "r"(__float_as_uint(v[1])), "r"(__float_as_uint(v[2])),
-                 "r"(__float_as_uint(v[3])), "r"(__float_as_uint(v[4])), "r"(__float_as_uint(v[5])),
-                 "r"(__float_as_uint(v[6])), "r"(__float_as_uint(v[7])) : "memory");
-  if constexpr (N == 16) {
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
-                 ::"r"(taddr + 8), "r"(__float_as_uint(v[8])), "r"(__float_as_uint(v[9])), "r"(__float_as_uint(v[10])),
-                   "r"(__float_as_uint(v[11])), "r"(__float_as_uint(v[12])), "r"(__float_as_uint(v[13])),
-                   "r"(__float_as_uint(v[14])), "r"(__float_as_uint(v[15])) : "memory");
-  }
-  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_st16_nowait(uint32_t taddr, const uint32_t (&v)[16]) {
-  asm volatile(
-      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
-      ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]),
-        "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]) : "memory");
-}
-__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
-__device__ __forceinline__ void umma_f16_ts(uint32_t d, uint32_t ta, uint64_t db, uint32_t idesc, uint32_t acc) {
-  asm volatile(
-      "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n}\n"
-      ::"r"(d), "r"(ta), "l"(db), "r"(idesc), "r"(acc) : "memory");
-}
-__device__ __forceinline__ uint4 lds128(uint32_t a) {
-  uint4 v;
-  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
-  return v;
-}
-__device__ __forceinline__ void sts128(uint32_t a, uint4 v) {
-  asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
-}
-__device__ __forceinline__ float ex2(float x) {
-  float y;
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
-// packed fp32 pairs (FFMA2 / FADD2): d = a * s + c and d = a + b on two lanes at once
-__device__ __forceinline__ void ffma2(float& d0, float& d1, float a0, float a1, float s, float c0, float c1) {
-  uint64_t av, sv, cv, dv;
-  asm("mov.b64 %0, {%1, %2};" : "=l"(av) : "f"(a0), "f"(a1));
-  asm("mov.b64 %0, {%1, %2};" : "=l"(sv) : "f"(s), "f"(s));
-  asm("mov.b64 %0, {%1, %2};" : "=l"(cv) : "f"(c0), "f"(c1));
-  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(dv) : "l"(av), "l"(sv), "l"(cv));
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(d0), "=f"(d1) : "l"(dv));
-}
-__device__ __forceinline__ void fadd2(float& d0, float& d1, float a0, float a1, float b0, float b1) {
-  uint64_t av, bv, dv;
-  asm("mov.b64 %0, {%1, %2};" : "=l"(av) : "f"(a0), "f"(a1));
-  asm("mov.b64 %0, {%1, %2};" : "=l"(bv) : "f"(b0), "f"(b1));
-  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(dv) : "l"(av), "l"(bv));
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(d0), "=f"(d1) : "l"(dv));
-}
-__device__ __forceinline__ uint32_t hmul2(uint32_t a, uint32_t b) {
-  uint32_t d;
-  asm("mul.rn.f16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b));
-  return d;
-}
-// four packed byte pairs of E2M1 codes -> four f16x2 registers (low nibble -> low half)
-__device__ __forceinline__ void cvt_e2m1x8(uint32_t w, uint32_t (&h)[4]) {
-  asm("{\n"
-      ".reg .b8 b0, b1, b2, b3;\n"
-      "mov.b32 {b0, b1, b2, b3}, %4;\n"
-      "cvt.rn.f16x2.e2m1x2 %0, b0;\n"
-      "cvt.rn.f16x2.e2m1x2 %1, b1;\n"
-      "cvt.rn.f16x2.e2m1x2 %2, b2;\n"
-      "cvt.rn.f16x2.e2m1x2 %3, b3;\n"
-      "}\n" : "=r"(h[0]), "=r"(h[1]), "=r"(h[2]), "=r"(h[3]) : "r"(w));
-}
-__device__ __forceinline__ float pow2i(int e) {   // 2^e, flushing to 0 below the fp32 normal range
-  const int f = e + 127;
-  return f > 0 ? __uint_as_float((uint32_t)min(f, 254) << 23) : 0.f;
-}
 
 // ---------------------------------------------------------------- per-CTA shared bookkeeping
 struct Shared {
@@ -889,28 +697,25 @@ extern "C" int32_t uq_decode_prefix_attention(const uq_config* cfg, const void* 
     set_error("decode_prefix: num_pages * num_kv_heads must be < 2^31");
     return UQ_ERR_INVALID_ARG;
   }
+  if (cfg->flags & UQ_FLAG_DEBUG_CHECKS) {
+    st = debug_check_tables("uq_decode_prefix_attention", block_tables, max_pages, batch, num_pages, nullptr, nullptr, 0,
+                            prefix_len / cfg->page_size, cfg->page_size, 2, (cudaStream_t)stream);
+    if (st != UQ_OK) return st;
+  }
   CUtensorMap tmap, tmap_q;
   st = k_code_map(cache, records, &tmap);
   if (st != UQ_OK) return st;
   st = q_map(q_fp8, (long long)batch * cfg->num_q_heads, &tmap_q);
   if (st != UQ_OK) return st;
   const float score_scale = resolved_sm_scale(cfg) * 1.4426950408889634f;
-  static int sm_count = 0;
-  if (sm_count == 0) {
-    int dev = 0, v = 0;
-    if (cudaGetDevice(&dev) == cudaSuccess &&
-        cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) sm_count = v;
-    else sm_count = 148;
-  }
+  int sm_count = 0;
+  st = current_device_sms(&sm_count);
+  if (st != UQ_OK) return st;
   const long long total = (long long)((batch + kNS - 1) / kNS) * cfg->num_kv_heads * (prefix_len / 128);
   const long long slots = (long long)sm_count * UQ_CTAS_PER_SM;
   const dim3 grid((unsigned)(total < slots ? total : slots));   // one wave, one balanced tile range per CTA
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(decode_prefix_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
-    if (e != cudaSuccess) return check_cuda(e, "decode_prefix: cudaFuncSetAttribute");
-    attr_set = true;
-  }
+  st = opt_in_dynamic_smem((const void*)decode_prefix_kernel, kSmemBytes, "decode_prefix: cudaFuncSetAttribute");
+  if (st != UQ_OK) return st;
   return check_cuda(launch_pdl(decode_prefix_kernel, grid, dim3(kThreads), (size_t)kSmemBytes, (cudaStream_t)stream, tmap,
                                tmap_q, (const uint8_t*)cache, block_tables, (int)max_pages, (int)(prefix_len / 128),
                                (int)batch, (int)cfg->num_q_heads, (int)cfg->num_kv_heads, (int)num_splits, score_scale,

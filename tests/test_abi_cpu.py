@@ -71,6 +71,23 @@ def test_prefix_decode_and_calibrate_validate_on_the_host(lib):
     assert uq.suggest_num_splits_max(uq.UQConfig(64, 4), 256, 16500, 98000) > uq.suggest_num_splits(uq.UQConfig(64, 4), 256, 16500)
 
 
+def test_workspace_query_and_debug_flag_on_the_host(lib):
+    """uq_decode_workspace_bytes: 0 bytes for any supported geometry, argument errors reported; the
+    debug flag is a known bit of uq_config.flags, other bits are refused."""
+    assert uq.decode_workspace_bytes(uq.UQConfig(64, 4), 32, 6) == 0
+    assert uq.decode_workspace_bytes(uq.UQConfig(48, 8), 2048, 64) == 0
+    c = uq.UQConfig(64, 4).c()
+    n = ctypes.c_size_t(7)
+    assert lib.uq_decode_workspace_bytes(ctypes.byref(c), 0, 1, ctypes.byref(n)) == 1
+    assert lib.uq_decode_workspace_bytes(ctypes.byref(c), 1, 1, None) == 1
+    bad = uq.UQConfig(64, 4, page_size=32).c()
+    assert lib.uq_decode_workspace_bytes(ctypes.byref(bad), 1, 1, ctypes.byref(n)) == 2
+    ok = uq.UQConfig(64, 4, flags=uq.FLAG_DEBUG_CHECKS | uq.FLAG_NO_BULK_APPEND)
+    assert uq.cache_record_bytes(ok) == 2176
+    assert uq.cache_record_bytes(uq.UQConfig(64, 4, flags=4)) == 0
+    assert b"flags" in lib.uq_last_error_string()
+
+
 def test_binding_refuses_cpu_tensors(lib):
     import torch
     cfg = uq.UQConfig(8, 1)

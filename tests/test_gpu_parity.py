@@ -664,3 +664,75 @@ def test_shared_prefix_decode_matches_the_oracle_and_the_plain_decode(hq, hkv, l
         H.check_out(out[b], ref, f"shared prefix seq {b}")
     pl = plain.float().cpu().numpy().astype(np.float64)
     assert np.all(np.abs(out - pl) <= 2 * (H.ATOL + H.RTOL * np.abs(pl)))
+
+
+def test_debug_checks_name_the_first_bad_table_entry_and_leave_good_calls_alone():
+    """UQ_FLAG_DEBUG_CHECKS (include/uq.h): with the flag a call whose block table names a page outside the
+    cache, whose length exceeds the table, whose cu_new is inconsistent or whose "shared" prefix is not shared is
+    refused with UQ_ERR_INVALID_ARG naming the offender — nothing is written; a valid call gives bit for bit the
+    result of the same call without the flag."""
+    wl = W.make_custom("dbg", 51, [300, 277, 512], 16, 2, prefix_len=256, extra_tokens=4)
+    cfg = H.cfg_of(wl)
+    dbg = H.cfg_of(wl, flags=uq.FLAG_DEBUG_CHECKS)
+    cache, bt = H.fill_cache(dbg, wl, DEV)                  # the fill itself runs under the checks
+    cache_ref, _ = H.fill_cache(cfg, wl, DEV)
+    assert torch.equal(cache, cache_ref)
+    q = W.gen_q(wl, DEV)
+    out_ref, q_fp8, bufs = H.run_decode(cfg, cache, bt, wl.ctx_lens, q, 3)
+    out_dbg, _, _ = H.run_decode(dbg, cache, bt, wl.ctx_lens, q, 3)
+    assert torch.equal(out_ref, out_dbg)
+    lens = torch.from_numpy(wl.ctx_lens.astype(np.int32)).to(DEV)
+    # (1) an entry outside the cache, inside the used range of sequence 1
+    bad = bt.clone(); bad[1, 17] = wl.num_pages
+    with pytest.raises(uq.UQError, match=r"block_tables\[1\]\[17\]"):
+        uq.decode_attention(dbg, q_fp8, cache, bad, lens, 3, bufs.partial_acc, bufs.partial_ml)
+    bad = bt.clone(); bad[0, 0] = -1
+    with pytest.raises(uq.UQError, match=r"block_tables\[0\]\[0\] = -1"):
+        uq.decode_attention(dbg, q_fp8, cache, bad, lens, 3, bufs.partial_acc, bufs.partial_ml)
+    # ... but not one beyond the sequence's last page (never read)
+    ok = bt.clone(); ok[1, 20] = 10 ** 6          # seq 1: 277 tokens = pages 0..17
+    uq.decode_attention(dbg, q_fp8, cache, ok, lens, 3, bufs.partial_acc, bufs.partial_ml)
+    # (2) a length the table cannot hold
+    long_lens = lens.clone(); long_lens[2] = bt.shape[1] * 16 + 1
+    with pytest.raises(uq.UQError, match="sequence 2"):
+        uq.decode_attention(dbg, q_fp8, cache, bt, long_lens, 3, bufs.partial_acc, bufs.partial_ml)
+    # (3) append: decreasing cu_new, a write past the table, a bad entry on the page written
+    k1, v1 = W.gen_kv(wl, 0, 0, 3, DEV)
+    before = cache.clone()
+    cu = torch.tensor([0, 2, 1, 3], dtype=torch.int32, device=DEV)
+    with pytest.raises(uq.UQError, match="cu_new"):
+        uq.rotate_quantize_append(dbg, k1, v1, cu, lens, bt, cache)
+    cu = torch.tensor([0, 1, 2, 3], dtype=torch.int32, device=DEV)
+    with pytest.raises(uq.UQError, match="sequence 2"):
+        uq.rotate_quantize_append(dbg, k1, v1, cu, long_lens, bt, cache)
+    bad = bt.clone(); bad[1, 277 // 16] = -5
+    with pytest.raises(uq.UQError, match=r"block_tables\[1\]\[17\] = -5"):
+        uq.rotate_quantize_append(dbg, k1, v1, cu, lens, bad, cache)
+    torch.cuda.synchronize()
+    assert torch.equal(cache, before)                       # nothing was written by the refused calls
+    uq.rotate_quantize_append(dbg, k1, v1, cu, lens, bt, cache)       # the valid append passes
+    # (4) shared prefix that is not shared
+    pb = uq.PrefixBuffers(cfg, wl.batch, 2, DEV)
+    pb.suffix_lens.copy_(lens - 256)
+    bufs2 = uq.StepBuffers(dbg, wl.batch, 2, DEV); bufs2.q_fp8.copy_(q_fp8)
+    bad = bt.clone(); bad[2, 7] = bt[2, 20]
+    with pytest.raises(uq.UQError, match="not shared"):
+        uq.decode_attention_shared_prefix(dbg, bufs2, pb, cache, bad, 256)
+    uq.decode_attention_shared_prefix(dbg, bufs2, pb, cache, bt, 256)
+    torch.cuda.synchronize()
+
+
+def test_second_device_of_one_process_if_there_is_one():
+    """The library keeps its per-device state (SM count, shared-memory opt-in, TMA descriptors) per device: a decode
+    on device 1 after one on device 0 in the same process gives the same output.  Skipped on one-GPU boxes."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("one visible device")
+    wl = W.make_custom("dev1", 52, [700, 130], 16, 2)
+    outs = []
+    for dev in ("cuda:0", "cuda:1"):
+        with torch.cuda.device(dev):
+            cfg = H.cfg_of(wl)
+            cache, bt = H.fill_cache(cfg, wl, dev)
+            out, _, _ = H.run_decode(cfg, cache, bt, wl.ctx_lens, W.gen_q(wl, dev), 3)
+            outs.append(out.cpu())
+    assert torch.equal(outs[0], outs[1])
