@@ -63,14 +63,43 @@ double uqo_kappa(int d) {
   }
 }
 
+/* The matrix is written out once per d (entries exactly +1.0 / -1.0 from the popcount rule) and then
+ * used as a plain dense matrix: y_i = kappa * sum_j H[i][j] * x[j], j ascending.  A product by +-1.0 is
+ * exact, so this is the same sum, term for term, as adding +x[j] or -x[j]. */
+#define UQ_MAX_D 256
+static double uqo_H[4][UQ_MAX_D * UQ_MAX_D];   /* d = 32, 64, 128, 256 */
+static int uqo_H_ready[4];
+
+static const double* uqo_hadamard_matrix(int d) {
+  const int slot = d == 32 ? 0 : d == 64 ? 1 : d == 128 ? 2 : d == 256 ? 3 : -1;
+  if (slot < 0) return NULL;
+  double* H = uqo_H[slot];
+  int ready;
+#pragma omp atomic read
+  ready = uqo_H_ready[slot];
+  if (!ready) {
+#pragma omp critical(uqo_hadamard_table)
+    {
+      if (!uqo_H_ready[slot]) {
+        for (int i = 0; i < d; ++i)
+          for (int j = 0; j < d; ++j)
+            H[i * d + j] = (popcount_u32((uint32_t)i & (uint32_t)j) & 1) ? -1.0 : 1.0;
+#pragma omp flush
+#pragma omp atomic write
+        uqo_H_ready[slot] = 1;
+      }
+    }
+  }
+  return H;
+}
+
 void uqo_hadamard(const double* x, int d, double* y) {
   const double kappa = uqo_kappa(d);
+  const double* H = uqo_hadamard_matrix(d);
+  if (!H) { for (int i = 0; i < d; ++i) y[i] = 0.0; return; }
   for (int i = 0; i < d; ++i) {
     double acc = 0.0;
-    for (int j = 0; j < d; ++j) {
-      int neg = popcount_u32((uint32_t)i & (uint32_t)j) & 1;
-      acc += neg ? -x[j] : x[j];
-    }
+    for (int j = 0; j < d; ++j) acc += H[i * d + j] * x[j];
     y[i] = acc * kappa;
   }
 }
