@@ -16,24 +16,30 @@ DEV = "cuda"
 
 
 def _full_check(wl, splits_list, sample_seqs=None, check_cache=True):
+    """Fill the cache through the ABI, decode with every slot count of splits_list, then sequence by sequence (the
+    oracle's arrays of one sequence at a time: config 3 holds 2.7 M tokens x 8 kv heads) compare the cache image bit
+    for bit and every output row of every head within tolerance.  Returns (worst err/bound, sequences checked)."""
     cfg = H.cfg_of(wl)
     cache, bt = H.fill_cache(cfg, wl, DEV)
     q = W.gen_q(wl, DEV)
     qb = H.bits(q)
-    seqs = range(wl.batch) if sample_seqs is None else sample_seqs
-    arrays = {b: H.oracle_sequence_cache(wl, b, int(wl.ctx_lens[b]), DEV) for b in seqs}
-    if check_cache:
-        for b in seqs:
-            H.compare_cache(cache, wl, b, int(wl.ctx_lens[b]), arrays[b])
-    worst = 0.0
+    seqs = list(range(wl.batch)) if sample_seqs is None else list(sample_seqs)
+    outs = []
     for S in splits_list:
         out, q_fp8, _ = H.run_decode(cfg, cache, bt, wl.ctx_lens, q, S)
-        out = out.float().cpu().numpy().astype(np.float64)
-        for b in seqs:
-            ref, q8 = H.oracle_out(wl, b, int(wl.ctx_lens[b]), qb[b], arrays[b])
-            assert np.array_equal(q_fp8[b].cpu().numpy(), q8), f"q_fp8 differs for seq {b}"
+        outs.append((S, out.float().cpu().numpy().astype(np.float64), q_fp8.cpu().numpy()))
+    worst = 0.0
+    for b in seqs:
+        L = int(wl.ctx_lens[b])
+        arrays = H.oracle_sequence_cache(wl, b, L, DEV)
+        if check_cache:
+            H.compare_cache(cache, wl, b, L, arrays)
+        ref, q8 = H.oracle_out(wl, b, L, qb[b], arrays)
+        for S, out, q_fp8 in outs:
+            assert np.array_equal(q_fp8[b], q8), f"q_fp8 differs for seq {b}"
             worst = max(worst, H.check_out(out[b], ref, f"{wl.name} seq {b} S={S}"))
-    return worst
+        del arrays
+    return worst, len(seqs)
 
 
 def test_cfg1_tiny_whole_cache_bit_exact_and_decode():
@@ -200,32 +206,55 @@ def test_permuting_physical_pages_leaves_output_unchanged():
     assert torch.equal(outs[0], outs[1])
 
 
-def test_full_size_cfg2_in_bench_launch_configuration_sampled():
-    """BASELINE.json config 2 at full size (32 x 32,768 tokens, 64/4 heads), decoded with the
-    num_splits bench.py uses; sampled sequences are checked row by row against the oracle."""
+def test_full_size_cfg2_all_32_sequences_in_bench_launch_configuration():
+    """BASELINE.json config 2 at FULL size (32 x 32,768 tokens, 64/4 heads) decoded with the num_splits bench.py uses:
+    ALL 32 sequences x 64 heads — every code / scale byte of the 1,048,576-token cache bit for bit, every output row
+    against the oracle ("attention outputs for all (b, h) on configs 1, 2, 3, 5")."""
     wl = W.make_config(2)
     cfg = H.cfg_of(wl)
     S = uq.suggest_num_splits(cfg, wl.batch, int(wl.ctx_lens.mean()))
-    _full_check(wl, [S], sample_seqs=[0, 17, 31], check_cache=True)
+    _, n = _full_check(wl, [S], check_cache=True)
+    assert n == 32
 
 
-@pytest.mark.parametrize("idx,seqs", [(3, "extremes"), (5, [3])])
-def test_full_size_configs_3_and_5_sampled(idx, seqs):
-    """BASELINE.json configs 3 (64 ragged sequences of 16k-64k tokens, 48/8 heads, GQA 6) and 5
-    (8 x 262,144 tokens) at FULL size with the split count bench.py would use; the cache image and
-    the decode output of the sampled sequences are checked against the oracle."""
-    wl = W.make_config(idx)
-    if seqs == "extremes":
-        seqs = [int(np.argmin(wl.ctx_lens)), int(np.argmax(wl.ctx_lens))]
+def test_full_size_cfg3_all_64_sequences():
+    """BASELINE.json config 3 at FULL size (64 ragged sequences of 16k-64k tokens, 48/8 heads, GQA 6; 2,720,570 tokens)
+    with the split count bench.py uses: ALL 64 sequences x 48 heads, cache image bit for bit and outputs."""
+    wl = W.make_config(3)
     cfg = H.cfg_of(wl)
     S = uq.suggest_num_splits(cfg, wl.batch, int(wl.ctx_lens.mean()))
-    _full_check(wl, [S], sample_seqs=seqs, check_cache=True)
+    _, n = _full_check(wl, [S], check_cache=True)
+    assert n == 64
 
 
-def test_full_size_cfg4_shared_prefix_step_sampled():
-    """BASELINE.json config 4 at FULL size: 256 sequences share a 30,000-token prefix (the same
-    physical pages in every block table) and have log-normal private suffixes; one timed-style step
-    (append 1 token per sequence, decode, merge); two sampled sequences against the oracle."""
+def test_full_size_cfg5_all_8_sequences():
+    """BASELINE.json config 5 at FULL size (8 x 262,144 tokens, 64/4 heads) with the split count bench.py uses: ALL 8
+    sequences x 64 heads, cache image bit for bit and outputs."""
+    wl = W.make_config(5)
+    cfg = H.cfg_of(wl)
+    S = uq.suggest_num_splits(cfg, wl.batch, int(wl.ctx_lens.mean()))
+    _, n = _full_check(wl, [S], check_cache=True)
+    assert n == 8
+
+
+def _cfg4_sample(wl, n=32):
+    """>= 32 sequences of config 4 chosen by the seed, always including the shortest, the median, the longest and every
+    capped (98,000-token) suffix."""
+    order = np.argsort(wl.ctx_lens, kind="stable")
+    capped = [int(b) for b in np.nonzero(wl.ctx_lens - wl.prefix_len >= 98000)[0]]
+    must = [int(order[0]), int(order[len(order) // 2]), int(order[-1])] + capped
+    rng = np.random.default_rng(wl.seed + 4444)
+    rest = [int(b) for b in rng.permutation(wl.batch) if int(b) not in must]
+    return sorted(set(must + rest[:max(0, n - len(set(must)))])), capped
+
+
+def test_full_size_cfg4_shared_prefix_step_32_sequences_both_decode_paths():
+    """BASELINE.json config 4 at FULL size: 256 sequences share a 30,000-token prefix (the same physical pages in every
+    block table) and have log-normal private suffixes capped at 98,000; one timed-style step (append 1 token per
+    sequence, decode, merge) through BOTH decode paths in bench.py's launch configurations — the plain split-K decode
+    and the shared-prefix path (uq_decode_prefix_attention + suffix decode + uq_merge_splits2).  32 seeded sequences
+    including the shortest, the median, the longest and all four capped suffixes: cache image (incl. the appended
+    token) bit for bit, outputs of both paths against the oracle; all 256 sequences: the two paths against each other."""
     wl = W.make_config(4)
     cfg = H.cfg_of(wl)
     cache, bt = H.fill_cache(cfg, wl, DEV)
@@ -239,8 +268,6 @@ def test_full_size_cfg4_shared_prefix_step_sampled():
     out = uq.decode_step(cfg, bufs, q, k_new, v_new, cu, before, after, bt, cache)
     torch.cuda.synchronize()
     out = out.float().cpu().numpy().astype(np.float64)
-    # the same step's decode through the shared-prefix path (bench.py --shared-prefix 1: 29,952 prefix tokens by
-    # uq_decode_prefix_attention, the suffixes by uq_decode_attention, uq_merge_splits2), in bench.py's launch configuration
     pfx = (int(wl.prefix_len) // 128) * 128
     suf = (wl.ctx_lens + 1 - pfx).astype(np.int64)
     bufs_sp = uq.StepBuffers(cfg, wl.batch, uq.suggest_num_splits_max(cfg, wl.batch, int(suf.mean()), int(suf.max())), DEV)
@@ -251,18 +278,23 @@ def test_full_size_cfg4_shared_prefix_step_sampled():
     torch.cuda.synchronize()
     out_sp = out_sp.float().cpu().numpy().astype(np.float64)
     assert np.all(np.abs(out_sp - out) <= 2 * (H.ATOL + H.RTOL * np.abs(out)))      # every sequence, against the plain path
-    order = np.argsort(wl.ctx_lens)
-    for b in (int(order[0]), int(order[len(order) // 2])):          # shortest and median sequence
+    sample, capped = _cfg4_sample(wl)
+    assert len(sample) >= 32 and len(capped) >= 1 and set(capped) <= set(sample)
+    assert int(np.argmax(wl.ctx_lens)) in sample and int(np.argmin(wl.ctx_lens)) in sample
+    q_bits, q_fp8 = H.bits(q), bufs.q_fp8.cpu().numpy()
+    kp, vp = W.gen_kv(wl, -1, 0, wl.prefix_len, DEV)                   # the shared prefix rows, generated once
+    for b in sample:
         L0 = int(wl.ctx_lens[b])
-        k0, v0 = W.seq_kv(wl, b, L0, DEV)
-        k = torch.cat([k0, k_new[b:b + 1]])
-        v = torch.cat([v0, v_new[b:b + 1]])
+        ks, vs = W.gen_kv(wl, b, 0, L0 - wl.prefix_len, DEV)
+        k = torch.cat([kp, ks, k_new[b:b + 1]])
+        v = torch.cat([vp, vs, v_new[b:b + 1]])
         arrays = oracle.encode_kv(H.bits(k), H.bits(v))
         H.compare_cache(cache, wl, b, L0 + 1, arrays)
-        ref, q8 = H.oracle_out(wl, b, L0 + 1, H.bits(q)[b], arrays)
-        assert np.array_equal(bufs.q_fp8[b].cpu().numpy(), q8)
-        H.check_out(out[b], ref, f"cfg4 full seq {b}")
-        H.check_out(out_sp[b], ref, f"cfg4 full seq {b}, shared-prefix path")
+        ref, q8 = H.oracle_out(wl, b, L0 + 1, q_bits[b], arrays)
+        assert np.array_equal(q_fp8[b], q8)
+        H.check_out(out[b], ref, f"cfg4 full seq {b} ({L0 + 1} tokens)")
+        H.check_out(out_sp[b], ref, f"cfg4 full seq {b} ({L0 + 1} tokens), shared-prefix path")
+        del arrays
 
 
 def test_host_staged_step_equals_device_step_and_oracle():
