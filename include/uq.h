@@ -169,7 +169,19 @@ int32_t uq_rotate_quantize_append(const uq_config* cfg, const void* k_new, const
  * UE8M0 group scales applied by the tensor core, fp32 accumulation in TMEM); exp in fp32
  * (ex2.approx); P and Vhat enter the PV product (tcgen05.mma kind::f16) as fp16, Vhat relative to
  * a running reference exponent (values more than 2^25 below the largest V scale seen so far
- * flush to zero); accumulation in fp32 in TMEM.  Error bound vs the float64 oracle: DESIGN.md "Tolerance".
+ * flush to zero); accumulation in fp32 in TMEM.
+ *
+ * Accuracy domain.  With p_t the softmax weights and A[h,d] = sum_t p_t |vhat[t,d]| the ABSOLUTE attention mass of an
+ * output element, the merged output satisfies
+ *     |out - ref| <= 2^-8 |ref| + 2^-10 A[h,d]        (ref = the float64 oracle on the same codes)
+ * — bf16 output rounding, fp32 accumulation and ex2.approx in the first term, the fp16 rounding of P (2^-11 per term,
+ * which cancelling terms do not cancel) in the second.  The north-star bound |out - ref| <= 2e-3 + 1e-2 |ref| is
+ * therefore GUARANTEED for A <= 2 (values of unit scale, the case of every BASELINE.json config: A ~ 0.8 for N(0,1)
+ * values) and for outputs that dominate their own mass (|ref| >= 0.2 A: peaked attention at any scale); it is not
+ * guaranteed where terms much larger than 2 cancel to a small output (V scaled by 2^12 with diffuse attention:
+ * measured errors of 0.05 on outputs of 1.3 with A = 279).  Softmax weights below 2^-24 of a split's reference weight
+ * underflow in fp16 and are dropped from the numerator: harmless unless more than 2^-10 of a row's mass sits on such
+ * tokens (a single token dominating > 10^4 others by exactly 2^24..2^25).  DESIGN.md "Tolerance" derives both.
  */
 int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, const void* cache,
                             int64_t num_pages, const int32_t* block_tables, int32_t max_pages,
