@@ -44,9 +44,33 @@ UNIT = "GB/s"
 NOMINAL_HBM_GBS = 8000.0          # BASELINE.json north_star: "the B200's ~8 TB/s peak"
 FALLBACK_HBM_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md fallback
 
-# dram__bytes_read.sum + dram__bytes_write.sum per decode_kernel launch from the committed
-# `ncu --set full` capture of this command (profiles/), keyed by config; None = not captured.
-NCU_TRAFFIC_BYTES = {2: 571_073_792 + 4_757_760}   # dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01_v16_decode_cfg2.md
+
+
+def _source_key() -> str:
+    """sha256 (first 16 hex digits) over the CUDA sources the library is built from, in name order: identifies the
+    BUILD a profile was taken of (the GPU box has no .git, so a commit id is not available at run time)."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2606_20474_b200", "csrc")
+    for fn in sorted(os.listdir(d)):
+        if fn.endswith((".cu", ".cuh")):
+            h.update(fn.encode()); h.update(open(os.path.join(d, fn), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def _ncu_traffic(kernel: str, workload_key: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the `ncu --set full` capture recorded
+    in profiles/ncu_traffic.json — only if that capture was taken of THIS build (same source key); else None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+            tab = json.load(f)
+    except Exception:
+        return None
+    key = _source_key()
+    for e in tab.get("captures", []):
+        if e.get("source_key") == key and e.get("kernel") == kernel and e.get("workload") == workload_key:
+            return int(e["dram_bytes_read"]) + int(e["dram_bytes_write"])
+    return None
 
 
 # ----------------------------------------------------------------------------- helpers
@@ -107,8 +131,8 @@ class ClockSampler(threading.Thread):
     def __init__(self, index: int, period_s: float = 0.005):
         super().__init__(daemon=True)
         self.period = period_s
-        self.samples = []            # (busy flag, sm_mhz, reasons bitmask)
-        self.busy = False
+        self.samples = []            # (window label or None/False, sm_mhz, reasons bitmask)
+        self.busy = False            # label of the timed window being sampled (True = the default one)
         self._stop_evt = threading.Event()
         self.ok = False
         self.max_mhz = None
@@ -138,11 +162,15 @@ class ClockSampler(threading.Thread):
     def stop(self):
         self._stop_evt.set()
 
-    def summary(self):
+    def summary(self, label=None):
+        """Clocks over the samples of one labelled window (label given) or of every timed window except 'sustain'."""
         if not self.ok:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml_unavailable"]}
         nv = self.nv
-        busy = [s for s in self.samples if s[0]] or self.samples
+        if label is not None:
+            busy = [s for s in self.samples if s[0] == label]
+        else:
+            busy = [s for s in self.samples if s[0] and s[0] != "sustain"] or self.samples
         names = {
             getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
             getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
@@ -265,15 +293,30 @@ def run_ours(args, rank, world, local_rank):
         step(i)
     ev1.record(stream)
     barrier()
+    sampler.busy = False
     ms_total = ev0.elapsed_time(ev1)
 
-    # ---- the same K steps once more with an event on both sides of every decode launch (the dominant kernel's
+    # ---- the spread over steps: the same K steps (at most 200) with an event after every step.  (An event between two
+    # steps ends the programmatic overlap of merge(i) with append(i+1), so these are a little longer than ms_per_step.)
+    n_sp = min(args.steps, 200)
+    sp_ev = [torch.cuda.Event(enable_timing=True) for _ in range(n_sp + 1)]
+    sampler.busy = True
+    sp_ev[0].record(stream)
+    for i in range(n_sp):
+        step(i)
+        sp_ev[i + 1].record(stream)
+    barrier()
+    sampler.busy = False
+    step_ms = [a.elapsed_time(b) for a, b in zip(sp_ev[:-1], sp_ev[1:])]
+
+    # ---- the same steps once more with an event on both sides of every decode launch (the dominant kernel's
     # duration for the roofline; an event between two launches ends their programmatic overlap, so this pass
     # is not the one `value` is taken from)
     # (at most 50 steps: on the long configs a second full-length pass runs into sw_power_cap and times the cap)
     n_inst = min(args.steps, 50)
     dec_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
               for _ in range(n_inst)]
+    sampler.busy = True
     for i in range(n_inst):
         k_new, v_new = kvs[i % n_in]
         uq.rotate_quantize_append(cfg, k_new, v_new, cu_dev, before_dev, bt_dev, cache,
@@ -286,6 +329,27 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     sampler.busy = False
     dec_ms = [a.elapsed_time(b) for a, b in dec_ev]
+
+    # ---- sustained: back-to-back steps for at least --sustain seconds between two events (north_star: "sustaining
+    # >= 70 % of B200 HBM peak"), with its own clock record — a 2 ms burst runs at boost clock, seconds of
+    # full-bandwidth load run under the 1 kW power cap
+    sustained = None
+    if args.sustain > 0:
+        est = max_over_ranks([ms_total / args.steps], world, dev)[0]
+        n_sus = max(args.steps, int(args.sustain * 1e3 / max(est, 1e-3)) + 1)
+        for i in range(3):
+            step(i)
+        barrier()
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        sampler.busy = "sustain"
+        s0.record(stream)
+        for i in range(n_sus):
+            step(i)
+        s1.record(stream)
+        barrier()
+        sampler.busy = False
+        sustained = (n_sus, s0.elapsed_time(s1))
+        time.sleep(0.5)                                # let the part cool off before the end-to-end leg
 
     # ---- end-to-end through the public host-buffer API: H2D of the step's inputs, D2H of O
     # one pinned staging block per entry of the input ring (the caller's own buffers: it writes a step's inputs
@@ -325,7 +389,9 @@ def run_ours(args, rank, world, local_rank):
 
     # ---- reduce over ranks: max time, summed bytes
     total_b, decode_b = step_bytes(wl, S, ctx_after, 1)
-    ms_total, ms_e2e, dec_ms_mean = max_over_ranks([ms_total, ms_e2e, statistics.fmean(dec_ms)], world, dev)
+    red = max_over_ranks([ms_total, ms_e2e, statistics.fmean(dec_ms), statistics.median(dec_ms), min(dec_ms),
+                          statistics.median(step_ms), min(step_ms), sustained[1] if sustained else 0.0], world, dev)
+    ms_total, ms_e2e, dec_ms_mean, dec_ms_med, dec_ms_min, step_ms_med, step_ms_min, ms_sus = red
     ms_step = ms_total / args.steps
     value = whole_job_value(total_b, world, ms_step)
     e2e_value = whole_job_value(total_b, world, ms_e2e / args.steps)
@@ -344,7 +410,10 @@ def run_ours(args, rank, world, local_rank):
                    "num_splits": S, "parallelism": f"replica x{world} (sequences sharded, no collective)",
                    "l2": f"KV working set {wl.kv_bytes_per_step() / 1e6:.0f} MB per step >> 126 MB L2 (no flush needed)"},
         "us_per_step": round(ms_step * 1e3, 2),
+        "us_per_step_spread": {"median": round(step_ms_med * 1e3, 2), "min": round(step_ms_min * 1e3, 2), "steps": n_sp,
+                               "note": "one event per step (ends the overlap of merge(i) with append(i+1))"},
         "decode_kernel_us": round(dec_ms_mean * 1e3, 2),
+        "decode_kernel_us_spread": {"median": round(dec_ms_med * 1e3, 2), "min": round(dec_ms_min * 1e3, 2), "launches": n_inst},
         "bytes_per_step": total_b,
         **({"shared_prefix": {
             "note": "bytes_per_step / value / roofline count LOGICAL bytes; the prefix pages are named by every block "
@@ -359,12 +428,20 @@ def run_ours(args, rank, world, local_rank):
                 "d2h_bytes_per_step": int(d2h), "us_per_step": round(ms_e2e / args.steps * 1e3, 2),
                 "note": "uq.HostStepGraph (one CUDA-graph launch per step): host pinned Q/K_new/V_new/lens/block tables -> device (one staged copy), three kernels, O -> host, sync every step; "
                         "the FP4 cache is resident state"},
-        "gpu_launches": 3 * args.steps,
+        "gpu_launches": (4 if pbufs is not None else 3) * args.steps,
         "clocks": sampler.summary(),
+        **({"sustained": {
+            "value": round(whole_job_value(total_b, world, ms_sus / sustained[0]), 1), "unit": UNIT,
+            "us_per_step": round(ms_sus / sustained[0] * 1e3, 2), "steps": sustained[0], "seconds": round(ms_sus * 1e-3, 3),
+            "frac_of_nominal_8TBs": round(whole_job_value(total_b, world, ms_sus / sustained[0]) / world / NOMINAL_HBM_GBS, 4),
+            "frac_of_measured_peak": round(whole_job_value(total_b, world, ms_sus / sustained[0]) / world / peak, 4),
+            "clocks": sampler.summary("sustain"),
+            "note": "the same step, back to back for at least --sustain seconds between two CUDA events"}} if sustained else {}),
         "roofline": {"bound": "hbm", "kernel": "uq::decode_kernel", "achieved": round(achieved, 1),
                      "peak": peak, "unit": "GB/s", "frac": round(achieved / peak, 4),
                      "frac_of_nominal_8TBs": round(achieved / NOMINAL_HBM_GBS, 4),
-                     "traffic": NCU_TRAFFIC_BYTES.get(args.config), "algorithmic_bytes": decode_b,
+                     "traffic": _ncu_traffic("decode_kernel", f"cfg{args.config}"), "algorithmic_bytes": decode_b,
+                     "source_key": _source_key(),
                      "peak_source": peak_src,
                      "timing": "CUDA events around every uq_decode_attention launch, mean over a second pass of the same K steps "
                                "(at most 50; events between launches would end the programmatic overlap of the timed pass)"},
@@ -425,10 +502,24 @@ def cpu_baseline(idx: int, budget_s: float = 15.0):
     t0 = time.perf_counter()
     nbytes = _oracle_step(oracle, wl, q, k_new, v_new, seqs)
     dt = time.perf_counter() - t0
+    # the same oracle on ONE core ("timed on 1 core and on all cores"), on a sample sized for ~budget/3
+    one = None
+    try:
+        oracle.set_num_threads(1)
+        len1 = int(min(full_len, max(1024, (int(tok_per_s / max(cores, 1) * budget_s / 3) // 16) * 16)))
+        wl1, q1, k1, v1, seqs1 = _oracle_sample(idx, 1, len1)
+        t0 = time.perf_counter()
+        nb1 = _oracle_step(oracle, wl1, q1, k1, v1, seqs1)
+        dt1 = time.perf_counter() - t0
+        one = {"value": round(nb1 / dt1 / 1e9, 5), "unit": UNIT, "cores": 1, "seconds": round(dt1, 3),
+               "sample": f"sequence 0 of config {idx} truncated to {seqs1[0][0]} tokens"}
+    finally:
+        oracle.set_num_threads(cores)
     return {"value": round(nbytes / dt / 1e9, 5), "unit": UNIT, "cores": cores, "kind": "oracle",
             "seconds": round(dt, 3),
             "sample": f"{n_seq} of {wl.batch} sequences of config {idx}, {seqs[0][0]} tokens each "
                       f"(append 1 token + Q encode + float64 attention, all {wl.num_q_heads} heads)",
+            "one_core": one,
             "quant_error_vs_bf16": _quant_error_context(oracle, idx)}
 
 
@@ -540,8 +631,7 @@ def run_bulk_append(args):
             "bytes_per_step": nbytes, "gpu_launches": args.steps,
             "roofline": {"bound": "hbm", "kernel": "uq::append_bulk_kernel", "achieved": round(gbs, 1), "peak": peak,
                          "unit": "GB/s", "frac": round(gbs / peak, 4),
-                         # dram__bytes_read.sum + write.sum of the ncu capture in profiles/r01_append_bulk_cfg2.md
-                         "traffic": 662109440 if (args.config, n, nseq) == (2, 32768, 8) else None,
+                         "traffic": _ncu_traffic("append_bulk_kernel", f"cfg{args.config}_bulk{n}x{nseq}"),
                          "algorithmic_bytes": nbytes, "peak_source": peak_src}}
 
 
@@ -613,6 +703,8 @@ def main():
                     help="instead of the decode step, time bulk quantize-on-append of TOKENS new tokens per call")
     ap.add_argument("--calibrate", type=int, default=0, metavar="VECTORS",
                     help="instead of the decode step, time uq_calibrate_c over VECTORS key vectors and 56 constants")
+    ap.add_argument("--sustain", type=float, default=2.0, metavar="SECONDS",
+                    help="also time back-to-back steps for at least SECONDS (own clock record); 0 = skip")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--ref-budget", type=float, default=90.0, help="seconds for the whole --impl reference run")
     args = ap.parse_args()

@@ -24,6 +24,7 @@ def _stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not (force or _stale()):
         return LIB
+    extra = os.environ.get("UQ_NVCC_EXTRA", "").split()      # experiments only (e.g. -DUQ_KSTAGES=2)
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     # ptxas -O1 for the decode kernel only: measured, not assumed — it is bound by the serial instruction streams of
     # twelve warps sharing four schedulers, and the -O3 schedule of the same SASS-level work is 2 % slower on config 2
@@ -33,7 +34,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
     objs = []
     for src in SOURCES:
         obj = os.path.join(HERE, src.replace(".cu", ".o"))
-        cmd = common + PTXAS_FLAGS.get(src, []) + ["-c", "-o", obj, os.path.join(CSRC, src)]
+        flags = PTXAS_FLAGS.get(src, [])
+        if os.environ.get("UQ_PTXAS_O") and flags:
+            flags = ["-Xptxas", "-O" + os.environ["UQ_PTXAS_O"]]
+        cmd = common + flags + extra + ["-c", "-o", obj, os.path.join(CSRC, src)]
         res = subprocess.run(cmd, capture_output=True, text=True)
         if verbose or res.returncode != 0:
             sys.stderr.write(res.stdout + res.stderr)
