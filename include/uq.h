@@ -27,12 +27,19 @@
  *  - The library may be used on several devices of one process: a call runs on the CURRENT device
  *    (cudaSetDevice), which must own every pointer passed; per-device state (SM count, shared-memory
  *    opt-in of the kernels, TMA descriptors) is kept per device and guarded by mutexes.
- *  - Supported geometry in this version: head_dim = 128, group_size = 32, page_size = 16,
- *    num_q_heads / num_kv_heads in 1..16, batch <= 2048 for uq_decode_attention
- *    (UQ_ERR_UNSUPPORTED otherwise).
+ *  - Supported geometry in this version: head_dim in {64, 128, 256} (the head sizes the paper validates,
+ *    PAPER.md:322), group_size = 32, page_size = 16, num_q_heads / num_kv_heads in 1..16, batch <= 2048 for
+ *    uq_decode_attention (UQ_ERR_UNSUPPORTED otherwise).  head_dim 128 — the geometry of every BASELINE.json
+ *    config — is the tuned path; at 64 and 256 uq_rotate_quantize_append runs its float64 kernel only (no float32
+ *    fast path, no bulk kernel), uq_decode_attention the same CTA design re-sized, and
+ *    uq_decode_prefix_attention / uq_calibrate_c return UQ_ERR_UNSUPPORTED.
  *  - GQA map: query head h reads KV head h / (num_q_heads/num_kv_heads).
  *
- * PHYSICAL CACHE LAYOUT (uint8).  cache[num_pages][num_kv_heads][UQ_RECORD_BYTES]; the record
+ * PHYSICAL CACHE LAYOUT (uint8), written out for head_dim 128; for head_dim D the record has 17 D bytes
+ * (uq_cache_record_bytes) and the four regions are [0, 8D) K codes (token t at (D/2) t), [8D, 16D) V codes (word at
+ * 8D + 4D (t>>3) + 128 (d>>5) + 4 (d&31)), [16D, 16D + D/2) K scales (token t's D/32 bytes at 16D + (D/32) t) and
+ * [16D + D/2, 17D) V scales (token t, group g at 16D + D/2 + (D/4)(t>>3) + 8 g + (t&7)).
+ * cache[num_pages][num_kv_heads][UQ_RECORD_BYTES]; the record
  * of (page p, kv head h) starts at byte (p*num_kv_heads + h)*2176 and holds 16 tokens with
  * exactly 4.25 bit/element and no padding.  The cache base must be 32-byte aligned (the K
  * codes are fetched by TMA as packed 4-bit tensors).  With t = token slot in the page
@@ -96,7 +103,7 @@ typedef struct {
 /* Host.  Static, thread-local description of the last error returned on this thread. */
 const char* uq_last_error_string(void);
 
-/* Host.  Bytes of one (page, kv_head) record: page_size*(d/2 + d/32)*2 = 2176; 0 if unsupported. */
+/* Host.  Bytes of one (page, kv_head) record: page_size*(d/2 + d/32)*2 = 17 d = 2176 at d = 128; 0 if unsupported. */
 size_t uq_cache_record_bytes(const uq_config* cfg);
 
 /* Host.  Device scratch uq_decode_attention / uq_decode_prefix_attention need beyond the caller's partial buffers for

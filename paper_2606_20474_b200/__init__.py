@@ -10,6 +10,7 @@ from .binding import (  # noqa: F401
     UQConfig,
     UQError,
     RECORD_BYTES,
+    record_bytes,
     StepBuffers,
     StepGraph,
     HostStage,

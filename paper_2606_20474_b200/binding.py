@@ -12,7 +12,12 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libuq.so")
 _lib = None
 
-RECORD_BYTES = 2176
+RECORD_BYTES = 2176          # head_dim 128; in general 17 * head_dim (record_bytes())
+
+
+def record_bytes(head_dim: int = 128) -> int:
+    """Bytes of one (page, kv head) record: 16 tokens x (d/2 + d/32) x 2 = 17 d (include/uq.h)."""
+    return 17 * int(head_dim)
 
 
 class UQError(RuntimeError):
@@ -138,8 +143,8 @@ def suggest_num_splits_max(cfg: UQConfig, batch: int, avg_seq_len: int, max_seq_
 
 
 def alloc_cache(cfg: UQConfig, num_pages: int, device="cuda") -> torch.Tensor:
-    """uint8 [num_pages, num_kv_heads, 2176] (layout: include/uq.h)."""
-    return torch.zeros((num_pages, cfg.num_kv_heads, RECORD_BYTES), dtype=torch.uint8, device=device)
+    """uint8 [num_pages, num_kv_heads, 17 * head_dim] (2176 at head_dim 128; layout: include/uq.h)."""
+    return torch.zeros((num_pages, cfg.num_kv_heads, record_bytes(cfg.head_dim)), dtype=torch.uint8, device=device)
 
 
 def rotate_quantize_append(cfg: UQConfig, k_new, v_new, cu_new, seq_lens, block_tables, cache,

@@ -39,8 +39,9 @@ int32_t check_config(const uq_config* cfg) {
     set_error("uq_config: unknown bit in flags");
     return UQ_ERR_INVALID_ARG;
   }
-  if (cfg->head_dim != kHeadDim || cfg->group_size != kGroup || cfg->page_size != kPage) {
-    set_error("unsupported geometry: head_dim %d group %d page %d (supported: 128/32/16)",
+  if ((cfg->head_dim != 64 && cfg->head_dim != 128 && cfg->head_dim != 256) || cfg->group_size != kGroup ||
+      cfg->page_size != kPage) {
+    set_error("unsupported geometry: head_dim %d group %d page %d (supported: 64|128|256 / 32 / 16)",
               cfg->head_dim, cfg->group_size, cfg->page_size);
     return UQ_ERR_UNSUPPORTED;
   }
@@ -49,6 +50,12 @@ int32_t check_config(const uq_config* cfg) {
     return UQ_ERR_UNSUPPORTED;
   }
   return UQ_OK;
+}
+
+int32_t require_head_dim_128(const uq_config* cfg, const char* who) {
+  if (cfg->head_dim == kHeadDim) return UQ_OK;
+  set_error("%s: head_dim %d is not supported by this entry point (128 only)", who, cfg->head_dim);
+  return UQ_ERR_UNSUPPORTED;
 }
 
 int32_t check_cuda(cudaError_t e, const char* what) {
@@ -141,7 +148,7 @@ extern "C" int32_t uq_suggest_num_splits(const uq_config* cfg, int32_t batch, in
   // (sequence, kv head) of T tiles then spans about T / range + 1 CTAs = slots.  Leave room for sequences
   // twice the average length.
   const int64_t items = (int64_t)batch * cfg->num_kv_heads;
-  const int64_t slots = (int64_t)sms * 2;
+  const int64_t slots = (int64_t)sms * (cfg->head_dim == 256 ? 1 : 2);   // resident decode CTAs
   const int64_t pages = (avg_seq_len + cfg->page_size - 1) / cfg->page_size;
   const int64_t tiles = (pages + 7) / 8 > 0 ? (pages + 7) / 8 : 1;
   int64_t range = (items * tiles + slots - 1) / slots;
@@ -164,7 +171,8 @@ extern "C" int32_t uq_suggest_num_splits_max(const uq_config* cfg, int32_t batch
   if (uq::current_device_sms(&sms) != UQ_OK) sms = 148;   // no device (a host-only caller sizing buffers): B200's count
   const int64_t tiles_avg = ((int64_t)avg_seq_len + 127) / 128 > 0 ? ((int64_t)avg_seq_len + 127) / 128 : 1;
   const int64_t tiles_max = ((int64_t)max_seq_len + 127) / 128;
-  int64_t range = ((int64_t)batch * cfg->num_kv_heads * tiles_avg + 2 * sms - 1) / (2 * sms);
+  const int64_t resident = (int64_t)sms * (cfg->head_dim == 256 ? 1 : 2);
+  int64_t range = ((int64_t)batch * cfg->num_kv_heads * tiles_avg + resident - 1) / resident;
   if (range < 1) range = 1;
   int64_t s = tiles_max / range + 2;
   if (s < base) s = base;

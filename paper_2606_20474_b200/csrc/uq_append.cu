@@ -664,6 +664,152 @@ int32_t rows_map(const void* rows, long long n_rows, int Hkv, CUtensorMap* out) 
   return UQ_OK;
 }
 
+
+// ---------------------------------------------------------------- head_dim 64 / 256: the float64 path, any D
+// One warp per (aligned octet of positions, kv head) or per query row, dealt out exactly as in append_kernel; a lane
+// owns N = D/32 consecutive channels (2 or 8), a 32-channel scale group is 32/N lanes.  Everything is float64 on exact
+// sums (uq_quant.cuh's rules: the decisions are the oracle's); no float32 fast path and no bulk kernel for these head
+// sizes — the tuned kernels above are written for head_dim 128, the geometry of every BASELINE.json config.
+template <int D>
+__device__ __forceinline__ void load_row(const uint16_t* row, int lane, double (&x)[D / 32]) {
+  if constexpr (D == 64) {
+    const uint32_t raw = *reinterpret_cast<const uint32_t*>(row + 2 * lane);
+    x[0] = bf16_bits_to_double(raw & 0xFFFFu);
+    x[1] = bf16_bits_to_double(raw >> 16);
+  } else if constexpr (D == 128) {
+    load4(row, lane, x);
+  } else {
+    const uint4 raw = *reinterpret_cast<const uint4*>(row + 8 * lane);
+    const uint32_t w[4] = {raw.x, raw.y, raw.z, raw.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      x[2 * i] = bf16_bits_to_double(w[i] & 0xFFFFu);
+      x[2 * i + 1] = bf16_bits_to_double(w[i] >> 16);
+    }
+  }
+}
+
+// y = H_D x / sqrt(D) (Sylvester order): index bits 0..log2(N)-1 inside the lane, the other five through shuffles
+template <int D>
+__device__ __forceinline__ void wht_any(double (&x)[D / 32], int lane) {
+  constexpr int N = D / 32;
+#pragma unroll
+  for (int h = 1; h < N; h <<= 1) {
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+      if ((i & h) == 0) {
+        const double a = x[i], b = x[i | h];
+        x[i] = __dadd_rn(a, b);
+        x[i | h] = __dadd_rn(a, -b);
+      }
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    const bool upper = (lane >> k) & 1;
+#pragma unroll
+    for (int r = 0; r < N; ++r) {
+      const double other = __shfl_xor_sync(kFull, x[r], 1 << k);
+      x[r] = upper ? __dadd_rn(other, -x[r]) : __dadd_rn(x[r], other);
+    }
+  }
+  // correctly rounded 2^(-log2(D)/2): exact powers of two for D = 64 and 256
+  const double kappa = D == 64 ? 0x1p-3 : D == 256 ? 0x1p-4 : 0x1.6a09e667f3bcdp-4;
+#pragma unroll
+  for (int r = 0; r < N; ++r) x[r] = __dmul_rn(x[r], kappa);
+}
+
+// scale exponent of the lane's 32-channel group (32/N lanes)
+template <int D>
+__device__ __forceinline__ int group_exponent_any(const double (&y)[D / 32], double c) {
+  constexpr int N = D / 32;
+  double m = fabs(y[0]);
+#pragma unroll
+  for (int r = 1; r < N; ++r) m = fmax(m, fabs(y[r]));
+#pragma unroll
+  for (int s = 1; s < 32 / N; s <<= 1) m = fmax(m, __shfl_xor_sync(kFull, m, s));
+  return scale_exponent(c, m);
+}
+
+template <int D>
+__device__ __forceinline__ void append_octet_any(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v_new,
+                                                 uint8_t* rec, int c0, int p0, int q0, int t_lo, int t_hi, int h, int Hkv,
+                                                 int lane, double c_k, double c_v) {
+  using R = RecordGeo<D>;
+  constexpr int N = D / 32, LPG = 32 / N;               // channels per lane, lanes per scale group
+  uint32_t* dst = reinterpret_cast<uint32_t*>(rec + R::kVCodes + 4 * D * ((q0 >> 3) & 1) + 4 * N * lane);
+  uint32_t vw[N];
+#pragma unroll
+  for (int r = 0; r < N; ++r) vw[r] = 0u;
+  for (int pos = t_lo; pos < t_hi; ++pos) {
+    const long long row = ((long long)(c0 + (pos - p0)) * Hkv + h) * D;
+    const int t = pos & 15;
+    double x[N];
+    // ---- K: rotate, group exponent, codes in logical order, scale bytes
+    load_row<D>(k_new + row, lane, x);
+    wht_any<D>(x, lane);
+    int E = group_exponent_any<D>(x, c_k);
+    uint32_t kc = 0u;
+#pragma unroll
+    for (int r = 0; r < N; ++r) kc |= e2m1_code(x[r], E) << (4 * r);
+    if constexpr (N == 2) rec[R::kKCodes + (D / 2) * t + lane] = (uint8_t)kc;
+    else *reinterpret_cast<uint32_t*>(rec + R::kKCodes + (D / 2) * t + 4 * lane) = kc;
+    if ((lane % LPG) == 0) rec[R::kKScales + (D / 32) * t + lane / LPG] = (uint8_t)(E + 127);
+    // ---- V: no rotation; the token's nibble of every channel word, scale bytes
+    load_row<D>(v_new + row, lane, x);
+    E = group_exponent_any<D>(x, c_v);
+#pragma unroll
+    for (int r = 0; r < N; ++r) vw[r] |= e2m1_code(x[r], E) << (4 * (pos & 7));
+    if ((lane % LPG) == 0) rec[R::kVScales + (D / 4) * (t >> 3) + 8 * (lane / LPG) + (t & 7)] = (uint8_t)(E + 127);
+  }
+  // the tokens of the octet that are not part of the call keep their nibbles
+  const uint32_t below_hi = (t_hi - q0 == 8) ? 0xFFFFFFFFu : ((1u << (4 * (t_hi - q0))) - 1u);
+  const uint32_t m = below_hi & ~((1u << (4 * (t_lo - q0))) - 1u);
+#pragma unroll
+  for (int r = 0; r < N; ++r) dst[r] = (m == 0xFFFFFFFFu) ? vw[r] : ((dst[r] & ~m) | (vw[r] & m));
+}
+
+template <int D>
+__global__ void __launch_bounds__(128)
+append_any_kernel(const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v_new,
+                  const int32_t* __restrict__ cu_new, const int32_t* __restrict__ seq_lens,
+                  const int32_t* __restrict__ block_tables, int max_pages, int batch, int total_new,
+                  int Hq, int Hkv, uint8_t* __restrict__ cache, const uint16_t* __restrict__ q,
+                  uint8_t* __restrict__ q_fp8, double c_k, double c_v) {
+  pdl_launch_dependents();
+  pdl_wait();
+  constexpr int N = D / 32;
+  const int lane = threadIdx.x & 31;
+  if ((int)blockIdx.y < Hkv) {                         // K/V units: see append_kernel
+    const int u = (int)blockIdx.x * 4 + (int)(threadIdx.x >> 5), h = (int)blockIdx.y;
+    const int n_units = (total_new >> 3) + 2 * batch;
+    if (total_new == 0 || u >= n_units) return;
+    const int b = find_sequence<3>(cu_new, batch, u, n_units, lane);
+    const int c0 = cu_new[b], cnt = cu_new[b + 1] - c0, p0 = seq_lens[b];
+    const int q0 = ((p0 >> 3) + (u - ((c0 >> 3) + 2 * b))) << 3;
+    const int t_lo = max(p0, q0), t_hi = min(p0 + cnt, q0 + 8);
+    if (t_lo >= t_hi) return;
+    const int page = block_tables[(long long)b * max_pages + (q0 >> 4)];
+    uint8_t* rec = cache + ((long long)page * Hkv + h) * RecordGeo<D>::kBytes;
+    append_octet_any<D>(k_new, v_new, rec, c0, p0, q0, t_lo, t_hi, h, Hkv, lane, c_k, c_v);
+    return;
+  }
+  const long long qu = ((long long)((int)blockIdx.y - Hkv) * gridDim.x + blockIdx.x) * 4 + (threadIdx.x >> 5);
+  if (q != nullptr && qu < (long long)batch * Hq) {    // query rows: rotate, E4M3 bytes
+    double x[N];
+    load_row<D>(q + qu * D, lane, x);
+    wht_any<D>(x, lane);
+    if constexpr (N == 2) {
+      *reinterpret_cast<uint16_t*>(q_fp8 + qu * D + 2 * lane) = (uint16_t)(e4m3_byte(x[0]) | (e4m3_byte(x[1]) << 8));
+    } else {
+#pragma unroll
+      for (int w = 0; w < N / 4; ++w)
+        *reinterpret_cast<uint32_t*>(q_fp8 + qu * D + N * lane + 4 * w) =
+            e4m3_byte(x[4 * w]) | (e4m3_byte(x[4 * w + 1]) << 8) | (e4m3_byte(x[4 * w + 2]) << 16) | (e4m3_byte(x[4 * w + 3]) << 24);
+    }
+  }
+}
+
 }  // namespace
 }  // namespace uq
 
@@ -699,6 +845,27 @@ extern "C" int32_t uq_rotate_quantize_append(const uq_config* cfg, const void* k
     st = debug_check_tables("uq_rotate_quantize_append", block_tables, max_pages, batch, num_pages, seq_lens, cu_new,
                             total_new, 0, cfg->page_size, 1, (cudaStream_t)stream);
     if (st != UQ_OK) return st;
+  }
+  if (cfg->head_dim == 256 && (((uintptr_t)k_new | (uintptr_t)v_new | (uintptr_t)q) & 15u)) {
+    set_error("append: head_dim 256 needs k_new / v_new / q 16-byte aligned");
+    return UQ_ERR_INVALID_ARG;
+  }
+  if (cfg->head_dim != kHeadDim) {                     // head_dim 64 / 256: the generic float64 kernel, same grid shape
+    long long gx = total_new > 0 ? (((long long)(total_new >> 3) + 2LL * batch) + 3) / 4 : 0;
+    gx = gx > (q_rows + 4 * 60000LL - 1) / (4 * 60000LL) ? gx : (q_rows + 4 * 60000LL - 1) / (4 * 60000LL);
+    if (gx < 1) gx = 1;
+    const long long gy = cfg->num_kv_heads + (q_rows + 4 * gx - 1) / (4 * gx);
+    if (gx > 0x7fffffffLL || gy > 65535) {
+      set_error("append: too many work units");
+      return UQ_ERR_INVALID_ARG;
+    }
+    auto kern = cfg->head_dim == 64 ? append_any_kernel<64> : append_any_kernel<256>;
+    return check_cuda(launch_pdl(kern, dim3((unsigned)gx, (unsigned)gy), dim3(128), 0, (cudaStream_t)stream,
+                                 (const uint16_t*)k_new, (const uint16_t*)v_new, cu_new, seq_lens, block_tables,
+                                 (int)max_pages, (int)batch, (int)total_new, (int)cfg->num_q_heads,
+                                 (int)cfg->num_kv_heads, (uint8_t*)cache, (const uint16_t*)q, (uint8_t*)q_fp8,
+                                 (double)cfg->c_k, (double)cfg->c_v),
+                      "uq_rotate_quantize_append (head_dim 64/256) launch");
   }
   // Prefill-sized calls (on average 64 or more new tokens per sequence): K/V through append_bulk_kernel, one warp per
   // page; the kernel below then only encodes the query rows.  Same bytes either way.

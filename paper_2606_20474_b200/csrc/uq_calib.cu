@@ -111,6 +111,8 @@ extern "C" int32_t uq_calibrate_c(const uq_config* cfg, const void* x, int64_t n
   using namespace uq;
   int32_t st = check_config(cfg);
   if (st != UQ_OK) return st;
+  st = require_head_dim_128(cfg, "uq_calibrate_c");
+  if (st != UQ_OK) return st;
   if (!x || !c_grid || !sq_err || !sq_norm || n_vec <= 0 || n_c <= 0) {
     set_error("calibrate: NULL pointer or non-positive size");
     return UQ_ERR_INVALID_ARG;

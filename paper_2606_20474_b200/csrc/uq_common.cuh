@@ -11,7 +11,7 @@
 
 namespace uq {
 
-constexpr int kHeadDim = 128;
+constexpr int kHeadDim = 128;                  // the head_dim the tuned kernels are written for
 constexpr int kGroup = 32;
 constexpr int kPage = 16;
 constexpr int kRecordBytes = UQ_RECORD_BYTES;  // 2176
@@ -19,6 +19,22 @@ constexpr int kOffKCodes = 0;
 constexpr int kOffVCodes = 1024;
 constexpr int kOffKScales = 2048;
 constexpr int kOffVScales = 2112;
+
+// Record geometry for head_dim D in {64, 128, 256} (include/uq.h "PHYSICAL CACHE LAYOUT"): 16 tokens x (D/2 + D/32)
+// bytes for K and the same for V = 17 D bytes; K codes | V codes | K scales | V scales.
+template <int D>
+struct RecordGeo {
+  static_assert(D == 64 || D == 128 || D == 256, "head_dim must be 64, 128 or 256");
+  static constexpr int kGroups = D / kGroup;           // scale bytes per vector
+  static constexpr int kBytes = 17 * D;                // 1088 / 2176 / 4352
+  static constexpr int kKCodes = 0;                    // 16 x D/2
+  static constexpr int kVCodes = 8 * D;                // 2 octets x D words
+  static constexpr int kKScales = 16 * D;              // 16 x D/32
+  static constexpr int kVScales = 16 * D + D / 2;      // 2 octets x D/32 groups x 8
+  static constexpr int kRest = 9 * D;                  // the record without its K codes
+};
+static_assert(RecordGeo<128>::kBytes == kRecordBytes && RecordGeo<128>::kVCodes == kOffVCodes &&
+              RecordGeo<128>::kKScales == kOffKScales && RecordGeo<128>::kVScales == kOffVScales, "layout");
 
 void set_error(const char* fmt, ...);
 int32_t check_config(const uq_config* cfg);  // UQ_OK / UQ_ERR_*; sets the error string
@@ -70,12 +86,15 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 EncodeTiledFn encode_tiled_fn();                                        // nullptr (error string set) if unavailable
-int32_t k_code_map(const void* cache, long long records, CUtensorMap* out);
-int32_t q_map(const void* q_fp8, long long rows, CUtensorMap* out);
+int32_t k_code_map(const void* cache, long long records, int head_dim, CUtensorMap* out);
+int32_t q_map(const void* q_fp8, long long rows, int head_dim, CUtensorMap* out);
 #endif
 
 inline float resolved_sm_scale(const uq_config* cfg) {
-  return cfg->sm_scale != 0.0f ? cfg->sm_scale : 0.08838834764831845f;  // 1/sqrt(128)
+  if (cfg->sm_scale != 0.0f) return cfg->sm_scale;
+  return cfg->head_dim == 64 ? 0.125f : cfg->head_dim == 256 ? 0.0625f : 0.08838834764831845f;  // 1/sqrt(head_dim)
 }
+// entry points whose kernels exist for head_dim 128 only
+int32_t require_head_dim_128(const uq_config* cfg, const char* who);
 
 }  // namespace uq

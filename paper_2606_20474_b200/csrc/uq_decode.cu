@@ -36,10 +36,8 @@
 namespace uq {
 namespace {
 
-constexpr int kComputeWarps = 8;                     // two per TMEM lane quarter: one softmax warp, one V warp
-constexpr int kSoftmaxWarps = 4;
+constexpr int kSoftmaxWarps = 4;                     // one per TMEM lane quarter
 constexpr int kIssuerWarps = 4;                      // QK issuer, PV issuer, K producer, V producer
-constexpr int kThreads = (kComputeWarps + kIssuerWarps) * 32;   // 12 warps: registers are allocated per 4 warps anyway
 #ifndef UQ_KSTAGES
 #define UQ_KSTAGES 3
 #endif
@@ -49,41 +47,69 @@ constexpr int kThreads = (kComputeWarps + kIssuerWarps) * 32;   // 12 warps: reg
 #ifndef UQ_CTAS_PER_SM
 #define UQ_CTAS_PER_SM 2
 #endif
-// Two rings: the K codes of a tile (16 KB once the TMA unit has expanded the nibbles) are needed by the QK
-// MMA only and leave early; the rest of the records (V codes, K scales, V scales: 9 KB) stays until the V
+#ifndef UQ_VBUFS
+#define UQ_VBUFS 2
+#endif
+// Two rings: the K codes of a tile (16 KB at head_dim 128 once the TMA unit has expanded the nibbles) are needed by
+// the QK MMA only and leave early; the rest of the records (V codes, K scales, V scales: 9 KB) stays until the V
 // warps have converted it.  Separate rings let the small one run deep (bytes in flight hide HBM latency).
 constexpr int kKStages = UQ_KSTAGES;
 constexpr int kVStages = UQ_VSTAGES;
 constexpr int kTilePages = 8;                        // 128 tokens per tile
-constexpr int kRestBytes = kRecordBytes - 1024;      // V codes + K scales + V scales = 1152
-constexpr int kKStageBytes = kTilePages * 2048;      // K codes, one byte per code: 16384
-constexpr int kVStageBytes = kTilePages * kRestBytes;   // 9216
 constexpr int kPBytes = 4096;                        // one P operand buffer: [token-core 16][head-core 2][8 tok][8 heads] f16
 constexpr float kThresh = 12.0f;                     // lazy-reference threshold (log2 units)
 constexpr int kMaxBatch = 2048;                      // sequences per call (tile prefix sums live in shared memory)
+constexpr int kVBufs = UQ_VBUFS;                     // Vhat^T buffers in TMEM
 
-// dynamic shared memory map (offsets from a 1024-byte aligned base)
-constexpr int kOffK = 0;                                       // kKStages x 16384, SW128
-constexpr int kOffV = kOffK + kKStages * kKStageBytes;         // kVStages x 9216
-constexpr int kOffQ = kOffV + kVStages * kVStageBytes;         // 2 x 2048, SW128 (one per unit in flight)
-constexpr int kOffSFA = kOffQ + 4096;                          // 2 x 512
-constexpr int kOffSFB = kOffSFA + 1024;                        // 512
-constexpr int kOffP = kOffSFB + 512;                           // 2 x 4096 (double-buffered)
-constexpr int kOffMul = kOffP + 2 * kPBytes;                   // 4 V warps x 256 B of fp16 multipliers
-constexpr int kOffEnd = kOffMul + kComputeWarps * 128;
-constexpr int kSmemBytes = kOffEnd + 1024;                     // + alignment slack
-
-// TMEM columns
-constexpr uint32_t kColS = 0;      // 2 x 16
-constexpr uint32_t kColO = 32;     // 16
-constexpr uint32_t kColSFA = 48;   // 2 x 4
-constexpr uint32_t kColSFB = 56;   // 4
-#ifndef UQ_VBUFS
-#define UQ_VBUFS 2
-#endif
-constexpr int kVBufs = UQ_VBUFS;   // Vhat^T buffers in TMEM
-constexpr uint32_t kColV = 64;     // kVBufs x 64: Vhat^T operand, lane = channel d, column c = tokens 2c, 2c+1 (f16x2)
-constexpr uint32_t kTmemCols = kVBufs == 1 ? 128 : 256;
+// Everything that depends on head_dim D (include/uq.h: 64, 128 or 256).  D = 128 is the geometry the kernel was tuned
+// on (one M = 128 PV product, 12 warps, 2 CTAs per SM); D = 64 runs the same CTA with the upper 64 accumulator rows
+// fed zeros (two V warps idle; the tensor pipe has the room), D = 256 splits the head into two 128-channel halves:
+// two K blocks per stage, two PV products per tile into two accumulators, eight V warps, one CTA of 16 warps per SM.
+template <int D>
+struct DecodeGeo {
+  using R = RecordGeo<D>;
+  static constexpr int kHalves = D == 256 ? 2 : 1;                  // 128-channel halves of the head
+  static constexpr int kVWarps = 4 * kHalves;                       // one per (half, TMEM lane quarter)
+  static constexpr int kComputeWarps = kSoftmaxWarps + kVWarps;
+  static constexpr int kThreads = (kComputeWarps + kIssuerWarps) * 32;   // 12 warps: registers are allocated per 4 warps anyway
+  static constexpr int kCtasPerSm = D == 256 ? 1 : UQ_CTAS_PER_SM;
+  static constexpr int kRecordBytes = R::kBytes;
+  static constexpr int kKPacked = 8 * D;                            // K codes of a page in HBM (1024 at D = 128)
+  static constexpr int kRestBytes = R::kRest;                       // V codes + K scales + V scales = 1152
+  static constexpr int kKRow = D < 128 ? D : 128;                   // bytes of a token row of a K block in smem (one per code)
+  static constexpr int kKPageBytes = 16 * kKRow;                    // a page inside a block: 2048
+  static constexpr int kKBlockBytes = kTilePages * kKPageBytes;     // 128 tokens x <= 128 channels: 16384
+  static constexpr int kKStageBytes = kHalves * kKBlockBytes;
+  static constexpr int kVStageBytes = kTilePages * kRestBytes;      // 9216
+  static constexpr int kQBlockBytes = 16 * kKRow;                   // 16 heads x <= 128 channels: 2048
+  static constexpr int kQBytes = kHalves * kQBlockBytes;
+  static constexpr uint32_t kSwz = D == 64 ? 4u : 2u;               // UMMA layout type: SWIZZLE_64B / SWIZZLE_128B
+  static constexpr uint32_t kSBO = 8 * kKRow;                       // eight rows of a swizzle atom
+  static constexpr int kQKMmas = D / 32;                            // one block-scaled MMA per 32-channel scale group
+  static constexpr int kSfaAtoms = (kQKMmas + 3) / 4;               // 512-byte scale-factor atoms (4 groups each) per tile
+  static constexpr int kSfaBytes = 512 * kSfaAtoms;
+  // dynamic shared memory map (offsets from a 1024-byte aligned base)
+  static constexpr int kOffK = 0;                                   // kKStages x 16384, SW128
+  static constexpr int kOffV = kOffK + kKStages * kKStageBytes;     // kVStages x 9216
+  static constexpr int kOffQ = kOffV + kVStages * kVStageBytes;     // 2 x 2048, SW128 (one per unit in flight)
+  static constexpr int kOffSFA = kOffQ + 2 * kQBytes;               // 2 x 512
+  static constexpr int kOffSFB = kOffSFA + 2 * kSfaBytes;           // 512
+  static constexpr int kOffP = kOffSFB + 512;                       // 2 x 4096 (double-buffered)
+  static constexpr int kOffMul = kOffP + 2 * kPBytes;               // V warps x 256 B of fp16 multipliers
+  static constexpr int kOffEnd = kOffMul + kVWarps * 256;
+  static constexpr int kSmemBytes = kOffEnd + 1024;                 // + alignment slack
+  static_assert(kOffQ % 1024 == 0 && kKStageBytes % 1024 == 0, "swizzled tiles need 1024-byte alignment");
+  // TMEM columns
+  static constexpr uint32_t kColS = 0;                              // 2 x 16
+  static constexpr uint32_t kColO = 32;                             // 16 per half
+  static constexpr uint32_t kColSFA = kColO + 16 * kHalves;         // 2 x 4 per atom
+  static constexpr uint32_t kSfaCols = 4 * kSfaAtoms;
+  static constexpr uint32_t kColSFB = kColSFA + 2 * kSfaCols;       // 4
+  static constexpr uint32_t kColV = D == 256 ? 128 : 64;            // kVBufs x 64 per half: Vhat^T operand, lane = channel d,
+  static constexpr uint32_t kVBufCols = 64 * kHalves;               //   column c = tokens 2c, 2c+1 (f16x2)
+  static constexpr uint32_t kTmemCols = D == 256 ? 512 : (kVBufs == 1 ? 128 : 256);
+  static_assert(kColSFB + 4 <= kColV && kColV + kVBufs * kVBufCols <= kTmemCols, "TMEM columns");
+};
 
 // ---------------------------------------------------------------- per-CTA shared bookkeeping
 struct Shared {
@@ -189,12 +215,22 @@ struct Sched {
 };
 
 // ---------------------------------------------------------------- the kernel
-__global__ void __launch_bounds__(kThreads, UQ_CTAS_PER_SM)
+template <int D>
+__global__ void __launch_bounds__(DecodeGeo<D>::kThreads, DecodeGeo<D>::kCtasPerSm)
 decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_q,
               const uint8_t* __restrict__ cache, const int32_t* __restrict__ block_tables, int max_pages,
               const int32_t* __restrict__ seq_lens, int batch, int Hq, int Hkv, int num_splits,
               float score_scale /* sm_scale * log2(e) */, float* __restrict__ partial_acc,
               float* __restrict__ partial_ml) {
+  using Geo = DecodeGeo<D>;
+  constexpr int kHalves = Geo::kHalves, kComputeWarps = Geo::kComputeWarps, kThreads = Geo::kThreads;
+  constexpr int kRecordBytes = Geo::kRecordBytes, kRestBytes = Geo::kRestBytes, kKStageBytes = Geo::kKStageBytes,
+                kVStageBytes = Geo::kVStageBytes, kKBlockBytes = Geo::kKBlockBytes, kKPageBytes = Geo::kKPageBytes,
+                kQBytes = Geo::kQBytes, kQBlockBytes = Geo::kQBlockBytes, kSfaBytes = Geo::kSfaBytes;
+  constexpr int kOffK = Geo::kOffK, kOffV = Geo::kOffV, kOffQ = Geo::kOffQ, kOffSFA = Geo::kOffSFA, kOffSFB = Geo::kOffSFB,
+                kOffP = Geo::kOffP, kOffMul = Geo::kOffMul;
+  constexpr uint32_t kColS = Geo::kColS, kColO = Geo::kColO, kColSFA = Geo::kColSFA, kColSFB = Geo::kColSFB,
+                     kColV = Geo::kColV, kVBufCols = Geo::kVBufCols, kSfaCols = Geo::kSfaCols, kTmemCols = Geo::kTmemCols;
   extern __shared__ uint8_t smem_raw[];
   __shared__ __align__(8) Shared sh;
 
@@ -303,8 +339,10 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     if (elect_one()) umma_cp_sf(tmem + kColSFB, make_desc(sSFB, 16, 128, 0));
     auto load_q = [&](const Unit& un, int k) {         // lane 0: Q tile of unit ordinal k
       if (elect_one()) {
-        mbar_expect_tx(bar_qfull + 8 * (k & 1), 2048);
-        tma_load_2d(sQ + 2048 * (k & 1), &tmap_q, 0, un.b * Hq + un.kvh * G, bar_qfull + 8 * (k & 1));
+        mbar_expect_tx(bar_qfull + 8 * (k & 1), kQBytes);
+        tma_load_2d(sQ + kQBytes * (k & 1), &tmap_q, 0, un.b * Hq + un.kvh * G, bar_qfull + 8 * (k & 1));
+        if constexpr (kHalves == 2)                      // channels 128..255: a second 128-byte-wide block
+          tma_load_2d(sQ + kQBytes * (k & 1) + kQBlockBytes, &tmap_q, 128, un.b * Hq + un.kvh * G, bar_qfull + 8 * (k & 1));
       }
     };
     Cursor cur, cur_nx;
@@ -327,26 +365,35 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
         if (i == 0) mbar_wait(bar_qfull + 8 * (k & 1), (k >> 1) & 1);
         mbar_wait(bar_fullv + 8 * sv, phv);
         const uint32_t st = base + kOffK + sk * kKStageBytes, rest = base + kOffV + sv * kVStageBytes;
-        // scale-factor atom: row r = 32 c + lane of the tile -> 16-byte line `lane`, word c
-        uint32_t v[4];
+        // scale-factor atom: row r = 32 c + lane of the tile -> 16-byte line `lane`, word c (a word = the row's scale
+        // bytes of four groups; head_dim 64 fills two of them, head_dim 256 a second atom with groups 4..7)
+        uint32_t v[4], v2[4];
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
           const int r = 32 * c + lane;
-          asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v[c]) : "r"(rest + kRestBytes * (r >> 4) + 1024 + 4 * (r & 15)));
+          const uint32_t a = rest + kRestBytes * (r >> 4) + 8 * D + (D / 32) * (r & 15);
+          if constexpr (D == 64) asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v[c]) : "r"(a));
+          else if constexpr (D == 128) asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v[c]) : "r"(a));
+          else asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v[c]), "=r"(v2[c]) : "r"(a));
         }
-        sts128(sSFA + 512 * sb + 16 * lane, make_uint4(v[0], v[1], v[2], v[3]));
+        sts128(sSFA + kSfaBytes * sb + 16 * lane, make_uint4(v[0], v[1], v[2], v[3]));
+        if constexpr (D == 256) sts128(sSFA + kSfaBytes * sb + 512 + 16 * lane, make_uint4(v2[0], v2[1], v2[2], v2[3]));
         fence_async_smem();
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_emptyv + 8 * sv);   // the K scales are copied: this warp is done with the V stage
         mbar_wait(bar_fullk + 8 * sk, phk);
         tc_fence_after();
         if (elect_one()) {
-          const uint32_t t_sfa = tmem + kColSFA + 4 * sb, qb = sQ + 2048 * (k & 1);
-          umma_cp_sf(t_sfa, make_desc(sSFA + 512 * sb, 16, 128, 0));
+          const uint32_t t_sfa = tmem + kColSFA + kSfaCols * sb, qb = sQ + kQBytes * (k & 1);
+          umma_cp_sf(t_sfa, make_desc(sSFA + kSfaBytes * sb, 16, 128, 0));
+          if constexpr (D == 256) umma_cp_sf(t_sfa + 4, make_desc(sSFA + kSfaBytes * sb + 512, 16, 128, 0));
 #pragma unroll
-          for (int kb = 0; kb < 4; ++kb)
-            umma_mxf8f6f4(tmem + kColS + 16 * sb, make_desc(st + 32 * kb, 16, 1024, 2), make_desc(qb + 32 * kb, 16, 1024, 2),
-                          idesc_qk | ((uint32_t)kb << 29), kb > 0, t_sfa + ((uint32_t)kb << 30), tmem + kColSFB);
+          for (int kb = 0; kb < Geo::kQKMmas; ++kb)       // one scale group (32 channels) per instruction
+            umma_mxf8f6f4(tmem + kColS + 16 * sb,
+                          make_desc(st + (kb >> 2) * kKBlockBytes + 32 * (kb & 3), 16, Geo::kSBO, Geo::kSwz),
+                          make_desc(qb + (kb >> 2) * kQBlockBytes + 32 * (kb & 3), 16, Geo::kSBO, Geo::kSwz),
+                          idesc_qk | ((uint32_t)(kb & 3) << 29), kb > 0,
+                          t_sfa + 4 * (kb >> 2) + ((uint32_t)(kb & 3) << 30), tmem + kColSFB);
           umma_commit(bar_sfull + 8 * sb);
           umma_commit(bar_emptyk + 8 * sk);
         }
@@ -370,11 +417,13 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
         mbar_wait(bar_ready + 8 * (gt & 1), (gt >> 1) & 1);
         tc_fence_after();
         if (lane == 0) {
-          const uint32_t pbuf = sP + kPBytes * (gt & 1), vbuf = tmem + kColV + 64 * ((gt & 1) % kVBufs);
+          const uint32_t pbuf = sP + kPBytes * (gt & 1), vbuf = tmem + kColV + kVBufCols * ((gt & 1) % kVBufs);
 #pragma unroll
-          for (int j = 0; j < 8; ++j)                    // 16 tokens per MMA = 8 columns of Vhat^T
-            umma_f16_ts(tmem + kColO, vbuf + 8 * j, make_desc(pbuf + 512 * j, 256, 128, 0), idesc_pv,
-                        (i > 0 || j > 0) ? 1u : 0u);
+          for (int c = 0; c < kHalves; ++c)              // 128 channels per accumulator
+#pragma unroll
+            for (int j = 0; j < 8; ++j)                  // 16 tokens per MMA = 8 columns of Vhat^T
+              umma_f16_ts(tmem + kColO + 16 * c, vbuf + 64 * c + 8 * j, make_desc(pbuf + 512 * j, 256, 128, 0), idesc_pv,
+                          (i > 0 || j > 0) ? 1u : 0u);
           umma_commit(bar_done + 8 * (gt & 1));
         }
         __syncwarp();
@@ -391,29 +440,33 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     const bool is_k = (role == 2);
     const int n_stages = is_k ? kKStages : kVStages;
     const uint32_t bar_e = is_k ? bar_emptyk : bar_emptyv, bar_f = is_k ? bar_fullk : bar_fullv;
-    const uint32_t page_tx = is_k ? 1024u : (uint32_t)kRestBytes;
+    const uint32_t page_tx = is_k ? (uint32_t)Geo::kKPacked : (uint32_t)kRestBytes;
+    const int pl = (kHalves == 2) ? (lane & 7) : lane;  // the lane's page of the tile; head_dim 256: lanes 8..15 of the
+    const int hl = (kHalves == 2) ? (lane >> 3) : 0;    // K producer copy the second 128-channel block of pages 0..7
+    const bool copier = (kHalves == 2 && is_k) ? lane < 2 * kTilePages : lane < kTilePages;
     const uint64_t pol = l2_evict_first_policy();
     Cursor cur;
     sc.start(cur);
     Unit un;
     int s = 0, ph = 1;                                 // stage, parity to wait for on empty[s]
     while (sc.next(cur, un)) {
-      const int32_t* bt = block_tables + (long long)un.b * max_pages + un.p0 + lane;
-      int page_next = (lane < kTilePages && un.p0 + lane < un.p1) ? bt[0] : 0;
+      const int32_t* bt = block_tables + (long long)un.b * max_pages + un.p0 + pl;
+      int page_next = (copier && un.p0 + pl < un.p1) ? bt[0] : 0;
       for (int i = 0; i < un.n_tiles; ++i) {
         const int page = page_next;
         const int npg = min(kTilePages, un.p1 - (un.p0 + kTilePages * i));
-        const int nb = un.p0 + kTilePages * (i + 1) + lane;
-        page_next = (lane < kTilePages && nb < un.p1) ? bt[kTilePages * (i + 1)] : 0;
+        const int nb = un.p0 + kTilePages * (i + 1) + pl;
+        page_next = (copier && nb < un.p1) ? bt[kTilePages * (i + 1)] : 0;
         mbar_wait(bar_e + 8 * s, ph);
         if (lane == 0) mbar_expect_tx(bar_f + 8 * s, (uint32_t)npg * page_tx);
         __syncwarp();
-        if (lane < npg) {
+        if ((kHalves == 2 && is_k) ? (copier && pl < npg) : (lane < npg)) {
           if (is_k)
-            tma_load_3d(base + kOffK + s * kKStageBytes + 2048 * lane, &tmap, 0, 0, page * Hkv + un.kvh, bar_f + 8 * s, pol);
+            tma_load_3d(base + kOffK + s * kKStageBytes + hl * kKBlockBytes + kKPageBytes * pl, &tmap, 128 * hl, 0,
+                        page * Hkv + un.kvh, bar_f + 8 * s, pol);
           else
             bulk_g2s(base + kOffV + s * kVStageBytes + kRestBytes * lane,
-                     cache + ((long long)page * Hkv + un.kvh) * kRecordBytes + 1024, kRestBytes, bar_f + 8 * s, pol);
+                     cache + ((long long)page * Hkv + un.kvh) * kRecordBytes + 8 * D, kRestBytes, bar_f + 8 * s, pol);
         }
         if (++s == n_stages) { s = 0; ph ^= 1; }
       }
@@ -538,12 +591,15 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
               if (i > 0) {  // every PV of this unit issued so far has to be in O before it is rescaled
                 mbar_wait(bar_done + 8 * (sb ^ 1), ((gt - 1) >> 1) & 1);
                 tc_fence_after();
-                float ov[NH];
-                const uint32_t t_o = tmem + lane_sel + kColO;      // channel r, heads 0..NH-1
-                tmem_ld<NH>(t_o, ov);
 #pragma unroll
-                for (int j = 0; j < NH; ++j) ov[j] *= f[j];
-                tmem_st<NH>(t_o, ov);
+                for (int c = 0; c < kHalves; ++c) {
+                  float ov[NH];
+                  const uint32_t t_o = tmem + lane_sel + kColO + 16 * c;   // channel 128 c + r, heads 0..NH-1
+                  tmem_ld<NH>(t_o, ov);
+#pragma unroll
+                  for (int j = 0; j < NH; ++j) ov[j] *= f[j];
+                  tmem_st<NH>(t_o, ov);
+                }
               }
               (void)softmax_pass();
               bar_softmax(1);                            // wmax may be rewritten only after every warp read it
@@ -602,9 +658,24 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
       // Warp of lane quarter q converts channel group g = q (channels 32 q .. 32 q + 31 = one UE8M0 scale
       // group of V): its reference exponent eref is its own, so the four V warps never have to agree on
       // anything.  Stored Vhat = code * 2^(byte - eref + 13) in fp16, written straight into TMEM.
-      const int g = q;
+      // head_dim 256: warps 4..7 of the compute warps take channels 0..127, warps 8..11 channels 128..255 (half hc,
+      // group 4 hc + q); head_dim 64: the warps of lane quarters 2 and 3 have no channels — they zero their rows of
+      // both Vhat^T buffers once (the PV product runs M = 128 with those accumulator rows unused) and only keep the
+      // barrier counts.
+      const int hc = (kHalves == 2) ? ((cw - kSoftmaxWarps) >> 2) : 0;   // 128-channel half
+      const int g = 4 * hc + q;
+      const bool active = (D >= 128) ? true : (q < 2);
       const uint32_t scratch = base + kOffMul + 256 * (cw - kSoftmaxWarps);
-      const uint32_t t_o = tmem + lane_sel + kColO;    // channel r, heads 0..15
+      const uint32_t t_o = tmem + lane_sel + kColO + 16 * hc;    // channel 128 hc + r, heads 0..15
+      if constexpr (D == 64) {
+        if (!active) {
+          const uint32_t z[16] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+#pragma unroll
+          for (int c16 = 0; c16 < (int)(kVBufs * kVBufCols) / 16; ++c16) tmem_st16_nowait(tmem + lane_sel + kColV + 16 * c16, z);
+          tmem_wait_st();
+          tc_fence_before();
+        }
+      }
       Cursor cur;
       sc.start(cur);
       Unit un;
@@ -617,11 +688,23 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
           const int sb = gt & 1;
           const uint32_t rest = base + kOffV + s * kVStageBytes;   // [V codes | K scales | V scales] of page 0
           mbar_wait(bar_fullv + 8 * s, ph_full);       // the tile's bytes have landed
+          if constexpr (D == 64) {
+            if (!active) {                             // no channels: nothing to convert, the barriers still count this warp
+              __syncwarp();
+              if (lane == 0) {
+                mbar_arrive(bar_ready + 8 * sb);
+                mbar_arrive(bar_emptyv + 8 * s);
+              }
+              ++gt;
+              if (++s == kVStages) { s = 0; ph_full ^= 1; }
+              continue;
+            }
+          }
 
           // ---- the tile's 128 scale bytes of group g: lane <-> tokens 4 lane .. 4 lane + 3
           uint32_t sw;
           asm volatile("ld.shared.u32 %0, [%1];" : "=r"(sw)
-                       : "r"(rest + kRestBytes * (lane >> 2) + 1088 + 32 * ((lane >> 1) & 1) + 8 * g + 4 * (lane & 1)));
+                       : "r"(rest + kRestBytes * (lane >> 2) + (8 * D + D / 2) + (D / 4) * ((lane >> 1) & 1) + 8 * g + 4 * (lane & 1)));
           if (rem < kTilePages * kPage) {              // bytes of tokens past the end (stale shared memory) -> 0
             const int nv = rem - 4 * lane;             // valid tokens among this lane's four
             sw = nv >= 4 ? sw : (nv <= 0 ? 0u : (sw & (0xFFFFFFFFu >> (8 * (4 - nv)))));
@@ -658,7 +741,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
             tc_fence_after();
           }
           // ---- V codes -> Vhat^T in TMEM buffer gt&1: lane = channel, column c = tokens 2c, 2c+1
-          const uint32_t t_v = tmem + lane_sel + kColV + 64 * sb;
+          const uint32_t t_v = tmem + lane_sel + kColV + kVBufCols * sb + 64 * hc;
           const uint32_t code0 = rest + 128 * g + 4 * lane;
 #pragma unroll
           for (int h = 0; h < 4; ++h) {                // 32 tokens (16 TMEM columns) at a time
@@ -667,7 +750,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
             for (int kk = 0; kk < 4; ++kk) {           // token octet k: page k>>1, half k&1
               const int k = 4 * h + kk;
               uint32_t cwd;
-              asm volatile("ld.shared.u32 %0, [%1];" : "=r"(cwd) : "r"(code0 + kRestBytes * (k >> 1) + 512 * (k & 1)));
+              asm volatile("ld.shared.u32 %0, [%1];" : "=r"(cwd) : "r"(code0 + kRestBytes * (k >> 1) + 4 * D * (k & 1)));
               const uint4 m4 = lds128(scratch + 16 * k);
               uint32_t f[4];
               cvt_e2m1x8(cwd, f);
@@ -692,13 +775,13 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
         // ============================================================== the unit's accumulator
         mbar_wait(bar_done + 8 * ((gt - 1) & 1), ((gt - 1) >> 1) & 1);
         tc_fence_after();
-        {
+        if (active) {
           float ov[16];
           tmem_ld<16>(t_o, ov);
           const float vscale = pow2i(eref - 13 - 127);  // stored Vhat = code * 2^(byte - eref + 13)
 #pragma unroll
           for (int j = 0; j < 16; ++j)
-            if (j < G) partial_acc[(un.row0 + (long long)j * num_splits) * kHeadDim + r] = ov[j] * vscale;
+            if (j < G) partial_acc[(un.row0 + (long long)j * num_splits) * D + 128 * hc + r] = ov[j] * vscale;
         }
         tc_fence_before();                              // the next unit's first PV overwrites O
       }
@@ -720,7 +803,7 @@ namespace {
 struct MapEntry {
   const void* cache;
   long long records;
-  int device;
+  int device, head_dim;
   CUtensorMap map;
 };
 std::mutex g_map_mu;
@@ -729,25 +812,28 @@ int g_map_n = 0, g_map_next = 0;
 
 }  // namespace
 
-// 3-D view of the cache for TMA: [record][16 tokens][128 x 4-bit]; box = one page of K codes.
-int32_t k_code_map(const void* cache, long long records, CUtensorMap* out) {
+// 3-D view of the cache for TMA: [record][16 tokens][head_dim x 4-bit]; box = one page of K codes, at most 128
+// channels wide (head_dim 256: two copies per page); 64-byte swizzle for head_dim 64 (a token row is 64 containers).
+int32_t k_code_map(const void* cache, long long records, int head_dim, CUtensorMap* out) {
   int dev = 0;
   (void)cudaGetDevice(&dev);                           // the same virtual address may be another allocation on another device
   const EncodeTiledFn encode = encode_tiled_fn();
   if (!encode) return UQ_ERR_CUDA;
   std::lock_guard<std::mutex> lock(g_map_mu);
   for (int i = 0; i < g_map_n; ++i)
-    if (g_maps[i].cache == cache && g_maps[i].records == records && g_maps[i].device == dev) {
+    if (g_maps[i].cache == cache && g_maps[i].records == records && g_maps[i].device == dev && g_maps[i].head_dim == head_dim) {
       *out = g_maps[i].map;
       return UQ_OK;
     }
-  const cuuint64_t gdim[3] = {128, 16, (cuuint64_t)records};
-  const cuuint64_t gstr[2] = {64, (cuuint64_t)kRecordBytes};
-  const cuuint32_t box[3] = {128, 16, 1};
+  const cuuint32_t wide = (cuuint32_t)(head_dim < 128 ? head_dim : 128);
+  const cuuint64_t gdim[3] = {(cuuint64_t)head_dim, 16, (cuuint64_t)records};
+  const cuuint64_t gstr[2] = {(cuuint64_t)head_dim / 2, (cuuint64_t)17 * head_dim};
+  const cuuint32_t box[3] = {wide, 16, 1};
   const cuuint32_t estr[3] = {1, 1, 1};
   CUtensorMap m;
   const CUresult cr = encode(&m, CU_TENSOR_MAP_DATA_TYPE_16U4_ALIGN16B, 3, const_cast<void*>(cache), gdim, gstr, box,
-                             estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                             estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                             head_dim == 64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_128B,
                              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (cr != CUDA_SUCCESS) {
     set_error("decode: cuTensorMapEncodeTiled failed with CUresult %d", (int)cr);
@@ -757,6 +843,7 @@ int32_t k_code_map(const void* cache, long long records, CUtensorMap* out) {
   e.cache = cache;
   e.records = records;
   e.device = dev;
+  e.head_dim = head_dim;
   e.map = m;
   g_map_next = (g_map_next + 1) % 8;
   if (g_map_n < 8) ++g_map_n;
@@ -764,23 +851,47 @@ int32_t k_code_map(const void* cache, long long records, CUtensorMap* out) {
   return UQ_OK;
 }
 
-// 2-D view of q_fp8 for TMA: [batch * Hq rows][128 bytes]; box = 16 rows (the heads of one kv head, padded).
-int32_t q_map(const void* q_fp8, long long rows, CUtensorMap* out) {
+// 2-D view of q_fp8 for TMA: [batch * Hq rows][head_dim bytes]; box = 16 rows (the heads of one kv head, padded) x at
+// most 128 bytes.
+int32_t q_map(const void* q_fp8, long long rows, int head_dim, CUtensorMap* out) {
   const EncodeTiledFn encode = encode_tiled_fn();
   if (!encode) return UQ_ERR_CUDA;
-  const cuuint64_t gdim[2] = {128, (cuuint64_t)rows};
-  const cuuint64_t gstr[1] = {128};
-  const cuuint32_t box[2] = {128, 16};
+  const cuuint32_t wide = (cuuint32_t)(head_dim < 128 ? head_dim : 128);
+  const cuuint64_t gdim[2] = {(cuuint64_t)head_dim, (cuuint64_t)rows};
+  const cuuint64_t gstr[1] = {(cuuint64_t)head_dim};
+  const cuuint32_t box[2] = {wide, 16};
   const cuuint32_t estr[2] = {1, 1};
   const CUresult cr = encode(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(q_fp8), gdim, gstr, box, estr,
-                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
-                             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                             CU_TENSOR_MAP_INTERLEAVE_NONE,
+                             head_dim == 64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_128B,
+                             CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (cr != CUDA_SUCCESS) {
     set_error("decode: cuTensorMapEncodeTiled (q_fp8) failed with CUresult %d", (int)cr);
     return UQ_ERR_CUDA;
   }
   return UQ_OK;
 }
+
+namespace {
+template <int D>
+int32_t launch_decode(const uq_config* cfg, const CUtensorMap& tmap, const CUtensorMap& tmap_q, const void* cache,
+                      const int32_t* block_tables, int32_t max_pages, const int32_t* seq_lens, int32_t batch,
+                      int32_t num_splits, float score_scale, float* partial_acc, float* partial_ml, int sm_count,
+                      cudaStream_t stream) {
+  using Geo = DecodeGeo<D>;
+  const long long slots = (long long)sm_count * Geo::kCtasPerSm;
+  const long long items = (long long)batch * cfg->num_kv_heads;
+  // num_splits == 1: a CTA per item (round-robin beyond the resident set); otherwise one balanced tile range per CTA
+  const dim3 grid((unsigned)((num_splits == 1 && items < slots) ? items : slots));
+  int32_t st = opt_in_dynamic_smem((const void*)decode_kernel<D>, Geo::kSmemBytes, "decode: cudaFuncSetAttribute");
+  if (st != UQ_OK) return st;
+  return check_cuda(launch_pdl(decode_kernel<D>, grid, dim3(Geo::kThreads), (size_t)Geo::kSmemBytes, stream, tmap, tmap_q,
+                               (const uint8_t*)cache, block_tables, (int)max_pages, seq_lens, (int)batch,
+                               (int)cfg->num_q_heads, (int)cfg->num_kv_heads, (int)num_splits, score_scale, partial_acc,
+                               partial_ml),
+                    "uq_decode_attention launch");
+}
+}  // namespace
 
 }  // namespace uq
 
@@ -813,10 +924,10 @@ extern "C" int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, 
     if (st != UQ_OK) return st;
   }
   CUtensorMap tmap;
-  st = k_code_map(cache, records, &tmap);
+  st = k_code_map(cache, records, cfg->head_dim, &tmap);
   if (st != UQ_OK) return st;
   CUtensorMap tmap_q;
-  st = q_map(q_fp8, (long long)batch * cfg->num_q_heads, &tmap_q);
+  st = q_map(q_fp8, (long long)batch * cfg->num_q_heads, cfg->head_dim, &tmap_q);
   if (st != UQ_OK) return st;
   const float score_scale = resolved_sm_scale(cfg) * 1.4426950408889634f;
   if (batch > kMaxBatch) {
@@ -826,15 +937,15 @@ extern "C" int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, 
   int sm_count = 0;
   st = current_device_sms(&sm_count);
   if (st != UQ_OK) return st;
-  const long long slots = (long long)sm_count * UQ_CTAS_PER_SM;
-  const long long items = (long long)batch * cfg->num_kv_heads;
-  // num_splits == 1: a CTA per item (round-robin beyond the resident set); otherwise one balanced tile range per CTA
-  const dim3 grid((unsigned)((num_splits == 1 && items < slots) ? items : slots));
-  st = opt_in_dynamic_smem((const void*)decode_kernel, kSmemBytes, "decode: cudaFuncSetAttribute");
-  if (st != UQ_OK) return st;
-  return check_cuda(launch_pdl(decode_kernel, grid, dim3(kThreads), (size_t)kSmemBytes, (cudaStream_t)stream, tmap, tmap_q,
-                               (const uint8_t*)cache, block_tables, (int)max_pages, seq_lens, (int)batch,
-                               (int)cfg->num_q_heads, (int)cfg->num_kv_heads, (int)num_splits, score_scale, partial_acc,
-                               partial_ml),
-                    "uq_decode_attention launch");
+  switch (cfg->head_dim) {
+    case 64:
+      return launch_decode<64>(cfg, tmap, tmap_q, cache, block_tables, max_pages, seq_lens, batch, num_splits, score_scale,
+                               partial_acc, partial_ml, sm_count, (cudaStream_t)stream);
+    case 256:
+      return launch_decode<256>(cfg, tmap, tmap_q, cache, block_tables, max_pages, seq_lens, batch, num_splits, score_scale,
+                                partial_acc, partial_ml, sm_count, (cudaStream_t)stream);
+    default:
+      return launch_decode<128>(cfg, tmap, tmap_q, cache, block_tables, max_pages, seq_lens, batch, num_splits, score_scale,
+                                partial_acc, partial_ml, sm_count, (cudaStream_t)stream);
+  }
 }

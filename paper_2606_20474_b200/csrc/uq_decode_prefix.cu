@@ -674,6 +674,8 @@ extern "C" int32_t uq_decode_prefix_attention(const uq_config* cfg, const void* 
   using namespace uq;
   int32_t st = check_config(cfg);
   if (st != UQ_OK) return st;
+  st = require_head_dim_128(cfg, "uq_decode_prefix_attention");
+  if (st != UQ_OK) return st;
   if (!q_fp8 || !cache || !block_tables || !partial_acc || !partial_ml || batch <= 0 || max_pages <= 0 ||
       num_pages <= 0) {
     set_error("decode_prefix: NULL pointer or non-positive size");
@@ -703,9 +705,9 @@ extern "C" int32_t uq_decode_prefix_attention(const uq_config* cfg, const void* 
     if (st != UQ_OK) return st;
   }
   CUtensorMap tmap, tmap_q;
-  st = k_code_map(cache, records, &tmap);
+  st = k_code_map(cache, records, 128, &tmap);
   if (st != UQ_OK) return st;
-  st = q_map(q_fp8, (long long)batch * cfg->num_q_heads, &tmap_q);
+  st = q_map(q_fp8, (long long)batch * cfg->num_q_heads, 128, &tmap_q);
   if (st != UQ_OK) return st;
   const float score_scale = resolved_sm_scale(cfg) * 1.4426950408889634f;
   int sm_count = 0;

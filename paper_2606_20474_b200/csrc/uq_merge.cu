@@ -130,6 +130,42 @@ merge2_kernel(const float* __restrict__ acc_a, const float* __restrict__ ml_a, i
   *reinterpret_cast<uint2*>(out + (long long)row * kHeadDim + 4 * lane) = packed;
 }
 
+// head_dim 64 / 256 (and a cross-check of the kernels above at 128): one warp per row, a lane takes channels
+// lane, lane + 32, ... (coalesced 128-byte reads); one or two sets of partials.
+__global__ void __launch_bounds__(128)
+merge_any_kernel(const float* __restrict__ acc_a, const float* __restrict__ ml_a, int Sa, const float* __restrict__ acc_b,
+                 const float* __restrict__ ml_b, int Sb, int rows, int D, __nv_bfloat16* __restrict__ out) {
+  pdl_launch_dependents();
+  pdl_wait();
+  const int lane = threadIdx.x & 31;
+  const int row = blockIdx.x * 4 + (threadIdx.x >> 5);
+  if (row >= rows) return;
+  const float2* mla = reinterpret_cast<const float2*>(ml_a) + (long long)row * Sa;
+  const float2* mlb = reinterpret_cast<const float2*>(ml_b) + (long long)row * Sb;
+  float M = -INFINITY;
+  for (int s = 0; s < Sa + Sb; ++s) {
+    const float2 v = s < Sa ? mla[s] : mlb[s - Sa];
+    if (v.y > 0.0f) M = fmaxf(M, v.x);
+  }
+  float num[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  float den = 0.f;
+  const int n = D >> 5;                                // channels per lane: 2, 4 or 8
+  for (int s = 0; s < Sa + Sb; ++s) {
+    const float2 v = s < Sa ? mla[s] : mlb[s - Sa];
+    if (!(v.y > 0.0f)) continue;                       // empty slot: its accumulator row is not read
+    const float* a = s < Sa ? acc_a + ((long long)row * Sa + s) * D : acc_b + ((long long)row * Sb + (s - Sa)) * D;
+    const float w = __expf(v.x - M);
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+      if (i < n) num[i] = fmaf(w, a[lane + 32 * i], num[i]);
+    den = fmaf(w, v.y, den);
+  }
+  const float inv = den > 0.f ? 1.0f / den : 0.f;
+#pragma unroll
+  for (int i = 0; i < 8; ++i)
+    if (i < n) out[(long long)row * D + lane + 32 * i] = __float2bfloat16_rn(num[i] * inv);
+}
+
 }  // namespace
 }  // namespace uq
 
@@ -147,6 +183,11 @@ extern "C" int32_t uq_merge_splits(const uq_config* cfg, const float* partial_ac
     return UQ_ERR_INVALID_ARG;
   }
   const int rows = batch * cfg->num_q_heads;
+  if (cfg->head_dim != kHeadDim)
+    return check_cuda(launch_pdl(merge_any_kernel, dim3((rows + 3) / 4), dim3(128), 0, (cudaStream_t)stream, partial_acc,
+                                 partial_ml, (int)num_splits, partial_acc, partial_ml, 0, rows, (int)cfg->head_dim,
+                                 (__nv_bfloat16*)out_bf16),
+                      "uq_merge_splits (head_dim 64/256) launch");
   return check_cuda(launch_pdl(merge_kernel, dim3((rows + 3) / 4), dim3(128), 0, (cudaStream_t)stream, partial_acc,
                                partial_ml, rows, (int)num_splits, (__nv_bfloat16*)out_bf16),
                     "uq_merge_splits launch");
@@ -167,6 +208,11 @@ extern "C" int32_t uq_merge_splits2(const uq_config* cfg, const float* acc_a, co
     return UQ_ERR_INVALID_ARG;
   }
   const int rows = batch * cfg->num_q_heads;
+  if (cfg->head_dim != kHeadDim)
+    return check_cuda(launch_pdl(merge_any_kernel, dim3((rows + 3) / 4), dim3(128), 0, (cudaStream_t)stream, acc_a, ml_a,
+                                 (int)splits_a, acc_b, ml_b, (int)splits_b, rows, (int)cfg->head_dim,
+                                 (__nv_bfloat16*)out_bf16),
+                      "uq_merge_splits2 (head_dim 64/256) launch");
   return check_cuda(launch_pdl(merge2_kernel, dim3((rows + 3) / 4), dim3(128), 0, (cudaStream_t)stream, acc_a, ml_a,
                                (int)splits_a, acc_b, ml_b, (int)splits_b, rows, (__nv_bfloat16*)out_bf16),
                     "uq_merge_splits2 launch");

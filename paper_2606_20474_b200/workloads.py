@@ -174,12 +174,14 @@ def _tables(rng, ctx_lens, prefix_len, page, extra_tokens, permute=True):
     return bt, max(num_pages, 1)
 
 
-def make_config(idx: int, scale: float = 1.0, peaked_frac: float | None = None) -> Workload:
+def make_config(idx: int, scale: float = 1.0, peaked_frac: float | None = None, head_dim: int = 128) -> Workload:
     """BASELINE.json config `idx` (1-5).  scale < 1 shrinks batch and context for CPU-sized
-    parity cases while keeping the structure (ragged lengths, shared prefix, outliers)."""
+    parity cases while keeping the structure (ragged lengths, shared prefix, outliers).
+    head_dim other than 128 (64, 256: the other head sizes the paper validates) keeps
+    everything else of the config."""
     seed = idx - 1
     rng = np.random.default_rng(seed)
-    d, page = 128, PAGE
+    d, page = int(head_dim), PAGE
 
     def sc(n, lo=1):
         return max(lo, int(round(n * scale)))
@@ -232,6 +234,8 @@ def make_config(idx: int, scale: float = 1.0, peaked_frac: float | None = None) 
     del ones
     if scale != 1.0:
         name += f"_x{scale:g}"
+    if d != 128:
+        name += f"_d{d}"
     return Workload(name=name, seed=seed, batch=B, num_q_heads=Hq, num_kv_heads=Hkv, head_dim=d,
                     page_size=page, ctx_lens=ctx, new_tokens=new, prefix_len=prefix,
                     block_tables=bt, num_pages=npg, k_chan_scale=ks, v_chan_scale=vs,
@@ -241,10 +245,10 @@ def make_config(idx: int, scale: float = 1.0, peaked_frac: float | None = None) 
 def make_custom(name: str, seed: int, ctx_lens, num_q_heads: int, num_kv_heads: int,
                 prefix_len: int = 0, new_tokens: int = 0, outlier_channels: int = 0,
                 outlier_gain: float = 1.0, peaked_frac: float = 0.0, permute: bool = True,
-                extra_tokens: int = 0) -> Workload:
+                extra_tokens: int = 0, head_dim: int = 128) -> Workload:
     """Free-form workload for edge cases (empty / ragged sequences, odd lengths)."""
     rng = np.random.default_rng(seed)
-    d, page = 128, PAGE
+    d, page = int(head_dim), PAGE
     ctx = np.asarray(ctx_lens, np.int32)
     ks = np.ones((num_kv_heads, d), np.float32)
     if outlier_channels:

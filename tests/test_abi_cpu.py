@@ -35,6 +35,11 @@ def test_record_bytes_is_4_25_bits_per_element(lib):
     assert 2176 * 8 / (16 * 128 * 2) == 4.25
     count = uq_layout.used_byte_mask()
     assert np.all(count[:1024] == 1) and np.all(count[1024:2048] == 2) and np.all(count[2048:] == 1)
+    for d in (64, 256):                                    # the other supported head sizes: 17 d bytes, no padding
+        assert uq.cache_record_bytes(uq.UQConfig(64, 4, head_dim=d)) == uq.record_bytes(d) == 17 * d
+        assert 17 * d * 8 / (16 * d * 2) == 4.25
+        count = uq_layout.used_byte_mask(d)
+        assert np.all(count[:8 * d] == 1) and np.all(count[8 * d:16 * d] == 2) and np.all(count[16 * d:] == 1)
 
 
 def test_host_side_validation(lib):
@@ -44,7 +49,7 @@ def test_host_side_validation(lib):
     assert b"NULL" in lib.uq_last_error_string()
     bad = uq.UQConfig(64, 5).c()
     assert f(ctypes.byref(bad), None, None, 1, 1, None, None) == 1
-    bad = uq.UQConfig(64, 4, head_dim=64).c()
+    bad = uq.UQConfig(64, 4, head_dim=96).c()
     assert f(ctypes.byref(bad), None, None, 1, 1, None, None) == 2   # UQ_ERR_UNSUPPORTED
     bad = uq.UQConfig(64, 2).c()                           # GQA group 32
     assert f(ctypes.byref(bad), None, None, 1, 1, None, None) == 2
@@ -69,6 +74,10 @@ def test_prefix_decode_and_calibrate_validate_on_the_host(lib):
     assert g(ctypes.byref(c), fake, 8, 1, fake, 4, 1, fake, fake, fake, None) == 1           # power-of-two scale + levels
     assert lib.uq_merge_splits2(ctypes.byref(c), None, None, 2, None, None, 2, 1, None, None) == 1
     assert uq.suggest_num_splits_max(uq.UQConfig(64, 4), 256, 16500, 98000) > uq.suggest_num_splits(uq.UQConfig(64, 4), 256, 16500)
+    for d in (64, 256):                                     # the shared-prefix decode and the calibration exist for head_dim 128
+        cd = uq.UQConfig(64, 4, head_dim=d).c()
+        assert f(ctypes.byref(cd), fake, fake, 64, fake, 64, 4, 128, 2, fake, fake, None) == 2
+        assert g(ctypes.byref(cd), fake, 8, 1, fake, 4, 1, None, fake, fake, None) == 2
 
 
 def test_workspace_query_and_debug_flag_on_the_host(lib):

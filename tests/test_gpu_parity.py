@@ -47,11 +47,12 @@ def test_cfg1_tiny_whole_cache_bit_exact_and_decode():
     _full_check(wl, [1, 4, 7])
 
 
+@pytest.mark.parametrize("d", [64, 128, 256])
 @pytest.mark.parametrize("hq,hkv", [(8, 8), (12, 2), (16, 2), (32, 2), (5, 1)])
-def test_ragged_batch_all_gqa_groups(hq, hkv):
-    # empty, 1-token, ragged tails, several pages; GQA groups 1, 6, 8, 16, 5
+def test_ragged_batch_all_gqa_groups(hq, hkv, d):
+    # empty, 1-token, ragged tails, several pages; GQA groups 1, 6, 8, 16, 5; head_dim 64 / 128 / 256
     wl = W.make_custom("ragged", 11, [0, 1, 17, 203, 1000, 16, 31, 32], hq, hkv,
-                       outlier_channels=3, outlier_gain=8.0, peaked_frac=0.3)
+                       outlier_channels=3, outlier_gain=8.0, peaked_frac=0.3, head_dim=d)
     _full_check(wl, [1, 3, 64])
 
 
@@ -128,9 +129,10 @@ def test_shared_prefix_steps_cfg4_scaled():
             H.check_out(out[b], ref, f"cfg4 step {step} seq {b}")
 
 
-@pytest.mark.parametrize("idx,scale", [(2, 1 / 16), (3, 1 / 16), (5, 1 / 32)])
-def test_scaled_configs(idx, scale):
-    wl = W.make_config(idx, scale=scale, peaked_frac=0.05)
+@pytest.mark.parametrize("idx,scale,d", [(2, 1 / 16, 128), (3, 1 / 16, 128), (5, 1 / 32, 128), (3, 1 / 16, 64), (3, 1 / 16, 256),
+                                         (2, 1 / 16, 256), (5, 1 / 64, 64)])
+def test_scaled_configs(idx, scale, d):
+    wl = W.make_config(idx, scale=scale, peaked_frac=0.05, head_dim=d)
     S = uq.suggest_num_splits(H.cfg_of(wl), wl.batch, int(wl.ctx_lens.mean()))
     _full_check(wl, sorted({1, S}), sample_seqs=list(range(min(wl.batch, 3))))
 
@@ -414,6 +416,40 @@ def test_step_graph_equals_direct_calls():
     assert torch.equal(cache_a, cache_b)
 
 
+@pytest.mark.parametrize("d", [64, 256])
+def test_append_on_rounding_boundaries_other_head_dims(d):
+    """The boundary rows of the test below (E2M1 ties, scale thresholds +- one bf16 step, constant / one-hot / huge /
+    tiny / zero rows) at head_dim 64 and 256 — the float64 kernel of those head sizes — bit for bit the oracle's image,
+    appended in one call and token by token; and the query bytes."""
+    L = 160
+    wl = W.make_custom("bound_d", 33 + d, [L], 8, 2, head_dim=d)
+    cfg = H.cfg_of(wl)
+    g = torch.Generator(device="cpu"); g.manual_seed(99 + d)
+    k, v = _boundary_rows(L, g, d)
+    k, v = k.to(torch.bfloat16).to(DEV), v.to(torch.bfloat16).to(DEV)
+    bt = torch.from_numpy(wl.block_tables).to(DEV)
+    ref = oracle.encode_kv(H.bits(k), H.bits(v))
+    cache = uq.alloc_cache(cfg, wl.num_pages, DEV); cache.fill_(0x5C)
+    H.append_tokens(cfg, cache, bt, np.zeros(1, np.int32), np.array([L], np.int32), k, v)
+    torch.cuda.synchronize()
+    H.compare_cache(cache, wl, 0, L, ref)
+    cache2 = uq.alloc_cache(cfg, wl.num_pages, DEV); cache2.fill_(0xC5)
+    pos = 0
+    for n in [1, 1, 3, 7, 1, 12, 30, 5, 100]:
+        n = min(n, L - pos)
+        H.append_tokens(cfg, cache2, bt, np.array([pos], np.int32), np.array([n], np.int32), k[pos:pos + n], v[pos:pos + n])
+        pos += n
+    torch.cuda.synchronize()
+    assert pos == L
+    H.compare_cache(cache2, wl, 0, L, ref)
+    q = torch.randn((1, 8, d), generator=g)
+    q[0, 0] = 0.75; q[0, 1] = 0; q[0, 1, 17] = -2.0; q[0, 2] *= 1e20; q[0, 3] *= 1e-20; q[0, 4] = 0
+    q[0, 5] = 448.0 / d ** 0.5
+    q = q.to(torch.bfloat16).to(DEV)
+    _, q_fp8, _ = H.run_decode(cfg, cache, bt, wl.ctx_lens, q, 1)
+    assert np.array_equal(q_fp8[0].cpu().numpy(), oracle.encode_q(H.bits(q)[0]))
+
+
 def test_append_on_rounding_boundaries_is_bit_exact():
     """The append kernel's float32 fast path must hand every close call to float64: V elements exactly on the
     E2M1 ties (0.25, 0.75, 1.25, 1.75, 2.5, 3.5, 5 times the group scale), group maxima on both sides of the
@@ -460,27 +496,27 @@ def test_append_on_rounding_boundaries_is_bit_exact():
     assert np.array_equal(q_fp8[0].cpu().numpy(), oracle.encode_q(H.bits(q)[0]))
 
 
-def _boundary_rows(L, g):
+def _boundary_rows(L, g, d=128):
     """K / V rows of test_append_on_rounding_boundaries_is_bit_exact (first 103 rows special, the rest N(0,1))."""
-    k = torch.randn((L, 2, 128), generator=g)
-    v = torch.randn((L, 2, 128), generator=g)
+    k = torch.randn((L, 2, d), generator=g)
+    v = torch.randn((L, 2, d), generator=g)
     ties = torch.tensor([0.25, 0.75, 1.25, 1.75, 2.5, 3.5, 5.0, 6.0, 0.5, 1.0, 1.5, 2.0, 3.0, 4.0, 0.0, -0.25])
     for t in range(0, 64):
         e = (t % 23) - 11
-        row = ties[torch.randint(0, 16, (2, 128), generator=g)] * (1.0 if t % 2 else -1.0)
+        row = ties[torch.randint(0, 16, (2, d), generator=g)] * (1.0 if t % 2 else -1.0)
         row[:, ::32] = 6.0
         v[t] = row * 2.0 ** e
     thr = [2.0 ** (kk - 0.5) / 0.15600000321865082 for kk in range(-6, 7)]
     for t in range(64, 96):
         x = torch.tensor(thr[t % len(thr)], dtype=torch.float32).to(torch.bfloat16)
         nb = (x.view(torch.int16) + (1 if t % 2 else -1)).view(torch.bfloat16)
-        row = torch.rand((2, 128), generator=g) * float(x) * 0.9
+        row = torch.rand((2, d), generator=g) * float(x) * 0.9
         row[:, ::32] = float(nb) if t % 3 else float(x)
         v[t] = row
     k[96] = 0.75
     k[97] = -3.0
     k[98] = 0; k[98, :, 5] = 2.0
-    k[99] = 0; k[99, :, 127] = -1.0 / 3.0
+    k[99] = 0; k[99, :, d - 1] = -1.0 / 3.0
     k[100] *= 1e20; k[101] *= 1e-20; v[100] *= 1e25; v[101] *= 1e-25
     k[102] = 0; v[102] = 0
     return k, v
