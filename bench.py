@@ -84,11 +84,14 @@ def _peaks():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s; MEASURED_PEAKS.json absent)"
 
 
+HEAD_DIM = 128                    # --head-dim: the config's shape at another head size (64 / 256)
+
+
 def _workload(idx: int, rank: int):
     import dataclasses
 
     from paper_2606_20474_b200 import workloads as W
-    wl = W.make_config(idx, peaked_frac=0.0)
+    wl = W.make_config(idx, peaked_frac=0.0, head_dim=HEAD_DIM)
     if rank:
         wl = dataclasses.replace(wl, seed=wl.seed + 1000 * rank)   # other values, same structure
     return wl
@@ -222,7 +225,7 @@ def run_ours(args, rank, world, local_rank):
     dev = torch.device("cuda", local_rank)
     torch.cuda.set_device(dev)
     wl = _workload(args.config, rank)
-    cfg = uq.UQConfig(num_q_heads=wl.num_q_heads, num_kv_heads=wl.num_kv_heads)
+    cfg = uq.UQConfig(num_q_heads=wl.num_q_heads, num_kv_heads=wl.num_kv_heads, head_dim=wl.head_dim)
     B, Hq, Hkv, d = wl.batch, wl.num_q_heads, wl.num_kv_heads, wl.head_dim
 
     # context AFTER the step's append = the config's lengths; the cache holds one token less
@@ -440,7 +443,8 @@ def run_ours(args, rank, world, local_rank):
         "roofline": {"bound": "hbm", "kernel": "uq::decode_kernel", "achieved": round(achieved, 1),
                      "peak": peak, "unit": "GB/s", "frac": round(achieved / peak, 4),
                      "frac_of_nominal_8TBs": round(achieved / NOMINAL_HBM_GBS, 4),
-                     "traffic": _ncu_traffic("decode_kernel", f"cfg{args.config}"), "algorithmic_bytes": decode_b,
+                     "traffic": _ncu_traffic("decode_kernel", f"cfg{args.config}" + (f"_d{d}" if d != 128 else "")),
+                     "algorithmic_bytes": decode_b,
                      "source_key": _source_key(),
                      "peak_source": peak_src,
                      "timing": "CUDA events around every uq_decode_attention launch, mean over a second pass of the same K steps "
@@ -703,12 +707,16 @@ def main():
                     help="instead of the decode step, time bulk quantize-on-append of TOKENS new tokens per call")
     ap.add_argument("--calibrate", type=int, default=0, metavar="VECTORS",
                     help="instead of the decode step, time uq_calibrate_c over VECTORS key vectors and 56 constants")
+    ap.add_argument("--head-dim", type=int, default=128, choices=[64, 128, 256],
+                    help="run the config's shape at another head size (the decode step only)")
     ap.add_argument("--sustain", type=float, default=2.0, metavar="SECONDS",
                     help="also time back-to-back steps for at least SECONDS (own clock record); 0 = skip")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--ref-budget", type=float, default=90.0, help="seconds for the whole --impl reference run")
     args = ap.parse_args()
 
+    global HEAD_DIM
+    HEAD_DIM = args.head_dim
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

@@ -83,8 +83,14 @@ struct DecodeGeo {
   static constexpr int kVStageBytes = kTilePages * kRestBytes;      // 9216
   static constexpr int kQBlockBytes = 16 * kKRow;                   // 16 heads x <= 128 channels: 2048
   static constexpr int kQBytes = kHalves * kQBlockBytes;
-  static constexpr uint32_t kSwz = D == 64 ? 4u : 2u;               // UMMA layout type: SWIZZLE_64B / SWIZZLE_128B
-  static constexpr uint32_t kSBO = 8 * kKRow;                       // eight rows of a swizzle atom
+  // head_dim 128 / 256: K-major tiles with the 128-byte swizzle, as the TMA unit writes them.  head_dim 64: the packed
+  // 4-bit tensor type of TMA takes 128-wide boxes only, so the packed codes arrive by plain bulk copies and an otherwise
+  // idle warp spreads them into the unswizzled core-matrix layout [16-byte chunk c][row r] (chunk = 16 codes, 8 bytes of
+  // nibbles + 8 of padding, as the tensor core reads 4-bit operands of kind::mxf8f6f4): LBO = the chunk stride.
+  static constexpr uint32_t kSwz = D == 64 ? 0u : 2u;               // UMMA layout type: none / SWIZZLE_128B
+  static constexpr uint32_t kSBO = D == 64 ? 128u : 1024u;          // eight rows
+  static constexpr uint32_t kLBOk = D == 64 ? 128u * 16u : 16u;     // K block: next chunk (ignored with a swizzle)
+  static constexpr uint32_t kLBOq = D == 64 ? 16u * 16u : 16u;      // Q block
   static constexpr int kQKMmas = D / 32;                            // one block-scaled MMA per 32-channel scale group
   static constexpr int kSfaAtoms = (kQKMmas + 3) / 4;               // 512-byte scale-factor atoms (4 groups each) per tile
   static constexpr int kSfaBytes = 512 * kSfaAtoms;
@@ -96,7 +102,9 @@ struct DecodeGeo {
   static constexpr int kOffSFB = kOffSFA + 2 * kSfaBytes;           // 512
   static constexpr int kOffP = kOffSFB + 512;                       // 2 x 4096 (double-buffered)
   static constexpr int kOffMul = kOffP + 2 * kPBytes;               // V warps x 256 B of fp16 multipliers
-  static constexpr int kOffEnd = kOffMul + kVWarps * 256;
+  static constexpr int kOffKP = kOffMul + kVWarps * 256;            // head_dim 64: kKStages x 4096 of packed K codes
+  static constexpr int kKPStage = D == 64 ? kTilePages * 8 * D : 0;
+  static constexpr int kOffEnd = kOffKP + kKStages * kKPStage;
   static constexpr int kSmemBytes = kOffEnd + 1024;                 // + alignment slack
   static_assert(kOffQ % 1024 == 0 && kKStageBytes % 1024 == 0, "swizzled tiles need 1024-byte alignment");
   // TMEM columns
@@ -129,6 +137,7 @@ struct Shared {
   float mref[16];
   int total_tiles, max_tiles;  // sum (x kv heads) and max over sequences of the tiles per (sequence, kv head)
   int pre[kMaxBatch + 1];      // pre[b] = tiles of sequences 0..b-1 (per kv head)
+  uint64_t full_kp[kKStages];  // head_dim 64 only: bulk-copy bytes of the PACKED K codes -> the expander warp
 };
 
 // ---------------------------------------------------------------- work schedule
@@ -260,6 +269,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     for (int s = 0; s < kKStages; ++s) {
       mbar_init(bar_fullk + 8 * s, 1);
       mbar_init(bar_emptyk + 8 * s, 1);
+      if constexpr (D == 64) mbar_init(smem_u32(&sh.full_kp[s]), 1);
     }
 #pragma unroll
     for (int s = 0; s < kVStages; ++s) {
@@ -340,7 +350,10 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     auto load_q = [&](const Unit& un, int k) {         // lane 0: Q tile of unit ordinal k
       if (elect_one()) {
         mbar_expect_tx(bar_qfull + 8 * (k & 1), kQBytes);
-        tma_load_2d(sQ + kQBytes * (k & 1), &tmap_q, 0, un.b * Hq + un.kvh * G, bar_qfull + 8 * (k & 1));
+        if constexpr (D == 64)                           // [chunk][row][16 B]: the unswizzled core-matrix order
+          tma_load_3d_plain(sQ + kQBytes * (k & 1), &tmap_q, 0, un.b * Hq + un.kvh * G, 0, bar_qfull + 8 * (k & 1));
+        else
+          tma_load_2d(sQ + kQBytes * (k & 1), &tmap_q, 0, un.b * Hq + un.kvh * G, bar_qfull + 8 * (k & 1));
         if constexpr (kHalves == 2)                      // channels 128..255: a second 128-byte-wide block
           tma_load_2d(sQ + kQBytes * (k & 1) + kQBlockBytes, &tmap_q, 128, un.b * Hq + un.kvh * G, bar_qfull + 8 * (k & 1));
       }
@@ -390,8 +403,10 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
 #pragma unroll
           for (int kb = 0; kb < Geo::kQKMmas; ++kb)       // one scale group (32 channels) per instruction
             umma_mxf8f6f4(tmem + kColS + 16 * sb,
-                          make_desc(st + (kb >> 2) * kKBlockBytes + 32 * (kb & 3), 16, Geo::kSBO, Geo::kSwz),
-                          make_desc(qb + (kb >> 2) * kQBlockBytes + 32 * (kb & 3), 16, Geo::kSBO, Geo::kSwz),
+                          make_desc(st + (kb >> 2) * kKBlockBytes + (D == 64 ? 2 * Geo::kLBOk : 32u) * (kb & 3), Geo::kLBOk,
+                                    Geo::kSBO, Geo::kSwz),
+                          make_desc(qb + (kb >> 2) * kQBlockBytes + (D == 64 ? 2 * Geo::kLBOq : 32u) * (kb & 3), Geo::kLBOq,
+                                    Geo::kSBO, Geo::kSwz),
                           idesc_qk | ((uint32_t)(kb & 3) << 29), kb > 0,
                           t_sfa + 4 * (kb >> 2) + ((uint32_t)(kb & 3) << 30), tmem + kColSFB);
           umma_commit(bar_sfull + 8 * sb);
@@ -439,7 +454,8 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     // 119.7 us on config 2, than one copy per lane — see elect_one().)
     const bool is_k = (role == 2);
     const int n_stages = is_k ? kKStages : kVStages;
-    const uint32_t bar_e = is_k ? bar_emptyk : bar_emptyv, bar_f = is_k ? bar_fullk : bar_fullv;
+    const uint32_t bar_e = is_k ? bar_emptyk : bar_emptyv,
+                   bar_f = is_k ? (D == 64 ? smem_u32(&sh.full_kp[0]) : bar_fullk) : bar_fullv;
     const uint32_t page_tx = is_k ? (uint32_t)Geo::kKPacked : (uint32_t)kRestBytes;
     const int pl = (kHalves == 2) ? (lane & 7) : lane;  // the lane's page of the tile; head_dim 256: lanes 8..15 of the
     const int hl = (kHalves == 2) ? (lane >> 3) : 0;    // K producer copy the second 128-channel block of pages 0..7
@@ -461,10 +477,14 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
         if (lane == 0) mbar_expect_tx(bar_f + 8 * s, (uint32_t)npg * page_tx);
         __syncwarp();
         if ((kHalves == 2 && is_k) ? (copier && pl < npg) : (lane < npg)) {
-          if (is_k)
-            tma_load_3d(base + kOffK + s * kKStageBytes + hl * kKBlockBytes + kKPageBytes * pl, &tmap, 128 * hl, 0,
-                        page * Hkv + un.kvh, bar_f + 8 * s, pol);
-          else
+          if (is_k) {
+            if constexpr (D == 64)
+              bulk_g2s(base + Geo::kOffKP + s * Geo::kKPStage + Geo::kKPacked * lane,
+                       cache + ((long long)page * Hkv + un.kvh) * kRecordBytes, Geo::kKPacked, bar_f + 8 * s, pol);
+            else
+              tma_load_3d(base + kOffK + s * kKStageBytes + hl * kKBlockBytes + kKPageBytes * pl, &tmap, 128 * hl, 0,
+                          page * Hkv + un.kvh, bar_f + 8 * s, pol);
+          } else
             bulk_g2s(base + kOffV + s * kVStageBytes + kRestBytes * lane,
                      cache + ((long long)page * Hkv + un.kvh) * kRecordBytes + 8 * D, kRestBytes, bar_f + 8 * s, pol);
         }
@@ -680,6 +700,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
       sc.start(cur);
       Unit un;
       int gt = 0, s = 0, ph_full = 0;                  // global tile counter, its V stage and full-barrier parity
+      [[maybe_unused]] int xk = 0, xph = 0;            // head_dim 64, expander warp: K stage and packed-full parity
       while (sc.next(cur, un)) {
         int eref = 28;
         int rem = un.tok_end - un.p0 * kPage;          // valid tokens from the first token of the tile on
@@ -690,6 +711,27 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
           mbar_wait(bar_fullv + 8 * s, ph_full);       // the tile's bytes have landed
           if constexpr (D == 64) {
             if (!active) {                             // no channels: nothing to convert, the barriers still count this warp
+              if (q == 2) {
+                // the K expander: packed codes of the tile [128 tokens][32 B] -> [chunk c][row r][8 B codes + 8 B pad]
+                mbar_wait(smem_u32(&sh.full_kp[xk]), xph);
+                const uint32_t src = base + Geo::kOffKP + xk * Geo::kKPStage, dstk = base + kOffK + xk * kKStageBytes;
+#pragma unroll
+                for (int rr = 0; rr < 4; ++rr) {
+                  const int row = lane + 32 * rr;
+                  const uint4 lo = lds128(src + 32 * row), hi = lds128(src + 32 * row + 16);
+                  asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(dstk + 16 * row), "r"(lo.x), "r"(lo.y) : "memory");
+                  asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(dstk + 2048 + 16 * row), "r"(lo.z), "r"(lo.w) : "memory");
+                  asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(dstk + 4096 + 16 * row), "r"(hi.x), "r"(hi.y) : "memory");
+                  asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(dstk + 6144 + 16 * row), "r"(hi.z), "r"(hi.w) : "memory");
+                }
+                fence_async_smem();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_fullk + 8 * xk);
+                if (++xk == kKStages) { xk = 0; xph ^= 1; }
+              }
+              // arrive for tile gt only once the `ready` phase of tile gt-2 (same buffer) is over, as the converting
+              // warps do: an early arrival would be counted into that phase
+              if (gt >= 2) mbar_wait(bar_done + 8 * sb, ((gt >> 1) - 1) & 1);
               __syncwarp();
               if (lane == 0) {
                 mbar_arrive(bar_ready + 8 * sb);
@@ -812,8 +854,8 @@ int g_map_n = 0, g_map_next = 0;
 
 }  // namespace
 
-// 3-D view of the cache for TMA: [record][16 tokens][head_dim x 4-bit]; box = one page of K codes, at most 128
-// channels wide (head_dim 256: two copies per page); 64-byte swizzle for head_dim 64 (a token row is 64 containers).
+// 3-D view of the cache for TMA: [record][16 tokens][head_dim x 4-bit]; box = one page of K codes, 128 channels wide
+// (head_dim 256: two copies per page; head_dim 64 does not use it).
 int32_t k_code_map(const void* cache, long long records, int head_dim, CUtensorMap* out) {
   int dev = 0;
   (void)cudaGetDevice(&dev);                           // the same virtual address may be another allocation on another device
@@ -825,15 +867,13 @@ int32_t k_code_map(const void* cache, long long records, int head_dim, CUtensorM
       *out = g_maps[i].map;
       return UQ_OK;
     }
-  const cuuint32_t wide = (cuuint32_t)(head_dim < 128 ? head_dim : 128);
   const cuuint64_t gdim[3] = {(cuuint64_t)head_dim, 16, (cuuint64_t)records};
   const cuuint64_t gstr[2] = {(cuuint64_t)head_dim / 2, (cuuint64_t)17 * head_dim};
-  const cuuint32_t box[3] = {wide, 16, 1};
+  const cuuint32_t box[3] = {128, 16, 1};              // the packed 4-bit tensor type takes 128-wide boxes only
   const cuuint32_t estr[3] = {1, 1, 1};
   CUtensorMap m;
   const CUresult cr = encode(&m, CU_TENSOR_MAP_DATA_TYPE_16U4_ALIGN16B, 3, const_cast<void*>(cache), gdim, gstr, box,
-                             estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                             head_dim == 64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_128B,
+                             estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (cr != CUDA_SUCCESS) {
     set_error("decode: cuTensorMapEncodeTiled failed with CUresult %d", (int)cr);
@@ -851,20 +891,30 @@ int32_t k_code_map(const void* cache, long long records, int head_dim, CUtensorM
   return UQ_OK;
 }
 
-// 2-D view of q_fp8 for TMA: [batch * Hq rows][head_dim bytes]; box = 16 rows (the heads of one kv head, padded) x at
-// most 128 bytes.
+// View of q_fp8 for TMA: [batch * Hq rows][head_dim bytes]; box = 16 rows (the heads of one kv head, padded) x 128
+// bytes, 128-byte swizzle; head_dim 64: 3-D, see below.
 int32_t q_map(const void* q_fp8, long long rows, int head_dim, CUtensorMap* out) {
   const EncodeTiledFn encode = encode_tiled_fn();
   if (!encode) return UQ_ERR_CUDA;
-  const cuuint32_t wide = (cuuint32_t)(head_dim < 128 ? head_dim : 128);
-  const cuuint64_t gdim[2] = {(cuuint64_t)head_dim, (cuuint64_t)rows};
-  const cuuint64_t gstr[1] = {(cuuint64_t)head_dim};
-  const cuuint32_t box[2] = {wide, 16};
-  const cuuint32_t estr[2] = {1, 1};
-  const CUresult cr = encode(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(q_fp8), gdim, gstr, box, estr,
-                             CU_TENSOR_MAP_INTERLEAVE_NONE,
-                             head_dim == 64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_128B,
-                             CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  CUresult cr;
+  if (head_dim == 64) {
+    // [16-byte chunk][row][16 B]: the copy lands in the unswizzled core-matrix order the MMA descriptor names
+    const cuuint64_t gdim[3] = {16, (cuuint64_t)rows, 4};
+    const cuuint64_t gstr[2] = {64, 16};
+    const cuuint32_t box[3] = {16, 16, 4};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    cr = encode(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(q_fp8), gdim, gstr, box, estr,
+                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  } else {
+    const cuuint64_t gdim[2] = {(cuuint64_t)head_dim, (cuuint64_t)rows};
+    const cuuint64_t gstr[1] = {(cuuint64_t)head_dim};
+    const cuuint32_t box[2] = {128, 16};
+    const cuuint32_t estr[2] = {1, 1};
+    cr = encode(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(q_fp8), gdim, gstr, box, estr,
+                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  }
   if (cr != CUDA_SUCCESS) {
     set_error("decode: cuTensorMapEncodeTiled (q_fp8) failed with CUresult %d", (int)cr);
     return UQ_ERR_CUDA;
@@ -923,9 +973,11 @@ extern "C" int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, 
                             cfg->page_size, 0, (cudaStream_t)stream);
     if (st != UQ_OK) return st;
   }
-  CUtensorMap tmap;
-  st = k_code_map(cache, records, cfg->head_dim, &tmap);
-  if (st != UQ_OK) return st;
+  CUtensorMap tmap = {};                               // head_dim 64 copies the packed K codes without a tensor map
+  if (cfg->head_dim != 64) {
+    st = k_code_map(cache, records, cfg->head_dim, &tmap);
+    if (st != UQ_OK) return st;
+  }
   CUtensorMap tmap_q;
   st = q_map(q_fp8, (long long)batch * cfg->num_q_heads, cfg->head_dim, &tmap_q);
   if (st != UQ_OK) return st;

@@ -137,10 +137,11 @@ def test_scaled_configs(idx, scale, d):
     _full_check(wl, sorted({1, S}), sample_seqs=list(range(min(wl.batch, 3))))
 
 
-def test_merge_on_hand_made_partials():
+@pytest.mark.parametrize("d", [128, 64, 256])
+def test_merge_on_hand_made_partials(d):
     rng = np.random.default_rng(21)
-    B, Hq, S, d = 3, 8, 5, 128
-    cfg = uq.UQConfig(Hq, 2)
+    B, Hq, S = 3, 8, 5
+    cfg = uq.UQConfig(Hq, 2, head_dim=d)
     acc = rng.standard_normal((B, Hq, S, d)).astype(np.float32)
     m = (rng.standard_normal((B, Hq, S)) * 20).astype(np.float32)
     l = rng.uniform(0.5, 50, (B, Hq, S)).astype(np.float32)
@@ -583,12 +584,14 @@ def test_bulk_append_many_sequences_irregular_counts():
             H.compare_cache(cache, wl, b, L, H.oracle_sequence_cache(wl, b, L, DEV))
 
 
-def test_random_small_configs():
+@pytest.mark.parametrize("d", [128, 64, 256])
+def test_random_small_configs(d):
     """Seeded sweep over head geometries, batch sizes (up to more items than resident CTAs), length mixes (empty,
-    one token, tile multiples +-1, ragged) and slot counts 1..6: cache image bit-exact, outputs in tolerance."""
-    rng = np.random.default_rng(7)
+    one token, tile multiples +-1, ragged) and slot counts 1..6: cache image bit-exact, outputs in tolerance.
+    head_dim 128 (24 cases) and 64 / 256 (16 cases each, other seeds)."""
+    rng = np.random.default_rng(7 if d == 128 else 7000 + d)
     heads = [(8, 8), (8, 1), (16, 1), (12, 2), (32, 2), (6, 1), (10, 2), (64, 4), (48, 8)]
-    for case in range(24):
+    for case in range(24 if d == 128 else 16):
         hq, hkv = heads[rng.integers(len(heads))]
         kind = int(rng.integers(6))
         B = int(rng.integers(1, 7)) if kind < 4 else int(rng.integers(40, 130))
@@ -600,7 +603,7 @@ def test_random_small_configs():
         if lens.sum() == 0: lens[0] = 1
         S = int(rng.integers(1, 7))
         wl = W.make_custom(f"rnd{case}", 1000 + case, [int(x) for x in lens], hq, hkv,
-                           peaked_frac=float(rng.choice([0.0, 0.3])))
+                           peaked_frac=float(rng.choice([0.0, 0.3])), head_dim=d)
         cfg = H.cfg_of(wl)
         cache, bt = H.fill_cache(cfg, wl, DEV)
         q = W.gen_q(wl, DEV)
