@@ -75,6 +75,10 @@ def _load():
     lib.uqo_calib_sq_err.argtypes = [u16p, ctypes.c_int64, ctypes.c_int, ctypes.c_int,
                                      ctypes.POINTER(ctypes.c_float), ctypes.c_int, ctypes.c_int,
                                      ctypes.POINTER(ctypes.c_float), f64p, f64p]
+    lib.uqo_cast_e4m3.restype = None
+    lib.uqo_cast_e4m3.argtypes = [u16p, ctypes.c_int64, u8p]
+    lib.uqo_e4m3_to_double.restype = None
+    lib.uqo_e4m3_to_double.argtypes = [u8p, ctypes.c_int64, f64p]
     lib.uqo_num_threads.restype = ctypes.c_int
     lib.uqo_set_num_threads.argtypes = [ctypes.c_int]
     _lib = lib
@@ -257,3 +261,32 @@ def attention_dense(q, k, v, sm_scale: float | None = None) -> np.ndarray:
                                 _ptr(v, ctypes.c_double), L, Hq, Hkv, d, float(sm_scale),
                                 _ptr(out, ctypes.c_double))
     return out
+
+
+# ------------------------------------------------------------------ comparison caches (DESIGN reading G19)
+def cast_e4m3(x_bits) -> np.ndarray:
+    """bf16 bit patterns -> OCP E4M3 bytes of the values themselves (no rotation, scale 1): the FP8-KV cache entry."""
+    x_bits = _c(x_bits, np.uint16)
+    out = np.empty(x_bits.shape, np.uint8)
+    _load().uqo_cast_e4m3(_ptr(x_bits, ctypes.c_uint16), x_bits.size, _ptr(out, ctypes.c_uint8))
+    return out
+
+
+def e4m3_to_double(b) -> np.ndarray:
+    b = _c(b, np.uint8)
+    out = np.empty(b.shape, np.float64)
+    _load().uqo_e4m3_to_double(_ptr(b, ctypes.c_uint8), b.size, _ptr(out, ctypes.c_double))
+    return out
+
+
+def attention_fp8kv(q_bits, k_bits, v_bits, sm_scale: float | None = None):
+    """FP8-E4M3 KV attention for ONE sequence: q bf16 bits [Hq, d], k / v bf16 bits [L, Hkv, d]; every tensor is cast to
+    E4M3 (cast_e4m3), then plain float64 softmax attention over the decoded values.  Returns (out [Hq, d], q8, k8, v8)."""
+    q8, k8, v8 = cast_e4m3(q_bits), cast_e4m3(k_bits), cast_e4m3(v_bits)
+    out = attention_dense(e4m3_to_double(q8), e4m3_to_double(k8), e4m3_to_double(v8), sm_scale)
+    return out, q8, k8, v8
+
+
+def attention_bf16kv(q_bits, k_bits, v_bits, sm_scale: float | None = None) -> np.ndarray:
+    """BF16 KV attention for ONE sequence: float64 softmax attention over the exact values of the bf16 inputs."""
+    return attention_dense(bf16_to_double(q_bits), bf16_to_double(k_bits), bf16_to_double(v_bits), sm_scale)

@@ -25,7 +25,8 @@
  * uqo_encode_q element for element against hadamard + e4m3_encode and against the library
  * cast of an independently rotated query, on random / one-hot / saturating rows (P12);
  * uqo_attention_dense against float64 SDPA and the L = 1 / equal-keys / dominant-key closed
- * forms (P13).
+ * forms (P13); the FP8-KV casts uqo_cast_e4m3 / uqo_e4m3_to_double element for element against
+ * e4m3_encode / e4m3_decode (P8) and the library cast (P14).
  * Parity unpinned: the attention *output values* for concrete inputs (the paper
  * prints no worked example) — pinned only through the closed forms above.
  */
@@ -400,6 +401,22 @@ void uqo_attention_dense(const double* q /*[Hq][d]*/, const double* k /*[L][Hkv]
     }
     free(z);
   }
+}
+
+/* ---- Comparison systems of the paper's Section 7 (PAPER.md:163-171; Table 3, :293-301): "hardware FP8 KV" and the
+ * BF16 baseline, as CACHES for the same attention.  The paper names them and nothing more;
+ * DESIGN.md reading G19: FP8 KV = K and V stored as OCP E4M3 bytes of the bf16 values themselves (no rotation, scale 1
+ * — the engine default without calibrated scales), round to nearest even, saturating, +0 only, i.e. uqo_e4m3_encode
+ * per element; the query is cast the same way; BF16 KV = the bf16 values as they are.  Attention over either is
+ * uqo_attention_dense on the decoded doubles (uqo_e4m3_decode / uqo_bf16_to_double): the textbook definition. */
+void uqo_cast_e4m3(const uint16_t* x_bf16, int64_t n, uint8_t* out) {
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < n; ++i) out[i] = uqo_e4m3_encode(uqo_bf16_to_double(x_bf16[i]));
+}
+
+void uqo_e4m3_to_double(const uint8_t* b, int64_t n, double* out) {
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < n; ++i) out[i] = uqo_e4m3_decode(b[i]);
 }
 
 /* Number of OpenMP threads the loops above will use (reported as cpu_baseline.cores). */

@@ -551,3 +551,50 @@ def test_p13_attention_dense_against_sdpa_and_closed_forms():
     for h in range(Hq):
         assert np.allclose(od[h], v[17, h // G], atol=1e-13)
     assert np.array_equal(oracle.attention_dense(q, k[:0], v[:0]), np.zeros((Hq, d)))
+
+
+# ----------------------------------------------------------------------------- P14 comparison caches (FP8 KV / BF16 KV)
+def test_p14_fp8_kv_cast_and_attention_are_the_pinned_parts():
+    """The FP8-KV comparison cache ("hardware FP8 KV"; DESIGN reading G19): `cast_e4m3` == e4m3_encode of the
+    bf16 value element for element (P8 pins that scalar) == the library cast (torch float8_e4m3fn) below 448, saturating
+    above, no -0; `e4m3_to_double` == the closed form for all 256 bytes; `attention_fp8kv` == float64 SDPA over the
+    library-decoded tensors; `attention_bf16kv` == float64 SDPA over the bf16 values."""
+    rng = np.random.default_rng(14)
+    x = np.concatenate([rng.standard_normal(4000) * 3, rng.standard_normal(300) * 300, [0.0, -0.0, 448.0, -448.0, 464.0, 1e30,
+                        -1e30, 2.0 ** -9, 2.0 ** -10, -(2.0 ** -10), 1.5 * 2.0 ** -9, 2.0 ** -6, 0.0175]])
+    xb = torch.from_numpy(x.astype(np.float32)).to(torch.bfloat16)
+    bits = xb.view(torch.uint16).numpy()
+    got = oracle.cast_e4m3(bits)
+    want = np.array([oracle.e4m3_encode(float(v)) for v in oracle.bf16_to_double(bits)], np.uint8)
+    assert np.array_equal(got, want)
+    xv = xb.double().numpy()
+    ok = np.abs(xv) < 448.0
+    lib = xb.to(torch.float8_e4m3fn).view(torch.uint8).numpy()
+    lib = np.where((lib & 0x7F) == 0, 0, lib)
+    assert np.array_equal(got[ok], lib[ok])
+    assert np.all((got[~ok] & 0x7F) == 0x7E) and (~ok).sum() > 20
+    assert not np.any(got == 0x80)
+    allb = np.arange(256, dtype=np.uint8)
+    dec = oracle.e4m3_to_double(allb)
+    ef, mf = (allb >> 3) & 0xF, allb & 7
+    closed = np.where(ef == 0, mf * 2.0 ** -9, (1 + mf / 8.0) * 2.0 ** (ef.astype(np.float64) - 7)) * np.where(allb & 0x80, -1.0, 1.0)
+    assert np.array_equal(dec, closed)
+    # attention over the two comparison caches
+    Hq, Hkv, d, L = 8, 2, 128, 77
+    G = Hq // Hkv
+    q = torch.from_numpy(rng.standard_normal((Hq, d)).astype(np.float32)).to(torch.bfloat16)
+    k = torch.from_numpy(rng.standard_normal((L, Hkv, d)).astype(np.float32) * 2).to(torch.bfloat16)
+    v = torch.from_numpy(rng.standard_normal((L, Hkv, d)).astype(np.float32)).to(torch.bfloat16)
+    qb, kb, vb = (t.view(torch.uint16).numpy() for t in (q, k, v))
+    def sdpa(tq, tk, tv):
+        tq = tq[None, :, None, :]
+        tk = tk.permute(1, 0, 2).repeat_interleave(G, dim=0)[None]
+        tv = tv.permute(1, 0, 2).repeat_interleave(G, dim=0)[None]
+        return torch.nn.functional.scaled_dot_product_attention(tq, tk, tv)[0, :, 0].numpy()
+    out8, q8, k8, v8 = oracle.attention_fp8kv(qb, kb, vb)
+    f8 = lambda t: t.to(torch.float8_e4m3fn).double()
+    assert np.allclose(out8, sdpa(f8(q), f8(k), f8(v)), atol=1e-12)
+    assert np.array_equal(k8, k.to(torch.float8_e4m3fn).view(torch.uint8).numpy() * (np.abs(k.double().numpy()) >= 2.0 ** -10))
+    out16 = oracle.attention_bf16kv(qb, kb, vb)
+    assert np.allclose(out16, sdpa(q.double(), k.double(), v.double()), atol=1e-12)
+    assert not np.allclose(out8, out16, atol=1e-3)                  # the two caches really differ
