@@ -84,6 +84,7 @@ def _peaks():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s; MEASURED_PEAKS.json absent)"
 
 
+KV_FORMAT = "fp4"                 # --kv: fp4 = UltraQuant (the product); fp8 / bf16 = the paper's comparison caches
 HEAD_DIM = 128                    # --head-dim: the config's shape at another head size (64 / 256)
 
 
@@ -101,6 +102,10 @@ def step_bytes(wl, num_splits: int, ctx_after: np.ndarray, new_per_seq: int):
     """Algorithmic bytes of one step; returns (total, decode_kernel_only)."""
     d, Hq, Hkv, B = wl.head_dim, wl.num_q_heads, wl.num_kv_heads, wl.batch
     per_tok = 2 * (d // 2 + d // 32)                                 # 136 B (PAPER.md:98)
+    if KV_FORMAT == "fp8":
+        per_tok = 2 * d                                              # comparison cache: one E4M3 byte per element
+    elif KV_FORMAT == "bf16":
+        per_tok = 4 * d
     tokens = int(ctx_after.astype(np.int64).sum())
     pages = int(((ctx_after.astype(np.int64) + wl.page_size - 1) // wl.page_size).sum())
     kv = tokens * Hkv * per_tok
@@ -193,7 +198,8 @@ class ClockSampler(threading.Thread):
 # ----------------------------------------------------------------------------- our arm
 def fill_cache(uq, W, cfg, wl, lens, device, chunk_tokens=1 << 16):
     """Prefill through uq_rotate_quantize_append (bulk appends); shared prefix written once."""
-    cache = uq.alloc_cache(cfg, wl.num_pages, device)
+    fmt = {"fp8": uq.KV_FP8_E4M3, "bf16": uq.KV_BF16}.get(KV_FORMAT)
+    cache = uq.alloc_cache(cfg, wl.num_pages, device) if fmt is None else uq.alloc_baseline_cache(cfg, fmt, wl.num_pages, device)
     bt_dev = torch.from_numpy(wl.block_tables).to(device)
     B = wl.batch
 
@@ -204,8 +210,12 @@ def fill_cache(uq, W, cfg, wl, lens, device, chunk_tokens=1 << 16):
             k, v = W.gen_kv(wl, b_gen, done, done + n, device)
             before = np.zeros(B, np.int32); before[b_tab] = start + done
             cu = np.zeros(B + 1, np.int32); cu[b_tab + 1:] = n
-            uq.rotate_quantize_append(cfg, k, v, torch.from_numpy(cu).to(device),
-                                      torch.from_numpy(before).to(device), bt_dev, cache)
+            if fmt is None:
+                uq.rotate_quantize_append(cfg, k, v, torch.from_numpy(cu).to(device),
+                                          torch.from_numpy(before).to(device), bt_dev, cache)
+            else:
+                uq.baseline_append(cfg, fmt, k, v, torch.from_numpy(cu).to(device), torch.from_numpy(before).to(device),
+                                   bt_dev, cache)
             done += n
 
     if wl.prefix_len:
@@ -265,7 +275,13 @@ def run_ours(args, rank, world, local_rank):
         S_suffix = args.splits or uq.suggest_num_splits_max(cfg, B, max(1, int(suf.mean())), int(suf.max()))
         bufs_sp = uq.StepBuffers(cfg, B, S_suffix, dev)
 
+    fmt = {"fp8": uq.KV_FP8_E4M3, "bf16": uq.KV_BF16}.get(KV_FORMAT)
+
     def step(i):
+        if fmt is not None:                              # comparison cache: append, decode, merge over FP8 / BF16 KV
+            k_new, v_new = kvs[i % n_in]
+            return uq.baseline_decode_step(cfg, fmt, bufs, qs[i % n_in], k_new, v_new, cu_dev, before_dev, after_dev,
+                                           bt_dev, cache, stream=stream)
         if pbufs is not None:
             k_new, v_new = kvs[i % n_in]
             uq.rotate_quantize_append(cfg, k_new, v_new, cu_dev, before_dev, bt_dev, cache, q=qs[i % n_in],
@@ -322,6 +338,16 @@ def run_ours(args, rank, world, local_rank):
     sampler.busy = True
     for i in range(n_inst):
         k_new, v_new = kvs[i % n_in]
+        if fmt is not None:
+            fp8 = fmt == uq.KV_FP8_E4M3
+            uq.baseline_append(cfg, fmt, k_new, v_new, cu_dev, before_dev, bt_dev, cache, q=qs[i % n_in] if fp8 else None,
+                               q_out=bufs.q_fp8 if fp8 else None, stream=stream)
+            dec_ev[i][0].record(stream)
+            uq.baseline_decode_attention(cfg, fmt, bufs.q_fp8 if fp8 else qs[i % n_in], cache, bt_dev, after_dev, S,
+                                         bufs.partial_acc, bufs.partial_ml, stream=stream)
+            dec_ev[i][1].record(stream)
+            uq.merge_splits(cfg, bufs.partial_acc, bufs.partial_ml, bufs.out, stream=stream)
+            continue
         uq.rotate_quantize_append(cfg, k_new, v_new, cu_dev, before_dev, bt_dev, cache,
                                   q=qs[i % n_in], q_fp8=bufs.q_fp8, stream=stream)
         dec_ev[i][0].record(stream)
@@ -358,7 +384,7 @@ def run_ours(args, rank, world, local_rank):
     # one pinned staging block per entry of the input ring (the caller's own buffers: it writes a step's inputs
     # there), uploaded in a single copy per step
     stages = []
-    for j in range(n_in):
+    for j in range(n_in if fmt is None else 0):
         st = uq.HostStage(cfg, B, int(kvs[j][0].shape[0]), int(bt_dev.shape[1]), dev)
         st.h["q"].copy_(qs[j].cpu()); st.h["k_new"].copy_(kvs[j][0].cpu()); st.h["v_new"].copy_(kvs[j][1].cpu())
         st.h["cu_new"].copy_(cu_dev.cpu()); st.h["seq_lens_before"].copy_(before_dev.cpu())
@@ -369,25 +395,27 @@ def run_ours(args, rank, world, local_rank):
     # the host step (one H2D copy, three kernels, one D2H copy) captured once per staging block as a CUDA graph: a
     # step costs the host one graph launch
     graphs = [uq.HostStepGraph(cfg, bufs, st, cache, out_host) for st in stages]
+    ms_e2e = 0.0
 
     def step_host(i):
         graphs[i % n_in].launch()
         stream.synchronize()           # the caller reads O before it can issue the next step
 
-    h2d = stages[0].nbytes                 # the staged block as it is copied (fields 256-byte aligned)
+    h2d = stages[0].nbytes if stages else 0  # the staged block as it is copied (fields 256-byte aligned)
     d2h = out_host.numel() * out_host.element_size()
-    for i in range(max(args.warmup, 3)):
-        step_host(i)
-    barrier()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    sampler.busy = True
-    e0.record(stream)
-    for i in range(args.steps):
-        step_host(i)
-    e1.record(stream)
-    barrier()
-    sampler.busy = False
-    ms_e2e = e0.elapsed_time(e1)
+    if stages:
+        for i in range(max(args.warmup, 3)):
+            step_host(i)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        sampler.busy = True
+        e0.record(stream)
+        for i in range(args.steps):
+            step_host(i)
+        e1.record(stream)
+        barrier()
+        sampler.busy = False
+        ms_e2e = e0.elapsed_time(e1)
     sampler.stop()
 
     # ---- reduce over ranks: max time, summed bytes
@@ -397,14 +425,17 @@ def run_ours(args, rank, world, local_rank):
     ms_total, ms_e2e, dec_ms_mean, dec_ms_med, dec_ms_min, step_ms_med, step_ms_min, ms_sus = red
     ms_step = ms_total / args.steps
     value = whole_job_value(total_b, world, ms_step)
-    e2e_value = whole_job_value(total_b, world, ms_e2e / args.steps)
+    e2e_value = whole_job_value(total_b, world, ms_e2e / args.steps) if ms_e2e > 0 else 0.0
     peak, peak_src = _peaks()
     achieved = decode_b / (dec_ms_mean * 1e-3) / 1e9
     line = {
         "metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": round(ms_step, 5),
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "fp8xfp4->f32",
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": {"fp4": "fp8xfp4->f32", "fp8": "fp8xfp8->f32", "bf16": "bf16xbf16->f32"}[KV_FORMAT],
         "data": "synthetic", "impl": "ours",
+        **({"kv_format": KV_FORMAT + " (comparison cache, PAPER.md:163 - not the headline metric; e2e not measured)"}
+           if fmt is not None else {}),
         "config": {"workload": f"BASELINE.json configs[{args.config - 1}] {wl.name}: batch {B}, "
                                f"{Hq} Q / {Hkv} KV heads, head_dim {d}, ctx {int(ctx_after.min())}"
                                f"..{int(ctx_after.max())} tokens, page_size {wl.page_size}, random block tables; "
@@ -440,10 +471,11 @@ def run_ours(args, rank, world, local_rank):
             "frac_of_measured_peak": round(whole_job_value(total_b, world, ms_sus / sustained[0]) / world / peak, 4),
             "clocks": sampler.summary("sustain"),
             "note": "the same step, back to back for at least --sustain seconds between two CUDA events"}} if sustained else {}),
-        "roofline": {"bound": "hbm", "kernel": "uq::decode_kernel", "achieved": round(achieved, 1),
+        "roofline": {"bound": "hbm", "kernel": "uq::decode_kernel" if fmt is None else "uq::decode_cmp_kernel", "achieved": round(achieved, 1),
                      "peak": peak, "unit": "GB/s", "frac": round(achieved / peak, 4),
                      "frac_of_nominal_8TBs": round(achieved / NOMINAL_HBM_GBS, 4),
-                     "traffic": _ncu_traffic("decode_kernel", f"cfg{args.config}" + (f"_d{d}" if d != 128 else "")),
+                     "traffic": _ncu_traffic("decode_kernel" if fmt is None else "decode_cmp_kernel",
+                                             f"cfg{args.config}" + (f"_d{d}" if d != 128 else "") + (f"_{KV_FORMAT}" if fmt else "")),
                      "algorithmic_bytes": decode_b,
                      "source_key": _source_key(),
                      "peak_source": peak_src,
@@ -707,6 +739,8 @@ def main():
                     help="instead of the decode step, time bulk quantize-on-append of TOKENS new tokens per call")
     ap.add_argument("--calibrate", type=int, default=0, metavar="VECTORS",
                     help="instead of the decode step, time uq_calibrate_c over VECTORS key vectors and 56 constants")
+    ap.add_argument("--kv", default="fp4", choices=["fp4", "fp8", "bf16"],
+                    help="fp4: UltraQuant (default).  fp8 / bf16: the same step over the paper's comparison caches")
     ap.add_argument("--head-dim", type=int, default=128, choices=[64, 128, 256],
                     help="run the config's shape at another head size (the decode step only)")
     ap.add_argument("--sustain", type=float, default=2.0, metavar="SECONDS",
@@ -715,8 +749,9 @@ def main():
     ap.add_argument("--ref-budget", type=float, default=90.0, help="seconds for the whole --impl reference run")
     args = ap.parse_args()
 
-    global HEAD_DIM
+    global HEAD_DIM, KV_FORMAT
     HEAD_DIM = args.head_dim
+    KV_FORMAT = args.kv
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

@@ -249,6 +249,35 @@ int32_t uq_calibrate_c(const uq_config* cfg, const void* x, int64_t n_vec, int32
                        const float* c_grid, int32_t n_c, int32_t scale_mode, const float* levels,
                        double* sq_err, double* sq_norm, void* stream);
 
+/*
+ * COMPARISON CACHES — not UltraQuant: the two systems the paper compares it with at kernel level,
+ * "hardware FP8 KV" and the BF16 baseline (PAPER.md:163; Table 3, :293-301), as paged caches under the same decode
+ * CTA design, so that the paper's relative claims (4-bit reads about half the bytes of FP8, :188; the FP4 kernel within
+ * 1.18 x of FP8 at 32K, :295-301) can be restated on B200.  The paper only names them; reading G19:
+ *   UQ_KV_FP8_E4M3  K and V stored as OCP E4M3 bytes of the bf16 values themselves (no rotation, scale 1, round to
+ *                   nearest even, saturating at 448, +0 only); the query is cast the same way (q_out of the append);
+ *   UQ_KV_BF16      K and V stored as they are; the query is the bf16 query (the append does not touch it).
+ * Record of (page, kv head): K rows [16 tokens][128 elements] then V [128 channels][16 tokens], 4096 / 8192 bytes; cache
+ * base 128-byte aligned.  head_dim 128 only.  uq_baseline_decode_attention writes the partial format of
+ * uq_decode_attention (same schedule, same num_splits meaning); uq_merge_splits finishes.  Scores: E4M3 x E4M3 by
+ * kind::f8f6f4 / bf16 x bf16 by kind::f16, fp32 accumulation; P enters the PV product as fp16, V as fp16 (from E4M3:
+ * exact) / bf16: the accuracy domain stated for uq_decode_attention applies.
+ */
+#define UQ_KV_FP8_E4M3 1
+#define UQ_KV_BF16 2
+size_t uq_baseline_record_bytes(const uq_config* cfg, int32_t kv_format);
+/* k_new, v_new, cu_new, seq_lens, block_tables, total_new: as uq_rotate_quantize_append.  q bf16 [batch, Hq, 128] and
+ * q_out uint8 [batch, Hq, 128] (FP8 only; both NULL or both given; ignored for BF16). */
+int32_t uq_baseline_append(const uq_config* cfg, int32_t kv_format, const void* k_new, const void* v_new,
+                           const int32_t* cu_new, const int32_t* seq_lens, const int32_t* block_tables,
+                           int32_t max_pages, int32_t batch, int32_t total_new, void* cache, int64_t num_pages,
+                           const void* q, void* q_out, void* stream);
+/* q_enc: uint8 E4M3 [batch, Hq, 128] (FP8) or bf16 [batch, Hq, 128] (BF16); everything else as uq_decode_attention. */
+int32_t uq_baseline_decode_attention(const uq_config* cfg, int32_t kv_format, const void* q_enc, const void* cache,
+                                     int64_t num_pages, const int32_t* block_tables, int32_t max_pages,
+                                     const int32_t* seq_lens, int32_t batch, int32_t num_splits,
+                                     float* partial_acc, float* partial_ml, void* stream);
+
 /* Host.  A num_splits (slot count) that lets uq_decode_attention balance `batch` sequences of about
  * `avg_seq_len` tokens over the current device with room for sequences twice that long (never below 1). */
 int32_t uq_suggest_num_splits(const uq_config* cfg, int32_t batch, int32_t avg_seq_len);

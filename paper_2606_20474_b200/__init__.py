@@ -16,6 +16,13 @@ from .binding import (  # noqa: F401
     HostStage,
     HostStepGraph,
     alloc_cache,
+    alloc_baseline_cache,
+    baseline_append,
+    baseline_decode_attention,
+    baseline_decode_step,
+    baseline_record_bytes,
+    KV_BF16,
+    KV_FP8_E4M3,
     cache_record_bytes,
     calibrate_c,
     PrefixBuffers,

@@ -80,6 +80,12 @@ def _load():
     lib.uq_calibrate_c.argtypes = [cfgp, vp, i64, i32, vp, i32, i32, vp, vp, vp, vp]
     lib.uq_decode_workspace_bytes.restype = i32
     lib.uq_decode_workspace_bytes.argtypes = [cfgp, i32, i32, ctypes.POINTER(ctypes.c_size_t)]
+    lib.uq_baseline_record_bytes.restype = ctypes.c_size_t
+    lib.uq_baseline_record_bytes.argtypes = [cfgp, i32]
+    lib.uq_baseline_append.restype = i32
+    lib.uq_baseline_append.argtypes = [cfgp, i32, vp, vp, vp, vp, vp, i32, i32, i32, vp, i64, vp, vp, vp]
+    lib.uq_baseline_decode_attention.restype = i32
+    lib.uq_baseline_decode_attention.argtypes = [cfgp, i32, vp, vp, i64, vp, i32, vp, i32, i32, vp, vp, vp]
     lib.uq_suggest_num_splits.restype = i32
     lib.uq_suggest_num_splits.argtypes = [cfgp, i32, i32]
     lib.uq_suggest_num_splits_max.restype = i32
@@ -367,3 +373,63 @@ class HostStepGraph:
     def launch(self) -> torch.Tensor:
         self.graph.replay()
         return self.out_host
+
+
+# ----------------------------------------------------------------------------- comparison caches (include/uq.h)
+KV_FP8_E4M3 = 1
+KV_BF16 = 2
+
+
+def baseline_record_bytes(cfg: UQConfig, kv_format: int) -> int:
+    c = cfg.c()
+    return int(_load().uq_baseline_record_bytes(ctypes.byref(c), int(kv_format)))
+
+
+def alloc_baseline_cache(cfg: UQConfig, kv_format: int, num_pages: int, device="cuda") -> torch.Tensor:
+    """uint8 [num_pages, num_kv_heads, 4096 (FP8) | 8192 (BF16)]: K rows [16 tok][128] then V [128 ch][16 tok]."""
+    n = baseline_record_bytes(cfg, kv_format)
+    if n == 0:
+        raise UQError(f"uq_baseline_record_bytes: {last_error()}")
+    return torch.zeros((num_pages, cfg.num_kv_heads, n), dtype=torch.uint8, device=device)
+
+
+def baseline_append(cfg: UQConfig, kv_format: int, k_new, v_new, cu_new, seq_lens, block_tables, cache, q=None, q_out=None,
+                    stream=None) -> None:
+    """uq_baseline_append: store new K/V rows in the FP8-E4M3 / BF16 comparison cache (FP8: also q -> q_out E4M3)."""
+    lib = _load()
+    _dev(k_new, torch.bfloat16, "k_new"); _dev(v_new, torch.bfloat16, "v_new")
+    _dev(cu_new, torch.int32, "cu_new"); _dev(seq_lens, torch.int32, "seq_lens")
+    _dev(block_tables, torch.int32, "block_tables"); _dev(cache, torch.uint8, "cache")
+    if q is not None and q_out is not None:
+        _dev(q, torch.bfloat16, "q"); _dev(q_out, torch.uint8, "q_out")
+    c = cfg.c()
+    st = lib.uq_baseline_append(ctypes.byref(c), int(kv_format), _p(k_new), _p(v_new), _p(cu_new), _p(seq_lens),
+                                _p(block_tables), block_tables.shape[1], seq_lens.shape[0], k_new.shape[0], _p(cache),
+                                cache.shape[0], _p(q) if q_out is not None else None, _p(q_out), _stream(stream))
+    _check(st, "uq_baseline_append")
+
+
+def baseline_decode_attention(cfg: UQConfig, kv_format: int, q_enc, cache, block_tables, seq_lens, num_splits: int,
+                              partial_acc, partial_ml, stream=None) -> None:
+    """uq_baseline_decode_attention: split-K partials over the comparison cache (q_enc: uint8 E4M3 or bf16)."""
+    lib = _load()
+    _dev(q_enc, torch.uint8 if kv_format == KV_FP8_E4M3 else torch.bfloat16, "q_enc"); _dev(cache, torch.uint8, "cache")
+    _dev(block_tables, torch.int32, "block_tables"); _dev(seq_lens, torch.int32, "seq_lens")
+    _dev(partial_acc, torch.float32, "partial_acc"); _dev(partial_ml, torch.float32, "partial_ml")
+    c = cfg.c()
+    st = lib.uq_baseline_decode_attention(ctypes.byref(c), int(kv_format), _p(q_enc), _p(cache), cache.shape[0],
+                                          _p(block_tables), block_tables.shape[1], _p(seq_lens), seq_lens.shape[0],
+                                          int(num_splits), _p(partial_acc), _p(partial_ml), _stream(stream))
+    _check(st, "uq_baseline_decode_attention")
+
+
+def baseline_decode_step(cfg: UQConfig, kv_format: int, bufs: "StepBuffers", q, k_new, v_new, cu_new, seq_lens_before,
+                         seq_lens_after, block_tables, cache, stream=None) -> torch.Tensor:
+    """One step over a comparison cache: append (+ query cast for FP8), split-K decode, merge.  Returns bufs.out."""
+    fp8 = kv_format == KV_FP8_E4M3
+    baseline_append(cfg, kv_format, k_new, v_new, cu_new, seq_lens_before, block_tables, cache,
+                    q=q if fp8 else None, q_out=bufs.q_fp8 if fp8 else None, stream=stream)
+    baseline_decode_attention(cfg, kv_format, bufs.q_fp8 if fp8 else q, cache, block_tables, seq_lens_after,
+                              bufs.num_splits, bufs.partial_acc, bufs.partial_ml, stream=stream)
+    merge_splits(cfg, bufs.partial_acc, bufs.partial_ml, bufs.out, stream=stream)
+    return bufs.out

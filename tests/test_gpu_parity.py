@@ -840,3 +840,75 @@ def test_second_device_of_one_process_if_there_is_one():
             out, _, _ = H.run_decode(cfg, cache, bt, wl.ctx_lens, W.gen_q(wl, dev), 3)
             outs.append(out.cpu())
     assert torch.equal(outs[0], outs[1])
+
+
+def _fill_baseline_cache(cfg, kv, wl):
+    cache = uq.alloc_baseline_cache(cfg, kv, wl.num_pages, DEV)
+    cache.fill_(0xFF)                                       # NaN patterns of E4M3 / bf16: stale bytes must never reach an output
+    bt = torch.from_numpy(wl.block_tables).to(DEV)
+    B = wl.batch
+    for b in range(B):
+        L = int(wl.ctx_lens[b])
+        done = 0
+        for n in ([L] if b % 2 == 0 else [min(L, 5), min(max(L - 5, 0), 40), max(L - 45, 0)]):   # one call, or in pieces
+            if n == 0:
+                continue
+            k, v = W.gen_kv(wl, b, done, done + n, DEV)
+            before = np.zeros(B, np.int32); before[b] = done
+            cu = np.zeros(B + 1, np.int32); cu[b + 1:] = n
+            uq.baseline_append(cfg, kv, k, v, torch.from_numpy(cu).to(DEV), torch.from_numpy(before).to(DEV), bt, cache)
+            done += n
+    torch.cuda.synchronize()
+    return cache, bt
+
+
+@pytest.mark.parametrize("kv", ["fp8", "bf16"])
+@pytest.mark.parametrize("hq,hkv", [(16, 1), (12, 2), (8, 8)])
+def test_comparison_caches_fp8_and_bf16_kv(kv, hq, hkv):
+    """The comparison kernels ("hardware FP8 KV" / BF16 baseline): cache image bit for
+    bit (E4M3 bytes of the bf16 values = oracle.cast_e4m3; the bf16 bits themselves), the FP8 query bytes, and the
+    decode output within 2e-3 + 1e-2 |ref| of oracle.attention_fp8kv / attention_bf16kv — ragged batch with empty,
+    one-token and multi-tile sequences, GQA 16 / 6 / 1, slot counts 1, 3 and 64, peaked queries."""
+    fmt = uq.KV_FP8_E4M3 if kv == "fp8" else uq.KV_BF16
+    wl = W.make_custom("cmp", 61, [0, 1, 17, 203, 1000, 16, 31, 129], hq, hkv, outlier_channels=3, outlier_gain=8.0,
+                       peaked_frac=0.3)
+    cfg = H.cfg_of(wl)
+    cache, bt = _fill_baseline_cache(cfg, fmt, wl)
+    q = W.gen_q(wl, DEV)
+    qb = H.bits(q)
+    host = cache.cpu().numpy()
+    kpage = 2048 if kv == "fp8" else 4096
+    lens = torch.from_numpy(wl.ctx_lens.astype(np.int32)).to(DEV)
+    empty = torch.zeros((0, hkv, 128), dtype=torch.bfloat16, device=DEV)
+    cu0 = torch.zeros(wl.batch + 1, dtype=torch.int32, device=DEV)
+    refs = {}
+    for b in range(wl.batch):
+        L = int(wl.ctx_lens[b])
+        if L == 0:
+            continue
+        k, v = W.seq_kv(wl, b, L, DEV)
+        kbits, vbits = H.bits(k), H.bits(v)
+        recs = host[wl.block_tables[b][:-(-L // 16)]]                          # [pages, Hkv, rec]
+        if kv == "fp8":
+            gk = recs[..., :kpage].reshape(-1, hkv, 16, 128).transpose(0, 2, 1, 3).reshape(-1, hkv, 128)[:L]
+            gv = recs[..., kpage:].reshape(-1, hkv, 128, 16).transpose(0, 3, 1, 2).reshape(-1, hkv, 128)[:L]
+            ref, q8, k8, v8 = oracle.attention_fp8kv(qb[b], kbits, vbits)
+            assert np.array_equal(gk, k8) and np.array_equal(gv, v8), f"seq {b}: FP8 cache image differs"
+            refs[b] = (ref, q8)
+        else:
+            r16 = recs.view(np.uint16)
+            gk = r16[..., :kpage // 2].reshape(-1, hkv, 16, 128).transpose(0, 2, 1, 3).reshape(-1, hkv, 128)[:L]
+            gv = r16[..., kpage // 2:].reshape(-1, hkv, 128, 16).transpose(0, 3, 1, 2).reshape(-1, hkv, 128)[:L]
+            assert np.array_equal(gk, kbits) and np.array_equal(gv, vbits), f"seq {b}: BF16 cache image differs"
+            refs[b] = (oracle.attention_bf16kv(qb[b], kbits, vbits), None)
+    for S in (1, 3, 64):
+        bufs = uq.StepBuffers(cfg, wl.batch, S, DEV)
+        bufs.partial_acc.fill_(float("nan")); bufs.partial_ml.fill_(float("nan"))
+        out = uq.baseline_decode_step(cfg, fmt, bufs, q, empty, empty, cu0, lens, lens, bt, cache)
+        torch.cuda.synchronize()
+        out = out.float().cpu().numpy().astype(np.float64)
+        assert np.all(out[0] == 0)                                              # the empty sequence
+        for b, (ref, q8) in refs.items():
+            if q8 is not None:
+                assert np.array_equal(bufs.q_fp8[b].cpu().numpy(), q8), f"seq {b}: FP8 query bytes differ"
+            H.check_out(out[b], ref, f"{kv} kv seq {b} S={S}")
