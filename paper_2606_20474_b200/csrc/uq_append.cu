@@ -820,6 +820,7 @@ extern "C" int32_t uq_rotate_quantize_append(const uq_config* cfg, const void* k
                                              int64_t num_pages, const void* q, void* q_fp8,
                                              void* stream) {
   using namespace uq;
+  NvtxRange nvtx_range("uq_rotate_quantize_append");
   int32_t st = check_config(cfg);
   if (st != UQ_OK) return st;
   if (batch <= 0 || total_new < 0 || max_pages <= 0 || num_pages <= 0) {

@@ -109,6 +109,7 @@ extern "C" int32_t uq_calibrate_c(const uq_config* cfg, const void* x, int64_t n
                                   const float* c_grid, int32_t n_c, int32_t scale_mode, const float* levels,
                                   double* sq_err, double* sq_norm, void* stream) {
   using namespace uq;
+  NvtxRange nvtx_range("uq_calibrate_c");
   int32_t st = check_config(cfg);
   if (st != UQ_OK) return st;
   st = require_head_dim_128(cfg, "uq_calibrate_c");

@@ -4,6 +4,7 @@
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>
 #include <stdint.h>
 #include <stdio.h>
 
@@ -35,6 +36,15 @@ struct RecordGeo {
 };
 static_assert(RecordGeo<128>::kBytes == kRecordBytes && RecordGeo<128>::kVCodes == kOffVCodes &&
               RecordGeo<128>::kKScales == kOffKScales && RecordGeo<128>::kVScales == kOffVScales, "layout");
+
+// NVTX range around an ABI call (tracing).  nvtx3 is header-only and does nothing unless a tool (nsys, ncu
+// --nvtx) has injected its library into the process: one predictable branch per call otherwise.
+struct NvtxRange {
+  explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+  ~NvtxRange() { nvtxRangePop(); }
+  NvtxRange(const NvtxRange&) = delete;
+  NvtxRange& operator=(const NvtxRange&) = delete;
+};
 
 void set_error(const char* fmt, ...);
 int32_t check_config(const uq_config* cfg);  // UQ_OK / UQ_ERR_*; sets the error string

@@ -868,6 +868,7 @@ extern "C" int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, 
                                        const int32_t* seq_lens, int32_t batch, int32_t num_splits,
                                        float* partial_acc, float* partial_ml, void* stream) {
   using namespace uq;
+  NvtxRange nvtx_range("uq_decode_attention");
   int32_t st = check_config(cfg);
   if (st != UQ_OK) return st;
   if (!q_fp8 || !cache || !block_tables || !seq_lens || !partial_acc || !partial_ml || batch <= 0 ||

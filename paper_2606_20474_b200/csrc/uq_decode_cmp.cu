@@ -686,6 +686,7 @@ extern "C" int32_t uq_baseline_append(const uq_config* cfg, int32_t kv_format, c
                                       int32_t max_pages, int32_t batch, int32_t total_new, void* cache, int64_t num_pages,
                                       const void* q, void* q_out, void* stream) {
   using namespace uq;
+  NvtxRange nvtx_range("uq_baseline_append");
   int32_t st = check_kv(cfg, kv_format, "uq_baseline_append");
   if (st != UQ_OK) return st;
   if (batch <= 0 || total_new < 0 || max_pages <= 0 || num_pages <= 0) {
@@ -730,6 +731,7 @@ extern "C" int32_t uq_baseline_decode_attention(const uq_config* cfg, int32_t kv
                                                 const int32_t* seq_lens, int32_t batch, int32_t num_splits,
                                                 float* partial_acc, float* partial_ml, void* stream) {
   using namespace uq;
+  NvtxRange nvtx_range("uq_baseline_decode_attention");
   int32_t st = check_kv(cfg, kv_format, "uq_baseline_decode_attention");
   if (st != UQ_OK) return st;
   if (!q_enc || !cache || !block_tables || !seq_lens || !partial_acc || !partial_ml || batch <= 0 || num_splits <= 0 ||

@@ -672,6 +672,7 @@ extern "C" int32_t uq_decode_prefix_attention(const uq_config* cfg, const void* 
                                               int32_t batch, int32_t prefix_len, int32_t num_splits,
                                               float* partial_acc, float* partial_ml, void* stream) {
   using namespace uq;
+  NvtxRange nvtx_range("uq_decode_prefix_attention");
   int32_t st = check_config(cfg);
   if (st != UQ_OK) return st;
   st = require_head_dim_128(cfg, "uq_decode_prefix_attention");

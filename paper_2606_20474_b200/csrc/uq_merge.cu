@@ -172,6 +172,7 @@ merge_any_kernel(const float* __restrict__ acc_a, const float* __restrict__ ml_a
 extern "C" int32_t uq_merge_splits(const uq_config* cfg, const float* partial_acc, const float* partial_ml,
                                    int32_t batch, int32_t num_splits, void* out_bf16, void* stream) {
   using namespace uq;
+  NvtxRange nvtx_range("uq_merge_splits");
   int32_t st = check_config(cfg);
   if (st != UQ_OK) return st;
   if (batch <= 0 || num_splits <= 0 || !partial_acc || !partial_ml || !out_bf16) {
@@ -197,6 +198,7 @@ extern "C" int32_t uq_merge_splits2(const uq_config* cfg, const float* acc_a, co
                                     const float* acc_b, const float* ml_b, int32_t splits_b, int32_t batch,
                                     void* out_bf16, void* stream) {
   using namespace uq;
+  NvtxRange nvtx_range("uq_merge_splits2");
   int32_t st = check_config(cfg);
   if (st != UQ_OK) return st;
   if (batch <= 0 || splits_a <= 0 || splits_b <= 0 || !acc_a || !ml_a || !acc_b || !ml_b || !out_bf16) {
