@@ -266,7 +266,7 @@ def run_ours(args, rank, world, local_rank):
     pbufs, pfx = None, 0
     if args.shared_prefix and wl.prefix_len >= 128:
         pfx = (int(wl.prefix_len) // 128) * 128
-        pbufs = uq.PrefixBuffers(cfg, B, 2, dev)
+        pbufs = uq.PrefixBuffers(cfg, B, uq.suggest_prefix_splits(cfg, B, pfx), dev)
         pbufs.suffix_lens.copy_(torch.from_numpy((ctx_after - pfx).astype(np.int32)))
         # slots of the suffix call: the suffix lengths are far more skewed than the whole lengths (config 4: mean 16.5k,
         # maximum 98k), and the balanced schedule lengthens every CTA's range until the longest item fits into S - 1

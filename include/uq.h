@@ -286,6 +286,9 @@ int32_t uq_suggest_num_splits(const uq_config* cfg, int32_t batch, int32_t avg_s
  * (a skewed length mix — e.g. the private suffixes of a shared-prefix batch — otherwise stretches every CTA's range). */
 int32_t uq_suggest_num_splits_max(const uq_config* cfg, int32_t batch, int32_t avg_seq_len, int32_t max_seq_len);
 
+/* Host.  A slot count for uq_decode_prefix_attention (>= 2) that lets every SM take an equal tile range of the prefix. */
+int32_t uq_suggest_prefix_splits(const uq_config* cfg, int32_t batch, int32_t prefix_len);
+
 #ifdef __cplusplus
 }
 #endif

@@ -38,5 +38,6 @@ from .binding import (  # noqa: F401
     merge_splits,
     rotate_quantize_append,
     suggest_num_splits,
+    suggest_prefix_splits,
     suggest_num_splits_max,
 )

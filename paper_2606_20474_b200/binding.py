@@ -88,6 +88,8 @@ def _load():
     lib.uq_baseline_decode_attention.argtypes = [cfgp, i32, vp, vp, i64, vp, i32, vp, i32, i32, vp, vp, vp]
     lib.uq_suggest_num_splits.restype = i32
     lib.uq_suggest_num_splits.argtypes = [cfgp, i32, i32]
+    lib.uq_suggest_prefix_splits.restype = i32
+    lib.uq_suggest_prefix_splits.argtypes = [cfgp, i32, i32]
     lib.uq_suggest_num_splits_max.restype = i32
     lib.uq_suggest_num_splits_max.argtypes = [cfgp, i32, i32, i32]
     _lib = lib
@@ -146,6 +148,11 @@ def suggest_num_splits(cfg: UQConfig, batch: int, avg_seq_len: int) -> int:
 def suggest_num_splits_max(cfg: UQConfig, batch: int, avg_seq_len: int, max_seq_len: int) -> int:
     c = cfg.c()
     return int(_load().uq_suggest_num_splits_max(ctypes.byref(c), int(batch), int(avg_seq_len), int(max_seq_len)))
+
+
+def suggest_prefix_splits(cfg: UQConfig, batch: int, prefix_len: int) -> int:
+    c = cfg.c()
+    return int(_load().uq_suggest_prefix_splits(ctypes.byref(c), int(batch), int(prefix_len)))
 
 
 def alloc_cache(cfg: UQConfig, num_pages: int, device="cuda") -> torch.Tensor:

@@ -179,3 +179,20 @@ extern "C" int32_t uq_suggest_num_splits_max(const uq_config* cfg, int32_t batch
   if (s > 64) s = 64;
   return (int32_t)s;
 }
+
+extern "C" int32_t uq_suggest_prefix_splits(const uq_config* cfg, int32_t batch, int32_t prefix_len) {
+  // uq_decode_prefix_attention: items = (group of 8 or 16 sequences, kv head), prefix_len / 128 tiles each, one equal
+  // tile range per SM; an item then spans about tiles / range + 1 ranges = slots.
+  if (uq::check_config(cfg) != UQ_OK || batch <= 0 || prefix_len < 128) return 2;
+  int sms = 148;
+  if (uq::current_device_sms(&sms) != UQ_OK) sms = 148;
+  const int nseq = (cfg->num_q_heads / cfg->num_kv_heads) > 8 ? 8 : 16;
+  const int64_t tiles = prefix_len / 128;
+  const int64_t total = (int64_t)((batch + nseq - 1) / nseq) * cfg->num_kv_heads * tiles;
+  int64_t range = (total + sms - 1) / sms;
+  if (range < 1) range = 1;
+  int64_t s = (tiles + range - 1) / range + 1;
+  if (s < 2) s = 2;
+  if (s > 64) s = 64;
+  return (int32_t)s;
+}

@@ -308,7 +308,7 @@ def test_full_size_cfg4_shared_prefix_step_32_sequences_both_decode_paths():
     suf = (wl.ctx_lens + 1 - pfx).astype(np.int64)
     bufs_sp = uq.StepBuffers(cfg, wl.batch, uq.suggest_num_splits_max(cfg, wl.batch, int(suf.mean()), int(suf.max())), DEV)
     bufs_sp.q_fp8.copy_(bufs.q_fp8)
-    pb = uq.PrefixBuffers(cfg, wl.batch, 2, DEV)
+    pb = uq.PrefixBuffers(cfg, wl.batch, uq.suggest_prefix_splits(cfg, wl.batch, pfx), DEV)
     pb.suffix_lens.copy_(torch.from_numpy((wl.ctx_lens + 1 - pfx).astype(np.int32)))
     out_sp = uq.decode_attention_shared_prefix(cfg, bufs_sp, pb, cache, bt, pfx)
     torch.cuda.synchronize()
