@@ -99,7 +99,7 @@ EncodeTiledFn encode_tiled_fn();                                        // nullp
 int32_t launch_prefix_m(const uq_config* cfg, const void* q_fp8, const void* cache, long long records,
                         const int32_t* block_tables, int32_t max_pages, int32_t batch, int32_t prefix_len,
                         int32_t num_splits, float* partial_acc, float* partial_ml, cudaStream_t stream);
-int32_t k_code_map(const void* cache, long long records, int head_dim, CUtensorMap* out);
+int32_t k_code_map(const void* cache, long long records, int head_dim, CUtensorMap* out, CUtensorMap* out_rest = nullptr);
 int32_t q_map(const void* q_fp8, long long rows, int head_dim, CUtensorMap* out);
 #endif
 

@@ -144,6 +144,7 @@ struct Shared {
 template <int D>
 __global__ void __launch_bounds__(DecodeGeo<D>::kThreads, DecodeGeo<D>::kCtasPerSm)
 decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_q,
+              const __grid_constant__ CUtensorMap tmap_v,
               const uint8_t* __restrict__ cache, const int32_t* __restrict__ block_tables, int max_pages,
               const int32_t* __restrict__ seq_lens, int batch, int Hq, int Hkv, int num_splits,
               float score_scale /* sm_scale * log2(e) */, float* __restrict__ partial_acc,
@@ -373,6 +374,9 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     const int n_stages = is_k ? kKStages : kVStages;
     const uint32_t bar_e = is_k ? bar_emptyk : bar_emptyv,
                    bar_f = is_k ? (D == 64 ? smem_u32(&sh.full_kp[0]) : bar_fullk) : bar_fullv;
+    // head_dim <= 128: the rest of FOUR records (V codes, K scales, V scales) per copy — cp.async.bulk.tensor ...
+    // tile::gather4 over the cache seen as [record][9 D bytes] rows of 8-byte elements: two copies a tile instead of eight
+    constexpr bool kGather = (D <= 128);
     const uint32_t page_tx = is_k ? (uint32_t)Geo::kKPacked : (uint32_t)kRestBytes;
     const int pl = (kHalves == 2) ? (lane & 7) : lane;  // the lane's page of the tile; head_dim 256: lanes 8..15 of the
     const int hl = (kHalves == 2) ? (lane >> 3) : 0;    // K producer copy the second 128-channel block of pages 0..7
@@ -391,6 +395,17 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
         const int nb = un.p0 + kTilePages * (i + 1) + pl;
         page_next = (copier && nb < un.p1) ? bt[kTilePages * (i + 1)] : 0;
         mbar_wait(bar_e + 8 * s, ph);
+        if (kGather && !is_k) {
+          const int nops = (npg + 3) >> 2;             // pages past the end name record 0: copied, never read
+          if (lane == 0) mbar_expect_tx(bar_f + 8 * s, (uint32_t)nops * 4u * page_tx);
+          const int l4 = 4 * (lane & 1);
+          const int r0 = __shfl_sync(kFull, page, l4) * Hkv + un.kvh, r1 = __shfl_sync(kFull, page, l4 + 1) * Hkv + un.kvh,
+                    r2 = __shfl_sync(kFull, page, l4 + 2) * Hkv + un.kvh, r3 = __shfl_sync(kFull, page, l4 + 3) * Hkv + un.kvh;
+          if (lane < nops)
+            tma_gather4(base + kOffV + s * kVStageBytes + 4 * kRestBytes * lane, &tmap_v, 0, r0, r1, r2, r3, bar_f + 8 * s, pol);
+          if (++s == n_stages) { s = 0; ph ^= 1; }
+          continue;
+        }
         if (lane == 0) mbar_expect_tx(bar_f + 8 * s, (uint32_t)npg * page_tx);
         __syncwarp();
         if ((kHalves == 2 && is_k) ? (copier && pl < npg) : (lane < npg)) {
@@ -763,7 +778,7 @@ struct MapEntry {
   const void* cache;
   long long records;
   int device, head_dim;
-  CUtensorMap map;
+  CUtensorMap map, rest;
 };
 std::mutex g_map_mu;
 MapEntry g_maps[8];
@@ -773,7 +788,7 @@ int g_map_n = 0, g_map_next = 0;
 
 // 3-D view of the cache for TMA: [record][16 tokens][head_dim x 4-bit]; box = one page of K codes, 128 channels wide
 // (head_dim 256: two copies per page; head_dim 64 does not use it).
-int32_t k_code_map(const void* cache, long long records, int head_dim, CUtensorMap* out) {
+int32_t k_code_map(const void* cache, long long records, int head_dim, CUtensorMap* out, CUtensorMap* out_rest) {
   int dev = 0;
   (void)cudaGetDevice(&dev);                           // the same virtual address may be another allocation on another device
   const EncodeTiledFn encode = encode_tiled_fn();
@@ -782,14 +797,31 @@ int32_t k_code_map(const void* cache, long long records, int head_dim, CUtensorM
   for (int i = 0; i < g_map_n; ++i)
     if (g_maps[i].cache == cache && g_maps[i].records == records && g_maps[i].device == dev && g_maps[i].head_dim == head_dim) {
       *out = g_maps[i].map;
+      if (out_rest) *out_rest = g_maps[i].rest;
       return UQ_OK;
     }
   const cuuint64_t gdim[3] = {(cuuint64_t)head_dim, 16, (cuuint64_t)records};
   const cuuint64_t gstr[2] = {(cuuint64_t)head_dim / 2, (cuuint64_t)17 * head_dim};
   const cuuint32_t box[3] = {128, 16, 1};              // the packed 4-bit tensor type takes 128-wide boxes only
   const cuuint32_t estr[3] = {1, 1, 1};
-  CUtensorMap m;
-  const CUresult cr = encode(&m, CU_TENSOR_MAP_DATA_TYPE_16U4_ALIGN16B, 3, const_cast<void*>(cache), gdim, gstr, box,
+  CUtensorMap m = {}, mr = {};
+  CUresult cr = CUDA_SUCCESS;
+  if (head_dim <= 128) {
+    // the rest of a record (9 D bytes from byte 8 D on) as a row of 8-byte elements: the source of the gather4 copies
+    const cuuint64_t rdim[2] = {(cuuint64_t)(9 * head_dim / 8), (cuuint64_t)records};
+    const cuuint64_t rstr[1] = {(cuuint64_t)17 * head_dim};
+    const cuuint32_t rbox[2] = {(cuuint32_t)(9 * head_dim / 8), 1};
+    const cuuint32_t rest_[2] = {1, 1};
+    cr = encode(&mr, CU_TENSOR_MAP_DATA_TYPE_UINT64, 2, const_cast<uint8_t*>((const uint8_t*)cache) + 8 * head_dim, rdim, rstr,
+                rbox, rest_, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (cr != CUDA_SUCCESS) {
+      set_error("decode: cuTensorMapEncodeTiled (record rest, gather4) failed with CUresult %d", (int)cr);
+      return UQ_ERR_CUDA;
+    }
+  }
+  if (head_dim >= 128)
+  cr = encode(&m, CU_TENSOR_MAP_DATA_TYPE_16U4_ALIGN16B, 3, const_cast<void*>(cache), gdim, gstr, box,
                              estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (cr != CUDA_SUCCESS) {
@@ -802,9 +834,11 @@ int32_t k_code_map(const void* cache, long long records, int head_dim, CUtensorM
   e.device = dev;
   e.head_dim = head_dim;
   e.map = m;
+  e.rest = mr;
   g_map_next = (g_map_next + 1) % 8;
   if (g_map_n < 8) ++g_map_n;
   *out = m;
+  if (out_rest) *out_rest = mr;
   return UQ_OK;
 }
 
@@ -841,7 +875,8 @@ int32_t q_map(const void* q_fp8, long long rows, int head_dim, CUtensorMap* out)
 
 namespace {
 template <int D>
-int32_t launch_decode(const uq_config* cfg, const CUtensorMap& tmap, const CUtensorMap& tmap_q, const void* cache,
+int32_t launch_decode(const uq_config* cfg, const CUtensorMap& tmap, const CUtensorMap& tmap_q, const CUtensorMap& tmap_v,
+                      const void* cache,
                       const int32_t* block_tables, int32_t max_pages, const int32_t* seq_lens, int32_t batch,
                       int32_t num_splits, float score_scale, float* partial_acc, float* partial_ml, int sm_count,
                       cudaStream_t stream) {
@@ -852,7 +887,7 @@ int32_t launch_decode(const uq_config* cfg, const CUtensorMap& tmap, const CUten
   const dim3 grid((unsigned)((num_splits == 1 && items < slots) ? items : slots));
   int32_t st = opt_in_dynamic_smem((const void*)decode_kernel<D>, Geo::kSmemBytes, "decode: cudaFuncSetAttribute");
   if (st != UQ_OK) return st;
-  return check_cuda(launch_pdl(decode_kernel<D>, grid, dim3(Geo::kThreads), (size_t)Geo::kSmemBytes, stream, tmap, tmap_q,
+  return check_cuda(launch_pdl(decode_kernel<D>, grid, dim3(Geo::kThreads), (size_t)Geo::kSmemBytes, stream, tmap, tmap_q, tmap_v,
                                (const uint8_t*)cache, block_tables, (int)max_pages, seq_lens, (int)batch,
                                (int)cfg->num_q_heads, (int)cfg->num_kv_heads, (int)num_splits, score_scale, partial_acc,
                                partial_ml),
@@ -891,11 +926,9 @@ extern "C" int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, 
                             cfg->page_size, 0, (cudaStream_t)stream);
     if (st != UQ_OK) return st;
   }
-  CUtensorMap tmap = {};                               // head_dim 64 copies the packed K codes without a tensor map
-  if (cfg->head_dim != 64) {
-    st = k_code_map(cache, records, cfg->head_dim, &tmap);
-    if (st != UQ_OK) return st;
-  }
+  CUtensorMap tmap = {}, tmap_v = {};                  // head_dim 64 copies the packed K codes without a tensor map
+  st = k_code_map(cache, records, cfg->head_dim, &tmap, &tmap_v);
+  if (st != UQ_OK) return st;
   CUtensorMap tmap_q;
   st = q_map(q_fp8, (long long)batch * cfg->num_q_heads, cfg->head_dim, &tmap_q);
   if (st != UQ_OK) return st;
@@ -909,13 +942,13 @@ extern "C" int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, 
   if (st != UQ_OK) return st;
   switch (cfg->head_dim) {
     case 64:
-      return launch_decode<64>(cfg, tmap, tmap_q, cache, block_tables, max_pages, seq_lens, batch, num_splits, score_scale,
+      return launch_decode<64>(cfg, tmap, tmap_q, tmap_v, cache, block_tables, max_pages, seq_lens, batch, num_splits, score_scale,
                                partial_acc, partial_ml, sm_count, (cudaStream_t)stream);
     case 256:
-      return launch_decode<256>(cfg, tmap, tmap_q, cache, block_tables, max_pages, seq_lens, batch, num_splits, score_scale,
+      return launch_decode<256>(cfg, tmap, tmap_q, tmap_v, cache, block_tables, max_pages, seq_lens, batch, num_splits, score_scale,
                                 partial_acc, partial_ml, sm_count, (cudaStream_t)stream);
     default:
-      return launch_decode<128>(cfg, tmap, tmap_q, cache, block_tables, max_pages, seq_lens, batch, num_splits, score_scale,
+      return launch_decode<128>(cfg, tmap, tmap_q, tmap_v, cache, block_tables, max_pages, seq_lens, batch, num_splits, score_scale,
                                 partial_acc, partial_ml, sm_count, (cudaStream_t)stream);
   }
 }
