@@ -295,7 +295,9 @@ class HostStage:
     """A step's inputs laid back to back in ONE pinned host block with a device block of the same layout, so
     that they cross PCIe in a single copy: q bf16 [batch, Hq, d], k_new / v_new bf16 [total_new, Hkv, d],
     cu_new i32 [batch + 1], seq_lens_before / seq_lens_after i32 [batch], block_tables i32 [batch, max_pages].
-    The caller writes the host views (`.h[name]`), `upload()` enqueues the copy, the kernels read `.d[name]`."""
+    The caller writes the host views (`.h[name]`), `upload()` enqueues the copy, the kernels read `.d[name]`.
+    The block tables come last in the block: they change only when a sequence crosses a page boundary (every 16th
+    token), so `upload(tables=False)` leaves them out and the caller sends them with `upload_tables()` when they did."""
 
     FIELDS = ("q", "k_new", "v_new", "cu_new", "seq_lens_before", "seq_lens_after", "block_tables")
 
@@ -317,6 +319,7 @@ class HostStage:
             offs[name] = (total, n)
             total = (total + n + 255) // 256 * 256          # every field 256-byte aligned (the kernels ask for 16)
         self.nbytes = total
+        self.step_nbytes = offs["block_tables"][0]          # everything before the block tables: a step's own inputs
         self.host = torch.empty(total, dtype=torch.uint8)
         if torch.device(device).type == "cuda":
             self.host = self.host.pin_memory()
@@ -326,15 +329,20 @@ class HostStage:
             return {name: block[o:o + n].view(spec[name][1]).view(spec[name][0]) for name, (o, n) in offs.items()}
         self.h, self.d = views(self.host), views(self.dev)
 
-    def upload(self):
-        self.dev.copy_(self.host, non_blocking=True)        # on the current stream
+    def upload(self, tables: bool = True):
+        n = self.nbytes if tables else self.step_nbytes
+        self.dev[:n].copy_(self.host[:n], non_blocking=True)    # on the current stream
+
+    def upload_tables(self):
+        self.dev[self.step_nbytes:].copy_(self.host[self.step_nbytes:], non_blocking=True)
 
 
-def decode_step_host(cfg: UQConfig, bufs: StepBuffers, stage: HostStage, cache, out_host, stream=None) -> torch.Tensor:
+def decode_step_host(cfg: UQConfig, bufs: StepBuffers, stage: HostStage, cache, out_host, stream=None,
+                     tables: bool = True) -> torch.Tensor:
     """The step with HOST (pinned) inputs and output: the step's query, new K/V rows, lengths and block tables
     (stage.h, filled by the caller) are copied host->device in one copy, the attention output device->host.
     The KV cache itself is the resident state and stays in HBM."""
-    stage.upload()
+    stage.upload(tables)
     dv = stage.d
     out = decode_step(cfg, bufs, dv["q"], dv["k_new"], dv["v_new"], dv["cu_new"], dv["seq_lens_before"],
                       dv["seq_lens_after"], dv["block_tables"], cache, stream=stream)
@@ -369,12 +377,14 @@ class HostStepGraph:
     the host one graph launch.  All addresses are those of `stage`, `bufs`, `cache` and `out_host`: the caller
     rewrites `stage.h[...]` between launches.  `launch()` enqueues on the current stream."""
 
-    def __init__(self, cfg: UQConfig, bufs: StepBuffers, stage: HostStage, cache, out_host):
+    def __init__(self, cfg: UQConfig, bufs: StepBuffers, stage: HostStage, cache, out_host, tables: bool = True):
+        """tables=False: the captured step uploads the step's own inputs only; the caller sends the block tables with
+        stage.upload_tables() whenever they change (the constructor sends them once)."""
         decode_step_host(cfg, bufs, stage, cache, out_host)          # first-call set-up happens outside the capture
         torch.cuda.current_stream().synchronize()
         self.graph = torch.cuda.CUDAGraph()
         with torch.cuda.graph(self.graph):                           # torch's capture stream becomes the current one
-            decode_step_host(cfg, bufs, stage, cache, out_host)
+            decode_step_host(cfg, bufs, stage, cache, out_host, tables=tables)
         self.out_host = out_host
 
     def launch(self) -> torch.Tensor:
