@@ -235,7 +235,9 @@ def run_ours(args, rank, world, local_rank):
     dev = torch.device("cuda", local_rank)
     torch.cuda.set_device(dev)
     wl = _workload(args.config, rank)
-    cfg = uq.UQConfig(num_q_heads=wl.num_q_heads, num_kv_heads=wl.num_kv_heads, head_dim=wl.head_dim)
+    # the timed step appends ONE token per sequence right before the decode: the promise of UQ_FLAG_SMALL_APPEND_AHEAD
+    cfg = uq.UQConfig(num_q_heads=wl.num_q_heads, num_kv_heads=wl.num_kv_heads, head_dim=wl.head_dim,
+                      flags=0 if args.no_early else uq.FLAG_SMALL_APPEND_AHEAD)
     B, Hq, Hkv, d = wl.batch, wl.num_q_heads, wl.num_kv_heads, wl.head_dim
 
     # context AFTER the step's append = the config's lengths; the cache holds one token less
@@ -741,6 +743,8 @@ def main():
                     help="instead of the decode step, time bulk quantize-on-append of TOKENS new tokens per call")
     ap.add_argument("--calibrate", type=int, default=0, metavar="VECTORS",
                     help="instead of the decode step, time uq_calibrate_c over VECTORS key vectors and 56 constants")
+    ap.add_argument("--no-early", action="store_true",
+                    help="do not set UQ_FLAG_SMALL_APPEND_AHEAD (the decode kernel then waits for the append before it reads anything)")
     ap.add_argument("--kv", default="fp4", choices=["fp4", "fp8", "bf16"],
                     help="fp4: UltraQuant (default).  fp8 / bf16: the same step over the paper's comparison caches")
     ap.add_argument("--head-dim", type=int, default=128, choices=[64, 128, 256],

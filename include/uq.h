@@ -87,6 +87,16 @@ extern "C" {
  * into a CUDA graph).  On an offender the call returns UQ_ERR_INVALID_ARG, names the first one in uq_last_error_string()
  * and launches nothing else.  Without the flag none of this runs. */
 #define UQ_FLAG_DEBUG_CHECKS 2u
+/* uq_config.flags, read by uq_decode_attention only: a promise about what runs AHEAD of the call in its stream.  The
+ * library's kernels are launched with programmatic stream serialization: a kernel's CTAs may become resident while the
+ * kernel before it still runs and normally wait for it before they touch global memory.  With this flag the caller
+ * guarantees that the work still running ahead (the step's uq_rotate_quantize_append and, before it, the previous step's
+ * merge) writes nothing this call reads except q_fp8, the partial buffers and the LAST TWO pages of each sequence's
+ * block-table range — i.e. the append adds at most 16 tokens per sequence, and seq_lens / block_tables were final before
+ * it started.  The decode kernel then waits only where it could meet those writes (query tiles, tiles holding one of a
+ * sequence's last two pages, every write of partials) and streams the rest of the cache under the append kernel: the
+ * fill of its pipelines leaves the step's critical path.  Results are identical with and without the flag. */
+#define UQ_FLAG_SMALL_APPEND_AHEAD 4u
 
 typedef struct {
   int32_t num_q_heads;   /* e.g. 64 */

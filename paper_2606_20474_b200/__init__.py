@@ -33,6 +33,7 @@ from .binding import (  # noqa: F401
     decode_workspace_bytes,
     FLAG_DEBUG_CHECKS,
     FLAG_NO_BULK_APPEND,
+    FLAG_SMALL_APPEND_AHEAD,
     last_error,
     library_path,
     merge_splits,

@@ -129,6 +129,7 @@ def cache_record_bytes(cfg: UQConfig) -> int:
 
 FLAG_NO_BULK_APPEND = 1
 FLAG_DEBUG_CHECKS = 2
+FLAG_SMALL_APPEND_AHEAD = 4
 
 
 def decode_workspace_bytes(cfg: UQConfig, batch: int, num_splits: int) -> int:

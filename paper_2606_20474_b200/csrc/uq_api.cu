@@ -35,7 +35,7 @@ int32_t check_config(const uq_config* cfg) {
     set_error("uq_config: c_k and c_v must be positive");
     return UQ_ERR_INVALID_ARG;
   }
-  if ((cfg->flags & ~(uint32_t)(UQ_FLAG_NO_BULK_APPEND | UQ_FLAG_DEBUG_CHECKS)) != 0) {
+  if ((cfg->flags & ~(uint32_t)(UQ_FLAG_NO_BULK_APPEND | UQ_FLAG_DEBUG_CHECKS | UQ_FLAG_SMALL_APPEND_AHEAD)) != 0) {
     set_error("uq_config: unknown bit in flags");
     return UQ_ERR_INVALID_ARG;
   }

@@ -148,7 +148,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
               const uint8_t* __restrict__ cache, const int32_t* __restrict__ block_tables, int max_pages,
               const int32_t* __restrict__ seq_lens, int batch, int Hq, int Hkv, int num_splits,
               float score_scale /* sm_scale * log2(e) */, float* __restrict__ partial_acc,
-              float* __restrict__ partial_ml) {
+              float* __restrict__ partial_ml, int early /* UQ_FLAG_SMALL_APPEND_AHEAD */) {
   using Geo = DecodeGeo<D>;
   constexpr int kHalves = Geo::kHalves, kComputeWarps = Geo::kComputeWarps, kThreads = Geo::kThreads;
   constexpr int kRecordBytes = Geo::kRecordBytes, kRestBytes = Geo::kRestBytes, kKStageBytes = Geo::kKStageBytes,
@@ -215,7 +215,12 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
   // Barriers, TMEM and scale constants are set up under the tail of the kernel before this one in the stream;
   // everything below reads global memory it may have written (programmatic dependent launch, uq_common.cuh).
   pdl_launch_dependents();
-  pdl_wait();
+  // UQ_FLAG_SMALL_APPEND_AHEAD (include/uq.h): the caller guarantees that what still runs ahead of this kernel in the
+  // stream writes q_fp8, the partial buffers and at most the last two pages of every sequence — nothing else this
+  // kernel reads.  Then only the accesses that could meet those writes wait for the grid ahead (the Q tiles, a tile
+  // holding one of a sequence's last two pages, every write of partials), and the K / V rings fill — the V warps
+  // convert — under the append kernel: the HBM latency of the first tiles is off the step's critical path.
+  if (!early) pdl_wait();
   // tiles per sequence -> inclusive prefix sums in shared memory (every CTA computes the same schedule)
   for (int b = tid; b < batch; b += kThreads) {
     const int L = seq_lens[b];
@@ -264,6 +269,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     // Per tile: S(gt)[128 tok x 16 heads] = K . Q^T once the tile's bytes have landed, the S buffer was read
     // by the softmax of global tile gt-2.
     const uint32_t idesc_qk = (5u << 7) | (0u << 10) | (2u << 17) | (1u << 23) | (8u << 24);   // E2M1 x E4M3, UE8M0, N=16, M=128
+    if (early) pdl_wait();                             // q_fp8 comes from the kernel ahead
     if (elect_one()) umma_cp_sf(tmem + kColSFB, make_desc(sSFB, 16, 128, 0));
     auto load_q = [&](const Unit& un, int k) {         // lane 0: Q tile of unit ordinal k
       if (elect_one()) {
@@ -386,7 +392,9 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     sc.start(cur);
     Unit un;
     int s = 0, ph = 1;                                 // stage, parity to wait for on empty[s]
+    bool waited = !early;                              // has this warp waited for the grid ahead
     while (sc.next(cur, un)) {
+      const int last_safe = ((un.L + kPage - 1) / kPage) - 2;   // pages from here on may still be written by the append ahead
       const int32_t* bt = block_tables + (long long)un.b * max_pages + un.p0 + pl;
       int page_next = (copier && un.p0 + pl < un.p1) ? bt[0] : 0;
       for (int i = 0; i < un.n_tiles; ++i) {
@@ -394,6 +402,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
         const int npg = min(kTilePages, un.p1 - (un.p0 + kTilePages * i));
         const int nb = un.p0 + kTilePages * (i + 1) + pl;
         page_next = (copier && nb < un.p1) ? bt[kTilePages * (i + 1)] : 0;
+        if (!waited && un.p0 + kTilePages * (i + 1) > last_safe) { pdl_wait(); waited = true; }
         mbar_wait(bar_e + 8 * s, ph);
         if (kGather && !is_k) {
           const int nops = (npg + 3) >> 2;             // pages past the end name record 0: copied, never read
@@ -440,6 +449,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
       // ============================================================== softmax warps
       const int atid = 32 * cw + lane;                 // 0..127
       float2* const ml_out = reinterpret_cast<float2*>(partial_ml);
+      if (early) pdl_wait();                           // the partial buffers may still be read by the merge ahead
 
       // items without any token: all their slots are empty, (m, l) = (-inf, 0)
       for (int it = blockIdx.x; it < batch * Hkv; it += gridDim.x) {
@@ -749,6 +759,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
         // ============================================================== the unit's accumulator
         mbar_wait(bar_done + 8 * ((gt - 1) & 1), ((gt - 1) >> 1) & 1);
         tc_fence_after();
+        if (early) pdl_wait();                         // (returns at once after the first time)
         if (active) {
           float ov[16];
           tmem_ld<16>(t_o, ov);
@@ -890,7 +901,7 @@ int32_t launch_decode(const uq_config* cfg, const CUtensorMap& tmap, const CUten
   return check_cuda(launch_pdl(decode_kernel<D>, grid, dim3(Geo::kThreads), (size_t)Geo::kSmemBytes, stream, tmap, tmap_q, tmap_v,
                                (const uint8_t*)cache, block_tables, (int)max_pages, seq_lens, (int)batch,
                                (int)cfg->num_q_heads, (int)cfg->num_kv_heads, (int)num_splits, score_scale, partial_acc,
-                               partial_ml),
+                               partial_ml, (int)((cfg->flags & UQ_FLAG_SMALL_APPEND_AHEAD) != 0)),
                     "uq_decode_attention launch");
 }
 }  // namespace

@@ -93,7 +93,8 @@ def test_workspace_query_and_debug_flag_on_the_host(lib):
     assert lib.uq_decode_workspace_bytes(ctypes.byref(bad), 1, 1, ctypes.byref(n)) == 2
     ok = uq.UQConfig(64, 4, flags=uq.FLAG_DEBUG_CHECKS | uq.FLAG_NO_BULK_APPEND)
     assert uq.cache_record_bytes(ok) == 2176
-    assert uq.cache_record_bytes(uq.UQConfig(64, 4, flags=4)) == 0
+    assert uq.cache_record_bytes(uq.UQConfig(64, 4, flags=uq.FLAG_SMALL_APPEND_AHEAD)) == 2176
+    assert uq.cache_record_bytes(uq.UQConfig(64, 4, flags=8)) == 0
     assert b"flags" in lib.uq_last_error_string()
 
 

@@ -96,11 +96,13 @@ def test_incremental_appends_match_bulk_and_oracle():
         H.check_out(out[b].float().cpu().numpy().astype(np.float64), ref, f"incr seq {b}")
 
 
-def test_shared_prefix_steps_cfg4_scaled():
+@pytest.mark.parametrize("flags", [0, uq.FLAG_SMALL_APPEND_AHEAD])
+def test_shared_prefix_steps_cfg4_scaled(flags):
     """Config 4 shape at 1/64 scale: shared prefix pages named by every block table, then three
-    timed-style steps (append 1 token per sequence, decode, merge)."""
+    timed-style steps (append 1 token per sequence, decode, merge) — also with UQ_FLAG_SMALL_APPEND_AHEAD, under which
+    the decode kernel streams every page but a sequence's last two before the append ahead of it has finished."""
     wl = W.make_config(4, scale=1 / 64, peaked_frac=0.05)
-    cfg = H.cfg_of(wl)
+    cfg = H.cfg_of(wl, flags=flags)
     cache, bt = H.fill_cache(cfg, wl, DEV)
     S = 3
     bufs = uq.StepBuffers(cfg, wl.batch, S, DEV)
@@ -383,12 +385,13 @@ def test_host_staged_step_equals_device_step_and_oracle():
         H.check_out(out_host[b].float().numpy().astype(np.float64), ref, f"staged seq {b}")
 
 
-def test_step_graph_equals_direct_calls():
+@pytest.mark.parametrize("flags", [0, uq.FLAG_SMALL_APPEND_AHEAD])
+def test_step_graph_equals_direct_calls(flags):
     """uq.StepGraph (decode_step captured as a CUDA graph, inputs rewritten in place between launches) gives the
     direct calls' output bit for bit over consecutive steps, and the same cache image."""
     steps = 3
     wl = W.make_custom("sgraph", 23, [130, 31, 64, 1000], 16, 2, extra_tokens=steps)
-    cfg = H.cfg_of(wl)
+    cfg = H.cfg_of(wl, flags=flags)
     B = wl.batch
     lens0 = (wl.ctx_lens - steps).astype(np.int32)
     (cache_a, bt), (cache_b, _) = H.fill_cache(cfg, wl, DEV, lens=lens0), H.fill_cache(cfg, wl, DEV, lens=lens0)
