@@ -288,6 +288,34 @@ int32_t uq_baseline_decode_attention(const uq_config* cfg, int32_t kv_format, co
                                      const int32_t* seq_lens, int32_t batch, int32_t num_splits,
                                      float* partial_acc, float* partial_ml, void* stream);
 
+/*
+ * Decode without allocation: uq_decode_attention followed by uq_merge_splits with the split partials held in a static
+ * device array inside libuq.so instead of caller buffers — for callers that cannot call cudaMalloc (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid it).  The call itself allocates nothing either: no
+ * cudaMalloc / cudaFree, no allocating library routine.
+ *
+ *  UQ_STATIC_SCRATCH_BYTES   size of that array: every GPU that loads the library holds this much until the process
+ *                            exits.  A call needs  round_up(batch * num_q_heads * num_splits * head_dim * 4, 256)
+ *                            + batch * num_q_heads * num_splits * 8  bytes (uq_decode_static_scratch_needed); config 2
+ *                            (32 x 64 heads, head_dim 128) needs 1.02 MiB per split.  A call that needs more returns
+ *                            UQ_ERR_UNSUPPORTED with the sizes in uq_last_error_string() and launches nothing.
+ *  q_fp8, cache, num_pages, block_tables, max_pages, seq_lens, batch, num_splits, stream: as uq_decode_attention.
+ *  out_bf16                  bf16 [batch, num_q_heads, head_dim], as uq_merge_splits.
+ *
+ * Result: identical to uq_decode_attention + uq_merge_splits with the same num_splits (the same kernels run).
+ * The array is shared by EVERY call on a device and keeps the last call's contents.  Nothing in it has to start at
+ * zero (the decode kernel writes (m, l) of every slot on every call and the merge reads an acc row only where l != 0),
+ * so no clear is issued.  Calls that may overlap on the GPU — two streams, two threads, two graphs replayed
+ * concurrently — RACE on it: serialise them on one stream or with events.  Each device has its own copy; the address
+ * is looked up once per device (cudaGetSymbolAddress, with that device current) on the first call there.
+ */
+#define UQ_STATIC_SCRATCH_BYTES (32u << 20)
+size_t uq_static_scratch_bytes(void);
+int32_t uq_decode_static_scratch_needed(const uq_config* cfg, int32_t batch, int32_t num_splits, size_t* bytes);
+int32_t uq_decode_attention_static(const uq_config* cfg, const void* q_fp8, const void* cache, int64_t num_pages,
+                                   const int32_t* block_tables, int32_t max_pages, const int32_t* seq_lens,
+                                   int32_t batch, int32_t num_splits, void* out_bf16, void* stream);
+
 /* Host.  A num_splits (slot count) that lets uq_decode_attention balance `batch` sequences of about
  * `avg_seq_len` tokens over the current device with room for sequences twice that long (never below 1). */
 int32_t uq_suggest_num_splits(const uq_config* cfg, int32_t batch, int32_t avg_seq_len);

@@ -28,6 +28,9 @@ from .binding import (  # noqa: F401
     PrefixBuffers,
     decode_attention,
     decode_attention_shared_prefix,
+    decode_attention_static,
+    decode_static_scratch_needed,
+    static_scratch_bytes,
     decode_step,
     decode_step_host,
     decode_workspace_bytes,

@@ -86,6 +86,12 @@ def _load():
     lib.uq_baseline_append.argtypes = [cfgp, i32, vp, vp, vp, vp, vp, i32, i32, i32, vp, i64, vp, vp, vp]
     lib.uq_baseline_decode_attention.restype = i32
     lib.uq_baseline_decode_attention.argtypes = [cfgp, i32, vp, vp, i64, vp, i32, vp, i32, i32, vp, vp, vp]
+    lib.uq_static_scratch_bytes.restype = ctypes.c_size_t
+    lib.uq_static_scratch_bytes.argtypes = []
+    lib.uq_decode_static_scratch_needed.restype = i32
+    lib.uq_decode_static_scratch_needed.argtypes = [cfgp, i32, i32, ctypes.POINTER(ctypes.c_size_t)]
+    lib.uq_decode_attention_static.restype = i32
+    lib.uq_decode_attention_static.argtypes = [cfgp, vp, vp, i64, vp, i32, vp, i32, i32, vp, vp]
     lib.uq_suggest_num_splits.restype = i32
     lib.uq_suggest_num_splits.argtypes = [cfgp, i32, i32]
     lib.uq_suggest_prefix_splits.restype = i32
@@ -225,6 +231,35 @@ def merge_splits(cfg: UQConfig, partial_acc, partial_ml, out, stream=None) -> No
     st = lib.uq_merge_splits(ctypes.byref(c), _p(partial_acc), _p(partial_ml), out.shape[0],
                              partial_ml.shape[2], _p(out), _stream(stream))
     _check(st, "uq_merge_splits")
+
+
+def static_scratch_bytes() -> int:
+    """uq_static_scratch_bytes: size of the library's static split-partial array (UQ_STATIC_SCRATCH_BYTES)."""
+    return int(_load().uq_static_scratch_bytes())
+
+
+def decode_static_scratch_needed(cfg: UQConfig, batch: int, num_splits: int) -> int:
+    """uq_decode_static_scratch_needed: bytes of that array a uq_decode_attention_static call of this shape uses."""
+    lib = _load()
+    n = ctypes.c_size_t(0)
+    c = cfg.c()
+    _check(lib.uq_decode_static_scratch_needed(ctypes.byref(c), int(batch), int(num_splits), ctypes.byref(n)),
+           "uq_decode_static_scratch_needed")
+    return int(n.value)
+
+
+def decode_attention_static(cfg: UQConfig, q_fp8, cache, block_tables, seq_lens, num_splits: int, out, stream=None) -> None:
+    """uq_decode_attention_static: decode + merge with the split partials in the library's static device array — the
+    call allocates nothing.  out bf16 [batch, Hq, d].  Calls that overlap on the GPU race on that array."""
+    lib = _load()
+    _dev(q_fp8, torch.uint8, "q_fp8"); _dev(cache, torch.uint8, "cache")
+    _dev(block_tables, torch.int32, "block_tables"); _dev(seq_lens, torch.int32, "seq_lens")
+    _dev(out, torch.bfloat16, "out")
+    c = cfg.c()
+    st = lib.uq_decode_attention_static(ctypes.byref(c), _p(q_fp8), _p(cache), cache.shape[0], _p(block_tables),
+                                        block_tables.shape[1], _p(seq_lens), seq_lens.shape[0], int(num_splits),
+                                        _p(out), _stream(stream))
+    _check(st, "uq_decode_attention_static")
 
 
 class PrefixBuffers:
