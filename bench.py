@@ -360,6 +360,21 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     sampler.busy = False
     dec_ms = [a.elapsed_time(b) for a, b in dec_ev]
+    # --shared-prefix 1: the two decode kernels of the step timed one by one as well (events between the launches)
+    sp_kernels = None
+    if pbufs is not None:
+        n_sp = min(n_inst, 20)
+        ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(n_sp)]
+        for i in range(n_sp):
+            k_new, v_new = kvs[i % n_in]
+            uq.rotate_quantize_append(cfg, k_new, v_new, cu_dev, before_dev, bt_dev, cache, q=qs[i % n_in],
+                                      q_fp8=bufs_sp.q_fp8, stream=stream)
+            uq.decode_attention_shared_prefix(cfg, bufs_sp, pbufs, cache, bt_dev, pfx, stream=stream,
+                                              mark=lambda j, e=ev[i]: e[j].record(stream))
+        barrier()
+        sp_kernels = {"prefix_kernel_us": round(statistics.fmean(e[0].elapsed_time(e[1]) for e in ev) * 1e3, 2),
+                      "suffix_kernel_us": round(statistics.fmean(e[1].elapsed_time(e[2]) for e in ev) * 1e3, 2),
+                      "launches": n_sp}
 
     # ---- sustained: back-to-back steps for at least --sustain seconds between two events (north_star: "sustaining
     # >= 70 % of B200 HBM peak"), with its own clock record — a 2 ms burst runs at boost clock, seconds of
@@ -451,6 +466,7 @@ def run_ours(args, rank, world, local_rank):
         "decode_kernel_us": round(dec_ms_mean * 1e3, 2),
         "decode_kernel_us_spread": {"median": round(dec_ms_med * 1e3, 2), "min": round(dec_ms_min * 1e3, 2), "launches": n_inst},
         "bytes_per_step": total_b,
+        **({"shared_prefix_kernels": sp_kernels} if sp_kernels else {}),
         **({"shared_prefix": {
             "note": "bytes_per_step / value / roofline count LOGICAL bytes; the prefix pages are named by every block "
                     "table and read from HBM once per step (L2 serves the rest), so the fractions of the HBM peak can "

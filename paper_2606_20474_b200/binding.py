@@ -275,25 +275,32 @@ class PrefixBuffers:
 
 
 def decode_attention_shared_prefix(cfg: UQConfig, bufs: "StepBuffers", pbufs: PrefixBuffers, cache, block_tables,
-                                   prefix_len: int, stream=None) -> torch.Tensor:
+                                   prefix_len: int, stream=None, mark=None) -> torch.Tensor:
     """Decode + merge for sequences that share their first prefix_len tokens (a multiple of 128; same pages in every
     block table): uq_decode_prefix_attention over the prefix, uq_decode_attention over the private suffixes
     (pbufs.suffix_lens, the block tables from page prefix_len / page_size on), uq_merge_splits2.  bufs.q_fp8 holds
-    the encoded queries.  Returns bufs.out."""
+    the encoded queries.  Returns bufs.out.  mark (timing only): called with 0, 1, 2 before the prefix call, between
+    the two decode calls and after the suffix call (bench.py records an event each time)."""
     lib = _load()
     _dev(cache, torch.uint8, "cache"); _dev(block_tables, torch.int32, "block_tables")
     c = cfg.c()
     batch, max_pages = block_tables.shape
     pp = prefix_len // cfg.page_size
+    if mark is not None:
+        mark(0)
     st = lib.uq_decode_prefix_attention(ctypes.byref(c), _p(bufs.q_fp8), _p(cache), cache.shape[0], _p(block_tables),
                                         max_pages, batch, int(prefix_len), pbufs.prefix_splits, _p(pbufs.partial_acc),
                                         _p(pbufs.partial_ml), _stream(stream))
     _check(st, "uq_decode_prefix_attention")
+    if mark is not None:
+        mark(1)
     bt_suffix = ctypes.c_void_p(block_tables.data_ptr() + 4 * pp)      # row stride stays max_pages
     st = lib.uq_decode_attention(ctypes.byref(c), _p(bufs.q_fp8), _p(cache), cache.shape[0], bt_suffix, max_pages,
                                  _p(pbufs.suffix_lens), batch, bufs.num_splits, _p(bufs.partial_acc),
                                  _p(bufs.partial_ml), _stream(stream))
     _check(st, "uq_decode_attention (suffix)")
+    if mark is not None:
+        mark(2)
     st = lib.uq_merge_splits2(ctypes.byref(c), _p(pbufs.partial_acc), _p(pbufs.partial_ml), pbufs.prefix_splits,
                               _p(bufs.partial_acc), _p(bufs.partial_ml), bufs.num_splits, batch, _p(bufs.out),
                               _stream(stream))

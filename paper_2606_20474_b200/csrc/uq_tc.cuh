@@ -29,6 +29,20 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
 // Measured and dropped on config 2: test_wait spin loops (157-161 us: the spin steals issue slots from the working
 // warps), nanosleep polling and suspend-time hints in the softmax warps (no change).
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+#ifdef UQ_WATCHDOG
+  // debug builds (-DUQ_WATCHDOG): a wait that does not end names itself and traps instead of hanging the GPU
+  for (uint32_t spins = 0;; ++spins) {
+    uint32_t ok;
+    asm volatile("{\n.reg .pred p;\nmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    if (ok) return;
+    if (spins == (1u << 20)) {
+      printf("uq watchdog: block %d warp %d lane %d waits on mbarrier at shared 0x%x parity %u\n", (int)blockIdx.x,
+             (int)(threadIdx.x >> 5), (int)(threadIdx.x & 31), bar, parity);
+      __trap();
+    }
+  }
+#endif
   asm volatile(
       "{\n"
       ".reg .pred p;\n"
