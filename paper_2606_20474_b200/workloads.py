@@ -22,6 +22,13 @@ import torch
 CHUNK = 4096          # tokens per generator chunk (fixed so every caller sees the same values)
 PAGE = 16
 
+# Input of the Ultra-TQ comparison path (Alg. 2 "Require: codebook C_K"): a 16-level codebook for the
+# coordinates of a 32-channel block scaled to unit l2 norm — the textbook 16-level Lloyd-Max levels of N(0, 1)
+# divided by sqrt(32).  The paper's own codebook is calibrated on captured activations (out of scope): this table is
+# data handed to both the CUDA path and the oracle, like every other input.
+_LM16 = (0.1284, 0.3881, 0.6568, 0.9424, 1.256, 1.618, 2.069, 2.733)
+TQ_CODEBOOK = tuple([-v / 32 ** 0.5 for v in reversed(_LM16)] + [v / 32 ** 0.5 for v in _LM16])
+
 
 @dataclasses.dataclass
 class Workload:

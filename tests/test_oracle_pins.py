@@ -598,3 +598,109 @@ def test_p14_fp8_kv_cast_and_attention_are_the_pinned_parts():
     out16 = oracle.attention_bf16kv(qb, kb, vb)
     assert np.allclose(out16, sdpa(q.double(), k.double(), v.double()), atol=1e-12)
     assert not np.allclose(out8, out16, atol=1e-3)                  # the two caches really differ
+
+
+# ----------------------------------------------------------------------------- P15-P17 Ultra-TQ (Alg. 2)
+def _bf16_bits_of(x):
+    return torch.from_numpy(np.asarray(x, np.float32)).to(torch.bfloat16).view(torch.uint16).numpy()
+
+
+def test_p15_bf16_rne_is_the_library_rounding():
+    """`ultra_tq.bf16_rne` (written from the definition: quantum 2^(e-7), ties to even) == the library cast float32 ->
+    bfloat16 on random magnitudes, on exact ties (odd / even neighbours) and at binade boundaries."""
+    from oracle import ultra_tq as T
+    rng = np.random.default_rng(15)
+    x = (rng.standard_normal(200000) * np.exp(rng.uniform(-30, 30, 200000))).astype(np.float32)
+    ties = np.array([1.0 + 2.0 ** -8, 1.0 + 3 * 2.0 ** -8, 1.0 + 2.0 ** -8 + 2.0 ** -20, 2.0 - 2.0 ** -8, 255.5, 256.5, -1.00390625,
+                     0.0, 3.0e-5, 65504.0], np.float32)
+    x = np.concatenate([x, ties, -ties])
+    want = torch.from_numpy(x).to(torch.bfloat16).double().numpy()
+    assert np.array_equal(T.bf16_rne(x.astype(np.float64)), want)
+    assert T.bf16_rne(np.array([1.0 + 2.0 ** -8]))[0] == 1.0 and T.bf16_rne(np.array([1.0 + 3 * 2.0 ** -8]))[0] == 1.0 + 2.0 ** -6
+    assert np.array_equal(T.bf16_bits(want), torch.from_numpy(x).to(torch.bfloat16).view(torch.uint16).numpy())
+
+
+def test_p16_ultra_tq_encoders_closed_forms_and_brute_force():
+    """Alg. 2 l.1-4.  K: a one-hot key a e_0 rotates to a/sqrt(d) (+-1 pattern of Hadamard row 0 = all +): every block has
+    norm a sqrt(32/d) and every coordinate u = 1/sqrt(32) -> the codebook entry nearest to 0.17678 (index 11 of the
+    input table), a e_1 alternates signs (indices 11, 4); the index is the brute-force nearest entry (python floats) and
+    the stored norm the bf16 of the plain l2 norm; reconstruction error of Gaussian keys is that of a 16-level
+    Lloyd-Max quantiser (relative MSE 0.0095 +- 15 %).  V: a block zero + scale * (codes) with bf16 scale / zero comes back
+    exactly; a constant block has scale 0, codes 0 and decodes exactly; |v - vhat| <= scale/2 + one bf16 rounding."""
+    from oracle import ultra_tq as T
+    from paper_2606_20474_b200 import workloads as W
+    cb = np.asarray(W.TQ_CODEBOOK, np.float32)
+    assert np.all(np.diff(cb) > 0) and np.allclose(cb, -cb[::-1])
+    d = 128
+    for j, want in ((0, [11] * 4), (1, [11, 4] * 2)):
+        k = np.zeros((1, d), np.float32); k[0, j] = 3.0
+        idx, norm = T.encode_k(_bf16_bits_of(k), cb)
+        assert np.array_equal(norm[0], T.bf16_rne(np.full(4, 3.0 * np.sqrt(32.0 / d))))
+        assert list(idx[0, :4]) == want and set(idx[0]) <= {4, 11}
+    rng = np.random.default_rng(16)
+    kb = _bf16_bits_of(rng.standard_normal((64, d)) * np.exp(rng.uniform(-3, 3, (64, 1))))
+    idx, norm = T.encode_k(kb, cb)
+    x = np.stack([oracle.hadamard(r) for r in oracle.bf16_to_double(kb)])
+    for r in range(0, 64, 7):                                  # brute force, scalar python arithmetic
+        for g in range(4):
+            blk = [float(v) for v in x[r, 32 * g:32 * g + 32]]
+            n2 = 0.0
+            for v in blk:
+                n2 = n2 + v * v
+            ns = float(T.bf16_rne(np.array([n2 ** 0.5]))[0])
+            assert ns == norm[r, g]
+            for c in range(32):
+                u = blk[c] / ns
+                best = min(range(16), key=lambda i: (abs(u - float(cb[i])), i))
+                assert best == idx[r, 32 * g + c]
+    kh = T.dequant_k(idx, norm, cb)
+    rel = float(((kh - x) ** 2).sum() / (x ** 2).sum())
+    assert 0.0080 < rel < 0.0110, rel                          # 16-level Lloyd-Max of a Gaussian: 0.0095
+    # V
+    scale, zero = 0.375, -2.5                                  # bf16 values
+    codes = rng.integers(0, 16, (5, d)); codes[:, ::32] = 0; codes[:, 1::32] = 15
+    v = zero + scale * codes                                   # exact in bf16 (<= 8 significant bits)
+    code, sc, ze = T.encode_v(_bf16_bits_of(v))
+    assert np.array_equal(code, codes) and np.all(sc == scale) and np.all(ze == zero)
+    assert np.array_equal(T.dequant_v(code, sc, ze), v)
+    const = np.full((2, d), 1.75)
+    code, sc, ze = T.encode_v(_bf16_bits_of(const))
+    assert not code.any() and not sc.any() and np.array_equal(T.dequant_v(code, sc, ze), const)
+    vb = _bf16_bits_of(rng.standard_normal((64, d)) * 3)
+    code, sc, ze = T.encode_v(vb)
+    v = oracle.bf16_to_double(vb)
+    vh = T.dequant_v(code, sc, ze)
+    bound = np.repeat(sc, 32, axis=1) * 0.5 * (1 + 2.0 ** -6) + np.abs(v) * 2.0 ** -8 + 16 * np.repeat(sc, 32, axis=1) * 2.0 ** -8
+    assert np.all(np.abs(v - vh) <= bound)
+    assert code.min() == 0 and code.max() == 15
+
+
+def test_p17_ultra_tq_attention_special_cases_and_sdpa():
+    """Alg. 2 l.5-8: one token -> the output is the dequantised value row of the head's kv head; every key equal -> the mean
+    of the value rows; in general == float64 torch SDPA over (bf16(R q), dequant_k, dequant_v)."""
+    from oracle import ultra_tq as T
+    from paper_2606_20474_b200 import workloads as W
+    cb = np.asarray(W.TQ_CODEBOOK, np.float32)
+    rng = np.random.default_rng(17)
+    Hq, Hkv, d, L = 8, 2, 128, 45
+    G = Hq // Hkv
+    qb = _bf16_bits_of(rng.standard_normal((Hq, d)))
+    kb = _bf16_bits_of(rng.standard_normal((L, Hkv, d)) * 2)
+    vb = _bf16_bits_of(rng.standard_normal((L, Hkv, d)))
+    ki, kn = T.encode_k(kb.reshape(L * Hkv, d), cb)
+    vc, vs, vz = T.encode_v(vb.reshape(L * Hkv, d))
+    sh = lambda a: a.reshape(L, Hkv, -1)
+    out = T.attention(qb, sh(ki), sh(kn), sh(vc), sh(vs), sh(vz), cb, Hkv)
+    q = torch.from_numpy(T.encode_q(qb))
+    k = torch.from_numpy(T.dequant_k(ki, kn, cb).reshape(L, Hkv, d))
+    v = torch.from_numpy(T.dequant_v(vc, vs, vz).reshape(L, Hkv, d))
+    ref = torch.nn.functional.scaled_dot_product_attention(
+        q.view(Hkv, G, d), k.permute(1, 0, 2), v.permute(1, 0, 2)).reshape(Hq, d).numpy()
+    assert np.abs(out - ref).max() < 1e-12
+    one = T.attention(qb, sh(ki)[:1], sh(kn)[:1], sh(vc)[:1], sh(vs)[:1], sh(vz)[:1], cb, Hkv)
+    assert np.array_equal(one, np.repeat(v[0].numpy(), G, axis=0))
+    same = lambda a: np.repeat(sh(a)[:1], L, axis=0)
+    eq = T.attention(qb, same(ki), same(kn), sh(vc), sh(vs), sh(vz), cb, Hkv)
+    assert np.abs(eq - np.repeat(v.numpy().mean(axis=0), G, axis=0)).max() < 1e-12
+    # the rotation is the pinned one (P1 / P12) and the query is rounded to bf16 once
+    assert np.array_equal(T.encode_q(qb)[3], T.bf16_rne(oracle.hadamard(oracle.bf16_to_double(qb[3]))))
