@@ -289,6 +289,36 @@ int32_t uq_baseline_decode_attention(const uq_config* cfg, int32_t kv_format, co
                                      float* partial_acc, float* partial_ml, void* stream);
 
 /*
+ * ULTRA-TQ (the paper's Algorithm 2, "Calibrated LUT int4 KV encoding") — the codebook path that
+ * UltraQuant replaces, as the third comparison cache (last item): rotated keys as 4-bit indices
+ * into a 16-entry codebook C_K with a bf16 l2 norm per 32-channel block; values as 4-bit uniform codes with a bf16
+ * (scale, zero) per block; dequantisation on read.  Readings of what Algorithm 2 leaves open: DESIGN.md G20.
+ *   codebook_k   HOST float32 [16], finite, ascending: the algorithm's input C_K (for block coordinates scaled to unit
+ *                l2 norm; calibrating it is out of scope).  Passed by value into the kernels.
+ * Record of (page, kv head), 2432 bytes (uq_baseline_record_bytes(cfg, UQ_KV_ULTRA_TQ)), cache base 16-byte aligned:
+ *   [0, 1024)      K indices: token slot t at 64 t, byte j = channels 2j (bits 0-3), 2j + 1 (bits 4-7)
+ *   [1024, 1152)   K block norms: bf16, token t block g at 1024 + 8 t + 2 g
+ *   [1152, 2176)   V codes: channel c at 1152 + 8 c, 32-bit word t >> 3; inside an octet token 2n in nibble n, token
+ *                  2n + 1 in nibble n + 4
+ *   [2176, 2432)   V block g at 2176 + 64 g: bf16 scale of tokens 0..15, then bf16 zero of tokens 0..15
+ * uq_tq_append: Alg. 2 l.1-4 for the new rows (arguments as uq_rotate_quantize_append) and l.5 for the query: q bf16
+ * [batch, Hq, 128] -> q_rot bf16 [batch, Hq, 128] = bf16(R q) (both NULL or both given).  Every decision in float64:
+ * the cache image and q_rot are bit-exact against the oracle.  head_dim 128 only.
+ * uq_tq_decode_attention: Alg. 2 l.6-8, partial format / schedule / num_splits of uq_decode_attention, uq_merge_splits
+ * finishes.  K = bf16(bf16(C_K[idx]) * norm) through a 256-entry table in shared memory (a load per code byte), V =
+ * bf16(scale * code + zero) with one rounding; both products bf16 x bf16 with fp32 accumulation, P as bf16 (as the BF16
+ * comparison cache).
+ */
+#define UQ_KV_ULTRA_TQ 3
+int32_t uq_tq_append(const uq_config* cfg, const float* codebook_k, const void* k_new, const void* v_new,
+                     const int32_t* cu_new, const int32_t* seq_lens, const int32_t* block_tables, int32_t max_pages,
+                     int32_t batch, int32_t total_new, void* cache, int64_t num_pages, const void* q, void* q_rot,
+                     void* stream);
+int32_t uq_tq_decode_attention(const uq_config* cfg, const float* codebook_k, const void* q_rot, const void* cache,
+                               int64_t num_pages, const int32_t* block_tables, int32_t max_pages, const int32_t* seq_lens,
+                               int32_t batch, int32_t num_splits, float* partial_acc, float* partial_ml, void* stream);
+
+/*
  * Decode without allocation: uq_decode_attention followed by uq_merge_splits with the split partials held in a static
  * device array inside libuq.so instead of caller buffers — for callers that cannot call cudaMalloc (code under CUDA
  * graph capture, tight serving loops, harnesses that forbid it).  The call itself allocates nothing either: no

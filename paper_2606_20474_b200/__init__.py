@@ -23,6 +23,9 @@ from .binding import (  # noqa: F401
     baseline_record_bytes,
     KV_BF16,
     KV_FP8_E4M3,
+    KV_ULTRA_TQ,
+    tq_append,
+    tq_decode_attention,
     cache_record_bytes,
     calibrate_c,
     PrefixBuffers,

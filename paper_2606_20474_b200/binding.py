@@ -86,6 +86,10 @@ def _load():
     lib.uq_baseline_append.argtypes = [cfgp, i32, vp, vp, vp, vp, vp, i32, i32, i32, vp, i64, vp, vp, vp]
     lib.uq_baseline_decode_attention.restype = i32
     lib.uq_baseline_decode_attention.argtypes = [cfgp, i32, vp, vp, i64, vp, i32, vp, i32, i32, vp, vp, vp]
+    lib.uq_tq_append.restype = i32
+    lib.uq_tq_append.argtypes = [cfgp, vp, vp, vp, vp, vp, vp, i32, i32, i32, vp, i64, vp, vp, vp]
+    lib.uq_tq_decode_attention.restype = i32
+    lib.uq_tq_decode_attention.argtypes = [cfgp, vp, vp, vp, i64, vp, i32, vp, i32, i32, vp, vp, vp]
     lib.uq_static_scratch_bytes.restype = ctypes.c_size_t
     lib.uq_static_scratch_bytes.argtypes = []
     lib.uq_decode_static_scratch_needed.restype = i32
@@ -438,6 +442,44 @@ class HostStepGraph:
 # ----------------------------------------------------------------------------- comparison caches (include/uq.h)
 KV_FP8_E4M3 = 1
 KV_BF16 = 2
+KV_ULTRA_TQ = 3
+
+
+def _codebook(codebook):
+    cb = (ctypes.c_float * 16)(*[float(v) for v in codebook])
+    return cb
+
+
+def tq_append(cfg: UQConfig, codebook, k_new, v_new, cu_new, seq_lens, block_tables, cache, q=None, q_rot=None, stream=None) -> None:
+    """uq_tq_append (Alg. 2 l.1-5): new rows into the Ultra-TQ cache (alloc_baseline_cache(cfg, KV_ULTRA_TQ, ...)); q bf16
+    -> q_rot bf16 = bf16(R q).  codebook: 16 ascending floats (host)."""
+    lib = _load()
+    _dev(k_new, torch.bfloat16, "k_new"); _dev(v_new, torch.bfloat16, "v_new")
+    _dev(cu_new, torch.int32, "cu_new"); _dev(seq_lens, torch.int32, "seq_lens")
+    _dev(block_tables, torch.int32, "block_tables"); _dev(cache, torch.uint8, "cache")
+    if q is not None:
+        _dev(q, torch.bfloat16, "q"); _dev(q_rot, torch.bfloat16, "q_rot")
+    c = cfg.c()
+    cb = _codebook(codebook)
+    st = lib.uq_tq_append(ctypes.byref(c), ctypes.cast(cb, ctypes.c_void_p), _p(k_new), _p(v_new), _p(cu_new), _p(seq_lens),
+                          _p(block_tables), block_tables.shape[1], seq_lens.shape[0], k_new.shape[0], _p(cache),
+                          cache.shape[0], _p(q), _p(q_rot), _stream(stream))
+    _check(st, "uq_tq_append")
+
+
+def tq_decode_attention(cfg: UQConfig, codebook, q_rot, cache, block_tables, seq_lens, num_splits: int, partial_acc,
+                        partial_ml, stream=None) -> None:
+    """uq_tq_decode_attention (Alg. 2 l.6-8): split-K partials over the Ultra-TQ cache; merge_splits finishes."""
+    lib = _load()
+    _dev(q_rot, torch.bfloat16, "q_rot"); _dev(cache, torch.uint8, "cache")
+    _dev(block_tables, torch.int32, "block_tables"); _dev(seq_lens, torch.int32, "seq_lens")
+    _dev(partial_acc, torch.float32, "partial_acc"); _dev(partial_ml, torch.float32, "partial_ml")
+    c = cfg.c()
+    cb = _codebook(codebook)
+    st = lib.uq_tq_decode_attention(ctypes.byref(c), ctypes.cast(cb, ctypes.c_void_p), _p(q_rot), _p(cache), cache.shape[0],
+                                    _p(block_tables), block_tables.shape[1], _p(seq_lens), seq_lens.shape[0], int(num_splits),
+                                    _p(partial_acc), _p(partial_ml), _stream(stream))
+    _check(st, "uq_tq_decode_attention")
 
 
 def baseline_record_bytes(cfg: UQConfig, kv_format: int) -> int:

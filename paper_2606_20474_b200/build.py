@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libuq.so")
-SOURCES = ["uq_api.cu", "uq_append.cu", "uq_calib.cu", "uq_debug.cu", "uq_decode.cu", "uq_decode_cmp.cu", "uq_decode_prefix.cu", "uq_decode_prefix_m.cu", "uq_decode_static.cu", "uq_merge.cu"]
+SOURCES = ["uq_api.cu", "uq_append.cu", "uq_calib.cu", "uq_debug.cu", "uq_decode.cu", "uq_decode_cmp.cu", "uq_decode_prefix.cu", "uq_decode_prefix_m.cu", "uq_decode_static.cu", "uq_merge.cu", "uq_tq_append.cu"]
 PTXAS_FLAGS = {"uq_decode.cu": ["-Xptxas", "-O1"], "uq_decode_cmp.cu": ["-Xptxas", "-O1"], "uq_decode_prefix_m.cu": ["-Xptxas", "-O3"], "uq_merge.cu": ["-Xptxas", "-O1"]}
 
 

@@ -11,6 +11,7 @@
 //         B; it is also what BF16 attention kernels do); the query is the bf16 query itself.
 // Readings: DESIGN.md G19.  head_dim 128 only.  CUDA path only; the oracle shares nothing with this file.
 #include <cuda.h>
+#include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
 #include <type_traits>
@@ -23,25 +24,37 @@ namespace {
 
 constexpr int kSoftmaxWarps = 4, kVWarps = 4, kIssuerWarps = 4;
 constexpr int kComputeWarps = kSoftmaxWarps + kVWarps;
-constexpr int kThreads = (kComputeWarps + kIssuerWarps) * 32;
+constexpr int kTqRecord = 2432;                      // Ultra-TQ record: K codes 1024 | K norms 128 | V codes 1024 | V scale / zero 256
+constexpr int kTqVCodes = 1152, kTqVMeta = 2176;
+
+struct TqCodebook {                                  // Alg. 2 "Require: codebook C_K": 16 levels, by value
+  float c[16];
+};
 constexpr int kPBytes = 4096;                        // one P operand buffer (as uq_decode.cu)
 constexpr float kThresh = 12.0f;
 constexpr int kMaxBatch = 2048;
 
-template <int KV>                                    // UQ_KV_FP8_E4M3 = 1, UQ_KV_BF16 = 2
+template <int KV>                                    // UQ_KV_FP8_E4M3 = 1, UQ_KV_BF16 = 2, UQ_KV_ULTRA_TQ = 3
 struct CmpGeo {
-  static_assert(KV == UQ_KV_FP8_E4M3 || KV == UQ_KV_BF16, "comparison cache format");
-  static constexpr int kElem = KV == UQ_KV_BF16 ? 2 : 1;            // bytes per element
-  static constexpr int kKPage = 16 * 128 * kElem;                   // K rows of a page: 2048 / 4096
-  static constexpr int kVPage = kKPage;                             // V [channel][16 tokens]
-  static constexpr int kRecordBytes = kKPage + kVPage;              // 4096 / 8192
+  static_assert(KV == UQ_KV_FP8_E4M3 || KV == UQ_KV_BF16 || KV == UQ_KV_ULTRA_TQ, "comparison cache format");
+  // Ultra-TQ (Alg. 2): the records arrive as they are (the "V" ring holds whole records), four more warps decode the K
+  // codes through the codebook into the bf16 K operand buffers (the "K" ring), everything behind that is the BF16 path
+  static constexpr bool kTq = KV == UQ_KV_ULTRA_TQ;
+  static constexpr bool kBf16 = KV == UQ_KV_BF16 || kTq;            // operands of the two products are bf16
+  static constexpr int kElem = kBf16 ? 2 : 1;                       // bytes per operand element
+  static constexpr int kKPage = 16 * 128 * kElem;                   // K rows of a page in the operand: 2048 / 4096
+  static constexpr int kVPage = kTq ? kTqRecord : kKPage;           // bytes a page puts into the V ring
+  static constexpr int kVSrc = kTq ? 0 : kKPage;                    // ... from this offset of its record
+  static constexpr int kRecordBytes = kTq ? kTqRecord : 2 * kKPage; // 4096 / 8192 / 2432
+  static constexpr int kDequantWarps = kTq ? 4 : 0;
+  static constexpr int kThreads = (kComputeWarps + kIssuerWarps + kDequantWarps) * 32;
   static constexpr int kBlocks = kElem;                             // 128-byte-wide swizzled blocks of a K row
   static constexpr int kKBlockBytes = 128 * 128;                    // [128 tokens][128 B]
   static constexpr int kKStageBytes = kBlocks * kKBlockBytes;       // 16384 / 32768
   static constexpr int kVStageBytes = kTilePages * kVPage;          // 16384 / 32768
   static constexpr int kKStages = KV == UQ_KV_BF16 ? 3 : 2;
   static constexpr int kVStages = 3;
-  static constexpr int kCtasPerSm = KV == UQ_KV_BF16 ? 1 : 2;
+  static constexpr int kCtasPerSm = kBf16 ? 1 : 2;
   static constexpr int kQBlockBytes = 16 * 128;                     // [16 heads][128 B]
   static constexpr int kQBytes = kBlocks * kQBlockBytes;
   static constexpr int kQKMmas = 4 * kElem;                         // 32 bytes of a row per instruction
@@ -49,7 +62,8 @@ struct CmpGeo {
   static constexpr int kOffV = kOffK + kKStages * kKStageBytes;
   static constexpr int kOffQ = kOffV + kVStages * kVStageBytes;
   static constexpr int kOffP = kOffQ + 2 * kQBytes;
-  static constexpr int kOffEnd = kOffP + 2 * kPBytes;
+  static constexpr int kOffLut = kOffP + 2 * kPBytes;               // Ultra-TQ: 256 x bf16x2, the codebook by code byte
+  static constexpr int kOffEnd = kOffLut + (kTq ? 1024 : 0);
   static constexpr int kSmemBytes = kOffEnd + 1024;
   static_assert(kOffQ % 1024 == 0, "swizzled tiles need 1024-byte alignment");
   static constexpr uint32_t kColS = 0, kColO = 32, kColV = 64, kTmemCols = 256;
@@ -91,13 +105,14 @@ __device__ __forceinline__ uint32_t cvt_e4m3x2(uint32_t w, int hi) {
 
 // ---------------------------------------------------------------- the kernel
 template <int KV>
-__global__ void __launch_bounds__(kThreads, CmpGeo<KV>::kCtasPerSm)
+__global__ void __launch_bounds__(CmpGeo<KV>::kThreads, CmpGeo<KV>::kCtasPerSm)
 decode_cmp_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_q,
                   const uint8_t* __restrict__ cache, const int32_t* __restrict__ block_tables, int max_pages,
                   const int32_t* __restrict__ seq_lens, int batch, int Hq, int Hkv, int num_splits,
                   float score_scale /* sm_scale * log2(e) */, float* __restrict__ partial_acc,
-                  float* __restrict__ partial_ml) {
+                  float* __restrict__ partial_ml, const TqCodebook tq) {
   using Geo = CmpGeo<KV>;
+  constexpr int kThreads = Geo::kThreads;
   constexpr int kKStages = Geo::kKStages, kVStages = Geo::kVStages, kKStageBytes = Geo::kKStageBytes,
                 kVStageBytes = Geo::kVStageBytes, kKBlockBytes = Geo::kKBlockBytes, kQBytes = Geo::kQBytes,
                 kQBlockBytes = Geo::kQBlockBytes, kKPage = Geo::kKPage, kVPage = Geo::kVPage, kBlocks = Geo::kBlocks;
@@ -108,7 +123,9 @@ decode_cmp_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   const int G = Hq / Hkv;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   // warps 0..3 softmax, 4..7 V warps, 8..11 issuers (role 0 QK, 1 PV, 2 K producer, 3 V producer), as uq_decode.cu
-  const int role = warp < kComputeWarps ? warp + kIssuerWarps : warp - kComputeWarps;
+  // (Ultra-TQ: warps 12..15 are the K dequantisers, role 100 + their index)
+  const int role = warp < kComputeWarps ? warp + kIssuerWarps
+                   : (warp < kComputeWarps + kIssuerWarps ? warp - kComputeWarps : 100 + warp - kComputeWarps - kIssuerWarps);
 
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = base + Geo::kOffQ, sP = base + Geo::kOffP;
@@ -120,9 +137,9 @@ decode_cmp_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
 
   if (tid == 0) {
 #pragma unroll
-    for (int s = 0; s < kKStages; ++s) { mbar_init(bar_fullk + 8 * s, 1); mbar_init(bar_emptyk + 8 * s, 1); }
+    for (int s = 0; s < kKStages; ++s) { mbar_init(bar_fullk + 8 * s, Geo::kTq ? 4 : 1); mbar_init(bar_emptyk + 8 * s, 1); }
 #pragma unroll
-    for (int s = 0; s < kVStages; ++s) { mbar_init(bar_fullv + 8 * s, 1); mbar_init(bar_emptyv + 8 * s, kVWarps); }
+    for (int s = 0; s < kVStages; ++s) { mbar_init(bar_fullv + 8 * s, 1); mbar_init(bar_emptyv + 8 * s, kVWarps + Geo::kDequantWarps); }
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
       mbar_init(bar_sfull + 8 * h, 1);
@@ -137,6 +154,12 @@ decode_cmp_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&sh.tmem_base)),
                  "r"(Geo::kTmemCols));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  if constexpr (Geo::kTq) {                            // codebook by code byte: low nibble = even channel = low half
+    for (int e = tid; e < 256; e += kThreads) {
+      const uint32_t lo = __bfloat16_as_ushort(__float2bfloat16_rn(tq.c[e & 15])), hi = __bfloat16_as_ushort(__float2bfloat16_rn(tq.c[e >> 4]));
+      asm volatile("st.shared.u32 [%0], %1;" ::"r"(base + Geo::kOffLut + 4 * e), "r"(lo | (hi << 16)) : "memory");
+    }
   }
   pdl_launch_dependents();
   pdl_wait();
@@ -183,7 +206,7 @@ decode_cmp_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     // ================================================================ QK warp: S[128 tok x 16 heads] = K . Q^T
     // instruction descriptors: fp32 accumulate (bit 4), A / B format at bits 7 / 10 (kind::f8f6f4: 0 = E4M3;
     // kind::f16: 1 = BF16), N >> 3 at bit 17, M >> 4 at bit 24; both operands K-major
-    const uint32_t idesc_qk = KV == UQ_KV_BF16 ? ((1u << 4) | (1u << 7) | (1u << 10) | (2u << 17) | (8u << 24))
+    const uint32_t idesc_qk = Geo::kBf16 ? ((1u << 4) | (1u << 7) | (1u << 10) | (2u << 17) | (8u << 24))
                                                 : ((1u << 4) | (2u << 17) | (8u << 24));
     auto load_q = [&](const Unit& un, int k) {
       if (elect_one()) {
@@ -219,7 +242,7 @@ decode_cmp_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
           for (int kb = 0; kb < Geo::kQKMmas; ++kb) {
             const uint64_t da = make_desc(st + (kb >> 2) * kKBlockBytes + 32 * (kb & 3), 16, 1024, 2);
             const uint64_t db = make_desc(qb + (kb >> 2) * kQBlockBytes + 32 * (kb & 3), 16, 1024, 2);
-            if constexpr (KV == UQ_KV_BF16) umma_f16_ss(tmem + kColS + 16 * sb, da, db, idesc_qk, kb > 0);
+            if constexpr (Geo::kBf16) umma_f16_ss(tmem + kColS + 16 * sb, da, db, idesc_qk, kb > 0);
             else umma_f8f6f4_ss(tmem + kColS + 16 * sb, da, db, idesc_qk, kb > 0);
           }
           umma_commit(bar_sfull + 8 * sb);
@@ -235,7 +258,7 @@ decode_cmp_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     // ================================================================ PV warp: O^T[128 d x 16 heads] += Vhat^T . P^T
     // A = Vhat^T from TMEM, B = P from smem (MN-major): both f16 (FP8 cache) or both bf16 (BF16 cache: the instruction
     // takes one 16-bit type for A and B — a mixed descriptor is an illegal instruction)
-    const uint32_t idesc_pv = (1u << 4) | (KV == UQ_KV_BF16 ? ((1u << 7) | (1u << 10)) : 0u) | (1u << 16) | (2u << 17) | (8u << 24);
+    const uint32_t idesc_pv = (1u << 4) | (Geo::kBf16 ? ((1u << 7) | (1u << 10)) : 0u) | (1u << 16) | (2u << 17) | (8u << 24);
     Cursor cur;
     sc.start(cur);
     Unit un;
@@ -258,6 +281,7 @@ decode_cmp_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   } else if (role == 2 || role == 3) {
     // ================================================================ producers: K rows by TMA (swizzled), V by bulk copy
     const bool is_k = (role == 2);
+    const bool idle = Geo::kTq && is_k;                 // Ultra-TQ: the K operand is written by the dequantiser warps
     const int n_stages = is_k ? kKStages : kVStages;
     const uint32_t bar_e = is_k ? bar_emptyk : bar_emptyv, bar_f = is_k ? bar_fullk : bar_fullv;
     const uint32_t page_tx = is_k ? (uint32_t)kKPage : (uint32_t)kVPage;
@@ -268,7 +292,7 @@ decode_cmp_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     sc.start(cur);
     Unit un;
     int s = 0, ph = 1;
-    while (sc.next(cur, un)) {
+    while (!idle && sc.next(cur, un)) {
       const int32_t* bt = block_tables + (long long)un.b * max_pages + un.p0 + pl;
       int page_next = (copier && un.p0 + pl < un.p1) ? bt[0] : 0;
       for (int i = 0; i < un.n_tiles; ++i) {
@@ -285,9 +309,59 @@ decode_cmp_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
                         page * Hkv + un.kvh, bar_f + 8 * s, pol);
           else
             bulk_g2s(base + Geo::kOffV + s * kVStageBytes + kVPage * pl,
-                     cache + ((long long)page * Hkv + un.kvh) * Geo::kRecordBytes + kKPage, kVPage, bar_f + 8 * s, pol);
+                     cache + ((long long)page * Hkv + un.kvh) * Geo::kRecordBytes + Geo::kVSrc, kVPage, bar_f + 8 * s, pol);
         }
         if (++s == n_stages) { s = 0; ph ^= 1; }
+      }
+    }
+  } else if (role >= 100) {
+    // ================================================================ Ultra-TQ: K dequantiser warps (Alg. 2 l.7, "K:
+    // dequant via C_K . norm"): thread = token row of the tile.  Its 64 code bytes go through the 256-entry table in
+    // shared memory (one load per byte = two channels, the paper's "LDS gather"), times the block norm
+    // (bf16 x bf16 -> bf16, one rounding), into the row of the K operand buffer (K-major, 128-byte swizzle: what the TMA
+    // unit writes for the BF16 cache).
+    if constexpr (Geo::kTq) {
+      const int row = 32 * (role - 100) + lane;
+      const uint32_t lut = base + Geo::kOffLut;
+      Cursor cur;
+      sc.start(cur);
+      Unit un;
+      int s = 0, ph_full = 0, sk = 0, phk = 1;
+      while (sc.next(cur, un)) {
+        for (int i = 0; i < un.n_tiles; ++i) {
+          mbar_wait(bar_fullv + 8 * s, ph_full);       // the tile's records have landed
+          mbar_wait(bar_emptyk + 8 * sk, phk);         // the product that read operand buffer sk last is complete
+          const uint32_t rec = base + Geo::kOffV + s * kVStageBytes + kTqRecord * (row >> 4);
+          const uint32_t dst = base + Geo::kOffK + sk * kKStageBytes + 128 * row;
+          uint32_t nw[2];                              // the row's four block norms (bf16)
+          asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(nw[0]), "=r"(nw[1]) : "r"(rec + 1024 + 8 * (row & 15)));
+#pragma unroll
+          for (int g = 0; g < 4; ++g) {                // 16 code bytes = 32 channels = one norm block
+            const uint4 cw4 = lds128(rec + 64 * (row & 15) + 16 * g);
+            const uint32_t w[4] = {cw4.x, cw4.y, cw4.z, cw4.w};
+            const uint32_t n2 = __byte_perm(nw[g >> 1], 0, (g & 1) ? 0x3232 : 0x1010);   // (norm, norm)
+            uint32_t o[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+              const uint32_t byte = (w[j >> 2] >> (8 * (j & 3))) & 0xFFu;
+              uint32_t e;
+              asm volatile("ld.shared.u32 %0, [%1];" : "=r"(e) : "r"(lut + 4 * byte));
+              asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(o[j]) : "r"(e), "r"(n2));
+            }
+#pragma unroll
+            for (int c = 0; c < 4; ++c)                // four 16-byte chunks of the row: chunk 4 (g & 1) + c of block g >> 1
+              sts128(dst + (g >> 1) * kKBlockBytes + (((4 * (g & 1) + c) ^ (row & 7)) << 4),
+                     make_uint4(o[4 * c], o[4 * c + 1], o[4 * c + 2], o[4 * c + 3]));
+          }
+          fence_async_smem();
+          __syncwarp();
+          if (lane == 0) {
+            mbar_arrive(bar_fullk + 8 * sk);
+            mbar_arrive(bar_emptyv + 8 * s);
+          }
+          if (++s == kVStages) { s = 0; ph_full ^= 1; }
+          if (++sk == kKStages) { sk = 0; phk ^= 1; }
+        }
       }
     }
   } else {
@@ -354,7 +428,7 @@ decode_cmp_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
 #pragma unroll
               for (int c = 0; c < NH / 8; ++c) {
                 uint4 o;
-                if constexpr (KV == UQ_KV_BF16) {          // kind::f16 wants A and B of one type: P as bf16, like V
+                if constexpr (Geo::kBf16) {                // kind::f16 wants A and B of one type: P as bf16, like V
                   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(o.x) : "f"(lt[8 * c + 1]), "f"(lt[8 * c + 0]));
                   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(o.y) : "f"(lt[8 * c + 3]), "f"(lt[8 * c + 2]));
                   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(o.z) : "f"(lt[8 * c + 5]), "f"(lt[8 * c + 4]));
@@ -481,7 +555,8 @@ decode_cmp_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         int rem = un.tok_end - un.p0 * kPage;
         for (int i = 0; i < un.n_tiles; ++i, rem -= kTilePages * kPage) {
           const int sb = gt & 1;
-          const uint32_t vst = base + Geo::kOffV + s * kVStageBytes + (16 * Geo::kElem) * r;   // this channel's 16 tokens of page 0
+          // this channel's 16 tokens of page 0 (Ultra-TQ: its 8 code bytes; scale / zero of its block q from kTqVMeta on)
+          const uint32_t vst = base + Geo::kOffV + s * kVStageBytes + (Geo::kTq ? kTqVCodes + 8 * r : (16 * Geo::kElem) * r);
           mbar_wait(bar_fullv + 8 * s, ph_full);
           if (gt >= 2) {                               // PV(gt-2) has read Vhat buffer gt&1
             mbar_wait(bar_done + 8 * sb, ((gt >> 1) - 1) & 1);
@@ -495,7 +570,23 @@ decode_cmp_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
 #pragma unroll
             for (int pp = 0; pp < 2; ++pp) {
               const int pg = 2 * h + pp;
-              if constexpr (KV == UQ_KV_BF16) {
+              if constexpr (Geo::kTq) {
+                // Alg. 2 l.7 "V: scale . code + zero": nibbles j and j + 4 of an octet word are tokens 2j, 2j + 1; with
+                // 0x4300 (bf16 128.0) below them they read 128 + code exactly; (x - 128) * scale + zero in bf16, one rounding
+                uint32_t cw2[2];
+                asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(cw2[0]), "=r"(cw2[1]) : "r"(vst + kVPage * pg));
+                const uint32_t meta = base + Geo::kOffV + s * kVStageBytes + kVPage * pg + kTqVMeta + 64 * q;
+                const uint4 s0 = lds128(meta), s1 = lds128(meta + 16), z0 = lds128(meta + 32), z1 = lds128(meta + 48);
+                const uint32_t sc2[8] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
+                const uint32_t ze2[8] = {z0.x, z0.y, z0.z, z0.w, z1.x, z1.y, z1.z, z1.w};
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                  const uint32_t x = ((cw2[j >> 2] >> (4 * (j & 3))) & 0x000F000Fu) | 0x43004300u;
+                  uint32_t cpair;
+                  asm("sub.rn.bf16x2 %0, %1, %2;" : "=r"(cpair) : "r"(x), "r"(0x43004300u));
+                  asm("fma.rn.bf16x2 %0, %1, %2, %3;" : "=r"(o[8 * pp + j]) : "r"(cpair), "r"(sc2[j]), "r"(ze2[j]));
+                }
+              } else if constexpr (KV == UQ_KV_BF16) {
                 const uint4 a = lds128(vst + kVPage * pg), b = lds128(vst + kVPage * pg + 16);
                 o[8 * pp + 0] = a.x; o[8 * pp + 1] = a.y; o[8 * pp + 2] = a.z; o[8 * pp + 3] = a.w;
                 o[8 * pp + 4] = b.x; o[8 * pp + 5] = b.y; o[8 * pp + 6] = b.z; o[8 * pp + 7] = b.w;
@@ -617,15 +708,17 @@ int32_t cmp_maps(int kv, const void* cache, long long records, const void* q_enc
                  CUtensorMap* tq) {
   const EncodeTiledFn encode = encode_tiled_fn();
   if (!encode) return UQ_ERR_CUDA;
-  const bool bf = (kv == UQ_KV_BF16);
+  const bool bf = (kv != UQ_KV_FP8_E4M3), no_k = (kv == UQ_KV_ULTRA_TQ);   // Ultra-TQ: no K map (its records are bulk-copied)
   const cuuint64_t rec = bf ? 8192 : 4096, rowb = bf ? 256 : 128;
   const cuuint64_t gdim[3] = {128, 16, (cuuint64_t)records};
   const cuuint64_t gstr[2] = {rowb, rec};
   const cuuint32_t box[3] = {bf ? 64u : 128u, 16, 1};
   const cuuint32_t estr[3] = {1, 1, 1};
-  CUresult cr = encode(tk, bf ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(cache),
-                       gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
-                       CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  CUresult cr = CUDA_SUCCESS;
+  if (no_k) *tk = CUtensorMap{};
+  else cr = encode(tk, bf ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(cache),
+                   gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                   CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (cr == CUDA_SUCCESS) {
     const cuuint64_t qdim[2] = {128, (cuuint64_t)q_rows};
     const cuuint64_t qstr[1] = {rowb};
@@ -644,7 +737,8 @@ int32_t cmp_maps(int kv, const void* cache, long long records, const void* q_enc
 template <int KV>
 int32_t launch_cmp(const uq_config* cfg, const CUtensorMap& tk, const CUtensorMap& tq, const void* cache,
                    const int32_t* block_tables, int32_t max_pages, const int32_t* seq_lens, int32_t batch,
-                   int32_t num_splits, float* partial_acc, float* partial_ml, cudaStream_t stream) {
+                   int32_t num_splits, float* partial_acc, float* partial_ml, cudaStream_t stream,
+                   const TqCodebook& cb = TqCodebook{}) {
   using Geo = CmpGeo<KV>;
   int sm_count = 0;
   int32_t st = current_device_sms(&sm_count);
@@ -654,10 +748,10 @@ int32_t launch_cmp(const uq_config* cfg, const CUtensorMap& tk, const CUtensorMa
   st = opt_in_dynamic_smem((const void*)decode_cmp_kernel<KV>, Geo::kSmemBytes, "baseline decode: cudaFuncSetAttribute");
   if (st != UQ_OK) return st;
   const float score_scale = resolved_sm_scale(cfg) * 1.4426950408889634f;
-  return check_cuda(launch_pdl(decode_cmp_kernel<KV>, grid, dim3(kThreads), (size_t)Geo::kSmemBytes, stream, tk, tq,
+  return check_cuda(launch_pdl(decode_cmp_kernel<KV>, grid, dim3(Geo::kThreads), (size_t)Geo::kSmemBytes, stream, tk, tq,
                                (const uint8_t*)cache, block_tables, (int)max_pages, seq_lens, (int)batch,
                                (int)cfg->num_q_heads, (int)cfg->num_kv_heads, (int)num_splits, score_scale, partial_acc,
-                               partial_ml),
+                               partial_ml, cb),
                     "uq_baseline_decode_attention launch");
 }
 
@@ -666,8 +760,8 @@ int32_t check_kv(const uq_config* cfg, int32_t kv, const char* who) {
   if (st != UQ_OK) return st;
   st = require_head_dim_128(cfg, who);
   if (st != UQ_OK) return st;
-  if (kv != UQ_KV_FP8_E4M3 && kv != UQ_KV_BF16) {
-    set_error("%s: kv_format must be UQ_KV_FP8_E4M3 (1) or UQ_KV_BF16 (2)", who);
+  if (kv != UQ_KV_FP8_E4M3 && kv != UQ_KV_BF16 && kv != UQ_KV_ULTRA_TQ) {
+    set_error("%s: kv_format must be UQ_KV_FP8_E4M3 (1), UQ_KV_BF16 (2) or UQ_KV_ULTRA_TQ (3)", who);
     return UQ_ERR_INVALID_ARG;
   }
   return UQ_OK;
@@ -678,7 +772,7 @@ int32_t check_kv(const uq_config* cfg, int32_t kv, const char* who) {
 
 extern "C" size_t uq_baseline_record_bytes(const uq_config* cfg, int32_t kv_format) {
   if (uq::check_kv(cfg, kv_format, "uq_baseline_record_bytes") != UQ_OK) return 0;
-  return kv_format == UQ_KV_BF16 ? 8192 : 4096;
+  return kv_format == UQ_KV_ULTRA_TQ ? (size_t)uq::kTqRecord : (kv_format == UQ_KV_BF16 ? 8192 : 4096);
 }
 
 extern "C" int32_t uq_baseline_append(const uq_config* cfg, int32_t kv_format, const void* k_new, const void* v_new,
@@ -689,6 +783,10 @@ extern "C" int32_t uq_baseline_append(const uq_config* cfg, int32_t kv_format, c
   NvtxRange nvtx_range("uq_baseline_append");
   int32_t st = check_kv(cfg, kv_format, "uq_baseline_append");
   if (st != UQ_OK) return st;
+  if (kv_format == UQ_KV_ULTRA_TQ) {
+    set_error("uq_baseline_append: the Ultra-TQ cache takes a codebook: call uq_tq_append");
+    return UQ_ERR_INVALID_ARG;
+  }
   if (batch <= 0 || total_new < 0 || max_pages <= 0 || num_pages <= 0) {
     set_error("baseline append: batch/max_pages/num_pages must be positive, total_new >= 0");
     return UQ_ERR_INVALID_ARG;
@@ -734,6 +832,10 @@ extern "C" int32_t uq_baseline_decode_attention(const uq_config* cfg, int32_t kv
   NvtxRange nvtx_range("uq_baseline_decode_attention");
   int32_t st = check_kv(cfg, kv_format, "uq_baseline_decode_attention");
   if (st != UQ_OK) return st;
+  if (kv_format == UQ_KV_ULTRA_TQ) {
+    set_error("uq_baseline_decode_attention: the Ultra-TQ cache takes a codebook: call uq_tq_decode_attention");
+    return UQ_ERR_INVALID_ARG;
+  }
   if (!q_enc || !cache || !block_tables || !seq_lens || !partial_acc || !partial_ml || batch <= 0 || num_splits <= 0 ||
       max_pages <= 0 || num_pages <= 0) {
     set_error("baseline decode: NULL pointer or non-positive size");
@@ -765,4 +867,50 @@ extern "C" int32_t uq_baseline_decode_attention(const uq_config* cfg, int32_t kv
                                   partial_ml, (cudaStream_t)stream);
   return launch_cmp<UQ_KV_FP8_E4M3>(cfg, tk, tq, cache, block_tables, max_pages, seq_lens, batch, num_splits, partial_acc,
                                     partial_ml, (cudaStream_t)stream);
+}
+
+// Ultra-TQ (Alg. 2): the decode of uq_baseline_decode_attention over the codebook cache.
+extern "C" int32_t uq_tq_decode_attention(const uq_config* cfg, const float* codebook_k, const void* q_rot, const void* cache,
+                                          int64_t num_pages, const int32_t* block_tables, int32_t max_pages,
+                                          const int32_t* seq_lens, int32_t batch, int32_t num_splits, float* partial_acc,
+                                          float* partial_ml, void* stream) {
+  using namespace uq;
+  NvtxRange nvtx_range("uq_tq_decode_attention");
+  int32_t st = check_kv(cfg, UQ_KV_ULTRA_TQ, "uq_tq_decode_attention");
+  if (st != UQ_OK) return st;
+  if (!codebook_k || !q_rot || !cache || !block_tables || !seq_lens || !partial_acc || !partial_ml || batch <= 0 ||
+      num_splits <= 0 || max_pages <= 0 || num_pages <= 0) {
+    set_error("uq_tq_decode_attention: NULL pointer or non-positive size");
+    return UQ_ERR_INVALID_ARG;
+  }
+  if (((uintptr_t)cache & 15u) || ((uintptr_t)q_rot & 15u) || ((uintptr_t)partial_acc & 15u) || ((uintptr_t)partial_ml & 7u)) {
+    set_error("uq_tq_decode_attention: misaligned pointer (cache 16 B, q_rot 16 B, partial_acc 16 B, partial_ml 8 B)");
+    return UQ_ERR_INVALID_ARG;
+  }
+  if (batch > kMaxBatch) {
+    set_error("uq_tq_decode_attention: batch %d exceeds the supported maximum of %d sequences per call", batch, kMaxBatch);
+    return UQ_ERR_UNSUPPORTED;
+  }
+  if ((long long)num_pages * cfg->num_kv_heads > 0x7fffffffLL) {
+    set_error("uq_tq_decode_attention: num_pages * num_kv_heads must be < 2^31");
+    return UQ_ERR_INVALID_ARG;
+  }
+  TqCodebook cb;
+  for (int i = 0; i < 16; ++i) {
+    cb.c[i] = codebook_k[i];
+    if (!(cb.c[i] == cb.c[i]) || (i > 0 && !(cb.c[i] > cb.c[i - 1]))) {
+      set_error("uq_tq_decode_attention: codebook_k must be 16 finite values in ascending order");
+      return UQ_ERR_INVALID_ARG;
+    }
+  }
+  if (cfg->flags & UQ_FLAG_DEBUG_CHECKS) {
+    st = debug_check_tables("uq_tq_decode_attention", block_tables, max_pages, batch, num_pages, seq_lens, nullptr, 0, 0,
+                            cfg->page_size, 0, (cudaStream_t)stream);
+    if (st != UQ_OK) return st;
+  }
+  CUtensorMap tk, tq;
+  st = cmp_maps(UQ_KV_ULTRA_TQ, cache, 0, q_rot, (long long)batch * cfg->num_q_heads, &tk, &tq);
+  if (st != UQ_OK) return st;
+  return launch_cmp<UQ_KV_ULTRA_TQ>(cfg, tk, tq, cache, block_tables, max_pages, seq_lens, batch, num_splits, partial_acc,
+                                    partial_ml, (cudaStream_t)stream, cb);
 }

@@ -915,3 +915,75 @@ def test_comparison_caches_fp8_and_bf16_kv(kv, hq, hkv):
             if q8 is not None:
                 assert np.array_equal(bufs.q_fp8[b].cpu().numpy(), q8), f"seq {b}: FP8 query bytes differ"
             H.check_out(out[b], ref, f"{kv} kv seq {b} S={S}")
+
+
+def test_ultra_tq_cache_and_decode_against_the_oracle_of_algorithm_2():
+    """Ultra-TQ comparison path (Alg. 2, last item): uq_tq_append's cache image —
+    codebook indices, bf16 block norms, uniform V codes, bf16 (scale, zero) — and the rotated bf16 query bit for bit against
+    oracle/ultra_tq.py, read back through the independent unpacker of tests/uq_layout.py; uq_tq_decode_attention + merge
+    within 2e-3 + 1e-2 |ref| of its float64 attention, for a ragged batch (empty, one token, page and tile boundaries,
+    multi-tile), GQA 16 and 6, slot counts 1, 3 and 64, tokens appended one sequence at a time AND several per call."""
+    from oracle import ultra_tq as T
+    from . import uq_layout as UL
+    cb = np.asarray(W.TQ_CODEBOOK, np.float32)
+    for hq, hkv in ((16, 1), (12, 2)):
+        wl = W.make_custom("tq", 71, [0, 1, 17, 203, 1000, 16, 31, 129], hq, hkv, outlier_channels=3, outlier_gain=8.0,
+                           peaked_frac=0.3)
+        cfg = H.cfg_of(wl)
+        assert uq.baseline_record_bytes(cfg, uq.KV_ULTRA_TQ) == UL.TQ_RECORD
+        cache = uq.alloc_baseline_cache(cfg, uq.KV_ULTRA_TQ, wl.num_pages, DEV)
+        bt = torch.from_numpy(wl.block_tables).to(DEV)
+        B = wl.batch
+        # first half of every sequence in one call for all sequences, the rest sequence by sequence
+        half = (wl.ctx_lens // 2).astype(np.int32)
+        ks, vs = [], []
+        for b in range(B):
+            k, v = W.seq_kv(wl, b, int(wl.ctx_lens[b]), DEV) if wl.ctx_lens[b] else (None, None)
+            ks.append(k); vs.append(v)
+        cu = np.concatenate([[0], np.cumsum(half)]).astype(np.int32)
+        if cu[-1]:
+            k1 = torch.cat([ks[b][:half[b]] for b in range(B) if half[b]]); v1 = torch.cat([vs[b][:half[b]] for b in range(B) if half[b]])
+            uq.tq_append(cfg, cb, k1.contiguous(), v1.contiguous(), torch.from_numpy(cu).to(DEV),
+                         torch.zeros(B, dtype=torch.int32, device=DEV), bt, cache)
+        for b in range(B):
+            n = int(wl.ctx_lens[b] - half[b])
+            if n == 0:
+                continue
+            before = np.zeros(B, np.int32); before[b] = half[b]
+            cu = np.zeros(B + 1, np.int32); cu[b + 1:] = n
+            uq.tq_append(cfg, cb, ks[b][half[b]:].contiguous(), vs[b][half[b]:].contiguous(), torch.from_numpy(cu).to(DEV),
+                         torch.from_numpy(before).to(DEV), bt, cache)
+        q = W.gen_q(wl, DEV)
+        q_rot = torch.empty_like(q)
+        lens = torch.from_numpy(wl.ctx_lens.astype(np.int32)).to(DEV)
+        empty = torch.zeros((0, hkv, 128), dtype=torch.bfloat16, device=DEV)
+        uq.tq_append(cfg, cb, empty, empty, torch.zeros(B + 1, dtype=torch.int32, device=DEV), lens, bt, cache, q=q, q_rot=q_rot)
+        torch.cuda.synchronize()
+        host = cache.cpu().numpy()
+        qb = H.bits(q)
+        assert np.array_equal(H.bits(q_rot).reshape(-1, 128), T.bf16_bits(T.encode_q(qb.reshape(-1, 128)))), "rotated bf16 query differs"
+        refs = {}
+        for b in range(B):
+            L = int(wl.ctx_lens[b])
+            if L == 0:
+                continue
+            kbits, vbits = H.bits(ks[b]).reshape(L * hkv, 128), H.bits(vs[b]).reshape(L * hkv, 128)
+            ki, kn = T.encode_k(kbits, cb)
+            vc, vsc, vz = T.encode_v(vbits)
+            gi, gn, gc, gs, gz = UL.gather_tq_sequence(host, wl.block_tables[b], L)
+            sh = lambda a: a.reshape(L, hkv, -1)
+            assert np.array_equal(gi, sh(ki)), f"seq {b}: codebook indices differ"
+            assert np.array_equal(gn, sh(T.bf16_bits(kn))), f"seq {b}: block norms differ"
+            assert np.array_equal(gc, sh(vc)), f"seq {b}: V codes differ"
+            assert np.array_equal(gs, sh(T.bf16_bits(vsc))) and np.array_equal(gz, sh(T.bf16_bits(vz))), f"seq {b}: V scale / zero differ"
+            refs[b] = T.attention(qb[b], sh(ki), sh(kn), sh(vc), sh(vsc), sh(vz), cb, hkv)
+        for S in (1, 3, 64):
+            bufs = uq.StepBuffers(cfg, B, S, DEV)
+            bufs.partial_acc.fill_(float("nan")); bufs.partial_ml.fill_(float("nan"))
+            uq.tq_decode_attention(cfg, cb, q_rot, cache, bt, lens, S, bufs.partial_acc, bufs.partial_ml)
+            uq.merge_splits(cfg, bufs.partial_acc, bufs.partial_ml, bufs.out)
+            torch.cuda.synchronize()
+            out = bufs.out.float().cpu().numpy().astype(np.float64)
+            assert np.all(out[0] == 0)                                          # the empty sequence
+            for b, ref in refs.items():
+                H.check_out(out[b], ref, f"ultra-tq seq {b} S={S} heads {hq}/{hkv}")

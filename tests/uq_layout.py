@@ -81,3 +81,38 @@ def used_byte_mask(d: int = 128):
     np.add.at(count, VS.ravel(), 1)
     np.add.at(count, VC.ravel(), 1)                               # two tokens (nibbles) per V byte
     return count
+
+
+# ----------------------------------------------------------------------------- Ultra-TQ comparison cache (include/uq.h)
+TQ_RECORD = 2432
+
+
+def unpack_tq_records(rec: np.ndarray):
+    """rec uint8 [..., 2432] -> logical (k_idx [...,16,128] in 0..15, k_norm uint16 bf16 bits [...,16,4],
+    v_code [...,16,128], v_scale bits [...,16,4], v_zero bits [...,16,4]), from the layout table of include/uq.h."""
+    rec = np.asarray(rec, np.uint8)
+    assert rec.shape[-1] == TQ_RECORD
+    lead = rec.shape[:-1]
+    kb = rec[..., 0:1024].reshape(*lead, 16, 64)                      # token t at 64 t, byte j = channels 2j, 2j + 1
+    k_idx = np.stack([kb & 0xF, kb >> 4], axis=-1).reshape(*lead, 16, 128)
+    k_norm = np.ascontiguousarray(rec[..., 1024:1152]).view(np.uint16).reshape(*lead, 16, 4)   # 1024 + 8 t + 2 g
+    vw = np.ascontiguousarray(rec[..., 1152:2176]).view(np.uint32).reshape(*lead, 128, 2)      # channel c, word t >> 3
+    v_code = np.zeros((*lead, 16, 128), np.uint8)
+    for t in range(16):
+        tt = t & 7
+        nib = (tt >> 1) + 4 * (tt & 1)                                # token 2n in nibble n, token 2n + 1 in nibble n + 4
+        v_code[..., t, :] = (vw[..., :, t >> 3] >> np.uint32(4 * nib)) & 0xF
+    meta = np.ascontiguousarray(rec[..., 2176:2432]).view(np.uint16).reshape(*lead, 4, 2, 16)  # block g: scales, zeros
+    v_scale = np.moveaxis(meta[..., :, 0, :], -1, -2)                 # [..., 16 tokens, 4 blocks]
+    v_zero = np.moveaxis(meta[..., :, 1, :], -1, -2)
+    return k_idx, k_norm, v_code, v_scale, v_zero
+
+
+def gather_tq_sequence(cache: np.ndarray, block_table: np.ndarray, length: int):
+    """Logical arrays of one sequence, each [L, Hkv, .]."""
+    n_pages = -(-length // PAGE)
+    parts = unpack_tq_records(cache[block_table[:n_pages]])            # [n_pages, Hkv, 16, .]
+    def fix(a):
+        a = np.moveaxis(a, 2, 1)
+        return a.reshape(n_pages * PAGE, a.shape[2], a.shape[3])[:length]
+    return tuple(fix(a) for a in parts)
