@@ -106,6 +106,8 @@ def step_bytes(wl, num_splits: int, ctx_after: np.ndarray, new_per_seq: int):
         per_tok = 2 * d                                              # comparison cache: one E4M3 byte per element
     elif KV_FORMAT == "bf16":
         per_tok = 4 * d
+    elif KV_FORMAT == "tq":
+        per_tok = 2432 // 16                                         # Ultra-TQ record: 152 B per (token, kv head)
     tokens = int(ctx_after.astype(np.int64).sum())
     pages = int(((ctx_after.astype(np.int64) + wl.page_size - 1) // wl.page_size).sum())
     kv = tokens * Hkv * per_tok
@@ -198,7 +200,7 @@ class ClockSampler(threading.Thread):
 # ----------------------------------------------------------------------------- our arm
 def fill_cache(uq, W, cfg, wl, lens, device, chunk_tokens=1 << 16):
     """Prefill through uq_rotate_quantize_append (bulk appends); shared prefix written once."""
-    fmt = {"fp8": uq.KV_FP8_E4M3, "bf16": uq.KV_BF16}.get(KV_FORMAT)
+    fmt = {"fp8": uq.KV_FP8_E4M3, "bf16": uq.KV_BF16, "tq": uq.KV_ULTRA_TQ}.get(KV_FORMAT)
     cache = uq.alloc_cache(cfg, wl.num_pages, device) if fmt is None else uq.alloc_baseline_cache(cfg, fmt, wl.num_pages, device)
     bt_dev = torch.from_numpy(wl.block_tables).to(device)
     B = wl.batch
@@ -213,6 +215,9 @@ def fill_cache(uq, W, cfg, wl, lens, device, chunk_tokens=1 << 16):
             if fmt is None:
                 uq.rotate_quantize_append(cfg, k, v, torch.from_numpy(cu).to(device),
                                           torch.from_numpy(before).to(device), bt_dev, cache)
+            elif fmt == uq.KV_ULTRA_TQ:
+                uq.tq_append(cfg, W.TQ_CODEBOOK, k, v, torch.from_numpy(cu).to(device), torch.from_numpy(before).to(device),
+                             bt_dev, cache)
             else:
                 uq.baseline_append(cfg, fmt, k, v, torch.from_numpy(cu).to(device), torch.from_numpy(before).to(device),
                                    bt_dev, cache)
@@ -277,9 +282,18 @@ def run_ours(args, rank, world, local_rank):
         S_suffix = args.splits or uq.suggest_num_splits_max(cfg, B, max(1, int(suf.mean())), int(suf.max()))
         bufs_sp = uq.StepBuffers(cfg, B, S_suffix, dev)
 
-    fmt = {"fp8": uq.KV_FP8_E4M3, "bf16": uq.KV_BF16}.get(KV_FORMAT)
+    fmt = {"fp8": uq.KV_FP8_E4M3, "bf16": uq.KV_BF16, "tq": uq.KV_ULTRA_TQ}.get(KV_FORMAT)
+    q_rot = torch.empty_like(qs[0]) if fmt == uq.KV_ULTRA_TQ else None
 
     def step(i):
+        if fmt == uq.KV_ULTRA_TQ:                        # Alg. 2: append + rotated bf16 query, codebook decode, merge
+            k_new, v_new = kvs[i % n_in]
+            uq.tq_append(cfg, W.TQ_CODEBOOK, k_new, v_new, cu_dev, before_dev, bt_dev, cache, q=qs[i % n_in], q_rot=q_rot,
+                         stream=stream)
+            uq.tq_decode_attention(cfg, W.TQ_CODEBOOK, q_rot, cache, bt_dev, after_dev, S, bufs.partial_acc, bufs.partial_ml,
+                                   stream=stream)
+            uq.merge_splits(cfg, bufs.partial_acc, bufs.partial_ml, bufs.out, stream=stream)
+            return bufs.out
         if fmt is not None:                              # comparison cache: append, decode, merge over FP8 / BF16 KV
             k_new, v_new = kvs[i % n_in]
             return uq.baseline_decode_step(cfg, fmt, bufs, qs[i % n_in], k_new, v_new, cu_dev, before_dev, after_dev,
@@ -340,6 +354,15 @@ def run_ours(args, rank, world, local_rank):
     sampler.busy = True
     for i in range(n_inst):
         k_new, v_new = kvs[i % n_in]
+        if fmt == uq.KV_ULTRA_TQ:
+            uq.tq_append(cfg, W.TQ_CODEBOOK, k_new, v_new, cu_dev, before_dev, bt_dev, cache, q=qs[i % n_in], q_rot=q_rot,
+                         stream=stream)
+            dec_ev[i][0].record(stream)
+            uq.tq_decode_attention(cfg, W.TQ_CODEBOOK, q_rot, cache, bt_dev, after_dev, S, bufs.partial_acc, bufs.partial_ml,
+                                   stream=stream)
+            dec_ev[i][1].record(stream)
+            uq.merge_splits(cfg, bufs.partial_acc, bufs.partial_ml, bufs.out, stream=stream)
+            continue
         if fmt is not None:
             fp8 = fmt == uq.KV_FP8_E4M3
             uq.baseline_append(cfg, fmt, k_new, v_new, cu_dev, before_dev, bt_dev, cache, q=qs[i % n_in] if fp8 else None,
@@ -449,7 +472,7 @@ def run_ours(args, rank, world, local_rank):
         "metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": round(ms_step, 5),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": {"fp4": "fp8xfp4->f32", "fp8": "fp8xfp8->f32", "bf16": "bf16xbf16->f32"}[KV_FORMAT],
+        "dtype": {"fp4": "fp8xfp4->f32", "fp8": "fp8xfp8->f32", "bf16": "bf16xbf16->f32", "tq": "bf16xbf16->f32 (codebook / uniform 4-bit dequantised on read)"}[KV_FORMAT],
         "data": "synthetic", "impl": "ours",
         **({"kv_format": KV_FORMAT + " (comparison cache, PAPER.md:163 - not the headline metric; e2e not measured)"}
            if fmt is not None else {}),
@@ -761,8 +784,9 @@ def main():
                     help="instead of the decode step, time uq_calibrate_c over VECTORS key vectors and 56 constants")
     ap.add_argument("--no-early", action="store_true",
                     help="do not set UQ_FLAG_SMALL_APPEND_AHEAD (the decode kernel then waits for the append before it reads anything)")
-    ap.add_argument("--kv", default="fp4", choices=["fp4", "fp8", "bf16"],
-                    help="fp4: UltraQuant (default).  fp8 / bf16: the same step over the paper's comparison caches")
+    ap.add_argument("--kv", default="fp4", choices=["fp4", "fp8", "bf16", "tq"],
+                    help="fp4: UltraQuant (default).  fp8 / bf16 / tq: the same step over the paper's comparison caches "
+                         "(tq = Ultra-TQ, the codebook encoding of Algorithm 2)")
     ap.add_argument("--head-dim", type=int, default=128, choices=[64, 128, 256],
                     help="run the config's shape at another head size (the decode step only)")
     ap.add_argument("--sustain", type=float, default=2.0, metavar="SECONDS",
