@@ -46,6 +46,14 @@ struct NvtxRange {
   NvtxRange& operator=(const NvtxRange&) = delete;
 };
 
+// Ultra-TQ comparison cache (Alg. 2; include/uq.h "ULTRA-TQ"): record regions and the codebook as it
+// is handed to the kernels (by value: 16 levels)
+constexpr int kTqRecord = 2432;                // K indices 1024 | K block norms 128 | V codes 1024 | V scale / zero 256
+constexpr int kTqKNorms = 1024, kTqVCodes = 1152, kTqVMeta = 2176;
+struct TqCodebook {
+  float c[16];
+};
+
 void set_error(const char* fmt, ...);
 int32_t check_config(const uq_config* cfg);  // UQ_OK / UQ_ERR_*; sets the error string
 int32_t check_cuda(cudaError_t e, const char* what);

@@ -24,12 +24,6 @@ namespace {
 
 constexpr int kSoftmaxWarps = 4, kVWarps = 4, kIssuerWarps = 4;
 constexpr int kComputeWarps = kSoftmaxWarps + kVWarps;
-constexpr int kTqRecord = 2432;                      // Ultra-TQ record: K codes 1024 | K norms 128 | V codes 1024 | V scale / zero 256
-constexpr int kTqVCodes = 1152, kTqVMeta = 2176;
-
-struct TqCodebook {                                  // Alg. 2 "Require: codebook C_K": 16 levels, by value
-  float c[16];
-};
 constexpr int kPBytes = 4096;                        // one P operand buffer (as uq_decode.cu)
 constexpr float kThresh = 12.0f;
 constexpr int kMaxBatch = 2048;

@@ -11,13 +11,6 @@
 namespace uq {
 namespace {
 
-constexpr int kTqRecord = 2432;                        // K codes 1024 | K norms 128 | V codes 1024 | V scale / zero 256
-constexpr int kTqKNorms = 1024, kTqVCodes = 1152, kTqVMeta = 2176;
-
-struct TqCodebook {
-  float c[16];
-};
-
 // double -> the nearest bf16 (ties to even) and back
 __device__ __forceinline__ double bf16_rne(double x, uint32_t* bits) {
   const __nv_bfloat16 h = __double2bfloat16(x);

@@ -987,3 +987,52 @@ def test_ultra_tq_cache_and_decode_against_the_oracle_of_algorithm_2():
             assert np.all(out[0] == 0)                                          # the empty sequence
             for b, ref in refs.items():
                 H.check_out(out[b], ref, f"ultra-tq seq {b} S={S} heads {hq}/{hkv}")
+
+
+def test_ultra_tq_scaled_config3_sampled_sequences():
+    """Ultra-TQ on config 3's shape at 0.2 x (13 ragged sequences of 4,180-13,037 tokens, 48/8 heads = GQA 6: several
+    units per CTA, slots from uq_suggest_num_splits): three sequences — the longest, the shortest, one in between — cache
+    image bit for bit and outputs within 2e-3 + 1e-2 |ref| of the oracle of Algorithm 2; the rest must be finite."""
+    from oracle import ultra_tq as T
+    from . import uq_layout as UL
+    cb = np.asarray(W.TQ_CODEBOOK, np.float32)
+    wl = W.make_config(3, scale=0.2)
+    cfg = H.cfg_of(wl)
+    B, hkv = wl.batch, wl.num_kv_heads
+    cache = uq.alloc_baseline_cache(cfg, uq.KV_ULTRA_TQ, wl.num_pages, DEV)
+    cache.fill_(0xFF)                                                        # stale bytes: NaN patterns in norms / scales
+    bt = torch.from_numpy(wl.block_tables).to(DEV)
+    for b in range(B):
+        L = int(wl.ctx_lens[b])
+        k, v = W.seq_kv(wl, b, L, DEV)
+        before = np.zeros(B, np.int32)
+        cu = np.zeros(B + 1, np.int32); cu[b + 1:] = L
+        uq.tq_append(cfg, cb, k.contiguous(), v.contiguous(), torch.from_numpy(cu).to(DEV), torch.from_numpy(before).to(DEV), bt, cache)
+    q = W.gen_q(wl, DEV)
+    q_rot = torch.empty_like(q)
+    lens = torch.from_numpy(wl.ctx_lens.astype(np.int32)).to(DEV)
+    empty = torch.zeros((0, hkv, 128), dtype=torch.bfloat16, device=DEV)
+    uq.tq_append(cfg, cb, empty, empty, torch.zeros(B + 1, dtype=torch.int32, device=DEV), lens, bt, cache, q=q, q_rot=q_rot)
+    S = uq.suggest_num_splits(cfg, B, int(wl.ctx_lens.mean()))
+    bufs = uq.StepBuffers(cfg, B, S, DEV)
+    bufs.partial_acc.fill_(float("nan")); bufs.partial_ml.fill_(float("nan"))
+    uq.tq_decode_attention(cfg, cb, q_rot, cache, bt, lens, S, bufs.partial_acc, bufs.partial_ml)
+    uq.merge_splits(cfg, bufs.partial_acc, bufs.partial_ml, bufs.out)
+    torch.cuda.synchronize()
+    out = bufs.out.float().cpu().numpy().astype(np.float64)
+    assert np.isfinite(out).all()
+    host = cache.cpu().numpy()
+    qb = H.bits(q)
+    order = np.argsort(wl.ctx_lens)
+    for b in (int(order[-1]), int(order[0]), int(order[len(order) // 2])):
+        L = int(wl.ctx_lens[b])
+        k, v = W.seq_kv(wl, b, L, DEV)
+        ki, kn = T.encode_k(H.bits(k).reshape(L * hkv, 128), cb)
+        vc, vsc, vz = T.encode_v(H.bits(v).reshape(L * hkv, 128))
+        gi, gn, gc, gs, gz = UL.gather_tq_sequence(host, wl.block_tables[b], L)
+        sh = lambda a: a.reshape(L, hkv, -1)
+        assert np.array_equal(gi, sh(ki)) and np.array_equal(gn, sh(T.bf16_bits(kn))), f"seq {b}: K image differs"
+        assert np.array_equal(gc, sh(vc)) and np.array_equal(gs, sh(T.bf16_bits(vsc))) and np.array_equal(gz, sh(T.bf16_bits(vz))), \
+            f"seq {b}: V image differs"
+        ref = T.attention(qb[b], sh(ki), sh(kn), sh(vc), sh(vsc), sh(vz), cb, hkv)
+        H.check_out(out[b], ref, f"ultra-tq config 3 x 0.2, seq {b} ({L} tokens), S={S}")
