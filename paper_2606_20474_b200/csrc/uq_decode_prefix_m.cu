@@ -12,6 +12,9 @@
 //   * P (fp16) goes back to TMEM and is the A operand of the PV product; Vhat (fp16, [channel][token], 128-byte swizzle)
 //     is written to shared memory ONCE per tile for all NSEQ sequences and is the B operand; O[128 rows x 128 channels]
 //     accumulates in TMEM;
+//   * the row sums of P come out of the same product: 16 constant rows of ones behind the 128 channel rows of Vhat
+//     (N = 144) put sum_t P[row][t] into accumulator columns 128..143 — the sum of exactly the fp16 values the numerator
+//     uses, and 64 additions per thread and tile less in the softmax warps (4 % of the kernel's time);
 //   * K codes x FP8 queries by tcgen05.mma kind::mxf8f6f4.block_scale with the K group scales as the B-side scale
 //     factors (the paper's FP8 x FP4 scaled MMA), the query-side factors constant 1.
 // V's reference exponent: a V warp (one 32-channel scale group) scans the scale bytes of its unit's tile range first —
@@ -40,7 +43,9 @@ constexpr int kTilePages = 8;                        // 128 tokens per tile
 constexpr int kRestBytes = kRecordBytes - 1024;      // V codes + K scales + V scales = 1152
 constexpr int kKStageBytes = kTilePages * 2048;      // K codes, one byte per code
 constexpr int kVStageBytes = kTilePages * kRestBytes;
-constexpr int kVhBytes = 128 * 256;                  // Vhat of a tile: [2 blocks of 64 tokens][128 channels][128 B]
+constexpr int kVhRows = 144;                         // 128 channels + 16 rows of ones: the PV product also sums each row of P
+constexpr int kVhBlock = kVhRows * 128;              // one block of 64 tokens: [144 rows][128 B], 128-byte swizzle
+constexpr int kVhBytes = 2 * kVhBlock;               // Vhat of a tile: two blocks of 64 tokens
 constexpr int kQBytes = 128 * 128;                   // the query rows of a unit: [128 rows][128 B E4M3]
 constexpr float kThresh = 12.0f;
 
@@ -59,9 +64,10 @@ static_assert(kOffVh % 1024 == 0 && kOffQ % 1024 == 0, "swizzled tiles need 1024
 constexpr uint32_t kColS = 0;      // 2 x 128: scores, lane = (sequence, head) row, column = token.  P (f16x2, column c =
                                    // tokens 2c, 2c+1) overwrites the first 64 columns of its score buffer IN PLACE, chunk
                                    // after chunk behind the softmax thread's reads: P is double-buffered for free
-constexpr uint32_t kColO = 256;    // 128: accumulator, column = channel
-constexpr uint32_t kColSFA = 384;  // 4
-constexpr uint32_t kColSFB = 388;  // 2 x 4
+constexpr uint32_t kColO = 256;    // 144: accumulator, column = channel; columns 128..143 = the row sum of P (the ones rows)
+constexpr uint32_t kColL = kColO + 128;
+constexpr uint32_t kColSFA = 400;  // 4
+constexpr uint32_t kColSFB = 404;  // 2 x 4
 constexpr uint32_t kTmemCols = 512;
 
 struct Shared {
@@ -74,7 +80,6 @@ struct Shared {
   uint32_t tmem_base;
   float vscale[4][4];              // [unit ordinal & 3][group]: 2^(eref - 13 - 127), for the epilogue of that unit
   float pmax[2][kSW][128];         // [tile parity][part][row]: partial row maxima of a tile (pass 1)
-  float lpart[kSW][128];           // [part][row]: partial running sums at the end of a unit
 };
 
 // Items = (group of NSEQ consecutive sequences, kv head), kv head fastest, PT tiles each; the tiles of all items form
@@ -173,6 +178,12 @@ decode_prefix_m_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_co
   if (tid < 128) {  // query-side scale factors: UE8M0 byte 127 = 2^0
     asm volatile("st.shared.u32 [%0], %1;" ::"r"(sSFA + 4 * tid), "r"(0x7F7F7F7Fu) : "memory");
   }
+  // the ones rows (f16 1.0) of both Vhat buffers: rows 128..143 of each 64-token block — the swizzle permutes equal chunks
+  for (int e = tid; e < 2 * 2 * 16 * 32; e += kThreads) {
+    const int blk = e >> 9, w = e & 511;
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(sVh + kVhBytes * (blk >> 1) + kVhBlock * (blk & 1) + 128 * 128 + 4 * w),
+                 "r"(0x3C003C00u) : "memory");
+  }
   pdl_launch_dependents();
   pdl_wait();
   fence_async_smem();
@@ -253,7 +264,7 @@ decode_prefix_m_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_co
   } else if (role == 1) {
     // ================================================================ PV warp: O[128 rows x 128 ch] += P . Vhat
     // A = P from TMEM (f16), B = Vhat from smem ([channel][token]: K-major, 128-byte swizzle), N = 128
-    const uint32_t idesc_pv = (1u << 4) | (16u << 17) | (8u << 24);
+    const uint32_t idesc_pv = (1u << 4) | ((uint32_t)(kVhRows >> 3) << 17) | (8u << 24);   // N = 144
     Unit un;
     int gt = 0;
     while (sc.next(un)) {
@@ -266,7 +277,7 @@ decode_prefix_m_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_co
           const uint32_t vb = sVh + kVhBytes * sb;
 #pragma unroll
           for (int j = 0; j < 8; ++j)                    // 16 tokens per MMA = 8 columns of P, 32 bytes of a Vhat row
-            umma_f16_ts(tmem + kColO, tmem + kColS + 128 * sb + kColsPart * (j / kCP) + 8 * (j % kCP), make_desc(vb + (j >> 2) * 16384 + 32 * (j & 3), 16, 1024, 2),
+            umma_f16_ts(tmem + kColO, tmem + kColS + 128 * sb + kColsPart * (j / kCP) + 8 * (j % kCP), make_desc(vb + (j >> 2) * kVhBlock + 32 * (j & 3), 16, 1024, 2),
                         idesc_pv, (i > 0 || j > 0) ? 1u : 0u);
           umma_commit(bar_done + 8 * sb);
         }
@@ -322,7 +333,7 @@ decode_prefix_m_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_co
         const int b = un.b0 + si;
         const bool valid = (b < batch) && (hh < G);
         const long long prow = (((long long)b * Hq + (long long)un.kvh * G + hh) * num_splits) + un.slot;
-        float nref = 0.f, lsum = 0.f;                  // minus the row's reference logit (log2 units), this part's running sum
+        float nref = 0.f;                              // minus the row's reference logit (log2 units)
         for (int i = 0; i < un.n_tiles; ++i, ++gt) {
           const int sb = gt & 1;
           // this part's columns of the score buffer; its P (f16 pairs) overwrites their first half in place
@@ -348,25 +359,23 @@ decode_prefix_m_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_co
           mx *= score_scale;
           if (i == 0) {
             nref = -mx;
-            lsum = 0.f;
           } else if (__builtin_expect(__any_sync(kFull, mx + nref > kThresh), 0)) {
             const float add = (mx + nref > kThresh) ? mx + nref : 0.f;   // factor 1 for the rows that stay
             const float f = ex2(-add);
             mbar_wait(bar_done + 8 * ((gt - 1) & 1), ((gt - 1) >> 1) & 1);   // every PV issued so far has to be in O
             tc_fence_after();
 #pragma unroll 1
-            for (int cc = 0; cc < kCP; ++cc) {          // this part's columns of the O row
+            for (int cc = 0; cc < kCP + (part == 0 ? 1 : 0); ++cc) {   // this part's columns of the O row (part 0: + the row sum)
+              const uint32_t t_oc = tmem + lane_sel + kColO + (cc < kCP ? kColsPart * part + 16 * cc : 128);
               float ov[16];
-              tmem_ld<16>(tmem + lane_sel + kColO + kColsPart * part + 16 * cc, ov);
+              tmem_ld<16>(t_oc, ov);
 #pragma unroll
               for (int j = 0; j < 16; ++j) ov[j] *= f;
-              tmem_st<16>(tmem + lane_sel + kColO + kColsPart * part + 16 * cc, ov);
+              tmem_st<16>(t_oc, ov);
             }
-            lsum *= f;
             nref -= add;
           }
           // ---- pass 2: P = 2^(s * scale - ref) as f16 pairs, written over the scores read above
-          float lt0 = 0.f, lt1 = 0.f;
 #pragma unroll
           for (int c = 0; c < kCP; ++c) {
             float t[16];
@@ -377,27 +386,22 @@ decode_prefix_m_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_co
 #pragma unroll
             for (int j = 0; j < 16; j += 2) {
               const float e0 = ex2(t[j]), e1 = ex2(t[j + 1]);
-              lt0 += e0; lt1 += e1;
               asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(o[j >> 1]) : "f"(e1), "f"(e0));
             }
             tmem_st8_nowait(t_s + 8 * c, o);
           }
-          lsum += lt0 + lt1;
           tmem_wait_st();
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(bar_pready + 8 * sb);
         }
         // ============================================================ the unit's partial: (m, l) and the accumulator row
-        sh.lpart[part][r] = lsum;
         mbar_wait(bar_done + 8 * ((gt - 1) & 1), ((gt - 1) >> 1) & 1);
         tc_fence_after();
-        asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "n"(32 * kSW) : "memory");
+        float lv[16];
+        if (part == 0) tmem_ld<16>(tmem + lane_sel + kColL, lv);   // 16 copies of the row sum (warp-uniform branch)
         if (valid && part == 0) {
-          float l = 0.f;
-#pragma unroll
-          for (int pp = 0; pp < kSW; ++pp) l += sh.lpart[pp][r];
-          ml_out[prow] = make_float2(-nref * 0.6931471805599453f, l);
+          ml_out[prow] = make_float2(-nref * 0.6931471805599453f, lv[0]);
           if (un.slots_used > 0)                       // item finished: its remaining slots are empty
             for (int sl = un.slots_used; sl < num_splits; ++sl) ml_out[prow - un.slot + sl] = make_float2(-INFINITY, 0.f);
         }
@@ -414,8 +418,8 @@ decode_prefix_m_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_co
               dst[j] = make_float4(ov[4 * j] * sc_, ov[4 * j + 1] * sc_, ov[4 * j + 2] * sc_, ov[4 * j + 3] * sc_);
           }
         }
-        tc_fence_before();
-        asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "n"(32 * kSW) : "memory");   // lpart is rewritten by the next unit
+        tc_fence_before();                             // (the next unit's first PV needs every softmax warp's P: it cannot
+                                                       //  overwrite O before all of them are through here)
         ++k;
       }
     } else {
@@ -476,7 +480,7 @@ decode_prefix_m_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_co
               cvt_e2m1x8(cwd, f);
               const uint4 o4 = make_uint4(hmul2(f[0], m4w.x), hmul2(f[1], m4w.y), hmul2(f[2], m4w.z), hmul2(f[3], m4w.w));
               const int chunk = 4 * (h & 1) + kk;
-              sts128(vrow + (h >> 1) * 16384 + (((chunk ^ (r & 7))) << 4), o4);
+              sts128(vrow + (h >> 1) * kVhBlock + (((chunk ^ (r & 7))) << 4), o4);
             }
           }
           fence_async_smem();
