@@ -268,8 +268,8 @@ def run_ours(args, rank, world, local_rank):
         step_graphs = [uq.StepGraph(cfg, bufs, qs[j], kvs[j][0], kvs[j][1], cu_dev, before_dev, after_dev, bt_dev, cache)
                        for j in range(n_in)]
 
-    # --shared-prefix 1 (configs with a shared prefix): the prefix through uq_decode_prefix_attention (two sequences per
-    # prefix tile), the private suffixes through uq_decode_attention, uq_merge_splits2 over both sets of partials
+    # --shared-prefix 1 (configs with a shared prefix): the prefix through uq_decode_prefix_attention (8 or 16 sequences
+    # per prefix tile), the private suffixes through uq_decode_attention, uq_merge_splits2 over both sets of partials
     pbufs, pfx = None, 0
     if args.shared_prefix and wl.prefix_len >= 128:
         pfx = (int(wl.prefix_len) // 128) * 128

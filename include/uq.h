@@ -218,7 +218,7 @@ int32_t uq_merge_splits(const uq_config* cfg, const float* partial_acc, const fl
  * Shared-prefix ("cascade") decode: the first prefix_len tokens of ALL `batch` sequences are the same physical pages
  * (block_tables[b][p] is the same for every b and p < prefix_len / page_size: the caller's guarantee — the long
  * shared prompt of the paper's agent workloads).  Computes the partials of exactly those tokens
- * for every sequence, each 128-token tile staged, converted and multiplied once for four sequences at a time; the
+ * for every sequence, each 128-token tile staged, converted and multiplied once for 8 sequences at a time (16 for GQA groups <= 8); the
  * remaining tokens of a sequence go through uq_decode_attention with block_tables + prefix_len / page_size and
  * seq_lens - prefix_len, and uq_merge_splits2 combines the two sets.
  *  prefix_len   a positive multiple of 128, <= every sequence's length.      num_splits >= 2.
