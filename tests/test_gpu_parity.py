@@ -1036,3 +1036,20 @@ def test_ultra_tq_scaled_config3_sampled_sequences():
             f"seq {b}: V image differs"
         ref = T.attention(qb[b], sh(ki), sh(kn), sh(vc), sh(vsc), sh(vz), cb, hkv)
         H.check_out(out[b], ref, f"ultra-tq config 3 x 0.2, seq {b} ({L} tokens), S={S}")
+
+
+def test_distortion_study_has_the_shape_of_fig_2b():
+    """paper_2606_20474_b200.distortion (the shape of Fig. 2b) on 4,096
+    vectors per head size: raw-absmax FP4 is an order of magnitude off; the constant closes most of the gap to the
+    Lloyd-Max codebook; 0.156 beats the MX rule with the continuous scale and 0.195 beats 0.156 with the power-of-two
+    scale (the paper's "power-of-two-optimal value"); the figures do not depend on d."""
+    from paper_2606_20474_b200 import distortion
+    rows = distortion.study(n_vectors=4096, seed=3, device=DEV)
+    assert set(rows) == {64, 128, 256}
+    for d, r in rows.items():
+        assert 0.0085 < r["lloyd-max"] < 0.0100, (d, r)
+        assert r["fp4 c=1.0"] > 8 * r["fp4 0.156"], (d, r)
+        assert r["lloyd-max"] < r["fp4 0.156"] < r["fp4 mx"], (d, r)
+        assert r["fp4 0.195p"] < r["fp4 0.156p"], (d, r)
+        assert r["fp4 0.156"] < r["fp4 0.195p"], (d, r)
+        assert abs(r["fp4 0.156"] - rows[128]["fp4 0.156"]) < 0.1 * rows[128]["fp4 0.156"], (d, r)
