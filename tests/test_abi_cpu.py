@@ -106,6 +106,33 @@ def test_binding_refuses_cpu_tensors(lib):
         uq.merge_splits(cfg, torch.zeros((1, 8, 1, 128)), torch.zeros((1, 8, 1, 2)), out)
 
 
+def test_argument_checks_of_the_round_2_entry_points_need_no_gpu(lib):
+    """Host-side validation of uq_decode_attention_static, uq_tq_append and uq_tq_decode_attention returns before any
+    CUDA call: sizes beyond the static scratch, a missing / unsorted codebook, the wrong entry point for a format."""
+    cfg = uq.UQConfig(64, 4).c()
+    n = ctypes.c_size_t(0)
+    assert lib.uq_decode_static_scratch_needed(ctypes.byref(cfg), 32, 6, ctypes.byref(n)) == 0
+    assert n.value == 32 * 64 * 6 * 128 * 4 + 32 * 64 * 6 * 8
+    assert lib.uq_static_scratch_bytes() == 32 << 20
+    one = ctypes.c_void_p(256)                          # never dereferenced: the size check comes first
+    assert lib.uq_decode_attention_static(ctypes.byref(cfg), one, one, 10, one, 4, one, 256, 8, one, None) == 2
+    assert b"static scratch" in lib.uq_last_error_string()
+    assert lib.uq_decode_static_scratch_needed(ctypes.byref(cfg), 0, 6, ctypes.byref(n)) == 1
+    assert lib.uq_baseline_record_bytes(ctypes.byref(cfg), 3) == 2432
+    good = (ctypes.c_float * 16)(*[float(i) - 7.5 for i in range(16)])
+    bad = (ctypes.c_float * 16)(*([0.0] * 16))
+    cb = lambda a: ctypes.cast(a, ctypes.c_void_p)
+    assert lib.uq_tq_append(ctypes.byref(cfg), None, one, one, one, one, one, 4, 1, 1, one, 10, None, None, None) == 1
+    assert lib.uq_tq_append(ctypes.byref(cfg), cb(bad), one, one, one, one, one, 4, 1, 1, one, 10, None, None, None) == 1
+    assert b"ascending" in lib.uq_last_error_string()
+    assert lib.uq_tq_append(ctypes.byref(cfg), cb(good), one, one, one, one, one, 4, 1, 1, one, 10, one, None, None) == 1
+    assert lib.uq_tq_decode_attention(ctypes.byref(cfg), cb(bad), one, one, 10, one, 4, one, 1, 1, one, one, None) == 1
+    assert lib.uq_baseline_append(ctypes.byref(cfg), 3, one, one, one, one, one, 4, 1, 1, one, 10, None, None, None) == 1
+    assert b"uq_tq_append" in lib.uq_last_error_string()
+    d64 = uq.UQConfig(64, 4, head_dim=64).c()
+    assert lib.uq_tq_append(ctypes.byref(d64), cb(good), one, one, one, one, one, 4, 1, 1, one, 10, None, None, None) == 2
+
+
 def test_product_package_never_imports_the_oracle():
     pkg = os.path.join(ROOT, "paper_2606_20474_b200")
     for dirpath, _, files in os.walk(pkg):
