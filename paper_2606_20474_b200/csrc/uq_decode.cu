@@ -173,13 +173,17 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
   const int role = warp;
 #endif
 
-  const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  // The two shared-memory base addresses go through an opaque move: as plain expressions of a symbol the compiler
+  // rematerialises them at every use (S2R CgaCtaId + MOV + LEA per mbarrier operation, ~140 instructions a tile).
+  uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u, sh_base = smem_u32(&sh);
+  asm volatile("mov.u32 %0, %0;" : "+r"(base));
+  asm volatile("mov.u32 %0, %0;" : "+r"(sh_base));
   const uint32_t sQ = base + kOffQ, sSFA = base + kOffSFA, sSFB = base + kOffSFB, sP = base + kOffP;
-  const uint32_t bar_fullk = smem_u32(&sh.full_k[0]), bar_emptyk = smem_u32(&sh.empty_k[0]),
-                 bar_fullv = smem_u32(&sh.full_v[0]), bar_emptyv = smem_u32(&sh.empty_v[0]),
-                 bar_sfull = smem_u32(&sh.s_full[0]), bar_sfree = smem_u32(&sh.s_free[0]),
-                 bar_ready = smem_u32(&sh.ready[0]), bar_done = smem_u32(&sh.done[0]),
-                 bar_qfull = smem_u32(&sh.q_full[0]);
+  const uint32_t bar_fullk = sh_base + offsetof(Shared, full_k), bar_emptyk = sh_base + offsetof(Shared, empty_k),
+                 bar_fullv = sh_base + offsetof(Shared, full_v), bar_emptyv = sh_base + offsetof(Shared, empty_v),
+                 bar_sfull = sh_base + offsetof(Shared, s_full), bar_sfree = sh_base + offsetof(Shared, s_free),
+                 bar_ready = sh_base + offsetof(Shared, ready), bar_done = sh_base + offsetof(Shared, done),
+                 bar_qfull = sh_base + offsetof(Shared, q_full);
 
   // ---------------- setup
   if (tid == 0) {
