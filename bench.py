@@ -762,6 +762,29 @@ def run_calibrate(args):
 
 
 # ----------------------------------------------------------------------------- main
+def dump_trace(path: str) -> None:
+    """--trace: the [tile][16 events] clock64 tables a -DUQ_TRACE build of libuq.so keeps for one CTA of the decode kernel
+    and one of the shared-prefix kernel (event numbers: the comments at TRD / TRP in csrc/).  Rows of zeros are left out."""
+    import ctypes
+
+    import paper_2606_20474_b200 as uq
+    lib = ctypes.CDLL(uq.library_path())
+    with open(path, "w") as f:
+        for name in ("decode", "prefix"):
+            try:
+                fn = getattr(lib, "uq_debug_trace_read_" + name)
+            except AttributeError:
+                f.write(f"# {name}: libuq.so was not built with -DUQ_TRACE\n")
+                continue
+            buf = np.zeros(256 * 16, np.uint64)
+            rc = fn(buf.ctypes.data_as(ctypes.c_void_p), ctypes.c_size_t(buf.nbytes))
+            t = buf.reshape(256, 16)
+            f.write(f"# {name} kernel, traced CTA: clock64 per (tile, event 0..15), cudaMemcpyFromSymbol rc={rc}\n")
+            for i, row in enumerate(t):
+                if row.any():
+                    f.write(f"{i} " + " ".join(str(int(v)) for v in row) + "\n")
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -782,6 +805,9 @@ def main():
                     help="instead of the decode step, time bulk quantize-on-append of TOKENS new tokens per call")
     ap.add_argument("--calibrate", type=int, default=0, metavar="VECTORS",
                     help="instead of the decode step, time uq_calibrate_c over VECTORS key vectors and 56 constants")
+    ap.add_argument("--trace", default="", metavar="FILE",
+                    help="debug builds only (UQ_NVCC_EXTRA=-DUQ_TRACE python -m paper_2606_20474_b200.build): after the run, write "
+                         "the per-tile clock64 tables of the traced CTAs (decode kernel, shared-prefix kernel) to FILE as text")
     ap.add_argument("--no-early", action="store_true",
                     help="do not set UQ_FLAG_SMALL_APPEND_AHEAD (the decode kernel then waits for the append before it reads anything)")
     ap.add_argument("--kv", default="fp4", choices=["fp4", "fp8", "bf16", "tq"],
@@ -823,6 +849,8 @@ def main():
         line = run_ours(args, rank, world, local_rank)
         if rank == 0:
             print(json.dumps(line), flush=True)
+            if args.trace:
+                dump_trace(args.trace)
     finally:
         if world > 1:
             torch.distributed.destroy_process_group()

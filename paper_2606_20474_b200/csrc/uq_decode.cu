@@ -57,6 +57,13 @@ constexpr int kIssuerWarps = 4;                      // QK issuer, PV issuer, K 
 constexpr int kKStages = UQ_KSTAGES;
 constexpr int kVStages = UQ_VSTAGES;
 constexpr int kPBytes = 4096;                        // one P operand buffer: [token-core 16][head-core 2][8 tok][8 heads] f16
+#ifdef UQ_TRACE
+__device__ unsigned long long g_trace_decode[UQ_TRACE_TILES * 16];
+#endif
+// trace events of CTA 5 (UQ_TR): 0 QK issue, 8 / 9 QK warp before / after the wait for a free score buffer, 5 PV issue,
+// 10 / 1 softmax warp 0 before / after the wait for S, 3 its tile done, 6 / 7 V warp 0 before / after the wait for the
+// tile's bytes, 11 / 12 before / after the wait for a free Vhat buffer, 4 its tile done
+#define TRD(ev, tile) UQ_TR(g_trace_decode, 5, ev, tile)
 constexpr float kThresh = 12.0f;                     // lazy-reference threshold (log2 units)
 constexpr int kMaxBatch = 2048;                      // sequences per call (tile prefix sums live in shared memory)
 constexpr int kVBufs = UQ_VBUFS;                     // Vhat^T buffers in TMEM
@@ -298,7 +305,9 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
       have_nx = sc.next(cur_nx, nx);
       for (int i = 0; i < un.n_tiles; ++i) {
         const int sb = gt & 1;
+        TRD(8, gt);
         if (gt >= 2) mbar_wait(bar_sfree + 8 * sb, ((gt >> 1) - 1) & 1);
+        TRD(9, gt);
         // here every QK up to global tile gt-2 has completed (its S was read): at i == 0 the Q buffer of
         // unit k-2 (= buffer k & 1), at i == 1 that of unit k-1 (= buffer (k+1) & 1) may be refilled
         if (i == 0 && k_q < k) { load_q(un, k); k_q = k; }
@@ -323,6 +332,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_emptyv + 8 * sv);   // the K scales are copied: this warp is done with the V stage
         mbar_wait(bar_fullk + 8 * sk, phk);
+        TRD(0, gt);
         tc_fence_after();
         if (elect_one()) {
           const uint32_t t_sfa = tmem + kColSFA + kSfaCols * sb, qb = sQ + kQBytes * (k & 1);
@@ -358,6 +368,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
     while (sc.next(cur, un)) {
       for (int i = 0; i < un.n_tiles; ++i, ++gt) {
         mbar_wait(bar_ready + 8 * (gt & 1), (gt >> 1) & 1);
+        TRD(5, gt);
         tc_fence_after();
         if (lane == 0) {
           const uint32_t pbuf = sP + kPBytes * (gt & 1), vbuf = tmem + kColV + kVBufCols * ((gt & 1) % kVBufs);
@@ -484,7 +495,9 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
             const uint32_t t_s = tmem + lane_sel + kColS + 16 * sb;
             const uint32_t p_addr = p_row + kPBytes * sb;
 
+            if (cw == 0) TRD(10, gt);
             mbar_wait(bar_sfull + 8 * sb, ph2);        // S(gt) is in TMEM
+            if (cw == 0) TRD(1, gt);
             if (gt >= 2) mbar_wait(bar_done + 8 * sb, ph2 ^ 1);   // PV(gt-2) has read P buffer gt&1 (the PV warp commits
                                                                    // once per tile: its issue stream bounds the tile period)
             tc_fence_after();
@@ -574,6 +587,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
             for (int j = 0; j < NH; j += 2) fadd2(lsum[j], lsum[j + 1], lsum[j], lsum[j + 1], lt[j], lt[j + 1]);
 
             // ---- S has been read (QK may overwrite the buffer), P is written, O is consistent with mref
+            if (cw == 0) TRD(3, gt);
             fence_async_smem();
             tc_fence_before();
             __syncwarp();
@@ -654,7 +668,9 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
         for (int i = 0; i < un.n_tiles; ++i, rem -= kTilePages * kPage) {
           const int sb = gt & 1;
           const uint32_t rest = base + kOffV + s * kVStageBytes;   // [V codes | K scales | V scales] of page 0
+          if (cw == kSoftmaxWarps) TRD(6, gt);
           mbar_wait(bar_fullv + 8 * s, ph_full);       // the tile's bytes have landed
+          if (cw == kSoftmaxWarps) TRD(7, gt);
           if constexpr (D == 64) {
             if (!active) {                             // no channels: nothing to convert, the barriers still count this warp
               if (q == 2) {
@@ -724,10 +740,12 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
           }
           __syncwarp();
 
+          if (cw == kSoftmaxWarps) TRD(11, gt);
           if (gt >= 2) {                               // PV(gt-2) has read Vhat buffer gt&1
             mbar_wait(bar_done + 8 * sb, ((gt >> 1) - 1) & 1);
             tc_fence_after();
           }
+          if (cw == kSoftmaxWarps) TRD(12, gt);
           // ---- V codes -> Vhat^T in TMEM buffer gt&1: lane = channel, column c = tokens 2c, 2c+1
           const uint32_t t_v = tmem + lane_sel + kColV + kVBufCols * sb + 64 * hc;
           const uint32_t code0 = rest + 128 * g + 4 * lane;
@@ -750,6 +768,7 @@ decode_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ 
             tmem_st16_nowait(t_v + 16 * h, o);
           }
           tmem_wait_st();
+          if (cw == kSoftmaxWarps) TRD(4, gt);
           tc_fence_before();
           __syncwarp();                                 // also: every lane has read the scratch of this tile
           if (lane == 0) {
@@ -967,3 +986,10 @@ extern "C" int32_t uq_decode_attention(const uq_config* cfg, const void* q_fp8, 
                                 partial_acc, partial_ml, sm_count, (cudaStream_t)stream);
   }
 }
+
+#ifdef UQ_TRACE
+// debug builds only (not part of include/uq.h): the [UQ_TRACE_TILES][16] clock64 table of the decode kernel's traced CTA
+extern "C" int uq_debug_trace_read_decode(void* host, size_t bytes) {
+  return (int)cudaMemcpyFromSymbol(host, uq::g_trace_decode, bytes);
+}
+#endif

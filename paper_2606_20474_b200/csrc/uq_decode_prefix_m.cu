@@ -48,6 +48,13 @@ constexpr int kVhBlock = kVhRows * 128;              // one block of 64 tokens: 
 constexpr int kVhBytes = 2 * kVhBlock;               // Vhat of a tile: two blocks of 64 tokens
 constexpr int kQBytes = 128 * 128;                   // the query rows of a unit: [128 rows][128 B E4M3]
 constexpr float kThresh = 12.0f;
+#ifdef UQ_TRACE
+__device__ unsigned long long g_trace_prefix[UQ_TRACE_TILES * 16];
+#endif
+// trace events of CTA 3 (UQ_TR): 0 QK issue, 6 the QK warp sees PV(gt-2) done, 9 / 5 PV warp: Vhat ready / issue, softmax
+// warp (part 0, quarter 0): 1 S seen, 10 pass 1 done, 2 maxima exchanged, 3 pass 2 done; V warp of quarter 0: 7 tile
+// bytes seen, 12 Vhat buffer free, 4 tile converted
+#define TRP(ev, tile) UQ_TR(g_trace_prefix, 3, ev, tile)
 
 constexpr int kOffK = 0;                                        // kKStages x 16384, SW128
 constexpr int kOffVh = kOffK + kKStages * kKStageBytes;         // 2 x 32768, SW128
@@ -238,11 +245,15 @@ decode_prefix_m_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_co
         fence_async_smem();
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_emptyv + 8 * sv);
-        if (gt >= 2) mbar_wait(bar_done + 8 * sb, ((gt >> 1) - 1) & 1);   // PV(gt-2) has read P out of this score buffer
+        if (gt >= 2) {
+          mbar_wait(bar_done + 8 * sb, ((gt >> 1) - 1) & 1);   // PV(gt-2) has read P out of this score buffer
+          TRP(6, gt - 2);
+        }
         if (i == 0 && k_q < k) { load_q(un, k); k_q = k; }
         if (i == 1 && have_nx) { load_q(nx, k + 1); k_q = k + 1; }
         if (i == 0) mbar_wait(bar_qfull + 8 * (k & 1), (k >> 1) & 1);
         mbar_wait(bar_fullk + 8 * sk, phk);
+        TRP(0, gt);
         tc_fence_after();
         if (elect_one()) {
           const uint32_t t_sfb = tmem + kColSFB + 4 * sb, qb = sQ + kQBytes * (k & 1);
@@ -271,7 +282,9 @@ decode_prefix_m_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_co
       for (int i = 0; i < un.n_tiles; ++i, ++gt) {
         const int sb = gt & 1;
         mbar_wait(bar_vready + 8 * sb, (gt >> 1) & 1);
+        TRP(9, gt);
         mbar_wait(bar_pready + 8 * sb, (gt >> 1) & 1);
+        TRP(5, gt);
         tc_fence_after();
         if (lane == 0) {
           const uint32_t vb = sVh + kVhBytes * sb;
@@ -339,6 +352,7 @@ decode_prefix_m_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_co
           // this part's columns of the score buffer; its P (f16 pairs) overwrites their first half in place
           const uint32_t t_s = tmem + lane_sel + kColS + 128 * sb + kColsPart * part;
           mbar_wait(bar_sfull + 8 * sb, (gt >> 1) & 1);
+          if (part == 0 && q == 0) TRP(1, gt);
           tc_fence_after();
           uint32_t sv[kCP][16];                        // the part's raw scores of the tile: kept for both passes
 #pragma unroll
@@ -353,7 +367,9 @@ decode_prefix_m_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_co
 #pragma unroll
             for (int j = 0; j < 16; j += 2) mx = fmaxf(mx, fmaxf(__uint_as_float(sv[c][j]), __uint_as_float(sv[c][j + 1])));
           sh.pmax[sb][part][r] = mx;
+          if (part == 0 && q == 0) TRP(10, gt);
           asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "n"(32 * kSW) : "memory");
+          if (part == 0 && q == 0) TRP(2, gt);
 #pragma unroll
           for (int pp = 0; pp < kSW; ++pp) mx = fmaxf(mx, sh.pmax[sb][pp][r]);
           mx *= score_scale;
@@ -391,6 +407,7 @@ decode_prefix_m_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_co
             tmem_st8_nowait(t_s + 8 * c, o);
           }
           tmem_wait_st();
+          if (part == 0 && q == 0) TRP(3, gt);
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(bar_pready + 8 * sb);
@@ -454,6 +471,7 @@ decode_prefix_m_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_co
           const int sb = gt & 1;
           const uint32_t rest = base + kOffV + s * kVStageBytes;
           mbar_wait(bar_fullv + 8 * s, ph_full);
+          if (q == 0) TRP(7, gt);
           uint32_t sw;                                 // the tile's scale bytes of group g: lane <-> tokens 4 lane .. 4 lane + 3
           asm volatile("ld.shared.u32 %0, [%1];" : "=r"(sw)
                        : "r"(rest + kRestBytes * (lane >> 2) + 1088 + 32 * ((lane >> 1) & 1) + 8 * g + 4 * (lane & 1)));
@@ -466,6 +484,7 @@ decode_prefix_m_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_co
           }
           __syncwarp();
           if (gt >= 2) mbar_wait(bar_done + 8 * sb, ((gt >> 1) - 1) & 1);   // PV(gt-2) has read Vhat buffer gt & 1
+          if (q == 0) TRP(12, gt);
           const uint32_t vrow = sVh + kVhBytes * sb + 128 * r;
           const uint32_t code0 = rest + 128 * g + 4 * lane;
 #pragma unroll
@@ -483,6 +502,7 @@ decode_prefix_m_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_co
               sts128(vrow + (h >> 1) * kVhBlock + (((chunk ^ (r & 7))) << 4), o4);
             }
           }
+          if (q == 0) TRP(4, gt);
           fence_async_smem();
           __syncwarp();                                // also: every lane has read the scratch of this tile
           if (lane == 0) {
@@ -551,3 +571,10 @@ int32_t launch_prefix_m(const uq_config* cfg, const void* q_fp8, const void* cac
 }
 
 }  // namespace uq
+
+#ifdef UQ_TRACE
+// debug builds only (not part of include/uq.h): the [UQ_TRACE_TILES][16] clock64 table of the prefix kernel's traced CTA
+extern "C" int uq_debug_trace_read_prefix(void* host, size_t bytes) {
+  return (int)cudaMemcpyFromSymbol(host, uq::g_trace_prefix, bytes);
+}
+#endif

@@ -53,6 +53,19 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "DONE_%=:\n"
       "}\n" ::"r"(bar), "r"(parity) : "memory");
 }
+// Debug builds (-DUQ_TRACE; bench.py --trace): clock64 at named events of the tile loop, for ONE CTA, written to a table
+// [tile][16 events] in global memory that uq_debug_trace_read_* copies out — the per-tile timelines of DESIGN.md 5.2 /
+// 5.5.  Without the macro UQ_TR expands to nothing (the kernels' SASS is unchanged).
+#ifdef UQ_TRACE
+#define UQ_TRACE_TILES 256
+#define UQ_TR(table, cta, ev, tile)                                                                            \
+  do {                                                                                                        \
+    if (blockIdx.x == (cta) && (tile) >= 0 && (tile) < UQ_TRACE_TILES && (threadIdx.x & 31) == 0)             \
+      (table)[(tile) * 16 + (ev)] = clock64();                                                                \
+  } while (0)
+#else
+#define UQ_TR(table, cta, ev, tile) do { } while (0)
+#endif
 // The KV stream is read once: L2 evict-first keeps it from flushing everything else (the kernel's own
 // instructions included) out of L2.
 __device__ __forceinline__ uint64_t l2_evict_first_policy() {
