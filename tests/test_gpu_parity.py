@@ -1053,3 +1053,17 @@ def test_distortion_study_has_the_shape_of_fig_2b():
         assert r["fp4 0.195p"] < r["fp4 0.156p"], (d, r)
         assert r["fp4 0.156"] < r["fp4 0.195p"], (d, r)
         assert abs(r["fp4 0.156"] - rows[128]["fp4 0.156"]) < 0.1 * rows[128]["fp4 0.156"], (d, r)
+
+
+@pytest.mark.parametrize("d", [256, 64])
+def test_full_size_cfg3_shape_at_other_head_dims_sampled_sequences(d):
+    """The shapes `bench.py --config 3 --head-dim 256 | 64` time (config 3: 64 ragged sequences of 16k-64k tokens, 48/8
+    heads), at FULL size and with the slot count bench.py uses: the longest, the shortest and a middle sequence — cache
+    image bit for bit, FP8 query bytes, every output row of every head within 2e-3 + 1e-2 |ref| (full-size
+    parity in the launch configuration that is timed; head sizes of PAPER.md:322)."""
+    wl = W.make_config(3, head_dim=d)
+    cfg = H.cfg_of(wl)
+    S = uq.suggest_num_splits(cfg, wl.batch, int(wl.ctx_lens.mean()))
+    order = np.argsort(wl.ctx_lens, kind="stable")
+    _, n = _full_check(wl, [S], sample_seqs=[int(order[-1]), int(order[0]), int(order[len(order) // 2])], check_cache=True)
+    assert n == 3
