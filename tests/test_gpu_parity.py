@@ -1067,3 +1067,57 @@ def test_full_size_cfg3_shape_at_other_head_dims_sampled_sequences(d):
     order = np.argsort(wl.ctx_lens, kind="stable")
     _, n = _full_check(wl, [S], sample_seqs=[int(order[-1]), int(order[0]), int(order[len(order) // 2])], check_cache=True)
     assert n == 3
+
+
+@pytest.mark.parametrize("kv", ["fp8", "bf16", "tq"])
+def test_full_size_cfg2_comparison_caches_sampled_sequences(kv):
+    """The comparison kernels on the shape `bench.py --config 2 --kv fp8 | bf16 | tq` times (32 x 32,768 tokens, 64/4 heads)
+    at FULL size with bench.py's slot count: sequences 0, 13 and 31, all 64 heads, within 2e-3 + 1e-2 |ref| of the float64
+    attention over that cache's own contents (oracle.attention_fp8kv / attention_bf16kv / ultra_tq.attention)."""
+    from oracle import ultra_tq as T
+    wl = W.make_config(2)
+    cfg = H.cfg_of(wl)
+    B, hkv = wl.batch, wl.num_kv_heads
+    S = uq.suggest_num_splits(cfg, B, int(wl.ctx_lens.mean()))
+    bt = torch.from_numpy(wl.block_tables).to(DEV)
+    lens = torch.from_numpy(wl.ctx_lens.astype(np.int32)).to(DEV)
+    empty = torch.zeros((0, hkv, 128), dtype=torch.bfloat16, device=DEV)
+    cu0 = torch.zeros(B + 1, dtype=torch.int32, device=DEV)
+    q = W.gen_q(wl, DEV)
+    qb = H.bits(q)
+    bufs = uq.StepBuffers(cfg, B, S, DEV)
+    cb = np.asarray(W.TQ_CODEBOOK, np.float32)
+    if kv == "tq":
+        cache = uq.alloc_baseline_cache(cfg, uq.KV_ULTRA_TQ, wl.num_pages, DEV)
+        for b in range(B):
+            L = int(wl.ctx_lens[b])
+            k, v = W.seq_kv(wl, b, L, DEV)
+            cu = np.zeros(B + 1, np.int32); cu[b + 1:] = L
+            uq.tq_append(cfg, cb, k.contiguous(), v.contiguous(), torch.from_numpy(cu).to(DEV),
+                         torch.zeros(B, dtype=torch.int32, device=DEV), bt, cache)
+        q_rot = torch.empty_like(q)
+        uq.tq_append(cfg, cb, empty, empty, cu0, lens, bt, cache, q=q, q_rot=q_rot)
+        uq.tq_decode_attention(cfg, cb, q_rot, cache, bt, lens, S, bufs.partial_acc, bufs.partial_ml)
+        uq.merge_splits(cfg, bufs.partial_acc, bufs.partial_ml, bufs.out)
+        out = bufs.out
+    else:
+        fmt = uq.KV_FP8_E4M3 if kv == "fp8" else uq.KV_BF16
+        cache, _ = _fill_baseline_cache(cfg, fmt, wl)
+        out = uq.baseline_decode_step(cfg, fmt, bufs, q, empty, empty, cu0, lens, lens, bt, cache)
+    torch.cuda.synchronize()
+    out = out.float().cpu().numpy().astype(np.float64)
+    assert np.isfinite(out).all()
+    for b in (0, 13, 31):
+        L = int(wl.ctx_lens[b])
+        k, v = W.seq_kv(wl, b, L, DEV)
+        kbits, vbits = H.bits(k), H.bits(v)
+        if kv == "fp8":
+            ref = oracle.attention_fp8kv(qb[b], kbits, vbits)[0]
+        elif kv == "bf16":
+            ref = oracle.attention_bf16kv(qb[b], kbits, vbits)
+        else:
+            ki, kn = T.encode_k(kbits.reshape(L * hkv, 128), cb)
+            vc, vsc, vz = T.encode_v(vbits.reshape(L * hkv, 128))
+            sh = lambda a: a.reshape(L, hkv, -1)
+            ref = T.attention(qb[b], sh(ki), sh(kn), sh(vc), sh(vsc), sh(vz), cb, hkv)
+        H.check_out(out[b], ref, f"{kv} kv, config 2 full size, seq {b}, S={S}")
